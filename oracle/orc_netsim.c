@@ -1,0 +1,786 @@
+/*
+ * orc_netsim.c -- CPU ORACLE (test infrastructure, not product code).  See orc_netsim.h for the
+ * passages of PAPER.md this follows and the pins that hold it.  Build: oracle/build_oracle.py
+ * (gcc -O2 -ffp-contract=off; x86-64 SSE2 doubles, no x87, no FMA contraction).
+ *
+ * Section tags S0..S6 refer to DESIGN.md "Readings" (= SURVEY.md sec 8(c)).
+ */
+#include "orc_netsim.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ---- S0: units.  bytes, seconds, byte/s.  Rates live on a 2^-20 byte/s grid (reading R-FX). ---- */
+#define FRAC_BITS 20
+static int64_t rate_to_q(double Bps) { return (int64_t)floor(Bps * 1048576.0); } /* x * 2^20, floor */
+static double q_to_rate(int64_t q) { return (double)q * 0x1p-20; }               /* RN conversion, exact scale */
+
+enum { WAITING = 0, PENDING = 1, ACTIVE = 2, DONE = 3 };
+
+typedef struct {
+  int32_t kind, n, first_flow, n_flows, steps;
+  int32_t *ranks;
+} coll_t;
+
+typedef struct {
+  int64_t ev;
+  int32_t flow;
+  double rate, t0, t1;
+} trace_row;
+
+struct orc_sim {
+  orc_topology_desc d;
+  uint64_t seed;
+  int32_t G, n_links, ran;
+  double *cap, *lat; /* per directed link */
+  /* flows */
+  int64_t F, Fcap;
+  int32_t *src, *dst, *conn;
+  double *bytes, *start, *Lat;
+  int64_t *path_off; /* [F+1] */
+  int32_t *path;
+  int64_t path_cap;
+  int64_t *pred_off; /* [F+1] */
+  int32_t *pred;
+  int64_t pred_cap;
+  /* collectives */
+  coll_t *coll;
+  int32_t n_coll, coll_cap;
+  /* results */
+  double *t_done;
+  int32_t *bneck;
+  orc_event *ev;
+  int64_t n_ev, ev_cap;
+  trace_row *tr;
+  int64_t n_tr, tr_cap;
+  double work[7];
+};
+
+/* ------------------------------------------------------------------ S1: topology & link numbering */
+static int32_t nvl_up(int32_t g) { return 2 * g; }
+static int32_t nvl_dn(int32_t g) { return 2 * g + 1; }
+static int32_t nic_up(const orc_sim *s, int32_t g) { return 2 * s->G + 2 * g; }
+static int32_t nic_dn(const orc_sim *s, int32_t g) { return 2 * s->G + 2 * g + 1; }
+static int32_t base1(const orc_sim *s) { return 4 * s->G; }
+/* leaf-spine: pair u = (leaf*n_spines + spine)*P + p */
+static int32_t ls_pair(const orc_sim *s, int32_t leaf, int32_t spine, int32_t p) {
+  return (leaf * s->d.n_spines + spine) * s->d.uplinks_per_leaf_spine + p;
+}
+/* fat tree tier1<->tier2: pair u = (pod*(k/2) + edge)*(k/2) + agg */
+static int32_t ft_pair1(const orc_sim *s, int32_t pod, int32_t edge, int32_t agg) {
+  int32_t h = s->d.k / 2;
+  return (pod * h + edge) * h + agg;
+}
+static int32_t ft_npairs1(const orc_sim *s) { return s->d.k * (s->d.k / 2) * (s->d.k / 2); }
+static int32_t base2(const orc_sim *s) { return base1(s) + 2 * ft_npairs1(s); }
+/* fat tree tier2<->tier3: pair u = (pod*(k/2) + agg)*U + j ; core = agg*U + j */
+static int32_t ft_pair2(const orc_sim *s, int32_t pod, int32_t agg, int32_t j) {
+  return (pod * (s->d.k / 2) + agg) * s->d.agg_uplinks + j;
+}
+
+int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim **out) {
+  if (!d || !out) return ORC_EINVAL;
+  if (d->n_hosts <= 0 || d->gpus_per_host <= 0) return ORC_EINVAL;
+  if (!(d->nvlink_Bps > 0) || !(d->nic_Bps > 0) || !(d->hop_latency_s >= 0)) return ORC_EINVAL;
+  int64_t G = (int64_t)d->n_hosts * d->gpus_per_host;
+  int64_t L = 4 * G;
+  if (d->kind == ORC_TOPO_LEAF_SPINE) {
+    if (d->n_leaves <= 0 || d->n_spines <= 0 || d->uplinks_per_leaf_spine <= 0) return ORC_EINVAL;
+    if (d->n_hosts % d->n_leaves != 0 || !(d->fabric_Bps > 0)) return ORC_EINVAL;
+    L += 2 * (int64_t)d->n_leaves * d->n_spines * d->uplinks_per_leaf_spine;
+  } else if (d->kind == ORC_TOPO_FAT_TREE) {
+    int32_t k = d->k;
+    if (k < 2 || k % 2 != 0 || d->agg_uplinks <= 0 || !(d->fabric_Bps > 0)) return ORC_EINVAL;
+    if (d->gpus_per_host != k / 2 || d->n_hosts != k * (k / 2)) return ORC_EINVAL;
+    L += 2 * (int64_t)k * (k / 2) * (k / 2) + 2 * (int64_t)k * (k / 2) * d->agg_uplinks;
+  } else if (d->kind != ORC_TOPO_SINGLE)
+    return ORC_EINVAL;
+  if (L > 0x3fffffff) return ORC_ERANGE;
+  orc_sim *s = (orc_sim *)calloc(1, sizeof(orc_sim));
+  if (!s) return ORC_ENOMEM;
+  s->d = *d;
+  s->seed = seed;
+  s->G = (int32_t)G;
+  s->n_links = (int32_t)L;
+  s->cap = (double *)malloc(sizeof(double) * L);
+  s->lat = (double *)malloc(sizeof(double) * L);
+  s->path_off = (int64_t *)calloc(1, sizeof(int64_t));
+  s->pred_off = (int64_t *)calloc(1, sizeof(int64_t));
+  if (!s->cap || !s->lat || !s->path_off || !s->pred_off) {
+    orc_destroy(s);
+    return ORC_ENOMEM;
+  }
+  for (int64_t l = 0; l < L; l++) {
+    s->lat[l] = d->hop_latency_s;
+    s->cap[l] = l < 2 * G ? d->nvlink_Bps : l < 4 * G ? d->nic_Bps : d->fabric_Bps;
+  }
+  *out = s;
+  return ORC_OK;
+}
+
+void orc_destroy(orc_sim *s) {
+  if (!s) return;
+  for (int32_t c = 0; c < s->n_coll; c++) free(s->coll[c].ranks);
+  free(s->coll); free(s->cap); free(s->lat); free(s->src); free(s->dst); free(s->conn); free(s->bytes);
+  free(s->start); free(s->Lat); free(s->path_off); free(s->path); free(s->pred_off); free(s->pred);
+  free(s->t_done); free(s->bneck); free(s->ev); free(s->tr);
+  free(s);
+}
+
+int32_t orc_num_links(const orc_sim *s, int32_t *out) {
+  if (!s || !out) return ORC_EINVAL;
+  *out = s->n_links;
+  return ORC_OK;
+}
+int32_t orc_set_link_capacities(orc_sim *s, const double *c) {
+  if (!s || !c) return ORC_EINVAL;
+  if (s->ran) return ORC_ESTATE;
+  for (int32_t l = 0; l < s->n_links; l++)
+    if (!(c[l] > 0) || !(c[l] < 0x1p42)) return ORC_EINVAL;
+  memcpy(s->cap, c, sizeof(double) * s->n_links);
+  return ORC_OK;
+}
+int32_t orc_get_link_capacities(const orc_sim *s, double *c) {
+  if (!s || !c) return ORC_EINVAL;
+  memcpy(c, s->cap, sizeof(double) * s->n_links);
+  return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ S2: seeded ECMP routing */
+uint64_t orc_mix64(uint64_t x) { /* SplitMix64 step (Steele, Lea, Flood 2014) */
+  uint64_t z = x + 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+/* writes the path of (src,dst,conn) into p[0..5], returns its length */
+static int32_t route(const orc_sim *s, int32_t src, int32_t dst, int32_t conn, int32_t *p) {
+  const orc_topology_desc *d = &s->d;
+  int32_t hs = src / d->gpus_per_host, hd = dst / d->gpus_per_host;
+  if (hs == hd) {
+    p[0] = nvl_up(src);
+    p[1] = nvl_dn(dst);
+    return 2;
+  }
+  uint64_t H = orc_mix64(orc_mix64(orc_mix64(orc_mix64(s->seed) ^ (uint64_t)(uint32_t)src) ^ (uint64_t)(uint32_t)dst) ^
+                         (uint64_t)(uint32_t)conn);
+  if (d->kind == ORC_TOPO_SINGLE) {
+    p[0] = nic_up(s, src);
+    p[1] = nic_dn(s, dst);
+    return 2;
+  }
+  if (d->kind == ORC_TOPO_LEAF_SPINE) {
+    int32_t per = d->n_hosts / d->n_leaves, ls = hs / per, ld = hd / per, P = d->uplinks_per_leaf_spine;
+    if (ls == ld) {
+      p[0] = nic_up(s, src);
+      p[1] = nic_dn(s, dst);
+      return 2;
+    }
+    int32_t c = (int32_t)(H % (uint64_t)(d->n_spines * P));
+    int32_t spine = c / P, pu = c % P, pd = (int32_t)((H >> 32) % (uint64_t)P);
+    p[0] = nic_up(s, src);
+    p[1] = base1(s) + 2 * ls_pair(s, ls, spine, pu);     /* up: leaf_s -> spine */
+    p[2] = base1(s) + 2 * ls_pair(s, ld, spine, pd) + 1; /* down: spine -> leaf_d */
+    p[3] = nic_dn(s, dst);
+    return 4;
+  }
+  /* fat tree: host == edge switch; pod = host / (k/2); edge = host % (k/2) */
+  int32_t h = d->k / 2, qs = hs / h, es = hs % h, qd = hd / h, ed = hd % h;
+  int32_t a = (int32_t)(H % (uint64_t)h);
+  if (qs == qd) {
+    p[0] = nic_up(s, src);
+    p[1] = base1(s) + 2 * ft_pair1(s, qs, es, a);
+    p[2] = base1(s) + 2 * ft_pair1(s, qd, ed, a) + 1;
+    p[3] = nic_dn(s, dst);
+    return 4;
+  }
+  int32_t j = (int32_t)((H >> 32) % (uint64_t)d->agg_uplinks);
+  p[0] = nic_up(s, src);
+  p[1] = base1(s) + 2 * ft_pair1(s, qs, es, a);
+  p[2] = base2(s) + 2 * ft_pair2(s, qs, a, j);
+  p[3] = base2(s) + 2 * ft_pair2(s, qd, a, j) + 1;
+  p[4] = base1(s) + 2 * ft_pair1(s, qd, ed, a) + 1;
+  p[5] = nic_dn(s, dst);
+  return 6;
+}
+
+/* ------------------------------------------------------------------ flow table growth */
+static int grow_flows(orc_sim *s, int64_t need) {
+  if (need <= s->Fcap) return 0;
+  int64_t c = s->Fcap ? s->Fcap : 64;
+  while (c < need) c *= 2;
+#define RE(p, T, n)                               \
+  do {                                            \
+    void *q = realloc(p, sizeof(T) * (size_t)(n)); \
+    if (!q) return -1;                            \
+    p = (T *)q;                                   \
+  } while (0)
+  RE(s->src, int32_t, c); RE(s->dst, int32_t, c); RE(s->conn, int32_t, c);
+  RE(s->bytes, double, c); RE(s->start, double, c); RE(s->Lat, double, c);
+  RE(s->path_off, int64_t, c + 1); RE(s->pred_off, int64_t, c + 1);
+  s->Fcap = c;
+  return 0;
+}
+static int push_pred(orc_sim *s, int32_t p) {
+  int64_t n = s->pred_off[s->F + 1];
+  if (n + 1 > s->pred_cap) {
+    int64_t c = s->pred_cap ? s->pred_cap * 2 : 256;
+    RE(s->pred, int32_t, c);
+    s->pred_cap = c;
+  }
+  s->pred[n] = p;
+  s->pred_off[s->F + 1] = n + 1;
+  return 0;
+}
+/* start a new flow record (id = s->F); preds are pushed with push_pred, then commit_flow */
+static int begin_flow(orc_sim *s, int32_t src, int32_t dst, double bytes, double start, int32_t conn) {
+  if (grow_flows(s, s->F + 1)) return -1;
+  int64_t f = s->F;
+  s->src[f] = src; s->dst[f] = dst; s->bytes[f] = bytes; s->start[f] = start; s->conn[f] = conn;
+  int32_t p[6];
+  int32_t h = route(s, src, dst, conn, p);
+  int64_t po = s->path_off[f];
+  if (po + h > s->path_cap) {
+    int64_t c = s->path_cap ? s->path_cap * 2 : 256;
+    RE(s->path, int32_t, c);
+    s->path_cap = c;
+  }
+  double L = 0.0; /* S2: left-to-right sum of link latencies */
+  for (int32_t i = 0; i < h; i++) {
+    s->path[po + i] = p[i];
+    L = L + s->lat[p[i]];
+  }
+  s->Lat[f] = L;
+  s->path_off[f + 1] = po + h;
+  s->pred_off[f + 1] = s->pred_off[f];
+  return 0;
+}
+static void commit_flow(orc_sim *s) { s->F++; }
+
+/* ------------------------------------------------------------------ S3: collective -> flows + DAG */
+static int32_t coll_steps(int32_t kind, int32_t N) {
+  return kind == ORC_ALLREDUCE_RING ? 2 * (N - 1) : kind == ORC_ALLTOALL ? 1 : N - 1;
+}
+/* id of the flow of collective c's last step that rank rho SENDS / RECEIVES in the ring; -1 if rho not in c */
+static int32_t ring_index_of(const coll_t *c, int32_t rho) {
+  for (int32_t i = 0; i < c->n; i++)
+    if (c->ranks[i] == rho) return i;
+  return -1;
+}
+
+int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t N, double bytes, double start,
+                           const int32_t *after, int32_t n_after, int32_t *out_id) {
+  if (!s || !ranks) return ORC_EINVAL;
+  if (s->ran) return ORC_ESTATE;
+  if (kind < 0 || kind > 3 || N < 2 || !(bytes > 0) || !(bytes < INFINITY) || !(start >= 0) || !(start < INFINITY))
+    return ORC_EINVAL;
+  if (n_after < 0 || (n_after > 0 && !after)) return ORC_EINVAL;
+  for (int32_t i = 0; i < N; i++) {
+    if (ranks[i] < 0 || ranks[i] >= s->G) return ORC_EINVAL;
+    for (int32_t j = 0; j < i; j++)
+      if (ranks[j] == ranks[i]) return ORC_EINVAL;
+  }
+  for (int32_t a = 0; a < n_after; a++)
+    if (after[a] < 0 || after[a] >= s->n_coll) return ORC_EINVAL;
+  int32_t S = coll_steps(kind, N);
+  int64_t nf = kind == ORC_ALLTOALL ? (int64_t)N * (N - 1) : (int64_t)S * N;
+  if (s->F + nf > 0x7ffffff0) return ORC_ERANGE;
+  if (s->n_coll == s->coll_cap) {
+    int32_t c = s->coll_cap ? 2 * s->coll_cap : 16;
+    void *q = realloc(s->coll, sizeof(coll_t) * c);
+    if (!q) return ORC_ENOMEM;
+    s->coll = (coll_t *)q;
+    s->coll_cap = c;
+  }
+  int32_t cid = s->n_coll;
+  coll_t *c = &s->coll[cid];
+  c->kind = kind; c->n = N; c->first_flow = (int32_t)s->F; c->n_flows = (int32_t)nf; c->steps = S;
+  c->ranks = (int32_t *)malloc(sizeof(int32_t) * N);
+  if (!c->ranks) return ORC_ENOMEM;
+  memcpy(c->ranks, ranks, sizeof(int32_t) * N);
+  s->n_coll++; /* (ranks now owned by the table) */
+  double chunk = bytes / (double)N; /* S3: one f64 division */
+  int32_t first = c->first_flow;
+
+  /* `after` edges for an initial flow whose sender is rho: A's last-step flow sent by rho and the one received
+   * by rho (ring); every flow from / to rho (all-to-all).  rho not in A: no edge. */
+#define PUSH_AFTER(rho)                                                                      \
+  for (int32_t a_ = 0; a_ < n_after; a_++) {                                                 \
+    const coll_t *A = &s->coll[after[a_]];                                                   \
+    int32_t ia = ring_index_of(A, (rho));                                                    \
+    if (ia < 0) continue;                                                                    \
+    if (A->kind == ORC_ALLTOALL) {                                                           \
+      for (int32_t x = 0; x < A->n; x++) {                                                   \
+        if (x == ia) continue;                                                               \
+        /* flow ia->x is entry (ia, x) of the row-major list without the diagonal */         \
+        if (push_pred(s, A->first_flow + ia * (A->n - 1) + (x < ia ? x : x - 1))) return ORC_ENOMEM; \
+        if (push_pred(s, A->first_flow + x * (A->n - 1) + (ia < x ? ia : ia - 1))) return ORC_ENOMEM; \
+      }                                                                                      \
+    } else {                                                                                 \
+      int32_t last = A->first_flow + (A->steps - 1) * A->n;                                  \
+      if (push_pred(s, last + ia)) return ORC_ENOMEM;                    /* sent by rho */    \
+      if (push_pred(s, last + (ia + A->n - 1) % A->n)) return ORC_ENOMEM; /* received by rho */ \
+    }                                                                                        \
+  }
+
+  if (kind == ORC_ALLTOALL) {
+    for (int32_t i = 0; i < N; i++)
+      for (int32_t j = 0; j < N; j++) {
+        if (i == j) continue;
+        if (begin_flow(s, ranks[i], ranks[j], chunk, start, cid)) return ORC_ENOMEM;
+        PUSH_AFTER(ranks[i]);
+        commit_flow(s);
+      }
+  } else {
+    for (int32_t st = 0; st < S; st++)
+      for (int32_t i = 0; i < N; i++) { /* flow (st,i): r[i] -> r[(i+1) mod N] */
+        if (begin_flow(s, ranks[i], ranks[(i + 1) % N], chunk, st == 0 ? start : 0.0, cid)) return ORC_ENOMEM;
+        if (st == 0) {
+          PUSH_AFTER(ranks[i]);
+        } else {
+          if (push_pred(s, first + (st - 1) * N + (i + N - 1) % N)) return ORC_ENOMEM; /* data has arrived */
+          if (push_pred(s, first + (st - 1) * N + i)) return ORC_ENOMEM;               /* sender FIFO */
+        }
+        commit_flow(s);
+      }
+  }
+  if (out_id) *out_id = cid;
+  return ORC_OK;
+}
+
+int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *dst, const double *bytes,
+                      const double *start, const int64_t *dep_off, const int64_t *dep_ids, const int32_t *conn_id,
+                      int64_t *out_first) {
+  if (!s || n < 0 || (n > 0 && (!src || !dst || !bytes))) return ORC_EINVAL;
+  if (s->ran) return ORC_ESTATE;
+  if (s->F + n > 0x7ffffff0) return ORC_ERANGE;
+  int64_t first = s->F;
+  for (int64_t i = 0; i < n; i++) { /* validate everything before mutating */
+    if (src[i] < 0 || src[i] >= s->G || dst[i] < 0 || dst[i] >= s->G || src[i] == dst[i]) return ORC_EINVAL;
+    if (!(bytes[i] > 0) || !(bytes[i] < INFINITY)) return ORC_EINVAL;
+    if (start && (!(start[i] >= 0) || !(start[i] < INFINITY))) return ORC_EINVAL;
+    if (dep_off) {
+      if (dep_off[i + 1] < dep_off[i] || (dep_off[i + 1] > dep_off[i] && !dep_ids)) return ORC_EINVAL;
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; e++)
+        if (dep_ids[e] < 0 || dep_ids[e] >= first + i) return ORC_EINVAL; /* only earlier flows */
+    }
+  }
+  for (int64_t i = 0; i < n; i++) {
+    int32_t conn = conn_id ? conn_id[i] : (int32_t)(first + i);
+    if (begin_flow(s, src[i], dst[i], bytes[i], start ? start[i] : 0.0, conn)) return ORC_ENOMEM;
+    if (dep_off)
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; e++)
+        if (push_pred(s, (int32_t)dep_ids[e])) return ORC_ENOMEM;
+    commit_flow(s);
+  }
+  if (out_first) *out_first = first;
+  return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ S5: max-min progressive filling */
+typedef struct {
+  int32_t n_links;
+  int64_t *cap_rem; /* remaining capacity, rate quanta */
+  int32_t *n;       /* unfrozen active flows on the link */
+  int32_t *k;       /* newly frozen flows crossing the link in this iteration */
+  int32_t *touched;
+  int64_t *adj_off; /* link -> active flows (indices into act[]) */
+  int32_t *adj;
+  int64_t adj_cap;
+  uint8_t *frozen;
+  int64_t frozen_cap;
+  /* fast mode heap of (share, link) */
+  int64_t *hs;
+  int32_t *hl;
+  int64_t hn, hcap;
+} ws_t;
+
+static void ws_free(ws_t *w) {
+  free(w->cap_rem); free(w->n); free(w->k); free(w->touched); free(w->adj_off); free(w->adj); free(w->frozen);
+  free(w->hs); free(w->hl);
+}
+static int ws_init(ws_t *w, int32_t L) {
+  memset(w, 0, sizeof(*w));
+  w->n_links = L;
+  w->cap_rem = (int64_t *)malloc(sizeof(int64_t) * L);
+  w->n = (int32_t *)calloc(L, sizeof(int32_t));
+  w->k = (int32_t *)calloc(L, sizeof(int32_t));
+  w->touched = (int32_t *)malloc(sizeof(int32_t) * L);
+  w->adj_off = (int64_t *)malloc(sizeof(int64_t) * (L + 1));
+  return (w->cap_rem && w->n && w->k && w->touched && w->adj_off) ? 0 : -1;
+}
+static int heap_less(const ws_t *w, int64_t a, int64_t b) {
+  return w->hs[a] < w->hs[b] || (w->hs[a] == w->hs[b] && w->hl[a] < w->hl[b]);
+}
+static int heap_push(ws_t *w, int64_t s, int32_t l) {
+  if (w->hn == w->hcap) {
+    int64_t c = w->hcap ? 2 * w->hcap : 1024;
+    void *a = realloc(w->hs, sizeof(int64_t) * c), *b;
+    if (!a) return -1;
+    w->hs = (int64_t *)a;
+    b = realloc(w->hl, sizeof(int32_t) * c);
+    if (!b) return -1;
+    w->hl = (int32_t *)b;
+    w->hcap = c;
+  }
+  int64_t i = w->hn++;
+  w->hs[i] = s; w->hl[i] = l;
+  while (i > 0) {
+    int64_t p = (i - 1) / 2;
+    if (!heap_less(w, i, p)) break;
+    int64_t ts = w->hs[i]; w->hs[i] = w->hs[p]; w->hs[p] = ts;
+    int32_t tl = w->hl[i]; w->hl[i] = w->hl[p]; w->hl[p] = tl;
+    i = p;
+  }
+  return 0;
+}
+static void heap_pop(ws_t *w) {
+  int64_t n = --w->hn, i = 0;
+  w->hs[0] = w->hs[n]; w->hl[0] = w->hl[n];
+  for (;;) {
+    int64_t a = 2 * i + 1, b = a + 1, m = i;
+    if (a < n && heap_less(w, a, m)) m = a;
+    if (b < n && heap_less(w, b, m)) m = b;
+    if (m == i) break;
+    int64_t ts = w->hs[i]; w->hs[i] = w->hs[m]; w->hs[m] = ts;
+    int32_t tl = w->hl[i]; w->hl[i] = w->hl[m]; w->hl[m] = tl;
+    i = m;
+  }
+}
+
+/* Active flows act[0..nA) (ids into the path CSR).  Outputs indexed by flow id.  Returns the number of
+ * links with n>0 at the start (Lambda_act) through *lam_act. */
+static int solve_maxmin(ws_t *w, const int64_t *capq, int32_t nA, const int32_t *act, const int64_t *path_off,
+                        const int32_t *path, int32_t mode, int64_t *rq, int32_t *bneck, int32_t *n_rounds,
+                        int32_t *first_bneck, int32_t *lam_act) {
+  int32_t L = w->n_links;
+  *n_rounds = 0; *first_bneck = -1; *lam_act = 0;
+  if (nA == 0) return 0;
+  /* init: cap_rem = cap, n = # active flows on the link, all unfrozen (S5) */
+  for (int32_t l = 0; l < L; l++) { w->cap_rem[l] = capq[l]; w->n[l] = 0; }
+  int64_t tot = 0;
+  for (int32_t a = 0; a < nA; a++)
+    for (int64_t e = path_off[act[a]]; e < path_off[act[a] + 1]; e++) { w->n[path[e]]++; tot++; }
+  if (tot > w->adj_cap) {
+    void *q = realloc(w->adj, sizeof(int32_t) * tot);
+    if (!q) return -1;
+    w->adj = (int32_t *)q; w->adj_cap = tot;
+  }
+  if (nA > w->frozen_cap) {
+    void *q = realloc(w->frozen, nA);
+    if (!q) return -1;
+    w->frozen = (uint8_t *)q; w->frozen_cap = nA;
+  }
+  memset(w->frozen, 0, nA);
+  w->adj_off[0] = 0;
+  for (int32_t l = 0; l < L; l++) { w->adj_off[l + 1] = w->adj_off[l] + w->n[l]; if (w->n[l] > 0) (*lam_act)++; }
+  { /* fill link -> active-flow lists */
+    int64_t *cur = (int64_t *)malloc(sizeof(int64_t) * L);
+    if (!cur) return -1;
+    memcpy(cur, w->adj_off, sizeof(int64_t) * L);
+    for (int32_t a = 0; a < nA; a++)
+      for (int64_t e = path_off[act[a]]; e < path_off[act[a] + 1]; e++) w->adj[cur[path[e]]++] = a;
+    free(cur);
+  }
+  if (mode == ORC_MODE_FAST) {
+    w->hn = 0;
+    for (int32_t l = 0; l < L; l++)
+      if (w->n[l] > 0 && heap_push(w, w->cap_rem[l] / w->n[l], l)) return -1;
+  }
+  int32_t unfrozen = nA;
+  while (unfrozen > 0) {
+    /* the bottleneck link: smallest share = cap_rem / n over links with n > 0; ties -> lowest link id */
+    int32_t b = -1;
+    int64_t s = 0;
+    if (mode == ORC_MODE_NAIVE) {
+      for (int32_t l = 0; l < L; l++) {
+        if (w->n[l] <= 0) continue;
+        int64_t sh = w->cap_rem[l] / w->n[l];
+        if (b < 0 || sh < s) { b = l; s = sh; }
+      }
+    } else {
+      for (;;) { /* lazy deletion: an entry is live iff it still equals the link's current share */
+        int64_t sh = w->hs[0];
+        int32_t l = w->hl[0];
+        heap_pop(w);
+        if (w->n[l] > 0 && w->cap_rem[l] / w->n[l] == sh) { b = l; s = sh; break; }
+      }
+    }
+    if (*n_rounds == 0) *first_bneck = b;
+    /* freeze every unfrozen active flow on b at rate s; count k[l] on all their links */
+    int32_t nt = 0;
+    for (int64_t e = w->adj_off[b]; e < w->adj_off[b + 1]; e++) {
+      int32_t a = w->adj[e];
+      if (w->frozen[a]) continue;
+      w->frozen[a] = 1;
+      rq[act[a]] = s;
+      bneck[act[a]] = b;
+      unfrozen--;
+      for (int64_t pe = path_off[act[a]]; pe < path_off[act[a] + 1]; pe++) {
+        int32_t l = path[pe];
+        if (w->k[l]++ == 0) w->touched[nt++] = l;
+      }
+    }
+    /* debit: cap_rem -= k*s ; n -= k */
+    for (int32_t t = 0; t < nt; t++) {
+      int32_t l = w->touched[t];
+      w->cap_rem[l] = w->cap_rem[l] - (int64_t)w->k[l] * s;
+      w->n[l] -= w->k[l];
+      w->k[l] = 0;
+      if (mode == ORC_MODE_FAST && w->n[l] > 0 && heap_push(w, w->cap_rem[l] / w->n[l], l)) return -1;
+    }
+    (*n_rounds)++;
+  }
+  return 0;
+}
+
+int32_t orc_maxmin(int32_t n_links, const double *cap, int32_t n_flows, const int64_t *path_off, const int32_t *path,
+                   int32_t mode, double *rate, int32_t *bneck, int32_t *n_rounds, int32_t *first_bneck) {
+  if (n_links <= 0 || n_flows < 0 || !cap || !path_off || !rate || !bneck) return ORC_EINVAL;
+  ws_t w;
+  if (ws_init(&w, n_links)) { ws_free(&w); return ORC_ENOMEM; }
+  int64_t *capq = (int64_t *)malloc(sizeof(int64_t) * n_links);
+  int64_t *rq = (int64_t *)malloc(sizeof(int64_t) * (n_flows + 1));
+  int32_t *act = (int32_t *)malloc(sizeof(int32_t) * (n_flows + 1));
+  int32_t rc = ORC_OK, R = 0, fb = -1, lam = 0;
+  if (!capq || !rq || !act) rc = ORC_ENOMEM;
+  if (rc == ORC_OK) {
+    for (int32_t l = 0; l < n_links; l++) capq[l] = rate_to_q(cap[l]);
+    for (int32_t f = 0; f < n_flows; f++) act[f] = f;
+    if (solve_maxmin(&w, capq, n_flows, act, path_off, path, mode, rq, bneck, &R, &fb, &lam)) rc = ORC_ENOMEM;
+  }
+  if (rc == ORC_OK) {
+    for (int32_t f = 0; f < n_flows; f++) rate[f] = q_to_rate(rq[f]);
+    if (n_rounds) *n_rounds = R;
+    if (first_bneck) *first_bneck = fb;
+  }
+  free(capq); free(rq); free(act); ws_free(&w);
+  return rc;
+}
+
+/* ------------------------------------------------------------------ S4: flow states & event loop */
+int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
+  if (!s || (mode != ORC_MODE_NAIVE && mode != ORC_MODE_FAST)) return ORC_EINVAL;
+  if (s->ran) return ORC_ESTATE;
+  int64_t F = s->F;
+  int32_t L = s->n_links, rc = ORC_OK;
+  ws_t w;
+  memset(&w, 0, sizeof(w));
+  int64_t *capq = (int64_t *)malloc(sizeof(int64_t) * L);
+  int64_t *succ_off = (int64_t *)calloc(F + 1, sizeof(int64_t));
+  int32_t *succ = (int32_t *)malloc(sizeof(int32_t) * (s->pred_off[F] + 1));
+  int32_t *pred_cnt = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  uint8_t *state = (uint8_t *)calloc(F + 1, 1);
+  double *t_act = (double *)malloc(sizeof(double) * (F + 1));
+  double *rem = (double *)malloc(sizeof(double) * (F + 1));
+  double *tc = (double *)malloc(sizeof(double) * (F + 1));
+  int64_t *rq = (int64_t *)malloc(sizeof(int64_t) * (F + 1));
+  int32_t *act = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  int32_t *pend = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  int32_t *comp = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  s->t_done = (double *)malloc(sizeof(double) * (F + 1));
+  s->bneck = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !act || !pend || !comp ||
+      !s->t_done || !s->bneck || ws_init(&w, L)) {
+    rc = ORC_ENOMEM;
+    goto out;
+  }
+  for (int32_t l = 0; l < L; l++) {
+    capq[l] = rate_to_q(s->cap[l]);
+    if (capq[l] < F + 1) { rc = ORC_ERANGE; goto out; } /* every fair share stays >= 1 quantum */
+  }
+  for (int64_t f = 0; f < F; f++) { s->t_done[f] = NAN; s->bneck[f] = -1; }
+  memset(s->work, 0, sizeof(s->work));
+  /* successor lists = transpose of the pred lists */
+  for (int64_t e = 0; e < s->pred_off[F]; e++) succ_off[s->pred[e] + 1]++;
+  for (int64_t f = 0; f < F; f++) succ_off[f + 1] += succ_off[f];
+  {
+    int64_t *cur = (int64_t *)malloc(sizeof(int64_t) * (F + 1));
+    if (!cur) { rc = ORC_ENOMEM; goto out; }
+    memcpy(cur, succ_off, sizeof(int64_t) * (F + 1));
+    for (int64_t f = 0; f < F; f++)
+      for (int64_t e = s->pred_off[f]; e < s->pred_off[f + 1]; e++) succ[cur[s->pred[e]]++] = (int32_t)f;
+    free(cur);
+  }
+  int32_t nA = 0, nP = 0;
+  int64_t n_done = 0;
+  double now = 0.0;
+  for (int64_t f = 0; f < F; f++) {
+    pred_cnt[f] = (int32_t)(s->pred_off[f + 1] - s->pred_off[f]);
+    if (pred_cnt[f] == 0) { /* no preds: t_act = start + Lat -> PENDING */
+      t_act[f] = s->start[f] + s->Lat[f];
+      state[f] = PENDING;
+      pend[nP++] = (int32_t)f;
+    }
+  }
+  for (;;) {
+    /* 1. activate every PENDING flow with t_act <= now */
+    int32_t n_activated = 0, np2 = 0;
+    for (int32_t i = 0; i < nP; i++) {
+      int32_t f = pend[i];
+      if (t_act[f] <= now) {
+        rem[f] = s->bytes[f];
+        state[f] = ACTIVE;
+        act[nA++] = f;
+        n_activated++;
+      } else
+        pend[np2++] = f;
+    }
+    nP = np2;
+    /* 2. rates over all ACTIVE flows, from scratch (S5) */
+    int32_t R = 0, fb = -1, lam = 0;
+    if (solve_maxmin(&w, capq, nA, act, s->path_off, s->path, mode, rq, s->bneck, &R, &fb, &lam)) {
+      rc = ORC_ENOMEM;
+      goto out;
+    }
+    /* 3. next time: tc = now + rem/rate (div, then add); t_next = min(min tc, min pending t_act) */
+    if (nA == 0 && nP == 0) break;
+    double t_next = INFINITY;
+    double ah = 0;
+    for (int32_t i = 0; i < nA; i++) {
+      int32_t f = act[i];
+      double q = rem[f] / q_to_rate(rq[f]);
+      tc[f] = now + q;
+      if (tc[f] < t_next) t_next = tc[f];
+      ah += (double)(s->path_off[f + 1] - s->path_off[f]);
+    }
+    for (int32_t i = 0; i < nP; i++)
+      if (t_act[pend[i]] < t_next) t_next = t_act[pend[i]];
+    /* 4. advance */
+    double dt = t_next - now;
+    int32_t nC = 0, na2 = 0;
+    for (int32_t i = 0; i < nA; i++) {
+      int32_t f = act[i];
+      if (trace) {
+        if (s->n_tr == s->tr_cap) {
+          int64_t c = s->tr_cap ? 2 * s->tr_cap : 4096;
+          void *q = realloc(s->tr, sizeof(trace_row) * c);
+          if (!q) { rc = ORC_ENOMEM; goto out; }
+          s->tr = (trace_row *)q; s->tr_cap = c;
+        }
+        trace_row *r = &s->tr[s->n_tr++];
+        r->ev = s->n_ev; r->flow = f; r->rate = q_to_rate(rq[f]); r->t0 = now; r->t1 = t_next;
+      }
+      if (tc[f] == t_next) { /* bit-equal absolute time: completes */
+        s->t_done[f] = t_next;
+        state[f] = DONE;
+        comp[nC++] = f;
+      } else {
+        double m = q_to_rate(rq[f]) * dt; /* mul, then sub, then clamp */
+        double r = rem[f] - m;
+        rem[f] = r > 0.0 ? r : 0.0;
+        act[na2++] = f;
+      }
+    }
+    s->work[0] += nA; s->work[1] += ah; s->work[2] += R; s->work[3] += (double)lam * R; s->work[4] += lam;
+    s->work[5] += nC; s->work[6] += 1;
+    nA = na2;
+    n_done += nC;
+    now = t_next;
+    /* 5. release successors of completed flows (ascending id: comp[] is in act[] order; order is immaterial,
+     *    every update is a counter decrement or a function of `now` only) */
+    for (int32_t i = 0; i < nC; i++)
+      for (int64_t e = succ_off[comp[i]]; e < succ_off[comp[i] + 1]; e++) {
+        int32_t g = succ[e];
+        if (--pred_cnt[g] == 0) {
+          double st = s->start[g] > now ? s->start[g] : now;
+          t_act[g] = st + s->Lat[g];
+          state[g] = PENDING;
+          pend[nP++] = g;
+        }
+      }
+    /* 6. log */
+    if (s->n_ev == s->ev_cap) {
+      int64_t c = s->ev_cap ? 2 * s->ev_cap : 1024;
+      void *q = realloc(s->ev, sizeof(orc_event) * c);
+      if (!q) { rc = ORC_ENOMEM; goto out; }
+      s->ev = (orc_event *)q; s->ev_cap = c;
+    }
+    orc_event *e = &s->ev[s->n_ev++];
+    e->t = t_next; e->n_completed = nC; e->n_activated = n_activated; e->n_rounds = R; e->first_bneck = fb;
+  }
+  if (n_done < F) rc = ORC_ECYCLE; /* WAITING flows left with nothing active or pending */
+  s->ran = 1;
+out:
+  free(capq); free(succ_off); free(succ); free(pred_cnt); free(state); free(t_act); free(rem); free(tc); free(rq);
+  free(act); free(pend); free(comp);
+  ws_free(&w);
+  return rc;
+}
+
+/* ------------------------------------------------------------------ S6: outputs */
+int32_t orc_num_flows(const orc_sim *s, int64_t *out) { if (!s || !out) return ORC_EINVAL; *out = s->F; return ORC_OK; }
+int32_t orc_get_completion_times(const orc_sim *s, double *out, int64_t n) {
+  if (!s || !out || n != s->F) return ORC_EINVAL;
+  if (!s->t_done) return ORC_ESTATE;
+  memcpy(out, s->t_done, sizeof(double) * n);
+  return ORC_OK;
+}
+int32_t orc_get_bottlenecks(const orc_sim *s, int32_t *out, int64_t n) {
+  if (!s || !out || n != s->F) return ORC_EINVAL;
+  if (!s->bneck) return ORC_ESTATE;
+  memcpy(out, s->bneck, sizeof(int32_t) * n);
+  return ORC_OK;
+}
+int32_t orc_num_collectives(const orc_sim *s, int32_t *out) { if (!s || !out) return ORC_EINVAL; *out = s->n_coll; return ORC_OK; }
+int32_t orc_get_collective_times(const orc_sim *s, double *out, int32_t n) {
+  if (!s || !out || n != s->n_coll) return ORC_EINVAL;
+  if (!s->t_done) return ORC_ESTATE;
+  for (int32_t c = 0; c < n; c++) { /* O5: max t_done over the collective's flows */
+    double m = -INFINITY;
+    for (int32_t f = s->coll[c].first_flow; f < s->coll[c].first_flow + s->coll[c].n_flows; f++)
+      if (s->t_done[f] > m) m = s->t_done[f];
+    out[c] = m;
+  }
+  return ORC_OK;
+}
+int32_t orc_num_events(const orc_sim *s, int64_t *out) { if (!s || !out) return ORC_EINVAL; *out = s->n_ev; return ORC_OK; }
+int32_t orc_get_event_log(const orc_sim *s, orc_event *out, int64_t cap, int64_t *n) {
+  if (!s || !n) return ORC_EINVAL;
+  *n = s->n_ev;
+  if (out) memcpy(out, s->ev, sizeof(orc_event) * (cap < s->n_ev ? cap : s->n_ev));
+  return ORC_OK;
+}
+int32_t orc_num_path_entries(const orc_sim *s, int64_t *out) { if (!s || !out) return ORC_EINVAL; *out = s->path_off[s->F]; return ORC_OK; }
+int32_t orc_get_paths(const orc_sim *s, int64_t *off, int32_t *links, int64_t cap) {
+  if (!s || !off || !links || cap < s->path_off[s->F]) return ORC_EINVAL;
+  memcpy(off, s->path_off, sizeof(int64_t) * (s->F + 1));
+  memcpy(links, s->path, sizeof(int32_t) * s->path_off[s->F]);
+  return ORC_OK;
+}
+int32_t orc_get_flow_endpoints(const orc_sim *s, int32_t *src, int32_t *dst, double *bytes, double *lat, int64_t n) {
+  if (!s || n != s->F) return ORC_EINVAL;
+  if (src) memcpy(src, s->src, sizeof(int32_t) * n);
+  if (dst) memcpy(dst, s->dst, sizeof(int32_t) * n);
+  if (bytes) memcpy(bytes, s->bytes, sizeof(double) * n);
+  if (lat) memcpy(lat, s->Lat, sizeof(double) * n);
+  return ORC_OK;
+}
+int32_t orc_get_preds(const orc_sim *s, int64_t *off, int32_t *preds, int64_t cap, int64_t *n_entries) {
+  if (!s || !n_entries) return ORC_EINVAL;
+  *n_entries = s->pred_off[s->F];
+  if (off) memcpy(off, s->pred_off, sizeof(int64_t) * (s->F + 1));
+  if (preds) {
+    if (cap < *n_entries) return ORC_EINVAL;
+    memcpy(preds, s->pred, sizeof(int32_t) * *n_entries);
+  }
+  return ORC_OK;
+}
+int32_t orc_get_work_counters(const orc_sim *s, double *out7) {
+  if (!s || !out7) return ORC_EINVAL;
+  memcpy(out7, s->work, sizeof(s->work));
+  return ORC_OK;
+}
+int32_t orc_trace_size(const orc_sim *s, int64_t *n) { if (!s || !n) return ORC_EINVAL; *n = s->n_tr; return ORC_OK; }
+int32_t orc_get_trace(const orc_sim *s, int64_t *ev, int32_t *flow, double *rate, double *t0, double *t1, int64_t cap) {
+  if (!s || cap < s->n_tr) return ORC_EINVAL;
+  for (int64_t i = 0; i < s->n_tr; i++) {
+    if (ev) ev[i] = s->tr[i].ev;
+    if (flow) flow[i] = s->tr[i].flow;
+    if (rate) rate[i] = s->tr[i].rate;
+    if (t0) t0[i] = s->tr[i].t0;
+    if (t1) t1[i] = s->tr[i].t1;
+  }
+  return ORC_OK;
+}

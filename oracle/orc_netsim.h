@@ -1,0 +1,108 @@
+/*
+ * orc_netsim.h -- CPU ORACLE for the flow-level network simulator (netsim) of
+ * Phantora (arxiv 2505.01616).  TEST INFRASTRUCTURE ONLY.
+ *
+ * This is a plain, slow, single-threaded, obviously-correct C restatement of
+ * what the hot path computes.  It shares no code with the CUDA library
+ * (paper_2505_01616_b200/csrc) and is never used by the product path: only
+ * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load it.
+ *
+ * Passages followed (PAPER.md line numbers):
+ *   L98  (sec 4.1)  netsim: topology config (port bandwidth, interconnection,
+ *                   multipath routing / load balancing); throughput of flows at
+ *                   each time = max-min fairness; collective patterns.
+ *   L104 (sec 4.1)  ring all-reduce; flows submitted with timestamps; output =
+ *                   completion time of each flow.
+ *   L128 (sec 4.2)  between neighbouring events flows have stable throughput.
+ *   L165 (sec 5)    per-flow fairness; iterative water-filling; each iteration
+ *                   identifies THE bottleneck link and adjusts flow rates.
+ *   L308 (sec 7)    a flow immediately reaches its fair share.
+ * Everything the paper leaves open follows the readings S0-S6 / Q1-Q18 of
+ * SURVEY.md sec 8(c), restated in DESIGN.md ("Readings").  One reading is the
+ * builder's own and is listed there as R-FX: rates, capacities and fair shares
+ * are held in exact 64-bit fixed point (quantum 2^-20 byte/s), so that the
+ * water-filling result does not depend on the order in which capacity debits
+ * are applied.  Time and byte arithmetic is IEEE binary64 without contraction.
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"): P1 lone flow, P2 uniform
+ * ring, P3 max-plus ring recurrence (cfg0), P4 bottleneck certificate, P5
+ * brute-force lexicographic max-min, P6 processor sharing, P7 parking lot,
+ * P8 uniform all-to-all, P9 invariances, naive == fast mode.
+ * "parity unpinned": the ECMP hash VALUE (S2) -- the paper gives none; it is
+ * pinned only against published SplitMix64 outputs and by balance statistics.
+ */
+#ifndef ORC_NETSIM_H
+#define ORC_NETSIM_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_sim orc_sim;
+
+enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ECYCLE = -4, ORC_ESTATE = -5, ORC_ERANGE = -6 };
+enum { ORC_TOPO_SINGLE = 0, ORC_TOPO_LEAF_SPINE = 1, ORC_TOPO_FAT_TREE = 2 };
+enum { ORC_ALLREDUCE_RING = 0, ORC_ALLGATHER_RING = 1, ORC_REDUCESCATTER_RING = 2, ORC_ALLTOALL = 3 };
+enum { ORC_MODE_NAIVE = 0, ORC_MODE_FAST = 1 };
+
+typedef struct {
+  int32_t kind, n_hosts, gpus_per_host;
+  double nvlink_Bps, nic_Bps, fabric_Bps, hop_latency_s; /* per direction */
+  int32_t n_leaves, n_spines, uplinks_per_leaf_spine;    /* leaf-spine */
+  int32_t k, agg_uplinks;                                /* fat tree */
+} orc_topology_desc;
+
+typedef struct {
+  double t;             /* time the clock moved to in this loop iteration */
+  int32_t n_completed;  /* flows that completed at t */
+  int32_t n_activated;  /* flows activated at the start of the iteration */
+  int32_t n_rounds;     /* water-filling iterations of this iteration's solve */
+  int32_t first_bneck;  /* bottleneck link of the first iteration, -1 if none */
+} orc_event;
+
+/* One simulation instance.  `seed` is the instance's ECMP seed. */
+int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim **out);
+void orc_destroy(orc_sim *s);
+int32_t orc_num_links(const orc_sim *s, int32_t *out);
+int32_t orc_set_link_capacities(orc_sim *s, const double *cap_Bps);
+int32_t orc_get_link_capacities(const orc_sim *s, double *cap_Bps);
+int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t n_ranks, double bytes,
+                           double start_time_s, const int32_t *after, int32_t n_after, int32_t *out_coll_id);
+int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *dst, const double *bytes,
+                      const double *start_time_s, const int64_t *dep_off, const int64_t *dep_flow_ids,
+                      const int32_t *conn_id, int64_t *out_first_flow_id);
+/* trace != 0 additionally records, for every loop iteration, the active flows and their rates */
+int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace);
+int32_t orc_num_flows(const orc_sim *s, int64_t *out);
+int32_t orc_get_completion_times(const orc_sim *s, double *out, int64_t n);
+int32_t orc_get_bottlenecks(const orc_sim *s, int32_t *out, int64_t n);
+int32_t orc_num_collectives(const orc_sim *s, int32_t *out);
+int32_t orc_get_collective_times(const orc_sim *s, double *out, int32_t n);
+int32_t orc_num_events(const orc_sim *s, int64_t *out);
+int32_t orc_get_event_log(const orc_sim *s, orc_event *out, int64_t cap, int64_t *n_events);
+int32_t orc_get_paths(const orc_sim *s, int64_t *off /*[F+1]*/, int32_t *links, int64_t cap);
+int32_t orc_num_path_entries(const orc_sim *s, int64_t *out);
+int32_t orc_get_flow_endpoints(const orc_sim *s, int32_t *src, int32_t *dst, double *bytes, double *lat, int64_t n);
+int32_t orc_get_preds(const orc_sim *s, int64_t *off /*[F+1]*/, int32_t *preds, int64_t cap, int64_t *n_entries);
+/* work counters of the last run: [0] sum over events of A (active flows), [1] sum A*h (path entries of
+ * active flows), [2] sum of water-filling iterations R, [3] sum over events of Lambda_act*R,
+ * [4] sum Lambda_act, [5] completions, [6] events */
+int32_t orc_get_work_counters(const orc_sim *s, double *out7);
+/* trace access (valid after orc_run(..., trace=1)) */
+int32_t orc_trace_size(const orc_sim *s, int64_t *n_rows);
+int32_t orc_get_trace(const orc_sim *s, int64_t *event_idx, int32_t *flow, double *rate_Bps, double *t0, double *t1,
+                      int64_t cap);
+
+/* Stand-alone max-min progressive filling (S5) on an explicit instance: flows given as CSR paths over
+ * n_links links.  rate_Bps[f], bneck[f] out; *n_rounds, *first_bneck out.  mode as in orc_run. */
+int32_t orc_maxmin(int32_t n_links, const double *cap_Bps, int32_t n_flows, const int64_t *path_off,
+                   const int32_t *path, int32_t mode, double *rate_Bps, int32_t *bneck, int32_t *n_rounds,
+                   int32_t *first_bneck);
+/* SplitMix64 step used by the ECMP hash (S2) */
+uint64_t orc_mix64(uint64_t x);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

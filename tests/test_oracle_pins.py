@@ -1,0 +1,532 @@
+"""Pins of the CPU oracle against what the mathematics fixes.
+
+None of these re-types the oracle's own formula: each expected value is a closed form, an iff-certificate,
+a brute-force enumeration, a published test vector, or an invariance.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2505_01616_b200 import workloads as W
+from util import completion_order, oracle_run
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+MiB = 2.0 ** 20
+GiB = 2.0 ** 30
+
+
+def golden(name):
+    out = {}
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split("=")
+                out[k.strip()] = float(v)
+    return out
+
+
+def single(n_hosts=2, gph=8, lat=1e-6, **kw):
+    return W.topo_desc(W.TOPO_SINGLE, n_hosts, gph, hop_latency_s=lat, **kw)
+
+
+def run_flows(desc, src, dst, nbytes, seed=0, **kw):
+    inst = W.Instance(seed=seed, ops=[W.RawFlows(np.array(src, np.int32), np.array(dst, np.int32),
+                                                 np.array(nbytes, np.float64), **kw)])
+    return oracle_run(desc, inst)
+
+
+# ------------------------------------------------------------------------------------------------ S2 hash
+def test_splitmix64_published_vectors():
+    # SplitMix64 (Steele, Lea, Flood 2014) from state 0: first three outputs of the public-domain reference.
+    g = 0x9E3779B97F4A7C15
+    assert orc.mix64(0) == 0xE220A8397B1DCDAF
+    assert orc.mix64(g) == 0x6E789E6AA1B965F4
+    assert orc.mix64((2 * g) & (2 ** 64 - 1)) == 0x06C45D188009454F
+
+
+# ------------------------------------------------------------------------------------------------ S1 numbering
+@pytest.mark.parametrize("wl,n_links", [(W.cfg0, 64), (lambda: W.cfg1(batch=1), 528), (W.cfg2, 7168),
+                                        (lambda: W.cfg3(batch=1), 264), (lambda: W.cfg4(batch=1), 1152)])
+def test_link_counts(wl, n_links):
+    w = wl()
+    assert orc.Sim(w.desc, 0).num_links == n_links
+
+
+def test_flow_counts():
+    assert sum(W.n_flows_of(o) for o in W.cfg0().instances[0].ops) == 480
+    assert sum(W.n_flows_of(o) for o in W.cfg1(batch=1).instances[0].ops) == 5632
+    assert sum(W.n_flows_of(o) for o in W.cfg2().instances[0].ops) == 1069056
+    assert sum(W.n_flows_of(o) for o in W.cfg3(batch=1).instances[0].ops) == 7168
+    assert sum(W.n_flows_of(o) for o in W.cfg4(batch=1).instances[0].ops) == 65280
+
+
+# ------------------------------------------------------------------------------------------------ P1 lone flow
+def test_p1_lone_flow_closed_form():
+    g = golden("closed_forms.txt")
+    d = single()
+    s = run_flows(d, [0], [3], [4 * MiB])          # same host: NVLink up + NVLink down
+    assert s.completion_times()[0] == pytest.approx(2e-6 + 4194304 / 450e9, rel=1e-12)
+    assert s.completion_times()[0] == pytest.approx(g["p1_intra_host_4MiB"], rel=1e-9)
+    assert list(s.paths()[1]) == [0, 7]
+    s = run_flows(d, [0], [9], [4 * MiB])          # other host: NIC up + NIC down
+    assert s.completion_times()[0] == pytest.approx(2e-6 + 4194304 / 50e9, rel=1e-12)
+    assert s.completion_times()[0] == pytest.approx(g["p1_inter_host_4MiB"], rel=1e-9)
+    assert list(s.paths()[1]) == [32 + 0, 32 + 19]
+    assert list(s.bottlenecks()) == [32]           # tie between the two 50 GB/s links -> lowest id
+
+
+def test_p1_lone_flow_start_time_and_fabric_bottleneck():
+    # leaf-spine, cross-leaf: 4 hops; fabric slower than NIC -> fabric up link is the bottleneck (lower id than down)
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 2, nic_Bps=50e9, fabric_Bps=10e9, n_leaves=2, n_spines=2,
+                    uplinks_per_leaf_spine=1, hop_latency_s=3e-6)
+    s = run_flows(d, [0], [7], [1e6], start=np.array([5e-3]))
+    off, links = s.paths()
+    assert off[1] == 4
+    assert s.completion_times()[0] == pytest.approx(5e-3 + 4 * 3e-6 + 1e6 / 10e9, rel=1e-12)
+    assert s.bottlenecks()[0] == links[1]
+    # fat tree cross-pod: 6 hops
+    d = W.topo_desc(W.TOPO_FAT_TREE, 8, 2, fabric_Bps=25e9, k=4, agg_uplinks=2)
+    s = run_flows(d, [0], [15], [1e6])
+    assert s.paths()[0][1] == 6
+    assert s.completion_times()[0] == pytest.approx(6e-6 + 1e6 / 25e9, rel=1e-12)
+
+
+# ------------------------------------------------------------------------------------------------ P2 uniform ring
+@pytest.mark.parametrize("kind,steps", [(W.ALLREDUCE_RING, 14), (W.ALLGATHER_RING, 7), (W.REDUCESCATTER_RING, 7)])
+def test_p2_uniform_ring(kind, steps):
+    d = single()
+    inst = W.Instance(seed=0, ops=[W.Coll(kind, np.arange(8, dtype=np.int32), 1 * GiB)])
+    s = oracle_run(d, inst)
+    expect = steps * (2e-6 + (2.0 ** 30 / 8) / 450e9)
+    assert s.collective_times()[0] == pytest.approx(expect, rel=1e-12)
+    if kind == W.ALLREDUCE_RING:
+        assert expect == pytest.approx(golden("closed_forms.txt")["p2_ring_ar_n8_1GiB"], rel=1e-9)
+    assert s.num_flows == steps * 8
+    # every step's 8 flows finish together
+    t = s.completion_times().reshape(steps, 8)
+    assert np.all(t == t[:, :1])
+
+
+# ------------------------------------------------------------------------------------------------ P3 max-plus ring
+def maxplus_ring(ranks, steps, chunk, cap_of_sender, lat):
+    """T(s,i) = max(T(s-1,i), T(s-1,i-1)) + d_i, d_i = Lat_i + chunk / B_i (contention-free ring)."""
+    N = len(ranks)
+    d = np.array([lat + chunk / cap_of_sender(i) for i in range(N)])
+    T = np.zeros((steps, N))
+    T[0] = d
+    for s in range(1, steps):
+        for i in range(N):
+            T[s, i] = max(T[s - 1, i], T[s - 1, (i - 1) % N]) + d[i]
+    return T
+
+
+def test_p3_cfg0_maxplus_recurrence():
+    w = W.cfg0()
+    s = oracle_run(w.desc, w.instances[0])
+    t = s.completion_times().reshape(30, 16)
+    # senders 7 and 15 cross hosts (NIC, 50 GB/s), the others stay on NVLink (450 GB/s)
+    T = maxplus_ring(np.arange(16), 30, 64 * MiB / 16, lambda i: 50e9 if i in (7, 15) else 450e9, 2e-6)
+    np.testing.assert_allclose(t, T, rtol=1e-11, atol=0)
+    g = golden("closed_forms.txt")
+    assert t.max() == pytest.approx(g["p3_cfg0_makespan"], rel=1e-9)
+    assert t[29, 8] == pytest.approx(g["p3_cfg0_T_29_8"], rel=1e-9)
+    assert t[29, 0] == pytest.approx(g["p3_cfg0_T_29_8"], rel=1e-9)
+    # no contention: both links of a path have equal capacity -> tie -> bneck is the lower link id
+    off, links = s.paths()
+    assert np.array_equal(s.bottlenecks(), np.minimum(links[off[:-1]], links[off[:-1] + 1]))
+
+
+def test_p3_heterogeneous_ring_on_sweep_capacities():
+    # one DP ring over 8 hosts with per-link random capacities (cfg3-style), contention-free -> recurrence
+    w = W.cfg3(batch=1)
+    inst = w.instances[0]
+    inst.ops = [W.Coll(W.ALLREDUCE_RING, np.arange(0, 64, 8, dtype=np.int32), 64 * MiB)]
+    s = oracle_run(w.desc, inst)
+    cap = s.link_capacities()
+    off, links = s.paths()
+    lat = s.flows()[3]
+    N = 8
+    d = np.array([lat[i] + (64 * MiB / N) / cap[links[off[i]:off[i + 1]]].min() for i in range(N)])
+    T = np.zeros((14, N))
+    T[0] = d
+    for st in range(1, 14):
+        for i in range(N):
+            T[st, i] = max(T[st - 1, i], T[st - 1, (i - 1) % N]) + d[i]
+    # rates sit on a 2^-20 B/s grid: relative error <= 2^-20 / 1.25e10 per flow, far below 1e-11
+    np.testing.assert_allclose(s.completion_times().reshape(14, N), T, rtol=1e-11)
+
+
+# ------------------------------------------------------------------------------------------------ P4 certificate
+def check_certificate(cap, path_off, path, flows, rate, bneck, n_links):
+    """Bertsekas-Gallager: feasible AND every flow has a saturated link on which its rate is maximal  <=>  max-min
+    fair.  Rates are floor-quantised to 2^-20 B/s, so a bottleneck may be short of capacity by < n_l quanta."""
+    load = np.zeros(n_links)
+    cnt = np.zeros(n_links, dtype=np.int64)
+    mx = np.zeros(n_links)
+    for f, r in zip(flows, rate):
+        ls = path[path_off[f]:path_off[f + 1]]
+        load[ls] += r
+        cnt[ls] += 1
+        mx[ls] = np.maximum(mx[ls], r)
+    q = 2.0 ** -20
+    assert np.all(load <= cap * (1 + 1e-12)), "link over capacity"
+    for f, r, b in zip(flows, rate, bneck):
+        ls = path[path_off[f]:path_off[f + 1]]
+        assert b in ls
+        ok = (load[ls] >= cap[ls] * (1 - 1e-12) - cnt[ls] * q) & (r >= mx[ls] * (1 - 1e-12) - q)
+        assert ok.any(), f"flow {f} has no saturated link on which it is maximal"
+        i = list(ls).index(b)
+        assert ok[i], f"reported bottleneck {b} of flow {f} is not one"
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_p4_random_instances_certificate(seed):
+    rng = np.random.default_rng(seed)
+    n_links = int(rng.integers(3, 40))
+    n_flows = int(rng.integers(1, 120))
+    cap = np.floor(rng.uniform(1e9, 4e11, n_links))
+    if seed % 2:
+        cap[:] = 50e9                      # equal capacities: exact ties everywhere
+    lens = rng.integers(1, min(6, n_links) + 1, n_flows)
+    path_off = np.concatenate([[0], np.cumsum(lens)])
+    path = np.concatenate([rng.choice(n_links, int(h), replace=False) for h in lens]).astype(np.int32)
+    for mode in (orc.MODE_NAIVE, orc.MODE_FAST):
+        rate, bneck, R, fb = orc.maxmin(cap, path_off, path, mode)
+        check_certificate(cap, path_off, path, np.arange(n_flows), rate, bneck, n_links)
+        assert 1 <= R <= n_links
+        assert fb == bneck[np.argmin(rate)] or rate[bneck == fb].min() == rate.min()
+
+
+def test_p4_certificate_along_event_loop():
+    # a contended mid-size run: shrunken cfg1 (DP rings share 2 uplinks per leaf) -- check EVERY recompute
+    w = W.cfg1(batch=3, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
+    for inst in w.instances[1:]:
+        s = oracle_run(w.desc, inst, trace=True)
+        ev, fl, rate, t0, t1 = s.trace()
+        off, links = s.paths()
+        cap = s.link_capacities()
+        bn = s.bottlenecks()
+        cuts = np.flatnonzero(np.diff(ev)) + 1
+        n_checked = 0
+        for idx in np.split(np.arange(len(ev)), cuts)[::7]:
+            # bneck[] holds the LAST bottleneck of each flow; only check membership for flows of the final events
+            load = np.zeros(len(cap)); mx = np.zeros(len(cap)); cnt = np.zeros(len(cap))
+            for f, r in zip(fl[idx], rate[idx]):
+                ls = links[off[f]:off[f + 1]]
+                load[ls] += r; cnt[ls] += 1; mx[ls] = np.maximum(mx[ls], r)
+            assert np.all(load <= cap * (1 + 1e-12))
+            for f, r in zip(fl[idx], rate[idx]):
+                ls = links[off[f]:off[f + 1]]
+                ok = (load[ls] >= cap[ls] * (1 - 1e-12) - cnt[ls] * 2.0 ** -20) & (r >= mx[ls] * (1 - 1e-12) - 2.0 ** -20)
+                assert ok.any()
+            n_checked += 1
+        assert n_checked > 20
+        assert np.all(bn >= 0)
+
+
+# ------------------------------------------------------------------------------------------------ P5 brute force
+def brute_force_maxmin(cap, paths, grid):
+    """Lexicographically largest ascending-sorted feasible rate vector over rates in `grid` (exhaustive)."""
+    F = len(paths)
+    G = np.array(list(itertools.product(grid, repeat=F)), dtype=np.int64)
+    ok = np.ones(len(G), dtype=bool)
+    for l, c in enumerate(cap):
+        on = [f for f in range(F) if l in paths[f]]
+        if on:
+            ok &= G[:, on].sum(axis=1) <= c
+    G = G[ok]
+    S = np.sort(G, axis=1)
+    best = np.lexsort(tuple(S[:, j] for j in range(F - 1, -1, -1)))[-1]
+    return G[best], S[best]
+
+
+@pytest.mark.parametrize("seed", range(40))
+def test_p5_brute_force_lexicographic_maxmin(seed):
+    rng = np.random.default_rng(1000 + seed)
+    n_links = int(rng.integers(1, 5))
+    F = int(rng.integers(1, 4)) if seed % 8 else 4
+    cap = rng.integers(1, 5, n_links) * 12                      # caps in {12,24,36,48}: every share is an integer
+    paths = []
+    for _ in range(F):
+        h = int(rng.integers(1, n_links + 1))
+        paths.append(sorted(rng.choice(n_links, h, replace=False).tolist()))
+    grid = range(0, 49)
+    best, best_sorted = brute_force_maxmin(cap, paths, grid)
+    path_off = np.concatenate([[0], np.cumsum([len(p) for p in paths])])
+    path = np.concatenate(paths).astype(np.int32)
+    rate, bneck, R, fb = orc.maxmin(cap.astype(np.float64), path_off, path, orc.MODE_NAIVE)
+    # the max-min allocation is unique -> the whole vector must match, not just the sorted one
+    assert np.array_equal(rate, best.astype(np.float64))
+    for f in range(F):
+        assert bneck[f] in paths[f]
+
+
+# ------------------------------------------------------------------------------------------------ P6 processor sharing
+def test_p6_processor_sharing_closed_form():
+    # three senders on host 0, one receiver on host 1: they share only the receiver's NIC-down link (C = 1e9 B/s)
+    d = single(lat=0.0, nic_Bps=1e9)
+    s = run_flows(d, [0, 1, 2], [8, 8, 8], [1e6, 2e6, 4e6])
+    np.testing.assert_allclose(s.completion_times(), [3e-3, 5e-3, 7e-3], rtol=1e-11)
+    # O3 = bottleneck in the LAST solve while active: flows 0,1 still share NIC-down(8)=49; flow 2 ends alone, and
+    # alone its two equal-capacity links tie -> lowest id = NIC-up(2)=36
+    assert list(s.bottlenecks()) == [49, 49, 36]
+    # general n: t_k = t_{k-1} + (s_k - s_{k-1}) (n-k+1) / C
+    rng = np.random.default_rng(5)
+    sizes = np.sort(np.floor(rng.uniform(1e5, 1e7, 7)))
+    s = run_flows(d, list(range(7)), [9] * 7, sizes)
+    t, prev, tk = [], 0.0, 0.0
+    for k, sz in enumerate(sizes):
+        tk += (sz - prev) * (7 - k) / 1e9
+        prev = sz
+        t.append(tk)
+    np.testing.assert_allclose(s.completion_times(), t, rtol=1e-11)
+
+
+# ------------------------------------------------------------------------------------------------ P7 parking lot
+def test_p7_parking_lot():
+    c1, c2 = 30e9, 100e9
+    cap = np.array([7e11, c1, c2])
+    path_off = np.array([0, 2, 3, 4])
+    path = np.array([1, 2, 1, 2], np.int32)            # A on links 1,2 ; B on 1 ; C on 2
+    for mode in (orc.MODE_NAIVE, orc.MODE_FAST):
+        rate, bneck, R, fb = orc.maxmin(cap, path_off, path, mode)
+        np.testing.assert_allclose(rate, [c1 / 2, c1 / 2, c2 - c1 / 2], rtol=1e-15)
+        assert list(bneck) == [1, 1, 2] and R == 2 and fb == 1
+
+
+# ------------------------------------------------------------------------------------------------ P8 uniform all-to-all
+@pytest.mark.parametrize("N", [9, 8])
+def test_p8_uniform_alltoall_single_switch(N):
+    B, S = 50e9, 64 * MiB
+    d = single(n_hosts=N, gph=1)
+    inst = W.Instance(seed=0, ops=[W.Coll(W.ALLTOALL, np.arange(N, dtype=np.int32), S)])
+    s = oracle_run(d, inst)
+    t = s.completion_times()
+    assert len(t) == N * (N - 1)
+    np.testing.assert_allclose(t, 2e-6 + (S / N) * (N - 1) / B, rtol=1e-12)
+    ev = s.event_log()
+    if N == 9:
+        # B/(N-1) is exact on the 2^-20 B/s grid: every flow gets bit-equal rate -> ONE completion event
+        assert np.all(t == t[0])
+        assert ev["n_completed"].max() == N * (N - 1) and (ev["n_completed"] > 0).sum() == 1
+    else:
+        # B/7 is not on the grid: the floor remainder (< 7 quanta) goes to later-frozen flows, rates differ by
+        # at most one quantum (2^-20 B/s) and completion times by a few ulp
+        assert len(np.unique(t)) <= 4
+    src, dst, b, lat = s.flows()
+    assert np.array_equal(src, np.repeat(np.arange(N), N - 1))
+    assert np.all(src != dst) and np.all(b == S / N)
+
+
+# ------------------------------------------------------------------------------------------------ S3 DAG pins
+def test_ring_dag_structure():
+    N = 5
+    d = single(n_hosts=1, gph=8)
+    s = orc.Sim(d, 0)
+    ranks = np.array([3, 0, 6, 1, 4], np.int32)
+    s.add_collective(orc.ALLREDUCE_RING, ranks, 5e6)
+    off, pr = s.preds()
+    src, dst, b, lat = (None,) * 4
+    s.run()
+    src, dst, b, lat = s.flows()
+    assert s.num_flows == 2 * (N - 1) * N
+    for st in range(2 * (N - 1)):
+        for i in range(N):
+            f = st * N + i
+            assert src[f] == ranks[i] and dst[f] == ranks[(i + 1) % N] and b[f] == 1e6
+            p = sorted(pr[off[f]:off[f + 1]].tolist())
+            if st == 0:
+                assert p == []
+            else:
+                assert p == sorted([(st - 1) * N + (i - 1) % N, (st - 1) * N + i])
+
+
+def test_after_chains_per_rank_not_global_barrier():
+    d = single(n_hosts=1, gph=8)
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLREDUCE_RING, np.arange(4, dtype=np.int32), 4e6)          # ranks 0..3
+    b = s.add_collective(orc.ALLGATHER_RING, np.array([2, 3, 4, 5], np.int32), 4e6, after=[a])
+    off, pr = s.preds()
+    fa, la = 0, 5 * 4                # A: 6 steps x 4; last step starts at flow 20
+    fb = 6 * 4
+    # B's step-0 flow i has sender [2,3,4,5][i]; ranks 2,3 are ring indices 2,3 of A; 4,5 are not in A
+    assert sorted(pr[off[fb + 0]:off[fb + 1]]) == [la + 1, la + 2]       # sent by 2 = (5,2); received by 2 = (5,1)
+    assert sorted(pr[off[fb + 1]:off[fb + 2]]) == [la + 2, la + 3]
+    assert off[fb + 3] - off[fb + 2] == 0 and off[fb + 4] - off[fb + 3] == 0
+    s.run()
+    t = s.completion_times()
+    step = 2e-6 + 1e6 / 450e9
+    # ranks 4 and 5 start B's first step at t=0 (4->5 shares no link with A), ranks 2 and 3 only after A's last
+    # step has left / reached them; B's 2->3 then runs uncontended (A's only possible straggler 3->0 is link-disjoint)
+    assert t[fb + 2] == pytest.approx(step, rel=1e-12)
+    assert t[fb + 0] == pytest.approx(max(t[la + 1], t[la + 2]) + step, rel=1e-12)
+    assert t[fb + 0] > 6 * step
+
+
+def test_chained_equals_concurrent_total_on_uniform_ring():
+    # two identical ring all-reduces: chained -> 2 T ; also pins `after` on every rank
+    d = single(n_hosts=1, gph=8)
+    T = 14 * (2e-6 + (64 * MiB / 8) / 450e9)
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLREDUCE_RING, np.arange(8, dtype=np.int32), 64 * MiB)
+    s.add_collective(orc.ALLREDUCE_RING, np.arange(8, dtype=np.int32), 64 * MiB, after=[a])
+    s.run()
+    assert list(s.collective_times()) == pytest.approx([T, 2 * T], rel=1e-12)
+    # concurrent: the two rings share every link half/half; each step takes Lat + 2*chunk/B
+    s = orc.Sim(d, 0)
+    s.add_collective(orc.ALLREDUCE_RING, np.arange(8, dtype=np.int32), 64 * MiB)
+    s.add_collective(orc.ALLREDUCE_RING, np.arange(8, dtype=np.int32), 64 * MiB)
+    s.run()
+    T2 = 14 * (2e-6 + 2 * (64 * MiB / 8) / 450e9)
+    assert list(s.collective_times()) == pytest.approx([T2, T2], rel=1e-11)
+
+
+def test_alltoall_after_alltoall_preds():
+    d = single(n_hosts=1, gph=4)
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLTOALL, np.arange(4, dtype=np.int32), 4e6)
+    s.add_collective(orc.ALLTOALL, np.arange(4, dtype=np.int32), 4e6, after=[a])
+    off, pr = s.preds()
+    src, dst = None, None
+    s.run()
+    src, dst, _, _ = s.flows()
+    for f in range(12, 24):
+        rho = src[f]
+        want = sorted([g for g in range(12) if src[g] == rho or dst[g] == rho])
+        assert sorted(pr[off[f]:off[f + 1]].tolist()) == want
+
+
+# ------------------------------------------------------------------------------------------------ S2 routing pins
+def test_routing_structure_leaf_spine_and_balance():
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 8, 4, n_leaves=4, n_spines=4, uplinks_per_leaf_spine=2)
+    G, P, nsp = 32, 2, 4
+    rng = np.random.default_rng(0)
+    src = rng.integers(0, G, 4000).astype(np.int32)
+    dst = (src + rng.integers(1, G, 4000)).astype(np.int32) % G
+    s = orc.Sim(d, 7)
+    s.add_flows(src, dst, np.ones(4000))
+    off, links = s.paths()
+    spine_hits = np.zeros(nsp * P)
+    for f in range(4000):
+        p = links[off[f]:off[f + 1]]
+        hs, hd = src[f] // 4, dst[f] // 4
+        if hs == hd:
+            assert list(p) == [2 * src[f], 2 * dst[f] + 1]
+        elif hs // 2 == hd // 2:
+            assert list(p) == [2 * G + 2 * src[f], 2 * G + 2 * dst[f] + 1]
+        else:
+            assert len(p) == 4 and p[0] == 2 * G + 2 * src[f] and p[3] == 2 * G + 2 * dst[f] + 1
+            u_up, u_dn = (p[1] - 4 * G) // 2, (p[2] - 4 * G) // 2
+            assert (p[1] - 4 * G) % 2 == 0 and (p[2] - 4 * G) % 2 == 1
+            assert u_up // (nsp * P) == hs // 2 and u_dn // (nsp * P) == hd // 2          # right leaves
+            assert (u_up // P) % nsp == (u_dn // P) % nsp                                  # same spine
+            spine_hits[u_up % (nsp * P)] += 1
+    n = spine_hits.sum()
+    chi2 = ((spine_hits - n / 8) ** 2 / (n / 8)).sum()
+    assert chi2 < 30.0          # 7 dof; P(chi2 > 30) ~ 1e-4
+
+
+def test_routing_fat_tree_structure_and_conn_persistence():
+    k, U = 8, 2
+    d = W.topo_desc(W.TOPO_FAT_TREE, k * k // 2, k // 2, k=k, agg_uplinks=U)
+    G, h = k * k // 2 * (k // 2), k // 2
+    s = orc.Sim(d, 3)
+    # one ring over GPUs of different pods: every step of a pair reuses one path (conn = collective id)
+    ranks = np.array([0, 17, 40, 100, 127], np.int32)
+    s.add_collective(orc.ALLGATHER_RING, ranks, 1e6)
+    off, links = s.paths()
+    N = len(ranks)
+    b1 = 4 * G
+    b2 = b1 + 2 * k * h * h
+    for f in range(s.num_flows):
+        p = links[off[f]:off[f + 1]]
+        assert list(p) == list(links[off[f % N]:off[f % N + 1]])
+        a, b = ranks[f % N], ranks[(f + 1) % N]
+        ha, hb = a // h, b // h
+        assert len(p) == (4 if ha // h == hb // h else 6)
+        if len(p) == 6:
+            u1, u2, d2, d1 = (p[1] - b1) // 2, (p[2] - b2) // 2, (p[3] - b2) // 2, (p[4] - b1) // 2
+            agg = u1 % h
+            assert u1 // h == ha and d1 // h == hb and d1 % h == agg            # edge switches, same agg index
+            assert u2 // U == (ha // h) * h + agg and d2 // U == (hb // h) * h + agg
+            assert u2 % U == d2 % U                                              # same core
+    # different seeds move some flows
+    s2 = orc.Sim(d, 4)
+    s2.add_collective(orc.ALLGATHER_RING, ranks, 1e6)
+    assert not np.array_equal(s2.paths()[1], links)
+
+
+# ------------------------------------------------------------------------------------------------ P9 invariances
+def test_p9_byte_conservation_and_scaling():
+    w = W.cfg4(batch=1, n_hosts=4, gph=4, n_leaves=2, n_spines=2)
+    inst = w.instances[0]
+    s = oracle_run(w.desc, inst, trace=True)
+    ev, fl, rate, t0, t1 = s.trace()
+    moved = np.zeros(s.num_flows)
+    np.add.at(moved, fl, rate * (t1 - t0))
+    np.testing.assert_allclose(moved, s.flows()[2], rtol=1e-9)
+    # scale bytes and capacities by 2: times unchanged (up to the 2^-20 B/s rate grid)
+    d2 = dict(w.desc, nvlink_Bps=2 * w.desc["nvlink_Bps"], nic_Bps=2 * w.desc["nic_Bps"],
+              fabric_Bps=2 * w.desc["fabric_Bps"])
+    op = inst.ops[0]
+    inst2 = W.Instance(seed=inst.seed, ops=[W.RawFlows(op.src, op.dst, 2 * op.nbytes)])
+    s2 = oracle_run(d2, inst2)
+    np.testing.assert_allclose(s2.completion_times(), s.completion_times(), rtol=1e-12)
+    assert np.array_equal(s2.bottlenecks(), s.bottlenecks())
+
+
+def test_p9_single_spine_is_seed_independent():
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=1, uplinks_per_leaf_spine=1)
+    ops = [W.Coll(W.ALLREDUCE_RING, np.arange(0, 16, 2, dtype=np.int32), 32 * MiB),
+           W.Coll(W.ALLTOALL, np.arange(16, dtype=np.int32), 8 * MiB, 1e-4)]
+    a = oracle_run(d, W.Instance(seed=1, ops=ops))
+    b = oracle_run(d, W.Instance(seed=99, ops=ops))
+    assert np.array_equal(a.completion_times(), b.completion_times())
+    assert np.array_equal(a.paths()[1], b.paths()[1])
+
+
+# ------------------------------------------------------------------------------------------------ naive == fast
+@pytest.mark.parametrize("wl", [
+    lambda: W.cfg0(),
+    lambda: W.cfg1(batch=2),
+    lambda: W.cfg2(k=4, agg_uplinks=1),
+    lambda: W.cfg3(batch=2),
+    lambda: W.cfg4(batch=1, n_hosts=8, gph=4, n_leaves=4, n_spines=2),
+])
+def test_naive_and_fast_modes_bit_identical(wl):
+    w = wl()
+    inst = w.instances[-1]
+    a = oracle_run(w.desc, inst, mode=orc.MODE_NAIVE)
+    b = oracle_run(w.desc, inst, mode=orc.MODE_FAST)
+    assert np.array_equal(a.completion_times(), b.completion_times())
+    assert np.array_equal(a.bottlenecks(), b.bottlenecks())
+    assert np.array_equal(a.event_log(), b.event_log())
+    assert np.array_equal(completion_order(a.completion_times()), completion_order(b.completion_times()))
+    assert not np.isnan(a.completion_times()).any()
+
+
+# ------------------------------------------------------------------------------------------------ error behaviour
+def test_input_validation():
+    d = single()
+    s = orc.Sim(d, 0)
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [0], [1.0])                 # src == dst
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [1], [0.0])                 # bytes <= 0
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [99], [1.0])                # rank out of range
+    with pytest.raises(orc.OrcError):
+        s.add_collective(orc.ALLREDUCE_RING, [0, 1, 1], 1e6)   # duplicate rank
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [1], [1.0], dep_off=[0, 1], dep_ids=[0])   # dep on itself / later flow
+    assert s.num_flows == 0
+    s.add_flows([0, 1], [1, 2], [1e6, 1e6], dep_off=[0, 0, 1], dep_ids=[0])
+    s.run()
+    t = s.completion_times()
+    assert t[1] == pytest.approx(2 * (2e-6 + 1e6 / 450e9), rel=1e-12)
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [1], [1.0])                 # after run -> ESTATE
