@@ -1,0 +1,155 @@
+/*
+ * phs.h -- C-ABI of libphs: a B200-native (sm_100a) batched flow-level network simulator, the netsim hot
+ * path of Phantora (arxiv 2505.01616).  All entry points are extern "C", take plain pointers and sizes and
+ * never throw.  Pointers are HOST pointers unless the argument says "device".
+ *
+ * What the calls mean, by passage of the paper (PAPER.md line numbers; DESIGN.md gives the readings S0-S6):
+ *   phs_create_topology      L98  "netsim takes a cluster topology configuration as input ... switch port
+ *                                  bandwidth, cluster interconnection, multipath routing and load balancing"
+ *   phs_add_collective       L98/L104 "we implement the communication patterns of different collective
+ *                                  operations ... all reduce using a ring-based approach"
+ *   phs_add_flows            L104 "submits the corresponding data transfer flows to netsim with the
+ *                                  appropriate timestamps"
+ *   phs_run                  L165 max-min fair allocation by iterative water-filling; L128 piecewise-constant
+ *                                  throughput between events; L308 flows reach their fair share at once
+ *   phs_get_completion_times L104 "computes the completion time of each flow"
+ *
+ * Ownership: the caller owns every array it passes; the library copies inputs before returning.  Outputs go
+ * to caller-provided buffers.  Ids are dense and assigned in call order: flow ids per instance start at 0, a
+ * collective's flows are contiguous (ring: step-major, then ring index; all-to-all: row-major without the
+ * diagonal).  A handle is not thread-safe; distinct handles are independent.
+ *
+ * Errors: every call returns a phs_status; <0 is an error and phs_last_error() gives a thread-local message.
+ * The library has NO CPU fallback: phs_finalize / phs_run return PHS_ECUDA when no CUDA device is usable.
+ */
+#ifndef PHS_H
+#define PHS_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct phs_sim phs_sim; /* opaque; owned by the library; freed by phs_destroy */
+typedef int32_t phs_status;
+enum {
+  PHS_OK = 0,
+  PHS_EINVAL = -1, /* bad argument: null pointer, bytes <= 0 or NaN, src == dst, rank out of range, ...   */
+  PHS_ENOMEM = -2, /* host or device allocation failed                                                    */
+  PHS_ECUDA = -3,  /* CUDA failure (no device, launch error, ...); message holds the CUDA string          */
+  PHS_ECYCLE = -4, /* flows left WAITING when nothing is active or pending (dependency never satisfied)   */
+  PHS_ESTATE = -5, /* call not valid in this state (adding after phs_finalize, reading before phs_run)    */
+  PHS_ERANGE = -6  /* size limit exceeded (>= 2^31 flows per instance, capacity < #flows quanta, ...)     */
+};
+typedef enum { PHS_TOPO_SINGLE = 0, PHS_TOPO_LEAF_SPINE = 1, PHS_TOPO_FAT_TREE = 2 } phs_topo_kind;
+typedef enum {
+  PHS_ALLREDUCE_RING = 0,     /* 2(N-1) steps of N flows, chunk = bytes/N      */
+  PHS_ALLGATHER_RING = 1,     /* (N-1) steps; bytes = total gathered size      */
+  PHS_REDUCESCATTER_RING = 2, /* (N-1) steps; bytes = total input size         */
+  PHS_ALLTOALL = 3            /* N(N-1) concurrent flows of bytes/N            */
+} phs_coll_kind;
+
+/* Topology descriptor (S1).  GPU g = host*gpus_per_host + local.  Every physical link is two
+ * directed links with the same capacity; capacities are byte/s PER DIRECTION; every link adds hop_latency_s. */
+typedef struct {
+  int32_t kind;                 /* phs_topo_kind                                                          */
+  int32_t n_hosts, gpus_per_host;
+  double nvlink_Bps;            /* GPU <-> its host's NVSwitch                                            */
+  double nic_Bps;               /* GPU <-> first-tier switch (one NIC per GPU)                            */
+  double fabric_Bps;            /* switch <-> switch                                                      */
+  double hop_latency_s;
+  int32_t n_leaves, n_spines, uplinks_per_leaf_spine; /* leaf-spine: hosts in contiguous blocks per leaf  */
+  int32_t k, agg_uplinks;       /* fat tree: k pods, k/2 edge (= hosts) and k/2 agg switches per pod,
+                                   gpus_per_host = k/2, n_hosts = k*k/2; agg_uplinks per agg switch       */
+} phs_topology_desc;
+
+/* One row of the event log (S6/O4): one loop iteration = one distinct time. */
+typedef struct {
+  double t;            /* time the clock moved to                                                         */
+  int32_t n_completed; /* flows that completed at t                                                       */
+  int32_t n_activated; /* flows activated at the start of the iteration                                   */
+  int32_t n_rounds;    /* bottleneck links frozen by this iteration's max-min solve                       */
+  int32_t first_bneck; /* link with the smallest fair share at the start of the solve, -1 if none active  */
+} phs_event;
+
+/* Per-run work counters, summed over the instances of the last phs_run. */
+typedef struct {
+  int64_t n_events;      /* loop iterations                                                               */
+  int64_t n_flow_events; /* activations + completions = 2 * flows                                         */
+  int64_t sum_active;    /* sum over events of active flows                                               */
+  int64_t sum_par_rounds;/* sum over events of parallel filling rounds executed by the kernels            */
+} phs_counters;
+
+/* Creates `batch` independent instances of one topology.  Instance i routes with ECMP seed `seed + i`.
+ * Host-only; never touches the GPU. */
+phs_status phs_create_topology(const phs_topology_desc *desc, uint64_t seed, int32_t batch, phs_sim **out);
+void phs_destroy(phs_sim *sim);
+phs_status phs_num_links(const phs_sim *sim, int32_t *out);
+phs_status phs_batch(const phs_sim *sim, int32_t *out);
+
+/* Overrides the capacities (byte/s, [n_links], S1 numbering) of one instance (-1: all). */
+phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double *cap_Bps);
+phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double *cap_Bps);
+
+/* Adds one collective over `ranks` (ring order) to `instance` (-1: every instance).  `after_coll_ids`
+ * (nullable) chains it per rank behind earlier collectives of the same instance (S3).
+ * out_coll_id (nullable) receives the collective's id. */
+phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                              double bytes, double start_time_s, const int32_t *after_coll_ids, int32_t n_after,
+                              int32_t *out_coll_id);
+/* Same collective on EVERY instance with per-instance sizes / start times: bytes[batch], start_time_s[batch]
+ * (nullable = 0). */
+phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                    const double *bytes, const double *start_time_s, const int32_t *after_coll_ids,
+                                    int32_t n_after, int32_t *out_coll_id);
+/* Adds n raw flows.  start_time_s nullable (= 0).  dep_off[n+1]/dep_flow_ids (nullable) list, per flow, ids of
+ * EARLIER flows of the same instance that must complete first.  conn_id (nullable = the flow's id) keys ECMP. */
+phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_t *src, const int32_t *dst,
+                         const double *bytes, const double *start_time_s, const int64_t *dep_off,
+                         const int64_t *dep_flow_ids, const int32_t *conn_id, int64_t *out_first_flow_id);
+
+/* Event log on/off (default off) for subsequent runs; must precede phs_finalize. */
+phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);
+
+/* Batch-scheduler policy; must precede phs_finalize.  path: 0 = automatic (one CTA per
+ * instance with shared-memory state when it fits, else one thread-block cluster per instance with state in L2),
+ * 1 = CTA path, 2 = cluster path for every instance.  cta_slots > 0 caps the CTA path's shared-memory slot count
+ * (active flows / pending flows per instance); an instance that exceeds it is re-run on the cluster path. */
+phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
+
+/* Builds the device-resident tables (flow records, flow->link CSR, successor CSR, capacities) and copies them
+ * to the current CUDA device on `cuda_stream` (cudaStream_t; NULL = default stream).  After this call the
+ * instance set is frozen (adds return PHS_ESTATE).  phs_run calls it implicitly if needed. */
+phs_status phs_finalize(phs_sim *sim, void *cuda_stream);
+/* Runs every instance to completion on the GPU (all steps of the hot path in CUDA kernels) and waits for the
+ * result status.  May be called repeatedly; each call restarts from t = 0. */
+phs_status phs_run(phs_sim *sim, void *cuda_stream);
+
+phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out);
+phs_status phs_total_flows(const phs_sim *sim, int64_t *out);
+phs_status phs_num_collectives(const phs_sim *sim, int32_t instance, int32_t *out);
+/* out[n] with n == flows of the instance; out_is_device != 0: `out` is a device pointer filled on the run's stream. */
+phs_status phs_get_completion_times(const phs_sim *sim, int32_t instance, double *out, int64_t n, int32_t out_is_device);
+phs_status phs_get_bottlenecks(const phs_sim *sim, int32_t instance, int32_t *out, int64_t n, int32_t out_is_device);
+/* All instances at once, concatenated in instance order: out[total_flows]. */
+phs_status phs_get_all_completion_times(const phs_sim *sim, double *out, int64_t n, int32_t out_is_device);
+phs_status phs_get_all_bottlenecks(const phs_sim *sim, int32_t *out, int64_t n, int32_t out_is_device);
+/* Per-collective finish time = max completion time over its flows (computed on the GPU). */
+phs_status phs_get_collective_times(const phs_sim *sim, int32_t instance, double *out, int32_t n);
+phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *out, int64_t cap, int64_t *n_events);
+/* Routing / decomposition artefacts (host side), for integer parity: paths as CSR off[F+1], links[cap];
+ * preds as CSR. */
+phs_status phs_num_path_entries(const phs_sim *sim, int32_t instance, int64_t *out);
+phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *links, int64_t cap);
+phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *preds, int64_t cap,
+                         int64_t *n_entries);
+phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,
+                              double *latency_s, int64_t n);
+phs_status phs_get_counters(const phs_sim *sim, phs_counters *out);
+/* Name of the kernel path the last run used for `instance`: "cta" or "cluster". */
+const char *phs_instance_path(const phs_sim *sim, int32_t instance);
+const char *phs_last_error(void); /* thread-local; valid until the next call on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,663 @@
+// phs_api.cu -- the C-ABI of libphs (include/phs.h): handle, host-side submission calls, device table
+// construction (phs_finalize), the batch scheduler that maps instances to kernels (phs_run)
+// and the result getters (a10).  No CPU fallback exists: without a usable CUDA device phs_finalize / phs_run fail.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "phs_device.h"
+
+using namespace phs;
+
+namespace {
+
+thread_local std::string g_err;
+
+phs_status fail(phs_status code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+
+#define PHS_CUDA(call)                                                                                   \
+  do {                                                                                                   \
+    cudaError_t e_ = (call);                                                                             \
+    if (e_ != cudaSuccess) return fail(PHS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+template <typename T>
+struct DevBuf {
+  T *p = nullptr;
+  size_t n = 0;
+  ~DevBuf() { release(); }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    n = 0;
+  }
+  cudaError_t alloc(size_t count) {
+    release();
+    n = count;
+    return cudaMalloc((void **)&p, std::max<size_t>(count, 1) * sizeof(T));
+  }
+  cudaError_t upload(const std::vector<T> &h, cudaStream_t st) {
+    cudaError_t e = alloc(h.size());
+    if (e != cudaSuccess || h.empty()) return e;
+    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+  }
+};
+
+}  // namespace
+
+struct phs_sim {
+  phs_topology_desc desc;
+  uint64_t seed;
+  int32_t batch;
+  std::unique_ptr<Fabric> fab;
+  std::vector<Instance> inst;
+  bool want_log = false, finalized = false, ran = false;
+  int32_t policy_path = 0, policy_slots = 0;
+
+  // ---- host mirrors built by finalize
+  std::vector<int64_t> flow_base;  // [B+1]
+  std::vector<int64_t> coll_base;  // [B+1]
+  std::vector<int64_t> log_base;   // [B+1] (only with the event log)
+  std::vector<InstDesc> h_desc;
+  std::vector<InstResult> h_res;
+  std::vector<int32_t> order;  // CTA-path instances, largest first
+  std::vector<int32_t> cluster_list;  // instances that go (or fell back) to the cluster path
+  int64_t total_flows = 0, total_colls = 0;
+
+  // ---- device tables
+  DevBuf<InstDesc> d_desc;
+  DevBuf<FlowRec> d_rec;
+  DevBuf<int32_t> d_path, d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n;
+  DevBuf<int64_t> d_capq, d_coll_first;
+  DevBuf<double> d_tdone, d_coll_t;
+  DevBuf<InstResult> d_res;
+  DevBuf<phs_event> d_log;
+  DevBuf<int> d_ticket;
+  // cluster-path scratch: one region per concurrently running cluster
+  DevBuf<int64_t> g_i64;
+  DevBuf<int32_t> g_i32, d_clist;
+  DevBuf<double> g_f64;
+  DevBuf<uint8_t> g_u8;
+  DevBuf<unsigned long long> g_ctrl;
+  DevBuf<int> d_cticket;
+  int64_t scratch_Fs = 0;
+  int scratch_regions = 0;
+  bool clist_dirty = true;
+
+  // launch configuration of the CTA path
+  int cta_threads = 0, cta_acap = 0, cta_pcap = 0, cta_grid = 0;
+  size_t cta_smem = 0;
+  int sm_count = 0;
+  cudaStream_t last_stream = nullptr;
+};
+
+extern "C" {
+
+const char *phs_last_error(void) { return g_err.c_str(); }
+
+phs_status phs_create_topology(const phs_topology_desc *desc, uint64_t seed, int32_t batch, phs_sim **out) {
+  if (!desc || !out) return fail(PHS_EINVAL, "null argument");
+  if (batch <= 0) return fail(PHS_EINVAL, "batch must be positive");
+  std::string why;
+  phs_status st = Fabric::validate(*desc, &why);
+  if (st != PHS_OK) return fail(st, why);
+  phs_sim *s = new (std::nothrow) phs_sim();
+  if (!s) return fail(PHS_ENOMEM, "out of host memory");
+  s->desc = *desc;
+  s->seed = seed;
+  s->batch = batch;
+  s->fab.reset(new Fabric(*desc));
+  s->inst.resize((size_t)batch);
+  for (int32_t i = 0; i < batch; ++i) s->inst[i].seed = seed + (uint64_t)i;
+  *out = s;
+  return PHS_OK;
+}
+
+void phs_destroy(phs_sim *sim) { delete sim; }
+
+phs_status phs_num_links(const phs_sim *sim, int32_t *out) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  *out = sim->fab->n_links();
+  return PHS_OK;
+}
+
+phs_status phs_batch(const phs_sim *sim, int32_t *out) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  *out = sim->batch;
+  return PHS_OK;
+}
+
+static phs_status check_instance(const phs_sim *sim, int32_t instance, bool allow_all) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (instance == -1 && allow_all) return PHS_OK;
+  if (instance < 0 || instance >= sim->batch) return fail(PHS_EINVAL, "instance out of range");
+  return PHS_OK;
+}
+
+phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double *cap) {
+  phs_status st = check_instance(sim, instance, true);
+  if (st != PHS_OK) return st;
+  if (!cap) return fail(PHS_EINVAL, "null capacities");
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  const int L = sim->fab->n_links();
+  for (int l = 0; l < L; ++l)
+    if (!(cap[l] > 0.0) || !(cap[l] < 0x1p42)) return fail(PHS_EINVAL, "capacity must be in (0, 2^42) byte/s");
+  const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
+  for (int i = lo; i < hi; ++i) sim->inst[i].cap.assign(cap, cap + L);
+  return PHS_OK;
+}
+
+phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double *cap) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!cap) return fail(PHS_EINVAL, "null output");
+  const int L = sim->fab->n_links();
+  const Instance &in = sim->inst[instance];
+  for (int l = 0; l < L; ++l) cap[l] = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
+  return PHS_OK;
+}
+
+phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                              double bytes, double start, const int32_t *after, int32_t n_after, int32_t *out_id) {
+  phs_status st = check_instance(sim, instance, true);
+  if (st != PHS_OK) return st;
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
+  if (instance < 0)
+    for (int i = 1; i < sim->batch; ++i)
+      if (sim->inst[i].colls.size() != sim->inst[0].colls.size())
+        return fail(PHS_ESTATE, "instance -1 needs the same number of collectives in every instance");
+  std::string why;
+  for (int i = lo; i < hi; ++i) {
+    st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes, start, after, n_after, &why);
+    if (st != PHS_OK) return fail(st, why);  // validation fails on the first instance, before any mutation
+  }
+  if (out_id) *out_id = (int32_t)sim->inst[lo].colls.size() - 1;
+  return PHS_OK;
+}
+
+phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                    const double *bytes, const double *start, const int32_t *after, int32_t n_after,
+                                    int32_t *out_id) {
+  if (!sim || !bytes) return fail(PHS_EINVAL, "null argument");
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  for (int i = 1; i < sim->batch; ++i)
+    if (sim->inst[i].colls.size() != sim->inst[0].colls.size())
+      return fail(PHS_ESTATE, "batch add needs the same number of collectives in every instance");
+  for (int i = 0; i < sim->batch; ++i) {  // validate all sizes first so that a failure leaves nothing half-added
+    if (!(bytes[i] > 0.0) || !std::isfinite(bytes[i])) return fail(PHS_EINVAL, "bytes must be positive and finite");
+    if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return fail(PHS_EINVAL, "bad start_time_s");
+  }
+  std::string why;
+  for (int i = 0; i < sim->batch; ++i) {
+    phs_status st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
+                                      after, n_after, &why);
+    if (st != PHS_OK) return fail(st, why);
+  }
+  if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;
+  return PHS_OK;
+}
+
+phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_t *src, const int32_t *dst,
+                         const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                         const int32_t *conn_id, int64_t *out_first) {
+  phs_status st = check_instance(sim, instance, true);
+  if (st != PHS_OK) return st;
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
+  if (instance < 0)
+    for (int i = 1; i < sim->batch; ++i)
+      if (sim->inst[i].n_flows() != sim->inst[0].n_flows())
+        return fail(PHS_ESTATE, "instance -1 needs the same number of flows in every instance");
+  const int64_t first = sim->inst[lo].n_flows();
+  std::string why;
+  for (int i = lo; i < hi; ++i) {
+    st = append_flows(*sim->fab, sim->inst[i], n, src, dst, bytes, start, dep_off, dep_ids, conn_id, &why);
+    if (st != PHS_OK) return fail(st, why);
+  }
+  if (out_first) *out_first = first;
+  return PHS_OK;
+}
+
+phs_status phs_enable_event_log(phs_sim *sim, int32_t enable) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (sim->finalized) return fail(PHS_ESTATE, "event log must be chosen before phs_finalize");
+  sim->want_log = enable != 0;
+  return PHS_OK;
+}
+
+phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (path < 0 || path > 2 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
+  if (sim->finalized) return fail(PHS_ESTATE, "scheduler policy must be chosen before phs_finalize");
+  sim->policy_path = path;
+  sim->policy_slots = cta_slots;
+  return PHS_OK;
+}
+
+phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!out) return fail(PHS_EINVAL, "null output");
+  *out = sim->inst[instance].n_flows();
+  return PHS_OK;
+}
+
+phs_status phs_total_flows(const phs_sim *sim, int64_t *out) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  int64_t t = 0;
+  for (const Instance &in : sim->inst) t += in.n_flows();
+  *out = t;
+  return PHS_OK;
+}
+
+phs_status phs_num_collectives(const phs_sim *sim, int32_t instance, int32_t *out) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!out) return fail(PHS_EINVAL, "null output");
+  *out = (int32_t)sim->inst[instance].colls.size();
+  return PHS_OK;
+}
+
+phs_status phs_num_path_entries(const phs_sim *sim, int32_t instance, int64_t *out) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!out) return fail(PHS_EINVAL, "null output");
+  *out = (int64_t)sim->inst[instance].path.size();
+  return PHS_OK;
+}
+
+phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *links, int64_t cap) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  const Instance &in = sim->inst[instance];
+  if (!off || !links || cap < (int64_t)in.path.size()) return fail(PHS_EINVAL, "output too small");
+  for (size_t f = 0; f < in.path_off.size(); ++f) off[f] = in.path_off[f];
+  std::copy(in.path.begin(), in.path.end(), links);
+  return PHS_OK;
+}
+
+phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *preds, int64_t cap,
+                         int64_t *n_entries) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  const Instance &in = sim->inst[instance];
+  if (!n_entries) return fail(PHS_EINVAL, "null n_entries");
+  *n_entries = (int64_t)in.pred.size();
+  if (off)
+    for (size_t f = 0; f < in.pred_off.size(); ++f) off[f] = in.pred_off[f];
+  if (preds) {
+    if (cap < (int64_t)in.pred.size()) return fail(PHS_EINVAL, "output too small");
+    std::copy(in.pred.begin(), in.pred.end(), preds);
+  }
+  return PHS_OK;
+}
+
+phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,
+                              double *lat, int64_t n) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  const Instance &in = sim->inst[instance];
+  if (n != in.n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
+  if (src) std::copy(in.src.begin(), in.src.end(), src);
+  if (dst) std::copy(in.dst.begin(), in.dst.end(), dst);
+  if (bytes) std::copy(in.bytes.begin(), in.bytes.end(), bytes);
+  if (lat) std::copy(in.lat.begin(), in.lat.end(), lat);
+  return PHS_OK;
+}
+
+}  // extern "C"
+
+// ================================================================================================ finalize
+// Builds the device-resident tables.  HBM layout: one 32-byte FlowRec per flow (+1
+// sentinel per instance), flow->link CSR values, successor CSR values (transpose of the dependency lists),
+// per-instance capacity rows in rate quanta, and the dynamic per-flow arrays (pred_cnt, t_done, bneck).
+extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (sim->finalized) return PHS_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  PHS_CUDA(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  PHS_CUDA(cudaGetDeviceProperties(&prop, dev));
+  sim->sm_count = prop.multiProcessorCount;
+  const int B = sim->batch, L = sim->fab->n_links();
+
+  sim->flow_base.assign(B + 1, 0);
+  sim->coll_base.assign(B + 1, 0);
+  sim->log_base.assign(B + 1, 0);
+  std::vector<int64_t> path_base(B + 1, 0), succ_base(B + 1, 0);
+  for (int i = 0; i < B; ++i) {
+    const Instance &in = sim->inst[i];
+    sim->flow_base[i + 1] = sim->flow_base[i] + in.n_flows();
+    sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)in.colls.size();
+    sim->log_base[i + 1] = sim->log_base[i] + 2 * in.n_flows() + 2;
+    path_base[i + 1] = path_base[i] + (int64_t)in.path.size();
+    succ_base[i + 1] = succ_base[i] + (int64_t)in.pred.size();
+  }
+  sim->total_flows = sim->flow_base[B];
+  sim->total_colls = sim->coll_base[B];
+  const int64_t Ft = sim->total_flows;
+
+  std::vector<FlowRec> rec((size_t)(Ft + B));
+  std::vector<int32_t> path((size_t)path_base[B]), succ((size_t)succ_base[B]), pc0((size_t)Ft);
+  std::vector<int64_t> capq((size_t)B * L), coll_first((size_t)sim->total_colls);
+  std::vector<int32_t> coll_n((size_t)sim->total_colls);
+  sim->h_desc.resize(B);
+  for (int i = 0; i < B; ++i) {
+    const Instance &in = sim->inst[i];
+    const int64_t F = in.n_flows();
+    // capacities -> rate quanta (floor); every fair share must stay >= 1 quantum
+    for (int l = 0; l < L; ++l) {
+      const double c = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
+      const int64_t q = (int64_t)std::floor(c * 1048576.0);
+      if (q < F + 1) return fail(PHS_ERANGE, "a link capacity is below (#flows + 1) rate quanta of 2^-20 byte/s");
+      capq[(size_t)i * L + l] = q;
+    }
+    // successor CSR = transpose of the pred lists (counting sort by predecessor)
+    std::vector<uint32_t> soff((size_t)F + 1, 0);
+    for (int32_t p : in.pred) soff[(size_t)p + 1]++;
+    for (int64_t f = 0; f < F; ++f) soff[f + 1] += soff[f];
+    {
+      std::vector<uint32_t> cur(soff.begin(), soff.end() - 1);
+      int32_t *sdst = succ.data() + succ_base[i];
+      for (int64_t f = 0; f < F; ++f)
+        for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
+    }
+    FlowRec *r = rec.data() + sim->flow_base[i] + i;
+    for (int64_t f = 0; f <= F; ++f) {
+      FlowRec x;
+      x.bytes = f < F ? in.bytes[f] : 0.0;
+      x.start = f < F ? in.start[f] : 0.0;
+      x.lat = f < F ? in.lat[f] : 0.0;
+      x.path_off = in.path_off[f];
+      x.succ_off = soff[f];
+      r[f] = x;
+    }
+    std::copy(in.path.begin(), in.path.end(), path.begin() + path_base[i]);
+    for (int64_t f = 0; f < F; ++f) pc0[sim->flow_base[i] + f] = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
+    for (size_t c = 0; c < in.colls.size(); ++c) {
+      coll_first[sim->coll_base[i] + c] = sim->flow_base[i] + in.colls[c].first_flow;
+      coll_n[sim->coll_base[i] + c] = in.colls[c].n_flows;
+    }
+    InstDesc d;
+    d.rec_base = sim->flow_base[i] + i;
+    d.flow_base = sim->flow_base[i];
+    d.path_base = path_base[i];
+    d.succ_base = succ_base[i];
+    d.log_base = sim->want_log ? sim->log_base[i] : -1;
+    d.coll_base = sim->coll_base[i];
+    d.n_flows = (int32_t)F;
+    d.n_colls = (int32_t)in.colls.size();
+    sim->h_desc[i] = d;
+  }
+
+  PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
+  PHS_CUDA(sim->d_rec.upload(rec, st));
+  PHS_CUDA(sim->d_path.upload(path, st));
+  PHS_CUDA(sim->d_succ.upload(succ, st));
+  PHS_CUDA(sim->d_pc0.upload(pc0, st));
+  PHS_CUDA(sim->d_capq.upload(capq, st));
+  PHS_CUDA(sim->d_coll_first.upload(coll_first, st));
+  PHS_CUDA(sim->d_coll_n.upload(coll_n, st));
+  PHS_CUDA(sim->d_pred_cnt.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_tdone.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_bneck.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_coll_t.alloc((size_t)sim->total_colls));
+  PHS_CUDA(sim->d_res.alloc((size_t)B));
+  PHS_CUDA(sim->d_ticket.alloc(1));
+  if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)sim->log_base[B]));
+  sim->h_res.assign(B, InstResult{});
+
+  // ---- a9: batch scheduler, static part.  Small instances -> one CTA each with shared-memory state, sized so
+  // that enough CTAs are resident per SM to cover the batch; instances whose link state alone does not fit go to
+  // the cluster path.  Instances that overflow their shared-memory slots at run time are re-run on the cluster path.
+  const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin;
+  int threads = L <= 320 ? 128 : 256;
+  int64_t maxF = 0;
+  for (int i = 0; i < B; ++i) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
+  const int want_ctas = std::max(1, std::min(2048 / threads / 2, (B + sim->sm_count - 1) / sim->sm_count));
+  const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
+  const size_t budget = std::min(smem_max, per_sm / want_ctas - 1024);
+  const size_t link_bytes = cta_smem_bytes(L, 0, 0);
+  sim->order.clear();
+  sim->cluster_list.clear();
+  int cap_slots = 0;
+  if (sim->policy_path != 2 && link_bytes + cta_smem_bytes(0, 64, 64) <= budget) {
+    int lo = 64, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 64), 1 << 20);
+    if (sim->policy_slots > 0) hi = std::max(64, std::min(hi, (int)sim->policy_slots));
+    hi = (hi + 31) / 32 * 32;
+    while (lo < hi) {  // largest multiple of 32 that fits the budget
+      const int mid = ((lo + hi + 32) / 64) * 32;
+      if (cta_smem_bytes(L, mid, mid) <= budget)
+        lo = mid;
+      else
+        hi = mid - 32;
+    }
+    cap_slots = lo;
+  }
+  if (cap_slots > 0) {
+    sim->cta_threads = threads;
+    sim->cta_acap = sim->cta_pcap = cap_slots;
+    sim->cta_smem = cta_smem_bytes(L, cap_slots, cap_slots);
+    for (int i = 0; i < B; ++i) sim->order.push_back(i);
+    std::stable_sort(sim->order.begin(), sim->order.end(),
+                     [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
+    const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta_smem + 1024)), 2048 / threads));
+    sim->cta_grid = std::min(B, per * sim->sm_count);
+    PHS_CUDA(sim->d_order.upload(sim->order, st));
+  } else {
+    for (int i = 0; i < B; ++i) sim->cluster_list.push_back(i);
+  }
+  PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
+  sim->finalized = true;
+  return PHS_OK;
+}
+
+// ================================================================================================ run
+namespace {
+
+DevTables tables_of(phs_sim *sim) {
+  DevTables t;
+  t.inst = sim->d_desc.p;
+  t.rec = sim->d_rec.p;
+  t.path = sim->d_path.p;
+  t.succ = sim->d_succ.p;
+  t.pred_cnt0 = sim->d_pc0.p;
+  t.capq = sim->d_capq.p;
+  t.pred_cnt = sim->d_pred_cnt.p;
+  t.t_done = sim->d_tdone.p;
+  t.bneck = sim->d_bneck.p;
+  t.res = sim->d_res.p;
+  t.log = sim->want_log ? sim->d_log.p : nullptr;
+  t.n_links = sim->fab->n_links();
+  return t;
+}
+
+// Cluster path (a9): every instance in `list` is simulated by one thread-block cluster; clusters pull instances
+// from the list until it is empty.
+phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, cudaStream_t st) {
+  if (list.empty()) return PHS_OK;
+  const int L = sim->fab->n_links();
+  int64_t maxF = 1;
+  for (int i : list) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
+  int want = 1;
+  while (want < 16 && (int64_t)want * kClusterThreads * 4 < maxF) want *= 2;  // ~4 flows per thread
+  int cs = 1, max_clusters = 1;
+  PHS_CUDA(cluster_path_limits(want, &cs, &max_clusters));
+  const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
+  if (maxF > sim->scratch_Fs || n_clusters > sim->scratch_regions) {
+    const int64_t Fs = std::max(maxF, sim->scratch_Fs);
+    const int R = std::max(n_clusters, sim->scratch_regions);
+    PHS_CUDA(sim->g_i64.alloc(cluster_i64_per_region(L, Fs) * R));
+    PHS_CUDA(sim->g_i32.alloc(cluster_i32_per_region(L, Fs) * R));
+    PHS_CUDA(sim->g_f64.alloc(cluster_f64_per_region(Fs) * R));
+    PHS_CUDA(sim->g_u8.alloc((size_t)L * R));
+    PHS_CUDA(sim->g_ctrl.alloc((size_t)64 * R));
+    PHS_CUDA(sim->d_cticket.alloc(1));
+    sim->scratch_Fs = Fs;
+    sim->scratch_regions = R;
+  }
+  std::vector<int32_t> sorted(list);
+  std::stable_sort(sorted.begin(), sorted.end(),
+                   [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
+  PHS_CUDA(sim->d_clist.upload(sorted, st));
+  PHS_CUDA(cudaMemsetAsync(sim->d_cticket.p, 0, sizeof(int), st));
+  PHS_CUDA(cudaMemsetAsync(sim->g_ctrl.p, 0, sizeof(unsigned long long) * 64 * sim->scratch_regions, st));
+  ClusterScratch sc;
+  sc.i64 = sim->g_i64.p;
+  sc.i32 = sim->g_i32.p;
+  sc.f64 = sim->g_f64.p;
+  sc.u8 = sim->g_u8.p;
+  sc.ctrl = sim->g_ctrl.p;
+  sc.Fs = sim->scratch_Fs;
+  PHS_CUDA(launch_cluster_path(tables_of(sim), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
+                               n_clusters, sim->want_log, st));
+  return PHS_OK;
+}
+
+}  // namespace
+
+extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (!sim->finalized) {
+    phs_status fs = phs_finalize(sim, cuda_stream);
+    if (fs != PHS_OK) return fs;
+  }
+  sim->last_stream = st;
+  const int B = sim->batch;
+  DevTables t = tables_of(sim);
+  if (!sim->order.empty()) {
+    PHS_CUDA(cudaMemsetAsync(sim->d_ticket.p, 0, sizeof(int), st));
+    PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta_threads,
+                             sim->cta_acap, sim->cta_pcap, sim->cta_grid, sim->cta_smem, sim->want_log, st));
+  }
+  {
+    phs_status gs = run_cluster_path(sim, sim->cluster_list, st);
+    if (gs != PHS_OK) return gs;
+  }
+  PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
+  PHS_CUDA(cudaStreamSynchronize(st));
+  // instances that ran out of shared-memory slots: re-run on the cluster path (and remember for later runs)
+  std::vector<int32_t> redo;
+  for (int i = 0; i < B; ++i)
+    if (sim->h_res[i].status == kOverflow) redo.push_back(i);
+  if (!redo.empty()) {
+    phs_status gs = run_cluster_path(sim, redo, st);
+    if (gs != PHS_OK) return gs;
+    for (int inst : redo) {
+      sim->cluster_list.push_back(inst);
+      sim->order.erase(std::find(sim->order.begin(), sim->order.end(), inst));
+    }
+    if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
+    sim->cta_grid = std::min<int>(sim->cta_grid, std::max<int>(1, (int)sim->order.size()));
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+  }
+  PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
+                                   sim->d_coll_t.p, st));
+  sim->ran = true;
+  for (int i = 0; i < B; ++i) {
+    if (sim->h_res[i].status == PHS_ECYCLE)
+      return fail(PHS_ECYCLE, "instance " + std::to_string(i) + ": flows left waiting on dependencies that never complete");
+    if (sim->h_res[i].status != PHS_OK)
+      return fail(PHS_ECUDA, "instance " + std::to_string(i) + ": unexpected kernel status " +
+                                 std::to_string(sim->h_res[i].status));
+  }
+  return PHS_OK;
+}
+
+// ================================================================================================ results (a10)
+namespace {
+template <typename T>
+phs_status fetch(const phs_sim *sim, const T *dev, int64_t first, int64_t count, T *out, int32_t out_is_device) {
+  if (count == 0) return PHS_OK;
+  PHS_CUDA(cudaMemcpyAsync(out, dev + first, sizeof(T) * (size_t)count,
+                           out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, sim->last_stream));
+  if (!out_is_device) PHS_CUDA(cudaStreamSynchronize(sim->last_stream));
+  return PHS_OK;
+}
+}  // namespace
+
+extern "C" {
+
+phs_status phs_get_completion_times(const phs_sim *sim, int32_t instance, double *out, int64_t n, int32_t dev) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (!out || n != sim->inst[instance].n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
+  return fetch(sim, sim->d_tdone.p, sim->flow_base[instance], n, out, dev);
+}
+
+phs_status phs_get_bottlenecks(const phs_sim *sim, int32_t instance, int32_t *out, int64_t n, int32_t dev) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (!out || n != sim->inst[instance].n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
+  return fetch(sim, sim->d_bneck.p, sim->flow_base[instance], n, out, dev);
+}
+
+phs_status phs_get_all_completion_times(const phs_sim *sim, double *out, int64_t n, int32_t dev) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
+  return fetch(sim, sim->d_tdone.p, 0, n, out, dev);
+}
+
+phs_status phs_get_all_bottlenecks(const phs_sim *sim, int32_t *out, int64_t n, int32_t dev) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
+  return fetch(sim, sim->d_bneck.p, 0, n, out, dev);
+}
+
+phs_status phs_get_collective_times(const phs_sim *sim, int32_t instance, double *out, int32_t n) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (!out || n != (int32_t)sim->inst[instance].colls.size()) return fail(PHS_EINVAL, "n must equal the collective count");
+  return fetch(sim, sim->d_coll_t.p, sim->coll_base[instance], (int64_t)n, out, 0);
+}
+
+phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *out, int64_t cap, int64_t *n_events) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (!sim->want_log) return fail(PHS_ESTATE, "event log was not enabled");
+  if (!n_events) return fail(PHS_EINVAL, "null n_events");
+  *n_events = sim->h_res[instance].n_events;
+  if (!out) return PHS_OK;
+  return fetch(sim, sim->d_log.p, sim->log_base[instance], std::min<int64_t>(cap, *n_events), out, 0);
+}
+
+phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
+  if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  phs_counters c{};
+  for (int i = 0; i < sim->batch; ++i) {
+    c.n_events += sim->h_res[i].n_events;
+    c.sum_active += sim->h_res[i].sum_active;
+    c.sum_par_rounds += sim->h_res[i].sum_par_rounds;
+  }
+  c.n_flow_events = 2 * sim->total_flows;
+  *out = c;
+  return PHS_OK;
+}
+
+const char *phs_instance_path(const phs_sim *sim, int32_t instance) {
+  if (!sim || instance < 0 || instance >= sim->batch || !sim->ran) return "";
+  return sim->h_res[instance].path == 0 ? "cta" : "cluster";
+}
+
+}  // extern "C"

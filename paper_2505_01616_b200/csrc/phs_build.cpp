@@ -1,0 +1,288 @@
+// phs_build.cpp -- host builder: link numbering, seeded ECMP routing (flow -> link CSR incidence) and the
+// collective -> flow decomposer with its dependency DAG.  Pure host C++, no CUDA.  DESIGN.md S1-S3; the
+// passages of the paper are PAPER.md L98 (topology, multipath routing) and L104 (ring all-reduce, flows with
+// timestamps).
+#include <cmath>
+#include <limits>
+
+#include "phs_internal.h"
+
+namespace phs {
+
+// ------------------------------------------------------------------------------------------------ Fabric (S1)
+// Directed link ids, in blocks:
+//   [0, 2G)            NVLink : 2g GPU->NVSwitch, 2g+1 NVSwitch->GPU
+//   [2G, 4G)           NIC    : 2G+2g GPU->tier-1 switch, 2G+2g+1 back
+//   [tier1_base, ...)  tier1<->tier2 pairs u: up tier1_base+2u, down tier1_base+2u+1
+//   [tier2_base, ...)  fat tree tier2<->tier3 pairs
+phs_status Fabric::validate(const phs_topology_desc &d, std::string *why) {
+  auto bad = [&](const char *m) {
+    if (why) *why = m;
+    return PHS_EINVAL;
+  };
+  auto cap_ok = [](double c) { return c > 0.0 && c < 0x1p42; };
+  if (d.n_hosts <= 0 || d.gpus_per_host <= 0) return bad("n_hosts and gpus_per_host must be positive");
+  if (!cap_ok(d.nvlink_Bps) || !cap_ok(d.nic_Bps)) return bad("nvlink_Bps / nic_Bps must be in (0, 2^42)");
+  if (!(d.hop_latency_s >= 0.0) || !std::isfinite(d.hop_latency_s)) return bad("hop_latency_s must be >= 0");
+  int64_t links = 4LL * d.n_hosts * d.gpus_per_host;
+  switch (d.kind) {
+    case PHS_TOPO_SINGLE:
+      break;
+    case PHS_TOPO_LEAF_SPINE:
+      if (d.n_leaves <= 0 || d.n_spines <= 0 || d.uplinks_per_leaf_spine <= 0)
+        return bad("leaf-spine needs n_leaves, n_spines, uplinks_per_leaf_spine > 0");
+      if (d.n_hosts % d.n_leaves) return bad("n_hosts must be a multiple of n_leaves");
+      if (!cap_ok(d.fabric_Bps)) return bad("fabric_Bps must be in (0, 2^42)");
+      links += 2LL * d.n_leaves * d.n_spines * d.uplinks_per_leaf_spine;
+      break;
+    case PHS_TOPO_FAT_TREE:
+      if (d.k < 2 || (d.k & 1) || d.agg_uplinks <= 0) return bad("fat tree needs even k >= 2 and agg_uplinks > 0");
+      if (d.gpus_per_host != d.k / 2 || d.n_hosts != d.k * (d.k / 2))
+        return bad("fat tree needs gpus_per_host = k/2 and n_hosts = k*k/2");
+      if (!cap_ok(d.fabric_Bps)) return bad("fabric_Bps must be in (0, 2^42)");
+      links += 2LL * d.k * (d.k / 2) * (d.k / 2) + 2LL * d.k * (d.k / 2) * d.agg_uplinks;
+      break;
+    default:
+      return bad("unknown topology kind");
+  }
+  if (links > 0x3fffffff) {
+    if (why) *why = "too many links";
+    return PHS_ERANGE;
+  }
+  return PHS_OK;
+}
+
+Fabric::Fabric(const phs_topology_desc &d) : d_(d) {
+  gpus_ = d.n_hosts * d.gpus_per_host;
+  tier1_base_ = 4 * gpus_;
+  tier2_base_ = tier1_base_;
+  links_ = tier1_base_;
+  if (d.kind == PHS_TOPO_LEAF_SPINE) {
+    links_ += 2 * d.n_leaves * d.n_spines * d.uplinks_per_leaf_spine;
+  } else if (d.kind == PHS_TOPO_FAT_TREE) {
+    const int half = d.k / 2;
+    tier2_base_ = tier1_base_ + 2 * d.k * half * half;
+    links_ = tier2_base_ + 2 * d.k * half * d.agg_uplinks;
+  }
+}
+
+double Fabric::default_capacity(int32_t link) const {
+  if (link < 2 * gpus_) return d_.nvlink_Bps;
+  if (link < 4 * gpus_) return d_.nic_Bps;
+  return d_.fabric_Bps;
+}
+
+// SplitMix64 step: add the golden-gamma constant, then the xor-shift-multiply finaliser.
+uint64_t splitmix64_step(uint64_t x) {
+  x += 0x9E3779B97F4A7C15ULL;
+  x ^= x >> 30;
+  x *= 0xBF58476D1CE4E5B9ULL;
+  x ^= x >> 27;
+  x *= 0x94D049BB133111EBULL;
+  x ^= x >> 31;
+  return x;
+}
+
+// ------------------------------------------------------------------------------------------------ ECMP (S2)
+int Fabric::route(uint64_t seed, int32_t src, int32_t dst, int32_t conn, int32_t *out) const {
+  const int gph = d_.gpus_per_host;
+  const int host_s = src / gph, host_d = dst / gph;
+  if (host_s == host_d) {  // stays on the host's NVSwitch
+    out[0] = 2 * src;
+    out[1] = 2 * dst + 1;
+    return 2;
+  }
+  const int32_t first = 2 * gpus_ + 2 * src, last = 2 * gpus_ + 2 * dst + 1;
+  int n = 0;
+  out[n++] = first;
+  if (d_.kind != PHS_TOPO_SINGLE) {
+    uint64_t h = splitmix64_step(seed);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)src);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)dst);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)conn);
+    const uint32_t hi_word = (uint32_t)(h >> 32);
+    if (d_.kind == PHS_TOPO_LEAF_SPINE) {
+      const int hosts_per_leaf = d_.n_hosts / d_.n_leaves;
+      const int leaf_s = host_s / hosts_per_leaf, leaf_d = host_d / hosts_per_leaf;
+      if (leaf_s != leaf_d) {
+        const int P = d_.uplinks_per_leaf_spine;
+        const int choice = (int)(h % (uint64_t)(d_.n_spines * P));
+        const int spine = choice / P, lane_up = choice % P, lane_dn = (int)((uint64_t)hi_word % (uint64_t)P);
+        out[n++] = tier1_base_ + 2 * ((leaf_s * d_.n_spines + spine) * P + lane_up);
+        out[n++] = tier1_base_ + 2 * ((leaf_d * d_.n_spines + spine) * P + lane_dn) + 1;
+      }
+    } else {  // fat tree: a host hangs off its own edge switch
+      const int half = d_.k / 2;
+      const int pod_s = host_s / half, edge_s = host_s % half, pod_d = host_d / half, edge_d = host_d % half;
+      const int agg = (int)(h % (uint64_t)half);
+      const int up1 = tier1_base_ + 2 * ((pod_s * half + edge_s) * half + agg);
+      const int dn1 = tier1_base_ + 2 * ((pod_d * half + edge_d) * half + agg) + 1;
+      out[n++] = up1;
+      if (pod_s != pod_d) {
+        const int U = d_.agg_uplinks;
+        const int core_lane = (int)((uint64_t)hi_word % (uint64_t)U);
+        out[n++] = tier2_base_ + 2 * ((pod_s * half + agg) * U + core_lane);
+        out[n++] = tier2_base_ + 2 * ((pod_d * half + agg) * U + core_lane) + 1;
+      }
+      out[n++] = dn1;
+    }
+  }
+  out[n++] = last;
+  return n;
+}
+
+// ------------------------------------------------------------------------------------------------ flows
+namespace {
+
+// Adds one flow (without dependencies) and returns its id.
+int32_t push_flow(const Fabric &fab, Instance &inst, int32_t src, int32_t dst, double bytes, double start,
+                  int32_t conn) {
+  int32_t hops[kMaxHops];
+  const int n = fab.route(inst.seed, src, dst, conn, hops);
+  double lat = 0.0;
+  for (int i = 0; i < n; ++i) {
+    inst.path.push_back(hops[i]);
+    lat = lat + fab.latency(hops[i]);
+  }
+  inst.src.push_back(src);
+  inst.dst.push_back(dst);
+  inst.bytes.push_back(bytes);
+  inst.start.push_back(start);
+  inst.lat.push_back(lat);
+  inst.path_off.push_back((uint32_t)inst.path.size());
+  inst.pred_off.push_back((uint32_t)inst.pred.size());
+  return (int32_t)inst.src.size() - 1;
+}
+
+// A dependency of the flow pushed last.
+inline void push_dep(Instance &inst, int32_t on) {
+  inst.pred.push_back(on);
+  inst.pred_off.back() = (uint32_t)inst.pred.size();
+}
+
+// Flows of collective `a` that must finish before rank `rho` may start a later collective: what rho sent and
+// what rho received in a's last step (ring), or everything from / to rho (all-to-all).
+void chain_after(Instance &inst, const Collective &a, int32_t rho) {
+  int pos = -1;
+  for (int i = 0; i < a.n_ranks; ++i)
+    if (a.ranks[i] == rho) {
+      pos = i;
+      break;
+    }
+  if (pos < 0) return;  // rho did not take part: no edge
+  if (a.kind == PHS_ALLTOALL) {
+    const int N = a.n_ranks;
+    for (int other = 0; other < N; ++other) {
+      if (other == pos) continue;
+      push_dep(inst, a.first_flow + pos * (N - 1) + (other > pos ? other - 1 : other));  // pos -> other
+      push_dep(inst, a.first_flow + other * (N - 1) + (pos > other ? pos - 1 : pos));    // other -> pos
+    }
+  } else {
+    const int32_t last_step = a.first_flow + (a.steps - 1) * a.n_ranks;
+    push_dep(inst, last_step + pos);                                  // sent by rho
+    push_dep(inst, last_step + (pos == 0 ? a.n_ranks - 1 : pos - 1));  // received by rho
+  }
+}
+
+}  // namespace
+
+phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t N,
+                             double bytes, double start, const int32_t *after, int32_t n_after, std::string *why) {
+  auto bad = [&](const char *m) {
+    if (why) *why = m;
+    return PHS_EINVAL;
+  };
+  if (!ranks) return bad("ranks is null");
+  if (kind < PHS_ALLREDUCE_RING || kind > PHS_ALLTOALL) return bad("unknown collective kind");
+  if (N < 2) return bad("a collective needs at least 2 ranks");
+  if (!(bytes > 0.0) || !std::isfinite(bytes)) return bad("bytes must be positive and finite");
+  if (!(start >= 0.0) || !std::isfinite(start)) return bad("start_time_s must be >= 0 and finite");
+  if (n_after < 0 || (n_after > 0 && !after)) return bad("bad after_coll_ids");
+  {
+    std::vector<uint8_t> seen((size_t)fab.n_gpus(), 0);
+    for (int i = 0; i < N; ++i) {
+      if (ranks[i] < 0 || ranks[i] >= fab.n_gpus()) return bad("rank out of range");
+      if (seen[ranks[i]]) return bad("duplicate rank in collective");
+      seen[ranks[i]] = 1;
+    }
+  }
+  for (int a = 0; a < n_after; ++a)
+    if (after[a] < 0 || after[a] >= (int32_t)inst.colls.size()) return bad("after_coll_ids names an unknown collective");
+  const int steps = kind == PHS_ALLREDUCE_RING ? 2 * (N - 1) : kind == PHS_ALLTOALL ? 1 : N - 1;
+  const int64_t nf = kind == PHS_ALLTOALL ? (int64_t)N * (N - 1) : (int64_t)steps * N;
+  if (inst.n_flows() + nf > 0x7ffffff0LL) {
+    if (why) *why = "too many flows in one instance";
+    return PHS_ERANGE;
+  }
+  Collective c;
+  c.kind = kind;
+  c.n_ranks = N;
+  c.first_flow = (int32_t)inst.n_flows();
+  c.n_flows = (int32_t)nf;
+  c.steps = steps;
+  c.ranks.assign(ranks, ranks + N);
+  const int32_t conn = (int32_t)inst.colls.size();  // ECMP key: one path per (pair, collective)
+  const double chunk = bytes / (double)N;
+  if (kind == PHS_ALLTOALL) {
+    for (int i = 0; i < N; ++i)
+      for (int j = 0; j < N; ++j) {
+        if (i == j) continue;
+        push_flow(fab, inst, ranks[i], ranks[j], chunk, start, conn);
+        for (int a = 0; a < n_after; ++a) chain_after(inst, inst.colls[after[a]], ranks[i]);
+      }
+  } else {
+    // step-major: flow (s, i) sends chunk from ranks[i] to ranks[i+1]; it waits for the chunk it forwards
+    // (s-1, i-1) and for the sender's previous send (s-1, i) -- FIFO per connection.
+    for (int s = 0; s < steps; ++s) {
+      const int32_t prev = c.first_flow + (s - 1) * N;
+      for (int i = 0; i < N; ++i) {
+        const int next_rank = i + 1 == N ? 0 : i + 1;
+        push_flow(fab, inst, ranks[i], ranks[next_rank], chunk, s == 0 ? start : 0.0, conn);
+        if (s == 0) {
+          for (int a = 0; a < n_after; ++a) chain_after(inst, inst.colls[after[a]], ranks[i]);
+        } else {
+          push_dep(inst, prev + (i == 0 ? N - 1 : i - 1));
+          push_dep(inst, prev + i);
+        }
+      }
+    }
+  }
+  inst.colls.push_back(std::move(c));
+  return PHS_OK;
+}
+
+phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,
+                        const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                        const int32_t *conn_id, std::string *why) {
+  auto bad = [&](const char *m) {
+    if (why) *why = m;
+    return PHS_EINVAL;
+  };
+  if (n < 0 || (n > 0 && (!src || !dst || !bytes))) return bad("null flow arrays");
+  const int64_t first = inst.n_flows();
+  if (first + n > 0x7ffffff0LL) {
+    if (why) *why = "too many flows in one instance";
+    return PHS_ERANGE;
+  }
+  for (int64_t i = 0; i < n; ++i) {  // validate first, mutate after
+    if (src[i] < 0 || src[i] >= fab.n_gpus() || dst[i] < 0 || dst[i] >= fab.n_gpus()) return bad("rank out of range");
+    if (src[i] == dst[i]) return bad("src == dst");
+    if (!(bytes[i] > 0.0) || !std::isfinite(bytes[i])) return bad("bytes must be positive and finite");
+    if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return bad("start_time_s must be >= 0 and finite");
+    if (dep_off) {
+      if (dep_off[i + 1] < dep_off[i]) return bad("dep_off must be non-decreasing");
+      if (dep_off[i + 1] > dep_off[i] && !dep_ids) return bad("dep_flow_ids is null");
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e)
+        if (dep_ids[e] < 0 || dep_ids[e] >= first + i) return bad("a flow may only depend on earlier flows");
+    }
+  }
+  for (int64_t i = 0; i < n; ++i) {
+    const int32_t id = (int32_t)(first + i);
+    push_flow(fab, inst, src[i], dst[i], bytes[i], start ? start[i] : 0.0, conn_id ? conn_id[i] : id);
+    if (dep_off)
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) push_dep(inst, (int32_t)dep_ids[e]);
+  }
+  return PHS_OK;
+}
+
+}  // namespace phs

@@ -1,0 +1,96 @@
+// phs_internal.h -- shared between the host builder (phs_build.cpp), the API (phs_api.cu) and the kernels
+// (phs_kernels.cu).  Nothing here is shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/phs.h"
+
+namespace phs {
+
+// ---- S0: rates and capacities live on an exact fixed-point grid of 2^-20 byte/s (reading R-FX) ----
+constexpr int kRateFracBits = 20;
+constexpr int kMaxHops = 6;  // longest path: fat tree cross-pod (S2)
+
+// Device-resident flow record, 32 bytes, one per flow plus one sentinel per instance (so that the path and
+// successor list of flow f end where those of f+1 begin).  Gathered once per flow, at activation / release.
+struct FlowRec {
+  double bytes;       // flow size
+  double start;       // earliest submission time (S4)
+  double lat;         // path latency, left-to-right sum over the path's links (S2)
+  uint32_t path_off;  // into the instance's slice of path[]
+  uint32_t succ_off;  // into the instance's slice of succ[]
+};
+static_assert(sizeof(FlowRec) == 32, "FlowRec must be 32 bytes");
+
+// Per-instance descriptor (device).
+struct InstDesc {
+  int64_t rec_base;   // first FlowRec of the instance (flow_base + instance index, because of the sentinels)
+  int64_t flow_base;  // first entry in the per-flow arrays (pred_cnt, t_done, bneck, ...)
+  int64_t path_base;  // first entry of the instance's slice of path[]
+  int64_t succ_base;  // first entry of the instance's slice of succ[]
+  int64_t log_base;   // first row of the instance's event log slice (capacity 2F+2 rows), -1 if disabled
+  int64_t coll_base;  // first entry in the per-collective arrays
+  int32_t n_flows;
+  int32_t n_colls;
+};
+
+// Per-instance result block (device, read back after a run).
+struct InstResult {
+  int32_t status;          // PHS_OK, PHS_ECYCLE, or kOverflow (re-run on the cluster path)
+  int32_t path;            // 0 = cta, 1 = cluster
+  int64_t n_events;
+  int64_t sum_active;
+  int64_t sum_par_rounds;
+  int32_t max_active;
+  int32_t max_pending;
+};
+constexpr int32_t kOverflow = 1;  // internal: the CTA path ran out of shared-memory slots
+
+// ---- host-side instance tables (built by phs_build.cpp) ----
+struct Collective {
+  int32_t kind, n_ranks, first_flow, n_flows, steps;
+  std::vector<int32_t> ranks;
+};
+
+struct Instance {
+  uint64_t seed = 0;
+  std::vector<double> cap;  // empty: descriptor defaults
+  std::vector<int32_t> src, dst;
+  std::vector<double> bytes, start, lat;
+  std::vector<uint32_t> path_off{0};
+  std::vector<int32_t> path;
+  std::vector<uint32_t> pred_off{0};
+  std::vector<int32_t> pred;
+  std::vector<Collective> colls;
+  int64_t n_flows() const { return (int64_t)src.size(); }
+};
+
+// Link numbering and ECMP routing of one topology (S1, S2).
+class Fabric {
+ public:
+  explicit Fabric(const phs_topology_desc &d);
+  static phs_status validate(const phs_topology_desc &d, std::string *why);
+  int32_t n_gpus() const { return gpus_; }
+  int32_t n_links() const { return links_; }
+  double default_capacity(int32_t link) const;
+  double latency(int32_t /*link*/) const { return d_.hop_latency_s; }
+  // writes the links of (src -> dst) for connection key `conn` into out[0..kMaxHops), returns the hop count
+  int route(uint64_t seed, int32_t src, int32_t dst, int32_t conn, int32_t *out) const;
+
+ private:
+  phs_topology_desc d_;
+  int32_t gpus_, links_, tier1_base_, tier2_base_;
+};
+
+uint64_t splitmix64_step(uint64_t x);
+
+// Appends flows / collectives to an instance (S3).  Return PHS_OK or an error with *why set.
+phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                             double bytes, double start, const int32_t *after, int32_t n_after, std::string *why);
+phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,
+                        const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                        const int32_t *conn_id, std::string *why);
+
+}  // namespace phs

@@ -1,0 +1,178 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Bar (BASELINE.json north_star): completion times within 1e-9 relative -- and in
+fact bit-equal, because both sides do the same IEEE operations in the same order per flow and every reduction is
+an integer count or a min; completion order identical (ties by flow id); bottleneck ids and the event log
+(time, completions, activations, filling iterations, first bottleneck) exact."""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2505_01616_b200 import binding as B
+from paper_2505_01616_b200 import workloads as W
+from util import completion_order, oracle_run
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+CTA, CLUSTER = 1, 2
+
+
+def assert_instance_matches(sim, i, o, check_log=True):
+    t, to = sim.completion_times(i), o.completion_times()
+    assert not np.isnan(t).any()
+    np.testing.assert_allclose(t, to, rtol=1e-9, atol=0)           # the stated bar
+    assert np.array_equal(t, to), "completion times are expected to be bit-equal"
+    assert np.array_equal(completion_order(t), completion_order(to))
+    assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+    assert np.array_equal(sim.collective_times(i), o.collective_times()) or o.num_collectives == 0
+    if check_log:
+        ev, evo = sim.event_log(i), o.event_log()
+        assert len(ev) == len(evo)
+        for k in ("t", "n_completed", "n_activated", "n_rounds", "first_bneck"):
+            assert np.array_equal(ev[k], evo[k]), k
+
+
+def run_and_compare(w, path=0, cta_slots=0, first=0, count=None, mode=orc.MODE_FAST, expect_path=None):
+    count = w.batch if count is None else count
+    sim = B.Sim.from_workload(w, event_log=True, instances=(first, count), path=path, cta_slots=cta_slots)
+    sim.run()
+    for i in range(count):
+        o = oracle_run(w.desc, w.instances[first + i], mode=mode, base_seed=w.base_seed)
+        assert_instance_matches(sim, i, o)
+        if expect_path:
+            assert sim.path_of(i) == expect_path
+    c = sim.counters()
+    assert c["n_flow_events"] == 2 * sim.total_flows
+    sim.close()
+    return c
+
+
+@pytest.mark.parametrize("path", [CTA, CLUSTER])
+def test_cfg0_full(path):
+    run_and_compare(W.cfg0(), path=path, mode=orc.MODE_NAIVE, expect_path="cta" if path == CTA else "cluster")
+
+
+def test_cfg1_instances_cta():
+    # instance 0 (16 MiB / 1 GiB, symmetric: exact ties everywhere) and three log-uniform ones; 5632 flows each
+    run_and_compare(W.cfg1(batch=4), path=0, expect_path="cta")
+
+
+def test_cfg1_instance_cluster():
+    run_and_compare(W.cfg1(batch=2), path=CLUSTER, first=1, count=1, expect_path="cluster")
+
+
+def test_cfg3_instances_cta():
+    run_and_compare(W.cfg3(batch=6), path=0, expect_path="cta")
+
+
+def test_cfg3_seed_is_instance_index_in_sub_batches():
+    run_and_compare(W.cfg3(batch=40), first=37, count=3)
+
+
+@pytest.mark.parametrize("path", [CTA, CLUSTER])
+def test_cfg2_shrunken_fat_tree(path):
+    # k=8: 128 GPUs, 3-tier paths of 2/4/6 hops, staggered start times, AR + AG + RS mix; ragged tails everywhere
+    run_and_compare(W.cfg2(k=8, agg_uplinks=2), path=path)
+
+
+@pytest.mark.parametrize("path", [CTA, CLUSTER])
+def test_cfg4_shrunken_alltoall(path):
+    # 64 GPUs, 4032 concurrent Zipf flows, many filling rounds per event
+    run_and_compare(W.cfg4(batch=2, n_hosts=8, gph=8, n_leaves=4, n_spines=2), path=path)
+
+
+def test_cta_slot_overflow_falls_back_to_cluster():
+    w = W.cfg4(batch=3, n_hosts=4, gph=8, n_leaves=2, n_spines=2)      # 992 flows pending at t=0 > 64 slots
+    sim = B.Sim.from_workload(w, event_log=True, cta_slots=64)
+    sim.run()
+    for i in range(3):
+        assert sim.path_of(i) == "cluster"
+        assert_instance_matches(sim, i, oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST))
+    sim.run()                                                           # second run goes straight to the cluster path
+    assert_instance_matches(sim, 1, oracle_run(w.desc, w.instances[1], mode=orc.MODE_FAST))
+    sim.close()
+
+
+def test_rerun_is_idempotent_and_batch_position_independent():
+    w = W.cfg3(batch=5)
+    a = B.Sim.from_workload(w)
+    a.run()
+    t1 = [a.completion_times(i) for i in range(5)]
+    a.run()
+    for i in range(5):
+        assert np.array_equal(a.completion_times(i), t1[i])
+    b = B.Sim.from_workload(w, instances=(3, 2))
+    b.run()
+    assert np.array_equal(b.completion_times(0), t1[3]) and np.array_equal(b.completion_times(1), t1[4])
+    a.close(); b.close()
+
+
+def test_edge_cases():
+    d = W.topo_desc(W.TOPO_SINGLE, 2, 8)
+    # empty instance next to a non-empty one; zero-latency chain; a flow that can never start (cycle-free API, so
+    # "never" = waits on nothing -> fine); simultaneous bit-equal completions
+    sim = B.Sim(d, batch=3, event_log=True)
+    B.phs_add_flows(sim.h, 1, [0, 1, 2], [8, 8, 8], [1e6, 2e6, 4e6])
+    B.phs_add_collective(sim.h, 2, B.ALLTOALL, np.arange(16, dtype=np.int32), 1e6)
+    sim.run()
+    assert sim.num_flows(0) == 0 and len(sim.completion_times(0)) == 0 and len(sim.event_log(0)) == 0
+    o = orc.Sim(d, 1); o.add_flows([0, 1, 2], [8, 8, 8], [1e6, 2e6, 4e6]); o.run()
+    assert_instance_matches(sim, 1, o)
+    o = orc.Sim(d, 2); o.add_collective(orc.ALLTOALL, np.arange(16, dtype=np.int32), 1e6); o.run()
+    assert_instance_matches(sim, 2, o)
+    sim.close()
+    d0 = W.topo_desc(W.TOPO_SINGLE, 2, 8, hop_latency_s=0.0)
+    sim = B.Sim(d0, batch=1, event_log=True)
+    n = 50
+    src = np.arange(n) % 16
+    dst = (src + 3) % 16
+    dep_off = np.concatenate([[0], np.arange(n)])          # flow i waits for flow i-1: a zero-latency chain
+    dep_ids = np.arange(n - 1)
+    B.phs_add_flows(sim.h, 0, src, dst, np.full(n, 1e5), None, dep_off, dep_ids)
+    sim.run()
+    o = orc.Sim(d0, 0); o.add_flows(src, dst, np.full(n, 1e5), None, dep_off, dep_ids); o.run()
+    assert_instance_matches(sim, 0, o)
+    sim.close()
+
+
+def test_device_output_pointer():
+    import torch
+    w = W.cfg0()
+    sim = B.Sim.from_workload(w)
+    st = torch.cuda.Stream()
+    sim.run(stream=st.cuda_stream)
+    out = torch.empty(sim.num_flows(0), dtype=torch.float64, device="cuda")
+    B.phs_get_completion_times(sim.h, 0, device_ptr=out.data_ptr())
+    st.synchronize()
+    assert np.array_equal(out.cpu().numpy(), sim.completion_times(0))
+    sim.close()
+
+
+def _golden(name):
+    z = np.load(os.path.join(GOLD, name))
+    return z["idx"], z["t_done"], z["bneck"], int(z["n_events"]), z["sha_t"].item()
+
+
+@pytest.mark.parametrize("name,make,inst", [
+    ("cfg4_inst0", lambda: W.cfg4(batch=1), 0),
+    ("cfg2_inst0", lambda: W.cfg2(), 0),
+])
+def test_full_size_against_stored_oracle_samples(name, make, inst):
+    """BASELINE.json's full sizes, in the launch configuration bench.py uses.  The expected values were written
+    by tests/golden/make_golden.py, which calls only oracle/ (fast mode)."""
+    import hashlib
+    path = os.path.join(GOLD, name + ".npz")
+    if not os.path.exists(path):
+        pytest.skip("golden file not generated")
+    idx, t_ref, b_ref, n_events, sha = _golden(name + ".npz")
+    w = make()
+    sim = B.Sim.from_workload(w)
+    sim.run()
+    t = sim.completion_times(inst)
+    assert np.array_equal(t[idx], t_ref)
+    assert np.array_equal(sim.bottlenecks(inst)[idx], b_ref)
+    assert hashlib.sha256(t.tobytes()).hexdigest() == sha
+    assert sim.counters()["n_events"] == n_events
+    sim.close()

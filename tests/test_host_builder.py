@@ -1,0 +1,142 @@
+"""CPU-side tests of the library: the C-ABI loads and exports every symbol of include/phs.h; the host builder's
+integer artefacts (ECMP paths, dependency DAG, flow table) equal the oracle's exactly; error behaviour; and the
+product path fails loudly (no CPU fallback) when no CUDA device is usable."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2505_01616_b200 import binding as B
+from paper_2505_01616_b200 import workloads as W
+from util import oracle_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "phs.h")).read()
+    declared = set(re.findall(r"\b(phs_[a-z_]+)\s*\(", hdr))
+    declared -= {"phs_sim", "phs_status"}
+    assert declared == set(B.SYMBOLS), declared ^ set(B.SYMBOLS)
+    lib = B.lib()
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def _compare_tables(w, first=0, count=None):
+    count = w.batch if count is None else count
+    sim = B.Sim.from_workload(w, instances=(first, count))
+    for i in range(count):
+        o = oracle_build(w.desc, w.instances[first + i], base_seed=w.base_seed)
+        off, links = sim.paths(i)
+        ooff, olinks = o.paths()
+        assert np.array_equal(off, ooff) and np.array_equal(links, olinks)
+        poff, pr = sim.preds(i)
+        opoff, opr = o.preds()
+        assert np.array_equal(poff, opoff) and np.array_equal(pr, opr)
+        for a, b in zip(sim.flows(i), o.flows()):
+            assert np.array_equal(a, b)
+        assert B.phs_num_collectives(sim.h, i) == o.num_collectives
+        assert np.array_equal(B.phs_get_link_capacities(sim.h, i), o.link_capacities())
+    sim.close()
+
+
+@pytest.mark.parametrize("wl", [
+    lambda: W.cfg0(),
+    lambda: W.cfg1(batch=3),
+    lambda: W.cfg2(k=8, agg_uplinks=2),
+    lambda: W.cfg3(batch=3),
+    lambda: W.cfg4(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2),
+])
+def test_paths_dag_and_flow_table_equal_the_oracle(wl):
+    _compare_tables(wl())
+
+
+def test_full_size_tables_equal_the_oracle():
+    _compare_tables(W.cfg2())                       # 1,069,056 flows, 6-hop fat-tree paths
+    _compare_tables(W.cfg4(batch=2), first=1, count=1)
+    _compare_tables(W.cfg3(batch=130), first=128, count=2)   # seed = instance survives sub-batching
+
+
+def test_after_and_alltoall_dag_equal_the_oracle():
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=2, uplinks_per_leaf_spine=2)
+    ops = [W.Coll(W.ALLTOALL, np.arange(0, 16, 2, dtype=np.int32), 8e6),
+           W.Coll(W.ALLREDUCE_RING, np.array([2, 3, 4, 9, 8], np.int32), 5e6, 1e-4, (0,)),
+           W.Coll(W.ALLTOALL, np.array([8, 4, 1], np.int32), 3e6, 0.0, (0, 1)),
+           W.RawFlows(np.array([0, 1, 2], np.int32), np.array([5, 6, 7], np.int32), np.array([1e5, 2e5, 3e5]),
+                      dep_off=np.array([0, 0, 1, 3]), dep_ids=np.array([0, 0, 1]), conn_id=np.array([7, 7, 9], np.int32)),
+           W.Coll(W.REDUCESCATTER_RING, np.array([15, 0, 7], np.int32), 6e6, 0.0, (2,))]
+    _compare_tables(W.Workload("mixed", d, 5, [W.Instance(seed=0, ops=ops), W.Instance(seed=1, ops=ops)]))
+
+
+def test_input_validation_and_state_errors():
+    d = W.topo_desc(W.TOPO_SINGLE, 2, 8)
+    h = B.phs_create_topology(d, 0, 2)
+    for bad in [lambda: B.phs_add_flows(h, 0, [0], [0], [1.0]),
+                lambda: B.phs_add_flows(h, 0, [0], [1], [0.0]),
+                lambda: B.phs_add_flows(h, 0, [0], [1], [float("nan")]),
+                lambda: B.phs_add_flows(h, 0, [0], [99], [1.0]),
+                lambda: B.phs_add_flows(h, 5, [0], [1], [1.0]),
+                lambda: B.phs_add_collective(h, 0, B.ALLREDUCE_RING, [0, 1, 1], 1e6),
+                lambda: B.phs_add_collective(h, 0, B.ALLREDUCE_RING, [0], 1e6),
+                lambda: B.phs_add_collective(h, 0, 9, [0, 1], 1e6),
+                lambda: B.phs_add_collective(h, 0, B.ALLREDUCE_RING, [0, 1], 1e6, after=[0]),
+                lambda: B.phs_add_flows(h, 0, [0], [1], [1.0], dep_off=[0, 1], dep_ids=[0])]:
+        with pytest.raises(B.PhsError) as e:
+            bad()
+        assert e.value.code == B.PHS_EINVAL
+    assert B.phs_num_flows(h, 0) == 0 and B.phs_num_flows(h, 1) == 0
+    assert B.phs_add_collective(h, -1, B.ALLGATHER_RING, [0, 1, 2], 3e6) == 0
+    assert B.phs_num_flows(h, 0) == 6 and B.phs_num_flows(h, 1) == 6
+    with pytest.raises(B.PhsError) as e:
+        B.phs_get_completion_times(h, 0)
+    assert e.value.code == B.PHS_ESTATE
+    with pytest.raises(B.PhsError):
+        B.phs_create_topology(dict(d, n_hosts=0), 0, 1)
+    with pytest.raises(B.PhsError):
+        B.phs_create_topology(W.topo_desc(W.TOPO_FAT_TREE, 7, 2, k=4, agg_uplinks=1), 0, 1)
+    B.phs_destroy(h)
+
+
+def test_no_cpu_fallback_without_a_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    w = W.cfg0()
+    sim = B.Sim.from_workload(w)
+    with pytest.raises(B.PhsError) as e:
+        sim.run()
+    assert e.value.code == B.PHS_ECUDA
+    sim.close()
+
+
+def test_world_size_2_sharding_over_gloo():
+    """N>1 path of bench.py: instances are sharded round-robin over ranks with no data-path collective; only the
+    timing max and the counts are reduced.  Run the sharding + reduction logic on CPU over gloo."""
+    import subprocess
+    import sys
+    code = r'''
+import os, sys, torch, torch.distributed as dist
+sys.path.insert(0, os.environ["PHS_ROOT"])
+import bench
+dist.init_process_group("gloo")
+r, n = dist.get_rank(), dist.get_world_size()
+mine = bench.shard_instances(64, r, n)
+cnt = torch.tensor([len(mine)], dtype=torch.int64); dist.all_reduce(cnt)
+ms = torch.tensor([10.0 + r], dtype=torch.float64); dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+allm = [None] * n; dist.all_gather_object(allm, mine)
+flat = sorted(sum(allm, []))
+assert flat == list(range(64)), flat
+assert cnt.item() == 64 and ms.item() == 10.0 + n - 1
+dist.destroy_process_group()
+'''
+    env = dict(os.environ, PHS_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29533", "-c", code],
+                       env=env, capture_output=True, text=True, timeout=300)
+    if r.returncode != 0 and "unrecognized arguments: -c" in (r.stderr + r.stdout):
+        pytest.skip("torchrun cannot take -c")
+    assert r.returncode == 0, r.stderr[-2000:]

@@ -5,7 +5,8 @@ from oracle import orc
 from paper_2505_01616_b200 import workloads as W
 
 
-def oracle_run(desc, inst, mode=orc.MODE_NAIVE, trace=False, base_seed=0):
+def oracle_build(desc, inst, base_seed=0):
+    """Oracle instance with the workload submitted but not run."""
     sim = orc.Sim(desc, seed=base_seed + inst.seed)
     cap = inst.capacities(desc, sim.num_links)
     if cap is not None:
@@ -14,6 +15,11 @@ def oracle_run(desc, inst, mode=orc.MODE_NAIVE, trace=False, base_seed=0):
             lambda kind, ranks, nbytes, start, after: sim.add_collective(kind, ranks, nbytes, start, after),
             lambda src, dst, nbytes, start, dep_off, dep_ids, conn: sim.add_flows(src, dst, nbytes, start, dep_off,
                                                                                    dep_ids, conn))
+    return sim
+
+
+def oracle_run(desc, inst, mode=orc.MODE_NAIVE, trace=False, base_seed=0):
+    sim = oracle_build(desc, inst, base_seed)
     sim.run(mode=mode, trace=trace)
     return sim
 
