@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (one "step" = one pass of the whole simulation over one batch of
+synthetic instances) on N GPUs of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1] [--impl ours|reference]
+
+N=1 workload = BASELINE.json configs[1] (cfg1: 64 instances x 5,632 flows, leaf-spine, TP + DP ring all-reduces).
+Prints ONE JSON line (rank 0).  `value` = flow-events/s with the tables already resident in HBM; `e2e` = the same
+metric through the C-ABI from HOST arrays (submission calls, table build, H2D, run, D2H inside the timed region).
+N>1: instances are independent, so each rank simulates its own block of instances (weak scaling, no data-path
+collective); time = max over ranks.
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+import numpy as np
+
+METRIC = "flow_events_per_sec"
+UNIT = "flow-events/s"
+
+
+def shard_instances(total, rank, world):
+    """Contiguous block of instance indices of rank `rank` (instances are independent: no collective)."""
+    per = total // world
+    extra = total % world
+    lo = rank * per + min(rank, extra)
+    return list(range(lo, lo + per + (1 if rank < extra else 0)))
+
+
+def make_workload(name, n_gpus):
+    from paper_2505_01616_b200 import workloads as W
+    if name == "cfg0":
+        return W.cfg0(), 1
+    if name == "cfg1":
+        return W.cfg1(batch=64 * n_gpus), 64
+    if name == "cfg2":
+        return W.cfg2(), 1
+    if name == "cfg3":
+        return W.cfg3(batch=4096 * n_gpus), 4096
+    if name == "cfg4":
+        return W.cfg4(batch=8 * n_gpus), 8
+    raise SystemExit(f"unknown workload {name}")
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except Exception:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------- oracle legs
+def oracle_time(w, indices, mode=1):
+    """Runs the CPU oracle (fast mode, single thread) over the given instances; returns (seconds in orc_run,
+    flow count, collectives, summed work counters)."""
+    from oracle import orc
+    from util import oracle_build
+    secs, flows, colls = 0.0, 0, 0
+    work = {}
+    for i in indices:
+        sim = oracle_build(w.desc, w.instances[i], base_seed=w.base_seed)
+        t0 = time.perf_counter()
+        sim.run(mode=mode)
+        secs += time.perf_counter() - t0
+        flows += sim.num_flows
+        colls += w.instances[i].n_collectives
+        for k, v in sim.work_counters().items():
+            work[k] = work.get(k, 0.0) + v
+        sim.close()
+    return secs, flows, colls, work
+
+
+def algorithmic_bytes(work):
+    """per event A(36+20h) + 12*Lambda_act + 40c  (every active flow's state and
+    path read/updated once, every active link's (cap_rem, n) touched once, retire + release per completion).
+    The survey's formula additionally re-reads the link state once per SEQUENTIAL filling iteration
+    (12*Lambda_act*R); that variant is reported separately as `survey_formula`."""
+    base = 36.0 * work["sum_A"] + 20.0 * work["sum_Ah"] + 40.0 * work["completions"]
+    return base + 12.0 * work["sum_Lam"], base + 12.0 * work["sum_LamR"]
+
+
+# ---------------------------------------------------------------------------------------------- reference arm
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    w, per_rank = make_workload(args.workload, 1)
+    # bounded sample: a few instances per step so the whole run stays within minutes
+    per_step = {"cfg0": 1, "cfg1": 4, "cfg2": 1, "cfg3": 8, "cfg4": 1}[args.workload]
+    if args.workload in ("cfg2", "cfg4"):
+        raise SystemExit("reference arm: cfg2/cfg4 take minutes per instance on the CPU oracle; use cfg0/cfg1/cfg3")
+    nxt = 0
+    def step():
+        nonlocal nxt
+        idx = [(nxt + k) % w.batch for k in range(per_step)]
+        nxt = (nxt + per_step) % w.batch
+        return oracle_time(w, idx)
+    for _ in range(args.warmup):
+        step()
+    secs = flows = colls = 0
+    for _ in range(args.steps):
+        s, f, c, _w = step()
+        secs += s; flows += f; colls += c
+    val = 2.0 * flows / secs
+    sample = f"{per_step} instances of {args.workload} per step (oracle fast mode, time inside orc_run only)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64+i64", "data": "synthetic",
+        "config": {"workload": args.workload, "sample": sample},
+        "collectives_per_sec": colls / secs,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+# ---------------------------------------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    from paper_2505_01616_b200 import binding as B
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    w, per_rank = make_workload(args.workload, world)
+    mine = shard_instances(w.batch, rank, world)
+    first, count = mine[0], len(mine)
+    stream = torch.cuda.Stream()
+    sp = stream.cuda_stream
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+
+    # ---- device-resident arm: tables built and uploaded once, each step = phs_run
+    sim = B.Sim.from_workload(w, instances=(first, count))
+    sim.finalize(stream=sp)
+    flows = sim.total_flows
+    colls = sum(w.instances[i].n_collectives for i in mine)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step():
+        flush_buf.zero_()                       # L2 flush between timed iterations (outside the events)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            sim.run(stream=sp)
+            e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), sim.counters()
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ms_total, kern_ms, launches = 0.0, 0.0, 0
+    for _ in range(args.steps):
+        ms, c = one_step()
+        ms_total += ms
+        kern_ms += c["main_kernel_ms"]
+        launches += c["n_kernel_launches"]
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    counters = sim.counters()
+    paths = sorted({sim.path_of(i) for i in range(count)})
+
+    # ---- end-to-end arm: host arrays -> C-ABI submission -> table build -> H2D -> run -> D2H, every step
+    def e2e_step():
+        t0 = time.perf_counter()
+        s2 = B.Sim.from_workload(w, instances=(first, count))
+        s2.run(stream=sp)
+        out = B.phs_get_all_completion_times(s2.h)
+        dt = time.perf_counter() - t0
+        c = s2.counters()
+        s2.close()
+        return dt, c["h2d_bytes"], out.nbytes + 40 * count
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_step()
+    barrier()
+    e2e_s, h2d, d2h = 0.0, 0, 0
+    for _ in range(e2e_steps):
+        dt, h2d, d2h = e2e_step()
+        e2e_s += dt
+    barrier()
+
+    # ---- reduce over ranks: time = max, work = sum
+    tot = torch.tensor([ms_total, e2e_s, kern_ms], dtype=torch.float64, device="cuda")
+    work = torch.tensor([flows, colls, launches], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work)
+    ms_total, e2e_s, kern_ms = tot.tolist()
+    flows_all, colls_all, launches_all = work.tolist()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    value = 2.0 * flows_all * args.steps / (ms_total * 1e-3)
+    e2e_value = 2.0 * flows_all * e2e_steps / e2e_s
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64+i64", "data": "synthetic",
+        "config": {"workload": args.workload, "instances_per_gpu": count, "flows_per_gpu": flows,
+                   "kernel_paths": paths, "l2": "flushed between timed steps (256 MiB write)",
+                   "events_per_step": counters["n_events"], "parallel_rounds_per_step": counters["sum_par_rounds"]},
+        "collectives_per_sec": colls_all * args.steps / (ms_total * 1e-3),
+        "sim_events_per_sec": counters["n_events"] * world * args.steps / (ms_total * 1e-3),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps, "note": "host arrays -> phs_add_* -> phs_finalize (H2D) -> phs_run -> D2H"},
+        "gpu_launches": int(launches_all),
+        "clocks": clocks,
+    }
+    # ---- CPU baseline (oracle, bounded sample) and roofline, rank 0 at N=1 only
+    if world == 1 and not args.no_cpu_baseline:
+        n_cpu = {"cfg0": 1, "cfg1": 64, "cfg2": 0, "cfg3": 96, "cfg4": 0}[args.workload]
+        if n_cpu:
+            idx = list(range(min(n_cpu, w.batch)))
+            secs, f_cpu, c_cpu, wk = oracle_time(w, idx)
+            sample = f"instances 0..{len(idx) - 1} of {args.workload} ({f_cpu} flows), oracle fast mode, 1 thread"
+            out["cpu_baseline"] = {"value": 2.0 * f_cpu / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                   "sample": sample, "seconds": secs, "host_cores": os.cpu_count()}
+            # algorithmic bytes of ONE step = the oracle's per-event work counts, scaled to the whole batch
+            scale = flows / float(f_cpu)
+            conservative, survey = algorithmic_bytes(wk)
+            peaks = {}
+            try:
+                peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            except Exception:
+                pass
+            peak = float(peaks.get("hbm_gbs", 6650.0))
+            k_s = (kern_ms / args.steps) * 1e-3
+            traffic = None
+            try:
+                traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.workload)
+            except Exception:
+                pass
+            out["roofline"] = {"bound": "hbm", "achieved": conservative * scale / k_s / 1e9, "peak": peak,
+                               "unit": "GB/s", "frac": conservative * scale / k_s / 1e9 / peak, "traffic": traffic,
+                               "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)" if peaks else "6650 (of fallback)",
+                               "kernel": "phs_cta_kernel" if paths == ["cta"] else "+".join(paths),
+                               "kernel_ms": kern_ms / args.steps,
+                               "algorithmic_bytes_per_step": conservative * scale,
+                               "survey_formula": {"bytes_per_step": survey * scale,
+                                                  "achieved": survey * scale / k_s / 1e9}}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -77,6 +77,10 @@ typedef struct {
   int64_t n_flow_events; /* activations + completions = 2 * flows                                         */
   int64_t sum_active;    /* sum over events of active flows                                               */
   int64_t sum_par_rounds;/* sum over events of parallel filling rounds executed by the kernels            */
+  int64_t n_kernel_launches; /* kernels launched by the last phs_run                                      */
+  int64_t h2d_bytes;     /* bytes phs_finalize copied to the device                                       */
+  double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
+                         /* the run's stream), excluding the result copies                                */
 } phs_counters;
 
 /* Creates `batch` independent instances of one topology.  Instance i routes with ECMP seed `seed + i`.

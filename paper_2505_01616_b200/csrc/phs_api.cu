@@ -77,7 +77,8 @@ struct phs_sim {
   // ---- device tables
   DevBuf<InstDesc> d_desc;
   DevBuf<FlowRec> d_rec;
-  DevBuf<int32_t> d_path, d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n;
+  DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n;
+  DevBuf<uint8_t> d_pc8;
   DevBuf<int64_t> d_capq, d_coll_first;
   DevBuf<double> d_tdone, d_coll_t;
   DevBuf<InstResult> d_res;
@@ -95,10 +96,16 @@ struct phs_sim {
   bool clist_dirty = true;
 
   // launch configuration of the CTA path
-  int cta_threads = 0, cta_acap = 0, cta_pcap = 0, cta_grid = 0;
-  size_t cta_smem = 0;
+  CtaLaunch cta{};
   int sm_count = 0;
   cudaStream_t last_stream = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  int64_t n_launches = 0, h2d_bytes = 0;
+  float main_kernel_ms = 0.f;
+  ~phs_sim() {
+    if (ev0) cudaEventDestroy(ev0);
+    if (ev1) cudaEventDestroy(ev1);
+  }
 };
 
 extern "C" {
@@ -336,21 +343,23 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   sim->flow_base.assign(B + 1, 0);
   sim->coll_base.assign(B + 1, 0);
   sim->log_base.assign(B + 1, 0);
-  std::vector<int64_t> path_base(B + 1, 0), succ_base(B + 1, 0);
+  std::vector<int64_t> succ_base(B + 1, 0), pc8_base(B + 1, 0);
+  int max_pred = 0;
   for (int i = 0; i < B; ++i) {
     const Instance &in = sim->inst[i];
     sim->flow_base[i + 1] = sim->flow_base[i] + in.n_flows();
     sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)in.colls.size();
     sim->log_base[i + 1] = sim->log_base[i] + 2 * in.n_flows() + 2;
-    path_base[i + 1] = path_base[i] + (int64_t)in.path.size();
     succ_base[i + 1] = succ_base[i] + (int64_t)in.pred.size();
+    pc8_base[i + 1] = pc8_base[i] + (in.n_flows() + 3) / 4 * 4;
   }
   sim->total_flows = sim->flow_base[B];
   sim->total_colls = sim->coll_base[B];
   const int64_t Ft = sim->total_flows;
 
-  std::vector<FlowRec> rec((size_t)(Ft + B));
-  std::vector<int32_t> path((size_t)path_base[B]), succ((size_t)succ_base[B]), pc0((size_t)Ft);
+  std::vector<FlowRec> rec((size_t)Ft);
+  std::vector<int32_t> succ((size_t)succ_base[B]), pc0((size_t)Ft);
+  std::vector<uint8_t> pc8((size_t)pc8_base[B], 0);
   std::vector<int64_t> capq((size_t)B * L), coll_first((size_t)sim->total_colls);
   std::vector<int32_t> coll_n((size_t)sim->total_colls);
   sim->h_desc.resize(B);
@@ -368,43 +377,50 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     std::vector<uint32_t> soff((size_t)F + 1, 0);
     for (int32_t p : in.pred) soff[(size_t)p + 1]++;
     for (int64_t f = 0; f < F; ++f) soff[f + 1] += soff[f];
+    int32_t *sdst = succ.data() + succ_base[i];
     {
       std::vector<uint32_t> cur(soff.begin(), soff.end() - 1);
-      int32_t *sdst = succ.data() + succ_base[i];
       for (int64_t f = 0; f < F; ++f)
         for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
     }
-    FlowRec *r = rec.data() + sim->flow_base[i] + i;
-    for (int64_t f = 0; f <= F; ++f) {
+    FlowRec *r = rec.data() + sim->flow_base[i];
+    for (int64_t f = 0; f < F; ++f) {
       FlowRec x;
-      x.bytes = f < F ? in.bytes[f] : 0.0;
-      x.start = f < F ? in.start[f] : 0.0;
-      x.lat = f < F ? in.lat[f] : 0.0;
-      x.path_off = in.path_off[f];
+      x.bytes = in.bytes[f];
+      x.start = in.start[f];
+      x.lat = in.lat[f];
+      const uint32_t p0 = in.path_off[f], p1 = in.path_off[f + 1];
+      for (int h = 0; h < kMaxHops; ++h) x.path[h] = p0 + h < p1 ? in.path[p0 + h] : -1;
       x.succ_off = soff[f];
+      x.succ_cnt = (int32_t)(soff[f + 1] - soff[f]);
+      x.succ_in[0] = x.succ_cnt > 0 ? sdst[soff[f]] : -1;
+      x.succ_in[1] = x.succ_cnt > 1 ? sdst[soff[f] + 1] : -1;
       r[f] = x;
+      const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
+      pc0[sim->flow_base[i] + f] = np;
+      max_pred = std::max(max_pred, np);
+      pc8[pc8_base[i] + f] = (uint8_t)std::min(np, 255);
     }
-    std::copy(in.path.begin(), in.path.end(), path.begin() + path_base[i]);
-    for (int64_t f = 0; f < F; ++f) pc0[sim->flow_base[i] + f] = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
     for (size_t c = 0; c < in.colls.size(); ++c) {
       coll_first[sim->coll_base[i] + c] = sim->flow_base[i] + in.colls[c].first_flow;
       coll_n[sim->coll_base[i] + c] = in.colls[c].n_flows;
     }
     InstDesc d;
-    d.rec_base = sim->flow_base[i] + i;
     d.flow_base = sim->flow_base[i];
-    d.path_base = path_base[i];
+    d.path_base = 0;
     d.succ_base = succ_base[i];
     d.log_base = sim->want_log ? sim->log_base[i] : -1;
     d.coll_base = sim->coll_base[i];
+    d.pc8_base = pc8_base[i];
     d.n_flows = (int32_t)F;
     d.n_colls = (int32_t)in.colls.size();
     sim->h_desc[i] = d;
   }
+  const bool pc8_ok = max_pred <= 255;
 
   PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
   PHS_CUDA(sim->d_rec.upload(rec, st));
-  PHS_CUDA(sim->d_path.upload(path, st));
+  if (pc8_ok) PHS_CUDA(sim->d_pc8.upload(pc8, st));
   PHS_CUDA(sim->d_succ.upload(succ, st));
   PHS_CUDA(sim->d_pc0.upload(pc0, st));
   PHS_CUDA(sim->d_capq.upload(capq, st));
@@ -423,43 +439,59 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   // that enough CTAs are resident per SM to cover the batch; instances whose link state alone does not fit go to
   // the cluster path.  Instances that overflow their shared-memory slots at run time are re-run on the cluster path.
   const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin;
-  int threads = L <= 320 ? 128 : 256;
+  const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
   int64_t maxF = 0;
   for (int i = 0; i < B; ++i) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
-  const int want_ctas = std::max(1, std::min(2048 / threads / 2, (B + sim->sm_count - 1) / sim->sm_count));
-  const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
-  const size_t budget = std::min(smem_max, per_sm / want_ctas - 1024);
-  const size_t link_bytes = cta_smem_bytes(L, 0, 0);
+  const int threads = L <= 320 ? 128 : 256;
+  const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
-  int cap_slots = 0;
-  if (sim->policy_path != 2 && link_bytes + cta_smem_bytes(0, 64, 64) <= budget) {
-    int lo = 64, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 64), 1 << 20);
-    if (sim->policy_slots > 0) hi = std::max(64, std::min(hi, (int)sim->policy_slots));
-    hi = (hi + 31) / 32 * 32;
-    while (lo < hi) {  // largest multiple of 32 that fits the budget
-      const int mid = ((lo + hi + 32) / 64) * 32;
-      if (cta_smem_bytes(L, mid, mid) <= budget)
-        lo = mid;
-      else
-        hi = mid - 32;
+  sim->cta = CtaLaunch{};
+  if (sim->policy_path != 2 && maxF > 0) {
+    // resident CTAs per SM wanted: enough to cover the batch, at most what the thread count allows; fewer if the
+    // slots would otherwise not hold a typical active set (min(F, 256) flows)
+    int want = std::max(1, std::min(2048 / threads / 2, (B + sim->sm_count - 1) / sim->sm_count));
+    const int need = (int)std::min<int64_t>(maxF, 256);
+    for (; want >= 1; --want) {
+      const size_t budget = std::min(smem_max, per_sm / want - 1024);
+      const int pcf = pc8_ok && cta_smem_bytes(L, need, (int)maxF, log) <= budget ? (int)maxF : 0;
+      if (cta_smem_bytes(L, 32, pcf, log) > budget) continue;
+      int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
+      if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
+      hi = (hi + 31) / 32 * 32;
+      while (lo < hi) {  // largest multiple of 32 that fits the budget
+        const int mid = ((lo + hi + 32) / 64) * 32;
+        if (cta_smem_bytes(L, mid, pcf, log) <= budget)
+          lo = mid;
+        else
+          hi = mid - 32;
+      }
+      if (lo >= need || want == 1 || sim->policy_slots > 0) {
+        sim->cta.threads = threads;
+        sim->cta.slots = lo;
+        sim->cta.pc_flows = pcf;
+        sim->cta.smem = cta_smem_bytes(L, lo, pcf, log);
+        sim->cta.log = log;
+        break;
+      }
     }
-    cap_slots = lo;
   }
-  if (cap_slots > 0) {
-    sim->cta_threads = threads;
-    sim->cta_acap = sim->cta_pcap = cap_slots;
-    sim->cta_smem = cta_smem_bytes(L, cap_slots, cap_slots);
+  if (sim->cta.slots > 0) {
     for (int i = 0; i < B; ++i) sim->order.push_back(i);
     std::stable_sort(sim->order.begin(), sim->order.end(),
                      [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
-    const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta_smem + 1024)), 2048 / threads));
-    sim->cta_grid = std::min(B, per * sim->sm_count);
+    const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta.smem + 1024)), 2048 / threads));
+    sim->cta.grid = std::min(B, per * sim->sm_count);
     PHS_CUDA(sim->d_order.upload(sim->order, st));
   } else {
     for (int i = 0; i < B; ++i) sim->cluster_list.push_back(i);
   }
   PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
+  sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
+                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
+                             (capq.size() + coll_first.size()) * 8);
+  PHS_CUDA(cudaEventCreate(&sim->ev0));
+  PHS_CUDA(cudaEventCreate(&sim->ev1));
   sim->finalized = true;
   return PHS_OK;
 }
@@ -471,9 +503,9 @@ DevTables tables_of(phs_sim *sim) {
   DevTables t;
   t.inst = sim->d_desc.p;
   t.rec = sim->d_rec.p;
-  t.path = sim->d_path.p;
   t.succ = sim->d_succ.p;
   t.pred_cnt0 = sim->d_pc0.p;
+  t.pred_cnt0_u8 = sim->d_pc8.p;
   t.capq = sim->d_capq.p;
   t.pred_cnt = sim->d_pred_cnt.p;
   t.t_done = sim->d_tdone.p;
@@ -538,33 +570,45 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   sim->last_stream = st;
   const int B = sim->batch;
   DevTables t = tables_of(sim);
+  sim->n_launches = 0;
+  PHS_CUDA(cudaEventRecord(sim->ev0, st));
   if (!sim->order.empty()) {
+    sim->n_launches++;
     PHS_CUDA(cudaMemsetAsync(sim->d_ticket.p, 0, sizeof(int), st));
-    PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta_threads,
-                             sim->cta_acap, sim->cta_pcap, sim->cta_grid, sim->cta_smem, sim->want_log, st));
+    PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta, st));
   }
   {
     phs_status gs = run_cluster_path(sim, sim->cluster_list, st);
     if (gs != PHS_OK) return gs;
+    if (!sim->cluster_list.empty()) sim->n_launches++;
   }
+  PHS_CUDA(cudaEventRecord(sim->ev1, st));
   PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
   PHS_CUDA(cudaStreamSynchronize(st));
   // instances that ran out of shared-memory slots: re-run on the cluster path (and remember for later runs)
   std::vector<int32_t> redo;
   for (int i = 0; i < B; ++i)
     if (sim->h_res[i].status == kOverflow) redo.push_back(i);
+  PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
   if (!redo.empty()) {
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
     phs_status gs = run_cluster_path(sim, redo, st);
     if (gs != PHS_OK) return gs;
+    sim->n_launches++;
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
     for (int inst : redo) {
       sim->cluster_list.push_back(inst);
       sim->order.erase(std::find(sim->order.begin(), sim->order.end(), inst));
     }
     if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
-    sim->cta_grid = std::min<int>(sim->cta_grid, std::max<int>(1, (int)sim->order.size()));
+    sim->cta.grid = std::min<int>(sim->cta.grid, std::max<int>(1, (int)sim->order.size()));
     PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
     PHS_CUDA(cudaStreamSynchronize(st));
+    float extra = 0.f;
+    PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
+    sim->main_kernel_ms += extra;
   }
+  if (sim->total_colls > 0) sim->n_launches++;
   PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
                                    sim->d_coll_t.p, st));
   sim->ran = true;
@@ -651,6 +695,9 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
     c.sum_par_rounds += sim->h_res[i].sum_par_rounds;
   }
   c.n_flow_events = 2 * sim->total_flows;
+  c.n_kernel_launches = sim->n_launches;
+  c.h2d_bytes = sim->h2d_bytes;
+  c.main_kernel_ms = sim->main_kernel_ms;
   *out = c;
   return PHS_OK;
 }

@@ -72,8 +72,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     if (qi >= n_list) break;
     const int inst = list[qi];
     const InstDesc D = T.inst[inst];
-    const FlowRec *__restrict__ rec = T.rec + D.rec_base;
-    const int32_t *__restrict__ path = T.path + D.path_base;
+    const FlowRec *__restrict__ rec = T.rec + D.flow_base;
     const int32_t *__restrict__ succ = T.succ + D.succ_base;
     const int32_t *__restrict__ pc0 = T.pred_cnt0 + D.flow_base;
     int32_t *pred_cnt = T.pred_cnt + D.flow_base;
@@ -132,15 +131,13 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           else
             slot = atomicAdd(&ctl[K_HI], 1);
           const FlowRec r = rec[f];
-          const uint32_t pe = rec[f + 1].path_off;
           a_flow[slot] = f;
           a_rem[slot] = r.bytes;
           a_bn[slot] = -1;
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
-            int l = -1;
-            if (r.path_off + h < pe) {
-              l = path[r.path_off + h];
+            const int l = r.path[h];
+            if (l >= 0) {
               atomicAdd(&nl[l], 1);
               dirty[l] = 1;
             }
@@ -337,7 +334,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           atomicSub(&ctl[K_NACTIVE], 1);
           atomicAdd(&ctl[K_DONE], 1);
           if (LOG) atomicAdd(&ctl[K_EV_NCOMP], 1);
-          const uint32_t e0 = rec[f].succ_off, e1 = rec[f + 1].succ_off;
+          const uint32_t e0 = rec[f].succ_off, e1 = e0 + (uint32_t)rec[f].succ_cnt;
           for (uint32_t e = e0; e < e1; ++e) {
             const int g = succ[e];
             if (atomicSub(&pred_cnt[g], 1) == 1) {

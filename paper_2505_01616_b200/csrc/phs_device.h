@@ -9,10 +9,10 @@ namespace phs {
 
 struct DevTables {
   const InstDesc *inst;      // [B]
-  const FlowRec *rec;        // [F_total + B]   (one sentinel per instance)
-  const int32_t *path;       // flow -> link CSR values (all instances)
+  const FlowRec *rec;        // [F_total]
   const int32_t *succ;       // successor CSR values (instance-relative flow ids)
   const int32_t *pred_cnt0;  // [F_total] number of predecessors
+  const uint8_t *pred_cnt0_u8;  // same as bytes (per-instance slices 4-byte aligned), or nullptr if a count > 255
   const int64_t *capq;       // [B][n_links] link capacity in rate quanta
   int32_t *pred_cnt;         // [F_total] outstanding predecessors (dynamic)
   double *t_done;            // [F_total] O1
@@ -22,13 +22,19 @@ struct DevTables {
   int32_t n_links;
 };
 
-// Shared-memory footprint of the CTA kernel for given capacities.
-size_t cta_smem_bytes(int n_links, int acap, int pcap);
+// Shared-memory footprint of the CTA kernel for given capacities (pc_flows > 0: predecessor counters of that
+// many flows are kept in shared memory as bytes).
+size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log);
 
 // One CTA per instance (persistent CTAs pull instance indices from order[0..n) through *ticket).
 // Instances that run out of shared-memory slots finish with status kOverflow.
-cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, int threads, int acap,
-                            int pcap, int grid, size_t smem, bool log, cudaStream_t stream);
+struct CtaLaunch {
+  int threads, slots, pc_flows, grid;
+  size_t smem;
+  bool log;
+};
+cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &cfg,
+                            cudaStream_t stream);
 
 // Cluster path: one thread-block cluster (up to 16 CTAs, hardware cluster barrier) per large instance, all state
 // in global memory (L2-resident).  Clusters pull instance indices from list[0..n) through *ticket; the cluster

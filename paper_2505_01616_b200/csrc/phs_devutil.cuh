@@ -10,9 +10,26 @@ constexpr double kInf = __builtin_huge_val();
 // rate quanta -> byte/s: round-to-nearest conversion, exact power-of-two scale
 __device__ __forceinline__ double rate_of(long long rq) { return __ll2double_rn(rq) * kQuantum; }
 
-// a5: fair share of a link = floor(cap_rem / n), exact 64-bit integer division
+// a5: fair share of a link = floor(cap_rem / n), EXACT.  Two double-precision quotient estimates, each followed by
+// an exact 64-bit remainder, then an integer correction: whatever the rounding of the estimates, the loop invariant
+// q*n + r == cap_rem (64-bit integer arithmetic) makes the result the true floor.  cap_rem >= 0, n >= 1.
 __device__ __forceinline__ long long fair_share(long long cap_rem, int n) {
-  return n == 1 ? cap_rem : cap_rem / (long long)n;
+  if (n == 1) return cap_rem;
+  const double inv = 1.0 / (double)n;
+  long long q = __double2ll_rz(__ll2double_rz(cap_rem) * inv);
+  long long r = cap_rem - q * (long long)n;
+  const long long q2 = __double2ll_rz(__ll2double_rn(r) * inv);
+  q += q2;
+  r -= q2 * (long long)n;
+  while (r < 0) {
+    --q;
+    r += n;
+  }
+  while (r >= n) {
+    ++q;
+    r -= n;
+  }
+  return q;
 }
 
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }

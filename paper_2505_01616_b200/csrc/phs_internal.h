@@ -13,25 +13,29 @@ namespace phs {
 constexpr int kRateFracBits = 20;
 constexpr int kMaxHops = 6;  // longest path: fat tree cross-pod (S2)
 
-// Device-resident flow record, 32 bytes, one per flow plus one sentinel per instance (so that the path and
-// successor list of flow f end where those of f+1 begin).  Gathered once per flow, at activation / release.
+// Device-resident flow record, 64 bytes (half a cache line), one per flow.  Everything activation and release
+// need sits in the one record, so each costs a single (non-chained) global load: size, timing, the path inline
+// (ECMP paths have at most kMaxHops links, -1 padded) and the first two successors inline (a ring flow has at
+// most two; longer lists spill to succ[] at succ_off).
 struct FlowRec {
-  double bytes;       // flow size
-  double start;       // earliest submission time (S4)
-  double lat;         // path latency, left-to-right sum over the path's links (S2)
-  uint32_t path_off;  // into the instance's slice of path[]
-  uint32_t succ_off;  // into the instance's slice of succ[]
+  double bytes;          // flow size
+  double start;          // earliest submission time (S4)
+  double lat;            // path latency, left-to-right sum over the path's links (S2)
+  int32_t path[kMaxHops];  // flow -> link incidence row
+  uint32_t succ_off;     // into the instance's slice of succ[] (all successors, including the inline two)
+  int32_t succ_cnt;      // number of successors
+  int32_t succ_in[2];    // first two successors (instance-relative flow ids), -1 if absent
 };
-static_assert(sizeof(FlowRec) == 32, "FlowRec must be 32 bytes");
+static_assert(sizeof(FlowRec) == 64, "FlowRec must be 64 bytes");
 
 // Per-instance descriptor (device).
 struct InstDesc {
-  int64_t rec_base;   // first FlowRec of the instance (flow_base + instance index, because of the sentinels)
-  int64_t flow_base;  // first entry in the per-flow arrays (pred_cnt, t_done, bneck, ...)
-  int64_t path_base;  // first entry of the instance's slice of path[]
+  int64_t flow_base;  // first entry in the per-flow arrays (rec, pred_cnt, t_done, bneck, ...)
+  int64_t path_base;  // unused (paths are inline in FlowRec)
   int64_t succ_base;  // first entry of the instance's slice of succ[]
   int64_t log_base;   // first row of the instance's event log slice (capacity 2F+2 rows), -1 if disabled
   int64_t coll_base;  // first entry in the per-collective arrays
+  int64_t pc8_base;   // first byte of the instance's slice of pred_cnt0_u8 (4-byte aligned), -1 if unused
   int32_t n_flows;
   int32_t n_colls;
 };

@@ -118,25 +118,9 @@ def test_world_size_2_sharding_over_gloo():
     timing max and the counts are reduced.  Run the sharding + reduction logic on CPU over gloo."""
     import subprocess
     import sys
-    code = r'''
-import os, sys, torch, torch.distributed as dist
-sys.path.insert(0, os.environ["PHS_ROOT"])
-import bench
-dist.init_process_group("gloo")
-r, n = dist.get_rank(), dist.get_world_size()
-mine = bench.shard_instances(64, r, n)
-cnt = torch.tensor([len(mine)], dtype=torch.int64); dist.all_reduce(cnt)
-ms = torch.tensor([10.0 + r], dtype=torch.float64); dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-allm = [None] * n; dist.all_gather_object(allm, mine)
-flat = sorted(sum(allm, []))
-assert flat == list(range(64)), flat
-assert cnt.item() == 64 and ms.item() == 10.0 + n - 1
-dist.destroy_process_group()
-'''
     env = dict(os.environ, PHS_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
     r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
-                        "--master-addr", "127.0.0.1", "--master-port", "29533", "-c", code],
+                        "--master-addr", "127.0.0.1", "--master-port", "29533",
+                        os.path.join(ROOT, "tests", "_gloo_shard_worker.py")],
                        env=env, capture_output=True, text=True, timeout=300)
-    if r.returncode != 0 and "unrecognized arguments: -c" in (r.stderr + r.stdout):
-        pytest.skip("torchrun cannot take -c")
     assert r.returncode == 0, r.stderr[-2000:]
