@@ -576,12 +576,14 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
   double *rem = (double *)malloc(sizeof(double) * (F + 1));
   double *tc = (double *)malloc(sizeof(double) * (F + 1));
   int64_t *rq = (int64_t *)malloc(sizeof(int64_t) * (F + 1));
+  int64_t *rq_cur = (int64_t *)malloc(sizeof(int64_t) * (F + 1)); /* rate in effect since t_last (R-LZ) */
+  double *t_last = (double *)malloc(sizeof(double) * (F + 1));    /* time rem[] refers to (R-LZ)         */
   int32_t *act = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *pend = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *comp = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   s->t_done = (double *)malloc(sizeof(double) * (F + 1));
   s->bneck = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
-  if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !act || !pend || !comp ||
+  if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !rq_cur || !t_last || !act || !pend || !comp ||
       !s->t_done || !s->bneck || ws_init(&w, L)) {
     rc = ORC_ENOMEM;
     goto out;
@@ -621,6 +623,7 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
       int32_t f = pend[i];
       if (t_act[f] <= now) {
         rem[f] = s->bytes[f];
+        rq_cur[f] = -1; /* no rate yet */
         state[f] = ACTIVE;
         act[nA++] = f;
         n_activated++;
@@ -634,21 +637,33 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
       rc = ORC_ENOMEM;
       goto out;
     }
-    /* 3. next time: tc = now + rem/rate (div, then add); t_next = min(min tc, min pending t_act) */
+    /* 3. settle + next time (reading R-LZ, PAPER.md L128 / L167: a flow's throughput is piecewise constant and
+     *    its state is a function of its OWN rate changes).  A flow whose rate quanta did not change since its
+     *    last rate change is not touched.  On a change at `now`: rem -= rate_old * (now - t_last) (mul, sub,
+     *    clamp at 0), t_last = now, tc = now + rem / rate_new (div, then add).
+     *    t_next = min(min tc, min pending t_act). */
     if (nA == 0 && nP == 0) break;
     double t_next = INFINITY;
     double ah = 0;
     for (int32_t i = 0; i < nA; i++) {
       int32_t f = act[i];
-      double q = rem[f] / q_to_rate(rq[f]);
-      tc[f] = now + q;
+      if (rq[f] != rq_cur[f]) {
+        if (rq_cur[f] >= 0) {
+          double m = q_to_rate(rq_cur[f]) * (now - t_last[f]);
+          double r = rem[f] - m;
+          rem[f] = r > 0.0 ? r : 0.0;
+        }
+        t_last[f] = now;
+        rq_cur[f] = rq[f];
+        double q = rem[f] / q_to_rate(rq[f]);
+        tc[f] = now + q;
+      }
       if (tc[f] < t_next) t_next = tc[f];
       ah += (double)(s->path_off[f + 1] - s->path_off[f]);
     }
     for (int32_t i = 0; i < nP; i++)
       if (t_act[pend[i]] < t_next) t_next = t_act[pend[i]];
-    /* 4. advance */
-    double dt = t_next - now;
+    /* 4. advance: flows whose completion time is bit-equal to t_next complete; nobody else changes */
     int32_t nC = 0, na2 = 0;
     for (int32_t i = 0; i < nA; i++) {
       int32_t f = act[i];
@@ -667,9 +682,6 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
         state[f] = DONE;
         comp[nC++] = f;
       } else {
-        double m = q_to_rate(rq[f]) * dt; /* mul, then sub, then clamp */
-        double r = rem[f] - m;
-        rem[f] = r > 0.0 ? r : 0.0;
         act[na2++] = f;
       }
     }
@@ -703,7 +715,7 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
   if (n_done < F) rc = ORC_ECYCLE; /* WAITING flows left with nothing active or pending */
   s->ran = 1;
 out:
-  free(capq); free(succ_off); free(succ); free(pred_cnt); free(state); free(t_act); free(rem); free(tc); free(rq);
+  free(capq); free(succ_off); free(succ); free(pred_cnt); free(state); free(t_act); free(rem); free(tc); free(rq); free(rq_cur); free(t_last);
   free(act); free(pend); free(comp);
   ws_free(&w);
   return rc;

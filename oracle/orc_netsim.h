@@ -24,6 +24,10 @@
  * are held in exact 64-bit fixed point (quantum 2^-20 byte/s), so that the
  * water-filling result does not depend on the order in which capacity debits
  * are applied.  Time and byte arithmetic is IEEE binary64 without contraction.
+ * A second builder's reading, R-LZ (from L128 "between neighboring events, network flows are assumed to have
+ * stable throughput" and L167, where a flow's history is "a few floating point numbers" per throughput
+ * change): a flow's remaining bytes are settled only when ITS rate changes, so its completion time is a
+ * function of its own rate history and not of unrelated events elsewhere in the network.
  *
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"): P1 lone flow, P2 uniform
  * ring, P3 max-plus ring recurrence (cfg0), P4 bottleneck certificate, P5

@@ -479,6 +479,27 @@ def test_p9_byte_conservation_and_scaling():
     assert np.array_equal(s2.bottlenecks(), s.bottlenecks())
 
 
+def test_p9_locality_unrelated_traffic_does_not_change_a_single_bit():
+    """Reading R-LZ (PAPER.md L128 / L167): a flow's state changes only when its own rate changes, so adding
+    traffic that shares no link and no dependency with a set of flows leaves their completion times and
+    bottlenecks BIT-identical, however many extra events it inserts into the clock."""
+    d = single(n_hosts=2, gph=8)
+    # group A: contended traffic among GPUs 0..3 and 8..11 (NVLink + NIC links of those GPUs only)
+    src_a = [0, 1, 2, 3, 0, 1, 8, 9, 10, 0]
+    dst_a = [8, 8, 8, 9, 1, 2, 0, 0, 1, 3]
+    by_a = [3e6, 5e6, 7e6, 1.1e7, 2e6, 9e6, 4e6, 6e6, 1.3e7, 1e6]
+    # group B: GPUs 4..7 and 12..15 only
+    rng = np.random.default_rng(5)
+    src_b = rng.integers(4, 8, 40); dst_b = rng.integers(12, 16, 40)
+    by_b = np.floor(rng.uniform(1e5, 2e7, 40))
+    a = run_flows(d, src_a, dst_a, by_a)
+    ab = run_flows(d, list(src_a) + list(src_b), list(dst_a) + list(dst_b), list(by_a) + list(by_b))
+    n = len(src_a)
+    assert len(ab.event_log()) > len(a.event_log()) + 20           # B really interleaves its own events
+    assert np.array_equal(ab.completion_times()[:n], a.completion_times())
+    assert np.array_equal(ab.bottlenecks()[:n], a.bottlenecks())
+
+
 def test_p9_single_spine_is_seed_independent():
     d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=1, uplinks_per_leaf_spine=1)
     ops = [W.Coll(W.ALLREDUCE_RING, np.arange(0, 16, 2, dtype=np.int32), 32 * MiB),
