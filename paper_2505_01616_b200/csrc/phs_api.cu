@@ -383,6 +383,22 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       for (int64_t f = 0; f < F; ++f)
         for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
     }
+    // static link components (union-find over the links, joined by every flow's path); the representative is
+    // the smallest link id, so component ids are link ids
+    std::vector<int32_t> parent((size_t)L);
+    std::iota(parent.begin(), parent.end(), 0);
+    auto find = [&](int32_t x) {
+      while (parent[x] != x) {
+        parent[x] = parent[parent[x]];
+        x = parent[x];
+      }
+      return x;
+    };
+    for (int64_t f = 0; f < F; ++f)
+      for (uint32_t e = in.path_off[f] + 1; e < in.path_off[f + 1]; ++e) {
+        const int32_t a = find(in.path[in.path_off[f]]), b = find(in.path[e]);
+        if (a != b) parent[std::max(a, b)] = std::min(a, b);
+      }
     FlowRec *r = rec.data() + sim->flow_base[i];
     for (int64_t f = 0; f < F; ++f) {
       FlowRec x;
@@ -391,10 +407,15 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       x.lat = in.lat[f];
       const uint32_t p0 = in.path_off[f], p1 = in.path_off[f + 1];
       for (int h = 0; h < kMaxHops; ++h) x.path[h] = p0 + h < p1 ? in.path[p0 + h] : -1;
-      x.succ_off = soff[f];
       x.succ_cnt = (int32_t)(soff[f + 1] - soff[f]);
-      x.succ_in[0] = x.succ_cnt > 0 ? sdst[soff[f]] : -1;
-      x.succ_in[1] = x.succ_cnt > 1 ? sdst[soff[f] + 1] : -1;
+      if (x.succ_cnt <= 2) {
+        x.succ_in[0] = x.succ_cnt > 0 ? sdst[soff[f]] : -1;
+        x.succ_in[1] = x.succ_cnt > 1 ? sdst[soff[f] + 1] : -1;
+      } else {
+        x.succ_in[0] = (int32_t)soff[f];
+        x.succ_in[1] = -1;
+      }
+      x.comp = p0 < p1 ? find(in.path[p0]) : 0;
       r[f] = x;
       const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
       pc0[sim->flow_base[i] + f] = np;

@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   int *a_path = p_flow1 + Fs;
   double *a_rem = SC.f64 + (size_t)region * cluster_f64_per_region(Fs);
   double *p_tact0 = a_rem + Fs, *p_tact1 = p_tact0 + Fs;
+  double *a_tl = p_tact1 + Fs, *a_tc = a_tl + Fs;  // R-LZ: time of the last rate change, completion time
   unsigned char *dirty = SC.u8 + (size_t)region * L;
   unsigned long long *ctrl64 = SC.ctrl + (size_t)region * 64;
   int *ctl = (int *)ctrl64;
@@ -133,6 +134,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           const FlowRec r = rec[f];
           a_flow[slot] = f;
           a_rem[slot] = r.bytes;
+          a_rq[slot] = -1;  // no rate yet
+          a_tc[slot] = kInf;
           a_bn[slot] = -1;
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
@@ -253,8 +256,19 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
             const int arg = a_arg[s];
             if (cnt[arg] == nsnap[arg]) {
               const long long rq = share[arg];
-              a_rq[s] = rq;
+              const long long old = a_rq[s];
               a_bn[s] = arg;
+              if (rq != old) {  // R-LZ: only a changed rate touches the flow: settle, then a new completion time
+                double rem = a_rem[s];
+                if (old >= 0) {
+                  rem = __dsub_rn(rem, __dmul_rn(rate_of(old), __dsub_rn(now, a_tl[s])));
+                  rem = rem > 0.0 ? rem : 0.0;
+                  a_rem[s] = rem;
+                }
+                a_tl[s] = now;
+                a_rq[s] = rq;
+                a_tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));
+              }
 #pragma unroll
               for (int h = 0; h < kMaxHops; ++h) {
                 const int l = a_path[(size_t)s * kMaxHops + h];
@@ -263,7 +277,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
                 atomicSub(&nl[l], 1);
                 dirty[l] = 1;
               }
-              mymin = dmin(mymin, __dadd_rn(now, __ddiv_rn(a_rem[s], rate_of(rq))));
+              mymin = dmin(mymin, a_tc[s]);
               if (LOG && leader[arg] == s) atomicAdd(&ctl[K_EV_ROUNDS], 1);
             } else {
               mine_left = true;
@@ -291,7 +305,6 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       }
       // ======== next time (a8)
       const double t_next = __longlong_as_double((long long)*(volatile unsigned long long *)&ctrl64[Q_TMIN0 + par]);
-      const double dt = __dsub_rn(t_next, now);
       int first_bneck = -1;
       if (LOG && ctid == 0 && nA > 0) {
         long long bk = LLONG_MAX;
@@ -310,10 +323,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         if (f < 0) continue;
         const long long rq = a_rq[s];
         const int bn = a_bn[s];
-        const double rate = rate_of(rq);
-        const double rem = a_rem[s];
-        const double tc = __dadd_rn(now, __ddiv_rn(rem, rate));
-        const bool done = tc == t_next;
+        const bool done = a_tc[s] == t_next;
         cnt0[bn] = 0;
         cnt1[bn] = 0;
         if (LOG) leader[bn] = INT_MAX;
@@ -334,9 +344,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           atomicSub(&ctl[K_NACTIVE], 1);
           atomicAdd(&ctl[K_DONE], 1);
           if (LOG) atomicAdd(&ctl[K_EV_NCOMP], 1);
-          const uint32_t e0 = rec[f].succ_off, e1 = e0 + (uint32_t)rec[f].succ_cnt;
-          for (uint32_t e = e0; e < e1; ++e) {
-            const int g = succ[e];
+          const int nsucc = rec[f].succ_cnt;
+          const int s0 = rec[f].succ_in[0], s1 = rec[f].succ_in[1];
+          for (int e = 0; e < nsucc; ++e) {
+            const int g = nsucc <= 2 ? (e == 0 ? s0 : s1) : succ[s0 + e];
             if (atomicSub(&pred_cnt[g], 1) == 1) {
               const FlowRec r = rec[g];
               const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
@@ -345,9 +356,6 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
               pt_oth[i] = ta;
             }
           }
-        } else {
-          const double r2 = __dsub_rn(rem, __dmul_rn(rate, dt));
-          a_rem[s] = r2 > 0.0 ? r2 : 0.0;
         }
       }
       if (ctid == 0) {

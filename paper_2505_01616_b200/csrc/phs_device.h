@@ -43,14 +43,14 @@ struct ClusterScratch {
   int64_t *i64;   // per region: cap_rem[L], share[L], a_rq[Fs]
   int32_t *i32;   // per region: n, nsnap, cnt0, cnt1, leader [L each]; a_flow, a_bn, a_arg, free_stack, p_flow0,
                   //             p_flow1 [Fs each]; a_path [kMaxHops * Fs]
-  double *f64;    // per region: a_rem, p_tact0, p_tact1 [Fs each]
+  double *f64;    // per region: a_rem, p_tact0, p_tact1, a_tl, a_tc [Fs each]
   uint8_t *u8;    // per region: dirty[L]
   unsigned long long *ctrl;  // per region: 64 words of control state
   int64_t Fs;     // slot capacity of a region (>= flows of the largest instance on this path)
 };
 __host__ __device__ inline size_t cluster_i64_per_region(int L, int64_t Fs) { return (size_t)(2 * (int64_t)L + Fs); }
 __host__ __device__ inline size_t cluster_i32_per_region(int L, int64_t Fs) { return (size_t)(5 * (int64_t)L + (6 + kMaxHops) * Fs); }
-__host__ __device__ inline size_t cluster_f64_per_region(int64_t Fs) { return (size_t)(3 * Fs); }
+__host__ __device__ inline size_t cluster_f64_per_region(int64_t Fs) { return (size_t)(5 * Fs); }
 constexpr int kClusterThreads = 1024;
 // Largest cluster size (<= want) that can be co-scheduled, and how many such clusters fit on the device at once.
 cudaError_t cluster_path_limits(int want, int *cluster_size, int *max_clusters);

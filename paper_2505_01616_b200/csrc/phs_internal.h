@@ -15,16 +15,19 @@ constexpr int kMaxHops = 6;  // longest path: fat tree cross-pod (S2)
 
 // Device-resident flow record, 64 bytes (half a cache line), one per flow.  Everything activation and release
 // need sits in the one record, so each costs a single (non-chained) global load: size, timing, the path inline
-// (ECMP paths have at most kMaxHops links, -1 padded) and the first two successors inline (a ring flow has at
-// most two; longer lists spill to succ[] at succ_off).
+// (ECMP paths have at most kMaxHops links, -1 padded), the successors and the flow's static link component.
+// Successors: a ring flow has at most two, held inline; a longer list lives in succ[] and succ_in[0] is its
+// offset into the instance's slice of succ[].
 struct FlowRec {
   double bytes;          // flow size
   double start;          // earliest submission time (S4)
   double lat;            // path latency, left-to-right sum over the path's links (S2)
   int32_t path[kMaxHops];  // flow -> link incidence row
-  uint32_t succ_off;     // into the instance's slice of succ[] (all successors, including the inline two)
   int32_t succ_cnt;      // number of successors
-  int32_t succ_in[2];    // first two successors (instance-relative flow ids), -1 if absent
+  int32_t succ_in[2];    // succ_cnt <= 2: the successors (instance-relative flow ids, -1 if absent);
+                         // succ_cnt > 2: succ_in[0] = offset of the list in succ[]
+  int32_t comp;          // static link component of the flow's path = smallest link id of the component:
+                         // two links are in one component iff some chain of flows of the instance connects them
 };
 static_assert(sizeof(FlowRec) == 64, "FlowRec must be 64 bytes");
 

@@ -2,16 +2,23 @@
 // share per link, bottleneck argmin, freeze/scatter), event advance, retire + DAG release.
 // a4-a9.  One CTA simulates one instance start to finish with ALL dynamic state in shared memory.
 //
-// Algorithm: the paper's water-filling freezes ONE bottleneck link per iteration (PAPER.md
+// Algorithm.  The paper's water-filling freezes ONE bottleneck link per iteration (PAPER.md
 // L165).  Because rates live on an exact integer grid (reading R-FX), freezing EVERY link whose (share, id) key is
 // smaller than the key of every link it shares an unfrozen flow with ("local minimum") in one parallel round gives
-// bit-identical rates, bottleneck ids and iteration count (proof in DESIGN.md).  A link is a local minimum iff every
-// unfrozen flow on it names it as the arg-min link of its own path: count the votes per link and compare with the
-// number of unfrozen flows on the link.  Phases of one event (barrier-separated):
-//   X   advance all active flows to t_next, retire + release successors, activate what is due (a8, a4)
-//   b0  first round: every flow computes the fair share of its own links (a5), votes for its arg-min (a6)
-//   c   links holding all votes freeze their flows; debit paths; fold candidate completion times (a7, a8)
-//   a,b later rounds: recompute the share of debited links (a5), vote again (a6)
+// bit-identical rates and bottleneck ids (proof in DESIGN.md).  A link is a local minimum iff no unfrozen flow on
+// it names another link as the arg-min of its own path: every flow stamps the links it does NOT vote for with the
+// round's number ("beaten"), and freezes if its own arg-min link carries no stamp of this round.  No counters, no
+// atomics, nothing to clear.
+// Rates are a function of the active set of a static link component only, and (reading R-LZ) a flow's state
+// changes only when its own rate changes, so an event re-solves just the components it touched.
+// Phases of one event (barrier-separated):
+//   X   flows whose completion time equals t_next retire and release their successors; slots whose activation
+//       time has come become ACTIVE (a8, a4); both stamp their component "to solve"
+//   V0  every flow of a stamped component refreshes the fair share of its links (a5), picks its arg-min (a6)
+//   F0  flows whose arg-min link is unbeaten freeze at its share (a7); a changed rate settles the flow's
+//       remaining bytes and gives a new completion time; all threads fold the slot times into the next t_next (a8)
+//   I/D/V/F  only when flows are left: working capacities are set up, frozen flows debit their paths, and the
+//       rounds repeat on the debited shares
 #include <cuda_runtime.h>
 
 #include <climits>
@@ -25,27 +32,34 @@ namespace {
 
 // ------------------------------------------------------------------------------------------------ smem layout
 struct CtaSmem {
-  long long *cap_rem, *share;      // [L]
-  int *n, *nsnap, *cnt0, *cnt1;    // [L]
-  int *leader;                     // [L] (event log only)
-  unsigned char *dirty;            // [L]
-  double *s_rem;                   // [S] remaining bytes
-  long long *s_rq;                 // [S] rate in quanta
-  int *s_flow, *s_bn, *s_arg;      // [S]
-  int *s_path;                     // [S * kMaxHops]
-  unsigned *s_succ_off;            // [S]
-  int *s_succ_cnt, *s_succ0, *s_succ1;  // [S]
-  int *free_q;                     // [S] FIFO of free slots
-  double *p_time0, *p_time1;       // [S] pending lists (double buffered): activation time
-  int *p_flow0, *p_flow1;          // [S]
-  unsigned *pc8;                   // [(PCF+3)/4] predecessor counters, one byte per flow
-  double *red;                     // [32] per-warp partial minima
-  long long *red_key;              // [32] per-warp partial (share) for first_bneck
-  int *red_id;                     // [32]
-  int *ctl;                        // [32] control words
+  // per link [L]
+  long long *l_cap, *l_share0, *l_caprem, *l_sharew;
+  int *l_n0;      // ACTIVE flows on the link
+  int *l_chg;     // solve id of the last change of l_n0 (share0 is stale for that solve until recomputed)
+  int *l_beat;    // round number in which some unfrozen flow on the link voted for another link
+  int *l_nw;      // working: unfrozen flows on the link (rounds >= 1)
+  int *l_deb;     // working: round number of the last debit
+  int *l_solve;   // per component (indexed by its representative link): id of the solve that must redo it
+  int *l_won;     // LOG: round in which the link froze flows (counts bottleneck links once)
+  // per slot [S]: one slot per PENDING or ACTIVE flow
+  double *s_tc;   // PENDING: activation time; ACTIVE: completion time; free: +inf
+  double *s_rem;  // remaining bytes at time s_tl
+  double *s_tl;   // time of the last rate change
+  long long *s_rq;  // rate in quanta, -1 before the first solve
+  int *s_flow;    // flow id, -1 = free
+  int *s_bn;      // -2 PENDING, -1 ACTIVE and unfrozen, >= 0 bottleneck link
+  int *s_comp, *s_arg;
+  int *s_path;    // [S * kMaxHops]
+  int *s_succ_cnt, *s_succ0, *s_succ1;
+  int *free_q;    // FIFO ring of free slots
+  unsigned *pc8;  // [(PCF+3)/4] predecessor counters, one byte per flow
+  double *red;    // [32] per-warp partial minima
+  long long *red_key;  // [32] LOG: per-warp partial first_bneck key
+  int *red_id;    // [32]
+  int *ctl;       // [32] control words
 };
 enum {
-  C_HI = 0, C_QHEAD, C_QTAIL, C_NP0, C_NP1, C_NACTIVE, C_OVERFLOW, C_DONE, C_EV_NCOMP, C_EV_ROUNDS, C_EV_NACT0,
+  C_HI = 0, C_QHEAD, C_QTAIL, C_NACTIVE, C_NPEND, C_OVERFLOW, C_DONE, C_EV_NCOMP, C_EV_ROUNDS, C_EV_NACT0,
   C_EV_NACT1, C_NCTL
 };
 
@@ -57,36 +71,57 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   a = o;                                                \
   o = align_up(o + sizeof(type) * (size_t)(count), 16); \
   if (s) s->field = (type *)(base + a);
-  PHS_TAKE(cap_rem, long long, L)
-  PHS_TAKE(share, long long, L)
+  PHS_TAKE(l_cap, long long, L)
+  PHS_TAKE(l_share0, long long, L)
+  PHS_TAKE(l_caprem, long long, L)
+  PHS_TAKE(l_sharew, long long, L)
+  PHS_TAKE(s_tc, double, S)
   PHS_TAKE(s_rem, double, S)
+  PHS_TAKE(s_tl, double, S)
   PHS_TAKE(s_rq, long long, S)
-  PHS_TAKE(p_time0, double, S)
-  PHS_TAKE(p_time1, double, S)
   PHS_TAKE(red, double, 32)
   PHS_TAKE(red_key, long long, 32)
-  PHS_TAKE(n, int, L)
-  PHS_TAKE(nsnap, int, L)
-  PHS_TAKE(cnt0, int, L)
-  PHS_TAKE(cnt1, int, L)
-  PHS_TAKE(leader, int, log ? L : 0)
+  PHS_TAKE(l_n0, int, L)
+  PHS_TAKE(l_chg, int, L)
+  PHS_TAKE(l_beat, int, L)
+  PHS_TAKE(l_nw, int, L)
+  PHS_TAKE(l_deb, int, L)
+  PHS_TAKE(l_solve, int, L)
+  PHS_TAKE(l_won, int, log ? L : 0)
   PHS_TAKE(s_flow, int, S)
   PHS_TAKE(s_bn, int, S)
+  PHS_TAKE(s_comp, int, S)
   PHS_TAKE(s_arg, int, S)
   PHS_TAKE(s_path, int, S * kMaxHops)
-  PHS_TAKE(s_succ_off, unsigned, S)
   PHS_TAKE(s_succ_cnt, int, S)
   PHS_TAKE(s_succ0, int, S)
   PHS_TAKE(s_succ1, int, S)
   PHS_TAKE(free_q, int, S)
-  PHS_TAKE(p_flow0, int, S)
-  PHS_TAKE(p_flow1, int, S)
   PHS_TAKE(pc8, unsigned, (pcf + 3) / 4)
   PHS_TAKE(red_id, int, 32)
   PHS_TAKE(ctl, int, 32)
-  PHS_TAKE(dirty, unsigned char, L)
 #undef PHS_TAKE
   return o;
+}
+
+// 64-bit add on a shared-memory word with two native 32-bit atomics (a 64-bit atomicAdd on shared memory compiles
+// to a compare-and-swap loop).  Exact once all adds of a phase have completed: every carry out of the low word is
+// added to the high word exactly once.
+__device__ __forceinline__ void smem_add64(long long *p, long long v) {
+  unsigned *w = (unsigned *)p;
+  const unsigned lo = (unsigned)(unsigned long long)v, hi = (unsigned)((unsigned long long)v >> 32);
+  const unsigned old = atomicAdd(w, lo);
+  const unsigned carry = (old + lo) < old ? 1u : 0u;
+  if (hi + carry) atomicAdd(w + 1, hi + carry);
+}
+
+// min over the warp of non-negative doubles (their bit patterns order like unsigned integers): two REDUX steps
+__device__ __forceinline__ double warp_min_nonneg(double v) {
+  const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+  const unsigned hi = (unsigned)(b >> 32), lo = (unsigned)b;
+  const unsigned mhi = __reduce_min_sync(0xffffffffu, hi);
+  const unsigned mlo = __reduce_min_sync(0xffffffffu, hi == mhi ? lo : 0xffffffffu);
+  return __longlong_as_double((long long)(((unsigned long long)mhi << 32) | mlo));
 }
 
 }  // namespace
@@ -96,7 +131,8 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
 }
 
 // ================================================================================================ CTA kernel
-// NT threads; LOG: write the event log; PCS: predecessor counters live in shared memory (one byte per flow).
+// NT threads; LOG: write the event log (and solve every component at every event, so that the log's iteration
+// count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory.
 template <int NT, bool LOG, bool PCS>
 __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
                                                      int *ticket, int SC, int pcf) {
@@ -126,18 +162,19 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
-    // ---- init: link state = full capacity, nothing active; flows without predecessors become PENDING (S4)
+    // ---- init: nothing active, every slot free
     for (int l = tid; l < L; l += NT) {
-      S.cap_rem[l] = capq[l];
-      S.n[l] = 0;
-      S.cnt0[l] = 0;
-      S.cnt1[l] = 0;
-      if (LOG) S.leader[l] = INT_MAX;
-      S.dirty[l] = 0;
+      S.l_cap[l] = capq[l];
+      S.l_n0[l] = 0;
+      S.l_chg[l] = 0;
+      S.l_beat[l] = 0;
+      S.l_deb[l] = 0;
+      S.l_solve[l] = 0;
+      if (LOG) S.l_won[l] = 0;
     }
     for (int s = tid; s < SC; s += NT) {
       S.s_flow[s] = -1;
-      S.s_bn[s] = -1;
+      S.s_tc[s] = kInf;
     }
     if (tid < C_NCTL) S.ctl[tid] = 0;
     if (PCS) {
@@ -145,6 +182,22 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
       for (int w = tid; w < (F + 3) / 4; w += NT) S.pc8[w] = src[w];
     }
     __syncthreads();
+
+    // one slot per flow that is PENDING or ACTIVE; the whole record is staged when the flow becomes PENDING
+    auto fill_slot = [&](int slot, int f, const FlowRec &r, double ta) {
+      S.s_flow[slot] = f;
+      S.s_rem[slot] = r.bytes;
+      S.s_bn[slot] = -2;
+      S.s_comp[slot] = r.comp;
+#pragma unroll
+      for (int h = 0; h < kMaxHops; ++h) S.s_path[slot * kMaxHops + h] = r.path[h];
+      S.s_succ_cnt[slot] = r.succ_cnt;
+      S.s_succ0[slot] = r.succ_in[0];
+      S.s_succ1[slot] = r.succ_in[1];
+      S.s_tc[slot] = ta;
+    };
+
+    // S4: flows without predecessors become PENDING at t_act = start + Lat
     {
       const int32_t *__restrict__ pc0 = T.pred_cnt0 + D.flow_base;
       for (int f = tid; f < F; f += NT) {
@@ -156,11 +209,11 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
           pred_cnt[f] = pc;
         }
         if (pc == 0) {
-          const double st = rec[f].start, la = rec[f].lat;
-          const int i = atomicAdd(&S.ctl[C_NP0], 1);
-          if (i < SC) {
-            S.p_flow0[i] = f;
-            S.p_time0[i] = __dadd_rn(st, la);
+          const FlowRec r = rec[f];
+          const int slot = atomicAdd(&S.ctl[C_HI], 1);
+          if (slot < SC) {
+            fill_slot(slot, f, r, __dadd_rn(r.start, r.lat));
+            atomicAdd(&S.ctl[C_NPEND], 1);
           } else {
             S.ctl[C_OVERFLOW] = 1;
           }
@@ -170,134 +223,102 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
     __syncthreads();
 
     double now = 0.0, t_next = 0.0;
-    int cur = 0;   // which pending buffer is live
-    int ev = -1;   // index of the event whose advance phase X is about to execute
+    int ev = -1;      // index of the event whose advance phase X is about to execute
+    int solve = 0;    // id of the solve that follows the current phase X
+    int g = 0;        // filling-round number, unique over the instance
     long long sum_active = 0, sum_rounds = 0;
     int max_active = 0, max_pending = 0;
     int status = PHS_OK;
     int first_bneck = -1;
 
     for (;;) {
-      // ======== phase X (a8 + a4): advance to t_next, retire, release successors, activate what is due
-      const double dt = __dsub_rn(t_next, now);
-      const int hi0 = S.ctl[C_HI];
+      // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
+      ++solve;
+      const int hi0 = min(S.ctl[C_HI], SC);
       const int qtail = S.ctl[C_QTAIL];
-      const int nP = min(S.ctl[C_NP0 + cur], SC);
-      int *const pf_cur = cur ? S.p_flow1 : S.p_flow0, *const pf_oth = cur ? S.p_flow0 : S.p_flow1;
-      double *const pt_cur = cur ? S.p_time1 : S.p_time0, *const pt_oth = cur ? S.p_time0 : S.p_time1;
-      int *const np_oth = &S.ctl[C_NP0 + (cur ^ 1)];
-      double mymin = kInf;  // running min: pending activation times, and tc of my flows once frozen
 
-      auto activate = [&](int f, const FlowRec &r) {
+      auto activate = [&](int slot) {  // PENDING -> ACTIVE: the flow now counts on its links
+#pragma unroll
+        for (int h = 0; h < kMaxHops; ++h) {
+          const int l = S.s_path[slot * kMaxHops + h];
+          if (l < 0) break;
+          atomicAdd(&S.l_n0[l], 1);
+          S.l_chg[l] = solve;
+        }
+        S.l_solve[S.s_comp[slot]] = solve;
+        S.s_rq[slot] = -1;
+        S.s_bn[slot] = -1;
+        S.s_tc[slot] = kInf;
+        atomicAdd(&S.ctl[C_NACTIVE], 1);
+        atomicSub(&S.ctl[C_NPEND], 1);
+        if (LOG) atomicAdd(&S.ctl[C_EV_NACT0 + ((ev + 1) & 1)], 1);
+        // the successors' records will be needed when this flow completes: pull them towards L2 now
+        const int nsucc = S.s_succ_cnt[slot];
+        if (nsucc > 0 && nsucc <= 2) {
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.s_succ0[slot]));
+          if (nsucc > 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.s_succ1[slot]));
+        }
+      };
+      auto release = [&](int gf) {  // S4.5: pred_cnt--, at 0 -> PENDING with t_act = max(start, now) + Lat
+        bool zero;
+        if (PCS) {
+          const unsigned sh = (unsigned)(gf & 3) * 8u;
+          const unsigned old = atomicSub(&S.pc8[gf >> 2], 1u << sh);
+          zero = ((old >> sh) & 0xffu) == 1u;
+        } else {
+          zero = atomicSub(&pred_cnt[gf], 1) == 1;
+        }
+        if (!zero) return;
+        const FlowRec r = rec[gf];
+        const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
         const int h = atomicAdd(&S.ctl[C_QHEAD], 1);
         const int slot = h < qtail ? S.free_q[h % SC] : atomicAdd(&S.ctl[C_HI], 1);
         if (slot >= SC) {
           S.ctl[C_OVERFLOW] = 1;
           return;
         }
-        S.s_flow[slot] = f;
-        S.s_rem[slot] = r.bytes;
-#pragma unroll
-        for (int h2 = 0; h2 < kMaxHops; ++h2) {
-          const int l = r.path[h2];
-          if (l >= 0) atomicAdd(&S.n[l], 1);
-          S.s_path[slot * kMaxHops + h2] = l;
-        }
-        S.s_succ_off[slot] = r.succ_off;
-        S.s_succ_cnt[slot] = r.succ_cnt;
-        S.s_succ0[slot] = r.succ_in[0];
-        S.s_succ1[slot] = r.succ_in[1];
-        atomicAdd(&S.ctl[C_NACTIVE], 1);
-        if (LOG) atomicAdd(&S.ctl[C_EV_NACT0 + ((ev + 1) & 1)], 1);
-      };
-      auto release = [&](int g) {  // S4.5: pred_cnt--, at 0 -> t_act = max(start, now) + Lat
-        bool zero;
-        if (PCS) {
-          const unsigned sh = (unsigned)(g & 3) * 8u;
-          const unsigned old = atomicSub(&S.pc8[g >> 2], 1u << sh);
-          zero = ((old >> sh) & 0xffu) == 1u;
-        } else {
-          zero = atomicSub(&pred_cnt[g], 1) == 1;
-        }
-        if (!zero) return;
-        const FlowRec r = rec[g];
-        const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
-        if (ta <= t_next) {
-          activate(g, r);  // zero path latency: due at this very timestamp
-        } else {
-          const int i = atomicAdd(np_oth, 1);
-          if (i < SC) {
-            pf_oth[i] = g;
-            pt_oth[i] = ta;
-          } else {
-            S.ctl[C_OVERFLOW] = 1;
-          }
-          mymin = dmin(mymin, ta);
-        }
+        atomicAdd(&S.ctl[C_NPEND], 1);
+        const bool due = ta <= t_next;  // zero path latency: due at this very timestamp
+        fill_slot(slot, gf, r, due ? kInf : ta);
+        if (due) activate(slot);
       };
 
       for (int s = tid; s < hi0; s += NT) {
-        const int bn = S.s_bn[s];
-        if (bn < 0) continue;  // free, or activated in this very phase
+        if (!(S.s_tc[s] <= t_next)) continue;  // free slots hold +inf
+        if (S.s_bn[s] == -2) {
+          activate(s);
+          continue;
+        }
+        // the flow completes at t_next (bit-equal absolute time, S4.4)
         const int f = S.s_flow[s];
-        const long long rq = S.s_rq[s];
-        const double rate = rate_of(rq);
-        const double rem = S.s_rem[s];
-        const double tc = __dadd_rn(now, __ddiv_rn(rem, rate));
-        const bool done = tc == t_next;  // bit-equal absolute time (S4.4)
-        S.cnt0[bn] = 0;
-        S.cnt1[bn] = 0;
-        if (LOG) S.leader[bn] = INT_MAX;
-        S.s_bn[s] = -1;
-        // undo the solve's debits (exact: integer arithmetic); survivors stay counted on their links
+        t_done[f] = t_next;
+        bneck_out[f] = S.s_bn[s];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
           const int l = S.s_path[s * kMaxHops + h];
           if (l < 0) break;
-          atomicAdd((unsigned long long *)&S.cap_rem[l], (unsigned long long)rq);
-          if (!done) atomicAdd(&S.n[l], 1);
+          atomicSub(&S.l_n0[l], 1);
+          S.l_chg[l] = solve;
         }
-        if (done) {
-          t_done[f] = t_next;
-          bneck_out[f] = bn;
-          S.s_flow[s] = -1;
-          S.free_q[atomicAdd(&S.ctl[C_QTAIL], 1) % SC] = s;
-          atomicSub(&S.ctl[C_NACTIVE], 1);
-          atomicAdd(&S.ctl[C_DONE], 1);
-          if (LOG) atomicAdd(&S.ctl[C_EV_NCOMP], 1);
-          const int nsucc = S.s_succ_cnt[s];
+        S.l_solve[S.s_comp[s]] = solve;
+        S.s_flow[s] = -1;
+        S.s_tc[s] = kInf;
+        S.free_q[atomicAdd(&S.ctl[C_QTAIL], 1) % SC] = s;
+        atomicSub(&S.ctl[C_NACTIVE], 1);
+        atomicAdd(&S.ctl[C_DONE], 1);
+        if (LOG) atomicAdd(&S.ctl[C_EV_NCOMP], 1);
+        const int nsucc = S.s_succ_cnt[s];
+        if (nsucc <= 2) {
           if (nsucc > 0) release(S.s_succ0[s]);
           if (nsucc > 1) release(S.s_succ1[s]);
-          if (nsucc > 2) {
-            const unsigned e0 = S.s_succ_off[s];
-            for (int e = 2; e < nsucc; ++e) release(succ[e0 + e]);
-          }
         } else {
-          const double r2 = __dsub_rn(rem, __dmul_rn(rate, dt));  // mul, then sub, then clamp
-          S.s_rem[s] = r2 > 0.0 ? r2 : 0.0;
-        }
-      }
-      for (int i = tid; i < nP; i += NT) {  // a4: PENDING flows whose activation time has come
-        const int f = pf_cur[i];
-        const double ta = pt_cur[i];
-        if (ta <= t_next) {
-          const FlowRec r = rec[f];
-          activate(f, r);
-        } else {
-          const int j = atomicAdd(np_oth, 1);
-          if (j < SC) {
-            pf_oth[j] = f;
-            pt_oth[j] = ta;
-          } else {
-            S.ctl[C_OVERFLOW] = 1;
-          }
-          mymin = dmin(mymin, ta);
+          const int e0 = S.s_succ0[s];
+          for (int e = 0; e < nsucc; ++e) release(succ[e0 + e]);
         }
       }
       __syncthreads();
       now = t_next;
       if (tid == 0) {
-        S.ctl[C_NP0 + cur] = 0;
         if (S.ctl[C_QHEAD] > qtail) S.ctl[C_QHEAD] = qtail;  // pops that found the queue empty took fresh slots
         if (LOG) {
           if (log && ev >= 0) {  // O4: the event that just finished
@@ -315,125 +336,203 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         }
       }
       ++ev;
-      cur ^= 1;
       if (S.ctl[C_OVERFLOW]) {
         status = kOverflow;
         break;
       }
       const int nA = S.ctl[C_NACTIVE];
-      const int nPend = S.ctl[C_NP0 + cur];
+      const int nPend = S.ctl[C_NPEND];
       if (nA == 0 && nPend == 0) break;  // S4.3: nothing active, nothing pending -> stop
-      const int hi = S.ctl[C_HI];
+      const int hi = min(S.ctl[C_HI], SC);
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 
-      // ======== rates: parallel progressive filling over the active set (a5-a7), tc folded in (a8)
-      int round = 0;
-      bool left = nA > 0;
-      for (;;) {
-        if (left) {
-          int *cnt = (round & 1) ? S.cnt1 : S.cnt0;
-          int *cnt_prev = (round & 1) ? S.cnt0 : S.cnt1;
-          if (round > 0) {
-            // (a) fair share of every link debited in the previous round
-            for (int l = tid; l < L; l += NT) {
-              if (S.dirty[l]) {
-                S.dirty[l] = 0;
-                const int nl = S.n[l];
-                S.nsnap[l] = nl;
-                if (nl > 0) S.share[l] = fair_share(S.cap_rem[l], nl);
-              }
-            }
-            __syncthreads();
+      // ======== rates (a5-a7): parallel progressive filling over the components this event touched
+      auto in_solve = [&](int s) {  // ACTIVE flow of a component that must be re-solved
+        if (S.s_flow[s] < 0 || S.s_bn[s] == -2) return false;
+        return LOG || S.l_solve[S.s_comp[s]] == solve;
+      };
+      auto freeze = [&](int s, int arg, long long rq) {  // a7; R-LZ: only a changed rate touches the flow's state
+        S.s_bn[s] = arg;
+        const long long old = S.s_rq[s];
+        if (rq != old) {
+          double rem = S.s_rem[s];
+          if (old >= 0) {  // settle at the old rate: mul, sub, clamp
+            rem = __dsub_rn(rem, __dmul_rn(rate_of(old), __dsub_rn(now, S.s_tl[s])));
+            rem = rem > 0.0 ? rem : 0.0;
+            S.s_rem[s] = rem;
           }
-          // (b) every unfrozen flow votes for the arg-min (share, id) link of its path.  In the first round the
-          // flow computes the shares of its own links itself (cap_rem = capacity, n is final after phase X) and
-          // publishes them, which saves the link pass and its barrier.
-          long long bk = LLONG_MAX;
-          int bl = INT_MAX;
+          S.s_tl[s] = now;
+          S.s_rq[s] = rq;
+          S.s_tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));  // S4.3: division, then addition
+        }
+        if (LOG && atomicExch(&S.l_won[arg], g) != g) atomicAdd(&S.ctl[C_EV_ROUNDS], 1);
+      };
+      int rounds = 1;
+      ++g;
+      {  // ---- V0: fair share of the links whose flow count changed (a5), arg-min link of every flow (a6)
+        long long bk = LLONG_MAX;
+        int bl = INT_MAX;
+        for (int s = tid; s < hi; s += NT) {
+          if (!in_solve(s)) continue;
+          S.s_bn[s] = -1;
+          int p[kMaxHops];
+          long long best = LLONG_MAX;
+          int arg = -1;
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = p[h] = S.s_path[s * kMaxHops + h];
+            if (l < 0) continue;
+            long long sh;
+            if (S.l_chg[l] == solve) {
+              sh = fair_share(S.l_cap[l], S.l_n0[l]);
+              S.l_share0[l] = sh;  // every flow on the link stores the same value
+            } else {
+              sh = S.l_share0[l];
+            }
+            if (sh < best || (sh == best && l < arg)) {
+              best = sh;
+              arg = l;
+            }
+          }
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h)
+            if (p[h] >= 0 && p[h] != arg) S.l_beat[p[h]] = g;  // an unfrozen flow on p[h] prefers another link
+          S.s_arg[s] = arg;
+          if (LOG && (best < bk || (best == bk && arg < bl))) {
+            bk = best;
+            bl = arg;
+          }
+        }
+        if (LOG) {  // O4 first_bneck = global arg-min = min over the flows' arg-mins
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) {
+            const long long ok = __shfl_xor_sync(0xffffffffu, bk, o);
+            const int ol = __shfl_xor_sync(0xffffffffu, bl, o);
+            if (ok < bk || (ok == bk && ol < bl)) {
+              bk = ok;
+              bl = ol;
+            }
+          }
+          if (lane == 0) {
+            S.red_key[warp] = bk;
+            S.red_id[warp] = bl;
+          }
+        }
+      }
+      __syncthreads();
+      bool left = false;
+      {  // ---- F0: unbeaten arg-min links freeze their flows (a7); fold the slot times (a8)
+        double mymin = kInf;
+        for (int s = tid; s < hi; s += NT) {
+          if (S.s_flow[s] < 0) continue;
+          if (S.s_bn[s] == -1) {
+            const int arg = S.s_arg[s];
+            if (S.l_beat[arg] != g)
+              freeze(s, arg, S.l_share0[arg]);
+            else
+              left = true;
+          }
+          mymin = dmin(mymin, S.s_tc[s]);
+        }
+        const double wm = warp_min_nonneg(mymin);
+        if (lane == 0) S.red[warp] = wm;
+      }
+      left = __syncthreads_or(left);
+      if (left) {
+        // ---- I: working capacities of the links of this solve (idempotent stores)
+        for (int s = tid; s < hi; s += NT) {
+          if (!in_solve(s)) continue;
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = S.s_path[s * kMaxHops + h];
+            if (l < 0) break;
+            S.l_caprem[l] = S.l_cap[l];
+            S.l_nw[l] = S.l_n0[l];
+            S.l_sharew[l] = S.l_share0[l];
+          }
+        }
+        __syncthreads();
+        // ---- D: flows frozen in the first round debit their paths (a7)
+        for (int s = tid; s < hi; s += NT) {
+          if (!in_solve(s) || S.s_bn[s] < 0) continue;
+          const long long rq = S.s_rq[s];
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = S.s_path[s * kMaxHops + h];
+            if (l < 0) break;
+            if (S.l_n0[l] > 1) {
+              smem_add64(&S.l_caprem[l], -rq);
+              atomicSub(&S.l_nw[l], 1);
+              S.l_deb[l] = g;
+            }
+          }
+        }
+        __syncthreads();
+        for (;;) {
+          ++g;
+          ++rounds;
+          // ---- V: shares of the links debited in the previous round, arg-min of every unfrozen flow
           for (int s = tid; s < hi; s += NT) {
-            if (S.s_flow[s] < 0 || S.s_bn[s] >= 0) continue;
-            if (round > 0) cnt_prev[S.s_arg[s]] = 0;
+            if (S.s_flow[s] < 0 || S.s_bn[s] != -1) continue;
+            int p[kMaxHops];
             long long best = LLONG_MAX;
             int arg = -1;
 #pragma unroll
             for (int h = 0; h < kMaxHops; ++h) {
-              const int l = S.s_path[s * kMaxHops + h];
-              if (l < 0) break;
+              const int l = p[h] = S.s_path[s * kMaxHops + h];
+              if (l < 0) continue;
               long long sh;
-              if (round == 0) {
-                const int nl = S.n[l];
-                sh = fair_share(S.cap_rem[l], nl);
-                S.share[l] = sh;
-                S.nsnap[l] = nl;
+              if (S.l_deb[l] == g - 1) {
+                sh = fair_share(S.l_caprem[l], S.l_nw[l]);
+                S.l_sharew[l] = sh;
               } else {
-                sh = S.share[l];
+                sh = S.l_sharew[l];
               }
               if (sh < best || (sh == best && l < arg)) {
                 best = sh;
                 arg = l;
               }
             }
-            S.s_arg[s] = arg;
-            atomicAdd(&cnt[arg], 1);
-            if (LOG) {
-              atomicMin(&S.leader[arg], s);
-              if (best < bk || (best == bk && arg < bl)) {
-                bk = best;
-                bl = arg;
-              }
-            }
-          }
-          if (LOG && round == 0) {  // O4 first_bneck = global arg-min = min over the flows' arg-mins
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-              const long long ok = __shfl_xor_sync(0xffffffffu, bk, o);
-              const int ol = __shfl_xor_sync(0xffffffffu, bl, o);
-              if (ok < bk || (ok == bk && ol < bl)) {
-                bk = ok;
-                bl = ol;
-              }
-            }
-            if (lane == 0) {
-              S.red_key[warp] = bk;
-              S.red_id[warp] = bl;
-            }
+            for (int h = 0; h < kMaxHops; ++h)
+              if (p[h] >= 0 && p[h] != arg) S.l_beat[p[h]] = g;
+            S.s_arg[s] = arg;
           }
           __syncthreads();
-          // (c) a link that collected the votes of ALL its unfrozen flows is a bottleneck: freeze them, debit paths
-          bool mine_left = false;
+          // ---- F: freeze, debit, fold
+          left = false;
+          double mymin = kInf;
           for (int s = tid; s < hi; s += NT) {
-            if (S.s_flow[s] < 0 || S.s_bn[s] >= 0) continue;
-            const int arg = S.s_arg[s];
-            if (cnt[arg] == S.nsnap[arg]) {
-              const long long rq = S.share[arg];
-              S.s_rq[s] = rq;
-              S.s_bn[s] = arg;
+            if (S.s_flow[s] < 0) continue;
+            if (S.s_bn[s] == -1) {
+              const int arg = S.s_arg[s];
+              if (S.l_beat[arg] != g) {
+                const long long rq = S.l_sharew[arg];
+                freeze(s, arg, rq);
 #pragma unroll
-              for (int h = 0; h < kMaxHops; ++h) {
-                const int l = S.s_path[s * kMaxHops + h];
-                if (l < 0) break;
-                atomicAdd((unsigned long long *)&S.cap_rem[l], (unsigned long long)(-rq));
-                atomicSub(&S.n[l], 1);
-                S.dirty[l] = 1;
+                for (int h = 0; h < kMaxHops; ++h) {
+                  const int l = S.s_path[s * kMaxHops + h];
+                  if (l < 0) break;
+                  if (S.l_n0[l] > 1) {
+                    smem_add64(&S.l_caprem[l], -rq);
+                    atomicSub(&S.l_nw[l], 1);
+                    S.l_deb[l] = g;
+                  }
+                }
+              } else {
+                left = true;
               }
-              // S4.3: candidate completion time, division then addition
-              mymin = dmin(mymin, __dadd_rn(now, __ddiv_rn(S.s_rem[s], rate_of(rq))));
-              if (LOG && S.leader[arg] == s) atomicAdd(&S.ctl[C_EV_ROUNDS], 1);
-            } else {
-              mine_left = true;
-              if (LOG) S.leader[arg] = INT_MAX;
             }
+            mymin = dmin(mymin, S.s_tc[s]);
           }
-          left = mine_left;
-          ++round;
+          const double wm = warp_min_nonneg(mymin);
+          if (lane == 0) S.red[warp] = wm;
+          left = __syncthreads_or(left);
+          if (!left) break;
         }
-        const double wm = warp_min(mymin);
-        if (lane == 0) S.red[warp] = wm;
-        left = __syncthreads_or(left);
-        if (!left) break;
       }
-      // ======== next time (a8): t_next = min over candidate completion times and pending activations
+      // ======== next time (a8): t_next = min over completion times and pending activation times
       t_next = S.red[0];
 #pragma unroll
       for (int w = 1; w < NW; ++w) t_next = dmin(t_next, S.red[w]);
@@ -450,7 +549,7 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         }
       }
       sum_active += nA;
-      sum_rounds += round;
+      sum_rounds += rounds;
     }
     if (tid == 0) {
       if (status == PHS_OK && S.ctl[C_DONE] < F) status = PHS_ECYCLE;  // WAITING flows left over
