@@ -38,18 +38,19 @@ def shard_instances(total, rank, world):
     return list(range(lo, lo + per + (1 if rank < extra else 0)))
 
 
-def make_workload(name, n_gpus):
+def make_workload(name, n_gpus, per_gpu=0):
+    """The named BASELINE.json config, `per_gpu` instances per GPU (0 = the config's own batch)."""
     from paper_2505_01616_b200 import workloads as W
     if name == "cfg0":
         return W.cfg0(), 1
     if name == "cfg1":
-        return W.cfg1(batch=64 * n_gpus), 64
+        return W.cfg1(batch=(per_gpu or 64) * n_gpus), per_gpu or 64
     if name == "cfg2":
         return W.cfg2(), 1
     if name == "cfg3":
-        return W.cfg3(batch=4096 * n_gpus), 4096
+        return W.cfg3(batch=(per_gpu or 4096) * n_gpus), per_gpu or 4096
     if name == "cfg4":
-        return W.cfg4(batch=8 * n_gpus), 8
+        return W.cfg4(batch=(per_gpu or 8) * n_gpus), per_gpu or 8
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -175,7 +176,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    w, per_rank = make_workload(args.workload, world)
+    w, per_rank = make_workload(args.workload, world, args.instances)
     mine = shard_instances(w.batch, rank, world)
     first, count = mine[0], len(mine)
     stream = torch.cuda.Stream()
@@ -232,14 +233,15 @@ def run_ours(args, rank, world, local_rank):
         c = s2.counters()
         s2.close()
         return dt, c["h2d_bytes"], out.nbytes + 40 * count
-    e2e_steps = max(1, min(args.steps, 3))
-    e2e_step()
-    barrier()
+    e2e_steps = 0 if args.no_e2e else max(1, min(args.steps, 3))
     e2e_s, h2d, d2h = 0.0, 0, 0
-    for _ in range(e2e_steps):
-        dt, h2d, d2h = e2e_step()
-        e2e_s += dt
-    barrier()
+    if e2e_steps:
+        e2e_step()
+        barrier()
+        for _ in range(e2e_steps):
+            dt, h2d, d2h = e2e_step()
+            e2e_s += dt
+        barrier()
 
     # ---- reduce over ranks: time = max, work = sum
     tot = torch.tensor([ms_total, e2e_s, kern_ms], dtype=torch.float64, device="cuda")
@@ -255,14 +257,15 @@ def run_ours(args, rank, world, local_rank):
         return
 
     value = 2.0 * flows_all * args.steps / (ms_total * 1e-3)
-    e2e_value = 2.0 * flows_all * e2e_steps / e2e_s
+    e2e_value = 2.0 * flows_all * e2e_steps / e2e_s if e2e_steps else None
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64+i64", "data": "synthetic",
         "config": {"workload": args.workload, "instances_per_gpu": count, "flows_per_gpu": flows,
                    "kernel_paths": paths, "l2": "flushed between timed steps (256 MiB write)",
-                   "events_per_step": counters["n_events"], "parallel_rounds_per_step": counters["sum_par_rounds"]},
+                   "events_per_step": counters["n_events"], "parallel_rounds_per_step": counters["sum_par_rounds"],
+                   "max_active_flows": counters["max_active"], "max_state_slots": counters["max_slots"]},
         "collectives_per_sec": colls_all * args.steps / (ms_total * 1e-3),
         "sim_events_per_sec": counters["n_events"] * world * args.steps / (ms_total * 1e-3),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -315,6 +318,9 @@ def main():
     ap.add_argument("--workload", default="cfg1")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end arm (profiling runs)")
+    ap.add_argument("--instances", type=int, default=0,
+                    help="instances per GPU (default: the config's own batch); smaller batches are for profiling")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -79,6 +79,8 @@ typedef struct {
   int64_t sum_par_rounds;/* sum over events of parallel filling rounds executed by the kernels            */
   int64_t n_kernel_launches; /* kernels launched by the last phs_run                                      */
   int64_t h2d_bytes;     /* bytes phs_finalize copied to the device                                       */
+  int32_t max_active;    /* largest number of simultaneously ACTIVE flows in one instance                 */
+  int32_t max_slots;     /* largest number of state slots (PENDING + ACTIVE flows) one instance ever used */
   double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
                          /* the run's stream), excluding the result copies                                */
 } phs_counters;

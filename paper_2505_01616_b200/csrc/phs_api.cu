@@ -85,19 +85,16 @@ struct phs_sim {
   DevBuf<phs_event> d_log;
   DevBuf<int> d_ticket;
   // cluster-path scratch: one region per concurrently running cluster
-  DevBuf<int64_t> g_i64;
-  DevBuf<int32_t> g_i32, d_clist;
-  DevBuf<double> g_f64;
-  DevBuf<uint8_t> g_u8;
-  DevBuf<unsigned long long> g_ctrl;
+  DevBuf<uint8_t> g_scratch;
+  DevBuf<int32_t> d_clist, d_lcomp;
   DevBuf<int> d_cticket;
-  int64_t scratch_Fs = 0;
-  int scratch_regions = 0;
-  bool clist_dirty = true;
+  int64_t scratch_Sc = 0, cluster_scale = 1;
+  int scratch_regions = 0, scratch_cs = 0;
 
   // launch configuration of the CTA path
   CtaLaunch cta{};
   int sm_count = 0;
+  size_t smem_optin = 0;
   cudaStream_t last_stream = nullptr;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   int64_t n_launches = 0, h2d_bytes = 0;
@@ -338,6 +335,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   cudaDeviceProp prop;
   PHS_CUDA(cudaGetDeviceProperties(&prop, dev));
   sim->sm_count = prop.multiProcessorCount;
+  sim->smem_optin = (size_t)prop.sharedMemPerBlockOptin;
   const int B = sim->batch, L = sim->fab->n_links();
 
   sim->flow_base.assign(B + 1, 0);
@@ -361,6 +359,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   std::vector<int32_t> succ((size_t)succ_base[B]), pc0((size_t)Ft);
   std::vector<uint8_t> pc8((size_t)pc8_base[B], 0);
   std::vector<int64_t> capq((size_t)B * L), coll_first((size_t)sim->total_colls);
+  std::vector<int32_t> lcomp((size_t)B * L);
   std::vector<int32_t> coll_n((size_t)sim->total_colls);
   sim->h_desc.resize(B);
   for (int i = 0; i < B; ++i) {
@@ -399,6 +398,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         const int32_t a = find(in.path[in.path_off[f]]), b = find(in.path[e]);
         if (a != b) parent[std::max(a, b)] = std::min(a, b);
       }
+    for (int l = 0; l < L; ++l) lcomp[(size_t)i * L + l] = find(l);
     FlowRec *r = rec.data() + sim->flow_base[i];
     for (int64_t f = 0; f < F; ++f) {
       FlowRec x;
@@ -445,6 +445,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(sim->d_succ.upload(succ, st));
   PHS_CUDA(sim->d_pc0.upload(pc0, st));
   PHS_CUDA(sim->d_capq.upload(capq, st));
+  PHS_CUDA(sim->d_lcomp.upload(lcomp, st));
   PHS_CUDA(sim->d_coll_first.upload(coll_first, st));
   PHS_CUDA(sim->d_coll_n.upload(coll_n, st));
   PHS_CUDA(sim->d_pred_cnt.alloc((size_t)Ft));
@@ -509,7 +510,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   }
   PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
   sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
-                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
+                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
                              (capq.size() + coll_first.size()) * 8);
   PHS_CUDA(cudaEventCreate(&sim->ev0));
   PHS_CUDA(cudaEventCreate(&sim->ev1));
@@ -528,6 +529,7 @@ DevTables tables_of(phs_sim *sim) {
   t.pred_cnt0 = sim->d_pc0.p;
   t.pred_cnt0_u8 = sim->d_pc8.p;
   t.capq = sim->d_capq.p;
+  t.lcomp = sim->d_lcomp.p;
   t.pred_cnt = sim->d_pred_cnt.p;
   t.t_done = sim->d_tdone.p;
   t.bneck = sim->d_bneck.p;
@@ -538,44 +540,52 @@ DevTables tables_of(phs_sim *sim) {
 }
 
 // Cluster path (a9): every instance in `list` is simulated by one thread-block cluster; clusters pull instances
-// from the list until it is empty.
-phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, cudaStream_t st) {
+// from the list until it is empty.  `slot_scale` multiplies the per-CTA slot capacity (retry after an overflow).
+phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, cudaStream_t st) {
   if (list.empty()) return PHS_OK;
   const int L = sim->fab->n_links();
   int64_t maxF = 1;
   for (int i : list) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
+  if (L >= 65535) return fail(PHS_ERANGE, "cluster path: topologies with 65535 or more links are not supported");
+  // shared memory per CTA: the flow slots (hot fields) and, if it fits next to 1024 slots, the debit accumulators
+  const size_t smem_max = sim->smem_optin - 2048;  // the kernel's static shared memory
+  const bool agg = cluster_smem_bytes(L, 1024, true) <= smem_max;
+  int64_t Sc_max = 64;
+  while (Sc_max < 65535 && cluster_smem_bytes(L, std::min<int64_t>(Sc_max * 2, 65535), agg) <= smem_max)
+    Sc_max = std::min<int64_t>(Sc_max * 2, 65535);
+  for (int64_t step = Sc_max / 2; step >= 16; step /= 2)  // refine to the largest capacity that fits
+    if (Sc_max + step <= 65535 && cluster_smem_bytes(L, Sc_max + step, agg) <= smem_max) Sc_max += step;
   int want = 1;
-  while (want < 16 && (int64_t)want * kClusterThreads * 4 < maxF) want *= 2;  // ~4 flows per thread
+  while (want < 16 && ((int64_t)want * kClusterThreads * 2 < maxF || (int64_t)want * Sc_max < maxF)) want *= 2;
   int cs = 1, max_clusters = 1;
-  PHS_CUDA(cluster_path_limits(want, &cs, &max_clusters));
+  PHS_CUDA(cluster_path_limits(want, cluster_smem_bytes(L, Sc_max, agg), &cs, &max_clusters));
   const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
-  if (maxF > sim->scratch_Fs || n_clusters > sim->scratch_regions) {
-    const int64_t Fs = std::max(maxF, sim->scratch_Fs);
+  // a flow is created in the partition of the CTA that released it: twice the even share plus slack at first,
+  // up to what shared memory holds
+  const int64_t Sc = std::min<int64_t>(Sc_max, std::max<int64_t>(64, std::min<int64_t>(maxF, (2 * maxF / cs + 256) * slot_scale)));
+  if (slot_scale > 1 && Sc == sim->scratch_Sc)
+    return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the cluster's shared memory");
+  if (Sc != sim->scratch_Sc || n_clusters > sim->scratch_regions || cs != sim->scratch_cs) {
     const int R = std::max(n_clusters, sim->scratch_regions);
-    PHS_CUDA(sim->g_i64.alloc(cluster_i64_per_region(L, Fs) * R));
-    PHS_CUDA(sim->g_i32.alloc(cluster_i32_per_region(L, Fs) * R));
-    PHS_CUDA(sim->g_f64.alloc(cluster_f64_per_region(Fs) * R));
-    PHS_CUDA(sim->g_u8.alloc((size_t)L * R));
-    PHS_CUDA(sim->g_ctrl.alloc((size_t)64 * R));
+    PHS_CUDA(sim->g_scratch.alloc(cluster_region_bytes(L, Sc, cs) * R));
     PHS_CUDA(sim->d_cticket.alloc(1));
-    sim->scratch_Fs = Fs;
+    sim->scratch_Sc = Sc;
     sim->scratch_regions = R;
+    sim->scratch_cs = cs;
   }
   std::vector<int32_t> sorted(list);
   std::stable_sort(sorted.begin(), sorted.end(),
                    [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
   PHS_CUDA(sim->d_clist.upload(sorted, st));
   PHS_CUDA(cudaMemsetAsync(sim->d_cticket.p, 0, sizeof(int), st));
-  PHS_CUDA(cudaMemsetAsync(sim->g_ctrl.p, 0, sizeof(unsigned long long) * 64 * sim->scratch_regions, st));
   ClusterScratch sc;
-  sc.i64 = sim->g_i64.p;
-  sc.i32 = sim->g_i32.p;
-  sc.f64 = sim->g_f64.p;
-  sc.u8 = sim->g_u8.p;
-  sc.ctrl = sim->g_ctrl.p;
-  sc.Fs = sim->scratch_Fs;
+  sc.base = sim->g_scratch.p;
+  sc.region_bytes = cluster_region_bytes(L, sim->scratch_Sc, cs);
+  sc.Sc = sim->scratch_Sc;
+  sc.aggregate = agg ? 1 : 0;
   PHS_CUDA(launch_cluster_path(tables_of(sim), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
                                n_clusters, sim->want_log, st));
+  PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy
   return PHS_OK;
 }
 
@@ -598,36 +608,44 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     PHS_CUDA(cudaMemsetAsync(sim->d_ticket.p, 0, sizeof(int), st));
     PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta, st));
   }
-  {
-    phs_status gs = run_cluster_path(sim, sim->cluster_list, st);
-    if (gs != PHS_OK) return gs;
-    if (!sim->cluster_list.empty()) sim->n_launches++;
-  }
   PHS_CUDA(cudaEventRecord(sim->ev1, st));
   PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
   PHS_CUDA(cudaStreamSynchronize(st));
-  // instances that ran out of shared-memory slots: re-run on the cluster path (and remember for later runs)
+  PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
+  // instances that ran out of shared-memory slots on the CTA path move to the cluster path (also for later runs)
   std::vector<int32_t> redo;
   for (int i = 0; i < B; ++i)
-    if (sim->h_res[i].status == kOverflow) redo.push_back(i);
-  PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
+    if (!sim->order.empty() && sim->h_res[i].status == kOverflow) redo.push_back(i);
   if (!redo.empty()) {
-    PHS_CUDA(cudaEventRecord(sim->ev0, st));
-    phs_status gs = run_cluster_path(sim, redo, st);
-    if (gs != PHS_OK) return gs;
-    sim->n_launches++;
-    PHS_CUDA(cudaEventRecord(sim->ev1, st));
     for (int inst : redo) {
       sim->cluster_list.push_back(inst);
       sim->order.erase(std::find(sim->order.begin(), sim->order.end(), inst));
     }
     if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
     sim->cta.grid = std::min<int>(sim->cta.grid, std::max<int>(1, (int)sim->order.size()));
+    PHS_CUDA(cudaStreamSynchronize(st));
+  }
+  // cluster path; an instance that overflows a CTA's slot partition is re-run with larger partitions
+  std::vector<int32_t> todo(sim->cluster_list);
+  for (int64_t scale = sim->cluster_scale; !todo.empty(); scale *= 2) {
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
+    phs_status gs = run_cluster_path(sim, todo, scale, st);
+    if (gs != PHS_OK) return gs;
+    sim->n_launches++;
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
     PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
     PHS_CUDA(cudaStreamSynchronize(st));
     float extra = 0.f;
     PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
     sim->main_kernel_ms += extra;
+    std::vector<int32_t> again;
+    for (int i : todo)
+      if (sim->h_res[i].status == kOverflow) again.push_back(i);
+    if (!again.empty()) {
+      if (scale > 64) return fail(PHS_ECUDA, "cluster path: slot partitions overflow even at full size");
+      sim->cluster_scale = scale * 2;  // remember for later runs
+    }
+    todo.swap(again);
   }
   if (sim->total_colls > 0) sim->n_launches++;
   PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
@@ -714,6 +732,8 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
     c.n_events += sim->h_res[i].n_events;
     c.sum_active += sim->h_res[i].sum_active;
     c.sum_par_rounds += sim->h_res[i].sum_par_rounds;
+    c.max_active = std::max(c.max_active, sim->h_res[i].max_active);
+    c.max_slots = std::max(c.max_slots, sim->h_res[i].max_slots);
   }
   c.n_flow_events = 2 * sim->total_flows;
   c.n_kernel_launches = sim->n_launches;

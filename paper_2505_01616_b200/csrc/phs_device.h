@@ -14,6 +14,7 @@ struct DevTables {
   const int32_t *pred_cnt0;  // [F_total] number of predecessors
   const uint8_t *pred_cnt0_u8;  // same as bytes (per-instance slices 4-byte aligned), or nullptr if a count > 255
   const int64_t *capq;       // [B][n_links] link capacity in rate quanta
+  const int32_t *lcomp;      // [B][n_links] static component (representative link) of every link
   int32_t *pred_cnt;         // [F_total] outstanding predecessors (dynamic)
   double *t_done;            // [F_total] O1
   int32_t *bneck;            // [F_total] O3
@@ -36,24 +37,34 @@ struct CtaLaunch {
 cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &cfg,
                             cudaStream_t stream);
 
-// Cluster path: one thread-block cluster (up to 16 CTAs, hardware cluster barrier) per large instance, all state
-// in global memory (L2-resident).  Clusters pull instance indices from list[0..n) through *ticket; the cluster
-// with rank k in the grid uses scratch region k.
-struct ClusterScratch {
-  int64_t *i64;   // per region: cap_rem[L], share[L], a_rq[Fs]
-  int32_t *i32;   // per region: n, nsnap, cnt0, cnt1, leader [L each]; a_flow, a_bn, a_arg, free_stack, p_flow0,
-                  //             p_flow1 [Fs each]; a_path [kMaxHops * Fs]
-  double *f64;    // per region: a_rem, p_tact0, p_tact1, a_tl, a_tc [Fs each]
-  uint8_t *u8;    // per region: dirty[L]
-  unsigned long long *ctrl;  // per region: 64 words of control state
-  int64_t Fs;     // slot capacity of a region (>= flows of the largest instance on this path)
+// Cluster path: one thread-block cluster (up to 16 CTAs, hardware cluster barrier) per large instance; link state
+// in global memory (L2-resident), flow slots in CTA-private partitions of a global slot array.  Clusters pull
+// instance indices from list[0..n) through *ticket; the cluster with rank k in the grid uses scratch region k.
+struct LinkS {          // 32 bytes = one L2 sector: everything a flow reads about a link when it votes
+  long long share0;     // floor(cap / n0): the link's fair share at the start of a solve
+  long long sharew;     // share after the debits of the current solve (valid iff wsolve == solve id)
+  int wsolve;
+  int n0;               // ACTIVE flows on the link
+  int beat;             // round number in which an unfrozen flow on the link voted for another link
+  int chg;              // solve id of the last change of n0
 };
-__host__ __device__ inline size_t cluster_i64_per_region(int L, int64_t Fs) { return (size_t)(2 * (int64_t)L + Fs); }
-__host__ __device__ inline size_t cluster_i32_per_region(int L, int64_t Fs) { return (size_t)(5 * (int64_t)L + (6 + kMaxHops) * Fs); }
-__host__ __device__ inline size_t cluster_f64_per_region(int64_t Fs) { return (size_t)(5 * Fs); }
+struct LinkW {          // 16 bytes: working state of the debits
+  long long caprem;
+  int nw;               // unfrozen flows on the link
+  int deb;              // round number of the last debit
+};
+struct ClusterScratch {
+  unsigned char *base;  // n_regions * region_bytes
+  size_t region_bytes;
+  int64_t Sc;           // slot capacity of one CTA's partition
+  int aggregate;        // 1: debits are pre-summed per CTA in shared memory (needs 16 bytes per link)
+};
 constexpr int kClusterThreads = 1024;
-// Largest cluster size (<= want) that can be co-scheduled, and how many such clusters fit on the device at once.
-cudaError_t cluster_path_limits(int want, int *cluster_size, int *max_clusters);
+size_t cluster_region_bytes(int n_links, int64_t Sc, int cluster_size);
+size_t cluster_smem_bytes(int n_links, int64_t Sc, bool aggregate);
+// Largest cluster size (<= want) that can be co-scheduled with `smem` bytes of dynamic shared memory per CTA, and
+// how many such clusters fit on the device at once.
+cudaError_t cluster_path_limits(int want, size_t smem, int *cluster_size, int *max_clusters);
 cudaError_t launch_cluster_path(const DevTables &t, const int32_t *list, int n, int *ticket, const ClusterScratch &s,
                                 int cluster_size, int n_clusters, bool log, cudaStream_t stream);
 

@@ -52,6 +52,8 @@ struct InstResult {
   int64_t sum_par_rounds;
   int32_t max_active;
   int32_t max_pending;
+  int32_t max_slots;       // high-water mark of the slot array
+  int32_t pad_;
 };
 constexpr int32_t kOverflow = 1;  // internal: the CTA path ran out of shared-memory slots
 

@@ -561,6 +561,7 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
       r.sum_par_rounds = sum_rounds;
       r.max_active = max_active;
       r.max_pending = max_pending;
+      r.max_slots = S.ctl[C_HI];
       T.res[inst] = r;
     }
     __syncthreads();
