@@ -51,6 +51,11 @@ def make_workload(name, n_gpus, per_gpu=0):
         return W.cfg3(batch=(per_gpu or 4096) * n_gpus), per_gpu or 4096
     if name == "cfg4":
         return W.cfg4(batch=(per_gpu or 8) * n_gpus), per_gpu or 8
+    # shrunken variants (the parity-test sizes), for profiling runs only
+    if name == "cfg2s":
+        return W.cfg2(k=8, agg_uplinks=2), 1
+    if name == "cfg4s":
+        return W.cfg4(batch=(per_gpu or 2) * n_gpus, n_hosts=8, gph=8, n_leaves=4, n_spines=2), per_gpu or 2
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -184,7 +189,7 @@ def run_ours(args, rank, world, local_rank):
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
     # ---- device-resident arm: tables built and uploaded once, each step = phs_run
-    sim = B.Sim.from_workload(w, instances=(first, count))
+    sim = B.Sim.from_workload(w, instances=(first, count), path=args.path)
     sim.finalize(stream=sp)
     flows = sim.total_flows
     colls = sum(w.instances[i].n_collectives for i in mine)
@@ -226,7 +231,7 @@ def run_ours(args, rank, world, local_rank):
     # ---- end-to-end arm: host arrays -> C-ABI submission -> table build -> H2D -> run -> D2H, every step
     def e2e_step():
         t0 = time.perf_counter()
-        s2 = B.Sim.from_workload(w, instances=(first, count))
+        s2 = B.Sim.from_workload(w, instances=(first, count), path=args.path)
         s2.run(stream=sp)
         out = B.phs_get_all_completion_times(s2.h)
         dt = time.perf_counter() - t0
@@ -318,6 +323,7 @@ def main():
     ap.add_argument("--workload", default="cfg1")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", type=int, default=0, help="scheduler policy: 0 auto, 1 CTA path, 2 cluster path")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end arm (profiling runs)")
     ap.add_argument("--instances", type=int, default=0,
                     help="instances per GPU (default: the config's own batch); smaller batches are for profiling")

@@ -555,15 +555,26 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
     Sc_max = std::min<int64_t>(Sc_max * 2, 65535);
   for (int64_t step = Sc_max / 2; step >= 16; step /= 2)  // refine to the largest capacity that fits
     if (Sc_max + step <= 65535 && cluster_smem_bytes(L, Sc_max + step, agg) <= smem_max) Sc_max += step;
+  // cluster size: enough shared memory for the flows that can be PENDING or ACTIVE at once.  A ring collective
+  // has at most one step in flight per rank (n_ranks flows) plus its successors waiting out their latency; an
+  // all-to-all or a raw flow set can be in flight as a whole.
+  int64_t bound = 1;
+  for (int i : list) {
+    const Instance &in = sim->inst[i];
+    int64_t b = in.n_flows();
+    for (const Collective &c : in.colls)
+      if (c.kind != PHS_ALLTOALL) b -= c.n_flows - std::min<int64_t>(c.n_flows, 2 * (int64_t)c.n_ranks);
+    bound = std::max(bound, b);
+  }
   int want = 1;
-  while (want < 16 && ((int64_t)want * kClusterThreads * 2 < maxF || (int64_t)want * Sc_max < maxF)) want *= 2;
+  while (want < 16 && (int64_t)want * Sc_max < bound * slot_scale) want *= 2;
   int cs = 1, max_clusters = 1;
   PHS_CUDA(cluster_path_limits(want, cluster_smem_bytes(L, Sc_max, agg), &cs, &max_clusters));
   const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
   // a flow is created in the partition of the CTA that released it: twice the even share plus slack at first,
   // up to what shared memory holds
-  const int64_t Sc = std::min<int64_t>(Sc_max, std::max<int64_t>(64, std::min<int64_t>(maxF, (2 * maxF / cs + 256) * slot_scale)));
-  if (slot_scale > 1 && Sc == sim->scratch_Sc)
+  const int64_t Sc = std::min<int64_t>(Sc_max, std::max<int64_t>(64, std::min<int64_t>(maxF, (2 * bound / cs + 256) * slot_scale)));
+  if (slot_scale > 1 && Sc == sim->scratch_Sc && cs == sim->scratch_cs)
     return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the cluster's shared memory");
   if (Sc != sim->scratch_Sc || n_clusters > sim->scratch_regions || cs != sim->scratch_cs) {
     const int R = std::max(n_clusters, sim->scratch_regions);

@@ -81,7 +81,7 @@ __device__ __forceinline__ void smem_add64(long long *p, long long v) {
 }
 
 __host__ __device__ inline size_t region_links_bytes(int L) {
-  size_t o = (size_t)L * sizeof(LinkS) + (size_t)L * sizeof(LinkW) + (size_t)L * 4 * 5;  // + solve, won, chglist, dlist x2
+  size_t o = (size_t)L * sizeof(LinkS) + (size_t)L * sizeof(LinkW) + (size_t)L * 4 * 2;  // + solve, won
   return (o + 255) / 256 * 256;
 }
 
@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   LinkS *LS = (LinkS *)rb;
   LinkW *LW = (LinkW *)(LS + L);
   int *solve_g = (int *)(LW + L);
-  int *won = solve_g + L, *chglist = won + L, *dlist0 = chglist + L, *dlist1 = dlist0 + L;
+  int *won = solve_g + L;
   unsigned long long *ctrl64 = (unsigned long long *)(rb + region_links_bytes(L));
   int *ctl_g = (int *)ctrl64;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -226,9 +226,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       ++solve;
       const int hi0 = min(ctl[M_HI], Sc);
       const int qtail = ctl[M_QTAIL];
-      auto touch_link = [&](int l, int delta) {  // the link's flow count changes: note it for this event's solve
-        atomicAdd(&LS[l].n0, delta);
-        if (atomicExch(&LS[l].chg, solve) != solve) __stcg(&chglist[atomicAdd(&ctl_g[K_NCHG], 1)], l);
+      auto touch_link = [&](int l, int delta) {  // the link's flow count changes: its share0 is stale for this
+        atomicAdd(&LS[l].n0, delta);             // event's solve (no value returns: both are fire-and-forget)
+        __stcg(&LS[l].chg, solve);
       };
       auto activate = [&](int slot) {
 #pragma unroll
@@ -244,9 +244,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         atomicAdd(&ctl[M_DACT], 1);
         atomicSub(&ctl[M_DPEND], 1);
       };
-      auto release = [&](int gf) {
-        if (atomicSub(&pred_cnt[gf], 1) != 1) return;
-        const FlowRec r = rec[gf];
+      auto make_pending = [&](int gf, const FlowRec &r) {  // S4.5: t_act = max(start, now) + Lat
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
         const int h = atomicAdd(&ctl[M_QHEAD], 1);
         const int slot = h < qtail ? S.freeq[h % Sc] : atomicAdd(&ctl[M_HI], 1);
@@ -258,6 +256,20 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         const bool due = ta <= t_next;
         fill_slot(slot, gf, r, due ? kInf : ta);
         if (due) activate(slot);
+      };
+      auto release = [&](int gf) {
+        if (atomicSub(&pred_cnt[gf], 1) != 1) return;
+        const FlowRec r = rec[gf];
+        make_pending(gf, r);
+      };
+      auto release2 = [&](int g0, int g1) {  // both counters, then both records: the round trips overlap
+        const bool z0 = g0 >= 0 && atomicSub(&pred_cnt[g0], 1) == 1;
+        const bool z1 = g1 >= 0 && atomicSub(&pred_cnt[g1], 1) == 1;
+        FlowRec r0, r1;
+        if (z0) r0 = rec[g0];
+        if (z1) r1 = rec[g1];
+        if (z0) make_pending(g0, r0);
+        if (z1) make_pending(g1, r1);
       };
       for (int s = tid; s < hi0; s += NT) {
         if (!(S.tc[s] <= t_next)) continue;
@@ -282,8 +294,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         atomicAdd(&ctl[M_DDONE], 1);
         const int nsucc = S.succ_cnt[s];
         if (nsucc <= 2) {
-          if (nsucc > 0) release(S.succ0[s]);
-          if (nsucc > 1) release(S.succ1[s]);
+          if (nsucc > 0) release2(S.succ0[s], nsucc > 1 ? S.succ1[s] : -1);
         } else {
           const int e0 = S.succ0[s];
           for (int e = 0; e < nsucc; ++e) release(succ[e0 + e]);
@@ -307,10 +318,6 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         atomicMax(&ctl_g[K_MAXSLOTS], ctl[M_HI]);
         ctl[M_NWL0] = 0;
         ctl[M_NWL1] = 0;
-      }
-      if (ctid == 0) {
-        __stcg(&ctl_g[K_NDL0], 0);
-        __stcg(&ctl_g[K_NDL1], 0);
       }
       cluster.sync();  // ---------------------------------------------------------------- cluster barrier X
       now = t_next;
@@ -341,45 +348,58 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       max_pending = max(max_pending, nPend);
       const int par = ev & 1;
 
-      // ======== P: fair share of the links whose flow count changed (a5; every CTA computes the same values),
-      // working capacities of the links that will be re-solved (split over the cluster)
-      {
-        const int nchg = __ldcg(&ctl_g[K_NCHG]);
-        for (int i = tid; i < nchg; i += NT) {
-          const int l = __ldcg(&chglist[i]);
-          const int n0 = __ldcg(&LS[l].n0);
-          if (n0 > 0) __stcg(&LS[l].share0, fair_share(__ldg(&capq[l]), n0));
-        }
-        for (int l = ctid; l < L; l += CT) {
-          if (LOG || __ldcg(&solve_g[__ldg(&lcomp[l])]) == solve) {
-            __stcg(&LW[l].caprem, (long long)__ldg(&capq[l]));
-            __stcg(&LW[l].nw, __ldcg(&LS[l].n0));
-          }
+      // ======== P: working capacities of the links that will be re-solved (split over the cluster; they are first
+      // debited after cluster barrier 1)
+      for (int l = ctid; l < L; l += CT) {
+        if (LOG || __ldcg(&solve_g[__ldg(&lcomp[l])]) == solve) {
+          __stcg(&LW[l].caprem, (long long)__ldg(&capq[l]));
+          __stcg(&LW[l].nw, __ldcg(&LS[l].n0));
         }
       }
-      __syncthreads();
-
       // ======== rates (a5-a7): parallel progressive filling over the components this event touched
       unsigned short *wl = S.wl0, *wl_next = S.wl1;
       int nwl_idx = M_NWL0;
       double mymin = kInf;  // completion / activation times of this thread's flows, folded as they become final
-      auto vote = [&](int s, bool first) {  // a6: arg-min (share, id) link of the flow's path; beat the others
+      // a5 + a6: the fair share of every link of the flow's path, refreshed by the flow itself where it is stale
+      // (every flow on such a link computes and stores the same value), arg-min (share, id), beat the other links
+      auto vote = [&](int s, bool first) {
         int p[kMaxHops], pb[kMaxHops];
-        long long best = LLONG_MAX;
-        int arg = -1;
+        long long sh[kMaxHops];
 #pragma unroll
-        for (int h = 0; h < kMaxHops; ++h) {
+        for (int h = 0; h < kMaxHops; ++h) {  // all loads first: one L2 round trip for the whole path
           const int l = p[h] = S.path[s * kMaxHops + h];
+          sh[h] = LLONG_MAX;
+          pb[h] = g;
           if (l == kNoLink) continue;
           const longlong2 a = __ldcg((const longlong2 *)&LS[l]);
           const int4 b = __ldcg((const int4 *)&LS[l] + 1);
-          const long long sh = (!first && b.x == solve) ? a.y : a.x;
           pb[h] = b.z;
-          if (sh < best || (sh == best && l < arg)) {
-            best = sh;
-            arg = l;
+          if (first) {
+            if (b.w == solve) {  // flow count changed in this event
+              sh[h] = fair_share(__ldg(&capq[l]), b.y);
+              __stcg(&LS[l].share0, sh[h]);
+            } else {
+              sh[h] = a.x;
+            }
+          } else {
+            const longlong2 w = __ldcg((const longlong2 *)&LW[l]);
+            if ((int)(w.y >> 32) == g - 1) {  // debited in the previous round
+              sh[h] = fair_share(w.x, (int)(unsigned)(unsigned long long)w.y);
+              __stcg(&LS[l].sharew, sh[h]);
+              __stcg(&LS[l].wsolve, solve);
+            } else {
+              sh[h] = b.x == solve ? a.y : a.x;
+            }
           }
         }
+        long long best = LLONG_MAX;
+        int arg = -1;
+#pragma unroll
+        for (int h = 0; h < kMaxHops; ++h)
+          if (p[h] != kNoLink && (sh[h] < best || (sh[h] == best && p[h] < arg))) {
+            best = sh[h];
+            arg = p[h];
+          }
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h)
           if (p[h] != kNoLink && p[h] != arg && pb[h] != g) __stcg(&LS[p[h]].beat, g);
@@ -412,10 +432,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           } else {
             atomicAdd((unsigned long long *)&LW[l].caprem, (unsigned long long)(-rq));
             atomicSub(&LW[l].nw, 1);
-            if (atomicExch(&LW[l].deb, g) != g) {
-              int *dl = (it & 1) ? dlist1 : dlist0;
-              __stcg(&dl[atomicAdd(&ctl_g[K_NDL0 + (it & 1)], 1)], l);
-            }
+            __stcg(&LW[l].deb, g);
           }
         }
       };
@@ -469,7 +486,6 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       for (;;) {
         cluster.sync();  // -------------------------------------------------------------- cluster barrier 1
         if (rounds == 0 && ctid == 0) {  // everybody has read these for this event
-          __stcg(&ctl_g[K_NCHG], 0);
           __stcg((long long *)&ctrl64[Q_TMIN0 + (par ^ 1)], __double_as_longlong(kInf));
         }
         ++rounds;
@@ -495,20 +511,20 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         // ---- combine: this CTA's debits, its minimum time and its "flows left" flag
         if (AGG) {
           const int nt = ctl[M_NTOUCH];
-          int *dl = (it & 1) ? dlist1 : dlist0;
           for (int i = tid; i < nt; i += NT) {
             const int l = touched[i];
             atomicAdd((unsigned long long *)&LW[l].caprem, (unsigned long long)(-dcap_loc[l]));
             atomicSub(&LW[l].nw, dn_loc[l]);
-            if (atomicExch(&LW[l].deb, g) != g) __stcg(&dl[atomicAdd(&ctl_g[K_NDL0 + (it & 1)], 1)], l);
+            __stcg(&LW[l].deb, g);
             dcap_loc[l] = 0;
             dn_loc[l] = 0;
           }
         }
+        if (warp == 0) {
+          const double m = warp_min(lane < NT / 32 ? red[lane] : kInf);
+          if (lane == 0) atomicMin(&ctrl64[Q_TMIN0 + par], (unsigned long long)__double_as_longlong(m));
+        }
         if (tid == 0) {
-          double m = red[0];
-          for (int w = 1; w < NT / 32; ++w) m = dmin(m, red[w]);
-          atomicMin(&ctrl64[Q_TMIN0 + par], (unsigned long long)__double_as_longlong(m));
           if (left) __stcg(&ctl_g[K_LEFT0 + it % 3], 1);
           if (crank == 0) __stcg(&ctl_g[K_LEFT0 + (it + 2) % 3], 0);  // last read two barriers ago
         }
@@ -519,24 +535,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           ctl[M_NTOUCH] = 0;
         }
         const bool any_left = __ldcg(&ctl_g[K_LEFT0 + it % 3]) != 0;
-        const int rpar = it & 1;
         ++it;
         if (!any_left) break;
-        // ---- R: fair share of the links debited in this round (a5; every CTA computes the same values)
-        {
-          const int ndl = __ldcg(&ctl_g[K_NDL0 + rpar]);
-          const int *dl = rpar ? dlist1 : dlist0;
-          for (int i = tid; i < ndl; i += NT) {
-            const int l = __ldcg(&dl[i]);
-            const longlong2 w = __ldcg((const longlong2 *)&LW[l]);
-            const int nw = (int)(unsigned)(unsigned long long)w.y;
-            if (nw > 0) {
-              __stcg(&LS[l].sharew, fair_share(w.x, nw));
-              __stcg(&LS[l].wsolve, solve);
-            }
-          }
-          if (ctid == 0) __stcg(&ctl_g[K_NDL0 + (rpar ^ 1)], 0);
-        }
         __syncthreads();
         // ---- V: the flows still listed vote on the new shares
         ++g;
