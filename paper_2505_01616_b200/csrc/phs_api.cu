@@ -539,51 +539,58 @@ DevTables tables_of(phs_sim *sim) {
   return t;
 }
 
-// Cluster path (a9): every instance in `list` is simulated by one thread-block cluster; clusters pull instances
-// from the list until it is empty.  `slot_scale` multiplies the per-CTA slot capacity (retry after an overflow).
+// Cluster path (a9): every instance in `list` is simulated by one thread-block cluster with all dynamic state in
+// the shared memory of its CTAs; clusters pull instances from the list until it is empty.  `slot_scale` scales the
+// guess of how many flows are PENDING or ACTIVE at once (doubled after an overflow).
 phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, cudaStream_t st) {
   if (list.empty()) return PHS_OK;
   const int L = sim->fab->n_links();
-  int64_t maxF = 1;
-  for (int i : list) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
   if (L >= 65535) return fail(PHS_ERANGE, "cluster path: topologies with 65535 or more links are not supported");
-  // shared memory per CTA: the flow slots (hot fields) and, if it fits next to 1024 slots, the debit accumulators
-  const size_t smem_max = sim->smem_optin - 2048;  // the kernel's static shared memory
-  const bool agg = cluster_smem_bytes(L, 1024, true) <= smem_max;
-  int64_t Sc_max = 64;
-  while (Sc_max < 65535 && cluster_smem_bytes(L, std::min<int64_t>(Sc_max * 2, 65535), agg) <= smem_max)
-    Sc_max = std::min<int64_t>(Sc_max * 2, 65535);
-  for (int64_t step = Sc_max / 2; step >= 16; step /= 2)  // refine to the largest capacity that fits
-    if (Sc_max + step <= 65535 && cluster_smem_bytes(L, Sc_max + step, agg) <= smem_max) Sc_max += step;
-  // cluster size: enough shared memory for the flows that can be PENDING or ACTIVE at once.  A ring collective
-  // has at most one step in flight per rank (n_ranks flows) plus its successors waiting out their latency; an
-  // all-to-all or a raw flow set can be in flight as a whole.
-  int64_t bound = 1;
+  // slots needed per instance: every flow without predecessors is PENDING from t = 0; later, a ring collective
+  // has at most one step in flight per rank plus the successors waiting out their latency, while an all-to-all
+  // or a raw flow set can be in flight as a whole.  Start from a quarter of that bound; overflow doubles it.
+  int64_t maxF = 1, target = 64;
   for (int i : list) {
     const Instance &in = sim->inst[i];
-    int64_t b = in.n_flows();
+    int64_t bound = in.n_flows(), initial = 0;
     for (const Collective &c : in.colls)
-      if (c.kind != PHS_ALLTOALL) b -= c.n_flows - std::min<int64_t>(c.n_flows, 2 * (int64_t)c.n_ranks);
-    bound = std::max(bound, b);
+      if (c.kind != PHS_ALLTOALL) bound -= c.n_flows - std::min<int64_t>(c.n_flows, 2 * (int64_t)c.n_ranks);
+    for (int64_t f = 0; f < in.n_flows(); ++f) initial += in.pred_off[f + 1] == in.pred_off[f];
+    maxF = std::max<int64_t>(maxF, in.n_flows());
+    target = std::max(target, std::max(initial, std::min(bound, bound * slot_scale / 4)));
+    if (slot_scale > 4) target = std::max(target, std::min<int64_t>(in.n_flows(), bound * slot_scale / 4));
   }
-  int want = 1;
-  while (want < 16 && (int64_t)want * Sc_max < bound * slot_scale) want *= 2;
-  int cs = 1, max_clusters = 1;
-  PHS_CUDA(cluster_path_limits(want, cluster_smem_bytes(L, Sc_max, agg), &cs, &max_clusters));
+  const size_t smem_max = sim->smem_optin - 4096;  // minus the kernel's static shared memory
+  const bool log = sim->want_log;
+  int cs = 0, max_clusters = 0;
+  int64_t Sc = 0;
+  bool agg = false, cold = false;
+  for (int c = 1; c <= 16 && !cs; c *= 2) {
+    if ((int64_t)c * kClusterThreads * 2 < target && c < 16) continue;  // at most ~2 slots per thread
+    const int64_t sc = std::min<int64_t>(65535, (target + c - 1) / c + 64);
+    const bool opts[4][2] = {{true, true}, {false, true}, {true, false}, {false, false}};  // {agg, cold in smem}
+    for (int k = 0; k < 4 && !cs; ++k) {
+      if (c < 16 && !opts[k][1]) continue;  // spill cold fields to global only at the largest cluster size
+      const size_t smem = cluster_smem_bytes(L, c, sc, opts[k][0], opts[k][1], log);
+      if (smem > smem_max) continue;
+      int n = 0;
+      PHS_CUDA(cluster_max_clusters(c, smem, &n));
+      if (n < 1) continue;
+      cs = c;
+      Sc = sc;
+      agg = opts[k][0];
+      cold = opts[k][1];
+      max_clusters = n;
+    }
+  }
+  if (!cs)
+    return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the shared memory of a cluster");
   const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
-  // a flow is created in the partition of the CTA that released it: twice the even share plus slack at first,
-  // up to what shared memory holds
-  const int64_t Sc = std::min<int64_t>(Sc_max, std::max<int64_t>(64, std::min<int64_t>(maxF, (2 * bound / cs + 256) * slot_scale)));
-  if (slot_scale > 1 && Sc == sim->scratch_Sc && cs == sim->scratch_cs)
-    return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the cluster's shared memory");
-  if (Sc != sim->scratch_Sc || n_clusters > sim->scratch_regions || cs != sim->scratch_cs) {
-    const int R = std::max(n_clusters, sim->scratch_regions);
-    PHS_CUDA(sim->g_scratch.alloc(cluster_region_bytes(L, Sc, cs) * R));
-    PHS_CUDA(sim->d_cticket.alloc(1));
-    sim->scratch_Sc = Sc;
-    sim->scratch_regions = R;
-    sim->scratch_cs = cs;
-  }
+  const size_t region = cold ? 0 : cluster_region_bytes(Sc, cs);
+  if (region * n_clusters > sim->g_scratch.n) PHS_CUDA(sim->g_scratch.alloc(region * n_clusters));
+  if (!sim->d_cticket.p) PHS_CUDA(sim->d_cticket.alloc(1));
+  sim->scratch_Sc = Sc;
+  sim->scratch_cs = cs;
   std::vector<int32_t> sorted(list);
   std::stable_sort(sorted.begin(), sorted.end(),
                    [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
@@ -591,11 +598,12 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   PHS_CUDA(cudaMemsetAsync(sim->d_cticket.p, 0, sizeof(int), st));
   ClusterScratch sc;
   sc.base = sim->g_scratch.p;
-  sc.region_bytes = cluster_region_bytes(L, sim->scratch_Sc, cs);
-  sc.Sc = sim->scratch_Sc;
+  sc.region_bytes = region;
+  sc.Sc = Sc;
   sc.aggregate = agg ? 1 : 0;
+  sc.cold_smem = cold ? 1 : 0;
   PHS_CUDA(launch_cluster_path(tables_of(sim), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
-                               n_clusters, sim->want_log, st));
+                               n_clusters, log, st));
   PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy
   return PHS_OK;
 }
@@ -653,7 +661,7 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     for (int i : todo)
       if (sim->h_res[i].status == kOverflow) again.push_back(i);
     if (!again.empty()) {
-      if (scale > 64) return fail(PHS_ECUDA, "cluster path: slot partitions overflow even at full size");
+      if (scale > 64) return fail(PHS_ERANGE, "cluster path: flow slots overflow even at full size");
       sim->cluster_scale = scale * 2;  // remember for later runs
     }
     todo.swap(again);

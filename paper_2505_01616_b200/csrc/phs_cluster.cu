@@ -1,14 +1,15 @@
 // phs_cluster.cu -- cluster path of the hot path: one thread-block cluster (up to 16 CTAs, hardware cluster
 // barrier) simulates one LARGE instance (SURVEY.md 8(a) a4-a9 for instances whose state does not fit one SM).
 // Same algorithm as the CTA path (phs_kernels.cu): stamp-based local-minimum test, static-component re-solve, lazy
-// settle (R-LZ).  What changes is where the state lives and how the CTAs combine:
-//   * link state (32-byte LinkS + 16-byte LinkW per link) lives in global memory and stays L2-resident; it is read
-//     with ld.cg and written with st.cg / atomics, because other SMs of the cluster write it;
-//   * flow slots live in global memory too, but each CTA owns a private partition of the slot array (a flow is
-//     created in the partition of the CTA that released it), so slot traffic is L1-cacheable and never contended;
-//   * capacity debits are first summed per CTA in shared memory, then each touched link is debited once per CTA;
-//   * per filling round: V (arg-min, beat stamps) | cluster barrier | F (freeze, settle, debit) + combine |
-//     cluster barrier | R (shares of the debited links).
+// settle (R-LZ).  ALL dynamic state stays on chip, spread over the shared memory of the cluster's CTAs:
+//   * link l is owned by CTA (l mod CS); its 64 bytes of state sit in the owner's shared memory and every CTA
+//     reads / stamps / debits them through distributed shared memory (DSMEM, ~200 cycles instead of an L2 trip);
+//   * each CTA owns a private set of flow slots in its own shared memory (a flow is created in the CTA that
+//     released it); cold slot fields spill to a CTA-private global partition only when shared memory is short;
+//   * per-CTA partial results (next-event time, flows-left flag, flow counts) are written to arrays in CTA 0's
+//     shared memory and read back by everybody after the barrier;
+//   * per filling round: V (shares, arg-min, beat stamps) | cluster barrier | F (freeze, settle, debit) | cluster
+//     barrier.  No value-returning global atomic and no L2 round trip sits on the per-round path.
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
@@ -24,55 +25,81 @@ namespace phs {
 namespace {
 
 constexpr int NT = kClusterThreads;
+constexpr unsigned short kNoLink = 0xffff;
+constexpr int kMaxCS = 16;
 
-// control block of one region, viewed as int[128] / unsigned long long[64]
-enum {
-  K_INST = 0, K_NACTIVE, K_NPEND, K_DONE, K_OVERFLOW, K_NCHG, K_NDL0, K_NDL1, K_LEFT0, K_LEFT1, K_LEFT2, K_EV_NACT0,
-  K_EV_NACT1, K_EV_NCOMP, K_EV_ROUNDS, K_MAXSLOTS, K_FB_ID0 = 32 /* 16 per-CTA first_bneck ids */
+struct LinkA {  // 32 bytes: what a flow reads when it votes in the first round
+  long long share0;  // floor(cap / n0), valid unless chg == current solve id
+  long long cap;
+  int n0;     // ACTIVE flows on the link
+  int chg;    // solve id of the last change of n0
+  int beat;   // round number in which an unfrozen flow on the link voted for another link
+  int solve;  // (indexed by a component's representative link) id of the solve that must redo the component
 };
-constexpr int Q_TMIN0 = 24 /* [24],[25]: t_next minima by event parity */, Q_FB_KEY0 = 32 /* 16 per-CTA keys */;
+struct LinkB {  // 32 bytes: working state of a solve's debits
+  long long caprem;
+  long long sharew;  // share after debits, valid iff wsolve == current solve id
+  int nw;            // unfrozen flows on the link
+  int deb;           // round number of the last debit
+  int wsolve;
+  int comp;          // static component (representative link) of the link
+};
 
-// Per-CTA private flow slots.  Hot fields (read every round) live in shared memory; cold fields (touched when a
-// flow's rate changes, or when it completes) live in a CTA-private partition of the region's global slot block.
+// per-CTA partial results, gathered in CTA 0's shared memory
+struct CombX {  // after phase X
+  int n_act, n_pend, n_done, over;
+  int hi, ev_ncomp, ev_nact, pad;
+};
+struct CombF {  // after a filling round
+  double tmin;
+  long long fb_key;
+  int fb_id, left, pad0, pad1;
+};
+struct Comb {
+  CombX x[kMaxCS];
+  CombF f[kMaxCS];
+  int ev_rounds;
+  int inst;
+};
+
 struct Slots {
-  // shared memory, 44 bytes per slot + two work lists
   double *tc;          // PENDING: activation time; ACTIVE: completion time; free: +inf
   long long *rq;       // rate in quanta, -1 before the first solve
   int *flow, *bn, *comp, *arg;
-  unsigned short *path;  // [Sc * kMaxHops], kNoLink = none
+  unsigned short *path;  // [Sc * kMaxHops]
   unsigned short *wl0, *wl1;
-  // global memory
+  // cold fields: shared memory when it fits, else global
   double *rem, *tl;
   int *succ_cnt, *succ0, *succ1, *freeq;
 };
-constexpr unsigned short kNoLink = 0xffff;
-constexpr int kSlotSmemBytes = 8 + 8 + 4 * 4 + 2 * kMaxHops + 2 * 2;  // 48
+constexpr int kSlotHotBytes = 8 + 8 + 4 * 4 + 2 * kMaxHops + 2 * 2;  // 48
+constexpr int kSlotColdBytes = 2 * 8 + 4 * 4;                        // 32
 
-__host__ __device__ inline size_t slot_bytes_per_cta(int64_t Sc) {  // global part
-  return ((size_t)Sc * (2 * 8 + 4 * 4) + 255) / 256 * 256;
+__host__ __device__ inline size_t up16(size_t x) { return (x + 15) / 16 * 16; }
+
+// dynamic shared memory of one CTA
+__host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool agg, bool cold_smem, bool log,
+                                              size_t *o_lb, size_t *o_won, size_t *o_beatf, size_t *o_agg,
+                                              size_t *o_hot, size_t *o_cold) {
+  const size_t Lc = (size_t)(L + CS - 1) / CS;
+  size_t o = 0;
+  o += Lc * sizeof(LinkA);
+  if (o_lb) *o_lb = o;
+  o += Lc * sizeof(LinkB);
+  if (o_won) *o_won = o;
+  o += up16(log ? Lc * 4 : 0);
+  if (o_beatf) *o_beatf = o;
+  o += up16((size_t)L * 4);
+  if (o_agg) *o_agg = o;
+  o += agg ? up16((size_t)L * 16) : 0;
+  if (o_hot) *o_hot = o;
+  o += up16((size_t)Sc * kSlotHotBytes);
+  if (o_cold) *o_cold = o;
+  o += cold_smem ? up16((size_t)Sc * kSlotColdBytes) : 0;
+  return o;
 }
-__device__ inline void carve_slots(Slots &s, unsigned char *sm, unsigned char *gl, int64_t Sc) {
-  s.tc = (double *)sm;
-  s.rq = (long long *)(s.tc + Sc);
-  s.flow = (int *)(s.rq + Sc);
-  s.bn = s.flow + Sc;
-  s.comp = s.bn + Sc;
-  s.arg = s.comp + Sc;
-  s.path = (unsigned short *)(s.arg + Sc);
-  s.wl0 = s.path + Sc * kMaxHops;
-  s.wl1 = s.wl0 + Sc;
-  s.rem = (double *)gl;
-  s.tl = s.rem + Sc;
-  s.succ_cnt = (int *)(s.tl + Sc);
-  s.succ0 = s.succ_cnt + Sc;
-  s.succ1 = s.succ0 + Sc;
-  s.freeq = s.succ1 + Sc;
-}
 
-// smem control words of a CTA
-enum { M_HI = 0, M_QHEAD, M_QTAIL, M_DACT, M_DPEND, M_DDONE, M_NWL0, M_NWL1, M_NTOUCH, M_OVER, M_NCTL };
-
-__device__ __forceinline__ void smem_add64(long long *p, long long v) {
+__device__ __forceinline__ void add64_2x32(long long *p, long long v) {  // works on local and remote smem
   unsigned *w = (unsigned *)p;
   const unsigned lo = (unsigned)(unsigned long long)v, hi = (unsigned)((unsigned long long)v >> 32);
   const unsigned old = atomicAdd(w, lo);
@@ -80,60 +107,85 @@ __device__ __forceinline__ void smem_add64(long long *p, long long v) {
   if (hi + carry) atomicAdd(w + 1, hi + carry);
 }
 
-__host__ __device__ inline size_t region_links_bytes(int L) {
-  size_t o = (size_t)L * sizeof(LinkS) + (size_t)L * sizeof(LinkW) + (size_t)L * 4 * 2;  // + solve, won
-  return (o + 255) / 256 * 256;
-}
+enum { M_HI = 0, M_QHEAD, M_QTAIL, M_NACT, M_NPEND, M_NDONE, M_NWL0, M_NWL1, M_NTOUCH, M_OVER, M_EVC, M_EVA, M_NCTL };
 
 }  // namespace
 
-size_t cluster_region_bytes(int L, int64_t Sc, int cluster_size) {
-  return region_links_bytes(L) + 512 + (size_t)cluster_size * slot_bytes_per_cta(Sc);
+size_t cluster_smem_bytes(int L, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log) {
+  return smem_layout(L, cluster_size, Sc, aggregate, cold_smem, log, nullptr, nullptr, nullptr, nullptr, nullptr,
+                     nullptr);
 }
-size_t cluster_smem_bytes(int L, int64_t Sc, bool aggregate) {
-  return (aggregate ? (size_t)L * 16 : 16) + (size_t)Sc * kSlotSmemBytes + 16;
+size_t cluster_region_bytes(int64_t Sc, int cluster_size) {  // global spill area of the cold slot fields
+  return (size_t)cluster_size * (((size_t)Sc * kSlotColdBytes + 255) / 256 * 256);
 }
 
 // ================================================================================================ cluster kernel
-// LOG: write the event log (and solve every component at every event); AGG: debits are pre-summed in shared memory.
+// LOG: write the event log (and solve every component at every event); AGG: a CTA first sums its debits per link
+// in its own shared memory and then debits each touched link once.
 template <bool LOG, bool AGG>
 __global__ void __launch_bounds__(kClusterThreads, 1)
     phs_cluster_kernel(DevTables T, const int32_t *__restrict__ list, int n_list, int *ticket, ClusterScratch SC) {
   cg::cluster_group cluster = cg::this_cluster();
   const int CS = (int)cluster.num_blocks();
   const int crank = (int)cluster.block_rank();
+  const int csh = 31 - __clz(CS), cmask = CS - 1;  // CS is a power of two
   const int region = blockIdx.x / CS;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int ctid = crank * NT + tid;  // thread index within the cluster
-  const int CT = CS * NT;             // threads in the cluster
+  const int ctid = crank * NT + tid;
   const int L = T.n_links;
+  const int Lc = (L + CS - 1) / CS;
   const int Sc = (int)SC.Sc;
 
-  // ---- carve this cluster's region
-  unsigned char *rb = SC.base + (size_t)region * SC.region_bytes;
-  LinkS *LS = (LinkS *)rb;
-  LinkW *LW = (LinkW *)(LS + L);
-  int *solve_g = (int *)(LW + L);
-  int *won = solve_g + L;
-  unsigned long long *ctrl64 = (unsigned long long *)(rb + region_links_bytes(L));
-  int *ctl_g = (int *)ctrl64;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  long long *dcap_loc = (long long *)smem_raw;  // [L]   (AGG)
-  int *dn_loc = (int *)(dcap_loc + L);          // [L]
-  int *touched = dn_loc + L;                    // [L]
+  size_t o_lb, o_won, o_beatf, o_agg, o_hot, o_cold;
+  smem_layout(L, CS, Sc, AGG, SC.cold_smem != 0, LOG, &o_lb, &o_won, &o_beatf, &o_agg, &o_hot, &o_cold);
+  LinkA *la = (LinkA *)smem_raw;
+  LinkB *lb = (LinkB *)(smem_raw + o_lb);
+  int *won = (int *)(smem_raw + o_won);
+  int *beatf = (int *)(smem_raw + o_beatf);
+  long long *dcap_loc = (long long *)(smem_raw + o_agg);
+  int *dn_loc = (int *)(dcap_loc + L);
+  int *touched = dn_loc + L;
   Slots S;
-  carve_slots(S, smem_raw + (AGG ? (size_t)L * 16 : 16),
-              rb + region_links_bytes(L) + 512 + (size_t)crank * slot_bytes_per_cta(Sc), Sc);
+  {
+    unsigned char *h = smem_raw + o_hot;
+    S.tc = (double *)h;
+    S.rq = (long long *)(S.tc + Sc);
+    S.flow = (int *)(S.rq + Sc);
+    S.bn = S.flow + Sc;
+    S.comp = S.bn + Sc;
+    S.arg = S.comp + Sc;
+    S.path = (unsigned short *)(S.arg + Sc);
+    S.wl0 = S.path + (size_t)Sc * kMaxHops;
+    S.wl1 = S.wl0 + Sc;
+    unsigned char *c = SC.cold_smem ? smem_raw + o_cold
+                                    : SC.base + (size_t)region * SC.region_bytes +
+                                          (size_t)crank * (((size_t)Sc * kSlotColdBytes + 255) / 256 * 256);
+    S.rem = (double *)c;
+    S.tl = S.rem + Sc;
+    S.succ_cnt = (int *)(S.tl + Sc);
+    S.succ0 = S.succ_cnt + Sc;
+    S.succ1 = S.succ0 + Sc;
+    S.freeq = S.succ1 + Sc;
+  }
+  __shared__ Comb comb;  // only CTA 0's copy is used
   __shared__ double red[32];
   __shared__ long long red_key[32];
   __shared__ int red_id[32];
   __shared__ int ctl[M_NCTL];
+  __shared__ int bc[8];       // broadcast of the cluster-wide counts to the CTA
+  __shared__ double bc_t;     // ... and of the next event time
+  Comb *comb0 = cluster.map_shared_rank(&comb, 0);
+
+  // state of link l lives in the shared memory of CTA (l mod CS)
+  auto LA = [&](int l) { return cluster.map_shared_rank(la + (l >> csh), (unsigned)(l & cmask)); };
+  auto LB = [&](int l) { return cluster.map_shared_rank(lb + (l >> csh), (unsigned)(l & cmask)); };
 
   for (;;) {
     // ---- a9: clusters pull instances from the list
-    if (ctid == 0) __stcg(&ctl_g[K_INST], atomicAdd(ticket, 1));
+    if (ctid == 0) comb.inst = atomicAdd(ticket, 1);
     cluster.sync();
-    const int qi = __ldcg(&ctl_g[K_INST]);
+    const int qi = comb0->inst;
     cluster.sync();
     if (qi >= n_list) break;
     const int inst = list[qi];
@@ -149,33 +201,31 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
-    // ---- init: no flow anywhere, every slot free
-    for (int l = ctid; l < L; l += CT) {
-      LinkS z;
-      z.share0 = 0; z.sharew = 0; z.wsolve = 0; z.n0 = 0; z.beat = 0; z.chg = 0;
-      LS[l] = z;
-      LinkW w;
-      w.caprem = 0; w.nw = 0; w.deb = 0;
-      LW[l] = w;
-      solve_g[l] = 0;
-      won[l] = 0;
+    // ---- init: own links, own slots
+    for (int li = tid; li < Lc; li += NT) {
+      const int l = li * CS + crank;
+      LinkA a;
+      a.share0 = 0; a.cap = l < L ? capq[l] : 0; a.n0 = 0; a.chg = 0; a.beat = 0; a.solve = 0;
+      la[li] = a;
+      LinkB b;
+      b.caprem = 0; b.sharew = 0; b.nw = 0; b.deb = 0; b.wsolve = 0; b.comp = l < L ? lcomp[l] : 0;
+      lb[li] = b;
+      if (LOG) won[li] = 0;
     }
-    if (ctid >= 1 && ctid < 128) ctl_g[ctid] = 0;
+    for (int l = tid; l < L; l += NT) {
+      beatf[l] = 0;
+      if (AGG) {
+        dcap_loc[l] = 0;
+        dn_loc[l] = 0;
+      }
+    }
     for (int s = tid; s < Sc; s += NT) {
       S.flow[s] = -1;
       S.tc[s] = kInf;
     }
     if (tid < M_NCTL) ctl[tid] = 0;
-    if (AGG)
-      for (int l = tid; l < L; l += NT) {
-        dcap_loc[l] = 0;
-        dn_loc[l] = 0;
-      }
-    cluster.sync();
-    if (ctid == 0) {
-      ctrl64[Q_TMIN0] = (unsigned long long)__double_as_longlong(kInf);
-      ctrl64[Q_TMIN0 + 1] = (unsigned long long)__double_as_longlong(kInf);
-    }
+    if (crank == 0 && tid == 0) comb.ev_rounds = 0;
+    __syncthreads();
 
     auto fill_slot = [&](int slot, int f, const FlowRec &r, double ta) {
       S.flow[slot] = f;
@@ -191,7 +241,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       S.tc[slot] = ta;
     };
 
-    // S4: flows without predecessors become PENDING; flow f starts in the partition of CTA f mod CS
+    // S4: flows without predecessors become PENDING; flow f starts in CTA f mod CS
     for (int64_t f = crank + (int64_t)CS * tid; f < F; f += (int64_t)CS * NT) {
       const int pc = pc0[f];
       pred_cnt[f] = pc;
@@ -200,35 +250,33 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         const int slot = atomicAdd(&ctl[M_HI], 1);
         if (slot < Sc) {
           fill_slot(slot, (int)f, r, __dadd_rn(r.start, r.lat));
-          atomicAdd(&ctl[M_DPEND], 1);
+          atomicAdd(&ctl[M_NPEND], 1);
         } else {
           ctl[M_OVER] = 1;
         }
       }
     }
-    __syncthreads();
-    if (tid == 0) {
-      if (ctl[M_DPEND]) atomicAdd(&ctl_g[K_NPEND], ctl[M_DPEND]);
-      ctl[M_DPEND] = 0;
-      if (ctl[M_OVER]) __stcg(&ctl_g[K_OVERFLOW], 1);
-    }
+    __threadfence();  // pred_cnt[] is decremented by other CTAs of the cluster
     cluster.sync();
 
     double now = 0.0, t_next = 0.0;
-    int ev = -1, solve = 0, g = 0, it = 0;
+    int ev = -1, solve = 0, g = 0;
     long long sum_active = 0, sum_rounds = 0;
-    int max_active = 0, max_pending = 0;
+    int max_active = 0, max_pending = 0, max_slots = 0;
     int status = PHS_OK;
     int first_bneck = -1;
+    int nDone = 0, prev_nact = 0;
+    double acc_min = kInf;  // (thread 0 of a CTA) minimum of the times folded in this event's rounds
 
     for (;;) {
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
       ++solve;
       const int hi0 = min(ctl[M_HI], Sc);
       const int qtail = ctl[M_QTAIL];
-      auto touch_link = [&](int l, int delta) {  // the link's flow count changes: its share0 is stale for this
-        atomicAdd(&LS[l].n0, delta);             // event's solve (no value returns: both are fire-and-forget)
-        __stcg(&LS[l].chg, solve);
+      auto touch_link = [&](int l, int delta) {  // the link's flow count changes: its share0 is stale for this solve
+        LinkA *a = LA(l);
+        atomicAdd(&a->n0, delta);
+        a->chg = solve;
       };
       auto activate = [&](int slot) {
 #pragma unroll
@@ -237,12 +285,18 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           if (l == kNoLink) break;
           touch_link(l, 1);
         }
-        __stcg(&solve_g[S.comp[slot]], solve);
+        LA(S.comp[slot])->solve = solve;
         S.rq[slot] = -1;
         S.bn[slot] = -1;
         S.tc[slot] = kInf;
-        atomicAdd(&ctl[M_DACT], 1);
-        atomicSub(&ctl[M_DPEND], 1);
+        atomicAdd(&ctl[M_NACT], 1);
+        atomicSub(&ctl[M_NPEND], 1);
+        if (LOG) atomicAdd(&ctl[M_EVA], 1);
+        const int nsucc = S.succ_cnt[slot];  // the successors' records will be needed: pull them towards L2
+        if (nsucc > 0 && nsucc <= 2) {
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.succ0[slot]));
+          if (nsucc > 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.succ1[slot]));
+        }
       };
       auto make_pending = [&](int gf, const FlowRec &r) {  // S4.5: t_act = max(start, now) + Lat
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
@@ -252,15 +306,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           ctl[M_OVER] = 1;
           return;
         }
-        atomicAdd(&ctl[M_DPEND], 1);
+        atomicAdd(&ctl[M_NPEND], 1);
         const bool due = ta <= t_next;
         fill_slot(slot, gf, r, due ? kInf : ta);
         if (due) activate(slot);
-      };
-      auto release = [&](int gf) {
-        if (atomicSub(&pred_cnt[gf], 1) != 1) return;
-        const FlowRec r = rec[gf];
-        make_pending(gf, r);
       };
       auto release2 = [&](int g0, int g1) {  // both counters, then both records: the round trips overlap
         const bool z0 = g0 >= 0 && atomicSub(&pred_cnt[g0], 1) == 1;
@@ -286,59 +335,66 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           if (l == kNoLink) break;
           touch_link(l, -1);
         }
-        __stcg(&solve_g[S.comp[s]], solve);
+        LA(S.comp[s])->solve = solve;
         S.flow[s] = -1;
         S.tc[s] = kInf;
         S.freeq[atomicAdd(&ctl[M_QTAIL], 1) % Sc] = s;
-        atomicSub(&ctl[M_DACT], 1);
-        atomicAdd(&ctl[M_DDONE], 1);
+        atomicSub(&ctl[M_NACT], 1);
+        atomicAdd(&ctl[M_NDONE], 1);
+        if (LOG) atomicAdd(&ctl[M_EVC], 1);
         const int nsucc = S.succ_cnt[s];
         if (nsucc <= 2) {
           if (nsucc > 0) release2(S.succ0[s], nsucc > 1 ? S.succ1[s] : -1);
         } else {
           const int e0 = S.succ0[s];
-          for (int e = 0; e < nsucc; ++e) release(succ[e0 + e]);
+          for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
         }
       }
       __syncthreads();
-      if (tid == 0) {  // this CTA's net changes of the cluster-wide counters
-        const int dact = ctl[M_DACT], dpend = ctl[M_DPEND], ddone = ctl[M_DDONE];
-        if (dact) atomicAdd(&ctl_g[K_NACTIVE], dact);
-        if (dpend) atomicAdd(&ctl_g[K_NPEND], dpend);
-        if (ddone) atomicAdd(&ctl_g[K_DONE], ddone);
-        if (LOG) {
-          if (ddone) atomicAdd(&ctl_g[K_EV_NCOMP], ddone);
-          if (dact + ddone) atomicAdd(&ctl_g[K_EV_NACT0 + ((ev + 1) & 1)], dact + ddone);  // activations
-        }
-        ctl[M_DACT] = 0;
-        ctl[M_DPEND] = 0;
-        ctl[M_DDONE] = 0;
+      if (tid == 0) {  // publish this CTA's counts in CTA 0
+        CombX x;
+        x.n_act = ctl[M_NACT]; x.n_pend = ctl[M_NPEND]; x.n_done = ctl[M_NDONE]; x.over = ctl[M_OVER];
+        x.hi = ctl[M_HI]; x.ev_ncomp = ctl[M_EVC]; x.ev_nact = ctl[M_EVA]; x.pad = 0;
+        comb0->x[crank] = x;
+        ctl[M_EVC] = 0;
+        ctl[M_EVA] = 0;
         if (ctl[M_QHEAD] > qtail) ctl[M_QHEAD] = qtail;
-        if (ctl[M_OVER]) __stcg(&ctl_g[K_OVERFLOW], 1);
-        atomicMax(&ctl_g[K_MAXSLOTS], ctl[M_HI]);
         ctl[M_NWL0] = 0;
         ctl[M_NWL1] = 0;
       }
       cluster.sync();  // ---------------------------------------------------------------- cluster barrier X
       now = t_next;
-      const int nA = __ldcg(&ctl_g[K_NACTIVE]);
-      const int nPend = __ldcg(&ctl_g[K_NPEND]);
+      if (warp == 0) {  // one warp per CTA sums the per-CTA counts and hands them to the CTA
+        CombX x;
+        x.n_act = x.n_pend = x.n_done = x.over = x.hi = x.ev_ncomp = x.ev_nact = 0;
+        if (lane < CS) x = comb0->x[lane];
+        const int a = __reduce_add_sync(0xffffffffu, x.n_act), b = __reduce_add_sync(0xffffffffu, x.n_pend);
+        const int c = __reduce_add_sync(0xffffffffu, x.n_done), d = __reduce_add_sync(0xffffffffu, x.over);
+        const int e = __reduce_max_sync(0xffffffffu, x.hi);
+        const int nc = __reduce_add_sync(0xffffffffu, x.ev_ncomp), na = __reduce_add_sync(0xffffffffu, x.ev_nact);
+        if (lane == 0) {
+          bc[0] = a; bc[1] = b; bc[2] = c; bc[3] = d; bc[4] = e; bc[5] = nc; bc[6] = na;
+        }
+      }
+      __syncthreads();
+      const int nA = bc[0], nPend = bc[1], over = bc[3];
+      nDone = bc[2];
+      max_slots = max(max_slots, bc[4]);
       if (LOG && ctid == 0) {
         if (log && ev >= 0) {  // O4: the event that just finished
           phs_event e;
           e.t = now;
-          e.n_completed = __ldcg(&ctl_g[K_EV_NCOMP]);
-          e.n_activated = __ldcg(&ctl_g[K_EV_NACT0 + (ev & 1)]);
-          e.n_rounds = __ldcg(&ctl_g[K_EV_ROUNDS]);
+          e.n_completed = bc[5];
+          e.n_activated = prev_nact;
+          e.n_rounds = comb.ev_rounds;
           e.first_bneck = first_bneck;
           log[ev] = e;
         }
-        __stcg(&ctl_g[K_EV_NCOMP], 0);
-        __stcg(&ctl_g[K_EV_ROUNDS], 0);
-        if (ev >= 0) __stcg(&ctl_g[K_EV_NACT0 + (ev & 1)], 0);
+        comb.ev_rounds = 0;
+        prev_nact = bc[6];
       }
       ++ev;
-      if (__ldcg(&ctl_g[K_OVERFLOW])) {
+      if (over) {
         status = kOverflow;
         break;
       }
@@ -346,16 +402,15 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       const int hi = min(ctl[M_HI], Sc);
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
-      const int par = ev & 1;
 
-      // ======== P: working capacities of the links that will be re-solved (split over the cluster; they are first
-      // debited after cluster barrier 1)
-      for (int l = ctid; l < L; l += CT) {
-        if (LOG || __ldcg(&solve_g[__ldg(&lcomp[l])]) == solve) {
-          __stcg(&LW[l].caprem, (long long)__ldg(&capq[l]));
-          __stcg(&LW[l].nw, __ldcg(&LS[l].n0));
+      // ======== P: working capacities of the own links that will be re-solved (first debited after barrier 1)
+      for (int li = tid; li < Lc; li += NT) {
+        if (LOG || LA(lb[li].comp)->solve == solve) {
+          lb[li].caprem = la[li].cap;
+          lb[li].nw = la[li].n0;
         }
       }
+
       // ======== rates (a5-a7): parallel progressive filling over the components this event touched
       unsigned short *wl = S.wl0, *wl_next = S.wl1;
       int nwl_idx = M_NWL0;
@@ -363,32 +418,33 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       // a5 + a6: the fair share of every link of the flow's path, refreshed by the flow itself where it is stale
       // (every flow on such a link computes and stores the same value), arg-min (share, id), beat the other links
       auto vote = [&](int s, bool first) {
-        int p[kMaxHops], pb[kMaxHops];
+        int p[kMaxHops];
         long long sh[kMaxHops];
 #pragma unroll
-        for (int h = 0; h < kMaxHops; ++h) {  // all loads first: one L2 round trip for the whole path
+        for (int h = 0; h < kMaxHops; ++h) {  // all loads first: one DSMEM round trip for the whole path
           const int l = p[h] = S.path[s * kMaxHops + h];
           sh[h] = LLONG_MAX;
-          pb[h] = g;
           if (l == kNoLink) continue;
-          const longlong2 a = __ldcg((const longlong2 *)&LS[l]);
-          const int4 b = __ldcg((const int4 *)&LS[l] + 1);
-          pb[h] = b.z;
+          LinkA *ap = LA(l);
+          const longlong2 a = *(const longlong2 *)ap;         // share0, cap
+          const int4 ai = *((const int4 *)ap + 1);            // n0, chg, beat, solve
           if (first) {
-            if (b.w == solve) {  // flow count changed in this event
-              sh[h] = fair_share(__ldg(&capq[l]), b.y);
-              __stcg(&LS[l].share0, sh[h]);
+            if (ai.y == solve) {  // flow count changed in this event
+              sh[h] = fair_share(a.y, ai.x);
+              ap->share0 = sh[h];
             } else {
               sh[h] = a.x;
             }
           } else {
-            const longlong2 w = __ldcg((const longlong2 *)&LW[l]);
-            if ((int)(w.y >> 32) == g - 1) {  // debited in the previous round
-              sh[h] = fair_share(w.x, (int)(unsigned)(unsigned long long)w.y);
-              __stcg(&LS[l].sharew, sh[h]);
-              __stcg(&LS[l].wsolve, solve);
+            LinkB *bp = LB(l);
+            const longlong2 b = *(const longlong2 *)bp;       // caprem, sharew
+            const int4 bi = *((const int4 *)bp + 1);          // nw, deb, wsolve, comp
+            if (bi.y == g - 1) {  // debited in the previous round
+              sh[h] = fair_share(b.x, bi.x);
+              bp->sharew = sh[h];
+              bp->wsolve = solve;
             } else {
-              sh[h] = b.x == solve ? a.y : a.x;
+              sh[h] = bi.z == solve ? b.y : a.x;
             }
           }
         }
@@ -402,7 +458,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           }
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h)
-          if (p[h] != kNoLink && p[h] != arg && pb[h] != g) __stcg(&LS[p[h]].beat, g);
+          if (p[h] != kNoLink && p[h] != arg && beatf[p[h]] != g) {  // one stamp per link, CTA and round
+            beatf[p[h]] = g;
+            LA(p[h])->beat = g;
+          }
         S.arg[s] = arg;
         return make_longlong2(best, (long long)arg);
       };
@@ -421,18 +480,20 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           S.tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));
         }
         mymin = dmin(mymin, S.tc[s]);
-        if (LOG && atomicExch(&won[arg], g) != g) atomicAdd(&ctl_g[K_EV_ROUNDS], 1);
+        if (LOG && atomicExch(cluster.map_shared_rank(won + (arg >> csh), (unsigned)(arg & cmask)), g) != g)
+          atomicAdd(&comb0->ev_rounds, 1);
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {  // debit the path
           const int l = S.path[s * kMaxHops + h];
           if (l == kNoLink) break;
           if (AGG) {
             if (atomicAdd(&dn_loc[l], 1) == 0) touched[atomicAdd(&ctl[M_NTOUCH], 1)] = l;
-            smem_add64(&dcap_loc[l], rq);
+            add64_2x32(&dcap_loc[l], rq);
           } else {
-            atomicAdd((unsigned long long *)&LW[l].caprem, (unsigned long long)(-rq));
-            atomicSub(&LW[l].nw, 1);
-            __stcg(&LW[l].deb, g);
+            LinkB *bp = LB(l);
+            add64_2x32(&bp->caprem, -rq);
+            atomicSub(&bp->nw, 1);
+            bp->deb = g;
           }
         }
       };
@@ -444,7 +505,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         int bl = INT_MAX;
         for (int s = tid; s < hi; s += NT) {
           if (S.flow[s] < 0) continue;
-          const bool in = S.bn[s] != -2 && (LOG || __ldcg(&solve_g[S.comp[s]]) == solve);
+          const bool in = S.bn[s] != -2 && (LOG || LA(S.comp[s])->solve == solve);
           if (!in) {
             mymin = dmin(mymin, S.tc[s]);
             continue;
@@ -478,16 +539,13 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
                 bk = red_key[w];
                 bl = red_id[w];
               }
-            __stcg((long long *)&ctrl64[Q_FB_KEY0 + crank], bk);
-            __stcg(&ctl_g[K_FB_ID0 + crank], bl);
+            comb0->f[crank].fb_key = bk;
+            comb0->f[crank].fb_id = bl;
           }
         }
       }
       for (;;) {
         cluster.sync();  // -------------------------------------------------------------- cluster barrier 1
-        if (rounds == 0 && ctid == 0) {  // everybody has read these for this event
-          __stcg((long long *)&ctrl64[Q_TMIN0 + (par ^ 1)], __double_as_longlong(kInf));
-        }
         ++rounds;
         // ---- F: flows whose arg-min link is unbeaten freeze (a7), settle (R-LZ) and debit; the rest stay listed
         const int nwl = ctl[nwl_idx];
@@ -496,10 +554,17 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         for (int i = tid; i < nwl; i += NT) {
           const int s = wl[i];
           const int arg = S.arg[s];
-          const longlong2 a = __ldcg((const longlong2 *)&LS[arg]);
-          const int4 b = __ldcg((const int4 *)&LS[arg] + 1);
-          if (b.z != g) {
-            freeze(s, arg, (rounds > 1 && b.x == solve) ? a.y : a.x);
+          LinkA *ap = LA(arg);
+          const long long share0 = ap->share0;
+          const int beat = ap->beat;
+          long long rq = share0;
+          if (rounds > 1) {
+            LinkB *bp = LB(arg);
+            const long long sw = bp->sharew;
+            if (bp->wsolve == solve) rq = sw;
+          }
+          if (beat != g) {
+            freeze(s, arg, rq);
           } else {
             wl_next[atomicAdd(&ctl[nxt_idx], 1)] = (unsigned short)s;
             left = true;
@@ -513,31 +578,41 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           const int nt = ctl[M_NTOUCH];
           for (int i = tid; i < nt; i += NT) {
             const int l = touched[i];
-            atomicAdd((unsigned long long *)&LW[l].caprem, (unsigned long long)(-dcap_loc[l]));
-            atomicSub(&LW[l].nw, dn_loc[l]);
-            __stcg(&LW[l].deb, g);
+            LinkB *bp = LB(l);
+            add64_2x32(&bp->caprem, -dcap_loc[l]);
+            atomicSub(&bp->nw, dn_loc[l]);
+            bp->deb = g;
             dcap_loc[l] = 0;
             dn_loc[l] = 0;
           }
         }
         if (warp == 0) {
           const double m = warp_min(lane < NT / 32 ? red[lane] : kInf);
-          if (lane == 0) atomicMin(&ctrl64[Q_TMIN0 + par], (unsigned long long)__double_as_longlong(m));
+          if (lane == 0) {
+            comb0->f[crank].tmin = m;
+            comb0->f[crank].left = left ? 1 : 0;
+          }
         }
-        if (tid == 0) {
-          if (left) __stcg(&ctl_g[K_LEFT0 + it % 3], 1);
-          if (crank == 0) __stcg(&ctl_g[K_LEFT0 + (it + 2) % 3], 0);  // last read two barriers ago
+        cluster.sync();  // -------------------------------------------------------------- cluster barrier 2
+        if (warp == 0) {
+          double m = kInf;
+          int lf = 0;
+          if (lane < CS) {
+            m = comb0->f[lane].tmin;
+            lf = comb0->f[lane].left;
+          }
+          m = warp_min(m);
+          lf = __reduce_or_sync(0xffffffffu, lf);
+          if (lane == 0) {
+            bc_t = acc_min = dmin(acc_min, m);
+            bc[7] = lf;
+            ctl[nwl_idx] = 0;
+            ctl[M_NTOUCH] = 0;
+          }
         }
         mymin = kInf;  // folded
-        cluster.sync();  // -------------------------------------------------------------- cluster barrier 2
-        if (tid == 0) {  // everybody has consumed this round's lists
-          ctl[nwl_idx] = 0;
-          ctl[M_NTOUCH] = 0;
-        }
-        const bool any_left = __ldcg(&ctl_g[K_LEFT0 + it % 3]) != 0;
-        ++it;
-        if (!any_left) break;
         __syncthreads();
+        if (!bc[7]) break;
         // ---- V: the flows still listed vote on the new shares
         ++g;
         {
@@ -550,14 +625,15 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         for (int i = tid; i < nv; i += NT) vote(wl[i], false);
       }
       // ======== next time (a8)
-      t_next = __longlong_as_double((long long)__ldcg(&ctrl64[Q_TMIN0 + par]));
+      t_next = bc_t;
+      acc_min = kInf;
       if (LOG && ctid == 0) {
         first_bneck = -1;
         if (nA > 0) {
           long long bk = LLONG_MAX;
           for (int c = 0; c < CS; ++c) {
-            const long long k = (long long)__ldcg(&ctrl64[Q_FB_KEY0 + c]);
-            const int id = __ldcg(&ctl_g[K_FB_ID0 + c]);
+            const long long k = comb.f[c].fb_key;
+            const int id = comb.f[c].fb_id;
             if (k < bk || (k == bk && id < first_bneck)) {
               bk = k;
               first_bneck = id;
@@ -570,14 +646,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     }
     if (ctid == 0) {
       InstResult r;
-      r.status = status != PHS_OK ? status : (__ldcg(&ctl_g[K_DONE]) < F ? PHS_ECYCLE : PHS_OK);
+      r.status = status != PHS_OK ? status : (nDone < F ? PHS_ECYCLE : PHS_OK);
       r.path = 1;
       r.n_events = ev;
       r.sum_active = sum_active;
       r.sum_par_rounds = sum_rounds;
       r.max_active = max_active;
       r.max_pending = max_pending;
-      r.max_slots = __ldcg(&ctl_g[K_MAXSLOTS]);
+      r.max_slots = max_slots;
       r.pad_ = 0;
       T.res[inst] = r;
     }
@@ -611,7 +687,7 @@ cudaError_t prepare(size_t smem) {
 template <bool LOG, bool AGG>
 cudaError_t launch_cluster_t(const DevTables &t, const int32_t *list, int n, int *ticket, const ClusterScratch &s,
                              int cluster_size, int n_clusters, cudaStream_t stream) {
-  const size_t smem = cluster_smem_bytes(t.n_links, s.Sc, AGG);
+  const size_t smem = cluster_smem_bytes(t.n_links, cluster_size, s.Sc, AGG, s.cold_smem != 0, LOG);
   cudaError_t e = prepare<LOG, AGG>(smem);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg{};
@@ -630,23 +706,20 @@ cudaError_t launch_cluster_path(const DevTables &t, const int32_t *list, int n, 
              : launch_cluster_t<false, false>(t, list, n, ticket, s, cluster_size, n_clusters, stream);
 }
 
-cudaError_t cluster_path_limits(int want, size_t smem, int *cluster_size, int *max_clusters) {
+cudaError_t cluster_max_clusters(int cluster_size, size_t smem, int *max_clusters) {
   cudaError_t e = prepare<true, true>(smem);
   if (e != cudaSuccess) return e;
-  for (int cs = want; cs >= 1; cs >>= 1) {
-    cudaLaunchConfig_t cfg{};
-    cudaLaunchAttribute attr[1];
-    set_cluster_attr(cfg, attr, cs, 1, smem, nullptr);
-    int n = 0;
-    e = cudaOccupancyMaxActiveClusters(&n, phs_cluster_kernel<true, true>, &cfg);
-    if (e == cudaSuccess && n >= 1) {
-      *cluster_size = cs;
-      *max_clusters = n;
-      return cudaSuccess;
-    }
+  cudaLaunchConfig_t cfg{};
+  cudaLaunchAttribute attr[1];
+  set_cluster_attr(cfg, attr, cluster_size, 1, smem, nullptr);
+  int n = 0;
+  e = cudaOccupancyMaxActiveClusters(&n, phs_cluster_kernel<true, true>, &cfg);
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    n = 0;
   }
-  (void)cudaGetLastError();
-  return cudaErrorLaunchOutOfResources;
+  *max_clusters = n;
+  return cudaSuccess;
 }
 
 }  // namespace phs

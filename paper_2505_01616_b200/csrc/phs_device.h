@@ -40,31 +40,19 @@ cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int
 // Cluster path: one thread-block cluster (up to 16 CTAs, hardware cluster barrier) per large instance; link state
 // in global memory (L2-resident), flow slots in CTA-private partitions of a global slot array.  Clusters pull
 // instance indices from list[0..n) through *ticket; the cluster with rank k in the grid uses scratch region k.
-struct LinkS {          // 32 bytes = one L2 sector: everything a flow reads about a link when it votes
-  long long share0;     // floor(cap / n0): the link's fair share at the start of a solve
-  long long sharew;     // share after the debits of the current solve (valid iff wsolve == solve id)
-  int wsolve;
-  int n0;               // ACTIVE flows on the link
-  int beat;             // round number in which an unfrozen flow on the link voted for another link
-  int chg;              // solve id of the last change of n0
-};
-struct LinkW {          // 16 bytes: working state of the debits
-  long long caprem;
-  int nw;               // unfrozen flows on the link
-  int deb;              // round number of the last debit
-};
 struct ClusterScratch {
-  unsigned char *base;  // n_regions * region_bytes
+  unsigned char *base;  // global spill area of the cold slot fields (n_regions * region_bytes), unused if cold_smem
   size_t region_bytes;
-  int64_t Sc;           // slot capacity of one CTA's partition
-  int aggregate;        // 1: debits are pre-summed per CTA in shared memory (needs 16 bytes per link)
+  int64_t Sc;           // flow slots per CTA
+  int aggregate;        // 1: a CTA pre-sums its debits per link in shared memory (16 bytes per link and CTA)
+  int cold_smem;        // 1: the cold slot fields live in shared memory too
 };
 constexpr int kClusterThreads = 1024;
-size_t cluster_region_bytes(int n_links, int64_t Sc, int cluster_size);
-size_t cluster_smem_bytes(int n_links, int64_t Sc, bool aggregate);
-// Largest cluster size (<= want) that can be co-scheduled with `smem` bytes of dynamic shared memory per CTA, and
-// how many such clusters fit on the device at once.
-cudaError_t cluster_path_limits(int want, size_t smem, int *cluster_size, int *max_clusters);
+// dynamic shared memory per CTA / global spill bytes per cluster
+size_t cluster_smem_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log);
+size_t cluster_region_bytes(int64_t Sc, int cluster_size);
+// how many clusters of this size and shared-memory footprint can be resident at once (0: it cannot launch)
+cudaError_t cluster_max_clusters(int cluster_size, size_t smem, int *max_clusters);
 cudaError_t launch_cluster_path(const DevTables &t, const int32_t *list, int n, int *ticket, const ClusterScratch &s,
                                 int cluster_size, int n_clusters, bool log, cudaStream_t stream);
 
