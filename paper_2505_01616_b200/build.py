@@ -28,7 +28,7 @@ def build(force=False, verbose=False):
     if not force and up_to_date():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc] + NVCC_FLAGS + os.environ.get("PHS_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + \
           [os.path.join(CSRC, f) for f in SOURCES] + ["-o", OUT]
     subprocess.check_call(cmd)
     return OUT

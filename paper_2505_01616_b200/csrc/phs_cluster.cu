@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include <climits>
+#include <cstdio>
 
 #include "phs_device.h"
 #include "phs_devutil.cuh"
@@ -89,7 +90,7 @@ __host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool ag
   if (o_won) *o_won = o;
   o += up16(log ? Lc * 4 : 0);
   if (o_beatf) *o_beatf = o;
-  o += up16((size_t)L * 4);
+  o += 2 * up16((size_t)L * 4);  // beatf[L], csolve[L]
   if (o_agg) *o_agg = o;
   o += agg ? up16((size_t)L * 16) : 0;
   if (o_hot) *o_hot = o;
@@ -143,6 +144,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   LinkB *lb = (LinkB *)(smem_raw + o_lb);
   int *won = (int *)(smem_raw + o_won);
   int *beatf = (int *)(smem_raw + o_beatf);
+  int *csolve = beatf + (up16((size_t)L * 4) / 4);  // per component (representative link): solve id that must redo it;
+                                                    // replicated in every CTA, because every flow and link reads it
   long long *dcap_loc = (long long *)(smem_raw + o_agg);
   int *dn_loc = (int *)(dcap_loc + L);
   int *touched = dn_loc + L;
@@ -214,6 +217,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     }
     for (int l = tid; l < L; l += NT) {
       beatf[l] = 0;
+      csolve[l] = 0;
       if (AGG) {
         dcap_loc[l] = 0;
         dn_loc[l] = 0;
@@ -265,6 +269,12 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     int max_active = 0, max_pending = 0, max_slots = 0;
     int status = PHS_OK;
     int first_bneck = -1;
+#ifdef PHS_PHASE_CLOCKS
+    long long pc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pt_ = clock64();
+#define PHS_TICK(i) { const long long t_ = clock64(); pc_[i] += t_ - pt_; pt_ = t_; }
+#else
+#define PHS_TICK(i)
+#endif
     int nDone = 0, prev_nact = 0;
     double acc_min = kInf;  // (thread 0 of a CTA) minimum of the times folded in this event's rounds
 
@@ -278,6 +288,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         atomicAdd(&a->n0, delta);
         a->chg = solve;
       };
+      auto mark_comp = [&](int c) {  // the component must be re-solved: tell every CTA
+        for (int r = 0; r < CS; ++r) cluster.map_shared_rank(csolve, (unsigned)r)[c] = solve;
+      };
       auto activate = [&](int slot) {
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
@@ -285,7 +298,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           if (l == kNoLink) break;
           touch_link(l, 1);
         }
-        LA(S.comp[slot])->solve = solve;
+        mark_comp(S.comp[slot]);
         S.rq[slot] = -1;
         S.bn[slot] = -1;
         S.tc[slot] = kInf;
@@ -335,7 +348,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           if (l == kNoLink) break;
           touch_link(l, -1);
         }
-        LA(S.comp[s])->solve = solve;
+        mark_comp(S.comp[s]);
         S.flow[s] = -1;
         S.tc[s] = kInf;
         S.freeq[atomicAdd(&ctl[M_QTAIL], 1) % Sc] = s;
@@ -350,6 +363,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
         }
       }
+      PHS_TICK(0)
       __syncthreads();
       if (tid == 0) {  // publish this CTA's counts in CTA 0
         CombX x;
@@ -362,7 +376,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         ctl[M_NWL0] = 0;
         ctl[M_NWL1] = 0;
       }
+      PHS_TICK(1)
       cluster.sync();  // ---------------------------------------------------------------- cluster barrier X
+      PHS_TICK(2)
       now = t_next;
       if (warp == 0) {  // one warp per CTA sums the per-CTA counts and hands them to the CTA
         CombX x;
@@ -405,7 +421,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
 
       // ======== P: working capacities of the own links that will be re-solved (first debited after barrier 1)
       for (int li = tid; li < Lc; li += NT) {
-        if (LOG || LA(lb[li].comp)->solve == solve) {
+        if (LOG || csolve[lb[li].comp] == solve) {
           lb[li].caprem = la[li].cap;
           lb[li].nw = la[li].n0;
         }
@@ -505,7 +521,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         int bl = INT_MAX;
         for (int s = tid; s < hi; s += NT) {
           if (S.flow[s] < 0) continue;
-          const bool in = S.bn[s] != -2 && (LOG || LA(S.comp[s])->solve == solve);
+          const bool in = S.bn[s] != -2 && (LOG || csolve[S.comp[s]] == solve);
           if (!in) {
             mymin = dmin(mymin, S.tc[s]);
             continue;
@@ -545,7 +561,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         }
       }
       for (;;) {
+        PHS_TICK(3)
         cluster.sync();  // -------------------------------------------------------------- cluster barrier 1
+        PHS_TICK(4)
         ++rounds;
         // ---- F: flows whose arg-min link is unbeaten freeze (a7), settle (R-LZ) and debit; the rest stay listed
         const int nwl = ctl[nwl_idx];
@@ -593,7 +611,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
             comb0->f[crank].left = left ? 1 : 0;
           }
         }
+        PHS_TICK(5)
         cluster.sync();  // -------------------------------------------------------------- cluster barrier 2
+        PHS_TICK(6)
         if (warp == 0) {
           double m = kInf;
           int lf = 0;
@@ -644,6 +664,11 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       sum_active += nA;
       sum_rounds += rounds;
     }
+#ifdef PHS_PHASE_CLOCKS
+    if (tid == 0 && (crank == 0 || crank == CS - 1))
+      printf("inst %d cta %d/%d events %d cycles: X %lld pub %lld barX %lld P+V %lld bar1 %lld F %lld bar2 %lld\n", inst, crank,
+             CS, ev, pc_[0], pc_[1], pc_[2], pc_[3], pc_[4], pc_[5], pc_[6]);
+#endif
     if (ctid == 0) {
       InstResult r;
       r.status = status != PHS_OK ? status : (nDone < F ? PHS_ECYCLE : PHS_OK);

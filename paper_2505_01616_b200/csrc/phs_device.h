@@ -47,7 +47,7 @@ struct ClusterScratch {
   int aggregate;        // 1: a CTA pre-sums its debits per link in shared memory (16 bytes per link and CTA)
   int cold_smem;        // 1: the cold slot fields live in shared memory too
 };
-constexpr int kClusterThreads = 1024;
+constexpr int kClusterThreads = 512;
 // dynamic shared memory per CTA / global spill bytes per cluster
 size_t cluster_smem_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log);
 size_t cluster_region_bytes(int64_t Sc, int cluster_size);
