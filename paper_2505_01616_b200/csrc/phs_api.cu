@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <numeric>
@@ -464,7 +465,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
   int64_t maxF = 0;
   for (int i = 0; i < B; ++i) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
-  const int threads = L <= 320 ? 128 : 256;
+  int threads = L <= 320 ? 128 : 256;
+  if (const char *e = getenv("PHS_CTA_THREADS")) threads = atoi(e);  // experiments only
   const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
@@ -473,7 +475,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     // resident CTAs per SM wanted: enough to cover the batch, at most what the thread count allows; fewer if the
     // slots would otherwise not hold a typical active set (min(F, 256) flows)
     int want = std::max(1, std::min(2048 / threads / 2, (B + sim->sm_count - 1) / sim->sm_count));
-    const int need = (int)std::min<int64_t>(maxF, 256);
+    int64_t bound = 32;  // slots an instance can need (Instance::slot_bound)
+    for (int i = 0; i < B; ++i) bound = std::max(bound, sim->inst[i].slot_bound());
+    const int need = (int)std::min<int64_t>(std::min<int64_t>(maxF, bound), 1 << 16);
     for (; want >= 1; --want) {
       const size_t budget = std::min(smem_max, per_sm / want - 1024);
       const int pcf = pc8_ok && cta_smem_bytes(L, need, (int)maxF, log) <= budget ? (int)maxF : 0;
@@ -489,6 +493,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           hi = mid - 32;
       }
       if (lo >= need || want == 1 || sim->policy_slots > 0) {
+        if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
         sim->cta.threads = threads;
         sim->cta.slots = lo;
         sim->cta.pc_flows = pcf;
@@ -552,9 +557,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   int64_t maxF = 1, target = 64;
   for (int i : list) {
     const Instance &in = sim->inst[i];
-    int64_t bound = in.n_flows(), initial = 0;
-    for (const Collective &c : in.colls)
-      if (c.kind != PHS_ALLTOALL) bound -= c.n_flows - std::min<int64_t>(c.n_flows, 2 * (int64_t)c.n_ranks);
+    int64_t bound = in.slot_bound(), initial = 0;
     for (int64_t f = 0; f < in.n_flows(); ++f) initial += in.pred_off[f + 1] == in.pred_off[f];
     maxF = std::max<int64_t>(maxF, in.n_flows());
     target = std::max(target, std::max(initial, std::min(bound, bound * slot_scale / 4)));

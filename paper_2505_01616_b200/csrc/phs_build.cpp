@@ -2,6 +2,7 @@
 // collective -> flow decomposer with its dependency DAG.  Pure host C++, no CUDA.  DESIGN.md S1-S3; the
 // passages of the paper are PAPER.md L98 (topology, multipath routing) and L104 (ring all-reduce, flows with
 // timestamps).
+#include <algorithm>
 #include <cmath>
 #include <limits>
 
@@ -221,6 +222,8 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   c.n_flows = (int32_t)nf;
   c.steps = steps;
   c.ranks.assign(ranks, ranks + N);
+  c.chain = (int32_t)inst.colls.size();
+  for (int a = 0; a < n_after; ++a) c.chain = std::min(c.chain, inst.colls[after[a]].chain);
   const int32_t conn = (int32_t)inst.colls.size();  // ECMP key: one path per (pair, collective)
   const double chunk = bytes / (double)N;
   if (kind == PHS_ALLTOALL) {

@@ -1,6 +1,7 @@
 // phs_internal.h -- shared between the host builder (phs_build.cpp), the API (phs_api.cu) and the kernels
 // (phs_kernels.cu).  Nothing here is shared with oracle/.
 #pragma once
+#include <algorithm>
 #include <cstdint>
 #include <string>
 #include <vector>
@@ -60,6 +61,7 @@ constexpr int32_t kOverflow = 1;  // internal: the CTA path ran out of shared-me
 // ---- host-side instance tables (built by phs_build.cpp) ----
 struct Collective {
   int32_t kind, n_ranks, first_flow, n_flows, steps;
+  int32_t chain;  // smallest id among the collectives this one is (transitively) chained `after`, else its own id
   std::vector<int32_t> ranks;
 };
 
@@ -74,6 +76,22 @@ struct Instance {
   std::vector<int32_t> pred;
   std::vector<Collective> colls;
   int64_t n_flows() const { return (int64_t)src.size(); }
+  // Upper estimate of how many flows can be PENDING or ACTIVE at once (sizes the on-chip slot arrays): raw flows
+  // and all-to-alls may be in flight as a whole; a ring collective keeps at most one flow per sender in flight and
+  // collectives chained with `after` follow each other per rank, so a chain counts once, with its largest member.
+  // Twice the ring size, because a slot freed in one phase is reused only in a later one.
+  int64_t slot_bound() const {
+    int64_t b = n_flows();
+    std::vector<int64_t> chain_max(colls.size(), 0);
+    for (size_t c = 0; c < colls.size(); ++c) {
+      b -= colls[c].n_flows;
+      const int64_t need = colls[c].kind == PHS_ALLTOALL ? colls[c].n_flows
+                                                          : std::min<int64_t>(colls[c].n_flows, 2 * (int64_t)colls[c].n_ranks);
+      chain_max[colls[c].chain] = std::max(chain_max[colls[c].chain], need);
+    }
+    for (int64_t m : chain_max) b += m;
+    return b;
+  }
 };
 
 // Link numbering and ECMP routing of one topology (S1, S2).

@@ -46,10 +46,9 @@ struct CtaSmem {
   double *s_rem;  // remaining bytes at time s_tl
   double *s_tl;   // time of the last rate change
   long long *s_rq;  // rate in quanta, -1 before the first solve
-  int *s_flow;    // flow id, -1 = free
-  int *s_bn;      // -2 PENDING, -1 ACTIVE and unfrozen, >= 0 bottleneck link
-  int *s_comp, *s_arg;
-  int *s_path;    // [S * kMaxHops]
+  int4 *s_meta;   // .x flow id (-1 = free); .y -2 PENDING, -1 ACTIVE and unfrozen, >= 0 bottleneck link;
+                  // .z static link component; .w arg-min link of the current round
+  uint4 *s_path;  // the path as 8 x uint16 (kNoLink = none): one 16-byte load brings the whole path
   int *s_succ_cnt, *s_succ0, *s_succ1;
   int *free_q;    // FIFO ring of free slots
   unsigned *pc8;  // [(PCF+3)/4] predecessor counters, one byte per flow
@@ -64,6 +63,14 @@ enum {
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+constexpr unsigned kNoLink = 0xffffu;
+static_assert(kMaxHops <= 8, "a path is stored as 8 x uint16");
+// unpack link h of a packed path
+__device__ __forceinline__ int path_at(const uint4 &p, int h) {
+  const unsigned w = h < 2 ? p.x : h < 4 ? p.y : h < 6 ? p.z : p.w;
+  return (int)((h & 1) ? (w >> 16) : (w & 0xffffu));
+}
 
 __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, int S, int pcf, bool log) {
   size_t o = 0, a;
@@ -88,11 +95,8 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   PHS_TAKE(l_deb, int, L)
   PHS_TAKE(l_solve, int, L)
   PHS_TAKE(l_won, int, log ? L : 0)
-  PHS_TAKE(s_flow, int, S)
-  PHS_TAKE(s_bn, int, S)
-  PHS_TAKE(s_comp, int, S)
-  PHS_TAKE(s_arg, int, S)
-  PHS_TAKE(s_path, int, S * kMaxHops)
+  PHS_TAKE(s_meta, int4, S)
+  PHS_TAKE(s_path, uint4, S)
   PHS_TAKE(s_succ_cnt, int, S)
   PHS_TAKE(s_succ0, int, S)
   PHS_TAKE(s_succ1, int, S)
@@ -134,7 +138,7 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
 // NT threads; LOG: write the event log (and solve every component at every event, so that the log's iteration
 // count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory.
 template <int NT, bool LOG, bool PCS>
-__global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
+__global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
                                                      int *ticket, int SC, int pcf) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int sh_inst;
@@ -173,7 +177,7 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
       if (LOG) S.l_won[l] = 0;
     }
     for (int s = tid; s < SC; s += NT) {
-      S.s_flow[s] = -1;
+      S.s_meta[s].x = -1;
       S.s_tc[s] = kInf;
     }
     if (tid < C_NCTL) S.ctl[tid] = 0;
@@ -185,12 +189,19 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
 
     // one slot per flow that is PENDING or ACTIVE; the whole record is staged when the flow becomes PENDING
     auto fill_slot = [&](int slot, int f, const FlowRec &r, double ta) {
-      S.s_flow[slot] = f;
+      S.s_meta[slot].x = f;
       S.s_rem[slot] = r.bytes;
-      S.s_bn[slot] = -2;
-      S.s_comp[slot] = r.comp;
+      S.s_meta[slot].y = -2;
+      S.s_meta[slot].z = r.comp;
+      {
+        unsigned w[4] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0xffffffffu};
 #pragma unroll
-      for (int h = 0; h < kMaxHops; ++h) S.s_path[slot * kMaxHops + h] = r.path[h];
+        for (int h = 0; h < kMaxHops; ++h) {
+          const unsigned l = r.path[h] < 0 ? kNoLink : (unsigned)r.path[h];
+          w[h >> 1] = (h & 1) ? ((w[h >> 1] & 0xffffu) | (l << 16)) : ((w[h >> 1] & 0xffff0000u) | l);
+        }
+        S.s_path[slot] = make_uint4(w[0], w[1], w[2], w[3]);
+      }
       S.s_succ_cnt[slot] = r.succ_cnt;
       S.s_succ0[slot] = r.succ_in[0];
       S.s_succ1[slot] = r.succ_in[1];
@@ -238,16 +249,18 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
       const int qtail = S.ctl[C_QTAIL];
 
       auto activate = [&](int slot) {  // PENDING -> ACTIVE: the flow now counts on its links
+        const uint4 pv = S.s_path[slot];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
-          const int l = S.s_path[slot * kMaxHops + h];
-          if (l < 0) break;
-          atomicAdd(&S.l_n0[l], 1);
-          S.l_chg[l] = solve;
+          const int l = path_at(pv, h);
+          if (l != (int)kNoLink) {
+            atomicAdd(&S.l_n0[l], 1);
+            S.l_chg[l] = solve;
+          }
         }
-        S.l_solve[S.s_comp[slot]] = solve;
+        S.l_solve[S.s_meta[slot].z] = solve;
         S.s_rq[slot] = -1;
-        S.s_bn[slot] = -1;
+        S.s_meta[slot].y = -1;
         S.s_tc[slot] = kInf;
         atomicAdd(&S.ctl[C_NACTIVE], 1);
         atomicSub(&S.ctl[C_NPEND], 1);
@@ -255,21 +268,19 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         // the successors' records will be needed when this flow completes: pull them towards L2 now
         const int nsucc = S.s_succ_cnt[slot];
         if (nsucc > 0 && nsucc <= 2) {
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.s_succ0[slot]));
-          if (nsucc > 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.s_succ1[slot]));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + S.s_succ0[slot]));
+          if (nsucc > 1) asm volatile("prefetch.global.L1 [%0];" ::"l"(rec + S.s_succ1[slot]));
         }
       };
-      auto release = [&](int gf) {  // S4.5: pred_cnt--, at 0 -> PENDING with t_act = max(start, now) + Lat
-        bool zero;
+      auto pred_done = [&](int gf) {  // S4.5: pred_cnt--; true when it reaches 0
         if (PCS) {
           const unsigned sh = (unsigned)(gf & 3) * 8u;
           const unsigned old = atomicSub(&S.pc8[gf >> 2], 1u << sh);
-          zero = ((old >> sh) & 0xffu) == 1u;
-        } else {
-          zero = atomicSub(&pred_cnt[gf], 1) == 1;
+          return ((old >> sh) & 0xffu) == 1u;
         }
-        if (!zero) return;
-        const FlowRec r = rec[gf];
+        return atomicSub(&pred_cnt[gf], 1) == 1;
+      };
+      auto make_pending = [&](int gf, const FlowRec &r) {  // -> PENDING with t_act = max(start, now) + Lat
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
         const int h = atomicAdd(&S.ctl[C_QHEAD], 1);
         const int slot = h < qtail ? S.free_q[h % SC] : atomicAdd(&S.ctl[C_HI], 1);
@@ -282,26 +293,37 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         fill_slot(slot, gf, r, due ? kInf : ta);
         if (due) activate(slot);
       };
+      auto release2 = [&](int g0, int g1) {  // both counters, then both records: the loads overlap
+        const bool z0 = g0 >= 0 && pred_done(g0);
+        const bool z1 = g1 >= 0 && pred_done(g1);
+        FlowRec r0, r1;
+        if (z0) r0 = rec[g0];
+        if (z1) r1 = rec[g1];
+        if (z0) make_pending(g0, r0);
+        if (z1) make_pending(g1, r1);
+      };
 
       for (int s = tid; s < hi0; s += NT) {
         if (!(S.s_tc[s] <= t_next)) continue;  // free slots hold +inf
-        if (S.s_bn[s] == -2) {
+        if (S.s_meta[s].y == -2) {
           activate(s);
           continue;
         }
         // the flow completes at t_next (bit-equal absolute time, S4.4)
-        const int f = S.s_flow[s];
+        const int f = S.s_meta[s].x;
         t_done[f] = t_next;
-        bneck_out[f] = S.s_bn[s];
+        bneck_out[f] = S.s_meta[s].y;
+        const uint4 pv = S.s_path[s];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
-          const int l = S.s_path[s * kMaxHops + h];
-          if (l < 0) break;
-          atomicSub(&S.l_n0[l], 1);
-          S.l_chg[l] = solve;
+          const int l = path_at(pv, h);
+          if (l != (int)kNoLink) {
+            atomicSub(&S.l_n0[l], 1);
+            S.l_chg[l] = solve;
+          }
         }
-        S.l_solve[S.s_comp[s]] = solve;
-        S.s_flow[s] = -1;
+        S.l_solve[S.s_meta[s].z] = solve;
+        S.s_meta[s].x = -1;
         S.s_tc[s] = kInf;
         S.free_q[atomicAdd(&S.ctl[C_QTAIL], 1) % SC] = s;
         atomicSub(&S.ctl[C_NACTIVE], 1);
@@ -309,11 +331,10 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         if (LOG) atomicAdd(&S.ctl[C_EV_NCOMP], 1);
         const int nsucc = S.s_succ_cnt[s];
         if (nsucc <= 2) {
-          if (nsucc > 0) release(S.s_succ0[s]);
-          if (nsucc > 1) release(S.s_succ1[s]);
+          if (nsucc > 0) release2(S.s_succ0[s], nsucc > 1 ? S.s_succ1[s] : -1);
         } else {
           const int e0 = S.s_succ0[s];
-          for (int e = 0; e < nsucc; ++e) release(succ[e0 + e]);
+          for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
         }
       }
       __syncthreads();
@@ -349,11 +370,12 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
 
       // ======== rates (a5-a7): parallel progressive filling over the components this event touched
       auto in_solve = [&](int s) {  // ACTIVE flow of a component that must be re-solved
-        if (S.s_flow[s] < 0 || S.s_bn[s] == -2) return false;
-        return LOG || S.l_solve[S.s_comp[s]] == solve;
+        const int4 m = S.s_meta[s];
+        if (m.x < 0 || m.y == -2) return false;
+        return LOG || S.l_solve[m.z] == solve;
       };
       auto freeze = [&](int s, int arg, long long rq) {  // a7; R-LZ: only a changed rate touches the flow's state
-        S.s_bn[s] = arg;
+        S.s_meta[s].y = arg;
         const long long old = S.s_rq[s];
         if (rq != old) {
           double rem = S.s_rem[s];
@@ -375,30 +397,36 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         int bl = INT_MAX;
         for (int s = tid; s < hi; s += NT) {
           if (!in_solve(s)) continue;
-          S.s_bn[s] = -1;
-          int p[kMaxHops];
+          S.s_meta[s].y = -1;
+          const uint4 pv = S.s_path[s];
+          int p[kMaxHops], chg[kMaxHops];
+          long long sh[kMaxHops];
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {  // all loads first
+            p[h] = path_at(pv, h);
+            const int l = p[h] != (int)kNoLink ? p[h] : 0;
+            chg[h] = S.l_chg[l];
+            sh[h] = S.l_share0[l];
+          }
           long long best = LLONG_MAX;
           int arg = -1;
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
-            const int l = p[h] = S.s_path[s * kMaxHops + h];
-            if (l < 0) continue;
-            long long sh;
-            if (S.l_chg[l] == solve) {
-              sh = fair_share(S.l_cap[l], S.l_n0[l]);
-              S.l_share0[l] = sh;  // every flow on the link stores the same value
-            } else {
-              sh = S.l_share0[l];
+            const int l = p[h];
+            if (l == (int)kNoLink) continue;
+            if (chg[h] == solve) {  // flow count changed in this event: every flow on the link stores the same value
+              sh[h] = fair_share(S.l_cap[l], S.l_n0[l]);
+              S.l_share0[l] = sh[h];
             }
-            if (sh < best || (sh == best && l < arg)) {
-              best = sh;
+            if (sh[h] < best || (sh[h] == best && l < arg)) {
+              best = sh[h];
               arg = l;
             }
           }
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h)
-            if (p[h] >= 0 && p[h] != arg) S.l_beat[p[h]] = g;  // an unfrozen flow on p[h] prefers another link
-          S.s_arg[s] = arg;
+            if (p[h] != (int)kNoLink && p[h] != arg) S.l_beat[p[h]] = g;  // an unfrozen flow on p[h] prefers another link
+          S.s_meta[s].w = arg;
           if (LOG && (best < bk || (best == bk && arg < bl))) {
             bk = best;
             bl = arg;
@@ -425,9 +453,9 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
       {  // ---- F0: unbeaten arg-min links freeze their flows (a7); fold the slot times (a8)
         double mymin = kInf;
         for (int s = tid; s < hi; s += NT) {
-          if (S.s_flow[s] < 0) continue;
-          if (S.s_bn[s] == -1) {
-            const int arg = S.s_arg[s];
+          if (S.s_meta[s].x < 0) continue;
+          if (S.s_meta[s].y == -1) {
+            const int arg = S.s_meta[s].w;
             if (S.l_beat[arg] != g)
               freeze(s, arg, S.l_share0[arg]);
             else
@@ -443,10 +471,11 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         // ---- I: working capacities of the links of this solve (idempotent stores)
         for (int s = tid; s < hi; s += NT) {
           if (!in_solve(s)) continue;
+          const uint4 pv = S.s_path[s];
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
-            const int l = S.s_path[s * kMaxHops + h];
-            if (l < 0) break;
+            const int l = path_at(pv, h);
+            if (l == (int)kNoLink) continue;
             S.l_caprem[l] = S.l_cap[l];
             S.l_nw[l] = S.l_n0[l];
             S.l_sharew[l] = S.l_share0[l];
@@ -455,12 +484,13 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
         __syncthreads();
         // ---- D: flows frozen in the first round debit their paths (a7)
         for (int s = tid; s < hi; s += NT) {
-          if (!in_solve(s) || S.s_bn[s] < 0) continue;
+          if (!in_solve(s) || S.s_meta[s].y < 0) continue;
           const long long rq = S.s_rq[s];
+          const uint4 pv = S.s_path[s];
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
-            const int l = S.s_path[s * kMaxHops + h];
-            if (l < 0) break;
+            const int l = path_at(pv, h);
+            if (l == (int)kNoLink) continue;
             if (S.l_n0[l] > 1) {
               smem_add64(&S.l_caprem[l], -rq);
               atomicSub(&S.l_nw[l], 1);
@@ -474,14 +504,15 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
           ++rounds;
           // ---- V: shares of the links debited in the previous round, arg-min of every unfrozen flow
           for (int s = tid; s < hi; s += NT) {
-            if (S.s_flow[s] < 0 || S.s_bn[s] != -1) continue;
+            if (S.s_meta[s].x < 0 || S.s_meta[s].y != -1) continue;
+            const uint4 pv = S.s_path[s];
             int p[kMaxHops];
             long long best = LLONG_MAX;
             int arg = -1;
 #pragma unroll
             for (int h = 0; h < kMaxHops; ++h) {
-              const int l = p[h] = S.s_path[s * kMaxHops + h];
-              if (l < 0) continue;
+              const int l = p[h] = path_at(pv, h);
+              if (l == (int)kNoLink) continue;
               long long sh;
               if (S.l_deb[l] == g - 1) {
                 sh = fair_share(S.l_caprem[l], S.l_nw[l]);
@@ -496,24 +527,25 @@ __global__ void __launch_bounds__(NT) phs_cta_kernel(DevTables T, const int32_t 
             }
 #pragma unroll
             for (int h = 0; h < kMaxHops; ++h)
-              if (p[h] >= 0 && p[h] != arg) S.l_beat[p[h]] = g;
-            S.s_arg[s] = arg;
+              if (p[h] != (int)kNoLink && p[h] != arg) S.l_beat[p[h]] = g;
+            S.s_meta[s].w = arg;
           }
           __syncthreads();
           // ---- F: freeze, debit, fold
           left = false;
           double mymin = kInf;
           for (int s = tid; s < hi; s += NT) {
-            if (S.s_flow[s] < 0) continue;
-            if (S.s_bn[s] == -1) {
-              const int arg = S.s_arg[s];
+            if (S.s_meta[s].x < 0) continue;
+            if (S.s_meta[s].y == -1) {
+              const int arg = S.s_meta[s].w;
               if (S.l_beat[arg] != g) {
                 const long long rq = S.l_sharew[arg];
                 freeze(s, arg, rq);
+                const uint4 pv = S.s_path[s];
 #pragma unroll
                 for (int h = 0; h < kMaxHops; ++h) {
-                  const int l = S.s_path[s * kMaxHops + h];
-                  if (l < 0) break;
+                  const int l = path_at(pv, h);
+                  if (l == (int)kNoLink) continue;
                   if (S.l_n0[l] > 1) {
                     smem_add64(&S.l_caprem[l], -rq);
                     atomicSub(&S.l_nw[l], 1);
