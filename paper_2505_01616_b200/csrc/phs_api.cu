@@ -465,8 +465,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
   int64_t maxF = 0;
   for (int i = 0; i < B; ++i) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
-  int threads = L <= 320 ? 128 : 256;
-  if (const char *e = getenv("PHS_CTA_THREADS")) threads = atoi(e);  // experiments only
+  const int threads = L <= 320 ? 128 : 256;  // measured on B200: 128 is best for cfg3-sized instances, 256+ for cfg1
   const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
