@@ -566,22 +566,27 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   const bool log = sim->want_log;
   int cs = 0, max_clusters = 0;
   int64_t Sc = 0;
-  bool agg = false, cold = false;
+  bool agg = false, cold = false, repl = false;
+  // replicated link shares pay when many flows share a link (every flow reads its links' shares every round)
+  const bool want_repl = target >= 8 * (int64_t)L;
   for (int c = 1; c <= 16 && !cs; c *= 2) {
     if ((int64_t)c * kClusterThreads * 2 < target && c < 16) continue;  // at most ~2 slots per thread
-    const int64_t sc = std::min<int64_t>(65535, (target + c - 1) / c + 64);
+    const int64_t sc = std::min<int64_t>(65535, (target + c - 1) / c + 16);
     const bool opts[4][2] = {{true, true}, {false, true}, {true, false}, {false, false}};  // {agg, cold in smem}
-    for (int k = 0; k < 4 && !cs; ++k) {
-      if (c < 16 && !opts[k][1]) continue;  // spill cold fields to global only at the largest cluster size
-      const size_t smem = cluster_smem_bytes(L, c, sc, opts[k][0], opts[k][1], log);
+    for (int k = 0; k < 8 && !cs; ++k) {
+      const bool o_agg = opts[k & 3][0], o_cold = opts[k & 3][1], o_repl = k < 4;
+      if (o_repl && !want_repl) continue;
+      if (c < 16 && !o_cold) continue;  // spill cold fields to global only at the largest cluster size
+      const size_t smem = cluster_smem_bytes(L, c, sc, o_agg, o_cold, log, o_repl);
       if (smem > smem_max) continue;
       int n = 0;
       PHS_CUDA(cluster_max_clusters(c, smem, &n));
       if (n < 1) continue;
       cs = c;
       Sc = sc;
-      agg = opts[k][0];
-      cold = opts[k][1];
+      agg = o_agg;
+      cold = o_cold;
+      repl = o_repl;
       max_clusters = n;
     }
   }
@@ -604,6 +609,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   sc.Sc = Sc;
   sc.aggregate = agg ? 1 : 0;
   sc.cold_smem = cold ? 1 : 0;
+  sc.replicate = repl ? 1 : 0;
   PHS_CUDA(launch_cluster_path(tables_of(sim), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
                                n_clusters, log, st));
   PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy

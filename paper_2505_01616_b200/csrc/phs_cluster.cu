@@ -66,22 +66,23 @@ struct Comb {
 struct Slots {
   double *tc;          // PENDING: activation time; ACTIVE: completion time; free: +inf
   long long *rq;       // rate in quanta, -1 before the first solve
-  int *flow, *bn, *comp, *arg;
+  int *bn;             // -3 free, -2 PENDING, -1 ACTIVE and unfrozen, >= 0 bottleneck link
+  unsigned short *comp, *arg;
   unsigned short *path;  // [Sc * kMaxHops]
   unsigned short *wl0, *wl1;
   // cold fields: shared memory when it fits, else global
   double *rem, *tl;
-  int *succ_cnt, *succ0, *succ1, *freeq;
+  int *flow, *succ_cnt, *succ0, *succ1, *freeq;
 };
-constexpr int kSlotHotBytes = 8 + 8 + 4 * 4 + 2 * kMaxHops + 2 * 2;  // 48
-constexpr int kSlotColdBytes = 2 * 8 + 4 * 4;                        // 32
+constexpr int kSlotHotBytes = 8 + 8 + 4 + 2 * 2 + 2 * kMaxHops + 2 * 2;  // 40
+constexpr int kSlotColdBytes = 2 * 8 + 5 * 4;                            // 36
 
 __host__ __device__ inline size_t up16(size_t x) { return (x + 15) / 16 * 16; }
 
 // dynamic shared memory of one CTA
-__host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool agg, bool cold_smem, bool log,
+__host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool agg, bool cold_smem, bool log, bool repl,
                                               size_t *o_lb, size_t *o_won, size_t *o_beatf, size_t *o_agg,
-                                              size_t *o_hot, size_t *o_cold) {
+                                              size_t *o_repl, size_t *o_hot, size_t *o_cold) {
   const size_t Lc = (size_t)(L + CS - 1) / CS;
   size_t o = 0;
   o += Lc * sizeof(LinkA);
@@ -93,6 +94,8 @@ __host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool ag
   o += 2 * up16((size_t)L * 4);  // beatf[L], csolve[L]
   if (o_agg) *o_agg = o;
   o += agg ? up16((size_t)L * 16) : 0;
+  if (o_repl) *o_repl = o;
+  o += repl ? up16((size_t)L * 22) : 0;  // sh_loc[L], sh0_loc[L] (8 each), chg_loc[L] (4), comp_loc[L] (2)
   if (o_hot) *o_hot = o;
   o += up16((size_t)Sc * kSlotHotBytes);
   if (o_cold) *o_cold = o;
@@ -112,9 +115,10 @@ enum { M_HI = 0, M_QHEAD, M_QTAIL, M_NACT, M_NPEND, M_NDONE, M_NWL0, M_NWL1, M_N
 
 }  // namespace
 
-size_t cluster_smem_bytes(int L, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log) {
-  return smem_layout(L, cluster_size, Sc, aggregate, cold_smem, log, nullptr, nullptr, nullptr, nullptr, nullptr,
-                     nullptr);
+size_t cluster_smem_bytes(int L, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log,
+                          bool replicate) {
+  return smem_layout(L, cluster_size, Sc, aggregate, cold_smem, log, replicate, nullptr, nullptr, nullptr, nullptr,
+                     nullptr, nullptr, nullptr);
 }
 size_t cluster_region_bytes(int64_t Sc, int cluster_size) {  // global spill area of the cold slot fields
   return (size_t)cluster_size * (((size_t)Sc * kSlotColdBytes + 255) / 256 * 256);
@@ -138,8 +142,16 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   const int Sc = (int)SC.Sc;
 
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  size_t o_lb, o_won, o_beatf, o_agg, o_hot, o_cold;
-  smem_layout(L, CS, Sc, AGG, SC.cold_smem != 0, LOG, &o_lb, &o_won, &o_beatf, &o_agg, &o_hot, &o_cold);
+  size_t o_lb, o_won, o_beatf, o_agg, o_repl, o_hot, o_cold;
+  const bool REPL = SC.replicate != 0;
+  smem_layout(L, CS, Sc, AGG, SC.cold_smem != 0, LOG, REPL, &o_lb, &o_won, &o_beatf, &o_agg, &o_repl, &o_hot, &o_cold);
+  // REPL: every CTA keeps its own copy of the links' current fair shares, so that voting reads local shared
+  // memory; owners broadcast the shares they recompute after debits, stale first-round shares are refreshed by the
+  // flows that need them
+  long long *sh_loc = (long long *)(smem_raw + o_repl);  // [L] share in the current round
+  long long *sh0_loc = sh_loc + L;                        // [L] share at the start of a solve
+  int *chg_loc = (int *)(sh0_loc + L);                    // [L] solve id of the last change of the link's flow count
+  unsigned short *comp_loc = (unsigned short *)(chg_loc + L);  // [L] static component of every link
   LinkA *la = (LinkA *)smem_raw;
   LinkB *lb = (LinkB *)(smem_raw + o_lb);
   int *won = (int *)(smem_raw + o_won);
@@ -154,11 +166,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     unsigned char *h = smem_raw + o_hot;
     S.tc = (double *)h;
     S.rq = (long long *)(S.tc + Sc);
-    S.flow = (int *)(S.rq + Sc);
-    S.bn = S.flow + Sc;
-    S.comp = S.bn + Sc;
+    S.bn = (int *)(S.rq + Sc);
+    S.comp = (unsigned short *)(S.bn + Sc);
     S.arg = S.comp + Sc;
-    S.path = (unsigned short *)(S.arg + Sc);
+    S.path = S.arg + Sc;
     S.wl0 = S.path + (size_t)Sc * kMaxHops;
     S.wl1 = S.wl0 + Sc;
     unsigned char *c = SC.cold_smem ? smem_raw + o_cold
@@ -166,7 +177,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
                                           (size_t)crank * (((size_t)Sc * kSlotColdBytes + 255) / 256 * 256);
     S.rem = (double *)c;
     S.tl = S.rem + Sc;
-    S.succ_cnt = (int *)(S.tl + Sc);
+    S.flow = (int *)(S.tl + Sc);
+    S.succ_cnt = S.flow + Sc;
     S.succ0 = S.succ_cnt + Sc;
     S.succ1 = S.succ0 + Sc;
     S.freeq = S.succ1 + Sc;
@@ -218,13 +230,19 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     for (int l = tid; l < L; l += NT) {
       beatf[l] = 0;
       csolve[l] = 0;
+      if (REPL) {
+        sh_loc[l] = 0;
+        sh0_loc[l] = 0;
+        chg_loc[l] = 0;
+        comp_loc[l] = (unsigned short)lcomp[l];
+      }
       if (AGG) {
         dcap_loc[l] = 0;
         dn_loc[l] = 0;
       }
     }
     for (int s = tid; s < Sc; s += NT) {
-      S.flow[s] = -1;
+      S.bn[s] = -3;
       S.tc[s] = kInf;
     }
     if (tid < M_NCTL) ctl[tid] = 0;
@@ -235,7 +253,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       S.flow[slot] = f;
       S.rem[slot] = r.bytes;
       S.bn[slot] = -2;
-      S.comp[slot] = r.comp;
+      S.comp[slot] = (unsigned short)r.comp;
 #pragma unroll
       for (int h = 0; h < kMaxHops; ++h)
         S.path[slot * kMaxHops + h] = r.path[h] < 0 ? kNoLink : (unsigned short)r.path[h];
@@ -287,6 +305,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         LinkA *a = LA(l);
         atomicAdd(&a->n0, delta);
         a->chg = solve;
+        if (REPL)
+          for (int r = 0; r < CS; ++r) cluster.map_shared_rank(chg_loc, (unsigned)r)[l] = solve;
       };
       auto mark_comp = [&](int c) {  // the component must be re-solved: tell every CTA
         for (int r = 0; r < CS; ++r) cluster.map_shared_rank(csolve, (unsigned)r)[c] = solve;
@@ -349,7 +369,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           touch_link(l, -1);
         }
         mark_comp(S.comp[s]);
-        S.flow[s] = -1;
+        S.bn[s] = -3;
         S.tc[s] = kInf;
         S.freeq[atomicAdd(&ctl[M_QTAIL], 1) % Sc] = s;
         atomicSub(&ctl[M_NACT], 1);
@@ -426,6 +446,11 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           lb[li].nw = la[li].n0;
         }
       }
+      if (REPL) {
+        for (int l = tid; l < L; l += NT)
+          if (LOG || csolve[comp_loc[l]] == solve) sh_loc[l] = sh0_loc[l];
+        __syncthreads();
+      }
 
       // ======== rates (a5-a7): parallel progressive filling over the components this event touched
       unsigned short *wl = S.wl0, *wl_next = S.wl1;
@@ -441,6 +466,19 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           const int l = p[h] = S.path[s * kMaxHops + h];
           sh[h] = LLONG_MAX;
           if (l == kNoLink) continue;
+          if (REPL) {
+            if (first && chg_loc[l] == solve) {  // flow count changed in this event: fetch it from the owner
+              LinkA *ap = LA(l);
+              const long long cap = ap->cap;
+              const int n0 = ap->n0;
+              sh[h] = fair_share(cap, n0);
+              sh0_loc[l] = sh[h];
+              sh_loc[l] = sh[h];
+            } else {
+              sh[h] = sh_loc[l];
+            }
+            continue;
+          }
           LinkA *ap = LA(l);
           const longlong2 a = *(const longlong2 *)ap;         // share0, cap
           const int4 ai = *((const int4 *)ap + 1);            // n0, chg, beat, solve
@@ -478,7 +516,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
             beatf[p[h]] = g;
             LA(p[h])->beat = g;
           }
-        S.arg[s] = arg;
+        S.arg[s] = (unsigned short)arg;
         return make_longlong2(best, (long long)arg);
       };
       auto freeze = [&](int s, int arg, long long rq) {  // a7 + R-LZ settle
@@ -520,8 +558,9 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         long long bk = LLONG_MAX;
         int bl = INT_MAX;
         for (int s = tid; s < hi; s += NT) {
-          if (S.flow[s] < 0) continue;
-          const bool in = S.bn[s] != -2 && (LOG || csolve[S.comp[s]] == solve);
+          const int bn0 = S.bn[s];
+          if (bn0 == -3) continue;
+          const bool in = bn0 != -2 && (LOG || csolve[S.comp[s]] == solve);
           if (!in) {
             mymin = dmin(mymin, S.tc[s]);
             continue;
@@ -573,10 +612,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           const int s = wl[i];
           const int arg = S.arg[s];
           LinkA *ap = LA(arg);
-          const long long share0 = ap->share0;
+          const long long share0 = REPL ? sh_loc[arg] : ap->share0;
           const int beat = ap->beat;
           long long rq = share0;
-          if (rounds > 1) {
+          if (!REPL && rounds > 1) {
             LinkB *bp = LB(arg);
             const long long sw = bp->sharew;
             if (bp->wsolve == solve) rq = sw;
@@ -633,6 +672,17 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         mymin = kInf;  // folded
         __syncthreads();
         if (!bc[7]) break;
+        if (REPL) {  // ---- R: owners recompute the share of their links debited in this round and tell every CTA
+          for (int li = tid; li < Lc; li += NT) {
+            if (lb[li].deb != g) continue;
+            const int nw = lb[li].nw;
+            if (nw <= 0) continue;
+            const long long shv = fair_share(lb[li].caprem, nw);
+            const int l = li * CS + crank;
+            for (int r = 0; r < CS; ++r) cluster.map_shared_rank(sh_loc, (unsigned)r)[l] = shv;
+          }
+          cluster.sync();  // ------------------------------------------------------------ cluster barrier 3
+        }
         // ---- V: the flows still listed vote on the new shares
         ++g;
         {
@@ -712,7 +762,7 @@ cudaError_t prepare(size_t smem) {
 template <bool LOG, bool AGG>
 cudaError_t launch_cluster_t(const DevTables &t, const int32_t *list, int n, int *ticket, const ClusterScratch &s,
                              int cluster_size, int n_clusters, cudaStream_t stream) {
-  const size_t smem = cluster_smem_bytes(t.n_links, cluster_size, s.Sc, AGG, s.cold_smem != 0, LOG);
+  const size_t smem = cluster_smem_bytes(t.n_links, cluster_size, s.Sc, AGG, s.cold_smem != 0, LOG, s.replicate != 0);
   cudaError_t e = prepare<LOG, AGG>(smem);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg{};

@@ -46,10 +46,12 @@ struct ClusterScratch {
   int64_t Sc;           // flow slots per CTA
   int aggregate;        // 1: a CTA pre-sums its debits per link in shared memory (16 bytes per link and CTA)
   int cold_smem;        // 1: the cold slot fields live in shared memory too
+  int replicate;        // 1: every CTA keeps a copy of the links' current fair shares (22 bytes per link and CTA)
 };
 constexpr int kClusterThreads = 512;
 // dynamic shared memory per CTA / global spill bytes per cluster
-size_t cluster_smem_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log);
+size_t cluster_smem_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log,
+                          bool replicate);
 size_t cluster_region_bytes(int64_t Sc, int cluster_size);
 // how many clusters of this size and shared-memory footprint can be resident at once (0: it cannot launch)
 cudaError_t cluster_max_clusters(int cluster_size, size_t smem, int *max_clusters);
