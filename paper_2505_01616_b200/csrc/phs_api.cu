@@ -350,7 +350,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)in.colls.size();
     sim->log_base[i + 1] = sim->log_base[i] + 2 * in.n_flows() + 2;
     succ_base[i + 1] = succ_base[i] + (int64_t)in.pred.size();
-    pc8_base[i + 1] = pc8_base[i] + (in.n_flows() + 3) / 4 * 4;
+    pc8_base[i + 1] = pc8_base[i] + (in.n_flows() + 7) / 8 * 4;  // 4 bits per flow, whole 32-bit words
   }
   sim->total_flows = sim->flow_base[B];
   sim->total_colls = sim->coll_base[B];
@@ -421,7 +421,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
       pc0[sim->flow_base[i] + f] = np;
       max_pred = std::max(max_pred, np);
-      pc8[pc8_base[i] + f] = (uint8_t)std::min(np, 255);
+      pc8[pc8_base[i] + f / 2] |= (uint8_t)(std::min(np, 15) << ((f & 1) * 4));
     }
     for (size_t c = 0; c < in.colls.size(); ++c) {
       coll_first[sim->coll_base[i] + c] = sim->flow_base[i] + in.colls[c].first_flow;
@@ -438,7 +438,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     d.n_colls = (int32_t)in.colls.size();
     sim->h_desc[i] = d;
   }
-  const bool pc8_ok = max_pred <= 255;
+  const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
 
   PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
   PHS_CUDA(sim->d_rec.upload(rec, st));
@@ -477,29 +477,41 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     int64_t bound = 32;  // slots an instance can need (Instance::slot_bound)
     for (int i = 0; i < B; ++i) bound = std::max(bound, sim->inst[i].slot_bound());
     const int need = (int)std::min<int64_t>(std::min<int64_t>(maxF, bound), 1 << 16);
-    for (; want >= 1; --want) {
-      const size_t budget = std::min(smem_max, per_sm / want - 1024);
-      const int pcf = pc8_ok && cta_smem_bytes(L, need, (int)maxF, log) <= budget ? (int)maxF : 0;
-      if (cta_smem_bytes(L, 32, pcf, log) > budget) continue;
-      int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
-      if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
-      hi = (hi + 31) / 32 * 32;
-      while (lo < hi) {  // largest multiple of 32 that fits the budget
-        const int mid = ((lo + hi + 32) / 64) * 32;
-        if (cta_smem_bytes(L, mid, pcf, log) <= budget)
-          lo = mid;
-        else
-          hi = mid - 32;
+    // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
+    // predecessor counters on chip; returns 0 if not even one fits
+    auto fit = [&](bool pcs, int *slots_out) {
+      const int pcf = pcs ? (int)maxF : 0;
+      for (int w = want; w >= 1; --w) {
+        const size_t budget = std::min(smem_max, per_sm / w - 1024);
+        if (cta_smem_bytes(L, 32, pcf, log) > budget) continue;
+        int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
+        if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
+        hi = (hi + 31) / 32 * 32;
+        while (lo < hi) {  // largest multiple of 32 that fits the budget
+          const int mid = ((lo + hi + 32) / 64) * 32;
+          if (cta_smem_bytes(L, mid, pcf, log) <= budget)
+            lo = mid;
+          else
+            hi = mid - 32;
+        }
+        if (lo >= need || w == 1 || sim->policy_slots > 0) {
+          if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
+          *slots_out = lo;
+          return w;
+        }
       }
-      if (lo >= need || want == 1 || sim->policy_slots > 0) {
-        if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
-        sim->cta.threads = threads;
-        sim->cta.slots = lo;
-        sim->cta.pc_flows = pcf;
-        sim->cta.smem = cta_smem_bytes(L, lo, pcf, log);
-        sim->cta.log = log;
-        break;
-      }
+      return 0;
+    };
+    int slots_p = 0, slots_n = 0;
+    const int w_p = pc8_ok ? fit(true, &slots_p) : 0, w_n = fit(false, &slots_n);
+    // counters on chip save an L2 round trip per release: worth one resident CTA less
+    const bool pcs = w_p > 0 && slots_p >= std::min(need, slots_n) && w_p >= w_n - 1;
+    if (pcs || w_n > 0) {
+      sim->cta.threads = threads;
+      sim->cta.slots = pcs ? slots_p : slots_n;
+      sim->cta.pc_flows = pcs ? (int)maxF : 0;
+      sim->cta.smem = cta_smem_bytes(L, sim->cta.slots, sim->cta.pc_flows, log);
+      sim->cta.log = log;
     }
   }
   if (sim->cta.slots > 0) {

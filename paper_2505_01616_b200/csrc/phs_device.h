@@ -12,7 +12,7 @@ struct DevTables {
   const FlowRec *rec;        // [F_total]
   const int32_t *succ;       // successor CSR values (instance-relative flow ids)
   const int32_t *pred_cnt0;  // [F_total] number of predecessors
-  const uint8_t *pred_cnt0_u8;  // same as bytes (per-instance slices 4-byte aligned), or nullptr if a count > 255
+  const uint8_t *pred_cnt0_u8;  // same, packed 4 bits per flow (per-instance slices 4-byte aligned); unused if a count > 15
   const int64_t *capq;       // [B][n_links] link capacity in rate quanta
   const int32_t *lcomp;      // [B][n_links] static component (representative link) of every link
   int32_t *pred_cnt;         // [F_total] outstanding predecessors (dynamic)

@@ -39,7 +39,7 @@ struct InstDesc {
   int64_t succ_base;  // first entry of the instance's slice of succ[]
   int64_t log_base;   // first row of the instance's event log slice (capacity 2F+2 rows), -1 if disabled
   int64_t coll_base;  // first entry in the per-collective arrays
-  int64_t pc8_base;   // first byte of the instance's slice of pred_cnt0_u8 (4-byte aligned), -1 if unused
+  int64_t pc8_base;   // first byte of the instance's slice of the packed predecessor counters (4-byte aligned)
   int32_t n_flows;
   int32_t n_colls;
 };

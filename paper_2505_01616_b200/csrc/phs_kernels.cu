@@ -22,6 +22,7 @@
 #include <cuda_runtime.h>
 
 #include <climits>
+#include <cstdio>
 
 #include "phs_device.h"
 #include "phs_devutil.cuh"
@@ -51,7 +52,7 @@ struct CtaSmem {
   uint4 *s_path;  // the path as 8 x uint16 (kNoLink = none): one 16-byte load brings the whole path
   int *s_succ_cnt, *s_succ0, *s_succ1;
   int *free_q;    // FIFO ring of free slots
-  unsigned *pc8;  // [(PCF+3)/4] predecessor counters, one byte per flow
+  unsigned *pc8;  // [(PCF+7)/8] predecessor counters, 4 bits per flow
   double *red;    // [32] per-warp partial minima
   long long *red_key;  // [32] LOG: per-warp partial first_bneck key
   int *red_id;    // [32]
@@ -101,7 +102,7 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   PHS_TAKE(s_succ0, int, S)
   PHS_TAKE(s_succ1, int, S)
   PHS_TAKE(free_q, int, S)
-  PHS_TAKE(pc8, unsigned, (pcf + 3) / 4)
+  PHS_TAKE(pc8, unsigned, (pcf + 7) / 8)
   PHS_TAKE(red_id, int, 32)
   PHS_TAKE(ctl, int, 32)
 #undef PHS_TAKE
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
     if (tid < C_NCTL) S.ctl[tid] = 0;
     if (PCS) {
       const unsigned *src = (const unsigned *)(T.pred_cnt0_u8 + D.pc8_base);
-      for (int w = tid; w < (F + 3) / 4; w += NT) S.pc8[w] = src[w];
+      for (int w = tid; w < (F + 7) / 8; w += NT) S.pc8[w] = src[w];
     }
     __syncthreads();
 
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
       for (int f = tid; f < F; f += NT) {
         int pc;
         if (PCS) {
-          pc = (S.pc8[f >> 2] >> ((f & 3) * 8)) & 0xff;
+          pc = (S.pc8[f >> 3] >> ((f & 7) * 4)) & 0xf;
         } else {
           pc = pc0[f];
           pred_cnt[f] = pc;
@@ -241,6 +242,13 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
     int max_active = 0, max_pending = 0;
     int status = PHS_OK;
     int first_bneck = -1;
+#ifdef PHS_PHASE_CLOCKS
+    long long pc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pt_ = clock64();
+// BAR.SYNC does not block at issue: read a barrier-protected word before taking the clock
+#define PHS_TICK(i) { if (*(volatile int *)&S.ctl[C_HI] < -5) pt_ = 0; const long long t_ = clock64(); pc_[i] += t_ - pt_; pt_ = t_; }
+#else
+#define PHS_TICK(i)
+#endif
 
     for (;;) {
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
@@ -274,9 +282,9 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
       };
       auto pred_done = [&](int gf) {  // S4.5: pred_cnt--; true when it reaches 0
         if (PCS) {
-          const unsigned sh = (unsigned)(gf & 3) * 8u;
-          const unsigned old = atomicSub(&S.pc8[gf >> 2], 1u << sh);
-          return ((old >> sh) & 0xffu) == 1u;
+          const unsigned sh = (unsigned)(gf & 7) * 4u;  // a counter is >= 1 here, so the subtraction never borrows
+          const unsigned old = atomicSub(&S.pc8[gf >> 3], 1u << sh);
+          return ((old >> sh) & 0xfu) == 1u;
         }
         return atomicSub(&pred_cnt[gf], 1) == 1;
       };
@@ -337,7 +345,9 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
           for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
         }
       }
+      PHS_TICK(0)
       __syncthreads();
+      PHS_TICK(1)
       now = t_next;
       if (tid == 0) {
         if (S.ctl[C_QHEAD] > qtail) S.ctl[C_QHEAD] = qtail;  // pops that found the queue empty took fresh slots
@@ -448,7 +458,9 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
           }
         }
       }
+      PHS_TICK(2)
       __syncthreads();
+      PHS_TICK(3)
       bool left = false;
       {  // ---- F0: unbeaten arg-min links freeze their flows (a7); fold the slot times (a8)
         double mymin = kInf;
@@ -466,7 +478,9 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
         const double wm = warp_min_nonneg(mymin);
         if (lane == 0) S.red[warp] = wm;
       }
+      PHS_TICK(4)
       left = __syncthreads_or(left);
+      PHS_TICK(5)
       if (left) {
         // ---- I: working capacities of the links of this solve (idempotent stores)
         for (int s = tid; s < hi; s += NT) {
@@ -582,7 +596,13 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
       }
       sum_active += nA;
       sum_rounds += rounds;
+      PHS_TICK(6)
     }
+#ifdef PHS_PHASE_CLOCKS
+    if ((tid == 0 || tid == NT - 1) && inst < 2)
+      printf("inst %d tid %d events %d cycles: X %lld waitX %lld V0 %lld wait1 %lld F0 %lld wait2 %lld rest %lld\n", inst, tid,
+             ev, pc_[0], pc_[1], pc_[2], pc_[3], pc_[4], pc_[5], pc_[6]);
+#endif
     if (tid == 0) {
       if (status == PHS_OK && S.ctl[C_DONE] < F) status = PHS_ECYCLE;  // WAITING flows left over
       InstResult r;
