@@ -273,7 +273,8 @@ def run_ours(args, rank, world, local_rank):
         "config": {"workload": args.workload, "instances_per_gpu": count, "flows_per_gpu": flows,
                    "kernel_paths": paths, "l2": "flushed between timed steps (256 MiB write)",
                    "events_per_step": counters["n_events"], "parallel_rounds_per_step": counters["sum_par_rounds"],
-                   "max_active_flows": counters["max_active"], "max_state_slots": counters["max_slots"]},
+                   "max_active_flows": counters["max_active"], "max_state_slots": counters["max_slots"],
+                   "cluster_size": counters["cluster_size"], "clusters_resident": counters["clusters_resident"]},
         "collectives_per_sec": colls_all * args.steps / (ms_total * 1e-3),
         "sim_events_per_sec": counters["n_events"] * world * args.steps / (ms_total * 1e-3),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),

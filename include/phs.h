@@ -81,6 +81,8 @@ typedef struct {
   int64_t h2d_bytes;     /* bytes phs_finalize copied to the device                                       */
   int32_t max_active;    /* largest number of simultaneously ACTIVE flows in one instance                 */
   int32_t max_slots;     /* largest number of state slots (PENDING + ACTIVE flows) one instance ever used */
+  int32_t cluster_size;  /* CTAs per cluster of the cluster path in the last run (0: path not used)            */
+  int32_t clusters_resident; /* clusters of that size the device keeps resident at once                        */
   double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
                          /* the run's stream), excluding the result copies                                */
 } phs_counters;

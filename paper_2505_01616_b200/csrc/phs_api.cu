@@ -90,7 +90,7 @@ struct phs_sim {
   DevBuf<int32_t> d_clist, d_lcomp;
   DevBuf<int> d_cticket;
   int64_t scratch_Sc = 0, cluster_scale = 1;
-  int scratch_regions = 0, scratch_cs = 0;
+  int scratch_regions = 0, scratch_cs = 0, clusters_resident = 0;
 
   // launch configuration of the CTA path
   CtaLaunch cta{};
@@ -610,6 +610,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   if (!sim->d_cticket.p) PHS_CUDA(sim->d_cticket.alloc(1));
   sim->scratch_Sc = Sc;
   sim->scratch_cs = cs;
+  sim->clusters_resident = max_clusters;
   std::vector<int32_t> sorted(list);
   std::stable_sort(sorted.begin(), sorted.end(),
                    [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
@@ -774,6 +775,8 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
     c.max_active = std::max(c.max_active, sim->h_res[i].max_active);
     c.max_slots = std::max(c.max_slots, sim->h_res[i].max_slots);
   }
+  c.cluster_size = sim->scratch_cs;
+  c.clusters_resident = sim->clusters_resident;
   c.n_flow_events = 2 * sim->total_flows;
   c.n_kernel_launches = sim->n_launches;
   c.h2d_bytes = sim->h2d_bytes;
