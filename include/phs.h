@@ -124,6 +124,12 @@ phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);
  * (active flows / pending flows per instance); an instance that exceeds it is re-run on the cluster path. */
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
 
+/* Decomposition (default on).  An instance whose flows fall into groups that share no link and no dependency is
+ * simulated as independent units, one CTA / cluster each; under reading R-LZ the results are
+ * bit-identical to simulating the instance as a whole.  Off: one unit per instance.  The event log needs the
+ * instance-wide event sequence, so enabling it turns decomposition off.  Must precede phs_finalize. */
+phs_status phs_set_decomposition(phs_sim *sim, int32_t enable);
+
 /* Builds the device-resident tables (flow records, flow->link CSR, successor CSR, capacities) and copies them
  * to the current CUDA device on `cuda_stream` (cudaStream_t; NULL = default stream).  After this call the
  * instance set is frozen (adds return PHS_ESTATE).  phs_run calls it implicitly if needed. */

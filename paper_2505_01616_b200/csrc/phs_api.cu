@@ -69,8 +69,16 @@ struct phs_sim {
   std::vector<int64_t> flow_base;  // [B+1]
   std::vector<int64_t> coll_base;  // [B+1]
   std::vector<int64_t> log_base;   // [B+1] (only with the event log)
-  std::vector<InstDesc> h_desc;
-  std::vector<InstResult> h_res;
+  struct Unit {  // what one CTA / cluster simulates (see InstDesc)
+    int32_t inst, n_flows, n_links;
+    int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (Instance::slot_bound, per unit)
+    int64_t initial;  // flows without predecessors: PENDING from t = 0
+  };
+  std::vector<Unit> units;
+  std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
+  bool decompose = true;
+  std::vector<InstDesc> h_desc;  // per unit
+  std::vector<InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first
   std::vector<int32_t> cluster_list;  // instances that go (or fell back) to the cluster path
   int64_t total_flows = 0, total_colls = 0;
@@ -78,7 +86,8 @@ struct phs_sim {
   // ---- device tables
   DevBuf<InstDesc> d_desc;
   DevBuf<FlowRec> d_rec;
-  DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n;
+  DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
+  DevBuf<uint32_t> d_fmap;
   DevBuf<uint8_t> d_pc8;
   DevBuf<int64_t> d_capq, d_coll_first;
   DevBuf<double> d_tdone, d_coll_t;
@@ -250,6 +259,13 @@ phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
   return PHS_OK;
 }
 
+phs_status phs_set_decomposition(phs_sim *sim, int32_t enable) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (sim->finalized) return fail(PHS_ESTATE, "decomposition must be chosen before phs_finalize");
+  sim->decompose = enable != 0;
+  return PHS_OK;
+}
+
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out) {
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
@@ -341,103 +357,207 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
 
   sim->flow_base.assign(B + 1, 0);
   sim->coll_base.assign(B + 1, 0);
-  sim->log_base.assign(B + 1, 0);
-  std::vector<int64_t> succ_base(B + 1, 0), pc8_base(B + 1, 0);
-  int max_pred = 0;
   for (int i = 0; i < B; ++i) {
-    const Instance &in = sim->inst[i];
-    sim->flow_base[i + 1] = sim->flow_base[i] + in.n_flows();
-    sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)in.colls.size();
-    sim->log_base[i + 1] = sim->log_base[i] + 2 * in.n_flows() + 2;
-    succ_base[i + 1] = succ_base[i] + (int64_t)in.pred.size();
-    pc8_base[i + 1] = pc8_base[i] + (in.n_flows() + 7) / 8 * 4;  // 4 bits per flow, whole 32-bit words
+    sim->flow_base[i + 1] = sim->flow_base[i] + sim->inst[i].n_flows();
+    sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)sim->inst[i].colls.size();
   }
   sim->total_flows = sim->flow_base[B];
   sim->total_colls = sim->coll_base[B];
   const int64_t Ft = sim->total_flows;
+  if (Ft >= 0x7fffffffLL) return fail(PHS_ERANGE, "more than 2^31 - 1 flows in one batch");
+  const bool split = sim->decompose && !sim->want_log;  // the event log is an instance-wide sequence
 
+  // ---- simulation units (a9).  Flows that share a link, directly or through a chain of flows, and flows joined by
+  // a dependency evolve together; such a group shares nothing with the rest of its instance, so (reading R-LZ) it
+  // can be simulated on its own with bit-identical results.  Every unit gets dense local flow and link ids.
   std::vector<FlowRec> rec((size_t)Ft);
-  std::vector<int32_t> succ((size_t)succ_base[B]), pc0((size_t)Ft);
-  std::vector<uint8_t> pc8((size_t)pc8_base[B], 0);
-  std::vector<int64_t> capq((size_t)B * L), coll_first((size_t)sim->total_colls);
-  std::vector<int32_t> lcomp((size_t)B * L);
+  std::vector<int32_t> succ, pc0((size_t)Ft), lcomp, linkid;
+  std::vector<uint32_t> fmap((size_t)Ft);
+  std::vector<uint8_t> pc8;
+  std::vector<int64_t> capq, coll_first((size_t)sim->total_colls);
   std::vector<int32_t> coll_n((size_t)sim->total_colls);
-  sim->h_desc.resize(B);
+  sim->units.clear();
+  sim->unit_first.assign(B + 1, 0);
+  sim->h_desc.clear();
+  int max_pred = 0;
+  int64_t flow_cursor = 0, log_cursor = 0;
+  std::vector<int64_t> capq_inst((size_t)L);
+  std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
   for (int i = 0; i < B; ++i) {
     const Instance &in = sim->inst[i];
     const int64_t F = in.n_flows();
+    sim->unit_first[i] = (int32_t)sim->units.size();
     // capacities -> rate quanta (floor); every fair share must stay >= 1 quantum
     for (int l = 0; l < L; ++l) {
       const double c = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
       const int64_t q = (int64_t)std::floor(c * 1048576.0);
       if (q < F + 1) return fail(PHS_ERANGE, "a link capacity is below (#flows + 1) rate quanta of 2^-20 byte/s");
-      capq[(size_t)i * L + l] = q;
-    }
-    // successor CSR = transpose of the pred lists (counting sort by predecessor)
-    std::vector<uint32_t> soff((size_t)F + 1, 0);
-    for (int32_t p : in.pred) soff[(size_t)p + 1]++;
-    for (int64_t f = 0; f < F; ++f) soff[f + 1] += soff[f];
-    int32_t *sdst = succ.data() + succ_base[i];
-    {
-      std::vector<uint32_t> cur(soff.begin(), soff.end() - 1);
-      for (int64_t f = 0; f < F; ++f)
-        for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
-    }
-    // static link components (union-find over the links, joined by every flow's path); the representative is
-    // the smallest link id, so component ids are link ids
-    std::vector<int32_t> parent((size_t)L);
-    std::iota(parent.begin(), parent.end(), 0);
-    auto find = [&](int32_t x) {
-      while (parent[x] != x) {
-        parent[x] = parent[parent[x]];
-        x = parent[x];
-      }
-      return x;
-    };
-    for (int64_t f = 0; f < F; ++f)
-      for (uint32_t e = in.path_off[f] + 1; e < in.path_off[f + 1]; ++e) {
-        const int32_t a = find(in.path[in.path_off[f]]), b = find(in.path[e]);
-        if (a != b) parent[std::max(a, b)] = std::min(a, b);
-      }
-    for (int l = 0; l < L; ++l) lcomp[(size_t)i * L + l] = find(l);
-    FlowRec *r = rec.data() + sim->flow_base[i];
-    for (int64_t f = 0; f < F; ++f) {
-      FlowRec x;
-      x.bytes = in.bytes[f];
-      x.start = in.start[f];
-      x.lat = in.lat[f];
-      const uint32_t p0 = in.path_off[f], p1 = in.path_off[f + 1];
-      for (int h = 0; h < kMaxHops; ++h) x.path[h] = p0 + h < p1 ? in.path[p0 + h] : -1;
-      x.succ_cnt = (int32_t)(soff[f + 1] - soff[f]);
-      if (x.succ_cnt <= 2) {
-        x.succ_in[0] = x.succ_cnt > 0 ? sdst[soff[f]] : -1;
-        x.succ_in[1] = x.succ_cnt > 1 ? sdst[soff[f] + 1] : -1;
-      } else {
-        x.succ_in[0] = (int32_t)soff[f];
-        x.succ_in[1] = -1;
-      }
-      x.comp = p0 < p1 ? find(in.path[p0]) : 0;
-      r[f] = x;
-      const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
-      pc0[sim->flow_base[i] + f] = np;
-      max_pred = std::max(max_pred, np);
-      pc8[pc8_base[i] + f / 2] |= (uint8_t)(std::min(np, 15) << ((f & 1) * 4));
+      capq_inst[l] = q;
     }
     for (size_t c = 0; c < in.colls.size(); ++c) {
       coll_first[sim->coll_base[i] + c] = sim->flow_base[i] + in.colls[c].first_flow;
       coll_n[sim->coll_base[i] + c] = in.colls[c].n_flows;
     }
-    InstDesc d;
-    d.flow_base = sim->flow_base[i];
-    d.path_base = 0;
-    d.succ_base = succ_base[i];
-    d.log_base = sim->want_log ? sim->log_base[i] : -1;
-    d.coll_base = sim->coll_base[i];
-    d.pc8_base = pc8_base[i];
-    d.n_flows = (int32_t)F;
-    d.n_colls = (int32_t)in.colls.size();
-    sim->h_desc[i] = d;
+    // successor CSR = transpose of the pred lists (counting sort by predecessor)
+    std::vector<uint32_t> soff((size_t)F + 1, 0);
+    std::vector<int32_t> sdst(in.pred.size());
+    for (int32_t p : in.pred) soff[(size_t)p + 1]++;
+    for (int64_t f = 0; f < F; ++f) soff[f + 1] += soff[f];
+    {
+      std::vector<uint32_t> cur(soff.begin(), soff.end() - 1);
+      for (int64_t f = 0; f < F; ++f)
+        for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
+    }
+    // static link components (union-find over the links, joined by every flow's path; the representative is the
+    // smallest link id), and on top of them the units (link components joined by dependencies)
+    std::iota(parent.begin(), parent.end(), 0);
+    auto find_in = [](std::vector<int32_t> &par, int32_t x) {
+      while (par[x] != x) {
+        par[x] = par[par[x]];
+        x = par[x];
+      }
+      return x;
+    };
+    auto unite = [&](std::vector<int32_t> &par, int32_t a, int32_t b) {
+      a = find_in(par, a);
+      b = find_in(par, b);
+      if (a != b) par[std::max(a, b)] = std::min(a, b);
+    };
+    for (int64_t f = 0; f < F; ++f)
+      for (uint32_t e = in.path_off[f] + 1; e < in.path_off[f + 1]; ++e)
+        unite(parent, in.path[in.path_off[f]], in.path[e]);
+    uparent = parent;
+    for (int64_t f = 0; f < F; ++f)
+      for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e)
+        unite(uparent, in.path[in.path_off[f]], in.path[in.path_off[in.pred[e]]]);
+    // unit of every flow: groups in order of first appearance; groups below 64 flows share bins of up to 256
+    std::vector<int32_t> unit_of((size_t)F, 0);
+    int32_t n_units = F > 0 ? 1 : 0;
+    if (split && F > 0) {
+      std::vector<int32_t> group_of_root((size_t)L, -1), gsize;
+      for (int64_t f = 0; f < F; ++f) {
+        const int32_t r = find_in(uparent, in.path[in.path_off[f]]);
+        if (group_of_root[r] < 0) {
+          group_of_root[r] = (int32_t)gsize.size();
+          gsize.push_back(0);
+        }
+        unit_of[f] = group_of_root[r];
+        gsize[unit_of[f]]++;
+      }
+      std::vector<int32_t> unit_of_group(gsize.size());
+      n_units = 0;
+      int32_t bin = -1, bin_flows = 0;
+      for (size_t g = 0; g < gsize.size(); ++g) {
+        if (gsize[g] >= 64) {
+          unit_of_group[g] = n_units++;
+        } else {
+          if (bin < 0 || bin_flows >= 256) {
+            bin = n_units++;
+            bin_flows = 0;
+          }
+          unit_of_group[g] = bin;
+          bin_flows += gsize[g];
+        }
+      }
+      for (int64_t f = 0; f < F; ++f) unit_of[f] = unit_of_group[unit_of[f]];
+    }
+    // flows of every unit in ascending flow id; local flow ids
+    std::vector<std::vector<int32_t>> uflows((size_t)n_units);
+    std::vector<int32_t> flow_loc((size_t)F);
+    for (int64_t f = 0; f < F; ++f) {
+      flow_loc[f] = (int32_t)uflows[unit_of[f]].size();
+      uflows[unit_of[f]].push_back((int32_t)f);
+    }
+    // slots a unit can need: Instance::slot_bound, per unit (a collective and its `after` chain lie in one unit)
+    std::vector<int64_t> ubound((size_t)n_units, 0), uinit((size_t)n_units, 0);
+    {
+      for (int u = 0; u < n_units; ++u) ubound[u] = (int64_t)uflows[u].size();
+      std::vector<int64_t> chain_max(in.colls.size(), 0);
+      for (size_t c = 0; c < in.colls.size(); ++c) {
+        if (in.colls[c].n_flows == 0) continue;
+        ubound[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
+        const int64_t need = in.colls[c].kind == PHS_ALLTOALL
+                                 ? in.colls[c].n_flows
+                                 : std::min<int64_t>(in.colls[c].n_flows, 2 * (int64_t)in.colls[c].n_ranks);
+        chain_max[in.colls[c].chain] = std::max(chain_max[in.colls[c].chain], need);
+      }
+      for (size_t c = 0; c < in.colls.size(); ++c)
+        if (chain_max[c] > 0) ubound[unit_of[in.colls[c].first_flow]] += chain_max[c];
+      for (int64_t f = 0; f < F; ++f) uinit[unit_of[f]] += in.pred_off[f + 1] == in.pred_off[f];
+    }
+    if (n_units == 0) {  // an instance without flows is one empty unit
+      n_units = 1;
+      uflows.resize(1);
+      ubound.assign(1, 0);
+      uinit.assign(1, 0);
+    }
+    for (int u = 0; u < n_units; ++u) {
+      const std::vector<int32_t> &fl = uflows[u];
+      // links of the unit, ascending; an undivided instance keeps the whole topology (local id = topology id)
+      std::vector<int32_t> links;
+      if (n_units == 1) {
+        links.resize((size_t)L);
+        std::iota(links.begin(), links.end(), 0);
+      } else {
+        for (int32_t f : fl)
+          for (uint32_t e = in.path_off[f]; e < in.path_off[f + 1]; ++e) links.push_back(in.path[e]);
+        std::sort(links.begin(), links.end());
+        links.erase(std::unique(links.begin(), links.end()), links.end());
+      }
+      for (size_t k = 0; k < links.size(); ++k) link_loc[links[k]] = (int32_t)k;
+      InstDesc d;
+      d.flow_base = flow_cursor;
+      d.link_base = (int64_t)capq.size();
+      d.succ_base = (int64_t)succ.size();
+      d.log_base = sim->want_log ? log_cursor : -1;
+      d.pc8_base = (int64_t)pc8.size();
+      d.n_flows = (int32_t)fl.size();
+      d.n_links = (int32_t)links.size();
+      for (int32_t l : links) {
+        capq.push_back(capq_inst[l]);
+        lcomp.push_back(link_loc[find_in(parent, l)]);  // the smallest link of a component is in the unit too
+        linkid.push_back(l);
+      }
+      pc8.resize(pc8.size() + (fl.size() + 7) / 8 * 4, 0);
+      for (size_t k = 0; k < fl.size(); ++k) {
+        const int32_t f = fl[k];
+        FlowRec x;
+        x.bytes = in.bytes[f];
+        x.start = in.start[f];
+        x.lat = in.lat[f];
+        const uint32_t p0 = in.path_off[f], p1 = in.path_off[f + 1];
+        for (int h = 0; h < kMaxHops; ++h) x.path[h] = p0 + h < p1 ? link_loc[in.path[p0 + h]] : -1;
+        x.succ_cnt = (int32_t)(soff[f + 1] - soff[f]);
+        if (x.succ_cnt <= 2) {
+          x.succ_in[0] = x.succ_cnt > 0 ? flow_loc[sdst[soff[f]]] : -1;
+          x.succ_in[1] = x.succ_cnt > 1 ? flow_loc[sdst[soff[f] + 1]] : -1;
+        } else {
+          x.succ_in[0] = (int32_t)((int64_t)succ.size() - d.succ_base);
+          x.succ_in[1] = -1;
+          for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) succ.push_back(flow_loc[sdst[e]]);
+        }
+        x.comp = p0 < p1 ? link_loc[find_in(parent, in.path[p0])] : 0;
+        rec[(size_t)flow_cursor + k] = x;
+        fmap[(size_t)flow_cursor + k] = (uint32_t)(sim->flow_base[i] + f);
+        const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
+        pc0[(size_t)flow_cursor + k] = np;
+        max_pred = std::max(max_pred, np);
+        pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
+      }
+      flow_cursor += (int64_t)fl.size();
+      log_cursor += 2 * (int64_t)fl.size() + 2;
+      sim->h_desc.push_back(d);
+      phs_sim::Unit un;
+      un.inst = i;
+      un.n_flows = d.n_flows;
+      un.n_links = d.n_links;
+      un.bound = ubound[u];
+      un.initial = uinit[u];
+      sim->units.push_back(un);
+    }
   }
+  sim->unit_first[B] = (int32_t)sim->units.size();
+  const int U = (int)sim->units.size();
   const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
 
   PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
@@ -445,56 +565,71 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   if (pc8_ok) PHS_CUDA(sim->d_pc8.upload(pc8, st));
   PHS_CUDA(sim->d_succ.upload(succ, st));
   PHS_CUDA(sim->d_pc0.upload(pc0, st));
+  PHS_CUDA(sim->d_fmap.upload(fmap, st));
   PHS_CUDA(sim->d_capq.upload(capq, st));
   PHS_CUDA(sim->d_lcomp.upload(lcomp, st));
+  PHS_CUDA(sim->d_linkid.upload(linkid, st));
   PHS_CUDA(sim->d_coll_first.upload(coll_first, st));
   PHS_CUDA(sim->d_coll_n.upload(coll_n, st));
   PHS_CUDA(sim->d_pred_cnt.alloc((size_t)Ft));
   PHS_CUDA(sim->d_tdone.alloc((size_t)Ft));
   PHS_CUDA(sim->d_bneck.alloc((size_t)Ft));
   PHS_CUDA(sim->d_coll_t.alloc((size_t)sim->total_colls));
-  PHS_CUDA(sim->d_res.alloc((size_t)B));
+  PHS_CUDA(sim->d_res.alloc((size_t)U));
   PHS_CUDA(sim->d_ticket.alloc(1));
-  if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)sim->log_base[B]));
-  sim->h_res.assign(B, InstResult{});
+  if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)log_cursor));
+  sim->h_res.assign(U, InstResult{});
 
-  // ---- a9: batch scheduler, static part.  Small instances -> one CTA each with shared-memory state, sized so
-  // that enough CTAs are resident per SM to cover the batch; instances whose link state alone does not fit go to
-  // the cluster path.  Instances that overflow their shared-memory slots at run time are re-run on the cluster path.
+  // ---- a9: batch scheduler, static part.  A unit whose state fits the shared memory of one SM goes to the CTA
+  // path (one launch configuration, sized for the largest such unit, with as many CTAs resident per SM as fit);
+  // the others go to the cluster path.  Units that overflow their slots at run time move to the cluster path.
   const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin;
   const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
-  int64_t maxF = 0;
-  for (int i = 0; i < B; ++i) maxF = std::max<int64_t>(maxF, sim->inst[i].n_flows());
-  const int threads = L <= 320 ? 128 : 256;  // measured on B200: 128 is best for cfg3-sized instances, 256+ for cfg1
   const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
   sim->cta = CtaLaunch{};
-  if (sim->policy_path != 2 && maxF > 0) {
-    // resident CTAs per SM wanted: enough to cover the batch, at most what the thread count allows; fewer if the
-    // slots would otherwise not hold a typical active set (min(F, 256) flows)
-    int want = std::max(1, std::min(2048 / threads / 2, (B + sim->sm_count - 1) / sim->sm_count));
-    int64_t bound = 32;  // slots an instance can need (Instance::slot_bound)
-    for (int i = 0; i < B; ++i) bound = std::max(bound, sim->inst[i].slot_bound());
-    const int need = (int)std::min<int64_t>(std::min<int64_t>(maxF, bound), 1 << 16);
+  auto need_of = [&](const phs_sim::Unit &u) {
+    return (int)std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(u.n_flows, 1), std::max<int64_t>(u.bound, 32)), 1 << 16);
+  };
+  std::vector<int32_t> cand;
+  for (int u = 0; u < U; ++u) {
+    const phs_sim::Unit &un = sim->units[u];
+    if (un.n_flows == 0) continue;  // nothing to simulate; its result block stays zero (status OK)
+    if (sim->policy_path == 2 || un.n_links >= 65535 ||
+        cta_smem_bytes(un.n_links, (need_of(un) + 31) / 32 * 32, 0, log) > smem_max)
+      sim->cluster_list.push_back(u);
+    else
+      cand.push_back(u);
+  }
+  while (!cand.empty()) {
+    int Lm = 1, need = 32;
+    int64_t maxF = 1;
+    for (int u : cand) {
+      Lm = std::max(Lm, sim->units[u].n_links);
+      need = std::max(need, need_of(sim->units[u]));
+      maxF = std::max<int64_t>(maxF, sim->units[u].n_flows);
+    }
+    const int threads = Lm <= 320 ? 128 : 256;  // measured on B200: 128 for cfg3-sized units, 256 for cfg1-sized
+    const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
     // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
     // predecessor counters on chip; returns 0 if not even one fits
     auto fit = [&](bool pcs, int *slots_out) {
       const int pcf = pcs ? (int)maxF : 0;
       for (int w = want; w >= 1; --w) {
         const size_t budget = std::min(smem_max, per_sm / w - 1024);
-        if (cta_smem_bytes(L, 32, pcf, log) > budget) continue;
+        if (cta_smem_bytes(Lm, 32, pcf, log) > budget) continue;
         int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
         if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
         hi = (hi + 31) / 32 * 32;
         while (lo < hi) {  // largest multiple of 32 that fits the budget
           const int mid = ((lo + hi + 32) / 64) * 32;
-          if (cta_smem_bytes(L, mid, pcf, log) <= budget)
+          if (cta_smem_bytes(Lm, mid, pcf, log) <= budget)
             lo = mid;
           else
             hi = mid - 32;
         }
-        if (lo >= need || w == 1 || sim->policy_slots > 0) {
+        if (lo >= need || (w == 1 && sim->policy_path == 1) || sim->policy_slots > 0) {
           if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
           *slots_out = lo;
           return w;
@@ -504,29 +639,36 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     };
     int slots_p = 0, slots_n = 0;
     const int w_p = pc8_ok ? fit(true, &slots_p) : 0, w_n = fit(false, &slots_n);
+    if (w_p == 0 && w_n == 0) {
+      // the largest links x slots combination does not fit one SM: the unit with the most flows goes to a cluster
+      auto big = std::max_element(cand.begin(), cand.end(), [&](int a, int b) {
+        return sim->units[a].n_flows < sim->units[b].n_flows;
+      });
+      sim->cluster_list.push_back(*big);
+      cand.erase(big);
+      continue;
+    }
     // counters on chip save an L2 round trip per release: worth one resident CTA less
     const bool pcs = w_p > 0 && slots_p >= std::min(need, slots_n) && w_p >= w_n - 1;
-    if (pcs || w_n > 0) {
-      sim->cta.threads = threads;
-      sim->cta.slots = pcs ? slots_p : slots_n;
-      sim->cta.pc_flows = pcs ? (int)maxF : 0;
-      sim->cta.smem = cta_smem_bytes(L, sim->cta.slots, sim->cta.pc_flows, log);
-      sim->cta.log = log;
-    }
-  }
-  if (sim->cta.slots > 0) {
-    for (int i = 0; i < B; ++i) sim->order.push_back(i);
+    sim->cta.threads = threads;
+    sim->cta.slots = pcs ? slots_p : slots_n;
+    sim->cta.pc_flows = pcs ? (int)maxF : 0;
+    sim->cta.smem = cta_smem_bytes(Lm, sim->cta.slots, sim->cta.pc_flows, log);
+    sim->cta.log = log;
+    sim->cta.n_links = Lm;
+    sim->order = cand;
     std::stable_sort(sim->order.begin(), sim->order.end(),
-                     [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
+                     [&](int a, int b) { return sim->units[a].n_flows > sim->units[b].n_flows; });
     const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta.smem + 1024)), 2048 / threads));
-    sim->cta.grid = std::min(B, per * sim->sm_count);
+    sim->cta.grid = std::min((int)cand.size(), per * sim->sm_count);
     PHS_CUDA(sim->d_order.upload(sim->order, st));
-  } else {
-    for (int i = 0; i < B; ++i) sim->cluster_list.push_back(i);
+    break;
   }
+  std::sort(sim->cluster_list.begin(), sim->cluster_list.end());
   PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
   sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
-                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
+                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size() + linkid.size() +
+                              fmap.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
                              (capq.size() + coll_first.size()) * 8);
   PHS_CUDA(cudaEventCreate(&sim->ev0));
   PHS_CUDA(cudaEventCreate(&sim->ev1));
@@ -537,21 +679,23 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
 // ================================================================================================ run
 namespace {
 
-DevTables tables_of(phs_sim *sim) {
+DevTables tables_of(phs_sim *sim, int n_links) {
   DevTables t;
   t.inst = sim->d_desc.p;
   t.rec = sim->d_rec.p;
   t.succ = sim->d_succ.p;
   t.pred_cnt0 = sim->d_pc0.p;
   t.pred_cnt0_u8 = sim->d_pc8.p;
+  t.fmap = sim->d_fmap.p;
   t.capq = sim->d_capq.p;
   t.lcomp = sim->d_lcomp.p;
+  t.linkid = sim->d_linkid.p;
   t.pred_cnt = sim->d_pred_cnt.p;
   t.t_done = sim->d_tdone.p;
   t.bneck = sim->d_bneck.p;
   t.res = sim->d_res.p;
   t.log = sim->want_log ? sim->d_log.p : nullptr;
-  t.n_links = sim->fab->n_links();
+  t.n_links = n_links;
   return t;
 }
 
@@ -560,19 +704,17 @@ DevTables tables_of(phs_sim *sim) {
 // guess of how many flows are PENDING or ACTIVE at once (doubled after an overflow).
 phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, cudaStream_t st) {
   if (list.empty()) return PHS_OK;
-  const int L = sim->fab->n_links();
-  if (L >= 65535) return fail(PHS_ERANGE, "cluster path: topologies with 65535 or more links are not supported");
+  int L = 1;  // the shared-memory layout is sized for the unit with the most links
+  for (int u : list) L = std::max(L, sim->units[u].n_links);
+  if (L >= 65535) return fail(PHS_ERANGE, "cluster path: units with 65535 or more links are not supported");
   // slots needed per instance: every flow without predecessors is PENDING from t = 0; later, a ring collective
   // has at most one step in flight per rank plus the successors waiting out their latency, while an all-to-all
   // or a raw flow set can be in flight as a whole.  Start from a quarter of that bound; overflow doubles it.
-  int64_t maxF = 1, target = 64;
-  for (int i : list) {
-    const Instance &in = sim->inst[i];
-    int64_t bound = in.slot_bound(), initial = 0;
-    for (int64_t f = 0; f < in.n_flows(); ++f) initial += in.pred_off[f + 1] == in.pred_off[f];
-    maxF = std::max<int64_t>(maxF, in.n_flows());
-    target = std::max(target, std::max(initial, std::min(bound, bound * slot_scale / 4)));
-    if (slot_scale > 4) target = std::max(target, std::min<int64_t>(in.n_flows(), bound * slot_scale / 4));
+  int64_t target = 64;
+  for (int u : list) {
+    const phs_sim::Unit &un = sim->units[u];
+    target = std::max(target, std::max(un.initial, std::min(un.bound, un.bound * slot_scale / 4)));
+    if (slot_scale > 4) target = std::max(target, std::min<int64_t>(un.n_flows, un.bound * slot_scale / 4));
   }
   const size_t smem_max = sim->smem_optin - 4096;  // minus the kernel's static shared memory
   const bool log = sim->want_log;
@@ -613,7 +755,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   sim->clusters_resident = max_clusters;
   std::vector<int32_t> sorted(list);
   std::stable_sort(sorted.begin(), sorted.end(),
-                   [&](int a, int b) { return sim->inst[a].n_flows() > sim->inst[b].n_flows(); });
+                   [&](int a, int b) { return sim->units[a].n_flows > sim->units[b].n_flows; });
   PHS_CUDA(sim->d_clist.upload(sorted, st));
   PHS_CUDA(cudaMemsetAsync(sim->d_cticket.p, 0, sizeof(int), st));
   ClusterScratch sc;
@@ -623,7 +765,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   sc.aggregate = agg ? 1 : 0;
   sc.cold_smem = cold ? 1 : 0;
   sc.replicate = repl ? 1 : 0;
-  PHS_CUDA(launch_cluster_path(tables_of(sim), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
+  PHS_CUDA(launch_cluster_path(tables_of(sim, L), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
                                n_clusters, log, st));
   PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy
   return PHS_OK;
@@ -639,9 +781,10 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     if (fs != PHS_OK) return fs;
   }
   sim->last_stream = st;
-  const int B = sim->batch;
-  DevTables t = tables_of(sim);
+  const int U = (int)sim->units.size();
+  DevTables t = tables_of(sim, sim->cta.n_links);
   sim->n_launches = 0;
+  PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
   PHS_CUDA(cudaEventRecord(sim->ev0, st));
   if (!sim->order.empty()) {
     sim->n_launches++;
@@ -649,13 +792,13 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta, st));
   }
   PHS_CUDA(cudaEventRecord(sim->ev1, st));
-  PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
+  PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
   PHS_CUDA(cudaStreamSynchronize(st));
   PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
   // instances that ran out of shared-memory slots on the CTA path move to the cluster path (also for later runs)
   std::vector<int32_t> redo;
-  for (int i = 0; i < B; ++i)
-    if (!sim->order.empty() && sim->h_res[i].status == kOverflow) redo.push_back(i);
+  for (int u : sim->order)
+    if (sim->h_res[u].status == kOverflow) redo.push_back(u);
   if (!redo.empty()) {
     for (int inst : redo) {
       sim->cluster_list.push_back(inst);
@@ -673,7 +816,7 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     if (gs != PHS_OK) return gs;
     sim->n_launches++;
     PHS_CUDA(cudaEventRecord(sim->ev1, st));
-    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * B, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
     PHS_CUDA(cudaStreamSynchronize(st));
     float extra = 0.f;
     PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
@@ -691,12 +834,13 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
                                    sim->d_coll_t.p, st));
   sim->ran = true;
-  for (int i = 0; i < B; ++i) {
-    if (sim->h_res[i].status == PHS_ECYCLE)
+  for (int u = 0; u < U; ++u) {
+    const int i = sim->units[u].inst;
+    if (sim->h_res[u].status == PHS_ECYCLE)
       return fail(PHS_ECYCLE, "instance " + std::to_string(i) + ": flows left waiting on dependencies that never complete");
-    if (sim->h_res[i].status != PHS_OK)
+    if (sim->h_res[u].status != PHS_OK)
       return fail(PHS_ECUDA, "instance " + std::to_string(i) + ": unexpected kernel status " +
-                                 std::to_string(sim->h_res[i].status));
+                                 std::to_string(sim->h_res[u].status));
   }
   return PHS_OK;
 }
@@ -759,16 +903,17 @@ phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *ou
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (!sim->want_log) return fail(PHS_ESTATE, "event log was not enabled");
   if (!n_events) return fail(PHS_EINVAL, "null n_events");
-  *n_events = sim->h_res[instance].n_events;
+  *n_events = sim->h_res[sim->unit_first[instance]].n_events;  // with the log on, an instance is one unit
   if (!out) return PHS_OK;
-  return fetch(sim, sim->d_log.p, sim->log_base[instance], std::min<int64_t>(cap, *n_events), out, 0);
+  return fetch(sim, sim->d_log.p, sim->h_desc[sim->unit_first[instance]].log_base, std::min<int64_t>(cap, *n_events),
+               out, 0);
 }
 
 phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   phs_counters c{};
-  for (int i = 0; i < sim->batch; ++i) {
+  for (size_t i = 0; i < sim->units.size(); ++i) {
     c.n_events += sim->h_res[i].n_events;
     c.sum_active += sim->h_res[i].sum_active;
     c.sum_par_rounds += sim->h_res[i].sum_par_rounds;
@@ -787,7 +932,10 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
 
 const char *phs_instance_path(const phs_sim *sim, int32_t instance) {
   if (!sim || instance < 0 || instance >= sim->batch || !sim->ran) return "";
-  return sim->h_res[instance].path == 0 ? "cta" : "cluster";
+  int best = sim->unit_first[instance];  // the path of the instance's largest unit
+  for (int u = best; u < sim->unit_first[instance + 1]; ++u)
+    if (sim->units[u].n_flows > sim->units[best].n_flows) best = u;
+  return sim->h_res[best].path == 0 ? "cta" : "cluster";
 }
 
 }  // extern "C"

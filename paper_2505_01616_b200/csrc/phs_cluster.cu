@@ -209,10 +209,13 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     const int32_t *__restrict__ succ = T.succ + D.succ_base;
     const int32_t *__restrict__ pc0 = T.pred_cnt0 + D.flow_base;
     int32_t *pred_cnt = T.pred_cnt + D.flow_base;
-    double *t_done = T.t_done + D.flow_base;
-    int32_t *bneck_out = T.bneck + D.flow_base;
-    const int64_t *__restrict__ capq = T.capq + (int64_t)inst * L;
-    const int32_t *__restrict__ lcomp = T.lcomp + (int64_t)inst * L;
+    const uint32_t *__restrict__ fmap = T.fmap + D.flow_base;  // unit-local flow -> position in the outputs
+    double *t_done = T.t_done;
+    int32_t *bneck_out = T.bneck;
+    const int64_t *__restrict__ capq = T.capq + D.link_base;
+    const int32_t *__restrict__ lcomp = T.lcomp + D.link_base;
+    const int32_t *__restrict__ linkid = T.linkid + D.link_base;
+    const int Li = D.n_links;  // <= L, the launch-wide maximum the shared-memory layout is sized for
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
@@ -220,10 +223,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     for (int li = tid; li < Lc; li += NT) {
       const int l = li * CS + crank;
       LinkA a;
-      a.share0 = 0; a.cap = l < L ? capq[l] : 0; a.n0 = 0; a.chg = 0; a.beat = 0; a.solve = 0;
+      a.share0 = 0; a.cap = l < Li ? capq[l] : 0; a.n0 = 0; a.chg = 0; a.beat = 0; a.solve = 0;
       la[li] = a;
       LinkB b;
-      b.caprem = 0; b.sharew = 0; b.nw = 0; b.deb = 0; b.wsolve = 0; b.comp = l < L ? lcomp[l] : 0;
+      b.caprem = 0; b.sharew = 0; b.nw = 0; b.deb = 0; b.wsolve = 0; b.comp = l < Li ? lcomp[l] : 0;
       lb[li] = b;
       if (LOG) won[li] = 0;
     }
@@ -234,7 +237,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         sh_loc[l] = 0;
         sh0_loc[l] = 0;
         chg_loc[l] = 0;
-        comp_loc[l] = (unsigned short)lcomp[l];
+        comp_loc[l] = l < Li ? (unsigned short)lcomp[l] : 0;
       }
       if (AGG) {
         dcap_loc[l] = 0;
@@ -249,8 +252,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     if (crank == 0 && tid == 0) comb.ev_rounds = 0;
     __syncthreads();
 
-    auto fill_slot = [&](int slot, int f, const FlowRec &r, double ta) {
-      S.flow[slot] = f;
+    auto fill_slot = [&](int slot, int out, const FlowRec &r, double ta) {
+      S.flow[slot] = out;  // where the flow's results go
       S.rem[slot] = r.bytes;
       S.bn[slot] = -2;
       S.comp[slot] = (unsigned short)r.comp;
@@ -271,7 +274,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         const FlowRec r = rec[f];
         const int slot = atomicAdd(&ctl[M_HI], 1);
         if (slot < Sc) {
-          fill_slot(slot, (int)f, r, __dadd_rn(r.start, r.lat));
+          fill_slot(slot, (int)fmap[f], r, __dadd_rn(r.start, r.lat));
           atomicAdd(&ctl[M_NPEND], 1);
         } else {
           ctl[M_OVER] = 1;
@@ -331,7 +334,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           if (nsucc > 1) asm volatile("prefetch.global.L2 [%0];" ::"l"(rec + S.succ1[slot]));
         }
       };
-      auto make_pending = [&](int gf, const FlowRec &r) {  // S4.5: t_act = max(start, now) + Lat
+      auto make_pending = [&](int out, const FlowRec &r) {  // S4.5: t_act = max(start, now) + Lat
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
         const int h = atomicAdd(&ctl[M_QHEAD], 1);
         const int slot = h < qtail ? S.freeq[h % Sc] : atomicAdd(&ctl[M_HI], 1);
@@ -341,17 +344,24 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         }
         atomicAdd(&ctl[M_NPEND], 1);
         const bool due = ta <= t_next;
-        fill_slot(slot, gf, r, due ? kInf : ta);
+        fill_slot(slot, out, r, due ? kInf : ta);
         if (due) activate(slot);
       };
       auto release2 = [&](int g0, int g1) {  // both counters, then both records: the round trips overlap
         const bool z0 = g0 >= 0 && atomicSub(&pred_cnt[g0], 1) == 1;
         const bool z1 = g1 >= 0 && atomicSub(&pred_cnt[g1], 1) == 1;
         FlowRec r0, r1;
-        if (z0) r0 = rec[g0];
-        if (z1) r1 = rec[g1];
-        if (z0) make_pending(g0, r0);
-        if (z1) make_pending(g1, r1);
+        int o0 = 0, o1 = 0;
+        if (z0) {
+          r0 = rec[g0];
+          o0 = (int)fmap[g0];
+        }
+        if (z1) {
+          r1 = rec[g1];
+          o1 = (int)fmap[g1];
+        }
+        if (z0) make_pending(o0, r0);
+        if (z1) make_pending(o1, r1);
       };
       for (int s = tid; s < hi0; s += NT) {
         if (!(S.tc[s] <= t_next)) continue;
@@ -361,7 +371,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         }
         const int f = S.flow[s];
         t_done[f] = t_next;
-        bneck_out[f] = S.bn[s];
+        bneck_out[f] = linkid[S.bn[s]];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
           const int l = S.path[s * kMaxHops + h];

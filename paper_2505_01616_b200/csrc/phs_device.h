@@ -8,19 +8,21 @@
 namespace phs {
 
 struct DevTables {
-  const InstDesc *inst;      // [B]
-  const FlowRec *rec;        // [F_total]
-  const int32_t *succ;       // successor CSR values (instance-relative flow ids)
+  const InstDesc *inst;      // [U] simulation units
+  const FlowRec *rec;        // [F_total] unit-local link / flow ids inside
+  const int32_t *succ;       // successor lists longer than two (unit-local flow ids)
   const int32_t *pred_cnt0;  // [F_total] number of predecessors
-  const uint8_t *pred_cnt0_u8;  // same, packed 4 bits per flow (per-instance slices 4-byte aligned); unused if a count > 15
-  const int64_t *capq;       // [B][n_links] link capacity in rate quanta
-  const int32_t *lcomp;      // [B][n_links] static component (representative link) of every link
+  const uint8_t *pred_cnt0_u8;  // same, packed 4 bits per flow (per-unit slices 4-byte aligned); unused if a count > 15
+  const uint32_t *fmap;      // [F_total] unit-local flow -> index of the flow in t_done[] / bneck[]
+  const int64_t *capq;       // per unit [n_links] link capacity in rate quanta
+  const int32_t *lcomp;      // per unit [n_links] static component (representative unit-local link) of every link
+  const int32_t *linkid;     // per unit [n_links] unit-local link -> link id of the topology
   int32_t *pred_cnt;         // [F_total] outstanding predecessors (dynamic)
-  double *t_done;            // [F_total] O1
-  int32_t *bneck;            // [F_total] O3
-  InstResult *res;           // [B]
+  double *t_done;            // [F_total] O1, in the caller's flow order
+  int32_t *bneck;            // [F_total] O3, topology link ids
+  InstResult *res;           // [U]
   phs_event *log;            // event log rows, or nullptr
-  int32_t n_links;
+  int32_t n_links;           // largest n_links among the units of this launch (sizes the shared-memory layout)
 };
 
 // Shared-memory footprint of the CTA kernel for given capacities (pc_flows > 0: predecessor counters of that
@@ -31,6 +33,7 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log);
 // Instances that run out of shared-memory slots finish with status kOverflow.
 struct CtaLaunch {
   int threads, slots, pc_flows, grid;
+  int n_links;  // largest link count among the units of the launch
   size_t smem;
   bool log;
 };

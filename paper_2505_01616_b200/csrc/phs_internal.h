@@ -32,16 +32,18 @@ struct FlowRec {
 };
 static_assert(sizeof(FlowRec) == 64, "FlowRec must be 64 bytes");
 
-// Per-instance descriptor (device).
+// Descriptor of one simulation unit (device).  A unit is what one CTA / cluster simulates: a whole instance, or --
+// when the instance decomposes -- a group of its flows that shares no link and no dependency with the rest (under
+// reading R-LZ such a group evolves exactly as it does inside the whole instance).  Flow and link ids inside a
+// unit are unit-local and dense.
 struct InstDesc {
-  int64_t flow_base;  // first entry in the per-flow arrays (rec, pred_cnt, t_done, bneck, ...)
-  int64_t path_base;  // unused (paths are inline in FlowRec)
-  int64_t succ_base;  // first entry of the instance's slice of succ[]
-  int64_t log_base;   // first row of the instance's event log slice (capacity 2F+2 rows), -1 if disabled
-  int64_t coll_base;  // first entry in the per-collective arrays
-  int64_t pc8_base;   // first byte of the instance's slice of the packed predecessor counters (4-byte aligned)
+  int64_t flow_base;  // first entry of the unit in the per-flow arrays (rec, pred_cnt, fmap, ...)
+  int64_t link_base;  // first entry of the unit in the per-link arrays (capq, lcomp, linkid)
+  int64_t succ_base;  // first entry of the unit's slice of succ[]
+  int64_t log_base;   // first row of the unit's event log slice (capacity 2F+2 rows), -1 if disabled
+  int64_t pc8_base;   // first byte of the unit's slice of the packed predecessor counters (4-byte aligned)
   int32_t n_flows;
-  int32_t n_colls;
+  int32_t n_links;
 };
 
 // Per-instance result block (device, read back after a run).

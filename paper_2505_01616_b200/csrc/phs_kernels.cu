@@ -42,6 +42,7 @@ struct CtaSmem {
   int *l_deb;     // working: round number of the last debit
   int *l_solve;   // per component (indexed by its representative link): id of the solve that must redo it
   int *l_won;     // LOG: round in which the link froze flows (counts bottleneck links once)
+  int *l_gid;     // link id of the topology (the links of a unit are numbered densely)
   // per slot [S]: one slot per PENDING or ACTIVE flow
   double *s_tc;   // PENDING: activation time; ACTIVE: completion time; free: +inf
   double *s_rem;  // remaining bytes at time s_tl
@@ -96,6 +97,7 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   PHS_TAKE(l_deb, int, L)
   PHS_TAKE(l_solve, int, L)
   PHS_TAKE(l_won, int, log ? L : 0)
+  PHS_TAKE(l_gid, int, L)
   PHS_TAKE(s_meta, int4, S)
   PHS_TAKE(s_path, uint4, S)
   PHS_TAKE(s_succ_cnt, int, S)
@@ -161,15 +163,19 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
     const FlowRec *__restrict__ rec = T.rec + D.flow_base;
     const int32_t *__restrict__ succ = T.succ + D.succ_base;
     int32_t *pred_cnt = T.pred_cnt + D.flow_base;
-    double *t_done = T.t_done + D.flow_base;
-    int32_t *bneck_out = T.bneck + D.flow_base;
-    const int64_t *__restrict__ capq = T.capq + (int64_t)inst * L;
+    const uint32_t *__restrict__ fmap = T.fmap + D.flow_base;  // unit-local flow -> position in the outputs
+    double *t_done = T.t_done;
+    int32_t *bneck_out = T.bneck;
+    const int64_t *__restrict__ capq = T.capq + D.link_base;
+    const int32_t *__restrict__ linkid = T.linkid + D.link_base;
+    const int Li = D.n_links;  // <= L, the launch-wide maximum the shared-memory layout is carved for
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
     // ---- init: nothing active, every slot free
-    for (int l = tid; l < L; l += NT) {
+    for (int l = tid; l < Li; l += NT) {
       S.l_cap[l] = capq[l];
+      S.l_gid[l] = linkid[l];
       S.l_n0[l] = 0;
       S.l_chg[l] = 0;
       S.l_beat[l] = 0;
@@ -189,8 +195,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
     __syncthreads();
 
     // one slot per flow that is PENDING or ACTIVE; the whole record is staged when the flow becomes PENDING
-    auto fill_slot = [&](int slot, int f, const FlowRec &r, double ta) {
-      S.s_meta[slot].x = f;
+    auto fill_slot = [&](int slot, int out, const FlowRec &r, double ta) {
+      S.s_meta[slot].x = out;  // where the flow's results go; its unit-local id is not needed any more
       S.s_rem[slot] = r.bytes;
       S.s_meta[slot].y = -2;
       S.s_meta[slot].z = r.comp;
@@ -224,7 +230,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
           const FlowRec r = rec[f];
           const int slot = atomicAdd(&S.ctl[C_HI], 1);
           if (slot < SC) {
-            fill_slot(slot, f, r, __dadd_rn(r.start, r.lat));
+            fill_slot(slot, (int)fmap[f], r, __dadd_rn(r.start, r.lat));
             atomicAdd(&S.ctl[C_NPEND], 1);
           } else {
             S.ctl[C_OVERFLOW] = 1;
@@ -288,7 +294,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
         }
         return atomicSub(&pred_cnt[gf], 1) == 1;
       };
-      auto make_pending = [&](int gf, const FlowRec &r) {  // -> PENDING with t_act = max(start, now) + Lat
+      auto make_pending = [&](int out, const FlowRec &r) {  // -> PENDING with t_act = max(start, now) + Lat
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
         const int h = atomicAdd(&S.ctl[C_QHEAD], 1);
         const int slot = h < qtail ? S.free_q[h % SC] : atomicAdd(&S.ctl[C_HI], 1);
@@ -298,17 +304,24 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
         }
         atomicAdd(&S.ctl[C_NPEND], 1);
         const bool due = ta <= t_next;  // zero path latency: due at this very timestamp
-        fill_slot(slot, gf, r, due ? kInf : ta);
+        fill_slot(slot, out, r, due ? kInf : ta);
         if (due) activate(slot);
       };
       auto release2 = [&](int g0, int g1) {  // both counters, then both records: the loads overlap
         const bool z0 = g0 >= 0 && pred_done(g0);
         const bool z1 = g1 >= 0 && pred_done(g1);
         FlowRec r0, r1;
-        if (z0) r0 = rec[g0];
-        if (z1) r1 = rec[g1];
-        if (z0) make_pending(g0, r0);
-        if (z1) make_pending(g1, r1);
+        int o0 = 0, o1 = 0;
+        if (z0) {
+          r0 = rec[g0];
+          o0 = (int)fmap[g0];
+        }
+        if (z1) {
+          r1 = rec[g1];
+          o1 = (int)fmap[g1];
+        }
+        if (z0) make_pending(o0, r0);
+        if (z1) make_pending(o1, r1);
       };
 
       for (int s = tid; s < hi0; s += NT) {
@@ -320,7 +333,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
         // the flow completes at t_next (bit-equal absolute time, S4.4)
         const int f = S.s_meta[s].x;
         t_done[f] = t_next;
-        bneck_out[f] = S.s_meta[s].y;
+        bneck_out[f] = S.l_gid[S.s_meta[s].y];
         const uint4 pv = S.s_path[s];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
