@@ -610,7 +610,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       need = std::max(need, need_of(sim->units[u]));
       maxF = std::max<int64_t>(maxF, sim->units[u].n_flows);
     }
-    const int threads = Lm <= 320 ? 128 : 256;  // measured on B200: 128 for cfg3-sized units, 256 for cfg1-sized
+    // about one slot per thread: measured on B200, 128 threads for cfg3-sized units, 256 for cfg1-sized ones
+    const int threads = (need <= 128 && Lm <= 320) ? 128 : 256;
     const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
     // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
     // predecessor counters on chip; returns 0 if not even one fits

@@ -612,7 +612,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kern
       PHS_TICK(6)
     }
 #ifdef PHS_PHASE_CLOCKS
-    if ((tid == 0 || tid == NT - 1) && inst < 2)
+    if ((tid == 0 || tid == NT - 1) && F > 3000 && inst < 40)
       printf("inst %d tid %d events %d cycles: X %lld waitX %lld V0 %lld wait1 %lld F0 %lld wait2 %lld rest %lld\n", inst, tid,
              ev, pc_[0], pc_[1], pc_[2], pc_[3], pc_[4], pc_[5], pc_[6]);
 #endif
