@@ -141,7 +141,7 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
 // NT threads; LOG: write the event log (and solve every component at every event, so that the log's iteration
 // count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory.
 template <int NT, bool LOG, bool PCS>
-__global__ void __launch_bounds__(NT, (NT <= 128 ? 768 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
+__global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
                                                      int *ticket, int SC, int pcf) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int sh_inst;
