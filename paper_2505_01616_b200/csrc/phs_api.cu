@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -11,6 +12,7 @@
 #include <memory>
 #include <numeric>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "phs_device.h"
@@ -31,6 +33,23 @@ phs_status fail(phs_status code, const std::string &msg) {
     cudaError_t e_ = (call);                                                                             \
     if (e_ != cudaSuccess) return fail(PHS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
   } while (0)
+
+// fn(i) for every i in [0, n) on up to `max_threads` (<= 16) host threads; the iterations must be independent
+template <typename F>
+void parallel_for(int n, F fn, int max_threads = 16) {
+  const int nt = std::min(std::min(n, max_threads), (int)std::min(16u, std::max(1u, std::thread::hardware_concurrency())));
+  if (nt <= 1) {
+    for (int i = 0; i < n; ++i) fn(i);
+    return;
+  }
+  std::atomic<int> next{0};
+  std::vector<std::thread> pool;
+  for (int t = 0; t < nt; ++t)
+    pool.emplace_back([&] {
+      for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+    });
+  for (std::thread &th : pool) th.join();
+}
 
 template <typename T>
 struct DevBuf {
@@ -212,12 +231,22 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
     if (!(bytes[i] > 0.0) || !std::isfinite(bytes[i])) return fail(PHS_EINVAL, "bytes must be positive and finite");
     if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return fail(PHS_EINVAL, "bad start_time_s");
   }
+  // instance 0 first: the arguments shared by all instances (kind, ranks, after) fail here before anything is added;
+  // the others are independent and are expanded on host threads
   std::string why;
-  for (int i = 0; i < sim->batch; ++i) {
-    phs_status st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
-                                      after, n_after, &why);
-    if (st != PHS_OK) return fail(st, why);
-  }
+  phs_status st0 = append_collective(*sim->fab, sim->inst[0], kind, ranks, n_ranks, bytes[0], start ? start[0] : 0.0,
+                                     after, n_after, &why);
+  if (st0 != PHS_OK) return fail(st0, why);
+  std::vector<phs_status> sts((size_t)sim->batch, PHS_OK);
+  std::vector<std::string> whys((size_t)sim->batch);
+  const int64_t work = (int64_t)sim->batch * sim->inst[0].colls.back().n_flows;  // a thread per ~8K flows
+  parallel_for(sim->batch - 1, [&](int k) {
+    const int i = k + 1;
+    sts[i] = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0, after,
+                               n_after, &whys[i]);
+  }, (int)std::max<int64_t>(1, work / 8192));
+  for (int i = 1; i < sim->batch; ++i)
+    if (sts[i] != PHS_OK) return fail(sts[i], whys[i]);
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;
   return PHS_OK;
 }
@@ -370,28 +399,42 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   // ---- simulation units (a9).  Flows that share a link, directly or through a chain of flows, and flows joined by
   // a dependency evolve together; such a group shares nothing with the rest of its instance, so (reading R-LZ) it
   // can be simulated on its own with bit-identical results.  Every unit gets dense local flow and link ids.
-  std::vector<FlowRec> rec((size_t)Ft);
-  std::vector<int32_t> succ, pc0((size_t)Ft), lcomp, linkid;
-  std::vector<uint32_t> fmap((size_t)Ft);
-  std::vector<uint8_t> pc8;
-  std::vector<int64_t> capq, coll_first((size_t)sim->total_colls);
+  // per-instance work is independent: every instance builds its own chunk of the tables on a host thread, the
+  // chunks are then laid out back to back
+  struct Chunk {
+    std::vector<FlowRec> rec;
+    std::vector<int32_t> succ, pc0, lcomp, linkid;
+    std::vector<uint32_t> fmap;
+    std::vector<uint8_t> pc8;
+    std::vector<int64_t> capq;
+    std::vector<InstDesc> desc;  // bases relative to the chunk
+    std::vector<phs_sim::Unit> units;
+    int max_pred = 0;
+    phs_status st = PHS_OK;
+    const char *err = "";
+  };
+  std::vector<Chunk> chunks((size_t)B);
+  std::vector<int64_t> coll_first((size_t)sim->total_colls);
   std::vector<int32_t> coll_n((size_t)sim->total_colls);
-  sim->units.clear();
-  sim->unit_first.assign(B + 1, 0);
-  sim->h_desc.clear();
-  int max_pred = 0;
-  int64_t flow_cursor = 0, log_cursor = 0;
-  std::vector<int64_t> capq_inst((size_t)L);
-  std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
-  for (int i = 0; i < B; ++i) {
+  auto build_instance = [&](int i) {
+    Chunk &c = chunks[(size_t)i];
     const Instance &in = sim->inst[i];
     const int64_t F = in.n_flows();
-    sim->unit_first[i] = (int32_t)sim->units.size();
+    c.rec.resize((size_t)F);
+    c.pc0.resize((size_t)F);
+    c.fmap.resize((size_t)F);
+    int64_t flow_cursor = 0, log_cursor = 0;
+    std::vector<int64_t> capq_inst((size_t)L);
+    std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
     // capacities -> rate quanta (floor); every fair share must stay >= 1 quantum
     for (int l = 0; l < L; ++l) {
-      const double c = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
-      const int64_t q = (int64_t)std::floor(c * 1048576.0);
-      if (q < F + 1) return fail(PHS_ERANGE, "a link capacity is below (#flows + 1) rate quanta of 2^-20 byte/s");
+      const double cap_l = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
+      const int64_t q = (int64_t)std::floor(cap_l * 1048576.0);
+      if (q < F + 1) {
+        c.st = PHS_ERANGE;
+        c.err = "a link capacity is below (#flows + 1) rate quanta of 2^-20 byte/s";
+        return;
+      }
       capq_inst[l] = q;
     }
     for (size_t c = 0; c < in.colls.size(); ++c) {
@@ -507,18 +550,18 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       for (size_t k = 0; k < links.size(); ++k) link_loc[links[k]] = (int32_t)k;
       InstDesc d;
       d.flow_base = flow_cursor;
-      d.link_base = (int64_t)capq.size();
-      d.succ_base = (int64_t)succ.size();
+      d.link_base = (int64_t)c.capq.size();
+      d.succ_base = (int64_t)c.succ.size();
       d.log_base = sim->want_log ? log_cursor : -1;
-      d.pc8_base = (int64_t)pc8.size();
+      d.pc8_base = (int64_t)c.pc8.size();
       d.n_flows = (int32_t)fl.size();
       d.n_links = (int32_t)links.size();
       for (int32_t l : links) {
-        capq.push_back(capq_inst[l]);
-        lcomp.push_back(link_loc[find_in(parent, l)]);  // the smallest link of a component is in the unit too
-        linkid.push_back(l);
+        c.capq.push_back(capq_inst[l]);
+        c.lcomp.push_back(link_loc[find_in(parent, l)]);  // the smallest link of a component is in the unit too
+        c.linkid.push_back(l);
       }
-      pc8.resize(pc8.size() + (fl.size() + 7) / 8 * 4, 0);
+      c.pc8.resize(c.pc8.size() + (fl.size() + 7) / 8 * 4, 0);
       for (size_t k = 0; k < fl.size(); ++k) {
         const int32_t f = fl[k];
         FlowRec x;
@@ -532,30 +575,78 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           x.succ_in[0] = x.succ_cnt > 0 ? flow_loc[sdst[soff[f]]] : -1;
           x.succ_in[1] = x.succ_cnt > 1 ? flow_loc[sdst[soff[f] + 1]] : -1;
         } else {
-          x.succ_in[0] = (int32_t)((int64_t)succ.size() - d.succ_base);
+          x.succ_in[0] = (int32_t)((int64_t)c.succ.size() - d.succ_base);
           x.succ_in[1] = -1;
-          for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) succ.push_back(flow_loc[sdst[e]]);
+          for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) c.succ.push_back(flow_loc[sdst[e]]);
         }
         x.comp = p0 < p1 ? link_loc[find_in(parent, in.path[p0])] : 0;
-        rec[(size_t)flow_cursor + k] = x;
-        fmap[(size_t)flow_cursor + k] = (uint32_t)(sim->flow_base[i] + f);
+        c.rec[(size_t)flow_cursor + k] = x;
+        c.fmap[(size_t)flow_cursor + k] = (uint32_t)(sim->flow_base[i] + f);
         const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
-        pc0[(size_t)flow_cursor + k] = np;
-        max_pred = std::max(max_pred, np);
-        pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
+        c.pc0[(size_t)flow_cursor + k] = np;
+        c.max_pred = std::max(c.max_pred, np);
+        c.pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
       }
       flow_cursor += (int64_t)fl.size();
       log_cursor += 2 * (int64_t)fl.size() + 2;
-      sim->h_desc.push_back(d);
+      c.desc.push_back(d);
       phs_sim::Unit un;
       un.inst = i;
       un.n_flows = d.n_flows;
       un.n_links = d.n_links;
       un.bound = ubound[u];
       un.initial = uinit[u];
-      sim->units.push_back(un);
+      c.units.push_back(un);
     }
+  };
+  parallel_for(B, build_instance);
+  for (int i = 0; i < B; ++i)
+    if (chunks[i].st != PHS_OK) return fail(chunks[i].st, chunks[i].err);
+  // lay the chunks out back to back
+  std::vector<int64_t> b_flow(B + 1, 0), b_link(B + 1, 0), b_succ(B + 1, 0), b_pc8(B + 1, 0), b_log(B + 1, 0);
+  sim->units.clear();
+  sim->unit_first.assign(B + 1, 0);
+  int max_pred = 0;
+  for (int i = 0; i < B; ++i) {
+    const Chunk &c = chunks[i];
+    b_flow[i + 1] = b_flow[i] + (int64_t)c.rec.size();
+    b_link[i + 1] = b_link[i] + (int64_t)c.capq.size();
+    b_succ[i + 1] = b_succ[i] + (int64_t)c.succ.size();
+    b_pc8[i + 1] = b_pc8[i] + (int64_t)c.pc8.size();
+    b_log[i + 1] = b_log[i] + 2 * (int64_t)c.rec.size() + 2 * (int64_t)c.units.size();
+    sim->unit_first[i] = (int32_t)sim->units.size();
+    sim->units.insert(sim->units.end(), c.units.begin(), c.units.end());
+    max_pred = std::max(max_pred, c.max_pred);
   }
+  const int64_t log_cursor = b_log[B];
+  std::vector<FlowRec> rec((size_t)Ft);
+  std::vector<int32_t> succ((size_t)b_succ[B]), pc0((size_t)Ft), lcomp((size_t)b_link[B]), linkid((size_t)b_link[B]);
+  std::vector<uint32_t> fmap((size_t)Ft);
+  std::vector<uint8_t> pc8((size_t)b_pc8[B]);
+  std::vector<int64_t> capq((size_t)b_link[B]);
+  sim->h_desc.assign(sim->units.size(), InstDesc{});
+  parallel_for(B, [&](int i) {
+    Chunk &c = chunks[i];
+    std::copy(c.rec.begin(), c.rec.end(), rec.begin() + b_flow[i]);
+    std::copy(c.pc0.begin(), c.pc0.end(), pc0.begin() + b_flow[i]);
+    std::copy(c.fmap.begin(), c.fmap.end(), fmap.begin() + b_flow[i]);
+    std::copy(c.succ.begin(), c.succ.end(), succ.begin() + b_succ[i]);
+    std::copy(c.pc8.begin(), c.pc8.end(), pc8.begin() + b_pc8[i]);
+    std::copy(c.capq.begin(), c.capq.end(), capq.begin() + b_link[i]);
+    std::copy(c.lcomp.begin(), c.lcomp.end(), lcomp.begin() + b_link[i]);
+    std::copy(c.linkid.begin(), c.linkid.end(), linkid.begin() + b_link[i]);
+    for (size_t k = 0; k < c.desc.size(); ++k) {
+      InstDesc d = c.desc[k];
+      d.flow_base += b_flow[i];
+      d.link_base += b_link[i];
+      d.succ_base += b_succ[i];
+      d.pc8_base += b_pc8[i];
+      if (d.log_base >= 0) d.log_base += b_log[i];
+      sim->h_desc[(size_t)sim->unit_first[i] + k] = d;
+    }
+    Chunk().rec.swap(c.rec);  // release the chunk's big arrays early
+    std::vector<uint32_t>().swap(c.fmap);
+  });
   sim->unit_first[B] = (int32_t)sim->units.size();
   const int U = (int)sim->units.size();
   const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
