@@ -816,7 +816,7 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   // replicated link shares pay when many flows share a link (every flow reads its links' shares every round)
   const bool want_repl = target >= 8 * (int64_t)L;
   for (int c = 1; c <= 16 && !cs; c *= 2) {
-    if ((int64_t)c * kClusterThreads * 2 < target && c < 16) continue;  // at most ~2 slots per thread
+    if ((int64_t)c * kClusterThreads * 4 < target && c < 16) continue;  // at most ~4 slots per thread
     const int64_t sc = std::min<int64_t>(65535, (target + c - 1) / c + 16);
     const bool opts[4][2] = {{true, true}, {false, true}, {true, false}, {false, false}};  // {agg, cold in smem}
     for (int k = 0; k < 8 && !cs; ++k) {
