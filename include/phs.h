@@ -71,7 +71,9 @@ typedef struct {
   int32_t first_bneck; /* link with the smallest fair share at the start of the solve, -1 if none active  */
 } phs_event;
 
-/* Per-run work counters, summed over the instances of the last phs_run. */
+/* Per-run work counters, summed over the simulation units of the last phs_run (an instance is one unit, or --
+ * with decomposition -- several independent ones; events that coincide in time in different units count once
+ * per unit). */
 typedef struct {
   int64_t n_events;      /* loop iterations                                                               */
   int64_t n_flow_events; /* activations + completions = 2 * flows                                         */

@@ -186,3 +186,31 @@ def test_full_size_against_stored_oracle_samples(name, make, inst):
     # independent units count their own events, so simultaneous events of different units count more than once
     assert sim.counters()["n_events"] >= n_events
     sim.close()
+
+
+def test_unit_larger_than_a_cluster_is_refused_not_silently_wrong():
+    """The cluster path keeps all dynamic state on chip; an instance whose concurrent flows exceed the shared memory
+    of 16 SMs is refused with PHS_ERANGE (there is no CPU or global-memory fallback)."""
+    d = W.topo_desc(W.TOPO_SINGLE, 38, 8)                      # 304 GPUs on one switch
+    sim = B.Sim(d, batch=1)
+    B.phs_add_collective(sim.h, 0, B.ALLTOALL, np.arange(304, dtype=np.int32), 304e6)   # 92,112 concurrent flows
+    with pytest.raises(B.PhsError) as e:
+        sim.run()
+    assert e.value.code == B.PHS_ERANGE
+    sim.close()
+
+
+def test_decomposition_knob_state_and_counters():
+    w = W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
+    a = B.Sim.from_workload(w)                       # decomposed: TP rings and the DP group are separate units
+    b = B.Sim.from_workload(w, decompose=False)
+    a.run(); b.run()
+    for i in range(2):
+        assert np.array_equal(a.completion_times(i), b.completion_times(i))
+        assert np.array_equal(a.bottlenecks(i), b.bottlenecks(i))
+        assert np.array_equal(a.collective_times(i), b.collective_times(i))
+    assert a.counters()["n_events"] >= b.counters()["n_events"]      # coinciding events count once per unit
+    with pytest.raises(B.PhsError) as e:
+        B.phs_set_decomposition(a.h, False)
+    assert e.value.code == B.PHS_ESTATE
+    a.close(); b.close()
