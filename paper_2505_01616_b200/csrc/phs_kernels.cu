@@ -294,10 +294,16 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         }
         return atomicSub(&pred_cnt[gf], 1) == 1;
       };
-      auto make_pending = [&](int out, const FlowRec &r) {  // -> PENDING with t_act = max(start, now) + Lat
+      // -> PENDING with t_act = max(start, now) + Lat.  `reuse` >= 0: the slot the releasing flow just vacated (no
+      // trip through the free queue); it is consumed by the first successor that needs a slot.
+      auto make_pending = [&](int out, const FlowRec &r, int &reuse) {
         const double ta = __dadd_rn(r.start > t_next ? r.start : t_next, r.lat);
-        const int h = atomicAdd(&S.ctl[C_QHEAD], 1);
-        const int slot = h < qtail ? S.free_q[h % SC] : atomicAdd(&S.ctl[C_HI], 1);
+        int slot = reuse;
+        reuse = -1;
+        if (slot < 0) {
+          const int h = atomicAdd(&S.ctl[C_QHEAD], 1);
+          slot = h < qtail ? S.free_q[h % SC] : atomicAdd(&S.ctl[C_HI], 1);
+        }
         if (slot >= SC) {
           S.ctl[C_OVERFLOW] = 1;
           return;
@@ -307,7 +313,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         fill_slot(slot, out, r, due ? kInf : ta);
         if (due) activate(slot);
       };
-      auto release2 = [&](int g0, int g1) {  // both counters, then both records: the loads overlap
+      auto release2 = [&](int g0, int g1, int &reuse) {  // both counters, then both records: the loads overlap
         const bool z0 = g0 >= 0 && pred_done(g0);
         const bool z1 = g1 >= 0 && pred_done(g1);
         FlowRec r0, r1;
@@ -320,8 +326,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           r1 = rec[g1];
           o1 = (int)fmap[g1];
         }
-        if (z0) make_pending(o0, r0);
-        if (z1) make_pending(o1, r1);
+        if (z0) make_pending(o0, r0, reuse);
+        if (z1) make_pending(o1, r1, reuse);
       };
 
       for (int s = tid; s < hi0; s += NT) {
@@ -344,19 +350,19 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           }
         }
         S.l_solve[S.s_meta[s].z] = solve;
+        const int nsucc = S.s_succ_cnt[s], sc0 = S.s_succ0[s], sc1 = S.s_succ1[s];
         S.s_meta[s].x = -1;
         S.s_tc[s] = kInf;
-        S.free_q[atomicAdd(&S.ctl[C_QTAIL], 1) % SC] = s;
         atomicSub(&S.ctl[C_NACTIVE], 1);
         atomicAdd(&S.ctl[C_DONE], 1);
         if (LOG) atomicAdd(&S.ctl[C_EV_NCOMP], 1);
-        const int nsucc = S.s_succ_cnt[s];
+        int reuse = s;  // the vacated slot goes to the first successor that becomes PENDING, else to the free queue
         if (nsucc <= 2) {
-          if (nsucc > 0) release2(S.s_succ0[s], nsucc > 1 ? S.s_succ1[s] : -1);
+          if (nsucc > 0) release2(sc0, nsucc > 1 ? sc1 : -1, reuse);
         } else {
-          const int e0 = S.s_succ0[s];
-          for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
+          for (int e = 0; e < nsucc; ++e) release2(succ[sc0 + e], -1, reuse);
         }
+        if (reuse >= 0) S.free_q[atomicAdd(&S.ctl[C_QTAIL], 1) % SC] = s;
       }
       PHS_TICK(0)
       __syncthreads();
@@ -391,7 +397,15 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 
-      // ======== rates (a5-a7): parallel progressive filling over the components this event touched
+      // ======== a5: fair share of the links whose flow count changed in this event, one thread per link
+      for (int l = tid; l < Li; l += NT) {
+        if (S.l_chg[l] != solve) continue;
+        const int n = S.l_n0[l];
+        if (n > 0) S.l_share0[l] = fair_share(S.l_cap[l], n);
+      }
+      __syncthreads();
+
+      // ======== rates (a6-a7): parallel progressive filling over the components this event touched
       auto in_solve = [&](int s) {  // ACTIVE flow of a component that must be re-solved
         const int4 m = S.s_meta[s];
         if (m.x < 0 || m.y == -2) return false;
@@ -422,14 +436,12 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           if (!in_solve(s)) continue;
           S.s_meta[s].y = -1;
           const uint4 pv = S.s_path[s];
-          int p[kMaxHops], chg[kMaxHops];
+          int p[kMaxHops];
           long long sh[kMaxHops];
 #pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {  // all loads first
             p[h] = path_at(pv, h);
-            const int l = p[h] != (int)kNoLink ? p[h] : 0;
-            chg[h] = S.l_chg[l];
-            sh[h] = S.l_share0[l];
+            sh[h] = S.l_share0[p[h] != (int)kNoLink ? p[h] : 0];
           }
           long long best = LLONG_MAX;
           int arg = -1;
@@ -437,10 +449,6 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           for (int h = 0; h < kMaxHops; ++h) {
             const int l = p[h];
             if (l == (int)kNoLink) continue;
-            if (chg[h] == solve) {  // flow count changed in this event: every flow on the link stores the same value
-              sh[h] = fair_share(S.l_cap[l], S.l_n0[l]);
-              S.l_share0[l] = sh[h];
-            }
             if (sh[h] < best || (sh[h] == best && l < arg)) {
               best = sh[h];
               arg = l;
