@@ -214,3 +214,43 @@ def test_decomposition_knob_state_and_counters():
         B.phs_set_decomposition(a.h, False)
     assert e.value.code == B.PHS_ESTATE
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_random_dags_of_raw_flows(seed):
+    """Differential test on irregular inputs: raw flows with random dependencies (fan-in up to 24, fan-out beyond the
+    two inline successors), random start times, a mix of zero and non-zero latency, groups that decompose into many
+    small units, on both kernel paths, with and without the event log."""
+    rng = np.random.default_rng(1000 + seed)
+    lat = [0.0, 1e-6][seed % 2]
+    if seed % 3 == 0:
+        d = W.topo_desc(W.TOPO_SINGLE, 4, 8, hop_latency_s=lat)
+    elif seed % 3 == 1:
+        d = W.topo_desc(W.TOPO_LEAF_SPINE, 8, 4, hop_latency_s=lat, fabric_Bps=W.gbps(400.0), n_leaves=4, n_spines=2,
+                        uplinks_per_leaf_spine=1)
+    else:
+        d = W.topo_desc(W.TOPO_FAT_TREE, 8, 2, hop_latency_s=lat, fabric_Bps=W.gbps(400.0), k=4, agg_uplinks=1)
+    G = d["n_hosts"] * d["gpus_per_host"]
+    insts = []
+    for i in range(3):
+        n = int(rng.integers(200, 900))
+        src = rng.integers(0, G, n).astype(np.int32)
+        dst = ((src + rng.integers(1, G, n)) % G).astype(np.int32)
+        if i == 2:                                   # many small independent groups: traffic stays inside GPU pairs
+            src = (2 * rng.integers(0, G // 2, n)).astype(np.int32)
+            dst = (src + 1).astype(np.int32)
+        nbytes = np.floor(np.exp(rng.uniform(np.log(1e3), np.log(5e7), n)))
+        start = np.where(rng.random(n) < 0.3, rng.uniform(0, 2e-3, n), 0.0)
+        dep_off, dep_ids = [0], []
+        for f in range(n):
+            k = 0 if f == 0 else int(rng.choice([0, 0, 1, 2, 3, 24], p=[0.3, 0.2, 0.25, 0.15, 0.08, 0.02]))
+            lo = max(0, f - 60)
+            deps = np.unique(rng.integers(lo, f, min(k, f - lo))) if k and f > lo else []
+            if i == 2 and len(deps):                 # keep the small groups independent: depend within the pair
+                deps = [p for p in deps if src[p] == src[f]]
+            dep_ids.extend(int(x) for x in deps)
+            dep_off.append(len(dep_ids))
+        insts.append(W.Instance(seed=i, ops=[W.RawFlows(src, dst, nbytes, start, np.array(dep_off, np.int64),
+                                                        np.array(dep_ids, np.int64))]))
+    w = W.Workload("fuzz", d, 7 * seed, insts)
+    run_and_compare(w, path=[0, CTA, CLUSTER][seed % 3], mode=orc.MODE_FAST)
