@@ -87,10 +87,9 @@ struct phs_sim {
   // ---- host mirrors built by finalize
   std::vector<int64_t> flow_base;  // [B+1]
   std::vector<int64_t> coll_base;  // [B+1]
-  std::vector<int64_t> log_base;   // [B+1] (only with the event log)
   struct Unit {  // what one CTA / cluster simulates (see InstDesc)
     int32_t inst, n_flows, n_links;
-    int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (Instance::slot_bound, per unit)
+    int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (see phs_finalize)
     int64_t initial;  // flows without predecessors: PENDING from t = 0
   };
   std::vector<Unit> units;
@@ -511,7 +510,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       flow_loc[f] = (int32_t)uflows[unit_of[f]].size();
       uflows[unit_of[f]].push_back((int32_t)f);
     }
-    // slots a unit can need: Instance::slot_bound, per unit (a collective and its `after` chain lie in one unit)
+    // slots a unit can need: raw flows and all-to-alls may be in flight as a whole; a ring collective keeps at most
+    // one flow per sender PENDING or ACTIVE, twice the ring size because a slot freed in a phase is reused only in a
+    // later one; collectives chained with `after` follow each other per rank, so a chain counts once, with its
+    // largest member (a collective and its chain lie in one unit)
     std::vector<int64_t> ubound((size_t)n_units, 0), uinit((size_t)n_units, 0);
     {
       for (int u = 0; u < n_units; ++u) ubound[u] = (int64_t)uflows[u].size();

@@ -78,22 +78,6 @@ struct Instance {
   std::vector<int32_t> pred;
   std::vector<Collective> colls;
   int64_t n_flows() const { return (int64_t)src.size(); }
-  // Upper estimate of how many flows can be PENDING or ACTIVE at once (sizes the on-chip slot arrays): raw flows
-  // and all-to-alls may be in flight as a whole; a ring collective keeps at most one flow per sender in flight and
-  // collectives chained with `after` follow each other per rank, so a chain counts once, with its largest member.
-  // Twice the ring size, because a slot freed in one phase is reused only in a later one.
-  int64_t slot_bound() const {
-    int64_t b = n_flows();
-    std::vector<int64_t> chain_max(colls.size(), 0);
-    for (size_t c = 0; c < colls.size(); ++c) {
-      b -= colls[c].n_flows;
-      const int64_t need = colls[c].kind == PHS_ALLTOALL ? colls[c].n_flows
-                                                          : std::min<int64_t>(colls[c].n_flows, 2 * (int64_t)colls[c].n_ranks);
-      chain_max[colls[c].chain] = std::max(chain_max[colls[c].chain], need);
-    }
-    for (int64_t m : chain_max) b += m;
-    return b;
-  }
 };
 
 // Link numbering and ECMP routing of one topology (S1, S2).
