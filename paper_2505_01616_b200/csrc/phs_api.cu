@@ -90,7 +90,7 @@ struct phs_sim {
   struct Unit {  // what one CTA / cluster simulates (see InstDesc)
     int32_t inst, n_flows, n_links;
     int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (see phs_finalize)
-    int64_t initial;  // flows without predecessors: PENDING from t = 0
+    int64_t bound_whole;  // the part of `bound` from raw flows and all-to-alls (may be in flight all at once)
   };
   std::vector<Unit> units;
   std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
@@ -106,9 +106,10 @@ struct phs_sim {
   DevBuf<FlowRec> d_rec;
   DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
   DevBuf<uint32_t> d_fmap;
+  DevBuf<int32_t> d_init_f;
   DevBuf<uint8_t> d_pc8;
   DevBuf<int64_t> d_capq, d_coll_first;
-  DevBuf<double> d_tdone, d_coll_t;
+  DevBuf<double> d_tdone, d_coll_t, d_init_t;
   DevBuf<InstResult> d_res;
   DevBuf<phs_event> d_log;
   DevBuf<int> d_ticket;
@@ -406,6 +407,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     std::vector<uint32_t> fmap;
     std::vector<uint8_t> pc8;
     std::vector<int64_t> capq;
+    std::vector<double> init_t;
+    std::vector<int32_t> init_f;
     std::vector<InstDesc> desc;  // bases relative to the chunk
     std::vector<phs_sim::Unit> units;
     int max_pred = 0;
@@ -514,9 +517,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     // one flow per sender PENDING or ACTIVE, twice the ring size because a slot freed in a phase is reused only in a
     // later one; collectives chained with `after` follow each other per rank, so a chain counts once, with its
     // largest member (a collective and its chain lie in one unit)
-    std::vector<int64_t> ubound((size_t)n_units, 0), uinit((size_t)n_units, 0);
+    std::vector<int64_t> ubound((size_t)n_units, 0), uwhole((size_t)n_units, 0);
     {
       for (int u = 0; u < n_units; ++u) ubound[u] = (int64_t)uflows[u].size();
+      for (int u = 0; u < n_units; ++u) uwhole[u] = (int64_t)uflows[u].size();  // minus the ring collectives' flows, below
       std::vector<int64_t> chain_max(in.colls.size(), 0);
       for (size_t c = 0; c < in.colls.size(); ++c) {
         if (in.colls[c].n_flows == 0) continue;
@@ -526,15 +530,17 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
                                  : std::min<int64_t>(in.colls[c].n_flows, 2 * (int64_t)in.colls[c].n_ranks);
         chain_max[in.colls[c].chain] = std::max(chain_max[in.colls[c].chain], need);
       }
-      for (size_t c = 0; c < in.colls.size(); ++c)
+      for (size_t c = 0; c < in.colls.size(); ++c) {
+        if (in.colls[c].n_flows > 0 && in.colls[c].kind != PHS_ALLTOALL)
+          uwhole[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
         if (chain_max[c] > 0) ubound[unit_of[in.colls[c].first_flow]] += chain_max[c];
-      for (int64_t f = 0; f < F; ++f) uinit[unit_of[f]] += in.pred_off[f + 1] == in.pred_off[f];
+      }
     }
     if (n_units == 0) {  // an instance without flows is one empty unit
       n_units = 1;
       uflows.resize(1);
       ubound.assign(1, 0);
-      uinit.assign(1, 0);
+      uwhole.assign(1, 0);
     }
     for (int u = 0; u < n_units; ++u) {
       const std::vector<int32_t> &fl = uflows[u];
@@ -556,6 +562,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       d.succ_base = (int64_t)c.succ.size();
       d.log_base = sim->want_log ? log_cursor : -1;
       d.pc8_base = (int64_t)c.pc8.size();
+      d.init_base = (int64_t)c.init_t.size();
+      d.pad_ = 0;
       d.n_flows = (int32_t)fl.size();
       d.n_links = (int32_t)links.size();
       for (int32_t l : links) {
@@ -589,6 +597,17 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         c.max_pred = std::max(c.max_pred, np);
         c.pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
       }
+      {  // flows without predecessors, by activation time start + Lat (the addition the kernels perform)
+        std::vector<std::pair<double, int32_t>> ini;
+        for (size_t k = 0; k < fl.size(); ++k)
+          if (in.pred_off[fl[k] + 1] == in.pred_off[fl[k]]) ini.emplace_back(in.start[fl[k]] + in.lat[fl[k]], (int32_t)k);
+        std::sort(ini.begin(), ini.end());
+        d.n_init = (int32_t)ini.size();
+        for (const auto &e : ini) {
+          c.init_t.push_back(e.first);
+          c.init_f.push_back(e.second);
+        }
+      }
       flow_cursor += (int64_t)fl.size();
       log_cursor += 2 * (int64_t)fl.size() + 2;
       c.desc.push_back(d);
@@ -597,7 +616,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       un.n_flows = d.n_flows;
       un.n_links = d.n_links;
       un.bound = ubound[u];
-      un.initial = uinit[u];
+      un.bound_whole = std::min(ubound[u], uwhole[u]);
       c.units.push_back(un);
     }
   };
@@ -605,7 +624,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   for (int i = 0; i < B; ++i)
     if (chunks[i].st != PHS_OK) return fail(chunks[i].st, chunks[i].err);
   // lay the chunks out back to back
-  std::vector<int64_t> b_flow(B + 1, 0), b_link(B + 1, 0), b_succ(B + 1, 0), b_pc8(B + 1, 0), b_log(B + 1, 0);
+  std::vector<int64_t> b_flow(B + 1, 0), b_link(B + 1, 0), b_succ(B + 1, 0), b_pc8(B + 1, 0), b_log(B + 1, 0),
+      b_init(B + 1, 0);
   sim->units.clear();
   sim->unit_first.assign(B + 1, 0);
   int max_pred = 0;
@@ -615,6 +635,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     b_link[i + 1] = b_link[i] + (int64_t)c.capq.size();
     b_succ[i + 1] = b_succ[i] + (int64_t)c.succ.size();
     b_pc8[i + 1] = b_pc8[i] + (int64_t)c.pc8.size();
+    b_init[i + 1] = b_init[i] + (int64_t)c.init_t.size();
     b_log[i + 1] = b_log[i] + 2 * (int64_t)c.rec.size() + 2 * (int64_t)c.units.size();
     sim->unit_first[i] = (int32_t)sim->units.size();
     sim->units.insert(sim->units.end(), c.units.begin(), c.units.end());
@@ -626,6 +647,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   std::vector<uint32_t> fmap((size_t)Ft);
   std::vector<uint8_t> pc8((size_t)b_pc8[B]);
   std::vector<int64_t> capq((size_t)b_link[B]);
+  std::vector<double> init_t((size_t)b_init[B]);
+  std::vector<int32_t> init_f((size_t)b_init[B]);
   sim->h_desc.assign(sim->units.size(), InstDesc{});
   parallel_for(B, [&](int i) {
     Chunk &c = chunks[i];
@@ -637,12 +660,15 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     std::copy(c.capq.begin(), c.capq.end(), capq.begin() + b_link[i]);
     std::copy(c.lcomp.begin(), c.lcomp.end(), lcomp.begin() + b_link[i]);
     std::copy(c.linkid.begin(), c.linkid.end(), linkid.begin() + b_link[i]);
+    std::copy(c.init_t.begin(), c.init_t.end(), init_t.begin() + b_init[i]);
+    std::copy(c.init_f.begin(), c.init_f.end(), init_f.begin() + b_init[i]);
     for (size_t k = 0; k < c.desc.size(); ++k) {
       InstDesc d = c.desc[k];
       d.flow_base += b_flow[i];
       d.link_base += b_link[i];
       d.succ_base += b_succ[i];
       d.pc8_base += b_pc8[i];
+      d.init_base += b_init[i];
       if (d.log_base >= 0) d.log_base += b_log[i];
       sim->h_desc[(size_t)sim->unit_first[i] + k] = d;
     }
@@ -659,6 +685,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(sim->d_succ.upload(succ, st));
   PHS_CUDA(sim->d_pc0.upload(pc0, st));
   PHS_CUDA(sim->d_fmap.upload(fmap, st));
+  PHS_CUDA(sim->d_init_t.upload(init_t, st));
+  PHS_CUDA(sim->d_init_f.upload(init_f, st));
   PHS_CUDA(sim->d_capq.upload(capq, st));
   PHS_CUDA(sim->d_lcomp.upload(lcomp, st));
   PHS_CUDA(sim->d_linkid.upload(linkid, st));
@@ -762,7 +790,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
   sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
                              (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size() + linkid.size() +
-                              fmap.size()) * 4 + (pc8_ok ? pc8.size() : 0) +
+                              fmap.size() + init_f.size()) * 4 + init_t.size() * 8 + (pc8_ok ? pc8.size() : 0) +
                              (capq.size() + coll_first.size()) * 8);
   PHS_CUDA(cudaEventCreate(&sim->ev0));
   PHS_CUDA(cudaEventCreate(&sim->ev1));
@@ -781,6 +809,8 @@ DevTables tables_of(phs_sim *sim, int n_links) {
   t.pred_cnt0 = sim->d_pc0.p;
   t.pred_cnt0_u8 = sim->d_pc8.p;
   t.fmap = sim->d_fmap.p;
+  t.init_t = sim->d_init_t.p;
+  t.init_f = sim->d_init_f.p;
   t.capq = sim->d_capq.p;
   t.lcomp = sim->d_lcomp.p;
   t.linkid = sim->d_linkid.p;
@@ -807,7 +837,8 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   int64_t target = 64;
   for (int u : list) {
     const phs_sim::Unit &un = sim->units[u];
-    target = std::max(target, std::max(un.initial, std::min(un.bound, un.bound * slot_scale / 4)));
+    const int64_t ring = un.bound - un.bound_whole;  // rarely all in flight at once: start from a quarter
+    target = std::max(target, un.bound_whole + std::min(ring, ring * slot_scale / 4));
     if (slot_scale > 4) target = std::max(target, std::min<int64_t>(un.n_flows, un.bound * slot_scale / 4));
   }
   const size_t smem_max = sim->smem_optin - 4096;  // minus the kernel's static shared memory

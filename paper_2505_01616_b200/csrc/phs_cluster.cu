@@ -137,6 +137,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   const int region = blockIdx.x / CS;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int ctid = crank * NT + tid;
+  const int CT = CS * NT;
   const int L = T.n_links;
   const int Lc = (L + CS - 1) / CS;
   const int Sc = (int)SC.Sc;
@@ -266,21 +267,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       S.tc[slot] = ta;
     };
 
-    // S4: flows without predecessors become PENDING; flow f starts in CTA f mod CS
-    for (int64_t f = crank + (int64_t)CS * tid; f < F; f += (int64_t)CS * NT) {
-      const int pc = pc0[f];
-      pred_cnt[f] = pc;
-      if (pc == 0) {
-        const FlowRec r = rec[f];
-        const int slot = atomicAdd(&ctl[M_HI], 1);
-        if (slot < Sc) {
-          fill_slot(slot, (int)fmap[f], r, __dadd_rn(r.start, r.lat));
-          atomicAdd(&ctl[M_NPEND], 1);
-        } else {
-          ctl[M_OVER] = 1;
-        }
-      }
-    }
+    // S4: outstanding predecessors.  Flows without predecessors are PENDING from t = 0 with t_act = start + Lat; they
+    // wait in the unit's list sorted by t_act (built by phs_finalize) and take a slot only when they activate.
+    for (int64_t f = ctid; f < F; f += CT) pred_cnt[f] = pc0[f];
+    const double *__restrict__ init_t = T.init_t + D.init_base;
+    const int32_t *__restrict__ init_f = T.init_f + D.init_base;
+    const int n_init = D.n_init;
+    int ip = 0;  // entries [0, ip) of the list have been activated (the same in every thread of the cluster)
+    double t_init = n_init > 0 ? __ldg(&init_t[0]) : kInf;
     __threadfence();  // pred_cnt[] is decremented by other CTAs of the cluster
     cluster.sync();
 
@@ -393,6 +387,28 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           for (int e = 0; e < nsucc; ++e) release2(succ[e0 + e], -1);
         }
       }
+      // flows without predecessors whose time has come: entry k of the sorted list is taken by CTA k mod CS
+      while (t_init <= t_next) {  // uniform over the cluster
+        const int k = ip + tid;
+        const bool due = k < n_init && __ldg(&init_t[k]) <= t_next;
+        if (due && (k & cmask) == crank) {
+          const int f = __ldg(&init_f[k]);
+          const FlowRec r = rec[f];
+          const int h = atomicAdd(&ctl[M_QHEAD], 1);
+          const int slot = h < qtail ? S.freeq[h % Sc] : atomicAdd(&ctl[M_HI], 1);
+          if (slot >= Sc) {
+            ctl[M_OVER] = 1;
+          } else {
+            atomicAdd(&ctl[M_NPEND], 1);  // activate() moves it from PENDING to ACTIVE
+            fill_slot(slot, (int)fmap[f], r, kInf);
+            activate(slot);
+          }
+        }
+        const int cnt = __syncthreads_count(due);
+        ip += cnt;
+        t_init = ip < n_init ? __ldg(&init_t[ip]) : kInf;
+        if (cnt < NT) break;
+      }
       PHS_TICK(0)
       __syncthreads();
       if (tid == 0) {  // publish this CTA's counts in CTA 0
@@ -423,7 +439,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         }
       }
       __syncthreads();
-      const int nA = bc[0], nPend = bc[1], over = bc[3];
+      const int nA = bc[0], nPend = bc[1] + (n_init - ip), over = bc[3];
       nDone = bc[2];
       max_slots = max(max_slots, bc[4]);
       if (LOG && ctid == 0) {
@@ -705,7 +721,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         for (int i = tid; i < nv; i += NT) vote(wl[i], false);
       }
       // ======== next time (a8)
-      t_next = bc_t;
+      t_next = dmin(bc_t, t_init);
       acc_min = kInf;
       if (LOG && ctid == 0) {
         first_bneck = -1;

@@ -14,6 +14,9 @@ struct DevTables {
   const int32_t *pred_cnt0;  // [F_total] number of predecessors
   const uint8_t *pred_cnt0_u8;  // same, packed 4 bits per flow (per-unit slices 4-byte aligned); unused if a count > 15
   const uint32_t *fmap;      // [F_total] unit-local flow -> index of the flow in t_done[] / bneck[]
+  const double *init_t;      // per unit [n_init] activation times start + Lat of the flows without predecessors,
+  const int32_t *init_f;     //   ascending (ties by flow id), and the flows themselves (cluster path: these flows
+                             //   take a slot only when they activate)
   const int64_t *capq;       // per unit [n_links] link capacity in rate quanta
   const int32_t *lcomp;      // per unit [n_links] static component (representative unit-local link) of every link
   const int32_t *linkid;     // per unit [n_links] unit-local link -> link id of the topology

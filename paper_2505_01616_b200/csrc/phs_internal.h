@@ -42,8 +42,11 @@ struct InstDesc {
   int64_t succ_base;  // first entry of the unit's slice of succ[]
   int64_t log_base;   // first row of the unit's event log slice (capacity 2F+2 rows), -1 if disabled
   int64_t pc8_base;   // first byte of the unit's slice of the packed predecessor counters (4-byte aligned)
+  int64_t init_base;  // first entry of the unit's slice of the initial-activation list (init_t / init_f)
   int32_t n_flows;
   int32_t n_links;
+  int32_t n_init;     // flows without predecessors
+  int32_t pad_;
 };
 
 // Per-instance result block (device, read back after a run).
