@@ -132,6 +132,19 @@ phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
  * instance-wide event sequence, so enabling it turns decomposition off.  Must precede phs_finalize. */
 phs_status phs_set_decomposition(phs_sim *sim, int32_t enable);
 
+/* Throughput history ("between neighboring events, network flows are assumed to have stable
+ * throughput"; L167: a flow's history is a few floating point numbers per throughput change, from which a time
+ * rollback reconstructs the state).  When enabled, every rate change of every flow is recorded as (time, new rate);
+ * a flow's records partition its life into intervals of constant throughput that end at its completion time.
+ * `max_records` bounds the records of one run over the whole batch; a run that produces more fails with PHS_ERANGE
+ * (the message names the number needed).  Must precede phs_finalize. */
+phs_status phs_enable_history(phs_sim *sim, int64_t max_records);
+/* History of one instance after phs_run, as CSR over its flows: off[F+1], then per record the time and the new
+ * rate in byte/s, chronological per flow.  n_records (nullable) receives the record count; t / rate_Bps may be
+ * null to query it; cap = capacity of t and rate_Bps. */
+phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *off, double *t, double *rate_Bps,
+                                int64_t cap, int64_t *n_records);
+
 /* Builds the device-resident tables (flow records, flow->link CSR, successor CSR, capacities) and copies them
  * to the current CUDA device on `cuda_stream` (cudaStream_t; NULL = default stream).  After this call the
  * instance set is frozen (adds return PHS_ESTATE).  phs_run calls it implicitly if needed. */

@@ -206,6 +206,16 @@ class Sim:
         _chk(lib().orc_get_work_counters(self._h, _p(out, C.c_double)), "orc_get_work_counters")
         return dict(zip(["sum_A", "sum_Ah", "sum_R", "sum_LamR", "sum_Lam", "completions", "events"], out.tolist()))
 
+    def history(self):
+        """Throughput history: (flow, t, rate) per rate change, sorted by (flow, t)."""
+        n = C.c_int64()
+        _chk(lib().orc_history_size(self._h, C.byref(n)), "orc_history_size")
+        fl = np.zeros(n.value, np.int32); t = np.zeros(n.value, np.float64); rate = np.zeros(n.value, np.float64)
+        _chk(lib().orc_get_history(self._h, _p(fl, C.c_int32), _p(t, C.c_double), _p(rate, C.c_double),
+                                   C.c_int64(n.value)), "orc_get_history")
+        order = np.lexsort((t, fl))
+        return fl[order], t[order], rate[order]
+
     def trace(self):
         n = C.c_int64()
         _chk(lib().orc_trace_size(self._h, C.byref(n)), "orc_trace_size")

@@ -53,6 +53,10 @@ struct orc_sim {
   int64_t n_ev, ev_cap;
   trace_row *tr;
   int64_t n_tr, tr_cap;
+  /* throughput history: one record per rate change of a flow */
+  int32_t *h_flow;
+  double *h_t, *h_rate;
+  int64_t n_h, h_cap;
   double work[7];
 };
 
@@ -124,6 +128,7 @@ void orc_destroy(orc_sim *s) {
   free(s->coll); free(s->cap); free(s->lat); free(s->src); free(s->dst); free(s->conn); free(s->bytes);
   free(s->start); free(s->Lat); free(s->path_off); free(s->path); free(s->pred_off); free(s->pred);
   free(s->t_done); free(s->bneck); free(s->ev); free(s->tr);
+  free(s->h_flow); free(s->h_t); free(s->h_rate);
   free(s);
 }
 
@@ -648,6 +653,20 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
     for (int32_t i = 0; i < nA; i++) {
       int32_t f = act[i];
       if (rq[f] != rq_cur[f]) {
+        if (s->n_h == s->h_cap) { /* history: the flow's throughput changes to rq[f] at `now` */
+          int64_t c = s->h_cap ? 2 * s->h_cap : 4096;
+          void *a = realloc(s->h_flow, sizeof(int32_t) * c), *b, *d;
+          if (!a) { rc = ORC_ENOMEM; goto out; }
+          s->h_flow = (int32_t *)a;
+          b = realloc(s->h_t, sizeof(double) * c);
+          if (!b) { rc = ORC_ENOMEM; goto out; }
+          s->h_t = (double *)b;
+          d = realloc(s->h_rate, sizeof(double) * c);
+          if (!d) { rc = ORC_ENOMEM; goto out; }
+          s->h_rate = (double *)d;
+          s->h_cap = c;
+        }
+        s->h_flow[s->n_h] = f; s->h_t[s->n_h] = now; s->h_rate[s->n_h] = q_to_rate(rq[f]); s->n_h++;
         if (rq_cur[f] >= 0) {
           double m = q_to_rate(rq_cur[f]) * (now - t_last[f]);
           double r = rem[f] - m;
@@ -782,6 +801,12 @@ int32_t orc_get_preds(const orc_sim *s, int64_t *off, int32_t *preds, int64_t ca
 int32_t orc_get_work_counters(const orc_sim *s, double *out7) {
   if (!s || !out7) return ORC_EINVAL;
   memcpy(out7, s->work, sizeof(s->work));
+  return ORC_OK;
+}
+int32_t orc_history_size(const orc_sim *s, int64_t *n) { if (!s || !n) return ORC_EINVAL; *n = s->n_h; return ORC_OK; }
+int32_t orc_get_history(const orc_sim *s, int32_t *flow, double *t, double *rate, int64_t cap) {
+  if (!s || cap < s->n_h) return ORC_EINVAL;
+  for (int64_t i = 0; i < s->n_h; i++) { flow[i] = s->h_flow[i]; t[i] = s->h_t[i]; rate[i] = s->h_rate[i]; }
   return ORC_OK;
 }
 int32_t orc_trace_size(const orc_sim *s, int64_t *n) { if (!s || !n) return ORC_EINVAL; *n = s->n_tr; return ORC_OK; }

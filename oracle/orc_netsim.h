@@ -93,6 +93,12 @@ int32_t orc_get_preds(const orc_sim *s, int64_t *off /*[F+1]*/, int32_t *preds, 
  * active flows), [2] sum of water-filling iterations R, [3] sum over events of Lambda_act*R,
  * [4] sum Lambda_act, [5] completions, [6] events */
 int32_t orc_get_work_counters(const orc_sim *s, double *out7);
+/* throughput history (PAPER.md L128 / L167; reading R-LZ): one record (flow, time, new rate in byte/s) per rate
+ * change of a flow, in the order the event loop produced them (chronological; within an event in the order of
+ * the active list).  A flow's records partition its life into intervals of constant throughput:
+ * bytes = sum rate_i * (t_{i+1} - t_i) with the completion time closing the last interval. */
+int32_t orc_history_size(const orc_sim *s, int64_t *n_records);
+int32_t orc_get_history(const orc_sim *s, int32_t *flow, double *t, double *rate_Bps, int64_t cap);
 /* trace access (valid after orc_run(..., trace=1)) */
 int32_t orc_trace_size(const orc_sim *s, int64_t *n_rows);
 int32_t orc_get_trace(const orc_sim *s, int64_t *event_idx, int32_t *flow, double *rate_Bps, double *t0, double *t1,

@@ -39,7 +39,8 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
 # every symbol include/phs.h declares (tests check that the library exports all of them)
 SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_batch", "phs_add_flows",
-           "phs_enable_event_log", "phs_set_scheduler", "phs_set_decomposition", "phs_finalize", "phs_run", "phs_num_flows", "phs_total_flows",
+           "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
+           "phs_set_decomposition", "phs_finalize", "phs_run", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
            "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
@@ -160,6 +161,22 @@ def phs_enable_event_log(h, enable=True):
 
 def phs_set_scheduler(h, path=0, cta_slots=0):
     _chk(lib().phs_set_scheduler(h, C.c_int32(path), C.c_int32(cta_slots)), "phs_set_scheduler")
+
+
+def phs_enable_history(h, max_records):
+    _chk(lib().phs_enable_history(h, C.c_int64(max_records)), "phs_enable_history")
+
+
+def phs_get_flow_history(h, instance):
+    """(off[F+1], t[n], rate_Bps[n]): the rate changes of every flow of the instance, chronological per flow."""
+    n = C.c_int64()
+    _chk(lib().phs_get_flow_history(h, C.c_int32(instance), None, None, None, C.c_int64(0), C.byref(n)),
+         "phs_get_flow_history")
+    F = phs_num_flows(h, instance)
+    off = np.zeros(F + 1, np.int64); t = np.zeros(n.value, np.float64); rate = np.zeros(n.value, np.float64)
+    _chk(lib().phs_get_flow_history(h, C.c_int32(instance), _p(off), _p(t), _p(rate), C.c_int64(n.value),
+                                    C.byref(n)), "phs_get_flow_history")
+    return off, t, rate
 
 
 def phs_set_decomposition(h, enable=True):
@@ -295,13 +312,15 @@ class Sim:
     """Owns a phs_sim handle.  Methods forward to the C-named calls above."""
 
     def __init__(self, desc: dict, seed: int = 0, batch: int = 1, event_log: bool = False, path: int = 0,
-                 cta_slots: int = 0, decompose: bool = True):
+                 cta_slots: int = 0, decompose: bool = True, history: int = 0):
         self.h = phs_create_topology(desc, seed, batch)
         self.batch = batch
         if event_log:
             phs_enable_event_log(self.h, True)
         if not decompose:
             phs_set_decomposition(self.h, False)
+        if history:
+            phs_enable_history(self.h, history)
         if path or cta_slots:
             phs_set_scheduler(self.h, path, cta_slots)
 
@@ -317,12 +336,12 @@ class Sim:
             pass
 
     @classmethod
-    def from_workload(cls, w, event_log=False, instances=None, path=0, cta_slots=0, decompose=True):
+    def from_workload(cls, w, event_log=False, instances=None, path=0, cta_slots=0, decompose=True, history=0):
         """Builds a batch from a workloads.Workload (optionally a subset of its instances; instance i keeps its own
         seed only if the subset is a contiguous range, so subsets are given as (first, count))."""
         first, count = (0, w.batch) if instances is None else instances
         sim = cls(w.desc, seed=w.base_seed + w.instances[first].seed, batch=count, event_log=event_log, path=path,
-                  cta_slots=cta_slots, decompose=decompose)
+                  cta_slots=cta_slots, decompose=decompose, history=history)
         n_links = phs_num_links(sim.h)
         insts = w.instances[first:first + count]
         for i, inst in enumerate(insts):
@@ -385,6 +404,9 @@ class Sim:
 
     def flows(self, i):
         return phs_get_flow_table(self.h, i)
+
+    def history(self, i):
+        return phs_get_flow_history(self.h, i)
 
     def counters(self):
         return phs_get_counters(self.h)

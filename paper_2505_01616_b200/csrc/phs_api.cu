@@ -106,6 +106,11 @@ struct phs_sim {
   DevBuf<FlowRec> d_rec;
   DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
   DevBuf<uint32_t> d_fmap;
+  // throughput history (optional)
+  int64_t hist_cap = 0;
+  DevBuf<HistRec> d_hist;
+  DevBuf<unsigned long long> d_hist_n;
+  std::vector<HistRec> h_hist;  // records of the last run, sorted by (flow, event), duplicates of re-runs removed
   DevBuf<int32_t> d_init_f;
   DevBuf<uint8_t> d_pc8;
   DevBuf<int64_t> d_capq, d_coll_first;
@@ -285,6 +290,14 @@ phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
   if (sim->finalized) return fail(PHS_ESTATE, "scheduler policy must be chosen before phs_finalize");
   sim->policy_path = path;
   sim->policy_slots = cta_slots;
+  return PHS_OK;
+}
+
+phs_status phs_enable_history(phs_sim *sim, int64_t max_records) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (max_records < 0) return fail(PHS_EINVAL, "max_records must be >= 0");
+  if (sim->finalized) return fail(PHS_ESTATE, "history must be chosen before phs_finalize");
+  sim->hist_cap = max_records;
   return PHS_OK;
 }
 
@@ -699,6 +712,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(sim->d_res.alloc((size_t)U));
   PHS_CUDA(sim->d_ticket.alloc(1));
   if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)log_cursor));
+  if (sim->hist_cap > 0) {
+    PHS_CUDA(sim->d_hist.alloc((size_t)sim->hist_cap));
+    PHS_CUDA(sim->d_hist_n.alloc(1));
+  }
   sim->h_res.assign(U, InstResult{});
 
   // ---- a9: batch scheduler, static part.  A unit whose state fits the shared memory of one SM goes to the CTA
@@ -819,6 +836,9 @@ DevTables tables_of(phs_sim *sim, int n_links) {
   t.bneck = sim->d_bneck.p;
   t.res = sim->d_res.p;
   t.log = sim->want_log ? sim->d_log.p : nullptr;
+  t.hist = sim->hist_cap > 0 ? sim->d_hist.p : nullptr;
+  t.hist_n = sim->d_hist_n.p;
+  t.hist_cap = sim->hist_cap;
   t.n_links = n_links;
   return t;
 }
@@ -910,6 +930,7 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   DevTables t = tables_of(sim, sim->cta.n_links);
   sim->n_launches = 0;
   PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
+  if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
   PHS_CUDA(cudaEventRecord(sim->ev0, st));
   if (!sim->order.empty()) {
     sim->n_launches++;
@@ -958,6 +979,23 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   if (sim->total_colls > 0) sim->n_launches++;
   PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
                                    sim->d_coll_t.p, st));
+  if (sim->hist_cap > 0) {  // throughput history: fetch, order by (flow, event); a re-run unit repeats its records
+    unsigned long long n = 0;
+    PHS_CUDA(cudaMemcpyAsync(&n, sim->d_hist_n.p, sizeof(n), cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    if (n > (unsigned long long)sim->hist_cap)
+      return fail(PHS_ERANGE, "throughput history needs " + std::to_string(n) + " records, max_records is " +
+                                  std::to_string(sim->hist_cap));
+    sim->h_hist.resize((size_t)n);
+    if (n) PHS_CUDA(cudaMemcpyAsync(sim->h_hist.data(), sim->d_hist.p, sizeof(HistRec) * n, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    std::sort(sim->h_hist.begin(), sim->h_hist.end(), [](const HistRec &a, const HistRec &b) {
+      return a.flow != b.flow ? a.flow < b.flow : a.ev < b.ev;
+    });
+    sim->h_hist.erase(std::unique(sim->h_hist.begin(), sim->h_hist.end(),
+                                  [](const HistRec &a, const HistRec &b) { return a.flow == b.flow && a.ev == b.ev; }),
+                      sim->h_hist.end());
+  }
   sim->ran = true;
   for (int u = 0; u < U; ++u) {
     const int i = sim->units[u].inst;
@@ -1032,6 +1070,33 @@ phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *ou
   if (!out) return PHS_OK;
   return fetch(sim, sim->d_log.p, sim->h_desc[sim->unit_first[instance]].log_base, std::min<int64_t>(cap, *n_events),
                out, 0);
+}
+
+phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *off, double *t, double *rate,
+                                int64_t cap, int64_t *n_records) {
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
+  if (sim->hist_cap <= 0) return fail(PHS_ESTATE, "throughput history was not enabled");
+  const uint32_t lo = (uint32_t)sim->flow_base[instance], hi = (uint32_t)sim->flow_base[instance + 1];
+  auto by_flow = [](const HistRec &r, uint32_t f) { return r.flow < f; };
+  const auto b = std::lower_bound(sim->h_hist.begin(), sim->h_hist.end(), lo, by_flow);
+  const auto e = std::lower_bound(sim->h_hist.begin(), sim->h_hist.end(), hi, by_flow);
+  const int64_t n = (int64_t)(e - b);
+  if (n_records) *n_records = n;
+  if (!t && !rate && !off) return PHS_OK;
+  if (!t || !rate || !off || cap < n) return fail(PHS_EINVAL, "output too small");
+  int64_t k = 0;
+  auto it = b;
+  for (uint32_t f = lo; f < hi; ++f) {
+    off[f - lo] = k;
+    for (; it != e && it->flow == f; ++it, ++k) {
+      t[k] = it->t;
+      rate[k] = it->rate;
+    }
+  }
+  off[hi - lo] = k;
+  return PHS_OK;
 }
 
 phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {

@@ -7,6 +7,13 @@
 
 namespace phs {
 
+struct HistRec {     // one rate change of one flow (throughput history, PAPER.md L128 / L167)
+  double t;          // when
+  double rate;       // new rate, byte/s
+  uint32_t flow;     // position of the flow in t_done[] / bneck[]
+  uint32_t ev;       // index of the unit's event that changed it (orders changes at one and the same time)
+};
+
 struct DevTables {
   const InstDesc *inst;      // [U] simulation units
   const FlowRec *rec;        // [F_total] unit-local link / flow ids inside
@@ -25,6 +32,9 @@ struct DevTables {
   int32_t *bneck;            // [F_total] O3, topology link ids
   InstResult *res;           // [U]
   phs_event *log;            // event log rows, or nullptr
+  HistRec *hist;             // throughput history records, or nullptr
+  unsigned long long *hist_n;  // records produced (may exceed hist_cap: the excess is dropped and reported)
+  long long hist_cap;
   int32_t n_links;           // largest n_links among the units of this launch (sizes the shared-memory layout)
 };
 

@@ -254,3 +254,30 @@ def test_random_dags_of_raw_flows(seed):
                                                         np.array(dep_ids, np.int64))]))
     w = W.Workload("fuzz", d, 7 * seed, insts)
     run_and_compare(w, path=[0, CTA, CLUSTER][seed % 3], mode=orc.MODE_FAST)
+
+
+@pytest.mark.parametrize("path", [CTA, CLUSTER])
+def test_throughput_history_equals_the_oracle(path):
+    """NEXT-1 groundwork (PAPER.md L128 / L167): the per-flow list of (time, new rate) rate changes.  Bit-equal to the
+    oracle's, with and without decomposition, and it reconstructs every flow's bytes."""
+    w = W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
+    for decompose in (True, False):
+        sim = B.Sim.from_workload(w, path=path, decompose=decompose, history=1 << 20)
+        sim.run()
+        for i in range(w.batch):
+            o = oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST)
+            fl, t, r = o.history()
+            off, tg, rg = sim.history(i)
+            assert off[-1] == len(fl)
+            assert np.array_equal(np.diff(off), np.bincount(fl, minlength=o.num_flows))
+            assert np.array_equal(tg, t) and np.array_equal(rg, r)
+            td, nbytes = sim.completion_times(i), o.flows()[2]
+            for f in range(0, o.num_flows, 37):      # constant-throughput intervals add up to the flow's size
+                tt = np.append(tg[off[f]:off[f + 1]], td[f])
+                assert abs(np.sum(rg[off[f]:off[f + 1]] * np.diff(tt)) - nbytes[f]) <= 1e-9 * nbytes[f]
+        sim.close()
+    small = B.Sim.from_workload(w, path=path, history=100)           # too small: refused, with the count needed
+    with pytest.raises(B.PhsError) as e:
+        small.run()
+    assert e.value.code == B.PHS_ERANGE and "needs" in str(e.value)
+    small.close()

@@ -500,6 +500,30 @@ def test_p9_locality_unrelated_traffic_does_not_change_a_single_bit():
     assert np.array_equal(ab.bottlenecks()[:n], a.bottlenecks())
 
 
+def test_p9_history_partitions_every_flow_into_constant_rate_intervals():
+    """Throughput history (PAPER.md L128 / L167): the recorded (time, rate) changes of a flow, closed by its
+    completion time, add up to its size; rates within one interval set never exceed a link (checked at the sampled
+    event times through the trace) and the first record of a flow is its activation."""
+    w = W.cfg4(batch=1, n_hosts=4, gph=4, n_leaves=2, n_spines=2)
+    o = oracle_run(w.desc, w.instances[0], trace=True)
+    fl, t, r = o.history()
+    td, (src, dst, nbytes, lat) = o.completion_times(), o.flows()
+    assert np.array_equal(np.unique(fl), np.arange(o.num_flows))          # every flow has at least one record
+    for f in range(o.num_flows):
+        m = fl == f
+        tt = np.append(t[m], td[f])
+        assert np.all(np.diff(tt) >= 0) and np.all(r[m] > 0)
+        assert tt[0] == lat[f]                                             # activation = start (0) + path latency
+        assert abs(np.sum(r[m] * np.diff(tt)) - nbytes[f]) <= 1e-12 * nbytes[f]
+    # the history is the trace with repeated rates dropped
+    ev, tfl, trate, t0, t1 = o.trace()
+    for f in (0, 7, 100):
+        m = tfl == f
+        rates, times = trate[m], t0[m]
+        keep = np.append([True], rates[1:] != rates[:-1])
+        assert np.array_equal(rates[keep], r[fl == f]) and np.array_equal(times[keep], t[fl == f])
+
+
 def test_p9_single_spine_is_seed_independent():
     d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=1, uplinks_per_leaf_spine=1)
     ops = [W.Coll(W.ALLREDUCE_RING, np.arange(0, 16, 2, dtype=np.int32), 32 * MiB),
