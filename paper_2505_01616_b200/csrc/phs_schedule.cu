@@ -1,0 +1,642 @@
+// phs_schedule.cu -- phs_finalize (simulation units, device-resident tables, static part of the batch scheduler)
+// and phs_run (launches, overflow handling, throughput-history fetch): SURVEY.md 8(a) a9.  No CPU fallback
+// exists: without a usable CUDA device both fail with PHS_ECUDA.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+
+#include "phs_sim.h"
+
+using namespace phs;
+
+#define fail phs_fail
+
+// ================================================================================================ finalize
+// Builds the device-resident tables.  HBM layout: one 32-byte FlowRec per flow (+1
+// sentinel per instance), flow->link CSR values, successor CSR values (transpose of the dependency lists),
+// per-instance capacity rows in rate quanta, and the dynamic per-flow arrays (pred_cnt, t_done, bneck).
+extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (sim->finalized) return PHS_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  PHS_CUDA(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  PHS_CUDA(cudaGetDeviceProperties(&prop, dev));
+  sim->sm_count = prop.multiProcessorCount;
+  sim->smem_optin = (size_t)prop.sharedMemPerBlockOptin;
+  const int B = sim->batch, L = sim->fab->n_links();
+
+  sim->flow_base.assign(B + 1, 0);
+  sim->coll_base.assign(B + 1, 0);
+  for (int i = 0; i < B; ++i) {
+    sim->flow_base[i + 1] = sim->flow_base[i] + sim->inst[i].n_flows();
+    sim->coll_base[i + 1] = sim->coll_base[i] + (int64_t)sim->inst[i].colls.size();
+  }
+  sim->total_flows = sim->flow_base[B];
+  sim->total_colls = sim->coll_base[B];
+  const int64_t Ft = sim->total_flows;
+  if (Ft >= 0x7fffffffLL) return fail(PHS_ERANGE, "more than 2^31 - 1 flows in one batch");
+  const bool split = sim->decompose && !sim->want_log;  // the event log is an instance-wide sequence
+
+  // ---- simulation units (a9).  Flows that share a link, directly or through a chain of flows, and flows joined by
+  // a dependency evolve together; such a group shares nothing with the rest of its instance, so (reading R-LZ) it
+  // can be simulated on its own with bit-identical results.  Every unit gets dense local flow and link ids.
+  // per-instance work is independent: every instance builds its own chunk of the tables on a host thread, the
+  // chunks are then laid out back to back
+  struct Chunk {
+    std::vector<FlowRec> rec;
+    std::vector<int32_t> succ, pc0, lcomp, linkid;
+    std::vector<uint32_t> fmap;
+    std::vector<uint8_t> pc8;
+    std::vector<int64_t> capq;
+    std::vector<double> init_t;
+    std::vector<int32_t> init_f;
+    std::vector<InstDesc> desc;  // bases relative to the chunk
+    std::vector<phs_sim::Unit> units;
+    int max_pred = 0;
+    phs_status st = PHS_OK;
+    const char *err = "";
+  };
+  std::vector<Chunk> chunks((size_t)B);
+  std::vector<int64_t> coll_first((size_t)sim->total_colls);
+  std::vector<int32_t> coll_n((size_t)sim->total_colls);
+  auto build_instance = [&](int i) {
+    Chunk &c = chunks[(size_t)i];
+    const Instance &in = sim->inst[i];
+    const int64_t F = in.n_flows();
+    c.rec.resize((size_t)F);
+    c.pc0.resize((size_t)F);
+    c.fmap.resize((size_t)F);
+    int64_t flow_cursor = 0, log_cursor = 0;
+    std::vector<int64_t> capq_inst((size_t)L);
+    std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
+    // capacities -> rate quanta (floor); every fair share must stay >= 1 quantum
+    for (int l = 0; l < L; ++l) {
+      const double cap_l = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
+      const int64_t q = (int64_t)std::floor(cap_l * 1048576.0);
+      if (q < F + 1) {
+        c.st = PHS_ERANGE;
+        c.err = "a link capacity is below (#flows + 1) rate quanta of 2^-20 byte/s";
+        return;
+      }
+      capq_inst[l] = q;
+    }
+    for (size_t c = 0; c < in.colls.size(); ++c) {
+      coll_first[sim->coll_base[i] + c] = sim->flow_base[i] + in.colls[c].first_flow;
+      coll_n[sim->coll_base[i] + c] = in.colls[c].n_flows;
+    }
+    // successor CSR = transpose of the pred lists (counting sort by predecessor)
+    std::vector<uint32_t> soff((size_t)F + 1, 0);
+    std::vector<int32_t> sdst(in.pred.size());
+    for (int32_t p : in.pred) soff[(size_t)p + 1]++;
+    for (int64_t f = 0; f < F; ++f) soff[f + 1] += soff[f];
+    {
+      std::vector<uint32_t> cur(soff.begin(), soff.end() - 1);
+      for (int64_t f = 0; f < F; ++f)
+        for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e) sdst[cur[in.pred[e]]++] = (int32_t)f;
+    }
+    // static link components (union-find over the links, joined by every flow's path; the representative is the
+    // smallest link id), and on top of them the units (link components joined by dependencies)
+    std::iota(parent.begin(), parent.end(), 0);
+    auto find_in = [](std::vector<int32_t> &par, int32_t x) {
+      while (par[x] != x) {
+        par[x] = par[par[x]];
+        x = par[x];
+      }
+      return x;
+    };
+    auto unite = [&](std::vector<int32_t> &par, int32_t a, int32_t b) {
+      a = find_in(par, a);
+      b = find_in(par, b);
+      if (a != b) par[std::max(a, b)] = std::min(a, b);
+    };
+    for (int64_t f = 0; f < F; ++f)
+      for (uint32_t e = in.path_off[f] + 1; e < in.path_off[f + 1]; ++e)
+        unite(parent, in.path[in.path_off[f]], in.path[e]);
+    uparent = parent;
+    for (int64_t f = 0; f < F; ++f)
+      for (uint32_t e = in.pred_off[f]; e < in.pred_off[f + 1]; ++e)
+        unite(uparent, in.path[in.path_off[f]], in.path[in.path_off[in.pred[e]]]);
+    // unit of every flow: groups in order of first appearance; groups below 64 flows share bins of up to 256
+    std::vector<int32_t> unit_of((size_t)F, 0);
+    int32_t n_units = F > 0 ? 1 : 0;
+    if (split && F > 0) {
+      std::vector<int32_t> group_of_root((size_t)L, -1), gsize;
+      for (int64_t f = 0; f < F; ++f) {
+        const int32_t r = find_in(uparent, in.path[in.path_off[f]]);
+        if (group_of_root[r] < 0) {
+          group_of_root[r] = (int32_t)gsize.size();
+          gsize.push_back(0);
+        }
+        unit_of[f] = group_of_root[r];
+        gsize[unit_of[f]]++;
+      }
+      std::vector<int32_t> unit_of_group(gsize.size());
+      n_units = 0;
+      int32_t bin = -1, bin_flows = 0;
+      for (size_t g = 0; g < gsize.size(); ++g) {
+        if (gsize[g] >= 64) {
+          unit_of_group[g] = n_units++;
+        } else {
+          if (bin < 0 || bin_flows >= 256) {
+            bin = n_units++;
+            bin_flows = 0;
+          }
+          unit_of_group[g] = bin;
+          bin_flows += gsize[g];
+        }
+      }
+      for (int64_t f = 0; f < F; ++f) unit_of[f] = unit_of_group[unit_of[f]];
+    }
+    // flows of every unit in ascending flow id; local flow ids
+    std::vector<std::vector<int32_t>> uflows((size_t)n_units);
+    std::vector<int32_t> flow_loc((size_t)F);
+    for (int64_t f = 0; f < F; ++f) {
+      flow_loc[f] = (int32_t)uflows[unit_of[f]].size();
+      uflows[unit_of[f]].push_back((int32_t)f);
+    }
+    // slots a unit can need: raw flows and all-to-alls may be in flight as a whole; a ring collective keeps at most
+    // one flow per sender PENDING or ACTIVE, twice the ring size because a slot freed in a phase is reused only in a
+    // later one; collectives chained with `after` follow each other per rank, so a chain counts once, with its
+    // largest member (a collective and its chain lie in one unit)
+    std::vector<int64_t> ubound((size_t)n_units, 0), uwhole((size_t)n_units, 0);
+    {
+      for (int u = 0; u < n_units; ++u) ubound[u] = (int64_t)uflows[u].size();
+      for (int u = 0; u < n_units; ++u) uwhole[u] = (int64_t)uflows[u].size();  // minus the ring collectives' flows, below
+      std::vector<int64_t> chain_max(in.colls.size(), 0);
+      for (size_t c = 0; c < in.colls.size(); ++c) {
+        if (in.colls[c].n_flows == 0) continue;
+        ubound[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
+        const int64_t need = in.colls[c].kind == PHS_ALLTOALL
+                                 ? in.colls[c].n_flows
+                                 : std::min<int64_t>(in.colls[c].n_flows, 2 * (int64_t)in.colls[c].n_ranks);
+        chain_max[in.colls[c].chain] = std::max(chain_max[in.colls[c].chain], need);
+      }
+      for (size_t c = 0; c < in.colls.size(); ++c) {
+        if (in.colls[c].n_flows > 0 && in.colls[c].kind != PHS_ALLTOALL)
+          uwhole[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
+        if (chain_max[c] > 0) ubound[unit_of[in.colls[c].first_flow]] += chain_max[c];
+      }
+    }
+    if (n_units == 0) {  // an instance without flows is one empty unit
+      n_units = 1;
+      uflows.resize(1);
+      ubound.assign(1, 0);
+      uwhole.assign(1, 0);
+    }
+    for (int u = 0; u < n_units; ++u) {
+      const std::vector<int32_t> &fl = uflows[u];
+      // links of the unit, ascending; an undivided instance keeps the whole topology (local id = topology id)
+      std::vector<int32_t> links;
+      if (n_units == 1) {
+        links.resize((size_t)L);
+        std::iota(links.begin(), links.end(), 0);
+      } else {
+        for (int32_t f : fl)
+          for (uint32_t e = in.path_off[f]; e < in.path_off[f + 1]; ++e) links.push_back(in.path[e]);
+        std::sort(links.begin(), links.end());
+        links.erase(std::unique(links.begin(), links.end()), links.end());
+      }
+      for (size_t k = 0; k < links.size(); ++k) link_loc[links[k]] = (int32_t)k;
+      InstDesc d;
+      d.flow_base = flow_cursor;
+      d.link_base = (int64_t)c.capq.size();
+      d.succ_base = (int64_t)c.succ.size();
+      d.log_base = sim->want_log ? log_cursor : -1;
+      d.pc8_base = (int64_t)c.pc8.size();
+      d.init_base = (int64_t)c.init_t.size();
+      d.pad_ = 0;
+      d.n_flows = (int32_t)fl.size();
+      d.n_links = (int32_t)links.size();
+      for (int32_t l : links) {
+        c.capq.push_back(capq_inst[l]);
+        c.lcomp.push_back(link_loc[find_in(parent, l)]);  // the smallest link of a component is in the unit too
+        c.linkid.push_back(l);
+      }
+      c.pc8.resize(c.pc8.size() + (fl.size() + 7) / 8 * 4, 0);
+      for (size_t k = 0; k < fl.size(); ++k) {
+        const int32_t f = fl[k];
+        FlowRec x;
+        x.bytes = in.bytes[f];
+        x.start = in.start[f];
+        x.lat = in.lat[f];
+        const uint32_t p0 = in.path_off[f], p1 = in.path_off[f + 1];
+        for (int h = 0; h < kMaxHops; ++h) x.path[h] = p0 + h < p1 ? link_loc[in.path[p0 + h]] : -1;
+        x.succ_cnt = (int32_t)(soff[f + 1] - soff[f]);
+        if (x.succ_cnt <= 2) {
+          x.succ_in[0] = x.succ_cnt > 0 ? flow_loc[sdst[soff[f]]] : -1;
+          x.succ_in[1] = x.succ_cnt > 1 ? flow_loc[sdst[soff[f] + 1]] : -1;
+        } else {
+          x.succ_in[0] = (int32_t)((int64_t)c.succ.size() - d.succ_base);
+          x.succ_in[1] = -1;
+          for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) c.succ.push_back(flow_loc[sdst[e]]);
+        }
+        x.comp = p0 < p1 ? link_loc[find_in(parent, in.path[p0])] : 0;
+        c.rec[(size_t)flow_cursor + k] = x;
+        c.fmap[(size_t)flow_cursor + k] = (uint32_t)(sim->flow_base[i] + f);
+        const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
+        c.pc0[(size_t)flow_cursor + k] = np;
+        c.max_pred = std::max(c.max_pred, np);
+        c.pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
+      }
+      {  // flows without predecessors, by activation time start + Lat (the addition the kernels perform)
+        std::vector<std::pair<double, int32_t>> ini;
+        for (size_t k = 0; k < fl.size(); ++k)
+          if (in.pred_off[fl[k] + 1] == in.pred_off[fl[k]]) ini.emplace_back(in.start[fl[k]] + in.lat[fl[k]], (int32_t)k);
+        std::sort(ini.begin(), ini.end());
+        d.n_init = (int32_t)ini.size();
+        for (const auto &e : ini) {
+          c.init_t.push_back(e.first);
+          c.init_f.push_back(e.second);
+        }
+      }
+      flow_cursor += (int64_t)fl.size();
+      log_cursor += 2 * (int64_t)fl.size() + 2;
+      c.desc.push_back(d);
+      phs_sim::Unit un;
+      un.inst = i;
+      un.n_flows = d.n_flows;
+      un.n_links = d.n_links;
+      un.bound = ubound[u];
+      un.bound_whole = std::min(ubound[u], uwhole[u]);
+      c.units.push_back(un);
+    }
+  };
+  parallel_for(B, build_instance);
+  for (int i = 0; i < B; ++i)
+    if (chunks[i].st != PHS_OK) return fail(chunks[i].st, chunks[i].err);
+  // lay the chunks out back to back
+  std::vector<int64_t> b_flow(B + 1, 0), b_link(B + 1, 0), b_succ(B + 1, 0), b_pc8(B + 1, 0), b_log(B + 1, 0),
+      b_init(B + 1, 0);
+  sim->units.clear();
+  sim->unit_first.assign(B + 1, 0);
+  int max_pred = 0;
+  for (int i = 0; i < B; ++i) {
+    const Chunk &c = chunks[i];
+    b_flow[i + 1] = b_flow[i] + (int64_t)c.rec.size();
+    b_link[i + 1] = b_link[i] + (int64_t)c.capq.size();
+    b_succ[i + 1] = b_succ[i] + (int64_t)c.succ.size();
+    b_pc8[i + 1] = b_pc8[i] + (int64_t)c.pc8.size();
+    b_init[i + 1] = b_init[i] + (int64_t)c.init_t.size();
+    b_log[i + 1] = b_log[i] + 2 * (int64_t)c.rec.size() + 2 * (int64_t)c.units.size();
+    sim->unit_first[i] = (int32_t)sim->units.size();
+    sim->units.insert(sim->units.end(), c.units.begin(), c.units.end());
+    max_pred = std::max(max_pred, c.max_pred);
+  }
+  const int64_t log_cursor = b_log[B];
+  std::vector<FlowRec> rec((size_t)Ft);
+  std::vector<int32_t> succ((size_t)b_succ[B]), pc0((size_t)Ft), lcomp((size_t)b_link[B]), linkid((size_t)b_link[B]);
+  std::vector<uint32_t> fmap((size_t)Ft);
+  std::vector<uint8_t> pc8((size_t)b_pc8[B]);
+  std::vector<int64_t> capq((size_t)b_link[B]);
+  std::vector<double> init_t((size_t)b_init[B]);
+  std::vector<int32_t> init_f((size_t)b_init[B]);
+  sim->h_desc.assign(sim->units.size(), InstDesc{});
+  parallel_for(B, [&](int i) {
+    Chunk &c = chunks[i];
+    std::copy(c.rec.begin(), c.rec.end(), rec.begin() + b_flow[i]);
+    std::copy(c.pc0.begin(), c.pc0.end(), pc0.begin() + b_flow[i]);
+    std::copy(c.fmap.begin(), c.fmap.end(), fmap.begin() + b_flow[i]);
+    std::copy(c.succ.begin(), c.succ.end(), succ.begin() + b_succ[i]);
+    std::copy(c.pc8.begin(), c.pc8.end(), pc8.begin() + b_pc8[i]);
+    std::copy(c.capq.begin(), c.capq.end(), capq.begin() + b_link[i]);
+    std::copy(c.lcomp.begin(), c.lcomp.end(), lcomp.begin() + b_link[i]);
+    std::copy(c.linkid.begin(), c.linkid.end(), linkid.begin() + b_link[i]);
+    std::copy(c.init_t.begin(), c.init_t.end(), init_t.begin() + b_init[i]);
+    std::copy(c.init_f.begin(), c.init_f.end(), init_f.begin() + b_init[i]);
+    for (size_t k = 0; k < c.desc.size(); ++k) {
+      InstDesc d = c.desc[k];
+      d.flow_base += b_flow[i];
+      d.link_base += b_link[i];
+      d.succ_base += b_succ[i];
+      d.pc8_base += b_pc8[i];
+      d.init_base += b_init[i];
+      if (d.log_base >= 0) d.log_base += b_log[i];
+      sim->h_desc[(size_t)sim->unit_first[i] + k] = d;
+    }
+    Chunk().rec.swap(c.rec);  // release the chunk's big arrays early
+    std::vector<uint32_t>().swap(c.fmap);
+  });
+  sim->unit_first[B] = (int32_t)sim->units.size();
+  const int U = (int)sim->units.size();
+  const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
+
+  PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
+  PHS_CUDA(sim->d_rec.upload(rec, st));
+  if (pc8_ok) PHS_CUDA(sim->d_pc8.upload(pc8, st));
+  PHS_CUDA(sim->d_succ.upload(succ, st));
+  PHS_CUDA(sim->d_pc0.upload(pc0, st));
+  PHS_CUDA(sim->d_fmap.upload(fmap, st));
+  PHS_CUDA(sim->d_init_t.upload(init_t, st));
+  PHS_CUDA(sim->d_init_f.upload(init_f, st));
+  PHS_CUDA(sim->d_capq.upload(capq, st));
+  PHS_CUDA(sim->d_lcomp.upload(lcomp, st));
+  PHS_CUDA(sim->d_linkid.upload(linkid, st));
+  PHS_CUDA(sim->d_coll_first.upload(coll_first, st));
+  PHS_CUDA(sim->d_coll_n.upload(coll_n, st));
+  PHS_CUDA(sim->d_pred_cnt.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_tdone.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_bneck.alloc((size_t)Ft));
+  PHS_CUDA(sim->d_coll_t.alloc((size_t)sim->total_colls));
+  PHS_CUDA(sim->d_res.alloc((size_t)U));
+  PHS_CUDA(sim->d_ticket.alloc(1));
+  if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)log_cursor));
+  if (sim->hist_cap > 0) {
+    PHS_CUDA(sim->d_hist.alloc((size_t)sim->hist_cap));
+    PHS_CUDA(sim->d_hist_n.alloc(1));
+  }
+  sim->h_res.assign(U, InstResult{});
+
+  // ---- a9: batch scheduler, static part.  A unit whose state fits the shared memory of one SM goes to the CTA
+  // path (one launch configuration, sized for the largest such unit, with as many CTAs resident per SM as fit);
+  // the others go to the cluster path.  Units that overflow their slots at run time move to the cluster path.
+  const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin;
+  const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
+  const bool log = sim->want_log;
+  sim->order.clear();
+  sim->cluster_list.clear();
+  sim->cta = CtaLaunch{};
+  auto need_of = [&](const phs_sim::Unit &u) {
+    return (int)std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(u.n_flows, 1), std::max<int64_t>(u.bound, 32)), 1 << 16);
+  };
+  std::vector<int32_t> cand;
+  for (int u = 0; u < U; ++u) {
+    const phs_sim::Unit &un = sim->units[u];
+    if (un.n_flows == 0) continue;  // nothing to simulate; its result block stays zero (status OK)
+    if (sim->policy_path == 2 || un.n_links >= 65535 ||
+        cta_smem_bytes(un.n_links, (need_of(un) + 31) / 32 * 32, 0, log) > smem_max)
+      sim->cluster_list.push_back(u);
+    else
+      cand.push_back(u);
+  }
+  while (!cand.empty()) {
+    int Lm = 1, need = 32;
+    int64_t maxF = 1;
+    for (int u : cand) {
+      Lm = std::max(Lm, sim->units[u].n_links);
+      need = std::max(need, need_of(sim->units[u]));
+      maxF = std::max<int64_t>(maxF, sim->units[u].n_flows);
+    }
+    // about one slot per thread: measured on B200, 128 threads for cfg3-sized units, 256 for cfg1-sized ones
+    const int threads = (need <= 128 && Lm <= 320) ? 128 : 256;
+    const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
+    // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
+    // predecessor counters on chip; returns 0 if not even one fits
+    auto fit = [&](bool pcs, int *slots_out) {
+      const int pcf = pcs ? (int)maxF : 0;
+      for (int w = want; w >= 1; --w) {
+        const size_t budget = std::min(smem_max, per_sm / w - 1024);
+        if (cta_smem_bytes(Lm, 32, pcf, log) > budget) continue;
+        int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
+        if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
+        hi = (hi + 31) / 32 * 32;
+        while (lo < hi) {  // largest multiple of 32 that fits the budget
+          const int mid = ((lo + hi + 32) / 64) * 32;
+          if (cta_smem_bytes(Lm, mid, pcf, log) <= budget)
+            lo = mid;
+          else
+            hi = mid - 32;
+        }
+        if (lo >= need || (w == 1 && sim->policy_path == 1) || sim->policy_slots > 0) {
+          if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
+          *slots_out = lo;
+          return w;
+        }
+      }
+      return 0;
+    };
+    int slots_p = 0, slots_n = 0;
+    const int w_p = pc8_ok ? fit(true, &slots_p) : 0, w_n = fit(false, &slots_n);
+    if (w_p == 0 && w_n == 0) {
+      // the largest links x slots combination does not fit one SM: the unit with the most flows goes to a cluster
+      auto big = std::max_element(cand.begin(), cand.end(), [&](int a, int b) {
+        return sim->units[a].n_flows < sim->units[b].n_flows;
+      });
+      sim->cluster_list.push_back(*big);
+      cand.erase(big);
+      continue;
+    }
+    // counters on chip save an L2 round trip per release: worth one resident CTA less
+    const bool pcs = w_p > 0 && slots_p >= std::min(need, slots_n) && w_p >= w_n - 1;
+    sim->cta.threads = threads;
+    sim->cta.slots = pcs ? slots_p : slots_n;
+    sim->cta.pc_flows = pcs ? (int)maxF : 0;
+    sim->cta.smem = cta_smem_bytes(Lm, sim->cta.slots, sim->cta.pc_flows, log);
+    sim->cta.log = log;
+    sim->cta.n_links = Lm;
+    sim->order = cand;
+    std::stable_sort(sim->order.begin(), sim->order.end(),
+                     [&](int a, int b) { return sim->units[a].n_flows > sim->units[b].n_flows; });
+    const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta.smem + 1024)), 2048 / threads));
+    sim->cta.grid = std::min((int)cand.size(), per * sim->sm_count);
+    PHS_CUDA(sim->d_order.upload(sim->order, st));
+    break;
+  }
+  std::sort(sim->cluster_list.begin(), sim->cluster_list.end());
+  PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
+  sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
+                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size() + linkid.size() +
+                              fmap.size() + init_f.size()) * 4 + init_t.size() * 8 + (pc8_ok ? pc8.size() : 0) +
+                             (capq.size() + coll_first.size()) * 8);
+  PHS_CUDA(cudaEventCreate(&sim->ev0));
+  PHS_CUDA(cudaEventCreate(&sim->ev1));
+  sim->finalized = true;
+  return PHS_OK;
+}
+
+// ================================================================================================ run
+namespace {
+
+DevTables tables_of(phs_sim *sim, int n_links) {
+  DevTables t;
+  t.inst = sim->d_desc.p;
+  t.rec = sim->d_rec.p;
+  t.succ = sim->d_succ.p;
+  t.pred_cnt0 = sim->d_pc0.p;
+  t.pred_cnt0_u8 = sim->d_pc8.p;
+  t.fmap = sim->d_fmap.p;
+  t.init_t = sim->d_init_t.p;
+  t.init_f = sim->d_init_f.p;
+  t.capq = sim->d_capq.p;
+  t.lcomp = sim->d_lcomp.p;
+  t.linkid = sim->d_linkid.p;
+  t.pred_cnt = sim->d_pred_cnt.p;
+  t.t_done = sim->d_tdone.p;
+  t.bneck = sim->d_bneck.p;
+  t.res = sim->d_res.p;
+  t.log = sim->want_log ? sim->d_log.p : nullptr;
+  t.hist = sim->hist_cap > 0 ? sim->d_hist.p : nullptr;
+  t.hist_n = sim->d_hist_n.p;
+  t.hist_cap = sim->hist_cap;
+  t.n_links = n_links;
+  return t;
+}
+
+// Cluster path (a9): every instance in `list` is simulated by one thread-block cluster with all dynamic state in
+// the shared memory of its CTAs; clusters pull instances from the list until it is empty.  `slot_scale` scales the
+// guess of how many flows are PENDING or ACTIVE at once (doubled after an overflow).
+phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, cudaStream_t st) {
+  if (list.empty()) return PHS_OK;
+  int L = 1;  // the shared-memory layout is sized for the unit with the most links
+  for (int u : list) L = std::max(L, sim->units[u].n_links);
+  if (L >= 65535) return fail(PHS_ERANGE, "cluster path: units with 65535 or more links are not supported");
+  // slots needed per instance: every flow without predecessors is PENDING from t = 0; later, a ring collective
+  // has at most one step in flight per rank plus the successors waiting out their latency, while an all-to-all
+  // or a raw flow set can be in flight as a whole.  Start from a quarter of that bound; overflow doubles it.
+  int64_t target = 64;
+  for (int u : list) {
+    const phs_sim::Unit &un = sim->units[u];
+    const int64_t ring = un.bound - un.bound_whole;  // rarely all in flight at once: start from a quarter
+    target = std::max(target, un.bound_whole + std::min(ring, ring * slot_scale / 4));
+    if (slot_scale > 4) target = std::max(target, std::min<int64_t>(un.n_flows, un.bound * slot_scale / 4));
+  }
+  const size_t smem_max = sim->smem_optin - 4096;  // minus the kernel's static shared memory
+  const bool log = sim->want_log;
+  int cs = 0, max_clusters = 0;
+  int64_t Sc = 0;
+  bool agg = false, cold = false, repl = false;
+  // replicated link shares pay when many flows share a link (every flow reads its links' shares every round)
+  const bool want_repl = target >= 8 * (int64_t)L;
+  for (int c = 1; c <= 16 && !cs; c *= 2) {
+    if ((int64_t)c * kClusterThreads * 4 < target && c < 16) continue;  // at most ~4 slots per thread
+    const int64_t sc = std::min<int64_t>(65535, (target + c - 1) / c + 16);
+    const bool opts[4][2] = {{true, true}, {false, true}, {true, false}, {false, false}};  // {agg, cold in smem}
+    for (int k = 0; k < 8 && !cs; ++k) {
+      const bool o_agg = opts[k & 3][0], o_cold = opts[k & 3][1], o_repl = k < 4;
+      if (o_repl && !want_repl) continue;
+      if (c < 16 && !o_cold) continue;  // spill cold fields to global only at the largest cluster size
+      const size_t smem = cluster_smem_bytes(L, c, sc, o_agg, o_cold, log, o_repl);
+      if (smem > smem_max) continue;
+      int n = 0;
+      PHS_CUDA(cluster_max_clusters(c, smem, &n));
+      if (n < 1) continue;
+      cs = c;
+      Sc = sc;
+      agg = o_agg;
+      cold = o_cold;
+      repl = o_repl;
+      max_clusters = n;
+    }
+  }
+  if (!cs)
+    return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the shared memory of a cluster");
+  const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
+  const size_t region = cold ? 0 : cluster_region_bytes(Sc, cs);
+  if (region * n_clusters > sim->g_scratch.n) PHS_CUDA(sim->g_scratch.alloc(region * n_clusters));
+  if (!sim->d_cticket.p) PHS_CUDA(sim->d_cticket.alloc(1));
+  sim->scratch_Sc = Sc;
+  sim->scratch_cs = cs;
+  sim->clusters_resident = max_clusters;
+  std::vector<int32_t> sorted(list);
+  std::stable_sort(sorted.begin(), sorted.end(),
+                   [&](int a, int b) { return sim->units[a].n_flows > sim->units[b].n_flows; });
+  PHS_CUDA(sim->d_clist.upload(sorted, st));
+  PHS_CUDA(cudaMemsetAsync(sim->d_cticket.p, 0, sizeof(int), st));
+  ClusterScratch sc;
+  sc.base = sim->g_scratch.p;
+  sc.region_bytes = region;
+  sc.Sc = Sc;
+  sc.aggregate = agg ? 1 : 0;
+  sc.cold_smem = cold ? 1 : 0;
+  sc.replicate = repl ? 1 : 0;
+  PHS_CUDA(launch_cluster_path(tables_of(sim, L), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
+                               n_clusters, log, st));
+  PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy
+  return PHS_OK;
+}
+
+}  // namespace
+
+extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (!sim->finalized) {
+    phs_status fs = phs_finalize(sim, cuda_stream);
+    if (fs != PHS_OK) return fs;
+  }
+  sim->last_stream = st;
+  const int U = (int)sim->units.size();
+  DevTables t = tables_of(sim, sim->cta.n_links);
+  sim->n_launches = 0;
+  PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
+  if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
+  PHS_CUDA(cudaEventRecord(sim->ev0, st));
+  if (!sim->order.empty()) {
+    sim->n_launches++;
+    PHS_CUDA(cudaMemsetAsync(sim->d_ticket.p, 0, sizeof(int), st));
+    PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta, st));
+  }
+  PHS_CUDA(cudaEventRecord(sim->ev1, st));
+  PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
+  PHS_CUDA(cudaStreamSynchronize(st));
+  PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
+  // instances that ran out of shared-memory slots on the CTA path move to the cluster path (also for later runs)
+  std::vector<int32_t> redo;
+  for (int u : sim->order)
+    if (sim->h_res[u].status == kOverflow) redo.push_back(u);
+  if (!redo.empty()) {
+    for (int inst : redo) {
+      sim->cluster_list.push_back(inst);
+      sim->order.erase(std::find(sim->order.begin(), sim->order.end(), inst));
+    }
+    if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
+    sim->cta.grid = std::min<int>(sim->cta.grid, std::max<int>(1, (int)sim->order.size()));
+    PHS_CUDA(cudaStreamSynchronize(st));
+  }
+  // cluster path; an instance that overflows a CTA's slot partition is re-run with larger partitions
+  std::vector<int32_t> todo(sim->cluster_list);
+  for (int64_t scale = sim->cluster_scale; !todo.empty(); scale *= 2) {
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
+    phs_status gs = run_cluster_path(sim, todo, scale, st);
+    if (gs != PHS_OK) return gs;
+    sim->n_launches++;
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    float extra = 0.f;
+    PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
+    sim->main_kernel_ms += extra;
+    std::vector<int32_t> again;
+    for (int i : todo)
+      if (sim->h_res[i].status == kOverflow) again.push_back(i);
+    if (!again.empty()) {
+      if (scale > 64) return fail(PHS_ERANGE, "cluster path: flow slots overflow even at full size");
+      sim->cluster_scale = scale * 2;  // remember for later runs
+    }
+    todo.swap(again);
+  }
+  if (sim->total_colls > 0) sim->n_launches++;
+  PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
+                                   sim->d_coll_t.p, st));
+  if (sim->hist_cap > 0) {  // throughput history: fetch, order by (flow, event); a re-run unit repeats its records
+    unsigned long long n = 0;
+    PHS_CUDA(cudaMemcpyAsync(&n, sim->d_hist_n.p, sizeof(n), cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    if (n > (unsigned long long)sim->hist_cap)
+      return fail(PHS_ERANGE, "throughput history needs " + std::to_string(n) + " records, max_records is " +
+                                  std::to_string(sim->hist_cap));
+    sim->h_hist.resize((size_t)n);
+    if (n) PHS_CUDA(cudaMemcpyAsync(sim->h_hist.data(), sim->d_hist.p, sizeof(HistRec) * n, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    std::sort(sim->h_hist.begin(), sim->h_hist.end(), [](const HistRec &a, const HistRec &b) {
+      return a.flow != b.flow ? a.flow < b.flow : a.ev < b.ev;
+    });
+    sim->h_hist.erase(std::unique(sim->h_hist.begin(), sim->h_hist.end(),
+                                  [](const HistRec &a, const HistRec &b) { return a.flow == b.flow && a.ev == b.ev; }),
+                      sim->h_hist.end());
+  }
+  sim->ran = true;
+  for (int u = 0; u < U; ++u) {
+    const int i = sim->units[u].inst;
+    if (sim->h_res[u].status == PHS_ECYCLE)
+      return fail(PHS_ECYCLE, "instance " + std::to_string(i) + ": flows left waiting on dependencies that never complete");
+    if (sim->h_res[u].status != PHS_OK)
+      return fail(PHS_ECUDA, "instance " + std::to_string(i) + ": unexpected kernel status " +
+                                 std::to_string(sim->h_res[u].status));
+  }
+  return PHS_OK;
+}
+

@@ -1,0 +1,129 @@
+// phs_sim.h -- the handle behind the C-ABI (struct phs_sim) and the small host helpers shared by phs_api.cu
+// (submission calls, result getters) and phs_schedule.cu (table construction, batch scheduler, phs_run).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <atomic>
+#include <memory>
+#include <string>
+#include <thread>
+#include <vector>
+
+#include "phs_device.h"
+
+// records the thread-local error message (phs_last_error) and returns `code`
+phs_status phs_fail(phs_status code, const std::string &msg);
+
+#define PHS_CUDA(call)                                                                                       \
+  do {                                                                                                       \
+    cudaError_t e_ = (call);                                                                                 \
+    if (e_ != cudaSuccess) return phs_fail(PHS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+namespace phs {
+
+// fn(i) for every i in [0, n) on up to `max_threads` (<= 16) host threads; the iterations must be independent
+template <typename F>
+void parallel_for(int n, F fn, int max_threads = 16) {
+  const int nt = std::min(std::min(n, max_threads), (int)std::min(16u, std::max(1u, std::thread::hardware_concurrency())));
+  if (nt <= 1) {
+    for (int i = 0; i < n; ++i) fn(i);
+    return;
+  }
+  std::atomic<int> next{0};
+  std::vector<std::thread> pool;
+  for (int t = 0; t < nt; ++t)
+    pool.emplace_back([&] {
+      for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+    });
+  for (std::thread &th : pool) th.join();
+}
+
+template <typename T>
+struct DevBuf {
+  T *p = nullptr;
+  size_t n = 0;
+  ~DevBuf() { release(); }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    n = 0;
+  }
+  cudaError_t alloc(size_t count) {
+    release();
+    n = count;
+    return cudaMalloc((void **)&p, std::max<size_t>(count, 1) * sizeof(T));
+  }
+  cudaError_t upload(const std::vector<T> &h, cudaStream_t st) {
+    cudaError_t e = alloc(h.size());
+    if (e != cudaSuccess || h.empty()) return e;
+    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+  }
+};
+
+}  // namespace phs
+
+struct phs_sim {
+  phs_topology_desc desc;
+  uint64_t seed;
+  int32_t batch;
+  std::unique_ptr<phs::Fabric> fab;
+  std::vector<phs::Instance> inst;
+  bool want_log = false, finalized = false, ran = false;
+  int32_t policy_path = 0, policy_slots = 0;
+
+  // ---- host mirrors built by finalize
+  std::vector<int64_t> flow_base;  // [B+1]
+  std::vector<int64_t> coll_base;  // [B+1]
+  struct Unit {  // what one CTA / cluster simulates (see phs::InstDesc)
+    int32_t inst, n_flows, n_links;
+    int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (see phs_finalize)
+    int64_t bound_whole;  // the part of `bound` from raw flows and all-to-alls (may be in flight all at once)
+  };
+  std::vector<Unit> units;
+  std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
+  bool decompose = true;
+  std::vector<phs::InstDesc> h_desc;  // per unit
+  std::vector<phs::InstResult> h_res; // per unit
+  std::vector<int32_t> order;  // CTA-path instances, largest first
+  std::vector<int32_t> cluster_list;  // instances that go (or fell back) to the cluster path
+  int64_t total_flows = 0, total_colls = 0;
+
+  // ---- device tables
+  phs::DevBuf<phs::InstDesc> d_desc;
+  phs::DevBuf<phs::FlowRec> d_rec;
+  phs::DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
+  phs::DevBuf<uint32_t> d_fmap;
+  // throughput history (optional)
+  int64_t hist_cap = 0;
+  phs::DevBuf<phs::HistRec> d_hist;
+  phs::DevBuf<unsigned long long> d_hist_n;
+  std::vector<phs::HistRec> h_hist;  // records of the last run, sorted by (flow, event), duplicates of re-runs removed
+  phs::DevBuf<int32_t> d_init_f;
+  phs::DevBuf<uint8_t> d_pc8;
+  phs::DevBuf<int64_t> d_capq, d_coll_first;
+  phs::DevBuf<double> d_tdone, d_coll_t, d_init_t;
+  phs::DevBuf<phs::InstResult> d_res;
+  phs::DevBuf<phs_event> d_log;
+  phs::DevBuf<int> d_ticket;
+  // cluster-path scratch: one region per concurrently running cluster
+  phs::DevBuf<uint8_t> g_scratch;
+  phs::DevBuf<int32_t> d_clist, d_lcomp;
+  phs::DevBuf<int> d_cticket;
+  int64_t scratch_Sc = 0, cluster_scale = 1;
+  int scratch_regions = 0, scratch_cs = 0, clusters_resident = 0;
+
+  // launch configuration of the CTA path
+  phs::CtaLaunch cta{};
+  int sm_count = 0;
+  size_t smem_optin = 0;
+  cudaStream_t last_stream = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  int64_t n_launches = 0, h2d_bytes = 0;
+  float main_kernel_ms = 0.f;
+  ~phs_sim() {
+    if (ev0) cudaEventDestroy(ev0);
+    if (ev1) cudaEventDestroy(ev1);
+  }
+};
