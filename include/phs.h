@@ -121,9 +121,10 @@ phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_
 phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);
 
 /* Batch-scheduler policy; must precede phs_finalize.  path: 0 = automatic (one CTA per
- * instance with shared-memory state when it fits, else one thread-block cluster per instance with state in L2),
- * 1 = CTA path, 2 = cluster path for every instance.  cta_slots > 0 caps the CTA path's shared-memory slot count
- * (active flows / pending flows per instance); an instance that exceeds it is re-run on the cluster path. */
+ * simulation unit with all state in its shared memory when it fits, else one thread-block cluster per unit with the
+ * state spread over the shared memory of its CTAs), 1 = CTA path, 2 = cluster path for every unit.  cta_slots > 0
+ * caps the CTA path's shared-memory slot count (flows PENDING or ACTIVE at once per unit); a unit that exceeds it
+ * is re-run on the cluster path. */
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
 
 /* Decomposition (default on).  An instance whose flows fall into groups that share no link and no dependency is

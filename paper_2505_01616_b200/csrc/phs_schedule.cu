@@ -14,9 +14,11 @@ using namespace phs;
 #define fail phs_fail
 
 // ================================================================================================ finalize
-// Builds the device-resident tables.  HBM layout: one 32-byte FlowRec per flow (+1
-// sentinel per instance), flow->link CSR values, successor CSR values (transpose of the dependency lists),
-// per-instance capacity rows in rate quanta, and the dynamic per-flow arrays (pred_cnt, t_done, bneck).
+// Splits the instances into simulation units and builds the device-resident tables.  HBM layout (DESIGN.md "Data
+// layout"): one 64-byte FlowRec per flow (path, successors and component inline, unit-local ids), successor lists
+// longer than two, predecessor counts (plain and 4-bit packed), the local-flow -> output-position map, per unit
+// the capacity row in rate quanta, the link components and the link ids of the topology, the sorted list of
+// initial activations, and the dynamic per-flow arrays (pred_cnt, t_done, bneck).
 extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return PHS_OK;
