@@ -153,6 +153,12 @@ phs_status phs_finalize(phs_sim *sim, void *cuda_stream);
 /* Runs every instance to completion on the GPU (all steps of the hot path in CUDA kernels) and waits for the
  * result status.  May be called repeatedly; each call restarts from t = 0. */
 phs_status phs_run(phs_sim *sim, void *cuda_stream);
+/* PAPER.md L167 "advancing the simulation ... up to a specified time": like phs_run, but stops before the first
+ * event later than t_stop_s.  Flows that complete later report completion time NaN and bottleneck -1, a collective
+ * with such flows reports NaN; event log and throughput history hold what happened up to t_stop_s.  Every call
+ * simulates from t = 0 (there is no resume yet: a later call with a larger time repeats the earlier part and, the
+ * simulation being deterministic, reproduces it). */
+phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
 
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out);
 phs_status phs_total_flows(const phs_sim *sim, int64_t *out);

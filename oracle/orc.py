@@ -138,8 +138,12 @@ class Sim:
                                  _p(dep_ids, C.c_int64), _p(conn_id, C.c_int32), C.byref(first)), "orc_add_flows")
         return first.value
 
-    def run(self, mode=MODE_NAIVE, trace=False):
-        _chk(lib().orc_run(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0)), "orc_run")
+    def run(self, mode=MODE_NAIVE, trace=False, until=None):
+        if until is None:
+            _chk(lib().orc_run(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0)), "orc_run")
+        else:
+            _chk(lib().orc_run_until(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0), C.c_double(until)),
+                 "orc_run_until")
 
     @property
     def num_flows(self):

@@ -565,7 +565,12 @@ int32_t orc_maxmin(int32_t n_links, const double *cap, int32_t n_flows, const in
 }
 
 /* ------------------------------------------------------------------ S4: flow states & event loop */
-int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
+int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) { return orc_run_until(s, mode, trace, INFINITY); }
+
+/* "advancing the simulation ... up to a specified time": the event loop stops before the first
+ * event later than t_stop.  Flows that have not completed by then keep t_done = NaN and bneck = -1; the event
+ * log and the throughput history hold what happened up to t_stop. */
+int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
   if (!s || (mode != ORC_MODE_NAIVE && mode != ORC_MODE_FAST)) return ORC_EINVAL;
   if (s->ran) return ORC_ESTATE;
   int64_t F = s->F;
@@ -610,7 +615,7 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
       for (int64_t e = s->pred_off[f]; e < s->pred_off[f + 1]; e++) succ[cur[s->pred[e]]++] = (int32_t)f;
     free(cur);
   }
-  int32_t nA = 0, nP = 0;
+  int32_t nA = 0, nP = 0, stopped = 0;
   int64_t n_done = 0;
   double now = 0.0;
   for (int64_t f = 0; f < F; f++) {
@@ -682,6 +687,7 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
     }
     for (int32_t i = 0; i < nP; i++)
       if (t_act[pend[i]] < t_next) t_next = t_act[pend[i]];
+    if (t_next > t_stop) { stopped = 1; break; } /* the next event lies beyond the requested time */
     /* 4. advance: flows whose completion time is bit-equal to t_next complete; nobody else changes */
     int32_t nC = 0, na2 = 0;
     for (int32_t i = 0; i < nA; i++) {
@@ -731,7 +737,10 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) {
     orc_event *e = &s->ev[s->n_ev++];
     e->t = t_next; e->n_completed = nC; e->n_activated = n_activated; e->n_rounds = R; e->first_bneck = fb;
   }
-  if (n_done < F) rc = ORC_ECYCLE; /* WAITING flows left with nothing active or pending */
+  if (stopped) { /* unfinished flows report no bottleneck */
+    for (int64_t f = 0; f < F; f++)
+      if (state[f] != DONE) s->bneck[f] = -1;
+  } else if (n_done < F) rc = ORC_ECYCLE; /* WAITING flows left with nothing active or pending */
   s->ran = 1;
 out:
   free(capq); free(succ_off); free(succ); free(pred_cnt); free(state); free(t_act); free(rem); free(tc); free(rq); free(rq_cur); free(t_last);
@@ -760,9 +769,12 @@ int32_t orc_get_collective_times(const orc_sim *s, double *out, int32_t n) {
   if (!s->t_done) return ORC_ESTATE;
   for (int32_t c = 0; c < n; c++) { /* O5: max t_done over the collective's flows */
     double m = -INFINITY;
-    for (int32_t f = s->coll[c].first_flow; f < s->coll[c].first_flow + s->coll[c].n_flows; f++)
+    int open_flows = 0; /* after orc_run_until: a collective with unfinished flows has no finish time yet */
+    for (int32_t f = s->coll[c].first_flow; f < s->coll[c].first_flow + s->coll[c].n_flows; f++) {
+      if (s->t_done[f] != s->t_done[f]) open_flows = 1;
       if (s->t_done[f] > m) m = s->t_done[f];
-    out[c] = m;
+    }
+    out[c] = open_flows ? NAN : m;
   }
   return ORC_OK;
 }

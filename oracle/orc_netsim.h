@@ -78,6 +78,9 @@ int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *
                       const int32_t *conn_id, int64_t *out_first_flow_id);
 /* trace != 0 additionally records, for every loop iteration, the active flows and their rates */
 int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace);
+/* same, but stops before the first event later than t_stop ("advancing the simulation ... up to a
+ * specified time"); unfinished flows keep t_done = NaN and bneck = -1 */
+int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop);
 int32_t orc_num_flows(const orc_sim *s, int64_t *out);
 int32_t orc_get_completion_times(const orc_sim *s, double *out, int64_t n);
 int32_t orc_get_bottlenecks(const orc_sim *s, int32_t *out, int64_t n);

@@ -40,7 +40,7 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
 SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
-           "phs_set_decomposition", "phs_finalize", "phs_run", "phs_num_flows", "phs_total_flows",
+           "phs_set_decomposition", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
            "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
@@ -185,6 +185,10 @@ def phs_set_decomposition(h, enable=True):
 
 def phs_finalize(h, stream=None):
     _chk(lib().phs_finalize(h, C.c_void_p(stream or 0)), "phs_finalize")
+
+
+def phs_run_until(h, t_stop_s, stream=None):
+    _chk(lib().phs_run_until(h, C.c_double(t_stop_s), C.c_void_p(stream or 0)), "phs_run_until")
 
 
 def phs_run(h, stream=None):
@@ -374,8 +378,11 @@ class Sim:
     def finalize(self, stream=None):
         phs_finalize(self.h, stream)
 
-    def run(self, stream=None):
-        phs_run(self.h, stream)
+    def run(self, stream=None, until=None):
+        if until is None:
+            phs_run(self.h, stream)
+        else:
+            phs_run_until(self.h, until, stream)
 
     def num_flows(self, i):
         return phs_num_flows(self.h, i)

@@ -750,6 +750,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       }
       sum_active += nA;
       sum_rounds += rounds;
+      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
+        status = kPaused;
+        break;
+      }
     }
 #ifdef PHS_PHASE_CLOCKS
     if (tid == 0 && (crank == 0 || crank == CS - 1))

@@ -35,6 +35,7 @@ struct DevTables {
   HistRec *hist;             // throughput history records, or nullptr
   unsigned long long *hist_n;  // records produced (may exceed hist_cap: the excess is dropped and reported)
   long long hist_cap;
+  double t_stop;             // phs_run_until: stop before the first event later than this (+inf: run to the end)
   int32_t n_links;           // largest n_links among the units of this launch (sizes the shared-memory layout)
 };
 

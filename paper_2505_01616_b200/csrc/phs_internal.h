@@ -62,6 +62,7 @@ struct InstResult {
   int32_t pad_;
 };
 constexpr int32_t kOverflow = 1;  // internal: the CTA path ran out of shared-memory slots
+constexpr int32_t kPaused = 2;    // internal: stopped before the first event later than the requested time
 
 // ---- host-side instance tables (built by phs_build.cpp) ----
 struct Collective {

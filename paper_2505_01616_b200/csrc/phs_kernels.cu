@@ -629,6 +629,10 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       sum_active += nA;
       sum_rounds += rounds;
       PHS_TICK(6)
+      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
+        status = kPaused;
+        break;
+      }
     }
 #ifdef PHS_PHASE_CLOCKS
     if ((tid == 0 || tid == NT - 1) && F > 3000 && inst < 40)
@@ -701,10 +705,15 @@ __global__ void phs_collective_times_kernel(const double *__restrict__ t_done, c
   const double *p = t_done + first[c];
   const int n = nflows[c];
   double m = 0.0;
-  for (int i = lane; i < n; i += 32) m = fmax(m, p[i]);
+  bool open_flows = false;  // after phs_run_until: a collective with unfinished flows (NaN) has no finish time yet
+  for (int i = lane; i < n; i += 32) {
+    open_flows |= p[i] != p[i];
+    m = fmax(m, p[i]);
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-  if (lane == 0) out[c] = m;
+  open_flows = __any_sync(0xffffffffu, open_flows);
+  if (lane == 0) out[c] = open_flows ? __longlong_as_double(0x7ff8000000000000LL) : m;
 }
 
 cudaError_t launch_collective_times(const double *t_done, const int64_t *coll_first, const int32_t *coll_nflows,

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <limits>
 #include <numeric>
 
 #include "phs_sim.h"
@@ -473,6 +474,7 @@ DevTables tables_of(phs_sim *sim, int n_links) {
   t.hist = sim->hist_cap > 0 ? sim->d_hist.p : nullptr;
   t.hist_n = sim->d_hist_n.p;
   t.hist_cap = sim->hist_cap;
+  t.t_stop = sim->t_stop;
   t.n_links = n_links;
   return t;
 }
@@ -553,7 +555,13 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
 }  // namespace
 
 extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
+  return phs_run_until(sim, std::numeric_limits<double>::infinity(), cuda_stream);
+}
+
+extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream) {
   if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (!(t_stop_s >= 0.0)) return fail(PHS_EINVAL, "t_stop_s must be >= 0");
+  sim->t_stop = t_stop_s;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (!sim->finalized) {
     phs_status fs = phs_finalize(sim, cuda_stream);
@@ -565,6 +573,10 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   sim->n_launches = 0;
   PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
   if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
+  if (std::isfinite(sim->t_stop) && sim->total_flows > 0) {  // flows that do not finish by t_stop: NaN / -1
+    PHS_CUDA(cudaMemsetAsync(sim->d_tdone.p, 0xff, sizeof(double) * (size_t)sim->total_flows, st));
+    PHS_CUDA(cudaMemsetAsync(sim->d_bneck.p, 0xff, sizeof(int32_t) * (size_t)sim->total_flows, st));
+  }
   PHS_CUDA(cudaEventRecord(sim->ev0, st));
   if (!sim->order.empty()) {
     sim->n_launches++;
@@ -635,7 +647,7 @@ extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
     const int i = sim->units[u].inst;
     if (sim->h_res[u].status == PHS_ECYCLE)
       return fail(PHS_ECYCLE, "instance " + std::to_string(i) + ": flows left waiting on dependencies that never complete");
-    if (sim->h_res[u].status != PHS_OK)
+    if (sim->h_res[u].status != PHS_OK && sim->h_res[u].status != kPaused)
       return fail(PHS_ECUDA, "instance " + std::to_string(i) + ": unexpected kernel status " +
                                  std::to_string(sim->h_res[u].status));
   }

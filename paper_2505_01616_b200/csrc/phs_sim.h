@@ -84,6 +84,7 @@ struct phs_sim {
   std::vector<Unit> units;
   std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
   bool decompose = true;
+  double t_stop = 0.0;  // stop time of the current / last run (phs_run_until), +inf for phs_run
   std::vector<phs::InstDesc> h_desc;  // per unit
   std::vector<phs::InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first

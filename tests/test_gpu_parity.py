@@ -11,7 +11,7 @@ import pytest
 from oracle import orc
 from paper_2505_01616_b200 import binding as B
 from paper_2505_01616_b200 import workloads as W
-from util import completion_order, oracle_run
+from util import completion_order, oracle_build, oracle_run
 
 pytestmark = pytest.mark.gpu
 
@@ -281,3 +281,34 @@ def test_throughput_history_equals_the_oracle(path):
         small.run()
     assert e.value.code == B.PHS_ERANGE and "needs" in str(e.value)
     small.close()
+
+
+@pytest.mark.parametrize("path", [CTA, CLUSTER])
+def test_run_until_stops_where_the_oracle_stops(path):
+    """PAPER.md L167 "advancing the simulation ... up to a specified time": completion times, bottlenecks, collective
+    times (NaN / -1 for what has not finished), event log and throughput history up to t_stop, bit-equal to the oracle
+    stopped at the same time."""
+    w = W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
+    full = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST).completion_times() for i in range(w.batch)]
+    t_end = max(t.max() for t in full)
+    for frac in (0.0, 0.31, 0.77, 2.0):
+        t_stop = frac * t_end
+        for log, decompose in ((True, False), (False, True)):
+            sim = B.Sim.from_workload(w, path=path, event_log=log, decompose=decompose, history=1 << 20)
+            sim.run(until=t_stop)
+            for i in range(w.batch):
+                inst = w.instances[i]
+                o = oracle_build(w.desc, inst)
+                o.run(mode=orc.MODE_FAST, until=t_stop)
+                t, to = sim.completion_times(i), o.completion_times()
+                assert np.array_equal(t, to, equal_nan=True)
+                assert np.isnan(to).any() == (frac < 1.0) and (frac == 0.0 or not np.isnan(to).all())
+                assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+                assert np.array_equal(sim.collective_times(i), o.collective_times(), equal_nan=True)
+                fl, th, rh = o.history()
+                off, tg, rg = sim.history(i)
+                assert np.array_equal(np.diff(off), np.bincount(fl, minlength=o.num_flows))
+                assert np.array_equal(tg, th) and np.array_equal(rg, rh)
+                if log:
+                    assert np.array_equal(sim.event_log(i), o.event_log())
+            sim.close()

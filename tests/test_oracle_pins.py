@@ -524,6 +524,31 @@ def test_p9_history_partitions_every_flow_into_constant_rate_intervals():
         assert np.array_equal(rates[keep], r[fl == f]) and np.array_equal(times[keep], t[fl == f])
 
 
+def test_p9_run_until_is_a_prefix_of_the_full_run():
+    """PAPER.md L167 "advancing the simulation ... up to a specified time": stopping at T changes nothing before T.
+    Flows done by T have the times of the full run, the others are NaN / -1, and event log and throughput history
+    are the full run's records with time <= T."""
+    from util import oracle_build
+    w = W.cfg1(batch=1, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
+    full = oracle_run(w.desc, w.instances[0])
+    t_full, ev_full = full.completion_times(), full.event_log()
+    ff, tf, rf = full.history()
+    for T in (0.0, 0.25 * t_full.max(), 0.6 * t_full.max(), t_full.max(), 2 * t_full.max()):
+        o = oracle_build(w.desc, w.instances[0])
+        o.run(until=T)
+        t = o.completion_times()
+        done = t_full <= T
+        assert np.array_equal(t[done], t_full[done]) and np.isnan(t[~done]).all()
+        assert np.array_equal(o.bottlenecks()[done], full.bottlenecks()[done]) and np.all(o.bottlenecks()[~done] == -1)
+        ev = o.event_log()
+        assert np.array_equal(ev, ev_full[ev_full["t"] <= T])
+        fo, to, ro = o.history()
+        keep = tf <= T
+        assert np.array_equal(fo, ff[keep]) and np.array_equal(to, tf[keep]) and np.array_equal(ro, rf[keep])
+        ct, ct_full = o.collective_times(), full.collective_times()
+        assert np.array_equal(ct[ct_full <= T], ct_full[ct_full <= T]) and np.isnan(ct[ct_full > T]).all()
+
+
 def test_p9_single_spine_is_seed_independent():
     d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=1, uplinks_per_leaf_spine=1)
     ops = [W.Coll(W.ALLREDUCE_RING, np.arange(0, 16, 2, dtype=np.int32), 32 * MiB),
