@@ -85,6 +85,8 @@ typedef struct {
   int32_t max_slots;     /* largest number of state slots (PENDING + ACTIVE flows) one instance ever used */
   int32_t cluster_size;  /* CTAs per cluster of the cluster path in the last run (0: path not used)            */
   int32_t clusters_resident; /* clusters of that size the device keeps resident at once                        */
+  int32_t resumed_units; /* units the last phs_run_until continued from their parked state (0: started at t = 0) */
+  int32_t pad_;
   double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
                          /* the run's stream), excluding the result copies                                */
 } phs_counters;
@@ -155,9 +157,10 @@ phs_status phs_finalize(phs_sim *sim, void *cuda_stream);
 phs_status phs_run(phs_sim *sim, void *cuda_stream);
 /* PAPER.md L167 "advancing the simulation ... up to a specified time": like phs_run, but stops before the first
  * event later than t_stop_s.  Flows that complete later report completion time NaN and bottleneck -1, a collective
- * with such flows reports NaN; event log and throughput history hold what happened up to t_stop_s.  Every call
- * simulates from t = 0 (there is no resume yet: a later call with a larger time repeats the earlier part and, the
- * simulation being deterministic, reproduces it). */
+ * with such flows reports NaN; event log and throughput history hold what happened up to t_stop_s.  A later call
+ * with a larger time continues: units on the CTA path resume from their parked state, units on the cluster path
+ * (and everything, if the time goes backwards) start again from t = 0 -- the simulation is deterministic, so the
+ * results are the same either way. */
 phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
 
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out);

@@ -30,7 +30,8 @@ class Counters(C.Structure):
     _fields_ = [("n_events", C.c_int64), ("n_flow_events", C.c_int64), ("sum_active", C.c_int64),
                 ("sum_par_rounds", C.c_int64), ("n_kernel_launches", C.c_int64), ("h2d_bytes", C.c_int64),
                 ("max_active", C.c_int32), ("max_slots", C.c_int32), ("cluster_size", C.c_int32),
-                ("clusters_resident", C.c_int32), ("main_kernel_ms", C.c_double)]
+                ("clusters_resident", C.c_int32), ("resumed_units", C.c_int32), ("pad_", C.c_int32),
+                ("main_kernel_ms", C.c_double)]
 
 
 EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<i4"), ("n_rounds", "<i4"),

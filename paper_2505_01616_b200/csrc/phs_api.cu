@@ -366,6 +366,7 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   }
   c.cluster_size = sim->scratch_cs;
   c.clusters_resident = sim->clusters_resident;
+  c.resumed_units = sim->resumed_units;
   c.n_flow_events = 2 * sim->total_flows;
   c.n_kernel_launches = sim->n_launches;
   c.h2d_bytes = sim->h2d_bytes;

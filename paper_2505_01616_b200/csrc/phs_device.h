@@ -14,6 +14,12 @@ struct HistRec {     // one rate change of one flow (throughput history, PAPER.m
   uint32_t ev;       // index of the unit's event that changed it (orders changes at one and the same time)
 };
 
+struct ParkRegs {  // the loop-carried registers of a parked unit (CTA path)
+  double now, t_next;
+  long long sum_active, sum_rounds;
+  int32_t ev, solve, g, max_active, max_pending, first_bneck, valid, pad_;
+};
+
 struct DevTables {
   const InstDesc *inst;      // [U] simulation units
   const FlowRec *rec;        // [F_total] unit-local link / flow ids inside
@@ -36,6 +42,9 @@ struct DevTables {
   unsigned long long *hist_n;  // records produced (may exceed hist_cap: the excess is dropped and reported)
   long long hist_cap;
   double t_stop;             // phs_run_until: stop before the first event later than this (+inf: run to the end)
+  unsigned char *park;       // CTA path: per unit, ParkRegs + a copy of the CTA's dynamic shared memory, written
+  size_t park_stride;        //   when a unit stops at t_stop so that a later phs_run_until can resume it; or nullptr
+  int32_t resume;            // 1: units with a valid parked state continue from it instead of starting at t = 0
   int32_t n_links;           // largest n_links among the units of this launch (sizes the shared-memory layout)
 };
 

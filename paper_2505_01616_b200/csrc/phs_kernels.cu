@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
   __shared__ int sh_inst;
   CtaSmem S;
   const int L = T.n_links;
-  carve(&S, smem_raw, L, SC, pcf, LOG);
+  const size_t smem_used = carve(&S, smem_raw, L, SC, pcf, LOG);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = NT / 32;
 
@@ -172,7 +172,11 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
+    // phs_run_until: a unit that stopped at an earlier t_stop continues from its parked state
+    ParkRegs *park = T.park ? (ParkRegs *)(T.park + (size_t)inst * T.park_stride) : nullptr;
+    const bool resuming = T.resume && park && park->valid;
     // ---- init: nothing active, every slot free
+    if (!resuming)
     for (int l = tid; l < Li; l += NT) {
       S.l_cap[l] = capq[l];
       S.l_gid[l] = linkid[l];
@@ -183,12 +187,14 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       S.l_solve[l] = 0;
       if (LOG) S.l_won[l] = 0;
     }
+    if (!resuming) {
     for (int s = tid; s < SC; s += NT) {
       S.s_meta[s].x = -1;
       S.s_tc[s] = kInf;
     }
     if (tid < C_NCTL) S.ctl[tid] = 0;
-    if (PCS) {
+    }
+    if (PCS && !resuming) {
       const unsigned *src = (const unsigned *)(T.pred_cnt0_u8 + D.pc8_base);
       for (int w = tid; w < (F + 7) / 8; w += NT) S.pc8[w] = src[w];
     }
@@ -216,7 +222,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     };
 
     // S4: flows without predecessors become PENDING at t_act = start + Lat
-    {
+    if (!resuming) {
       const int32_t *__restrict__ pc0 = T.pred_cnt0 + D.flow_base;
       for (int f = tid; f < F; f += NT) {
         int pc;
@@ -248,6 +254,22 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     int max_active = 0, max_pending = 0;
     int status = PHS_OK;
     int first_bneck = -1;
+    if (resuming) {  // shared memory and the loop-carried registers as they were when the unit stopped
+      const uint4 *src = (const uint4 *)((const unsigned char *)park + sizeof(ParkRegs));
+      uint4 *dst = (uint4 *)smem_raw;
+      for (size_t i = tid; i < smem_used / 16; i += NT) dst[i] = src[i];
+      now = park->now;
+      t_next = park->t_next;
+      sum_active = park->sum_active;
+      sum_rounds = park->sum_rounds;
+      ev = park->ev;
+      solve = park->solve;
+      g = park->g;
+      max_active = park->max_active;
+      max_pending = park->max_pending;
+      first_bneck = park->first_bneck;
+      __syncthreads();
+    }
 #ifdef PHS_PHASE_CLOCKS
     long long pc_[8] = {0, 0, 0, 0, 0, 0, 0, 0}, pt_ = clock64();
 // BAR.SYNC does not block at issue: read a barrier-protected word before taking the clock
@@ -257,6 +279,10 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
 #endif
 
     for (;;) {
+      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
+        status = kPaused;
+        break;
+      }
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
       ++solve;
       const int hi0 = min(S.ctl[C_HI], SC);
@@ -629,9 +655,20 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       sum_active += nA;
       sum_rounds += rounds;
       PHS_TICK(6)
-      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
-        status = kPaused;
-        break;
+    }
+    if (park) {  // park the unit if it stopped at t_stop; a finished unit has nothing to resume
+      if (status == kPaused) {
+        __syncthreads();
+        uint4 *dst = (uint4 *)((unsigned char *)park + sizeof(ParkRegs));
+        const uint4 *src = (const uint4 *)smem_raw;
+        for (size_t i = tid; i < smem_used / 16; i += NT) dst[i] = src[i];
+      }
+      if (tid == 0) {
+        ParkRegs r;
+        r.now = now; r.t_next = t_next; r.sum_active = sum_active; r.sum_rounds = sum_rounds;
+        r.ev = ev; r.solve = solve; r.g = g; r.max_active = max_active; r.max_pending = max_pending;
+        r.first_bneck = first_bneck; r.valid = status == kPaused ? 1 : 0; r.pad_ = 0;
+        *park = r;
       }
     }
 #ifdef PHS_PHASE_CLOCKS

@@ -475,6 +475,9 @@ DevTables tables_of(phs_sim *sim, int n_links) {
   t.hist_n = sim->d_hist_n.p;
   t.hist_cap = sim->hist_cap;
   t.t_stop = sim->t_stop;
+  t.park = nullptr;  // set by phs_run_until for the CTA path
+  t.park_stride = 0;
+  t.resume = 0;
   t.n_links = n_links;
   return t;
 }
@@ -569,19 +572,46 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   }
   sim->last_stream = st;
   const int U = (int)sim->units.size();
+  const bool finite = std::isfinite(sim->t_stop);
+  // Resume: a run that stopped at an earlier time left the CTA-path units parked (shared memory + registers in
+  // global memory); a later stop time continues them from there.  Cluster-path units, and everything when the time
+  // goes backwards, start again from t = 0 -- the simulation is deterministic, so the results are the same.
+  const bool resume = sim->have_park && sim->ran && sim->t_stop >= sim->parked_until;
+  if (finite && !sim->order.empty() && sim->park_stride == 0) {
+    sim->park_stride = (sizeof(ParkRegs) + sim->cta.smem + 255) / 256 * 256;
+    PHS_CUDA(sim->d_park.alloc(sim->park_stride * (size_t)U));
+    PHS_CUDA(cudaMemsetAsync(sim->d_park.p, 0, sim->park_stride * (size_t)U, st));
+  }
   DevTables t = tables_of(sim, sim->cta.n_links);
+  t.park = (finite || resume) && sim->park_stride ? sim->d_park.p : nullptr;
+  t.park_stride = sim->park_stride;
+  t.resume = resume ? 1 : 0;
   sim->n_launches = 0;
-  PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
-  if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
-  if (std::isfinite(sim->t_stop) && sim->total_flows > 0) {  // flows that do not finish by t_stop: NaN / -1
-    PHS_CUDA(cudaMemsetAsync(sim->d_tdone.p, 0xff, sizeof(double) * (size_t)sim->total_flows, st));
-    PHS_CUDA(cudaMemsetAsync(sim->d_bneck.p, 0xff, sizeof(int32_t) * (size_t)sim->total_flows, st));
+  sim->resumed_units = 0;
+  std::vector<int32_t> cta_list(sim->order), cluster_todo(sim->cluster_list);
+  if (resume) {  // only what has not finished yet
+    auto paused = [&](int u) { return sim->h_res[u].status == kPaused; };
+    cta_list.erase(std::remove_if(cta_list.begin(), cta_list.end(), [&](int u) { return !paused(u); }), cta_list.end());
+    cluster_todo.erase(std::remove_if(cluster_todo.begin(), cluster_todo.end(), [&](int u) { return !paused(u); }),
+                       cluster_todo.end());
+    if (!cta_list.empty()) PHS_CUDA(sim->d_order2.upload(cta_list, st));
+    sim->resumed_units = (int)cta_list.size();
+  } else {
+    PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
+    if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
+    if (finite && sim->total_flows > 0) {  // flows that do not finish by t_stop: NaN / -1
+      PHS_CUDA(cudaMemsetAsync(sim->d_tdone.p, 0xff, sizeof(double) * (size_t)sim->total_flows, st));
+      PHS_CUDA(cudaMemsetAsync(sim->d_bneck.p, 0xff, sizeof(int32_t) * (size_t)sim->total_flows, st));
+    }
   }
   PHS_CUDA(cudaEventRecord(sim->ev0, st));
-  if (!sim->order.empty()) {
+  if (!cta_list.empty()) {
     sim->n_launches++;
     PHS_CUDA(cudaMemsetAsync(sim->d_ticket.p, 0, sizeof(int), st));
-    PHS_CUDA(launch_cta_path(t, sim->d_order.p, (int)sim->order.size(), sim->d_ticket.p, sim->cta, st));
+    CtaLaunch cfg = sim->cta;
+    cfg.grid = std::min<int>(cfg.grid, (int)cta_list.size());
+    PHS_CUDA(launch_cta_path(t, resume ? sim->d_order2.p : sim->d_order.p, (int)cta_list.size(), sim->d_ticket.p, cfg,
+                             st));
   }
   PHS_CUDA(cudaEventRecord(sim->ev1, st));
   PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
@@ -589,11 +619,12 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
   // instances that ran out of shared-memory slots on the CTA path move to the cluster path (also for later runs)
   std::vector<int32_t> redo;
-  for (int u : sim->order)
+  for (int u : cta_list)
     if (sim->h_res[u].status == kOverflow) redo.push_back(u);
   if (!redo.empty()) {
     for (int inst : redo) {
       sim->cluster_list.push_back(inst);
+      cluster_todo.push_back(inst);
       sim->order.erase(std::find(sim->order.begin(), sim->order.end(), inst));
     }
     if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
@@ -601,7 +632,7 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
     PHS_CUDA(cudaStreamSynchronize(st));
   }
   // cluster path; an instance that overflows a CTA's slot partition is re-run with larger partitions
-  std::vector<int32_t> todo(sim->cluster_list);
+  std::vector<int32_t> todo(cluster_todo);
   for (int64_t scale = sim->cluster_scale; !todo.empty(); scale *= 2) {
     PHS_CUDA(cudaEventRecord(sim->ev0, st));
     phs_status gs = run_cluster_path(sim, todo, scale, st);
@@ -643,6 +674,8 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
                       sim->h_hist.end());
   }
   sim->ran = true;
+  sim->have_park = finite;
+  sim->parked_until = sim->t_stop;
   for (int u = 0; u < U; ++u) {
     const int i = sim->units[u].inst;
     if (sim->h_res[u].status == PHS_ECYCLE)

@@ -85,6 +85,13 @@ struct phs_sim {
   std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
   bool decompose = true;
   double t_stop = 0.0;  // stop time of the current / last run (phs_run_until), +inf for phs_run
+  // parked state of the CTA-path units of a run that stopped at parked_until (phs_run_until resumes from it)
+  phs::DevBuf<unsigned char> d_park;
+  phs::DevBuf<int32_t> d_order2;
+  size_t park_stride = 0;
+  bool have_park = false;
+  int resumed_units = 0;
+  double parked_until = 0.0;
   std::vector<phs::InstDesc> h_desc;  // per unit
   std::vector<phs::InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first

@@ -312,3 +312,35 @@ def test_run_until_stops_where_the_oracle_stops(path):
                 if log:
                     assert np.array_equal(sim.event_log(i), o.event_log())
             sim.close()
+
+
+def test_run_until_resumes_from_the_parked_state():
+    """Successive phs_run_until calls with growing stop times continue the CTA-path units from where they stopped
+    (shared memory and registers parked in global memory); the result at every stop equals the oracle stopped there,
+    and the final state equals a single full run."""
+    w = W.cfg3(batch=3)
+    ref = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST) for i in range(w.batch)]
+    t_end = max(o.completion_times().max() for o in ref)
+    for log, decompose in ((False, True), (True, False)):
+        sim = B.Sim.from_workload(w, event_log=log, decompose=decompose, history=1 << 21)
+        prev = None
+        for frac in (0.1, 0.1, 0.45, 0.8, 0.3, 1.5):           # growing, repeated, backwards, past the end
+            sim.run(until=frac * t_end)
+            resumed = sim.counters()["resumed_units"]
+            assert (resumed > 0) == (prev is not None and frac >= prev), (frac, prev, resumed)
+            prev = frac
+            for i in range(w.batch):
+                o = oracle_build(w.desc, w.instances[i])
+                o.run(mode=orc.MODE_FAST, until=frac * t_end)
+                assert np.array_equal(sim.completion_times(i), o.completion_times(), equal_nan=True), (frac, i)
+                assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+                assert np.array_equal(sim.collective_times(i), o.collective_times(), equal_nan=True)
+                fl, th, rh = o.history()
+                off, tg, rg = sim.history(i)
+                assert np.array_equal(np.diff(off), np.bincount(fl, minlength=o.num_flows))
+                assert np.array_equal(tg, th) and np.array_equal(rg, rh)
+                if log:
+                    assert np.array_equal(sim.event_log(i), o.event_log())
+        for i in range(w.batch):
+            assert np.array_equal(sim.completion_times(i), ref[i].completion_times())
+        sim.close()
