@@ -557,17 +557,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           }
           S.tl[s] = now;
           S.rq[s] = rq;
-          if (T.hist) {  // throughput history: the flow's rate changes to rq at `now`
-            const unsigned long long i = atomicAdd(T.hist_n, 1ull);
-            if (i < (unsigned long long)T.hist_cap) {
-              HistRec h;
-              h.t = now;
-              h.rate = rate_of(rq);
-              h.flow = (uint32_t)S.flow[s];
-              h.ev = (uint32_t)ev;
-              T.hist[i] = h;
-            }
-          }
+          if (T.hist) append_history(T.hist, T.hist_n, T.hist_cap, now, rq, (uint32_t)S.flow[s], (uint32_t)ev);
           S.tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));
         }
         mymin = dmin(mymin, S.tc[s]);

@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "phs_device.h"
+
 namespace phs {
 
 constexpr double kQuantum = 1.0 / 1048576.0;  // 2^-20 byte/s (reading R-FX)
@@ -42,6 +44,21 @@ __device__ __forceinline__ long long fair_share(long long cap_rem, int n) {
 }
 
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+
+// Throughput history (optional, off the hot path: not inlined): the flow at output position `flow` changes its rate
+// to `rq` quanta at time `now`, in the unit's event `ev`.
+static __device__ __noinline__ void append_history(HistRec *hist, unsigned long long *hist_n, long long hist_cap, double now,
+                                            long long rq, uint32_t flow, uint32_t ev) {
+  const unsigned long long i = atomicAdd(hist_n, 1ull);
+  if (i < (unsigned long long)hist_cap) {
+    HistRec h;
+    h.t = now;
+    h.rate = rate_of(rq);
+    h.flow = flow;
+    h.ev = ev;
+    hist[i] = h;
+  }
+}
 
 // non-negative doubles order like their bit patterns
 __device__ __forceinline__ double warp_min(double v) {

@@ -449,17 +449,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           }
           S.s_tl[s] = now;
           S.s_rq[s] = rq;
-          if (T.hist) {  // throughput history: the flow's rate changes to rq at `now`
-            const unsigned long long i = atomicAdd(T.hist_n, 1ull);
-            if (i < (unsigned long long)T.hist_cap) {
-              HistRec h;
-              h.t = now;
-              h.rate = rate_of(rq);
-              h.flow = (uint32_t)S.s_meta[s].x;
-              h.ev = (uint32_t)ev;
-              T.hist[i] = h;
-            }
-          }
+          if (T.hist) append_history(T.hist, T.hist_n, T.hist_cap, now, rq, (uint32_t)S.s_meta[s].x, (uint32_t)ev);
           S.s_tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));  // S4.3: division, then addition
         }
         if (LOG && atomicExch(&S.l_won[arg], g) != g) atomicAdd(&S.ctl[C_EV_ROUNDS], 1);
