@@ -173,8 +173,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     const int F = D.n_flows;
 
     // phs_run_until: a unit that stopped at an earlier t_stop continues from its parked state
-    ParkRegs *park = T.park ? (ParkRegs *)(T.park + (size_t)inst * T.park_stride) : nullptr;
-    const bool resuming = T.resume && park && park->valid;
+    const bool resuming =
+        T.resume && T.park && ((const ParkRegs *)(T.park + (size_t)inst * T.park_stride))->valid;
     // ---- init: nothing active, every slot free
     if (!resuming)
     for (int l = tid; l < Li; l += NT) {
@@ -255,6 +255,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     int status = PHS_OK;
     int first_bneck = -1;
     if (resuming) {  // shared memory and the loop-carried registers as they were when the unit stopped
+      const ParkRegs *park = (const ParkRegs *)(T.park + (size_t)inst * T.park_stride);
       const uint4 *src = (const uint4 *)((const unsigned char *)park + sizeof(ParkRegs));
       uint4 *dst = (uint4 *)smem_raw;
       for (size_t i = tid; i < smem_used / 16; i += NT) dst[i] = src[i];
@@ -646,7 +647,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       sum_rounds += rounds;
       PHS_TICK(6)
     }
-    if (park) {  // park the unit if it stopped at t_stop; a finished unit has nothing to resume
+    if (T.park) {  // park the unit if it stopped at t_stop; a finished unit has nothing to resume
+      ParkRegs *park = (ParkRegs *)(T.park + (size_t)inst * T.park_stride);
       if (status == kPaused) {
         __syncthreads();
         uint4 *dst = (uint4 *)((unsigned char *)park + sizeof(ParkRegs));
