@@ -158,9 +158,9 @@ phs_status phs_run(phs_sim *sim, void *cuda_stream);
 /* PAPER.md L167 "advancing the simulation ... up to a specified time": like phs_run, but stops before the first
  * event later than t_stop_s.  Flows that complete later report completion time NaN and bottleneck -1, a collective
  * with such flows reports NaN; event log and throughput history hold what happened up to t_stop_s.  A later call
- * with a larger time continues: units on the CTA path resume from their parked state, units on the cluster path
- * (and everything, if the time goes backwards) start again from t = 0 -- the simulation is deterministic, so the
- * results are the same either way. */
+ * with a larger time continues: a unit that stopped keeps a copy of its on-chip state in global memory and resumes
+ * from it; if the time goes backwards everything starts again from t = 0 -- the simulation is deterministic, so
+ * the results are the same either way. */
 phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
 
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out);

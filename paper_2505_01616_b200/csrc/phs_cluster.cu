@@ -120,6 +120,12 @@ size_t cluster_smem_bytes(int L, int cluster_size, int64_t Sc, bool aggregate, b
   return smem_layout(L, cluster_size, Sc, aggregate, cold_smem, log, replicate, nullptr, nullptr, nullptr, nullptr,
                      nullptr, nullptr, nullptr);
 }
+size_t cluster_park_cta_bytes(int L, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log,
+                              bool replicate) {
+  const size_t b = cluster_smem_bytes(L, cluster_size, Sc, aggregate, cold_smem, log, replicate) + 64 + sizeof(Comb) +
+                   (cold_smem ? 0 : (size_t)Sc * kSlotColdBytes + 16);  // + 16: the copies move whole 16-byte words
+  return (b + 255) / 256 * 256;
+}
 size_t cluster_region_bytes(int64_t Sc, int cluster_size) {  // global spill area of the cold slot fields
   return (size_t)cluster_size * (((size_t)Sc * kSlotColdBytes + 255) / 256 * 256);
 }
@@ -145,7 +151,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   size_t o_lb, o_won, o_beatf, o_agg, o_repl, o_hot, o_cold;
   const bool REPL = SC.replicate != 0;
-  smem_layout(L, CS, Sc, AGG, SC.cold_smem != 0, LOG, REPL, &o_lb, &o_won, &o_beatf, &o_agg, &o_repl, &o_hot, &o_cold);
+  const size_t smem_used = smem_layout(L, CS, Sc, AGG, SC.cold_smem != 0, LOG, REPL, &o_lb, &o_won, &o_beatf, &o_agg,
+                                       &o_repl, &o_hot, &o_cold);
   // REPL: every CTA keeps its own copy of the links' current fair shares, so that voting reads local shared
   // memory; owners broadcast the shares they recompute after debits, stale first-round shares are refreshed by the
   // flows that need them
@@ -220,7 +227,13 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     phs_event *log = (LOG && D.log_base >= 0) ? T.log + D.log_base : nullptr;
     const int F = D.n_flows;
 
+    // phs_run_until: a unit that stopped at an earlier t_stop continues from its parked state
+    const int pidx = SC.park ? SC.park_index[inst] : -1;
+    unsigned char *upark = pidx >= 0 ? SC.park + (size_t)pidx * SC.park_unit_stride : nullptr;
+    unsigned char *cpark = upark ? upark + kClusterParkHeader + (size_t)crank * SC.park_cta_stride : nullptr;
+    const bool resuming = SC.resume && upark && ((const ClusterParkRegs *)upark)->valid;  // the same in every CTA
     // ---- init: own links, own slots
+    if (!resuming) {
     for (int li = tid; li < Lc; li += NT) {
       const int l = li * CS + crank;
       LinkA a;
@@ -252,6 +265,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     if (tid < M_NCTL) ctl[tid] = 0;
     if (crank == 0 && tid == 0) comb.ev_rounds = 0;
     __syncthreads();
+    }
 
     auto fill_slot = [&](int slot, int out, const FlowRec &r, double ta) {
       S.flow[slot] = out;  // where the flow's results go
@@ -269,12 +283,26 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
 
     // S4: outstanding predecessors.  Flows without predecessors are PENDING from t = 0 with t_act = start + Lat; they
     // wait in the unit's list sorted by t_act (built by phs_finalize) and take a slot only when they activate.
-    for (int64_t f = ctid; f < F; f += CT) pred_cnt[f] = pc0[f];
+    if (!resuming)
+      for (int64_t f = ctid; f < F; f += CT) pred_cnt[f] = pc0[f];
     const double *__restrict__ init_t = T.init_t + D.init_base;
     const int32_t *__restrict__ init_f = T.init_f + D.init_base;
     const int n_init = D.n_init;
     int ip = 0;  // entries [0, ip) of the list have been activated (the same in every thread of the cluster)
     double t_init = n_init > 0 ? __ldg(&init_t[0]) : kInf;
+    if (resuming) {  // this CTA's shared memory, control words and cold slot fields as they were when the unit stopped
+      const uint4 *src = (const uint4 *)cpark;
+      uint4 *dst = (uint4 *)smem_raw;
+      for (size_t i = tid; i < smem_used / 16; i += NT) dst[i] = src[i];
+      const int *pctl = (const int *)(cpark + smem_used);
+      if (tid < M_NCTL) ctl[tid] = pctl[tid];
+      if (crank == 0 && tid == 0) comb = *(const Comb *)(cpark + smem_used + 64);
+      if (!SC.cold_smem) {
+        const uint4 *cs = (const uint4 *)(cpark + smem_used + 64 + sizeof(Comb));
+        uint4 *cd = (uint4 *)S.rem;
+        for (size_t i = tid; i < ((size_t)Sc * kSlotColdBytes + 15) / 16; i += NT) cd[i] = cs[i];
+      }
+    }
     __threadfence();  // pred_cnt[] is decremented by other CTAs of the cluster
     cluster.sync();
 
@@ -292,8 +320,20 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
 #endif
     int nDone = 0, prev_nact = 0;
     double acc_min = kInf;  // (thread 0 of a CTA) minimum of the times folded in this event's rounds
+    if (resuming) {
+      const ClusterParkRegs *pr = (const ClusterParkRegs *)upark;
+      now = pr->now; t_next = pr->t_next; t_init = pr->t_init;
+      sum_active = pr->sum_active; sum_rounds = pr->sum_rounds;
+      ev = pr->ev; solve = pr->solve; g = pr->g; ip = pr->ip; nDone = pr->n_done; prev_nact = pr->prev_nact;
+      max_active = pr->max_active; max_pending = pr->max_pending; max_slots = pr->max_slots;
+      first_bneck = pr->first_bneck;
+    }
 
     for (;;) {
+      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
+        status = kPaused;
+        break;
+      }
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
       ++solve;
       const int hi0 = min(ctl[M_HI], Sc);
@@ -740,9 +780,29 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       }
       sum_active += nA;
       sum_rounds += rounds;
-      if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
-        status = kPaused;
-        break;
+    }
+    if (upark) {  // park the unit if it stopped at t_stop; a finished unit has nothing to resume
+      if (status == kPaused) {
+        __syncthreads();
+        uint4 *dst = (uint4 *)cpark;
+        const uint4 *src = (const uint4 *)smem_raw;
+        for (size_t i = tid; i < smem_used / 16; i += NT) dst[i] = src[i];
+        int *pctl = (int *)(cpark + smem_used);
+        if (tid < M_NCTL) pctl[tid] = ctl[tid];
+        if (crank == 0 && tid == 0) *(Comb *)(cpark + smem_used + 64) = comb;
+        if (!SC.cold_smem) {
+          uint4 *cd = (uint4 *)(cpark + smem_used + 64 + sizeof(Comb));
+          const uint4 *cs = (const uint4 *)S.rem;
+          for (size_t i = tid; i < ((size_t)Sc * kSlotColdBytes + 15) / 16; i += NT) cd[i] = cs[i];
+        }
+      }
+      if (ctid == 0) {
+        ClusterParkRegs r;
+        r.now = now; r.t_next = t_next; r.t_init = t_init; r.sum_active = sum_active; r.sum_rounds = sum_rounds;
+        r.ev = ev; r.solve = solve; r.g = g; r.ip = ip; r.n_done = nDone; r.prev_nact = prev_nact;
+        r.max_active = max_active; r.max_pending = max_pending; r.max_slots = max_slots; r.first_bneck = first_bneck;
+        r.valid = status == kPaused ? 1 : 0; r.pad_ = 0;
+        *(ClusterParkRegs *)upark = r;
       }
     }
 #ifdef PHS_PHASE_CLOCKS

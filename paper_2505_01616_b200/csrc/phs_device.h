@@ -73,7 +73,21 @@ struct ClusterScratch {
   int aggregate;        // 1: a CTA pre-sums its debits per link in shared memory (16 bytes per link and CTA)
   int cold_smem;        // 1: the cold slot fields live in shared memory too
   int replicate;        // 1: every CTA keeps a copy of the links' current fair shares (22 bytes per link and CTA)
+  // phs_run_until: parking areas of units that stopped at t_stop (per unit: ClusterParkRegs, then per CTA a copy
+  // of its shared memory, control words and cold slot fields), or nullptr
+  unsigned char *park;
+  size_t park_unit_stride, park_cta_stride;
+  const int32_t *park_index;  // [units] index of the unit's parking area, -1 = none
+  int resume;                 // 1: units with a valid parked state continue from it
 };
+struct ClusterParkRegs {  // the loop-carried registers of a parked unit (cluster path)
+  double now, t_next, t_init;
+  long long sum_active, sum_rounds;
+  int32_t ev, solve, g, ip, n_done, prev_nact, max_active, max_pending, max_slots, first_bneck, valid, pad_;
+};
+constexpr size_t kClusterParkHeader = 256;  // bytes reserved for ClusterParkRegs at the start of a unit's area
+size_t cluster_park_cta_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log,
+                              bool replicate);
 constexpr int kClusterThreads = 512;
 // dynamic shared memory per CTA / global spill bytes per cluster
 size_t cluster_smem_bytes(int n_links, int cluster_size, int64_t Sc, bool aggregate, bool cold_smem, bool log,

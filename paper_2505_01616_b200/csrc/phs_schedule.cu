@@ -485,7 +485,8 @@ DevTables tables_of(phs_sim *sim, int n_links) {
 // Cluster path (a9): every instance in `list` is simulated by one thread-block cluster with all dynamic state in
 // the shared memory of its CTAs; clusters pull instances from the list until it is empty.  `slot_scale` scales the
 // guess of how many flows are PENDING or ACTIVE at once (doubled after an overflow).
-phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, cudaStream_t st) {
+phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, bool park,
+                            bool resume, cudaStream_t st) {
   if (list.empty()) return PHS_OK;
   int L = 1;  // the shared-memory layout is sized for the unit with the most links
   for (int u : list) L = std::max(L, sim->units[u].n_links);
@@ -549,6 +550,42 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   sc.aggregate = agg ? 1 : 0;
   sc.cold_smem = cold ? 1 : 0;
   sc.replicate = repl ? 1 : 0;
+  // phs_run_until: parking areas, one per cluster-path unit, valid for one launch configuration
+  sc.park = nullptr;
+  sc.park_unit_stride = sc.park_cta_stride = 0;
+  sc.park_index = nullptr;
+  sc.resume = 0;
+  if (park || resume) {
+    const size_t cta_bytes = cluster_park_cta_bytes(L, cs, Sc, agg, cold, log, repl);
+    const size_t unit_bytes = kClusterParkHeader + (size_t)cs * cta_bytes;
+    const bool same = sim->cpark_unit_bytes == unit_bytes && sim->cpark_cs == cs && sim->cpark_Sc == Sc &&
+                      sim->cpark_L == L && sim->d_cpark.p;
+    if (!same) {  // (re)build: every unit of the cluster list gets an area; what was parked before is void
+      std::vector<int32_t> index(sim->units.size(), -1);
+      int32_t n = 0;
+      for (int u : sim->cluster_list) index[u] = n++;
+      for (int u : list)
+        if (index[u] < 0) index[u] = n++;
+      PHS_CUDA(sim->d_cpark.alloc(unit_bytes * (size_t)std::max(n, 1)));
+      PHS_CUDA(cudaMemsetAsync(sim->d_cpark.p, 0, unit_bytes * (size_t)std::max(n, 1), st));
+      PHS_CUDA(sim->d_cpark_index.upload(index, st));
+      PHS_CUDA(cudaStreamSynchronize(st));
+      sim->cpark_index = index;
+      sim->cpark_unit_bytes = unit_bytes;
+      sim->cpark_cs = cs;
+      sim->cpark_Sc = Sc;
+      sim->cpark_L = L;
+    }
+    bool all_indexed = true;
+    for (int u : list) all_indexed = all_indexed && sim->cpark_index[u] >= 0;
+    if (all_indexed) {  // units that joined the cluster path later (slot overflow) simply start from t = 0
+      sc.park = sim->d_cpark.p;
+      sc.park_unit_stride = unit_bytes;
+      sc.park_cta_stride = cta_bytes;
+      sc.park_index = sim->d_cpark_index.p;
+      sc.resume = resume && same ? 1 : 0;
+    }
+  }
   PHS_CUDA(launch_cluster_path(tables_of(sim, L), sim->d_clist.p, (int)sorted.size(), sim->d_cticket.p, sc, cs,
                                n_clusters, log, st));
   PHS_CUDA(cudaStreamSynchronize(st));  // `sorted` is pageable host memory read by the async copy
@@ -573,9 +610,10 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   sim->last_stream = st;
   const int U = (int)sim->units.size();
   const bool finite = std::isfinite(sim->t_stop);
-  // Resume: a run that stopped at an earlier time left the CTA-path units parked (shared memory + registers in
-  // global memory); a later stop time continues them from there.  Cluster-path units, and everything when the time
-  // goes backwards, start again from t = 0 -- the simulation is deterministic, so the results are the same.
+  // Resume: a run that stopped at an earlier time left its units parked (shared memory + registers in global
+  // memory); a later stop time continues them from there.  When the time goes backwards (or a unit changed its
+  // launch configuration after an overflow) the simulation starts again from t = 0 -- it is deterministic, so the
+  // results are the same.
   const bool resume = sim->have_park && sim->ran && sim->t_stop >= sim->parked_until;
   if (finite && !sim->order.empty() && sim->park_stride == 0) {
     sim->park_stride = (sizeof(ParkRegs) + sim->cta.smem + 255) / 256 * 256;
@@ -595,7 +633,7 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
     cluster_todo.erase(std::remove_if(cluster_todo.begin(), cluster_todo.end(), [&](int u) { return !paused(u); }),
                        cluster_todo.end());
     if (!cta_list.empty()) PHS_CUDA(sim->d_order2.upload(cta_list, st));
-    sim->resumed_units = (int)cta_list.size();
+    sim->resumed_units = (int)cta_list.size() + (sim->d_cpark.p ? (int)cluster_todo.size() : 0);
   } else {
     PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * U, st));  // empty units report status OK
     if (sim->hist_cap > 0) PHS_CUDA(cudaMemsetAsync(sim->d_hist_n.p, 0, sizeof(unsigned long long), st));
@@ -635,7 +673,7 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   std::vector<int32_t> todo(cluster_todo);
   for (int64_t scale = sim->cluster_scale; !todo.empty(); scale *= 2) {
     PHS_CUDA(cudaEventRecord(sim->ev0, st));
-    phs_status gs = run_cluster_path(sim, todo, scale, st);
+    phs_status gs = run_cluster_path(sim, todo, scale, finite, resume, st);
     if (gs != PHS_OK) return gs;
     sim->n_launches++;
     PHS_CUDA(cudaEventRecord(sim->ev1, st));

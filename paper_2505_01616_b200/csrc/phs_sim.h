@@ -91,6 +91,13 @@ struct phs_sim {
   size_t park_stride = 0;
   bool have_park = false;
   int resumed_units = 0;
+  // cluster path: parking areas (one launch configuration at a time)
+  phs::DevBuf<unsigned char> d_cpark;
+  phs::DevBuf<int32_t> d_cpark_index;
+  std::vector<int32_t> cpark_index;
+  size_t cpark_unit_bytes = 0;
+  int cpark_cs = 0, cpark_L = 0;
+  int64_t cpark_Sc = 0;
   double parked_until = 0.0;
   std::vector<phs::InstDesc> h_desc;  // per unit
   std::vector<phs::InstResult> h_res; // per unit

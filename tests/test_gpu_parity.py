@@ -314,15 +314,16 @@ def test_run_until_stops_where_the_oracle_stops(path):
             sim.close()
 
 
-def test_run_until_resumes_from_the_parked_state():
-    """Successive phs_run_until calls with growing stop times continue the CTA-path units from where they stopped
-    (shared memory and registers parked in global memory); the result at every stop equals the oracle stopped there,
-    and the final state equals a single full run."""
+@pytest.mark.parametrize("path", [0, CLUSTER])
+def test_run_until_resumes_from_the_parked_state(path):
+    """Successive phs_run_until calls with growing stop times continue the units from where they stopped (shared
+    memory and registers parked in global memory, on both kernel paths); the result at every stop equals the oracle
+    stopped there, and the final state equals a single full run."""
     w = W.cfg3(batch=3)
     ref = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST) for i in range(w.batch)]
     t_end = max(o.completion_times().max() for o in ref)
     for log, decompose in ((False, True), (True, False)):
-        sim = B.Sim.from_workload(w, event_log=log, decompose=decompose, history=1 << 21)
+        sim = B.Sim.from_workload(w, event_log=log, decompose=decompose, history=1 << 21, path=path)
         prev = None
         for frac in (0.1, 0.1, 0.45, 0.8, 0.3, 1.5):           # growing, repeated, backwards, past the end
             sim.run(until=frac * t_end)
@@ -344,3 +345,26 @@ def test_run_until_resumes_from_the_parked_state():
         for i in range(w.batch):
             assert np.array_equal(sim.completion_times(i), ref[i].completion_times())
         sim.close()
+
+
+def test_run_until_resumes_a_multi_cta_cluster():
+    """Parking on the cluster path with several CTAs per unit (replicated shares, debit pre-aggregation): 4032
+    concurrent flows per instance, stopped twice on the way."""
+    w = W.cfg4(batch=2, n_hosts=8, gph=8, n_leaves=4, n_spines=2)
+    sim = B.Sim.from_workload(w, path=CLUSTER, history=1 << 22)
+    ref = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST) for i in range(w.batch)]
+    t_end = max(o.completion_times().max() for o in ref)
+    for k, frac in enumerate((0.2, 0.6, 1.2)):
+        sim.run(until=frac * t_end)
+        c = sim.counters()
+        assert c["cluster_size"] > 1 and (c["resumed_units"] > 0) == (k > 0)
+        for i in range(w.batch):
+            o = oracle_build(w.desc, w.instances[i])
+            o.run(mode=orc.MODE_FAST, until=frac * t_end)
+            assert np.array_equal(sim.completion_times(i), o.completion_times(), equal_nan=True), (frac, i)
+            assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+            fl, th, rh = o.history()
+            off, tg, rg = sim.history(i)
+            assert np.array_equal(np.diff(off), np.bincount(fl, minlength=o.num_flows))
+            assert np.array_equal(tg, th) and np.array_equal(rg, rh)
+    sim.close()
