@@ -139,8 +139,9 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
 
 // ================================================================================================ CTA kernel
 // NT threads; LOG: write the event log (and solve every component at every event, so that the log's iteration
-// count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory.
-template <int NT, bool LOG, bool PCS>
+// count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory;
+// HIST: record the throughput history (a call in the hottest block of the kernel: compiled out when not wanted).
+template <int NT, bool LOG, bool PCS, bool HIST>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
                                                      int *ticket, int SC, int pcf) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -450,7 +451,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           }
           S.s_tl[s] = now;
           S.s_rq[s] = rq;
-          if (T.hist) append_history(T.hist, T.hist_n, T.hist_cap, now, rq, (uint32_t)S.s_meta[s].x, (uint32_t)ev);
+          if (HIST) append_history(T.hist, T.hist_n, T.hist_cap, now, rq, (uint32_t)S.s_meta[s].x, (uint32_t)ev);
           S.s_tc[s] = __dadd_rn(now, __ddiv_rn(rem, rate_of(rq)));  // S4.3: division, then addition
         }
         if (LOG && atomicExch(&S.l_won[arg], g) != g) atomicAdd(&S.ctl[C_EV_ROUNDS], 1);
@@ -687,14 +688,20 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
 
 // ------------------------------------------------------------------------------------------------ launchers
 namespace {
+template <int NT, bool LOG, bool PCS, bool HIST>
+cudaError_t launch_hist(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
+                        cudaStream_t stream) {
+  cudaError_t e = cudaFuncSetAttribute(phs_cta_kernel<NT, LOG, PCS, HIST>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  phs_cta_kernel<NT, LOG, PCS, HIST><<<c.grid, NT, c.smem, stream>>>(t, order, n, ticket, c.slots, c.pc_flows);
+  return cudaGetLastError();
+}
 template <int NT, bool LOG, bool PCS>
 cudaError_t launch_one(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
                        cudaStream_t stream) {
-  cudaError_t e = cudaFuncSetAttribute(phs_cta_kernel<NT, LOG, PCS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)c.smem);
-  if (e != cudaSuccess) return e;
-  phs_cta_kernel<NT, LOG, PCS><<<c.grid, NT, c.smem, stream>>>(t, order, n, ticket, c.slots, c.pc_flows);
-  return cudaGetLastError();
+  return t.hist ? launch_hist<NT, LOG, PCS, true>(t, order, n, ticket, c, stream)
+                : launch_hist<NT, LOG, PCS, false>(t, order, n, ticket, c, stream);
 }
 template <int NT>
 cudaError_t launch_nt(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
