@@ -356,10 +356,11 @@ class Sim:
                 phs_set_link_capacities(sim.h, i, cap)
         # identical op structure across instances -> batched submission; else per instance
         from . import workloads as W
-        same = all(len(x.ops) == len(insts[0].ops) for x in insts) and all(
-            isinstance(o, W.Coll) for x in insts for o in x.ops)
-        if same and count > 1:
-            for k, op0 in enumerate(insts[0].ops):
+        same = getattr(w, "uniform_ops", False)      # the generator states it; otherwise compare
+        if not same and count > 1:
+            same = all(len(x.ops) == len(insts[0].ops) for x in insts) and all(
+                isinstance(o, W.Coll) for x in insts for o in x.ops)
+            for k, op0 in enumerate(insts[0].ops) if same else ():
                 ok = all(x.ops[k].kind == op0.kind and np.array_equal(x.ops[k].ranks, op0.ranks)
                          and tuple(x.ops[k].after) == tuple(op0.after) for x in insts)
                 if not ok:

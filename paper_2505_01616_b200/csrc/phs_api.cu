@@ -56,6 +56,14 @@ phs_status phs_batch(const phs_sim *sim, int32_t *out) {
   return PHS_OK;
 }
 
+// The instance with every submitted collective expanded into flows.  Expansion is deferred bookkeeping, not a change
+// of the handle's observable state, hence the const_cast.
+static const Instance &expanded(const phs_sim *sim, int32_t instance) {
+  Instance &in = const_cast<phs_sim *>(sim)->inst[(size_t)instance];
+  expand_pending(*sim->fab, in);
+  return in;
+}
+
 static phs_status check_instance(const phs_sim *sim, int32_t instance, bool allow_all) {
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (instance == -1 && allow_all) return PHS_OK;
@@ -117,22 +125,14 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
     if (!(bytes[i] > 0.0) || !std::isfinite(bytes[i])) return fail(PHS_EINVAL, "bytes must be positive and finite");
     if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return fail(PHS_EINVAL, "bad start_time_s");
   }
-  // instance 0 first: the arguments shared by all instances (kind, ranks, after) fail here before anything is added;
-  // the others are independent and are expanded on host threads
+  // the arguments shared by all instances (kind, ranks, after) fail on instance 0, before anything is added.  Only
+  // the descriptor is recorded here: the flows are expanded per instance on the host threads of phs_finalize.
   std::string why;
-  phs_status st0 = append_collective(*sim->fab, sim->inst[0], kind, ranks, n_ranks, bytes[0], start ? start[0] : 0.0,
-                                     after, n_after, &why);
-  if (st0 != PHS_OK) return fail(st0, why);
-  std::vector<phs_status> sts((size_t)sim->batch, PHS_OK);
-  std::vector<std::string> whys((size_t)sim->batch);
-  const int64_t work = (int64_t)sim->batch * sim->inst[0].colls.back().n_flows;  // a thread per ~8K flows
-  parallel_for(sim->batch - 1, [&](int k) {
-    const int i = k + 1;
-    sts[i] = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0, after,
-                               n_after, &whys[i]);
-  }, (int)std::max<int64_t>(1, work / 8192));
-  for (int i = 1; i < sim->batch; ++i)
-    if (sts[i] != PHS_OK) return fail(sts[i], whys[i]);
+  for (int i = 0; i < sim->batch; ++i) {
+    phs_status sti = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
+                                       after, n_after, &why);
+    if (sti != PHS_OK) return fail(sti, why);
+  }
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;
   return PHS_OK;
 }
@@ -217,14 +217,14 @@ phs_status phs_num_path_entries(const phs_sim *sim, int32_t instance, int64_t *o
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!out) return fail(PHS_EINVAL, "null output");
-  *out = (int64_t)sim->inst[instance].path.size();
+  *out = (int64_t)expanded(sim, instance).path.size();
   return PHS_OK;
 }
 
 phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *links, int64_t cap) {
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
-  const Instance &in = sim->inst[instance];
+  const Instance &in = expanded(sim, instance);
   if (!off || !links || cap < (int64_t)in.path.size()) return fail(PHS_EINVAL, "output too small");
   for (size_t f = 0; f < in.path_off.size(); ++f) off[f] = in.path_off[f];
   std::copy(in.path.begin(), in.path.end(), links);
@@ -235,7 +235,7 @@ phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int
                          int64_t *n_entries) {
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
-  const Instance &in = sim->inst[instance];
+  const Instance &in = expanded(sim, instance);
   if (!n_entries) return fail(PHS_EINVAL, "null n_entries");
   *n_entries = (int64_t)in.pred.size();
   if (off)
@@ -251,7 +251,7 @@ phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src
                               double *lat, int64_t n) {
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
-  const Instance &in = sim->inst[instance];
+  const Instance &in = expanded(sim, instance);
   if (n != in.n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
   if (src) std::copy(in.src.begin(), in.src.end(), src);
   if (dst) std::copy(in.dst.begin(), in.dst.end(), dst);

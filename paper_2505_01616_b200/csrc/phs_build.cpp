@@ -155,6 +155,21 @@ int32_t push_flow(const Fabric &fab, Instance &inst, int32_t src, int32_t dst, d
   return (int32_t)inst.src.size() - 1;
 }
 
+// Adds a copy of flow `of` that starts at 0 and has no dependencies yet: same endpoints, bytes, path and latency.
+void repeat_flow(Instance &inst, size_t of) {
+  int32_t hops[kMaxHops];
+  const uint32_t p0 = inst.path_off[of], n = inst.path_off[of + 1] - p0;
+  for (uint32_t h = 0; h < n; ++h) hops[h] = inst.path[p0 + h];
+  inst.path.insert(inst.path.end(), hops, hops + n);
+  inst.src.push_back(inst.src[of]);
+  inst.dst.push_back(inst.dst[of]);
+  inst.bytes.push_back(inst.bytes[of]);
+  inst.start.push_back(0.0);
+  inst.lat.push_back(inst.lat[of]);
+  inst.path_off.push_back((uint32_t)inst.path.size());
+  inst.pred_off.push_back((uint32_t)inst.pred.size());
+}
+
 // A dependency of the flow pushed last.
 inline void push_dep(Instance &inst, int32_t on) {
   inst.pred.push_back(on);
@@ -224,9 +239,27 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   c.ranks.assign(ranks, ranks + N);
   c.chain = (int32_t)inst.colls.size();
   for (int a = 0; a < n_after; ++a) c.chain = std::min(c.chain, inst.colls[after[a]].chain);
-  const int32_t conn = (int32_t)inst.colls.size();  // ECMP key: one path per (pair, collective)
-  const double chunk = bytes / (double)N;
-  if (kind == PHS_ALLTOALL) {
+  c.bytes = bytes;
+  c.start = start;
+  c.after.assign(after, after + n_after);
+  inst.flow_count += nf;
+  inst.colls.push_back(std::move(c));
+  return PHS_OK;
+}
+
+namespace {
+
+// S3: the flows and dependencies of collective `id`, appended at flow id first_flow.
+void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
+  const Collective &c = inst.colls[(size_t)id];
+  const int N = c.n_ranks, steps = c.steps;
+  const int32_t *ranks = c.ranks.data();
+  const int32_t *after = c.after.data();
+  const int n_after = (int)c.after.size();
+  const double start = c.start;
+  const int32_t conn = id;  // ECMP key: one path per (pair, collective)
+  const double chunk = c.bytes / (double)N;
+  if (c.kind == PHS_ALLTOALL) {
     for (int i = 0; i < N; ++i)
       for (int j = 0; j < N; ++j) {
         if (i == j) continue;
@@ -235,23 +268,38 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
       }
   } else {
     // step-major: flow (s, i) sends chunk from ranks[i] to ranks[i+1]; it waits for the chunk it forwards
-    // (s-1, i-1) and for the sender's previous send (s-1, i) -- FIFO per connection.
+    // (s-1, i-1) and for the sender's previous send (s-1, i) -- FIFO per connection.  ECMP keys on (pair,
+    // collective), so step s > 0 of ring position i takes the path of step 0 and copies it.
     for (int s = 0; s < steps; ++s) {
       const int32_t prev = c.first_flow + (s - 1) * N;
       for (int i = 0; i < N; ++i) {
-        const int next_rank = i + 1 == N ? 0 : i + 1;
-        push_flow(fab, inst, ranks[i], ranks[next_rank], chunk, s == 0 ? start : 0.0, conn);
         if (s == 0) {
+          const int next_rank = i + 1 == N ? 0 : i + 1;
+          push_flow(fab, inst, ranks[i], ranks[next_rank], chunk, start, conn);
           for (int a = 0; a < n_after; ++a) chain_after(inst, inst.colls[after[a]], ranks[i]);
         } else {
+          repeat_flow(inst, (size_t)c.first_flow + (size_t)i);
           push_dep(inst, prev + (i == 0 ? N - 1 : i - 1));
           push_dep(inst, prev + i);
         }
       }
     }
   }
-  inst.colls.push_back(std::move(c));
-  return PHS_OK;
+}
+
+}  // namespace
+
+void expand_pending(const Fabric &fab, Instance &inst) {
+  if (inst.expanded == inst.colls.size()) return;
+  const size_t F = (size_t)inst.flow_count;
+  inst.src.reserve(F);
+  inst.dst.reserve(F);
+  inst.bytes.reserve(F);
+  inst.start.reserve(F);
+  inst.lat.reserve(F);
+  inst.path_off.reserve(F + 1);
+  inst.pred_off.reserve(F + 1);
+  for (; inst.expanded < inst.colls.size(); ++inst.expanded) expand_collective(fab, inst, (int32_t)inst.expanded);
 }
 
 phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,
@@ -262,6 +310,7 @@ phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int3
     return PHS_EINVAL;
   };
   if (n < 0 || (n > 0 && (!src || !dst || !bytes))) return bad("null flow arrays");
+  expand_pending(fab, inst);  // flow ids follow submission order
   const int64_t first = inst.n_flows();
   if (first + n > 0x7ffffff0LL) {
     if (why) *why = "too many flows in one instance";
@@ -285,6 +334,7 @@ phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int3
     if (dep_off)
       for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) push_dep(inst, (int32_t)dep_ids[e]);
   }
+  inst.flow_count += n;
   return PHS_OK;
 }
 

@@ -69,6 +69,10 @@ struct Collective {
   int32_t kind, n_ranks, first_flow, n_flows, steps;
   int32_t chain;  // smallest id among the collectives this one is (transitively) chained `after`, else its own id
   std::vector<int32_t> ranks;
+  // as submitted: the flows are appended to the instance arrays later (Instance::expanded), on the host threads
+  // that build the instance's tables
+  double bytes = 0.0, start = 0.0;
+  std::vector<int32_t> after;
 };
 
 struct Instance {
@@ -81,7 +85,9 @@ struct Instance {
   std::vector<uint32_t> pred_off{0};
   std::vector<int32_t> pred;
   std::vector<Collective> colls;
-  int64_t n_flows() const { return (int64_t)src.size(); }
+  int64_t flow_count = 0;  // flows submitted so far, including those of collectives not expanded yet
+  size_t expanded = 0;     // colls[0 .. expanded) have their flows in the arrays above
+  int64_t n_flows() const { return flow_count; }
 };
 
 // Link numbering and ECMP routing of one topology (S1, S2).
@@ -103,7 +109,11 @@ class Fabric {
 
 uint64_t splitmix64_step(uint64_t x);
 
-// Appends flows / collectives to an instance (S3).  Return PHS_OK or an error with *why set.
+// Appends the flows of every collective that was submitted but not expanded yet (S3); idempotent.
+void expand_pending(const Fabric &fab, Instance &inst);
+
+// Appends flows / collectives to an instance (S3).  Return PHS_OK or an error with *why set.  append_collective
+// validates and records the collective; its flows appear with the next expand_pending.
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                              double bytes, double start, const int32_t *after, int32_t n_after, std::string *why);
 phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,

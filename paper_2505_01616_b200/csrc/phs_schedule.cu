@@ -9,8 +9,18 @@
 #include <numeric>
 
 #include "phs_sim.h"
+#include <chrono>
+#include <cstdio>
+#include <cstdlib>
 
 using namespace phs;
+
+namespace phs {
+StagingArea &staging_area() {
+  static StagingArea area;  // never freed: the CUDA context may be gone when static destructors run
+  return area;
+}
+}  // namespace phs
 
 #define fail phs_fail
 
@@ -24,12 +34,17 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return PHS_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  const bool timing_ = getenv("PHS_TIMING") != nullptr;
+  auto tp_ = std::chrono::steady_clock::now();
+#define PHS_T(name) if (timing_) { auto n_ = std::chrono::steady_clock::now(); fprintf(stderr, "[phs_finalize] %-22s %8.2f ms\n", name, std::chrono::duration<double, std::milli>(n_ - tp_).count()); tp_ = n_; }
   int dev = 0;
   PHS_CUDA(cudaGetDevice(&dev));
-  cudaDeviceProp prop;
-  PHS_CUDA(cudaGetDeviceProperties(&prop, dev));
-  sim->sm_count = prop.multiProcessorCount;
-  sim->smem_optin = (size_t)prop.sharedMemPerBlockOptin;
+  int sm_count = 0, smem_optin = 0, smem_per_sm = 0;  // three attributes: cudaGetDeviceProperties costs milliseconds
+  PHS_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+  PHS_CUDA(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  PHS_CUDA(cudaDeviceGetAttribute(&smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+  sim->sm_count = sm_count;
+  sim->smem_optin = (size_t)smem_optin;
   const int B = sim->batch, L = sim->fab->n_links();
 
   sim->flow_base.assign(B + 1, 0);
@@ -50,9 +65,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   // per-instance work is independent: every instance builds its own chunk of the tables on a host thread, the
   // chunks are then laid out back to back
   struct Chunk {
-    std::vector<FlowRec> rec;
-    std::vector<int32_t> succ, pc0, lcomp, linkid;
-    std::vector<uint32_t> fmap;
+    std::vector<int32_t> succ, lcomp, linkid;
     std::vector<uint8_t> pc8;
     std::vector<int64_t> capq;
     std::vector<double> init_t;
@@ -64,15 +77,24 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const char *err = "";
   };
   std::vector<Chunk> chunks((size_t)B);
+  // the per-flow tables (72 of the ~80 bytes per flow) have a known place per instance: the host threads write them
+  // straight into the page-locked staging area, unit after unit from flow_base[i] on
+  StagingArea &stage = staging_area();
+  std::lock_guard<std::mutex> stage_lock(stage.mu);
+  const size_t rec_bytes = ((size_t)Ft * sizeof(FlowRec) + 255) / 256 * 256, i32_bytes = ((size_t)Ft * 4 + 255) / 256 * 256;
+  unsigned char *stage_p = stage.get(rec_bytes + 2 * i32_bytes);
+  if (!stage_p) return fail(PHS_ENOMEM, "out of host memory for the table staging area");
+  FlowRec *const rec = (FlowRec *)stage_p;
+  int32_t *const pc0 = (int32_t *)(stage_p + rec_bytes);
+  uint32_t *const fmap = (uint32_t *)(stage_p + rec_bytes + i32_bytes);
   std::vector<int64_t> coll_first((size_t)sim->total_colls);
   std::vector<int32_t> coll_n((size_t)sim->total_colls);
   auto build_instance = [&](int i) {
     Chunk &c = chunks[(size_t)i];
+    expand_pending(*sim->fab, sim->inst[i]);  // a2 + a3 of the collectives submitted since the last expansion
     const Instance &in = sim->inst[i];
     const int64_t F = in.n_flows();
-    c.rec.resize((size_t)F);
-    c.pc0.resize((size_t)F);
-    c.fmap.resize((size_t)F);
+    const int64_t fb = sim->flow_base[i];
     int64_t flow_cursor = 0, log_cursor = 0;
     std::vector<int64_t> capq_inst((size_t)L);
     std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
@@ -238,10 +260,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) c.succ.push_back(flow_loc[sdst[e]]);
         }
         x.comp = p0 < p1 ? link_loc[find_in(parent, in.path[p0])] : 0;
-        c.rec[(size_t)flow_cursor + k] = x;
-        c.fmap[(size_t)flow_cursor + k] = (uint32_t)(sim->flow_base[i] + f);
+        rec[(size_t)(fb + flow_cursor) + k] = x;
+        fmap[(size_t)(fb + flow_cursor) + k] = (uint32_t)(fb + f);
         const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
-        c.pc0[(size_t)flow_cursor + k] = np;
+        pc0[(size_t)(fb + flow_cursor) + k] = np;
         c.max_pred = std::max(c.max_pred, np);
         c.pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
       }
@@ -268,7 +290,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       c.units.push_back(un);
     }
   };
+  PHS_T("setup");
   parallel_for(B, build_instance);
+  PHS_T("build_instances");
   for (int i = 0; i < B; ++i)
     if (chunks[i].st != PHS_OK) return fail(chunks[i].st, chunks[i].err);
   // lay the chunks out back to back
@@ -279,20 +303,18 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   int max_pred = 0;
   for (int i = 0; i < B; ++i) {
     const Chunk &c = chunks[i];
-    b_flow[i + 1] = b_flow[i] + (int64_t)c.rec.size();
+    b_flow[i + 1] = sim->flow_base[i + 1];
     b_link[i + 1] = b_link[i] + (int64_t)c.capq.size();
     b_succ[i + 1] = b_succ[i] + (int64_t)c.succ.size();
     b_pc8[i + 1] = b_pc8[i] + (int64_t)c.pc8.size();
     b_init[i + 1] = b_init[i] + (int64_t)c.init_t.size();
-    b_log[i + 1] = b_log[i] + 2 * (int64_t)c.rec.size() + 2 * (int64_t)c.units.size();
+    b_log[i + 1] = b_log[i] + 2 * (sim->flow_base[i + 1] - sim->flow_base[i]) + 2 * (int64_t)c.units.size();
     sim->unit_first[i] = (int32_t)sim->units.size();
     sim->units.insert(sim->units.end(), c.units.begin(), c.units.end());
     max_pred = std::max(max_pred, c.max_pred);
   }
   const int64_t log_cursor = b_log[B];
-  std::vector<FlowRec> rec((size_t)Ft);
-  std::vector<int32_t> succ((size_t)b_succ[B]), pc0((size_t)Ft), lcomp((size_t)b_link[B]), linkid((size_t)b_link[B]);
-  std::vector<uint32_t> fmap((size_t)Ft);
+  std::vector<int32_t> succ((size_t)b_succ[B]), lcomp((size_t)b_link[B]), linkid((size_t)b_link[B]);
   std::vector<uint8_t> pc8((size_t)b_pc8[B]);
   std::vector<int64_t> capq((size_t)b_link[B]);
   std::vector<double> init_t((size_t)b_init[B]);
@@ -300,9 +322,6 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   sim->h_desc.assign(sim->units.size(), InstDesc{});
   parallel_for(B, [&](int i) {
     Chunk &c = chunks[i];
-    std::copy(c.rec.begin(), c.rec.end(), rec.begin() + b_flow[i]);
-    std::copy(c.pc0.begin(), c.pc0.end(), pc0.begin() + b_flow[i]);
-    std::copy(c.fmap.begin(), c.fmap.end(), fmap.begin() + b_flow[i]);
     std::copy(c.succ.begin(), c.succ.end(), succ.begin() + b_succ[i]);
     std::copy(c.pc8.begin(), c.pc8.end(), pc8.begin() + b_pc8[i]);
     std::copy(c.capq.begin(), c.capq.end(), capq.begin() + b_link[i]);
@@ -320,19 +339,18 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       if (d.log_base >= 0) d.log_base += b_log[i];
       sim->h_desc[(size_t)sim->unit_first[i] + k] = d;
     }
-    Chunk().rec.swap(c.rec);  // release the chunk's big arrays early
-    std::vector<uint32_t>().swap(c.fmap);
   });
+  PHS_T("concat");
   sim->unit_first[B] = (int32_t)sim->units.size();
   const int U = (int)sim->units.size();
   const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
 
   PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
-  PHS_CUDA(sim->d_rec.upload(rec, st));
+  PHS_CUDA(sim->d_rec.upload(rec, (size_t)Ft, st));
   if (pc8_ok) PHS_CUDA(sim->d_pc8.upload(pc8, st));
   PHS_CUDA(sim->d_succ.upload(succ, st));
-  PHS_CUDA(sim->d_pc0.upload(pc0, st));
-  PHS_CUDA(sim->d_fmap.upload(fmap, st));
+  PHS_CUDA(sim->d_pc0.upload(pc0, (size_t)Ft, st));
+  PHS_CUDA(sim->d_fmap.upload(fmap, (size_t)Ft, st));
   PHS_CUDA(sim->d_init_t.upload(init_t, st));
   PHS_CUDA(sim->d_init_f.upload(init_f, st));
   PHS_CUDA(sim->d_capq.upload(capq, st));
@@ -352,12 +370,13 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     PHS_CUDA(sim->d_hist_n.alloc(1));
   }
   sim->h_res.assign(U, InstResult{});
+  PHS_T("upload+alloc issued");
 
   // ---- a9: batch scheduler, static part.  A unit whose state fits the shared memory of one SM goes to the CTA
   // path (one launch configuration, sized for the largest such unit, with as many CTAs resident per SM as fit);
   // the others go to the cluster path.  Units that overflow their slots at run time move to the cluster path.
-  const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin;
-  const size_t per_sm = (size_t)prop.sharedMemPerMultiprocessor;
+  const size_t smem_max = (size_t)smem_optin;
+  const size_t per_sm = (size_t)smem_per_sm;
   const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
@@ -439,10 +458,12 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     break;
   }
   std::sort(sim->cluster_list.begin(), sim->cluster_list.end());
+  PHS_T("scheduler");
   PHS_CUDA(cudaStreamSynchronize(st));  // the staging vectors die here
-  sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + rec.size() * sizeof(FlowRec) +
-                             (succ.size() + pc0.size() + coll_n.size() + sim->order.size() + lcomp.size() + linkid.size() +
-                              fmap.size() + init_f.size()) * 4 + init_t.size() * 8 + (pc8_ok ? pc8.size() : 0) +
+  PHS_T("sync");
+  sim->h2d_bytes = (int64_t)(sim->h_desc.size() * sizeof(InstDesc) + (size_t)Ft * sizeof(FlowRec) +
+                             (succ.size() + (size_t)Ft + coll_n.size() + sim->order.size() + lcomp.size() + linkid.size() +
+                              (size_t)Ft + init_f.size()) * 4 + init_t.size() * 8 + (pc8_ok ? pc8.size() : 0) +
                              (capq.size() + coll_first.size()) * 8);
   PHS_CUDA(cudaEventCreate(&sim->ev0));
   PHS_CUDA(cudaEventCreate(&sim->ev1));

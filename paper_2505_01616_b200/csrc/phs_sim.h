@@ -5,9 +5,11 @@
 
 #include <algorithm>
 #include <atomic>
+#include <cstdlib>
 #include <memory>
 #include <string>
 #include <thread>
+#include <mutex>
 #include <vector>
 
 #include "phs_device.h"
@@ -55,12 +57,46 @@ struct DevBuf {
     n = count;
     return cudaMalloc((void **)&p, std::max<size_t>(count, 1) * sizeof(T));
   }
-  cudaError_t upload(const std::vector<T> &h, cudaStream_t st) {
-    cudaError_t e = alloc(h.size());
-    if (e != cudaSuccess || h.empty()) return e;
-    return cudaMemcpyAsync(p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+  cudaError_t upload(const T *h, size_t count, cudaStream_t st) {
+    cudaError_t e = alloc(count);
+    if (e != cudaSuccess || count == 0) return e;
+    return cudaMemcpyAsync(p, h, count * sizeof(T), cudaMemcpyHostToDevice, st);
+  }
+  cudaError_t upload(const std::vector<T> &h, cudaStream_t st) { return upload(h.data(), h.size(), st); }
+};
+
+// Process-wide page-locked staging area for the tables phs_finalize builds (the per-flow tables are written into
+// it by the host threads and copied to HBM at full PCIe / C2C rate).  It grows to the largest request and is
+// reused by later handles, so only the first phs_finalize pays for pinning; `mu` is held from the build to the
+// end of the copy.  If pinning fails the area is ordinary pageable memory (the copy is slower, nothing else changes).
+struct StagingArea {
+  std::mutex mu;
+  unsigned char *p = nullptr;
+  size_t cap = 0;
+  bool pinned = false;
+  unsigned char *get(size_t bytes) {  // call with `mu` held; nullptr if out of memory
+    if (bytes <= cap) return p;
+    drop();
+    const size_t want = bytes + bytes / 8 + (1u << 20);
+    if (cudaHostAlloc((void **)&p, want, cudaHostAllocDefault) == cudaSuccess) {
+      pinned = true;
+    } else {
+      (void)cudaGetLastError();
+      p = (unsigned char *)std::malloc(want);
+      pinned = false;
+    }
+    cap = p ? want : 0;
+    return p;
+  }
+  void drop() {
+    if (p) {
+      if (pinned) cudaFreeHost(p); else std::free(p);
+    }
+    p = nullptr;
+    cap = 0;
   }
 };
+StagingArea &staging_area();
 
 }  // namespace phs
 

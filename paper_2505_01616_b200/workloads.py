@@ -82,6 +82,7 @@ class Workload:
     desc: dict
     base_seed: int
     instances: List[Instance]
+    uniform_ops: bool = False   # every instance has the same collectives (kind, ranks, after); only sizes / starts differ
 
     @property
     def batch(self):
@@ -140,7 +141,7 @@ def cfg1(batch=64, n_hosts=16, gph=8, n_leaves=4, n_spines=2):
             sz = 1 * GiB if i == 0 else float(_loguniform(rng, 1 * MiB, 4 * GiB))
             ops.append(Coll(ALLREDUCE_RING, np.arange(j, n_hosts * gph, gph, dtype=np.int32), sz))
         insts.append(Instance(seed=i, ops=ops))
-    return Workload("cfg1", d, 0, insts)
+    return Workload("cfg1", d, 0, insts, uniform_ops=True)
 
 
 # ---------------------------------------------------------------------------------------------- cfg2
@@ -190,7 +191,7 @@ def cfg3(batch=4096, n_hosts=8, gph=8, n_leaves=2, n_spines=2, layers=4, buckets
                 ops.append(Coll(ALLREDUCE_RING, np.arange(j, G, gph, dtype=np.int32),
                                 float(_loguniform(rng, 1 * MiB, 1 * GiB)), 0.0, after))
         insts.append(Instance(seed=i, ops=ops, cap_pairs_Gbps=caps))
-    return Workload("cfg3", d, 0, insts)
+    return Workload("cfg3", d, 0, insts, uniform_ops=True)
 
 
 # ---------------------------------------------------------------------------------------------- cfg4

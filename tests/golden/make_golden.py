@@ -30,8 +30,12 @@ def make(name):
     b = o.bottlenecks()
     rng = np.random.default_rng(12345)
     idx = np.sort(rng.choice(len(t), size=4096, replace=False))
+    wk = o.work_counters()   # per-event work summed over the run (the roofline's algorithmic bytes)
+    secs = time.time() - t0
     np.savez_compressed(os.path.join(HERE, f"{name}_inst0.npz"), idx=idx, t_done=t[idx], bneck=b[idx],
-                        n_events=np.int64(len(o.event_log())), sha_t=np.array(hashlib.sha256(t.tobytes()).hexdigest()))
+                        n_events=np.int64(len(o.event_log())), sha_t=np.array(hashlib.sha256(t.tobytes()).hexdigest()),
+                        work_keys=np.array(sorted(wk)), work_vals=np.array([wk[k] for k in sorted(wk)], np.float64),
+                        oracle_seconds=np.float64(secs), n_flows=np.int64(len(t)))
     print(name, "flows", len(t), "events", len(o.event_log()), "oracle seconds", round(time.time() - t0, 1))
 
 
