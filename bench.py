@@ -128,6 +128,28 @@ def oracle_time(w, indices, mode=1):
     return secs, flows, colls, work
 
 
+def oracle_prefix_time(w, workload):
+    """cfg2 / cfg4 (one instance takes the oracle minutes): instance 0 run up to the simulated time by which a
+    fraction q of its flows is done (orc_run_until; the time comes from the stored oracle output under
+    tests/golden/, q chosen for 10-20 s of CPU work).  Returns (seconds in the run, flow-events processed, events,
+    sample description, the golden file's contents)."""
+    from oracle import orc
+    from util import oracle_build
+    g = np.load(os.path.join(ROOT, "tests", "golden", f"{workload}_inst0.npz"))
+    q = {"cfg2": 0.10, "cfg4": 0.025}[workload]
+    t_stop = float(np.quantile(g["t_done"], q))
+    osim = oracle_build(w.desc, w.instances[0], base_seed=w.base_seed)
+    t0 = time.perf_counter()
+    osim.run(mode=orc.MODE_FAST, until=t_stop)
+    secs = time.perf_counter() - t0
+    elog = osim.event_log()
+    fe = int(elog["n_completed"].sum()) + int(elog["n_activated"].sum())
+    osim.close()
+    sample = (f"instance 0 of {workload} up to simulated time {t_stop:.6g} s ({100 * q:g} % of its flows done: "
+              f"{len(elog)} events, {fe} flow-events), oracle fast mode, 1 thread")
+    return secs, fe, len(elog), sample, g
+
+
 def algorithmic_bytes(work):
     """Algorithmic bytes of a run, summed over its events:
         Bytes_e = A(36 + 20h) + 12 Lambda_act + 40 c
@@ -147,11 +169,15 @@ def run_reference(args, rank, world):
     w, per_rank = make_workload(args.workload, 1)
     # bounded sample: a few instances per step so the whole run stays within minutes
     per_step = {"cfg0": 1, "cfg1": 4, "cfg2": 1, "cfg3": 8, "cfg4": 1}[args.workload]
-    if args.workload in ("cfg2", "cfg4"):
-        raise SystemExit("reference arm: cfg2/cfg4 take minutes per instance on the CPU oracle; use cfg0/cfg1/cfg3")
     nxt = 0
+    prefix = args.workload in ("cfg2", "cfg4")
+    sample_txt = [f"{per_step} instances of {args.workload} per step (oracle fast mode, time inside orc_run only)"]
     def step():
         nonlocal nxt
+        if prefix:   # minutes per instance: each step is the same time prefix of instance 0
+            secs, fe, _ne, smp, _g = oracle_prefix_time(w, args.workload)
+            sample_txt[0] = smp + ", every step"
+            return secs, fe / 2.0, 0, None
         idx = [(nxt + k) % w.batch for k in range(per_step)]
         nxt = (nxt + per_step) % w.batch
         return oracle_time(w, idx)
@@ -162,7 +188,7 @@ def run_reference(args, rank, world):
         s, f, c, _w = step()
         secs += s; flows += f; colls += c
     val = 2.0 * flows / secs
-    sample = f"{per_step} instances of {args.workload} per step (oracle fast mode, time inside orc_run only)"
+    sample = sample_txt[0]
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -284,7 +310,9 @@ def run_ours(args, rank, world, local_rank):
     }
     # ---- CPU baseline (oracle, bounded sample) and roofline, rank 0 at N=1 only
     if world == 1 and not args.no_cpu_baseline:
-        n_cpu = {"cfg0": 1, "cfg1": 64, "cfg2": 0, "cfg3": 96, "cfg4": 0}[args.workload]
+        n_cpu = {"cfg0": 1, "cfg1": 64, "cfg2": 0, "cfg3": 96, "cfg4": 0}.get(args.workload, 0)
+        golden = os.path.join(ROOT, "tests", "golden", f"{args.workload}_inst0.npz")
+        wk = None
         if n_cpu:
             idx = list(range(min(n_cpu, w.batch)))
             secs, f_cpu, c_cpu, wk = oracle_time(w, idx)
@@ -293,6 +321,22 @@ def run_ours(args, rank, world, local_rank):
                                    "sample": sample, "seconds": secs, "host_cores": os.cpu_count()}
             # algorithmic bytes of ONE step = the oracle's per-event work counts, scaled to the whole batch
             scale = flows / float(f_cpu)
+            counted = "counted by the oracle on the cpu_baseline sample and scaled by flows"
+        elif os.path.exists(golden):
+            # cfg2 / cfg4: timed sample = a time prefix of instance 0 (oracle_prefix_time); the work counters of the
+            # FULL oracle run are stored beside the golden values by tests/golden/make_golden.py
+            secs, fe, _ne, sample, g = oracle_prefix_time(w, args.workload)
+            out["cpu_baseline"] = {"value": fe / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                                   "seconds": secs, "host_cores": os.cpu_count(),
+                                   "stored_full_run": {"seconds": float(g["oracle_seconds"]), "flows": int(g["n_flows"]),
+                                                       "events": int(g["n_events"]),
+                                                       "note": "whole instance 0, timed where make_golden.py ran "
+                                                               "(another machine): context only"}}
+            wk = dict(zip(g["work_keys"].tolist(), g["work_vals"].tolist()))
+            scale = flows / float(g["n_flows"])
+            counted = ("counted by the oracle over the whole of instance 0 (stored by tests/golden/make_golden.py) "
+                       "and scaled by flows")
+        if wk is not None:
             alg, survey = algorithmic_bytes(wk)
             peaks = {}
             try:
@@ -317,7 +361,7 @@ def run_ours(args, rank, world, local_rank):
                                "kernel_ms": kern_ms / args.steps,
                                "algorithmic_bytes_per_step": alg * scale,
                                "formula": "sum over events of A(36+20h) + 12*Lambda_act + 40c (DESIGN.md sec 5), "
-                                          "counted by the oracle on the cpu_baseline sample and scaled by flows",
+                                          + counted,
                                "survey_formula": {"bytes_per_step": survey * scale,
                                                   "achieved": survey * scale / k_s / 1e9,
                                                   "note": "SURVEY.md 8(d): link term charged once per sequential "

@@ -72,6 +72,43 @@ def test_after_and_alltoall_dag_equal_the_oracle():
     _compare_tables(W.Workload("mixed", d, 5, [W.Instance(seed=0, ops=ops), W.Instance(seed=1, ops=ops)]))
 
 
+def test_deferred_expansion_keeps_submission_order():
+    """phs_add_collective records the collective and its flows are expanded later (by the next raw-flow submission,
+    a table getter, or phs_finalize).  Flow ids must still follow submission order, and reading tables between
+    submissions must not change what is finally built."""
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 4, n_leaves=2, n_spines=2, uplinks_per_leaf_spine=2)
+    ring = np.array([1, 6, 11, 12, 3], np.int32)
+
+    def submit(h, peek):
+        a = B.phs_add_collective(h, 0, B.ALLREDUCE_RING, ring, 5e6, 1e-5)
+        assert a == 0 and B.phs_num_flows(h, 0) == 2 * 4 * 5          # counted before it is expanded
+        if peek:
+            off, _links = B.phs_get_paths(h, 0)
+            assert len(off) == 41
+        first = B.phs_add_flows(h, 0, [0, 2], [9, 13], [1e5, 2e5], dep_off=[0, 1, 3], dep_ids=[39, 0, 38])
+        assert first == 40                                            # raw flows come after the ring's 40 flows
+        b = B.phs_add_collective(h, 0, B.ALLTOALL, [0, 5, 10, 15], 3e6, 0.0, after=[0])
+        if peek:
+            B.phs_get_preds(h, 0)
+        c = B.phs_add_collective(h, 0, B.ALLGATHER_RING, [15, 5, 0], 2e6, 0.0, after=[b])
+        assert (b, c) == (1, 2) and B.phs_num_flows(h, 0) == 40 + 2 + 12 + 6
+        return B.phs_get_paths(h, 0), B.phs_get_preds(h, 0), B.phs_get_flow_table(h, 0)
+
+    h1, h2 = B.phs_create_topology(d, 3, 1), B.phs_create_topology(d, 3, 1)
+    t1, t2 = submit(h1, peek=True), submit(h2, peek=False)
+    for x, y in zip(t1, t2):
+        for u, v in zip(x, y):
+            assert np.array_equal(u, v)
+    # ring step s > 0 repeats the path of step 0 (ECMP keys on pair + collective)
+    off, links = t1[0]
+    for s_ in range(1, 8):
+        for i in range(5):
+            f0, f = i, s_ * 5 + i
+            assert np.array_equal(links[off[f]:off[f + 1]], links[off[f0]:off[f0 + 1]])
+    B.phs_destroy(h1)
+    B.phs_destroy(h2)
+
+
 def test_input_validation_and_state_errors():
     d = W.topo_desc(W.TOPO_SINGLE, 2, 8)
     h = B.phs_create_topology(d, 0, 2)
