@@ -717,6 +717,8 @@ cudaError_t launch_nt(const DevTables &t, const int32_t *order, int n, int *tick
 cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
                             cudaStream_t stream) {
   switch (c.threads) {
+    case 32:
+      return launch_nt<32>(t, order, n, ticket, c, stream);
     case 64:
       return launch_nt<64>(t, order, n, ticket, c, stream);
     case 128:

@@ -403,7 +403,13 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       maxF = std::max<int64_t>(maxF, sim->units[u].n_flows);
     }
     // about one slot per thread: measured on B200, 128 threads for cfg3-sized units, 256 for cfg1-sized ones
-    const int threads = (need <= 128 && Lm <= 320) ? 128 : 256;
+    // about one slot per thread makes one unit's event shortest (cfg1, bound by its 64 longest units: 256 threads
+    // 10.8 ms, 128 threads 12.5 ms, 64 threads 15.9 ms).  With many times more units than can be resident the SMs'
+    // issue slots are the limit, not the length of one event, and half as many threads waste fewer of them (cfg3,
+    // 36,864 units: 128 threads 57 ms, 64 threads 47 ms, 32 threads 58 ms).  Measured on B200.
+    int threads = (need <= 128 && Lm <= 320) ? 128 : 256;
+    if ((int64_t)cand.size() >= 64LL * sim->sm_count) threads /= 2;
+    if (const char *ev = getenv("PHS_CTA_THREADS")) threads = atoi(ev);  // tuning experiments: 32, 64, 128, 256, 512
     const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
     // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
     // predecessor counters on chip; returns 0 if not even one fits
@@ -455,6 +461,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta.smem + 1024)), 2048 / threads));
     sim->cta.grid = std::min((int)cand.size(), per * sim->sm_count);
     PHS_CUDA(sim->d_order.upload(sim->order, st));
+    if (timing_)
+      fprintf(stderr, "[phs_finalize] cta path: %d units, threads %d, need %d, links %d, slots %d, smem %zu, grid %d (%d per SM)\n",
+              (int)cand.size(), threads, need, Lm, sim->cta.slots, sim->cta.smem, sim->cta.grid, per);
     break;
   }
   std::sort(sim->cluster_list.begin(), sim->cluster_list.end());

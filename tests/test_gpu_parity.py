@@ -68,6 +68,31 @@ def test_cfg1_instances_cta():
     run_and_compare(W.cfg1(batch=4), path=0, expect_path="cta")
 
 
+def _full_batch_sampled(w, sample):
+    """The whole batch in the launch configuration bench.py times (no log, decomposed); sampled instances against
+    the oracle element by element, every instance's flow-event count through the counters."""
+    sim = B.Sim.from_workload(w)
+    sim.run()
+    for i in sample:
+        o = oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST, base_seed=w.base_seed)
+        assert_instance_matches(sim, i, o, check_log=False)
+        assert sim.path_of(i) == "cta"
+    c = sim.counters()
+    assert c["n_flow_events"] == 2 * sim.total_flows
+    t = B.phs_get_all_completion_times(sim.h)
+    assert np.isfinite(t).all() and (t > 0).all()
+    sim.close()
+
+
+def test_cfg1_full_batch_as_benchmarked():
+    _full_batch_sampled(W.cfg1(), [0, 1, 17, 42, 63])
+
+
+def test_cfg3_full_batch_as_benchmarked():
+    # 4,096 instances = 36,864 units: the scheduler's many-units configuration (64 threads per CTA)
+    _full_batch_sampled(W.cfg3(), [0, 1, 777, 2048, 3333, 4095])
+
+
 def test_cfg1_instance_cluster():
     run_and_compare(W.cfg1(batch=2), path=CLUSTER, first=1, count=1, expect_path="cluster")
 
