@@ -267,8 +267,26 @@ namespace {
 template <typename T>
 phs_status fetch(const phs_sim *sim, const T *dev, int64_t first, int64_t count, T *out, int32_t out_is_device) {
   if (count == 0) return PHS_OK;
-  PHS_CUDA(cudaMemcpyAsync(out, dev + first, sizeof(T) * (size_t)count,
-                           out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, sim->last_stream));
+  const size_t bytes = sizeof(T) * (size_t)count;
+  if (!out_is_device && bytes >= (256u << 10)) {
+    // host output: through the page-locked staging area (phs_finalize sized it for the tables, so results fit),
+    // then into the caller's pageable buffer with host threads -- several times faster than a pageable D2H copy
+    StagingArea &stage = staging_area();
+    std::lock_guard<std::mutex> lock(stage.mu);
+    if (stage.pinned && stage.cap >= bytes) {
+      PHS_CUDA(cudaMemcpyAsync(stage.p, dev + first, bytes, cudaMemcpyDeviceToHost, sim->last_stream));
+      PHS_CUDA(cudaStreamSynchronize(sim->last_stream));
+      const size_t piece = 4u << 20;
+      const int n_pieces = (int)((bytes + piece - 1) / piece);
+      parallel_for(n_pieces, [&](int k) {
+        const size_t lo = (size_t)k * piece, len = std::min(piece, bytes - lo);
+        std::memcpy((unsigned char *)out + lo, stage.p + lo, len);
+      });
+      return PHS_OK;
+    }
+  }
+  PHS_CUDA(cudaMemcpyAsync(out, dev + first, bytes, out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                           sim->last_stream));
   if (!out_is_device) PHS_CUDA(cudaStreamSynchronize(sim->last_stream));
   return PHS_OK;
 }

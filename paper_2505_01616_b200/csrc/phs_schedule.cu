@@ -186,15 +186,26 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     // slots a unit can need: raw flows and all-to-alls may be in flight as a whole; a ring collective keeps at most
     // one flow per sender PENDING or ACTIVE, twice the ring size because a slot freed in a phase is reused only in a
     // later one; collectives chained with `after` follow each other per rank, so a chain counts once, with its
-    // largest member (a collective and its chain lie in one unit)
-    std::vector<int64_t> ubound((size_t)n_units, 0), uwhole((size_t)n_units, 0);
+    // largest member (a collective and its chain lie in one unit).  The CTA kernel hands a vacated slot straight to
+    // the first successor its flow releases, so there a ring of N needs at most N + N/2 slots: N live flows (one
+    // per sender) plus one fresh slot per completing flow that releases two successors, and those are at most
+    // every second flow of a step (each of the N successors is released once; a flow that releases none queues its
+    // slot for the next phase) -- `ubound_cta`.
+    std::vector<int64_t> ubound((size_t)n_units, 0), uwhole((size_t)n_units, 0), ubound_cta((size_t)n_units, 0);
     {
       for (int u = 0; u < n_units; ++u) ubound[u] = (int64_t)uflows[u].size();
       for (int u = 0; u < n_units; ++u) uwhole[u] = (int64_t)uflows[u].size();  // minus the ring collectives' flows, below
-      std::vector<int64_t> chain_max(in.colls.size(), 0);
+      for (int u = 0; u < n_units; ++u) ubound_cta[u] = (int64_t)uflows[u].size();
+      std::vector<int64_t> chain_max(in.colls.size(), 0), chain_max_cta(in.colls.size(), 0);
       for (size_t c = 0; c < in.colls.size(); ++c) {
         if (in.colls[c].n_flows == 0) continue;
         ubound[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
+        ubound_cta[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
+        const int64_t nr = in.colls[c].n_ranks;
+        const int64_t need_cta = in.colls[c].kind == PHS_ALLTOALL
+                                     ? in.colls[c].n_flows
+                                     : std::min<int64_t>(in.colls[c].n_flows, nr + (nr + 1) / 2);
+        chain_max_cta[in.colls[c].chain] = std::max(chain_max_cta[in.colls[c].chain], need_cta);
         const int64_t need = in.colls[c].kind == PHS_ALLTOALL
                                  ? in.colls[c].n_flows
                                  : std::min<int64_t>(in.colls[c].n_flows, 2 * (int64_t)in.colls[c].n_ranks);
@@ -204,12 +215,14 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         if (in.colls[c].n_flows > 0 && in.colls[c].kind != PHS_ALLTOALL)
           uwhole[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
         if (chain_max[c] > 0) ubound[unit_of[in.colls[c].first_flow]] += chain_max[c];
+        if (chain_max_cta[c] > 0) ubound_cta[unit_of[in.colls[c].first_flow]] += chain_max_cta[c];
       }
     }
     if (n_units == 0) {  // an instance without flows is one empty unit
       n_units = 1;
       uflows.resize(1);
       ubound.assign(1, 0);
+      ubound_cta.assign(1, 0);
       uwhole.assign(1, 0);
     }
     for (int u = 0; u < n_units; ++u) {
@@ -286,6 +299,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       un.n_flows = d.n_flows;
       un.n_links = d.n_links;
       un.bound = ubound[u];
+      un.bound_cta = ubound_cta[u];
       un.bound_whole = std::min(ubound[u], uwhole[u]);
       c.units.push_back(un);
     }
@@ -382,7 +396,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   sim->cluster_list.clear();
   sim->cta = CtaLaunch{};
   auto need_of = [&](const phs_sim::Unit &u) {
-    return (int)std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(u.n_flows, 1), std::max<int64_t>(u.bound, 32)), 1 << 16);
+    return (int)std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(u.n_flows, 1), std::max<int64_t>(u.bound_cta, 32)), 1 << 16);
   };
   std::vector<int32_t> cand;
   for (int u = 0; u < U; ++u) {

@@ -115,6 +115,7 @@ struct phs_sim {
   struct Unit {  // what one CTA / cluster simulates (see phs::InstDesc)
     int32_t inst, n_flows, n_links;
     int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (see phs_finalize)
+    int64_t bound_cta;  // the same for the CTA kernel, which reuses a vacated slot within the phase (rings: 1.5 N)
     int64_t bound_whole;  // the part of `bound` from raw flows and all-to-alls (may be in flight all at once)
   };
   std::vector<Unit> units;
