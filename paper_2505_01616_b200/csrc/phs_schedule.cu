@@ -7,6 +7,7 @@
 #include <cstring>
 #include <limits>
 #include <numeric>
+#include <type_traits>
 
 #include "phs_sim.h"
 #include <chrono>
@@ -359,25 +360,49 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   const int U = (int)sim->units.size();
   const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
 
-  PHS_CUDA(sim->d_desc.upload(sim->h_desc, st));
-  PHS_CUDA(sim->d_rec.upload(rec, (size_t)Ft, st));
-  if (pc8_ok) PHS_CUDA(sim->d_pc8.upload(pc8, st));
-  PHS_CUDA(sim->d_succ.upload(succ, st));
-  PHS_CUDA(sim->d_pc0.upload(pc0, (size_t)Ft, st));
-  PHS_CUDA(sim->d_fmap.upload(fmap, (size_t)Ft, st));
-  PHS_CUDA(sim->d_init_t.upload(init_t, st));
-  PHS_CUDA(sim->d_init_f.upload(init_f, st));
-  PHS_CUDA(sim->d_capq.upload(capq, st));
-  PHS_CUDA(sim->d_lcomp.upload(lcomp, st));
-  PHS_CUDA(sim->d_linkid.upload(linkid, st));
-  PHS_CUDA(sim->d_coll_first.upload(coll_first, st));
-  PHS_CUDA(sim->d_coll_n.upload(coll_n, st));
-  PHS_CUDA(sim->d_pred_cnt.alloc((size_t)Ft));
-  PHS_CUDA(sim->d_tdone.alloc((size_t)Ft));
-  PHS_CUDA(sim->d_bneck.alloc((size_t)Ft));
-  PHS_CUDA(sim->d_coll_t.alloc((size_t)sim->total_colls));
-  PHS_CUDA(sim->d_res.alloc((size_t)U));
-  PHS_CUDA(sim->d_ticket.alloc(1));
+  // one device allocation for all tables and result arrays (a cudaMalloc costs about 0.1 ms, and there are 19 of
+  // them): first pass sizes, second pass places the views and issues the copies
+  {
+    unsigned char *base = nullptr;
+    size_t cursor = 0;
+    cudaError_t err = cudaSuccess;
+    auto put = [&](auto &buf, const auto *h, size_t count) {
+      using T = typename std::remove_pointer<decltype(buf.p)>::type;
+      if (base) {
+        buf.view((T *)(base + cursor), count);
+        if (h && count && err == cudaSuccess)
+          err = cudaMemcpyAsync(buf.p, h, count * sizeof(T), cudaMemcpyHostToDevice, st);
+      }
+      cursor += (std::max<size_t>(count, 1) * sizeof(T) + 255) / 256 * 256;
+    };
+    auto put_all = [&] {
+      cursor = 0;
+      put(sim->d_desc, sim->h_desc.data(), sim->h_desc.size());
+      put(sim->d_rec, (const FlowRec *)rec, (size_t)Ft);
+      if (pc8_ok) put(sim->d_pc8, pc8.data(), pc8.size());
+      put(sim->d_succ, succ.data(), succ.size());
+      put(sim->d_pc0, (const int32_t *)pc0, (size_t)Ft);
+      put(sim->d_fmap, (const uint32_t *)fmap, (size_t)Ft);
+      put(sim->d_init_t, init_t.data(), init_t.size());
+      put(sim->d_init_f, init_f.data(), init_f.size());
+      put(sim->d_capq, capq.data(), capq.size());
+      put(sim->d_lcomp, lcomp.data(), lcomp.size());
+      put(sim->d_linkid, linkid.data(), linkid.size());
+      put(sim->d_coll_first, coll_first.data(), coll_first.size());
+      put(sim->d_coll_n, coll_n.data(), coll_n.size());
+      put(sim->d_pred_cnt, (const int32_t *)nullptr, (size_t)Ft);
+      put(sim->d_tdone, (const double *)nullptr, (size_t)Ft);
+      put(sim->d_bneck, (const int32_t *)nullptr, (size_t)Ft);
+      put(sim->d_coll_t, (const double *)nullptr, (size_t)sim->total_colls);
+      put(sim->d_res, (const InstResult *)nullptr, (size_t)U);
+      put(sim->d_ticket, (const int *)nullptr, 1);
+    };
+    put_all();
+    PHS_CUDA(sim->d_arena.alloc(cursor));
+    base = sim->d_arena.p;
+    put_all();
+    PHS_CUDA(err);
+  }
   if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)log_cursor));
   if (sim->hist_cap > 0) {
     PHS_CUDA(sim->d_hist.alloc((size_t)sim->hist_cap));

@@ -46,11 +46,19 @@ template <typename T>
 struct DevBuf {
   T *p = nullptr;
   size_t n = 0;
+  bool owned = true;  // false: a view into another allocation (phs_sim::d_arena)
   ~DevBuf() { release(); }
   void release() {
-    if (p) cudaFree(p);
+    if (p && owned) cudaFree(p);
     p = nullptr;
     n = 0;
+    owned = true;
+  }
+  void view(T *ptr, size_t count) {
+    release();
+    p = ptr;
+    n = count;
+    owned = false;
   }
   cudaError_t alloc(size_t count) {
     release();
@@ -143,6 +151,7 @@ struct phs_sim {
   int64_t total_flows = 0, total_colls = 0;
 
   // ---- device tables
+  phs::DevBuf<unsigned char> d_arena;  // one allocation for every table phs_finalize places (the buffers below are views)
   phs::DevBuf<phs::InstDesc> d_desc;
   phs::DevBuf<phs::FlowRec> d_rec;
   phs::DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
