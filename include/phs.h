@@ -101,6 +101,10 @@ phs_status phs_batch(const phs_sim *sim, int32_t *out);
 /* Overrides the capacities (byte/s, [n_links], S1 numbering) of one instance (-1: all). */
 phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double *cap_Bps);
 phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double *cap_Bps);
+/* The same for every instance at once (the parameter sweep of BASELINE.json configs[3]): cap_Bps is a host array
+ * [batch][n_links], row i for instance i; the library copies it.  PHS_EINVAL (nothing changed) if any entry is
+ * outside (0, 2^42) byte/s; PHS_ESTATE after phs_finalize. */
+phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap_Bps);
 
 /* Adds one collective over `ranks` (ring order) to `instance` (-1: every instance).  `after_coll_ids`
  * (nullable) chains it per rank behind earlier collectives of the same instance (S3).

@@ -39,6 +39,7 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
 
 # every symbol include/phs.h declares (tests check that the library exports all of them)
 SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
+           "phs_set_link_capacities_batch",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
            "phs_set_decomposition", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
@@ -108,6 +109,15 @@ def phs_set_link_capacities(h, instance, cap):
     if len(cap) != phs_num_links(h):
         raise ValueError("capacity array must have n_links entries")
     _chk(lib().phs_set_link_capacities(h, C.c_int32(instance), _p(cap)), "phs_set_link_capacities")
+
+
+def phs_set_link_capacities_batch(h, cap):
+    cap = _arr(cap, np.float64)
+    b = C.c_int32()
+    _chk(lib().phs_batch(h, C.byref(b)), "phs_batch")
+    if cap.shape != (b.value, phs_num_links(h)):
+        raise ValueError("capacity array must be [batch][n_links]")
+    _chk(lib().phs_set_link_capacities_batch(h, _p(cap)), "phs_set_link_capacities_batch")
 
 
 def phs_get_link_capacities(h, instance):
@@ -349,13 +359,17 @@ class Sim:
                   cta_slots=cta_slots, decompose=decompose, history=history)
         n_links = phs_num_links(sim.h)
         insts = w.instances[first:first + count]
-        for i, inst in enumerate(insts):
-            assert inst.seed == insts[0].seed + i, "instance seeds must be consecutive"
-            cap = inst.capacities(w.desc, n_links)
-            if cap is not None:
-                phs_set_link_capacities(sim.h, i, cap)
-        # identical op structure across instances -> batched submission; else per instance
+        assert all(inst.seed == insts[0].seed + i for i, inst in enumerate(insts)), "instance seeds must be consecutive"
         from . import workloads as W
+        caps = W.capacity_matrix(w.desc, insts, n_links)    # [count][n_links] if every instance overrides them
+        if caps is not None and count > 1:
+            phs_set_link_capacities_batch(sim.h, caps)
+        else:
+            for i, inst in enumerate(insts):
+                cap = inst.capacities(w.desc, n_links)
+                if cap is not None:
+                    phs_set_link_capacities(sim.h, i, cap)
+        # identical op structure across instances -> batched submission; else per instance
         same = getattr(w, "uniform_ops", False)      # the generator states it; otherwise compare
         if not same and count > 1:
             same = all(len(x.ops) == len(insts[0].ops) for x in insts) and all(

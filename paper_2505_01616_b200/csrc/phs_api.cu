@@ -84,6 +84,16 @@ phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double 
   return PHS_OK;
 }
 
+phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap) {
+  if (!sim || !cap) return fail(PHS_EINVAL, "null argument");
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  const size_t L = (size_t)sim->fab->n_links(), n = L * (size_t)sim->batch;
+  for (size_t k = 0; k < n; ++k)  // validate everything first so that a failure changes nothing
+    if (!(cap[k] > 0.0) || !(cap[k] < 0x1p42)) return fail(PHS_EINVAL, "capacity must be in (0, 2^42) byte/s");
+  for (int i = 0; i < sim->batch; ++i) sim->inst[i].cap.assign(cap + (size_t)i * L, cap + (size_t)(i + 1) * L);
+  return PHS_OK;
+}
+
 phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double *cap) {
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;

@@ -76,6 +76,21 @@ class Instance:
         return n if n else 1      # a raw-flow instance counts as one all-to-all-equivalent (cfg4)
 
 
+def capacity_matrix(desc, insts, n_links):
+    """Instance.capacities of every instance as one [len(insts)][n_links] array (same numbering convention), or None
+    unless all of them override the capacities."""
+    if not insts or any(x.cap_pairs_Gbps is None for x in insts):
+        return None
+    G = desc["n_hosts"] * desc["gpus_per_host"]
+    pairs = (n_links - 2 * G) // 2
+    p = np.stack([np.asarray(x.cap_pairs_Gbps, dtype=np.float64) for x in insts])
+    assert p.shape == (len(insts), pairs)
+    cap = np.full((len(insts), n_links), desc["nvlink_Bps"], dtype=np.float64)
+    cap[:, 2 * G::2] = gbps(p)
+    cap[:, 2 * G + 1::2] = gbps(p)
+    return cap
+
+
 @dataclass
 class Workload:
     name: str

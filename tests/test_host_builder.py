@@ -109,6 +109,28 @@ def test_deferred_expansion_keeps_submission_order():
     B.phs_destroy(h2)
 
 
+def test_batched_capacities_equal_per_instance_calls():
+    w = W.cfg3(batch=5)
+    h = B.phs_create_topology(w.desc, 0, 5)
+    L = B.phs_num_links(h)
+    m = W.capacity_matrix(w.desc, w.instances, L)
+    assert m.shape == (5, L)
+    for i, inst in enumerate(w.instances):
+        assert np.array_equal(m[i], inst.capacities(w.desc, L))     # the vectorised form of Instance.capacities
+    B.phs_set_link_capacities_batch(h, m)
+    for i in range(5):
+        assert np.array_equal(B.phs_get_link_capacities(h, i), m[i])
+    bad = m.copy()
+    bad[3, 7] = 0.0
+    with pytest.raises(B.PhsError) as e:
+        B.phs_set_link_capacities_batch(h, bad)
+    assert e.value.code == B.PHS_EINVAL
+    assert np.array_equal(B.phs_get_link_capacities(h, 0), m[0])    # a refused call changes nothing
+    with pytest.raises(ValueError):
+        B.phs_set_link_capacities_batch(h, m[:4])
+    B.phs_destroy(h)
+
+
 def test_input_validation_and_state_errors():
     d = W.topo_desc(W.TOPO_SINGLE, 2, 8)
     h = B.phs_create_topology(d, 0, 2)
