@@ -108,7 +108,9 @@ phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap_Bps);
 
 /* Adds one collective over `ranks` (ring order) to `instance` (-1: every instance).  `after_coll_ids`
  * (nullable) chains it per rank behind earlier collectives of the same instance (S3).
- * out_coll_id (nullable) receives the collective's id. */
+ * out_coll_id (nullable) receives the collective's id.  The call validates its arguments, copies them and assigns
+ * the flow ids at once (phs_num_flows counts them); the flows themselves -- routes and DAG edges, PAPER.md L98 / L104 --
+ * are materialised by the next phs_add_flows on that instance, a table getter or phs_finalize. */
 phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                               double bytes, double start_time_s, const int32_t *after_coll_ids, int32_t n_after,
                               int32_t *out_coll_id);
