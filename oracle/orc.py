@@ -15,6 +15,7 @@ OK, EINVAL, ENOMEM, ECYCLE, ESTATE, ERANGE = 0, -1, -2, -4, -5, -6
 TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE = 0, 1, 2
 ALLREDUCE_RING, ALLGATHER_RING, REDUCESCATTER_RING, ALLTOALL = 0, 1, 2, 3
 MODE_NAIVE, MODE_FAST = 0, 1
+FLAG_SETTLE_EVERY_EVENT, FLAG_F64_SHARES = 1, 2     # orc_run_ex: SURVEY.md 8(c) S4.4 / S5 as written (see orc_netsim.h)
 
 
 class TopologyDesc(C.Structure):
@@ -38,10 +39,13 @@ def lib():
         spec = importlib.util.spec_from_file_location("_orc_build", os.path.join(_HERE, "build_oracle.py"))
         mod = importlib.util.module_from_spec(spec)
         spec.loader.exec_module(mod)
-        _lib = C.CDLL(mod.build())
+        # ORC_LIB_PATH: a pre-built variant of the oracle (tests/test_oracle_mutants.py loads mutated copies through it)
+        _lib = C.CDLL(os.environ.get("ORC_LIB_PATH") or mod.build())
         _lib.orc_mix64.restype = C.c_uint64
         _lib.orc_mix64.argtypes = [C.c_uint64]
         _lib.orc_destroy.restype = None
+        _lib.orc_settle.restype = C.c_double
+        _lib.orc_settle.argtypes = [C.c_double, C.c_double, C.c_double]
     return _lib
 
 
@@ -62,6 +66,11 @@ def _chk(rc, what):
 
 def mix64(x: int) -> int:
     return int(lib().orc_mix64(C.c_uint64(x & 0xFFFFFFFFFFFFFFFF)))
+
+
+def settle(rem, rate_Bps, dt):
+    """S4.4 / Q11 settle step: max(rem - rate * dt, 0)."""
+    return float(lib().orc_settle(rem, rate_Bps, dt))
 
 
 def maxmin(cap, path_off, path, mode=MODE_NAIVE):
@@ -138,8 +147,11 @@ class Sim:
                                  _p(dep_ids, C.c_int64), _p(conn_id, C.c_int32), C.byref(first)), "orc_add_flows")
         return first.value
 
-    def run(self, mode=MODE_NAIVE, trace=False, until=None):
-        if until is None:
+    def run(self, mode=MODE_NAIVE, trace=False, until=None, flags=0):
+        if flags:
+            _chk(lib().orc_run_ex(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0),
+                                  C.c_double(float("inf") if until is None else until), C.c_int32(flags)), "orc_run_ex")
+        elif until is None:
             _chk(lib().orc_run(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0)), "orc_run")
         else:
             _chk(lib().orc_run_until(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0), C.c_double(until)),

@@ -540,6 +540,63 @@ static int solve_maxmin(ws_t *w, const int64_t *capq, int32_t nA, const int32_t 
   return 0;
 }
 
+/* SURVEY.md 8(c) S5 exactly as written there (binary64 shares), one bottleneck link per iteration, dense argmin.
+ * Kept beside the R-FX solver to measure how far the two readings are apart (tests: < 1e-9 relative on times). */
+static int solve_maxmin_f64(ws_t *w, const double *cap, int32_t nA, const int32_t *act, const int64_t *path_off,
+                            const int32_t *path, double *rate, int32_t *bneck, int32_t *n_rounds, int32_t *first_bneck,
+                            int32_t *lam_act) {
+  int32_t L = w->n_links;
+  *n_rounds = 0; *first_bneck = -1; *lam_act = 0;
+  if (nA == 0) return 0;
+  double *cap_rem = (double *)malloc(sizeof(double) * L);
+  if (!cap_rem) return -1;
+  for (int32_t l = 0; l < L; l++) { cap_rem[l] = cap[l]; w->n[l] = 0; }
+  if (nA > w->frozen_cap) {
+    void *q = realloc(w->frozen, nA);
+    if (!q) { free(cap_rem); return -1; }
+    w->frozen = (uint8_t *)q; w->frozen_cap = nA;
+  }
+  memset(w->frozen, 0, nA);
+  for (int32_t a = 0; a < nA; a++)
+    for (int64_t e = path_off[act[a]]; e < path_off[act[a] + 1]; e++) w->n[path[e]]++;
+  for (int32_t l = 0; l < L; l++) if (w->n[l] > 0) (*lam_act)++;
+  int32_t unfrozen = nA;
+  while (unfrozen > 0) {
+    int32_t b = -1;
+    double s = 0.0;
+    for (int32_t l = 0; l < L; l++) {
+      if (w->n[l] <= 0) continue;
+      double sh = cap_rem[l] / (double)w->n[l];
+      if (b < 0 || sh < s) { b = l; s = sh; }
+    }
+    if (*n_rounds == 0) *first_bneck = b;
+    int32_t nt = 0;
+    for (int32_t a = 0; a < nA; a++) { /* every unfrozen active flow crossing b */
+      if (w->frozen[a]) continue;
+      int on_b = 0;
+      for (int64_t pe = path_off[act[a]]; pe < path_off[act[a] + 1]; pe++) if (path[pe] == b) on_b = 1;
+      if (!on_b) continue;
+      w->frozen[a] = 1;
+      rate[act[a]] = s;
+      bneck[act[a]] = b;
+      unfrozen--;
+      for (int64_t pe = path_off[act[a]]; pe < path_off[act[a] + 1]; pe++) {
+        int32_t l = path[pe];
+        if (w->k[l]++ == 0) w->touched[nt++] = l;
+      }
+    }
+    for (int32_t t = 0; t < nt; t++) {
+      int32_t l = w->touched[t];
+      cap_rem[l] = cap_rem[l] - (double)w->k[l] * s;
+      w->n[l] -= w->k[l];
+      w->k[l] = 0;
+    }
+    (*n_rounds)++;
+  }
+  free(cap_rem);
+  return 0;
+}
+
 int32_t orc_maxmin(int32_t n_links, const double *cap, int32_t n_flows, const int64_t *path_off, const int32_t *path,
                    int32_t mode, double *rate, int32_t *bneck, int32_t *n_rounds, int32_t *first_bneck) {
   if (n_links <= 0 || n_flows < 0 || !cap || !path_off || !rate || !bneck) return ORC_EINVAL;
@@ -565,13 +622,33 @@ int32_t orc_maxmin(int32_t n_links, const double *cap, int32_t n_flows, const in
 }
 
 /* ------------------------------------------------------------------ S4: flow states & event loop */
-int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) { return orc_run_until(s, mode, trace, INFINITY); }
+/* S4.4 / Q11: remaining bytes after draining at `rate` for dt seconds: mul, then sub, then clamp at 0.  (Under
+ * R-LZ the clamp is a guard: DESIGN.md sec 2 argues that a flow still active at `now` < tc cannot have drained
+ * more than it holds; the function is exported so that the branch is pinned directly.) */
+static double settle(double rem, double rate, double dt) {
+  double m = rate * dt;
+  double r = rem - m;
+  return r > 0.0 ? r : 0.0;
+}
+double orc_settle(double rem, double rate_Bps, double dt) { return settle(rem, rate_Bps, dt); }
+
+int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace) { return orc_run_ex(s, mode, trace, INFINITY, 0); }
+int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
+  return orc_run_ex(s, mode, trace, t_stop, 0);
+}
 
 /* "advancing the simulation ... up to a specified time": the event loop stops before the first
  * event later than t_stop.  Flows that have not completed by then keep t_done = NaN and bneck = -1; the event
  * log and the throughput history hold what happened up to t_stop. */
-int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
+/* flags (the two readings DESIGN.md sec 2 CHANGED, kept so that the change can be measured against the tolerance
+ * BASELINE.json states, 1e-9 relative): ORC_FLAG_SETTLE_EVERY_EVENT = SURVEY.md 8(c) S4.4 as written (every ACTIVE
+ * flow is debited at every event: rem = max(rem - rate*dt, 0), tc = now + rem/rate) instead of R-LZ;
+ * ORC_FLAG_F64_SHARES = SURVEY.md 8(c) S5 as written (cap_rem and share are binary64: share = cap_rem / n,
+ * cap_rem -= k * share) instead of R-FX.  Neither is used by any parity test of the CUDA path. */
+int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32_t flags) {
   if (!s || (mode != ORC_MODE_NAIVE && mode != ORC_MODE_FAST)) return ORC_EINVAL;
+  if (flags & ~(ORC_FLAG_SETTLE_EVERY_EVENT | ORC_FLAG_F64_SHARES)) return ORC_EINVAL;
+  if ((flags & ORC_FLAG_F64_SHARES) && mode != ORC_MODE_NAIVE) return ORC_EINVAL; /* dense argmin only */
   if (s->ran) return ORC_ESTATE;
   int64_t F = s->F;
   int32_t L = s->n_links, rc = ORC_OK;
@@ -588,12 +665,14 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
   int64_t *rq = (int64_t *)malloc(sizeof(int64_t) * (F + 1));
   int64_t *rq_cur = (int64_t *)malloc(sizeof(int64_t) * (F + 1)); /* rate in effect since t_last (R-LZ) */
   double *t_last = (double *)malloc(sizeof(double) * (F + 1));    /* time rem[] refers to (R-LZ)         */
+  double *rate_d = (double *)malloc(sizeof(double) * (F + 1));     /* ORC_FLAG_F64_SHARES: binary64 rates       */
+  double *rate_cur = (double *)malloc(sizeof(double) * (F + 1));   /* rate in effect since t_last, byte/s       */
   int32_t *act = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *pend = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *comp = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   s->t_done = (double *)malloc(sizeof(double) * (F + 1));
   s->bneck = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
-  if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !rq_cur || !t_last || !act || !pend || !comp ||
+  if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !rq_cur || !t_last || !rate_d || !rate_cur || !act || !pend || !comp ||
       !s->t_done || !s->bneck || ws_init(&w, L)) {
     rc = ORC_ENOMEM;
     goto out;
@@ -643,7 +722,12 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
     nP = np2;
     /* 2. rates over all ACTIVE flows, from scratch (S5) */
     int32_t R = 0, fb = -1, lam = 0;
-    if (solve_maxmin(&w, capq, nA, act, s->path_off, s->path, mode, rq, s->bneck, &R, &fb, &lam)) {
+    if (flags & ORC_FLAG_F64_SHARES) {
+      if (solve_maxmin_f64(&w, s->cap, nA, act, s->path_off, s->path, rate_d, s->bneck, &R, &fb, &lam)) {
+        rc = ORC_ENOMEM;
+        goto out;
+      }
+    } else if (solve_maxmin(&w, capq, nA, act, s->path_off, s->path, mode, rq, s->bneck, &R, &fb, &lam)) {
       rc = ORC_ENOMEM;
       goto out;
     }
@@ -657,8 +741,10 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
     double ah = 0;
     for (int32_t i = 0; i < nA; i++) {
       int32_t f = act[i];
-      if (rq[f] != rq_cur[f]) {
-        if (s->n_h == s->h_cap) { /* history: the flow's throughput changes to rq[f] at `now` */
+      double new_rate = (flags & ORC_FLAG_F64_SHARES) ? rate_d[f] : q_to_rate(rq[f]);
+      int changed = (flags & ORC_FLAG_F64_SHARES) ? (rq_cur[f] < 0 || new_rate != rate_cur[f]) : (rq[f] != rq_cur[f]);
+      if (changed) {
+        if (s->n_h == s->h_cap) { /* history: the flow's throughput changes to new_rate at `now` */
           int64_t c = s->h_cap ? 2 * s->h_cap : 4096;
           void *a = realloc(s->h_flow, sizeof(int32_t) * c), *b, *d;
           if (!a) { rc = ORC_ENOMEM; goto out; }
@@ -671,15 +757,14 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
           s->h_rate = (double *)d;
           s->h_cap = c;
         }
-        s->h_flow[s->n_h] = f; s->h_t[s->n_h] = now; s->h_rate[s->n_h] = q_to_rate(rq[f]); s->n_h++;
-        if (rq_cur[f] >= 0) {
-          double m = q_to_rate(rq_cur[f]) * (now - t_last[f]);
-          double r = rem[f] - m;
-          rem[f] = r > 0.0 ? r : 0.0;
-        }
+        s->h_flow[s->n_h] = f; s->h_t[s->n_h] = now; s->h_rate[s->n_h] = new_rate; s->n_h++;
+      }
+      if (changed || ((flags & ORC_FLAG_SETTLE_EVERY_EVENT) && rq_cur[f] >= 0)) {
+        if (rq_cur[f] >= 0) rem[f] = settle(rem[f], rate_cur[f], now - t_last[f]);
         t_last[f] = now;
-        rq_cur[f] = rq[f];
-        double q = rem[f] / q_to_rate(rq[f]);
+        rq_cur[f] = (flags & ORC_FLAG_F64_SHARES) ? 0 : rq[f];
+        rate_cur[f] = new_rate;
+        double q = rem[f] / new_rate;
         tc[f] = now + q;
       }
       if (tc[f] < t_next) t_next = tc[f];
@@ -700,7 +785,7 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
           s->tr = (trace_row *)q; s->tr_cap = c;
         }
         trace_row *r = &s->tr[s->n_tr++];
-        r->ev = s->n_ev; r->flow = f; r->rate = q_to_rate(rq[f]); r->t0 = now; r->t1 = t_next;
+        r->ev = s->n_ev; r->flow = f; r->rate = rate_cur[f]; r->t0 = now; r->t1 = t_next;
       }
       if (tc[f] == t_next) { /* bit-equal absolute time: completes */
         s->t_done[f] = t_next;
@@ -744,7 +829,7 @@ int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop) {
   s->ran = 1;
 out:
   free(capq); free(succ_off); free(succ); free(pred_cnt); free(state); free(t_act); free(rem); free(tc); free(rq); free(rq_cur); free(t_last);
-  free(act); free(pend); free(comp);
+  free(rate_d); free(rate_cur); free(act); free(pend); free(comp);
   ws_free(&w);
   return rc;
 }

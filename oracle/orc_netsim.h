@@ -49,6 +49,9 @@ enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ECYCLE = -4, ORC_ESTATE
 enum { ORC_TOPO_SINGLE = 0, ORC_TOPO_LEAF_SPINE = 1, ORC_TOPO_FAT_TREE = 2 };
 enum { ORC_ALLREDUCE_RING = 0, ORC_ALLGATHER_RING = 1, ORC_REDUCESCATTER_RING = 2, ORC_ALLTOALL = 3 };
 enum { ORC_MODE_NAIVE = 0, ORC_MODE_FAST = 1 };
+/* orc_run_ex flags: the two readings of SURVEY.md 8(c) that DESIGN.md sec 2 replaced, kept for comparison */
+enum { ORC_FLAG_SETTLE_EVERY_EVENT = 1, /* S4.4 as written: every ACTIVE flow is debited at every event (not R-LZ) */
+       ORC_FLAG_F64_SHARES = 2 };       /* S5 as written: binary64 cap_rem / share (not R-FX); naive mode only      */
 
 typedef struct {
   int32_t kind, n_hosts, gpus_per_host;
@@ -81,6 +84,10 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace);
 /* same, but stops before the first event later than t_stop ("advancing the simulation ... up to a
  * specified time"); unfinished flows keep t_done = NaN and bneck = -1 */
 int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop);
+/* the same with `flags` (see above); flags = 0 is orc_run_until */
+int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32_t flags);
+/* S4.4 / Q11 settle step on its own: max(rem - rate * dt, 0) with mul, sub, clamp in that order */
+double orc_settle(double rem, double rate_Bps, double dt);
 int32_t orc_num_flows(const orc_sim *s, int64_t *out);
 int32_t orc_get_completion_times(const orc_sim *s, double *out, int64_t n);
 int32_t orc_get_bottlenecks(const orc_sim *s, int32_t *out, int64_t n);

@@ -2,6 +2,19 @@
 
 None of these re-types the oracle's own formula: each expected value is a closed form, an iff-certificate,
 a brute-force enumeration, a published test vector, or an invariance.
+
+Mutants these pins are required to kill (tests/test_oracle_mutants.py applies each to a scratch copy of
+oracle/orc_netsim.c and demands that at least one test of this file fails):
+  M1  a released flow ignores its own start time            (st = now)                  -> test_p1_dependent_flow_...
+  M2  the Q11 clamp removed from the settle step                                          -> test_q11_settle_clamp...
+  M3  work counter sum_Lam doubled                                                        -> test_work_counters_...
+  M4  leaf-spine down lane taken from the LOW hash bits instead of H >> 32                -> test_routing_leaf_spine_down_lane...
+  M5  the FIFO predecessor (s-1, i) dropped                                               -> test_ring_dag_structure
+  M6  `after` edge "received by rho" dropped                                              -> test_after_chains_...
+  M7  argmin tie-break to the HIGHEST link id                                             -> test_p1 / test_p3
+  M8  latency not added on release                                                        -> test_input_validation / P2
+  M9  ring-after-all-to-all: edges to rho dropped                                         -> test_mixed_kind_after_edges_...
+  M10 work counter sum_R counts events instead of iterations                              -> test_work_counters_...
 """
 import itertools
 import os
@@ -93,6 +106,104 @@ def test_p1_lone_flow_start_time_and_fabric_bottleneck():
     s = run_flows(d, [0], [15], [1e6])
     assert s.paths()[0][1] == 6
     assert s.completion_times()[0] == pytest.approx(6e-6 + 1e6 / 25e9, rel=1e-12)
+
+
+def test_p1_dependent_flow_waits_for_its_own_start_time():
+    """SURVEY.md 8(c) S4 step 5 / PAPER.md L104 ("flows ... with the appropriate timestamps"): a released flow becomes
+    active at max(start, t_pred) + Lat.  Closed form for a two-flow chain on link-disjoint pairs:
+    t1 = max(start1, t0) + Lat + bytes1 / B, for start1 later than, equal to and earlier than t0."""
+    d = single()
+    B, Lat = 450e9, 2e-6
+    t0 = Lat + 4e6 / B
+    for start1 in (5 * t0, t0, 0.25 * t0, 0.0):
+        s = run_flows(d, [0, 2], [1, 3], [4e6, 9e6], start=np.array([0.0, start1]),
+                      dep_off=np.array([0, 0, 1]), dep_ids=np.array([0]))
+        t = s.completion_times()
+        assert t[0] == pytest.approx(t0, rel=1e-12)
+        assert t[1] == pytest.approx(max(start1, t0) + Lat + 9e6 / B, rel=1e-12)
+    # the same through a collective: step-0 flows of a ring chained `after` another one, with a later start time
+    s = orc.Sim(single(n_hosts=1, gph=8), 0)
+    a = s.add_collective(orc.ALLGATHER_RING, np.arange(4, dtype=np.int32), 4e6)
+    T = 3 * (Lat + 1e6 / B)
+    s.add_collective(orc.ALLGATHER_RING, np.arange(4, dtype=np.int32), 4e6, start=10 * T, after=[a])
+    s.run()
+    assert list(s.collective_times()) == pytest.approx([T, 10 * T + T], rel=1e-12)
+
+
+def test_q11_settle_clamp_and_time_never_runs_backwards():
+    """rem = max(rem - rate*dt, 0).  The step is pinned on its own (mul, sub, clamp), and
+    through the property it protects: the clock of a run never goes backwards and no completion precedes its
+    activation, on a workload full of near-simultaneous completions."""
+    assert orc.settle(10.0, 2.0, 3.0) == 4.0
+    assert orc.settle(1.0, 1e9, 1.0) == 0.0                      # drained more than it holds: clamped, not negative
+    assert orc.settle(5e-324, 1.0, 1.0) == 0.0
+    assert orc.settle(3.0, 0.5, 0.0) == 3.0
+    d = single(lat=0.0, nic_Bps=1e9)
+    rng = np.random.default_rng(11)
+    base = np.floor(rng.uniform(1e5, 1e6, 40))
+    sizes = np.concatenate([base, np.nextafter(base, np.inf), base + 2.0 ** -20])    # clusters of almost-equal sizes
+    s = run_flows(d, list(rng.integers(0, 8, len(sizes))), [8 + i % 4 for i in range(len(sizes))], sizes)
+    ev = s.event_log()
+    assert np.all(np.diff(ev["t"]) >= 0)
+    assert np.all(s.completion_times() > 0) and not np.isnan(s.completion_times()).any()
+
+
+def test_work_counters_against_hand_counts():
+    """orc_get_work_counters feeds the roofline's algorithmic bytes, so it is pinned against counts
+    made by hand.  P6 (three flows, one shared link, zero latency): iteration 1 has A=3 on 4 links, one filling
+    iteration; then A=2 on 3 links, A=1 on 2 links."""
+    d = single(lat=0.0, nic_Bps=1e9)
+    s = run_flows(d, [0, 1, 2], [8, 8, 8], [1e6, 2e6, 4e6])
+    wk = s.work_counters()
+    assert wk == {"sum_A": 6.0, "sum_Ah": 12.0, "sum_R": 3.0, "sum_LamR": 9.0, "sum_Lam": 9.0, "completions": 3.0,
+                  "events": 3.0}
+    # P7-like: A on two links, B, C on one each: 2 filling iterations on 5 links (3 NIC-up + 2 NIC-down)
+    d = single(lat=0.0, nic_Bps=1e9)
+    s = run_flows(d, [0, 1, 2], [8, 8, 9], [1e6, 1e6, 1e6])      # flows 0,1 share NIC-down(8); flow 2 alone
+    wk = s.work_counters()
+    # iteration 1: A=3, links {up0, up1, up2, dn8, dn9} = 5; bottleneck dn8 (0.5e9 each), then flow 2 (tie up2 / dn9): 2
+    # flow 2 finishes at 1 ms, flows 0,1 at 2 ms: iteration 2: A=2, links 3, one filling iteration
+    assert wk["sum_A"] == 5 and wk["sum_Ah"] == 10 and wk["sum_R"] == 3 and wk["sum_Lam"] == 8
+    assert wk["sum_LamR"] == 5 * 2 + 3 * 1 and wk["completions"] == 3 and wk["events"] == 2
+    # cfg0: no link is shared, so per event Lambda_act = 2A (two links per flow) and every flow is its own filling
+    # iteration (R = A); the max-plus recurrence (P3) gives every activation and completion time, hence the events
+    w = W.cfg0()
+    o = oracle_run(w.desc, w.instances[0])
+    T = maxplus_ring(np.arange(16), 30, 64 * MiB / 16, lambda i: 50e9 if i in (7, 15) else 450e9, 2e-6)
+    dur = np.array([(64 * MiB / 16) / (50e9 if i in (7, 15) else 450e9) for i in range(16)])
+    act = T - dur[None, :]                       # a flow is ACTIVE from T - chunk/B to T
+    times = np.sort(np.concatenate([act.ravel(), T.ravel()]))
+    events = [times[0]]
+    for x in times[1:]:                          # distinct times (the recurrence is exact up to rounding)
+        if x - events[-1] > 1e-12 * x:
+            events.append(x)
+    events = np.array(events)
+    # flow f is counted in every iteration whose interval (e_{k-1}, e_k] lies inside (act_f, T_f]
+    spans = np.searchsorted(events, T.ravel() * (1 + 1e-12)) - np.searchsorted(events, act.ravel() * (1 + 1e-12))
+    wk = o.work_counters()
+    assert wk["events"] == len(events) and wk["completions"] == 480
+    assert wk["sum_A"] == spans.sum() and wk["sum_Ah"] == 2 * spans.sum() and wk["sum_Lam"] == 2 * spans.sum()
+    assert wk["sum_R"] == spans.sum()
+    # per-event A from the same intervals -> sum of A * 2A
+    A_e = np.array([np.sum((act.ravel() < e * (1 - 1e-12)) & (T.ravel() >= e * (1 - 1e-12))) for e in events])
+    assert wk["sum_LamR"] == np.sum(2 * A_e * A_e)
+
+
+def test_comparison_modes_agree_within_the_stated_tolerance():
+    """DESIGN.md sec 2 replaces two readings of SURVEY.md 8(c): R-LZ (settle a flow only when its rate changes) for
+    S4.4 (debit every active flow at every event), and R-FX (integer rate quanta) for binary64 shares.  BASELINE.json
+    states 1e-9 relative on completion times: the oracle keeps both original readings as modes (orc_run_ex flags) and
+    they must agree with the default within that tolerance on the shrunken configs."""
+    for w in (W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2), W.cfg2(k=4, agg_uplinks=1), W.cfg3(batch=2),
+              W.cfg4(batch=1, n_hosts=8, gph=4, n_leaves=4, n_spines=2)):
+        inst = w.instances[-1]
+        ref = oracle_run(w.desc, inst).completion_times()
+        for flags in (orc.FLAG_SETTLE_EVERY_EVENT, orc.FLAG_F64_SHARES, orc.FLAG_SETTLE_EVERY_EVENT | orc.FLAG_F64_SHARES):
+            from util import oracle_build
+            o = oracle_build(w.desc, inst)
+            o.run(flags=flags)
+            np.testing.assert_allclose(o.completion_times(), ref, rtol=1e-9, atol=0)
+            assert not np.array_equal(o.completion_times(), ref) or flags == orc.FLAG_F64_SHARES   # the modes are live
 
 
 # ------------------------------------------------------------------------------------------------ P2 uniform ring
@@ -400,7 +511,66 @@ def test_alltoall_after_alltoall_preds():
         assert sorted(pr[off[f]:off[f + 1]].tolist()) == want
 
 
+def test_mixed_kind_after_edges_against_hand_written_lists():
+    """S3 `after` between different collective kinds, against lists written out by hand (N = 3)."""
+    d = single(n_hosts=1, gph=8)
+    # all-to-all over [0,1,2]: flows 0:0->1 1:0->2 2:1->0 3:1->2 4:2->0 5:2->1 ; then a ring all-gather over [2,0,1]
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLTOALL, np.array([0, 1, 2], np.int32), 3e6)
+    s.add_collective(orc.ALLGATHER_RING, np.array([2, 0, 1], np.int32), 3e6, after=[a])
+    off, pr = s.preds()
+    want = {6: [1, 3, 4, 5],      # sender 2: everything from / to rank 2
+            7: [0, 1, 2, 4],      # sender 0
+            8: [0, 2, 3, 5]}      # sender 1
+    for f, p in want.items():
+        assert sorted(pr[off[f]:off[f + 1]].tolist()) == p
+    assert sorted(pr[off[9]:off[10]].tolist()) == [6, 8] and sorted(pr[off[10]:off[11]].tolist()) == [6, 7]
+    # ring all-reduce over [1,2,3] (4 steps x 3; last step = flows 9,10,11: 1->2, 2->3, 3->1); then an all-to-all
+    # over [0,1,2]: rank 0 is not in the ring (no edge), rank 1 sent 9 and received 11, rank 2 sent 10 and received 9
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLREDUCE_RING, np.array([1, 2, 3], np.int32), 3e6)
+    s.add_collective(orc.ALLTOALL, np.array([0, 1, 2], np.int32), 3e6, after=[a])
+    off, pr = s.preds()
+    want = {12: [], 13: [], 14: [9, 11], 15: [9, 11], 16: [9, 10], 17: [9, 10]}
+    for f, p in want.items():
+        assert sorted(pr[off[f]:off[f + 1]].tolist()) == p
+
+
 # ------------------------------------------------------------------------------------------------ S2 routing pins
+def test_routing_leaf_spine_down_lane_comes_from_the_high_hash_word():
+    """S2: with P parallel uplinks per (leaf, spine) the up lane is (H mod (n_spines P)) mod P and the down lane
+    (H >> 32) mod P, H = mix(mix(mix(mix(seed) ^ src) ^ dst) ^ conn) with the published SplitMix64 step -- re-derived
+    here in Python integers from the published constants, not from the oracle."""
+    M = (1 << 64) - 1
+
+    def mix(x):
+        z = (x + 0x9E3779B97F4A7C15) & M
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & M
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & M
+        return z ^ (z >> 31)
+
+    assert mix(0) == 0xE220A8397B1DCDAF            # the published first output, so this restatement is pinned too
+    P, nsp, G, seed = 4, 2, 32, 21
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 8, 4, n_leaves=4, n_spines=nsp, uplinks_per_leaf_spine=P)
+    rng = np.random.default_rng(2)
+    src = rng.integers(0, G, 600).astype(np.int32)
+    dst = ((src + rng.integers(1, G, 600)) % G).astype(np.int32)
+    conn = rng.integers(0, 1000, 600).astype(np.int32)
+    s = orc.Sim(d, seed)
+    s.add_flows(src, dst, np.ones(600), conn_id=conn)
+    off, links = s.paths()
+    n_cross = 0
+    for f in range(600):
+        if src[f] // 8 == dst[f] // 8:             # same leaf (2 hosts x 4 GPUs per leaf)
+            continue
+        H = mix(mix(mix(mix(seed) ^ int(src[f])) ^ int(dst[f])) ^ int(conn[f]))
+        c = H % (nsp * P)
+        up = 4 * G + 2 * (((src[f] // 8) * nsp + c // P) * P + c % P)
+        dn = 4 * G + 2 * (((dst[f] // 8) * nsp + c // P) * P + (H >> 32) % P) + 1
+        assert list(links[off[f]:off[f + 1]]) == [2 * G + 2 * src[f], up, dn, 2 * G + 2 * dst[f] + 1]
+        n_cross += 1
+    assert n_cross > 300
+
 def test_routing_structure_leaf_spine_and_balance():
     d = W.topo_desc(W.TOPO_LEAF_SPINE, 8, 4, n_leaves=4, n_spines=4, uplinks_per_leaf_spine=2)
     G, P, nsp = 32, 2, 4
