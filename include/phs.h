@@ -159,7 +159,9 @@ phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *o
  * instance set is frozen (adds return PHS_ESTATE).  phs_run calls it implicitly if needed. */
 phs_status phs_finalize(phs_sim *sim, void *cuda_stream);
 /* Runs every instance to completion on the GPU (all steps of the hot path in CUDA kernels) and waits for the
- * result status.  May be called repeatedly; each call restarts from t = 0. */
+ * result status.  May be called repeatedly: after a complete run it starts again from t = 0; after a phs_run_until
+ * that stopped early it continues from the parked state.  After an error return the handle holds no results (getters
+ * return PHS_ESTATE) and the next run starts from t = 0. */
 phs_status phs_run(phs_sim *sim, void *cuda_stream);
 /* PAPER.md L167 "advancing the simulation ... up to a specified time": like phs_run, but stops before the first
  * event later than t_stop_s.  Flows that complete later report completion time NaN and bottleneck -1, a collective

@@ -25,35 +25,40 @@ extern "C" {
 const char *phs_last_error(void) { return g_err.c_str(); }
 
 phs_status phs_create_topology(const phs_topology_desc *desc, uint64_t seed, int32_t batch, phs_sim **out) {
+  PHS_API_BEGIN
   if (!desc || !out) return fail(PHS_EINVAL, "null argument");
   if (batch <= 0) return fail(PHS_EINVAL, "batch must be positive");
   std::string why;
   phs_status st = Fabric::validate(*desc, &why);
   if (st != PHS_OK) return fail(st, why);
-  phs_sim *s = new (std::nothrow) phs_sim();
-  if (!s) return fail(PHS_ENOMEM, "out of host memory");
+  std::unique_ptr<phs_sim> s(new phs_sim());  // bad_alloc -> PHS_ENOMEM (PHS_API_END)
   s->desc = *desc;
   s->seed = seed;
   s->batch = batch;
   s->fab.reset(new Fabric(*desc));
   s->inst.resize((size_t)batch);
   for (int32_t i = 0; i < batch; ++i) s->inst[i].seed = seed + (uint64_t)i;
-  *out = s;
+  *out = s.release();
   return PHS_OK;
+  PHS_API_END
 }
 
 void phs_destroy(phs_sim *sim) { delete sim; }
 
 phs_status phs_num_links(const phs_sim *sim, int32_t *out) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   *out = sim->fab->n_links();
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_batch(const phs_sim *sim, int32_t *out) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   *out = sim->batch;
   return PHS_OK;
+  PHS_API_END
 }
 
 // The instance with every submitted collective expanded into flows.  Expansion is deferred bookkeeping, not a change
@@ -72,6 +77,7 @@ static phs_status check_instance(const phs_sim *sim, int32_t instance, bool allo
 }
 
 phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double *cap) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
   if (!cap) return fail(PHS_EINVAL, "null capacities");
@@ -82,9 +88,11 @@ phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double 
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   for (int i = lo; i < hi; ++i) sim->inst[i].cap.assign(cap, cap + L);
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap) {
+  PHS_API_BEGIN
   if (!sim || !cap) return fail(PHS_EINVAL, "null argument");
   if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
   const size_t L = (size_t)sim->fab->n_links(), n = L * (size_t)sim->batch;
@@ -92,9 +100,11 @@ phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap) {
     if (!(cap[k] > 0.0) || !(cap[k] < 0x1p42)) return fail(PHS_EINVAL, "capacity must be in (0, 2^42) byte/s");
   for (int i = 0; i < sim->batch; ++i) sim->inst[i].cap.assign(cap + (size_t)i * L, cap + (size_t)(i + 1) * L);
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double *cap) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!cap) return fail(PHS_EINVAL, "null output");
@@ -102,10 +112,12 @@ phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double 
   const Instance &in = sim->inst[instance];
   for (int l = 0; l < L; ++l) cap[l] = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                               double bytes, double start, const int32_t *after, int32_t n_after, int32_t *out_id) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
   if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
@@ -121,11 +133,13 @@ phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, cons
   }
   if (out_id) *out_id = (int32_t)sim->inst[lo].colls.size() - 1;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                                     const double *bytes, const double *start, const int32_t *after, int32_t n_after,
                                     int32_t *out_id) {
+  PHS_API_BEGIN
   if (!sim || !bytes) return fail(PHS_EINVAL, "null argument");
   if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
   for (int i = 1; i < sim->batch; ++i)
@@ -145,11 +159,13 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
   }
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_t *src, const int32_t *dst,
                          const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
                          const int32_t *conn_id, int64_t *out_first) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
   if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
@@ -166,72 +182,90 @@ phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_
   }
   if (out_first) *out_first = first;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_enable_event_log(phs_sim *sim, int32_t enable) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return fail(PHS_ESTATE, "event log must be chosen before phs_finalize");
   sim->want_log = enable != 0;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (path < 0 || path > 2 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
   if (sim->finalized) return fail(PHS_ESTATE, "scheduler policy must be chosen before phs_finalize");
   sim->policy_path = path;
   sim->policy_slots = cta_slots;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_enable_history(phs_sim *sim, int64_t max_records) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (max_records < 0) return fail(PHS_EINVAL, "max_records must be >= 0");
   if (sim->finalized) return fail(PHS_ESTATE, "history must be chosen before phs_finalize");
   sim->hist_cap = max_records;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_set_decomposition(phs_sim *sim, int32_t enable) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return fail(PHS_ESTATE, "decomposition must be chosen before phs_finalize");
   sim->decompose = enable != 0;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!out) return fail(PHS_EINVAL, "null output");
   *out = sim->inst[instance].n_flows();
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_total_flows(const phs_sim *sim, int64_t *out) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   int64_t t = 0;
   for (const Instance &in : sim->inst) t += in.n_flows();
   *out = t;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_num_collectives(const phs_sim *sim, int32_t instance, int32_t *out) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!out) return fail(PHS_EINVAL, "null output");
   *out = (int32_t)sim->inst[instance].colls.size();
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_num_path_entries(const phs_sim *sim, int32_t instance, int64_t *out) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!out) return fail(PHS_EINVAL, "null output");
   *out = (int64_t)expanded(sim, instance).path.size();
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *links, int64_t cap) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   const Instance &in = expanded(sim, instance);
@@ -239,10 +273,12 @@ phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int
   for (size_t f = 0; f < in.path_off.size(); ++f) off[f] = in.path_off[f];
   std::copy(in.path.begin(), in.path.end(), links);
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *preds, int64_t cap,
                          int64_t *n_entries) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   const Instance &in = expanded(sim, instance);
@@ -255,10 +291,12 @@ phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int
     std::copy(in.pred.begin(), in.pred.end(), preds);
   }
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,
                               double *lat, int64_t n) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   const Instance &in = expanded(sim, instance);
@@ -268,6 +306,7 @@ phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src
   if (bytes) std::copy(in.bytes.begin(), in.bytes.end(), bytes);
   if (lat) std::copy(in.lat.begin(), in.lat.end(), lat);
   return PHS_OK;
+  PHS_API_END
 }
 
 }  // extern "C"
@@ -305,44 +344,55 @@ phs_status fetch(const phs_sim *sim, const T *dev, int64_t first, int64_t count,
 extern "C" {
 
 phs_status phs_get_completion_times(const phs_sim *sim, int32_t instance, double *out, int64_t n, int32_t dev) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (!out || n != sim->inst[instance].n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
   return fetch(sim, sim->d_tdone.p, sim->flow_base[instance], n, out, dev);
+  PHS_API_END
 }
 
 phs_status phs_get_bottlenecks(const phs_sim *sim, int32_t instance, int32_t *out, int64_t n, int32_t dev) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (!out || n != sim->inst[instance].n_flows()) return fail(PHS_EINVAL, "n must equal the instance's flow count");
   return fetch(sim, sim->d_bneck.p, sim->flow_base[instance], n, out, dev);
+  PHS_API_END
 }
 
 phs_status phs_get_all_completion_times(const phs_sim *sim, double *out, int64_t n, int32_t dev) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
   return fetch(sim, sim->d_tdone.p, 0, n, out, dev);
+  PHS_API_END
 }
 
 phs_status phs_get_all_bottlenecks(const phs_sim *sim, int32_t *out, int64_t n, int32_t dev) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
   return fetch(sim, sim->d_bneck.p, 0, n, out, dev);
+  PHS_API_END
 }
 
 phs_status phs_get_collective_times(const phs_sim *sim, int32_t instance, double *out, int32_t n) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (!out || n != (int32_t)sim->inst[instance].colls.size()) return fail(PHS_EINVAL, "n must equal the collective count");
   return fetch(sim, sim->d_coll_t.p, sim->coll_base[instance], (int64_t)n, out, 0);
+  PHS_API_END
 }
 
 phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *out, int64_t cap, int64_t *n_events) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -352,10 +402,12 @@ phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *ou
   if (!out) return PHS_OK;
   return fetch(sim, sim->d_log.p, sim->h_desc[sim->unit_first[instance]].log_base, std::min<int64_t>(cap, *n_events),
                out, 0);
+  PHS_API_END
 }
 
 phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *off, double *t, double *rate,
                                 int64_t cap, int64_t *n_records) {
+  PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -379,9 +431,11 @@ phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *o
   }
   off[hi - lo] = k;
   return PHS_OK;
+  PHS_API_END
 }
 
 phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
+  PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   phs_counters c{};
@@ -401,6 +455,7 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   c.main_kernel_ms = sim->main_kernel_ms;
   *out = c;
   return PHS_OK;
+  PHS_API_END
 }
 
 const char *phs_instance_path(const phs_sim *sim, int32_t instance) {

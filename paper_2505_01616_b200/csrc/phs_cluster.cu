@@ -329,6 +329,11 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       first_bneck = pr->first_bneck;
     }
 
+    // this CTA's slot high-water mark and free-queue tail as the next phase X must see them: read where a barrier
+    // protects the read (here and after the X barrier of every event), never at the top of phase X, where warps
+    // that are already inside the phase bump both words
+    int hi_carry = min(ctl[M_HI], Sc), qtail_carry = ctl[M_QTAIL];
+
     for (;;) {
       if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
         status = kPaused;
@@ -336,8 +341,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       }
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
       ++solve;
-      const int hi0 = min(ctl[M_HI], Sc);
-      const int qtail = ctl[M_QTAIL];
+      const int hi0 = hi_carry;
+      const int qtail = qtail_carry;
       auto touch_link = [&](int l, int delta) {  // the link's flow count changes: its share0 is stale for this solve
         LinkA *a = LA(l);
         atomicAdd(&a->n0, delta);
@@ -501,7 +506,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         break;
       }
       if (nA == 0 && nPend == 0) break;
-      const int hi = min(ctl[M_HI], Sc);
+      const int hi = hi_carry = min(ctl[M_HI], Sc);
+      qtail_carry = ctl[M_QTAIL];
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 

@@ -280,6 +280,12 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
 #define PHS_TICK(i)
 #endif
 
+    // Snapshot of the slot high-water mark and of the free queue's tail as phase X of the next event must see them.
+    // Taken where a barrier protects it (here, and right after the X barrier of every event): nothing changes the two
+    // words between an X barrier and the next phase X, while a read at the top of phase X would race with the atomics
+    // of warps that are already inside it.
+    int hi_carry = min(S.ctl[C_HI], SC), qtail_carry = S.ctl[C_QTAIL];
+
     for (;;) {
       if (t_next > T.t_stop) {  // phs_run_until: the next event lies beyond the requested time
         status = kPaused;
@@ -287,8 +293,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       }
       // ======== phase X (a8 + a4): retire what completes at t_next, release successors, activate what is due
       ++solve;
-      const int hi0 = min(S.ctl[C_HI], SC);
-      const int qtail = S.ctl[C_QTAIL];
+      const int hi0 = hi_carry;
+      const int qtail = qtail_carry;
 
       auto activate = [&](int slot) {  // PENDING -> ACTIVE: the flow now counts on its links
         const uint4 pv = S.s_path[slot];
@@ -421,7 +427,8 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       const int nA = S.ctl[C_NACTIVE];
       const int nPend = S.ctl[C_NPEND];
       if (nA == 0 && nPend == 0) break;  // S4.3: nothing active, nothing pending -> stop
-      const int hi = min(S.ctl[C_HI], SC);
+      const int hi = hi_carry = min(S.ctl[C_HI], SC);
+      qtail_carry = S.ctl[C_QTAIL];
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 

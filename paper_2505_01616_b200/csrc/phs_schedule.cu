@@ -32,6 +32,7 @@ StagingArea &staging_area() {
 // the capacity row in rate quanta, the link components and the link ids of the topology, the sorted list of
 // initial activations, and the dynamic per-flow arrays (pred_cnt, t_done, bneck).
 extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return PHS_OK;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -448,7 +449,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     // 36,864 units: 128 threads 57 ms, 64 threads 47 ms, 32 threads 58 ms).  Measured on B200.
     int threads = (need <= 128 && Lm <= 320) ? 128 : 256;
     if ((int64_t)cand.size() >= 64LL * sim->sm_count) threads /= 2;
-    if (const char *ev = getenv("PHS_CTA_THREADS")) threads = atoi(ev);  // tuning experiments: 32, 64, 128, 256, 512
+    if (const char *ev = getenv("PHS_CTA_THREADS")) {  // tuning experiments; anything but a supported size is ignored
+      const int v = atoi(ev);
+      if (v == 32 || v == 64 || v == 128 || v == 256 || v == 512) threads = v;
+    }
     const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
     // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
     // predecessor counters on chip; returns 0 if not even one fits
@@ -517,6 +521,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_CUDA(cudaEventCreate(&sim->ev1));
   sim->finalized = true;
   return PHS_OK;
+  PHS_API_END
 }
 
 // ================================================================================================ run
@@ -664,10 +669,13 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
 }  // namespace
 
 extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
+  PHS_API_BEGIN
   return phs_run_until(sim, std::numeric_limits<double>::infinity(), cuda_stream);
+  PHS_API_END
 }
 
 extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream) {
+  PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (!(t_stop_s >= 0.0)) return fail(PHS_EINVAL, "t_stop_s must be >= 0");
   sim->t_stop = t_stop_s;
@@ -684,6 +692,11 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   // launch configuration after an overflow) the simulation starts again from t = 0 -- it is deterministic, so the
   // results are the same.
   const bool resume = sim->have_park && sim->ran && sim->t_stop >= sim->parked_until;
+  // Until this call succeeds the handle has no results and no parked state: an error return below (history overflow,
+  // a unit that does not fit, a CUDA failure) leaves units parked at the NEW stop time, which a later call with an
+  // earlier time must not resume from.  Both flags are set again at the end.
+  sim->have_park = false;
+  sim->ran = false;
   if (finite && !sim->order.empty() && sim->park_stride == 0) {
     sim->park_stride = (sizeof(ParkRegs) + sim->cta.smem + 255) / 256 * 256;
     PHS_CUDA(sim->d_park.alloc(sim->park_stride * (size_t)U));
@@ -792,5 +805,6 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
                                  std::to_string(sim->h_res[u].status));
   }
   return PHS_OK;
+  PHS_API_END
 }
 

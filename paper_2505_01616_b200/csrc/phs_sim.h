@@ -10,6 +10,9 @@
 #include <string>
 #include <thread>
 #include <mutex>
+#include <exception>
+#include <new>
+#include <stdexcept>
 #include <vector>
 
 #include "phs_device.h"
@@ -23,6 +26,22 @@ phs_status phs_fail(phs_status code, const std::string &msg);
     if (e_ != cudaSuccess) return phs_fail(PHS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_)); \
   } while (0)
 
+// Every extern "C" entry point that returns a status runs between these two: no exception crosses the C-ABI
+// (include/phs.h "never throw").  Host allocations (std::vector growth in the submission calls and phs_finalize) are
+// the realistic source: they become PHS_ENOMEM.
+#define PHS_API_BEGIN try {
+#define PHS_API_END                                                       \
+  }                                                                       \
+  catch (const std::bad_alloc &) {                                        \
+    return phs_fail(PHS_ENOMEM, "out of host memory");                    \
+  }                                                                       \
+  catch (const std::exception &e_) {                                      \
+    return phs_fail(PHS_EINVAL, std::string("unexpected exception: ") + e_.what()); \
+  }                                                                       \
+  catch (...) {                                                           \
+    return phs_fail(PHS_EINVAL, "unexpected exception");                  \
+  }
+
 namespace phs {
 
 // fn(i) for every i in [0, n) on up to `max_threads` (<= 16) host threads; the iterations must be independent
@@ -34,12 +53,21 @@ void parallel_for(int n, F fn, int max_threads = 16) {
     return;
   }
   std::atomic<int> next{0};
+  std::exception_ptr err;  // an exception in a worker (std::bad_alloc) is rethrown in the caller, not std::terminate
+  std::mutex err_mu;
   std::vector<std::thread> pool;
   for (int t = 0; t < nt; ++t)
     pool.emplace_back([&] {
-      for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+      try {
+        for (int i = next.fetch_add(1); i < n; i = next.fetch_add(1)) fn(i);
+      } catch (...) {
+        std::lock_guard<std::mutex> g(err_mu);
+        if (!err) err = std::current_exception();
+        next.store(n);
+      }
     });
   for (std::thread &th : pool) th.join();
+  if (err) std::rethrow_exception(err);
 }
 
 template <typename T>

@@ -186,30 +186,62 @@ def test_device_output_pointer():
 
 def _golden(name):
     z = np.load(os.path.join(GOLD, name))
-    return z["idx"], z["t_done"], z["bneck"], int(z["n_events"]), z["sha_t"].item()
+    return z
 
 
-@pytest.mark.parametrize("name,make,inst", [
-    ("cfg4_inst0", lambda: W.cfg4(batch=1), 0),
-    ("cfg2_inst0", lambda: W.cfg2(), 0),
-])
-def test_full_size_against_stored_oracle_samples(name, make, inst):
-    """BASELINE.json's full sizes, in the launch configuration bench.py uses.  The expected values were written
-    by tests/golden/make_golden.py, which calls only oracle/ (fast mode)."""
+def _check_against_golden(sim, inst, z):
     import hashlib
-    path = os.path.join(GOLD, name + ".npz")
-    if not os.path.exists(path):
-        pytest.skip("golden file not generated")
-    idx, t_ref, b_ref, n_events, sha = _golden(name + ".npz")
-    w = make()
+    t, b = sim.completion_times(inst), sim.bottlenecks(inst)
+    assert np.array_equal(t[z["idx"]], z["t_done"])
+    assert np.array_equal(b[z["idx"]], z["bneck"])
+    assert hashlib.sha256(t.tobytes()).hexdigest() == z["sha_t"].item()
+    assert hashlib.sha256(b.tobytes()).hexdigest() == z["sha_bneck"].item()
+
+
+def _check_log_against_golden(sim, inst, z):
+    import hashlib
+    ev = sim.event_log(inst)
+    assert len(ev) == int(z["n_events"])
+    assert hashlib.sha256(np.ascontiguousarray(ev["t"]).tobytes()).hexdigest() == z["sha_event_t"].item()
+
+
+def test_cfg4_full_size_whole_batch_as_benchmarked():
+    """BASELINE.json configs[4] at full size, all 8 instances in the launch bench.py times (W.cfg4(), no log,
+    scheduler on automatic), every instance against the stored oracle output (4096 sampled flows, SHA-256 of all
+    completion times and of all bottleneck ids).  The expected values were written by tests/golden/make_golden.py,
+    which calls only oracle/ (fast mode).  Then the same batch with the event log on: event count and SHA-256 of the
+    log's time column per instance."""
+    w = W.cfg4()
+    assert w.batch == 8
+    zs = [_golden(f"cfg4_inst{i}.npz") for i in range(w.batch)]
     sim = B.Sim.from_workload(w)
     sim.run()
-    t = sim.completion_times(inst)
-    assert np.array_equal(t[idx], t_ref)
-    assert np.array_equal(sim.bottlenecks(inst)[idx], b_ref)
-    assert hashlib.sha256(t.tobytes()).hexdigest() == sha
+    for i in range(w.batch):
+        _check_against_golden(sim, i, zs[i])
+    c = sim.counters()
+    assert c["n_events"] == sum(int(z["n_events"]) for z in zs)       # one unit per instance: same event sequence
+    if c["cluster_size"] > 0 and sim.path_of(0) == "cluster":
+        # more units than resident clusters: some cluster simulated two units back to back (ticket, re-init, scratch reuse)
+        print("cfg4 launch: cluster size", c["cluster_size"], "resident", c["clusters_resident"])
+    sim.close()
+    sim = B.Sim.from_workload(w, event_log=True)
+    sim.run()
+    for i in range(w.batch):
+        _check_against_golden(sim, i, zs[i])
+        _check_log_against_golden(sim, i, zs[i])
+    sim.close()
+
+
+def test_cfg2_full_size_as_benchmarked():
+    """BASELINE.json configs[2] at full size (1,069,056 flows in one instance) in the launch configuration bench.py
+    uses, against the stored oracle output."""
+    z = _golden("cfg2_inst0.npz")
+    w = W.cfg2()
+    sim = B.Sim.from_workload(w)
+    sim.run()
+    _check_against_golden(sim, 0, z)
     # independent units count their own events, so simultaneous events of different units count more than once
-    assert sim.counters()["n_events"] >= n_events
+    assert sim.counters()["n_events"] >= int(z["n_events"])
     sim.close()
 
 
