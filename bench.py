@@ -218,7 +218,7 @@ def run_ours(args, rank, world, local_rank):
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
     # ---- device-resident arm: tables built and uploaded once, each step = phs_run
-    sim = B.Sim.from_workload(w, instances=(first, count), path=args.path)
+    sim = B.Sim.from_workload(w, instances=(first, count), path=args.path, cta_slots=args.gang, windows=not args.no_windows)
     sim.finalize(stream=sp)
     flows = sim.total_flows
     colls = sum(w.instances[i].n_collectives for i in mine)
@@ -260,7 +260,8 @@ def run_ours(args, rank, world, local_rank):
     # ---- end-to-end arm: host arrays -> C-ABI submission -> table build -> H2D -> run -> D2H, every step
     def e2e_step():
         t0 = time.perf_counter()
-        s2 = B.Sim.from_workload(w, instances=(first, count), path=args.path)
+        s2 = B.Sim.from_workload(w, instances=(first, count), path=args.path, cta_slots=args.gang,
+                                 windows=not args.no_windows)
         s2.run(stream=sp)
         out = B.phs_get_all_completion_times(s2.h)
         dt = time.perf_counter() - t0
@@ -298,9 +299,12 @@ def run_ours(args, rank, world, local_rank):
         "dtype": "f64+i64", "data": "synthetic",
         "config": {"workload": args.workload, "instances_per_gpu": count, "flows_per_gpu": flows,
                    "kernel_paths": paths, "l2": "flushed between timed steps (256 MiB write)",
-                   "events_per_step": counters["n_events"], "parallel_rounds_per_step": counters["sum_par_rounds"],
+                   "iterations_per_step": counters["n_events"], "windows_per_step": counters["n_windows"],
+                   "lookahead_windows": not args.no_windows,
+                   "parallel_rounds_per_step": counters["sum_par_rounds"],
                    "max_active_flows": counters["max_active"], "max_state_slots": counters["max_slots"],
-                   "cluster_size": counters["cluster_size"], "clusters_resident": counters["clusters_resident"]},
+                   "cluster_size": counters["cluster_size"], "clusters_resident": counters["clusters_resident"],
+                   "window_gang": counters["window_gang"]},
         "collectives_per_sec": colls_all * args.steps / (ms_total * 1e-3),
         "sim_events_per_sec": counters["n_events"] * world * args.steps / (ms_total * 1e-3),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -382,8 +386,12 @@ def main():
     ap.add_argument("--workload", default="cfg1")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--path", type=int, default=0, help="scheduler policy: 0 auto, 1 CTA path, 2 cluster path")
+    ap.add_argument("--path", type=int, default=0,
+                    help="scheduler policy: 0 auto, 1 CTA path, 2 cluster path, 3 window path")
+    ap.add_argument("--gang", type=int, default=0, help="with --path 3: smallest gang (CTAs per unit) of the window path")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end arm (profiling runs)")
+    ap.add_argument("--no-windows", action="store_true",
+                    help="one global event per kernel loop iteration instead of the lookahead-window schedule")
     ap.add_argument("--instances", type=int, default=0,
                     help="instances per GPU (default: the config's own batch); smaller batches are for profiling")
     args = ap.parse_args()

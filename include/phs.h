@@ -86,9 +86,12 @@ typedef struct {
   int32_t cluster_size;  /* CTAs per cluster of the cluster path in the last run (0: path not used)            */
   int32_t clusters_resident; /* clusters of that size the device keeps resident at once                        */
   int32_t resumed_units; /* units the last phs_run_until continued from their parked state (0: started at t = 0) */
-  int32_t pad_;
+  int32_t window_gang;   /* CTAs per unit of the window path in the last run (largest gang; 0: path not used)     */
   double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
                          /* the run's stream), excluding the result copies                                */
+  int64_t n_windows;     /* lookahead windows executed (phs_set_windows); = n_events where the window schedule  */
+                         /* is off.  n_events then counts window ITERATIONS: one iteration advances every       */
+                         /* component that has an event inside the window by one event                          */
 } phs_counters;
 
 /* Creates `batch` independent instances of one topology.  Instance i routes with ECMP seed `seed + i`.
@@ -128,11 +131,14 @@ phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_
 /* Event log on/off (default off) for subsequent runs; must precede phs_finalize. */
 phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);
 
-/* Batch-scheduler policy; must precede phs_finalize.  path: 0 = automatic (one CTA per
+/* Batch-scheduler policy; must precede phs_finalize.  path: 0 = automatic (units whose events
+ * are dense in simulated time run the lookahead-window schedule on a gang of CTAs; of the others, one CTA per
  * simulation unit with all state in its shared memory when it fits, else one thread-block cluster per unit with the
- * state spread over the shared memory of its CTAs), 1 = CTA path, 2 = cluster path for every unit.  cta_slots > 0
- * caps the CTA path's shared-memory slot count (flows PENDING or ACTIVE at once per unit); a unit that exceeds it
- * is re-run on the cluster path. */
+ * state spread over the shared memory of its CTAs), 1 = CTA path, 2 = cluster path for every unit, 3 = window path
+ * for every unit that can run there (positive latency, no event log, no history).  cta_slots > 0 caps the CTA
+ * path's shared-memory slot count (flows PENDING or ACTIVE at once per unit); a unit that exceeds it is re-run on
+ * the cluster path.  With path = 3, cta_slots is instead the smallest gang (CTAs per unit: 1, 2, 4, 8, 16) to use
+ * for units that have enough components. */
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
 
 /* Decomposition (default on).  An instance whose flows fall into groups that share no link and no dependency is
@@ -140,6 +146,14 @@ phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots);
  * bit-identical to simulating the instance as a whole.  Off: one unit per instance.  The event log needs the
  * instance-wide event sequence, so enabling it turns decomposition off.  Must precede phs_finalize. */
 phs_status phs_set_decomposition(phs_sim *sim, int32_t enable);
+
+/* Lookahead windows (default on).  A flow released by an event at time t starts no earlier than t + L, L = the
+ * smallest path latency of the unit's dependent flows, and static link components influence each other only through
+ * such releases; so the events of different components inside [T0, T0 + L) are independent and one loop iteration
+ * of the kernels advances all of them, each at its own time.  Results are bit-identical to the one-event-per-
+ * iteration schedule (reading R-LZ).  Units with zero latency, the event log or the throughput history
+ * always run one event per iteration.  Must precede phs_finalize. */
+phs_status phs_set_windows(phs_sim *sim, int32_t enable);
 
 /* Throughput history ("between neighboring events, network flows are assumed to have stable
  * throughput"; L167: a flow's history is a few floating point numbers per throughput change, from which a time
@@ -192,7 +206,7 @@ phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int
 phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,
                               double *latency_s, int64_t n);
 phs_status phs_get_counters(const phs_sim *sim, phs_counters *out);
-/* Name of the kernel path the last run used for `instance`: "cta" or "cluster". */
+/* Name of the kernel path the last run used for the largest unit of `instance`: "cta", "cluster" or "window". */
 const char *phs_instance_path(const phs_sim *sim, int32_t instance);
 const char *phs_last_error(void); /* thread-local; valid until the next call on this thread */
 

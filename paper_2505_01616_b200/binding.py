@@ -30,8 +30,8 @@ class Counters(C.Structure):
     _fields_ = [("n_events", C.c_int64), ("n_flow_events", C.c_int64), ("sum_active", C.c_int64),
                 ("sum_par_rounds", C.c_int64), ("n_kernel_launches", C.c_int64), ("h2d_bytes", C.c_int64),
                 ("max_active", C.c_int32), ("max_slots", C.c_int32), ("cluster_size", C.c_int32),
-                ("clusters_resident", C.c_int32), ("resumed_units", C.c_int32), ("pad_", C.c_int32),
-                ("main_kernel_ms", C.c_double)]
+                ("clusters_resident", C.c_int32), ("resumed_units", C.c_int32), ("window_gang", C.c_int32),
+                ("main_kernel_ms", C.c_double), ("n_windows", C.c_int64)]
 
 
 EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<i4"), ("n_rounds", "<i4"),
@@ -42,7 +42,7 @@ SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "
            "phs_set_link_capacities_batch",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
-           "phs_set_decomposition", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
+           "phs_set_decomposition", "phs_set_windows", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
            "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
@@ -194,6 +194,10 @@ def phs_set_decomposition(h, enable=True):
     _chk(lib().phs_set_decomposition(h, C.c_int32(1 if enable else 0)), "phs_set_decomposition")
 
 
+def phs_set_windows(h, enable=True):
+    _chk(lib().phs_set_windows(h, C.c_int32(1 if enable else 0)), "phs_set_windows")
+
+
 def phs_finalize(h, stream=None):
     _chk(lib().phs_finalize(h, C.c_void_p(stream or 0)), "phs_finalize")
 
@@ -327,7 +331,7 @@ class Sim:
     """Owns a phs_sim handle.  Methods forward to the C-named calls above."""
 
     def __init__(self, desc: dict, seed: int = 0, batch: int = 1, event_log: bool = False, path: int = 0,
-                 cta_slots: int = 0, decompose: bool = True, history: int = 0):
+                 cta_slots: int = 0, decompose: bool = True, history: int = 0, windows: bool = True):
         self.h = phs_create_topology(desc, seed, batch)
         self.batch = batch
         if event_log:
@@ -336,6 +340,8 @@ class Sim:
             phs_set_decomposition(self.h, False)
         if history:
             phs_enable_history(self.h, history)
+        if not windows:
+            phs_set_windows(self.h, False)
         if path or cta_slots:
             phs_set_scheduler(self.h, path, cta_slots)
 
@@ -351,12 +357,13 @@ class Sim:
             pass
 
     @classmethod
-    def from_workload(cls, w, event_log=False, instances=None, path=0, cta_slots=0, decompose=True, history=0):
+    def from_workload(cls, w, event_log=False, instances=None, path=0, cta_slots=0, decompose=True, history=0,
+                      windows=True):
         """Builds a batch from a workloads.Workload (optionally a subset of its instances; instance i keeps its own
         seed only if the subset is a contiguous range, so subsets are given as (first, count))."""
         first, count = (0, w.batch) if instances is None else instances
         sim = cls(w.desc, seed=w.base_seed + w.instances[first].seed, batch=count, event_log=event_log, path=path,
-                  cta_slots=cta_slots, decompose=decompose, history=history)
+                  cta_slots=cta_slots, decompose=decompose, history=history, windows=windows)
         n_links = phs_num_links(sim.h)
         insts = w.instances[first:first + count]
         assert all(inst.seed == insts[0].seed + i for i, inst in enumerate(insts)), "instance seeds must be consecutive"

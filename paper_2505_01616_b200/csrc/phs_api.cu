@@ -197,7 +197,7 @@ phs_status phs_enable_event_log(phs_sim *sim, int32_t enable) {
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
   PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
-  if (path < 0 || path > 2 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
+  if (path < 0 || path > 3 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
   if (sim->finalized) return fail(PHS_ESTATE, "scheduler policy must be chosen before phs_finalize");
   sim->policy_path = path;
   sim->policy_slots = cta_slots;
@@ -220,6 +220,15 @@ phs_status phs_set_decomposition(phs_sim *sim, int32_t enable) {
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return fail(PHS_ESTATE, "decomposition must be chosen before phs_finalize");
   sim->decompose = enable != 0;
+  return PHS_OK;
+  PHS_API_END
+}
+
+phs_status phs_set_windows(phs_sim *sim, int32_t enable) {
+  PHS_API_BEGIN
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (sim->finalized) return fail(PHS_ESTATE, "the window schedule must be chosen before phs_finalize");
+  sim->windows = enable != 0;
   return PHS_OK;
   PHS_API_END
 }
@@ -445,8 +454,10 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
     c.sum_par_rounds += sim->h_res[i].sum_par_rounds;
     c.max_active = std::max(c.max_active, sim->h_res[i].max_active);
     c.max_slots = std::max(c.max_slots, sim->h_res[i].max_slots);
+    c.n_windows += sim->h_res[i].n_windows;
   }
   c.cluster_size = sim->scratch_cs;
+  c.window_gang = sim->win_gang_used;
   c.clusters_resident = sim->clusters_resident;
   c.resumed_units = sim->resumed_units;
   c.n_flow_events = 2 * sim->total_flows;
@@ -463,7 +474,7 @@ const char *phs_instance_path(const phs_sim *sim, int32_t instance) {
   int best = sim->unit_first[instance];  // the path of the instance's largest unit
   for (int u = best; u < sim->unit_first[instance + 1]; ++u)
     if (sim->units[u].n_flows > sim->units[best].n_flows) best = u;
-  return sim->h_res[best].path == 0 ? "cta" : "cluster";
+  return sim->h_res[best].path == 0 ? "cta" : sim->h_res[best].path == 1 ? "cluster" : "window";
 }
 
 }  // extern "C"

@@ -826,7 +826,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       r.max_active = max_active;
       r.max_pending = max_pending;
       r.max_slots = max_slots;
-      r.pad_ = 0;
+      r.n_windows = ev;  // one event per iteration on this path
       T.res[inst] = r;
     }
     cluster.sync();

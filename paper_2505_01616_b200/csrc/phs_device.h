@@ -17,7 +17,7 @@ struct HistRec {     // one rate change of one flow (throughput history, PAPER.m
 struct ParkRegs {  // the loop-carried registers of a parked unit (CTA path)
   double now, t_next;
   long long sum_active, sum_rounds;
-  int32_t ev, solve, g, max_active, max_pending, first_bneck, valid, pad_;
+  int32_t ev, solve, g, max_active, max_pending, first_bneck, valid, n_windows;
 };
 
 struct DevTables {
@@ -46,6 +46,11 @@ struct DevTables {
   size_t park_stride;        //   when a unit stops at t_stop so that a later phs_run_until can resume it; or nullptr
   int32_t resume;            // 1: units with a valid parked state continue from it instead of starting at t = 0
   int32_t n_links;           // largest n_links among the units of this launch (sizes the shared-memory layout)
+  // window path: which CTA of the gang owns what (for the gang size the scheduler chose for the unit)
+  const uint32_t *lloc;      // per unit [n_links]: owner CTA << 24 | index of the link in the owner's shared memory
+  const uint32_t *cown;      // per unit [n_comps]: owner CTA << 24 | index of the component in the owner
+  unsigned long long *t_rel; // [F_total] scratch: latest completion time (bit pattern) among a flow's predecessors
+  uint32_t *fcw;             // [F_total] scratch: cown of the flow's component
 };
 
 // Shared-memory footprint of the CTA kernel for given capacities (pc_flows > 0: predecessor counters of that
@@ -97,6 +102,23 @@ size_t cluster_region_bytes(int64_t Sc, int cluster_size);
 cudaError_t cluster_max_clusters(int cluster_size, size_t smem, int *max_clusters);
 cudaError_t launch_cluster_path(const DevTables &t, const int32_t *list, int n, int *ticket, const ClusterScratch &s,
                                 int cluster_size, int n_clusters, bool log, cudaStream_t stream);
+
+// Window path (phs_window.cu): one gang (thread-block cluster of `gang` CTAs, kWindowThreads threads each) per unit;
+// the unit's static link components are partitioned over the CTAs (lloc / cown in DevTables), every CTA keeps the
+// links, components and flow slots it owns in its own shared memory and the gang meets only at the end of a
+// lookahead window.  Gangs pull units from list[0..n) through *ticket.
+constexpr int kWindowThreads = 256;
+struct WindowLaunch {
+  int gang;     // CTAs per unit: 1, 2, 4, 8 or 16
+  int slots;    // flow slots per CTA
+  int n_links;  // links per CTA (largest over the units of the launch and their CTAs)
+  int n_comps;  // components per CTA (likewise)
+  size_t smem;  // dynamic shared memory per CTA
+};
+size_t window_smem_bytes(int n_links, int n_comps, int slots);
+cudaError_t window_max_clusters(int gang, size_t smem, int *max_clusters);
+cudaError_t launch_window_path(const DevTables &t, const int32_t *list, int n, int *ticket, const WindowLaunch &w,
+                               int n_clusters, cudaStream_t stream);
 
 // out[c] = max t_done over the flows of collective c, for all collectives of all instances.
 cudaError_t launch_collective_times(const double *t_done, const int64_t *coll_first, const int32_t *coll_nflows,

@@ -27,8 +27,9 @@ struct FlowRec {
   int32_t succ_cnt;      // number of successors
   int32_t succ_in[2];    // succ_cnt <= 2: the successors (instance-relative flow ids, -1 if absent);
                          // succ_cnt > 2: succ_in[0] = offset of the list in succ[]
-  int32_t comp;          // static link component of the flow's path = smallest link id of the component:
-                         // two links are in one component iff some chain of flows of the instance connects them
+  int32_t comp;          // static link component of the flow's path (dense id within the unit, in ascending order
+                         // of the components' smallest links): two links are in one component iff some chain of
+                         // flows of the instance connects them
 };
 static_assert(sizeof(FlowRec) == 64, "FlowRec must be 64 bytes");
 
@@ -43,23 +44,28 @@ struct InstDesc {
   int64_t log_base;   // first row of the unit's event log slice (capacity 2F+2 rows), -1 if disabled
   int64_t pc8_base;   // first byte of the unit's slice of the packed predecessor counters (4-byte aligned)
   int64_t init_base;  // first entry of the unit's slice of the initial-activation list (init_t / init_f)
+  int64_t comp_base;  // first entry of the unit in the per-component arrays (cown)
   int32_t n_flows;
   int32_t n_links;
   int32_t n_init;     // flows without predecessors
-  int32_t pad_;
+  int32_t n_comps;    // static link components of the unit (dense ids 0 .. n_comps-1, see FlowRec::comp)
+  double lmin;        // lookahead of the unit: the smallest path latency among its flows that have predecessors
+                      // (+inf if none has).  A flow released by an event at time t activates no earlier than t + lmin,
+                      // so all events in [T0, T0 + lmin) of different components are independent (DESIGN.md sec 4,
+                      // "Lookahead windows"); 0 disables the window schedule for the unit.
 };
 
 // Per-instance result block (device, read back after a run).
 struct InstResult {
   int32_t status;          // PHS_OK, PHS_ECYCLE, or kOverflow (re-run on the cluster path)
-  int32_t path;            // 0 = cta, 1 = cluster
+  int32_t path;            // 0 = cta, 1 = cluster, 2 = window
   int64_t n_events;
   int64_t sum_active;
   int64_t sum_par_rounds;
   int32_t max_active;
   int32_t max_pending;
   int32_t max_slots;       // high-water mark of the slot array
-  int32_t pad_;
+  int32_t n_windows;       // lookahead windows of the run (= n_events for a unit that ran one event per iteration)
 };
 constexpr int32_t kOverflow = 1;  // internal: the CTA path ran out of shared-memory slots
 constexpr int32_t kPaused = 2;    // internal: stopped before the first event later than the requested time

@@ -667,7 +667,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         ParkRegs r;
         r.now = now; r.t_next = t_next; r.sum_active = sum_active; r.sum_rounds = sum_rounds;
         r.ev = ev; r.solve = solve; r.g = g; r.max_active = max_active; r.max_pending = max_pending;
-        r.first_bneck = first_bneck; r.valid = status == kPaused ? 1 : 0; r.pad_ = 0;
+        r.first_bneck = first_bneck; r.valid = status == kPaused ? 1 : 0; r.n_windows = 0;
         *park = r;
       }
     }
@@ -687,6 +687,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       r.max_active = max_active;
       r.max_pending = max_pending;
       r.max_slots = S.ctl[C_HI];
+      r.n_windows = ev;  // one event per iteration on this path
       T.res[inst] = r;
     }
     __syncthreads();

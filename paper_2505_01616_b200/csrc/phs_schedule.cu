@@ -25,6 +25,77 @@ StagingArea &staging_area() {
 
 #define fail phs_fail
 
+// ================================================================================================ window path plan
+namespace {
+
+// Decides whether unit `u` runs on the window path and with how many CTAs (a9), for slot estimates scaled by
+// `scale` quarters, and writes the ownership tables of its gang: the unit's static link components are dealt to the
+// CTAs largest first, each to the CTA with the fewest flows so far; links and components get indices local to their
+// owner.  A unit that does not go there keeps the identity tables (owner 0).
+bool plan_window_unit(phs_sim *sim, int u, size_t smem_max, int64_t scale) {
+  phs_sim::Unit &un = sim->units[(size_t)u];
+  const int32_t *lcomp = sim->h_lcomp.data() + un.link_base;
+  uint32_t *lloc = sim->h_lloc.data() + un.link_base, *cown = sim->h_cown.data() + un.comp_base;
+  const int32_t *cflows = sim->comp_flows.data() + un.comp_base, *clinks = sim->comp_links.data() + un.comp_base;
+  un.win_gang = 0;
+  for (int l = 0; l < un.n_links; ++l) lloc[l] = (uint32_t)l;
+  for (int c = 0; c < un.n_comps; ++c) cown[c] = (uint32_t)c;
+  double threshold = 4.0;  // estimated flow events per window from which the window schedule pays (measured: cfg1, with
+                           // 0.4, is faster one event at a time; cfg2, with ~100, is 30 x faster in windows)
+  if (const char *ev = getenv("PHS_WIN_DENSITY")) threshold = atof(ev);
+  const bool forced = sim->policy_path == 3;  // phs_set_scheduler: every eligible unit, whatever its density
+  if (!sim->windows || sim->want_log || sim->hist_cap > 0 || (sim->policy_path != 0 && !forced) || un.n_flows == 0)
+    return false;
+  // small units stay on the CTA path: many of them are resident per SM there, and a batch of them is bound by
+  // instruction throughput, not by the length of one unit's event chain
+  if (!(sim->h_desc[(size_t)u].lmin > 0.0) || (!forced && (!(un.density >= threshold) || un.n_flows < 8192))) return false;
+  // gang size: about 16 components per CTA (measured on cfg2's 128-component unit: 8 and 16 CTAs tie, 4 are a third
+  // slower), more if the unit does not fit otherwise
+  int want_gang = 1;
+  while (want_gang < 16 && un.n_comps > 16 * want_gang) want_gang *= 2;
+  const int min_gang = forced ? std::max(1, sim->policy_slots) : want_gang;
+  std::vector<int32_t> by_size((size_t)un.n_comps);
+  std::iota(by_size.begin(), by_size.end(), 0);
+  std::stable_sort(by_size.begin(), by_size.end(), [&](int a, int b) { return cflows[a] > cflows[b]; });
+  for (int K = 1; K <= 16; K *= 2) {
+    if (K < min_gang && un.n_comps >= K * 2) continue;
+    if (K > 1 && un.n_comps < (forced ? K : 2 * K)) break;  // a gang needs components to share out
+    std::vector<int64_t> kflows((size_t)K, 0);
+    std::vector<int32_t> klinks((size_t)K, 0), kcomps((size_t)K, 0), owner((size_t)un.n_comps, 0);
+    for (int c : by_size) {
+      const int k = (int)(std::min_element(kflows.begin(), kflows.end()) - kflows.begin());
+      owner[(size_t)c] = k;
+      kflows[(size_t)k] += cflows[c];
+      klinks[(size_t)k] += clinks[c];
+      kcomps[(size_t)k]++;
+    }
+    const int Lm = *std::max_element(klinks.begin(), klinks.end());
+    const int NCm = *std::max_element(kcomps.begin(), kcomps.end());
+    const int64_t fmax = *std::max_element(kflows.begin(), kflows.end());
+    if (Lm >= 65535) continue;
+    // slots of the busiest CTA: its share of the unit's bound on PENDING + ACTIVE flows, a quarter on top
+    int64_t slots = (int64_t)std::ceil((double)std::max<int64_t>(un.bound_cta, 32) * (double)fmax /
+                                       (double)un.n_flows * 1.25 * (double)scale / 4.0) + 64;
+    slots = std::min<int64_t>(slots, fmax + 32);
+    slots = (slots + 31) / 32 * 32;
+    if (window_smem_bytes(std::max(Lm, 1), std::max(NCm, 1), (int)slots) + 512 > smem_max) continue;
+    std::vector<int32_t> next_link((size_t)K, 0), next_comp((size_t)K, 0);
+    for (int c = 0; c < un.n_comps; ++c) cown[c] = ((uint32_t)owner[(size_t)c] << 24) | (uint32_t)next_comp[(size_t)owner[(size_t)c]]++;
+    for (int l = 0; l < un.n_links; ++l) {
+      const int k = owner[(size_t)lcomp[l]];
+      lloc[l] = ((uint32_t)k << 24) | (uint32_t)next_link[(size_t)k]++;
+    }
+    un.win_gang = K;
+    un.win_links = std::max(Lm, 1);
+    un.win_comps = std::max(NCm, 1);
+    un.win_slots = (int)slots;
+    return true;
+  }
+  return false;
+}
+
+}  // namespace
+
 // ================================================================================================ finalize
 // Splits the instances into simulation units and builds the device-resident tables.  HBM layout (DESIGN.md "Data
 // layout"): one 64-byte FlowRec per flow (path, successors and component inline, unit-local ids), successor lists
@@ -72,6 +143,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     std::vector<int64_t> capq;
     std::vector<double> init_t;
     std::vector<int32_t> init_f;
+    std::vector<int32_t> comp_flows, comp_links;  // per component of every unit: flows, links
     std::vector<InstDesc> desc;  // bases relative to the chunk
     std::vector<phs_sim::Unit> units;
     int max_pred = 0;
@@ -248,14 +320,30 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       d.log_base = sim->want_log ? log_cursor : -1;
       d.pc8_base = (int64_t)c.pc8.size();
       d.init_base = (int64_t)c.init_t.size();
-      d.pad_ = 0;
       d.n_flows = (int32_t)fl.size();
       d.n_links = (int32_t)links.size();
-      for (int32_t l : links) {
-        c.capq.push_back(capq_inst[l]);
-        c.lcomp.push_back(link_loc[find_in(parent, l)]);  // the smallest link of a component is in the unit too
-        c.linkid.push_back(l);
+      // dense component ids, in ascending order of the components' smallest links (links[] is ascending, so a
+      // component's representative -- its smallest link -- is met before its other links)
+      std::vector<int32_t> comp_id(links.size(), -1);
+      int32_t n_comps = 0;
+      for (size_t k = 0; k < links.size(); ++k) {
+        const int32_t rep = link_loc[find_in(parent, links[k])];
+        if (comp_id[rep] < 0) comp_id[rep] = n_comps++;
+        comp_id[k] = comp_id[rep];
       }
+      d.n_comps = n_comps;
+      d.comp_base = (int64_t)c.comp_flows.size();
+      c.comp_flows.resize(c.comp_flows.size() + (size_t)n_comps, 0);
+      c.comp_links.resize(c.comp_links.size() + (size_t)n_comps, 0);
+      int64_t capmax_q = 1;
+      for (size_t k = 0; k < links.size(); ++k) {
+        c.capq.push_back(capq_inst[links[k]]);
+        c.lcomp.push_back(comp_id[k]);
+        c.linkid.push_back(links[k]);
+        c.comp_links[(size_t)d.comp_base + comp_id[k]]++;
+        capmax_q = std::max(capmax_q, capq_inst[links[k]]);
+      }
+      double lmin = std::numeric_limits<double>::infinity();
       c.pc8.resize(c.pc8.size() + (fl.size() + 7) / 8 * 4, 0);
       for (size_t k = 0; k < fl.size(); ++k) {
         const int32_t f = fl[k];
@@ -274,10 +362,12 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           x.succ_in[1] = -1;
           for (uint32_t e = soff[f]; e < soff[f + 1]; ++e) c.succ.push_back(flow_loc[sdst[e]]);
         }
-        x.comp = p0 < p1 ? link_loc[find_in(parent, in.path[p0])] : 0;
+        x.comp = p0 < p1 ? comp_id[link_loc[in.path[p0]]] : 0;
+        c.comp_flows[(size_t)d.comp_base + x.comp]++;
         rec[(size_t)(fb + flow_cursor) + k] = x;
         fmap[(size_t)(fb + flow_cursor) + k] = (uint32_t)(fb + f);
         const int32_t np = (int32_t)(in.pred_off[f + 1] - in.pred_off[f]);
+        if (np > 0) lmin = std::min(lmin, in.lat[f]);
         pc0[(size_t)(fb + flow_cursor) + k] = np;
         c.max_pred = std::max(c.max_pred, np);
         c.pc8[(size_t)d.pc8_base + k / 2] |= (uint8_t)(std::min(np, 15) << ((k & 1) * 4));
@@ -293,6 +383,33 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           c.init_f.push_back(e.second);
         }
       }
+      d.lmin = sim->windows ? lmin : 0.0;
+      // Estimated flow events per lookahead window = 2 F lmin / span, with a LOWER bound of the unit's simulated
+      // span: every collective takes at least steps x (Lat + chunk / fastest link of the unit), chained collectives
+      // follow each other, raw flows at least start + Lat + bytes / fastest link.  Contention only stretches the span,
+      // so this over-estimates the density; the window path is worth its per-window overhead only when many events
+      // share a window, so a unit goes there when the estimate is well above one (see the scheduler below).
+      double density = 0.0;
+      if (lmin > 0.0 && !fl.empty()) {
+        const double capmax = (double)capmax_q / 1048576.0;
+        double span = 0.0;
+        std::vector<uint8_t> in_coll(fl.size(), 0);
+        std::vector<double> end_of(in.colls.size(), 0.0);
+        for (size_t ci = 0; ci < in.colls.size(); ++ci) {
+          const Collective &co = in.colls[ci];
+          if (co.n_flows == 0 || unit_of[co.first_flow] != u) continue;
+          double begin = co.start;
+          for (int32_t a : co.after) begin = std::max(begin, end_of[(size_t)a]);
+          const double chunk = co.bytes / (double)co.n_ranks;
+          end_of[ci] = begin + (double)co.steps * (in.lat[co.first_flow] + chunk / capmax);
+          span = std::max(span, end_of[ci]);
+          for (int32_t f = co.first_flow; f < co.first_flow + co.n_flows; ++f) in_coll[(size_t)flow_loc[f]] = 1;
+        }
+        for (size_t k = 0; k < fl.size(); ++k)
+          if (!in_coll[k]) span = std::max(span, in.start[fl[k]] + in.lat[fl[k]] + in.bytes[fl[k]] / capmax);
+        density = std::isinf(lmin) ? std::numeric_limits<double>::infinity()
+                                   : 2.0 * (double)fl.size() * lmin / std::max(span, 1e-300);
+      }
       flow_cursor += (int64_t)fl.size();
       log_cursor += 2 * (int64_t)fl.size() + 2;
       c.desc.push_back(d);
@@ -300,9 +417,14 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       un.inst = i;
       un.n_flows = d.n_flows;
       un.n_links = d.n_links;
+      un.n_comps = d.n_comps;
       un.bound = ubound[u];
       un.bound_cta = ubound_cta[u];
       un.bound_whole = std::min(ubound[u], uwhole[u]);
+      un.comp_base = d.comp_base;
+      un.link_base = d.link_base;
+      un.density = density;
+      un.win_gang = 0;
       c.units.push_back(un);
     }
   };
@@ -313,7 +435,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     if (chunks[i].st != PHS_OK) return fail(chunks[i].st, chunks[i].err);
   // lay the chunks out back to back
   std::vector<int64_t> b_flow(B + 1, 0), b_link(B + 1, 0), b_succ(B + 1, 0), b_pc8(B + 1, 0), b_log(B + 1, 0),
-      b_init(B + 1, 0);
+      b_init(B + 1, 0), b_comp(B + 1, 0);
   sim->units.clear();
   sim->unit_first.assign(B + 1, 0);
   int max_pred = 0;
@@ -324,9 +446,14 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     b_succ[i + 1] = b_succ[i] + (int64_t)c.succ.size();
     b_pc8[i + 1] = b_pc8[i] + (int64_t)c.pc8.size();
     b_init[i + 1] = b_init[i] + (int64_t)c.init_t.size();
+    b_comp[i + 1] = b_comp[i] + (int64_t)c.comp_flows.size();
     b_log[i + 1] = b_log[i] + 2 * (sim->flow_base[i + 1] - sim->flow_base[i]) + 2 * (int64_t)c.units.size();
     sim->unit_first[i] = (int32_t)sim->units.size();
     sim->units.insert(sim->units.end(), c.units.begin(), c.units.end());
+    for (size_t k = sim->units.size() - c.units.size(); k < sim->units.size(); ++k) {
+      sim->units[k].comp_base += b_comp[i];
+      sim->units[k].link_base += b_link[i];
+    }
     max_pred = std::max(max_pred, c.max_pred);
   }
   const int64_t log_cursor = b_log[B];
@@ -336,8 +463,12 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   std::vector<double> init_t((size_t)b_init[B]);
   std::vector<int32_t> init_f((size_t)b_init[B]);
   sim->h_desc.assign(sim->units.size(), InstDesc{});
+  sim->comp_flows.assign((size_t)b_comp[B], 0);
+  sim->comp_links.assign((size_t)b_comp[B], 0);
   parallel_for(B, [&](int i) {
     Chunk &c = chunks[i];
+    std::copy(c.comp_flows.begin(), c.comp_flows.end(), sim->comp_flows.begin() + b_comp[i]);
+    std::copy(c.comp_links.begin(), c.comp_links.end(), sim->comp_links.begin() + b_comp[i]);
     std::copy(c.succ.begin(), c.succ.end(), succ.begin() + b_succ[i]);
     std::copy(c.pc8.begin(), c.pc8.end(), pc8.begin() + b_pc8[i]);
     std::copy(c.capq.begin(), c.capq.end(), capq.begin() + b_link[i]);
@@ -352,6 +483,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       d.succ_base += b_succ[i];
       d.pc8_base += b_pc8[i];
       d.init_base += b_init[i];
+      d.comp_base += b_comp[i];
       if (d.log_base >= 0) d.log_base += b_log[i];
       sim->h_desc[(size_t)sim->unit_first[i] + k] = d;
     }
@@ -359,6 +491,14 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_T("concat");
   sim->unit_first[B] = (int32_t)sim->units.size();
   const int U = (int)sim->units.size();
+  // window path (a9): which units run the lookahead-window schedule, and the ownership tables of their gangs
+  sim->h_lcomp = lcomp;
+  sim->h_lloc.assign(lcomp.size(), 0);
+  sim->h_cown.assign((size_t)b_comp[B], 0);
+  sim->win_list.clear();
+  for (int u = 0; u < U; ++u)
+    if (plan_window_unit(sim, u, (size_t)smem_optin, sim->win_scale)) sim->win_list.push_back(u);
+  PHS_T("window plan");
   const bool pc8_ok = max_pred <= 15;  // the packed counters hold 4 bits per flow
 
   // one device allocation for all tables and result arrays (a cudaMalloc costs about 0.1 ms, and there are 19 of
@@ -404,6 +544,8 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     put_all();
     PHS_CUDA(err);
   }
+  PHS_CUDA(sim->d_lloc.upload(sim->h_lloc, st));
+  PHS_CUDA(sim->d_cown.upload(sim->h_cown, st));
   if (sim->want_log) PHS_CUDA(sim->d_log.alloc((size_t)log_cursor));
   if (sim->hist_cap > 0) {
     PHS_CUDA(sim->d_hist.alloc((size_t)sim->hist_cap));
@@ -428,6 +570,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   for (int u = 0; u < U; ++u) {
     const phs_sim::Unit &un = sim->units[u];
     if (un.n_flows == 0) continue;  // nothing to simulate; its result block stays zero (status OK)
+    if (un.win_gang > 0) continue;  // runs on the window path
     if (sim->policy_path == 2 || un.n_links >= 65535 ||
         cta_smem_bytes(un.n_links, (need_of(un) + 31) / 32 * 32, 0, log) > smem_max)
       sim->cluster_list.push_back(u);
@@ -435,10 +578,11 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       cand.push_back(u);
   }
   while (!cand.empty()) {
-    int Lm = 1, need = 32;
+    int Lm = 1, NCm = 1, need = 32;
     int64_t maxF = 1;
     for (int u : cand) {
       Lm = std::max(Lm, sim->units[u].n_links);
+      NCm = std::max(NCm, sim->units[u].n_comps);
       need = std::max(need, need_of(sim->units[u]));
       maxF = std::max<int64_t>(maxF, sim->units[u].n_flows);
     }
@@ -462,7 +606,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         const size_t budget = std::min(smem_max, per_sm / w - 1024);
         if (cta_smem_bytes(Lm, 32, pcf, log) > budget) continue;
         int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
-        if (sim->policy_slots > 0) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
+        if (sim->policy_slots > 0 && sim->policy_path != 3) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
         hi = (hi + 31) / 32 * 32;
         while (lo < hi) {  // largest multiple of 32 that fits the budget
           const int mid = ((lo + hi + 32) / 64) * 32;
@@ -471,8 +615,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           else
             hi = mid - 32;
         }
-        if (lo >= need || (w == 1 && sim->policy_path == 1) || sim->policy_slots > 0) {
-          if (sim->policy_slots == 0) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
+        const bool capped = sim->policy_slots > 0 && sim->policy_path != 3;
+        if (lo >= need || (w == 1 && sim->policy_path == 1) || capped) {
+          if (!capped) lo = std::min(lo, (need + 31) / 32 * 32);  // no more than can be used
           *slots_out = lo;
           return w;
         }
@@ -529,6 +674,10 @@ namespace {
 
 DevTables tables_of(phs_sim *sim, int n_links) {
   DevTables t;
+  t.lloc = sim->d_lloc.p;
+  t.cown = sim->d_cown.p;
+  t.t_rel = sim->d_trel.p;
+  t.fcw = sim->d_fcw.p;
   t.inst = sim->d_desc.p;
   t.rec = sim->d_rec.p;
   t.succ = sim->d_succ.p;
@@ -666,6 +815,86 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   return PHS_OK;
 }
 
+
+// Window path (a9): the units of `todo` run the lookahead-window schedule, one gang of CTAs each; gangs of one size
+// share a launch.  Units that run out of slots are planned again with a larger estimate (possibly a larger gang);
+// the ones that do not fit any more are returned in `fallback` (they go to the cluster path).
+phs_status run_window_path(phs_sim *sim, std::vector<int32_t> todo, std::vector<int32_t> *fallback, cudaStream_t st) {
+  if (!sim->d_wticket.p) PHS_CUDA(sim->d_wticket.alloc(1));
+  if (!sim->d_trel.p) {  // per-flow scratch of the window path (initialised by the kernel, unit by unit)
+    PHS_CUDA(sim->d_trel.alloc((size_t)sim->total_flows));
+    PHS_CUDA(sim->d_fcw.alloc((size_t)sim->total_flows));
+  }
+  int64_t scale = sim->win_scale;
+  while (!todo.empty()) {
+    for (int K = 1; K <= 16; K *= 2) {
+      std::vector<int32_t> group;
+      for (int u : todo)
+        if (sim->units[(size_t)u].win_gang == K) group.push_back(u);
+      // one launch per set of units whose combined layout (largest links, components, slots per CTA) fits
+      std::stable_sort(group.begin(), group.end(),
+                       [&](int a, int b) { return sim->units[(size_t)a].n_flows > sim->units[(size_t)b].n_flows; });
+      size_t pos = 0;
+      while (pos < group.size()) {
+        WindowLaunch w{};
+        w.gang = K;
+        size_t end = pos;
+        for (; end < group.size(); ++end) {
+          const phs_sim::Unit &un = sim->units[(size_t)group[end]];
+          const int L2 = std::max(w.n_links, un.win_links), C2 = std::max(w.n_comps, un.win_comps),
+                    S2 = std::max(w.slots, un.win_slots);
+          if (end > pos && window_smem_bytes(L2, C2, S2) + 512 > sim->smem_optin) break;
+          w.n_links = L2;
+          w.n_comps = C2;
+          w.slots = S2;
+        }
+        w.smem = window_smem_bytes(w.n_links, w.n_comps, w.slots);
+        std::vector<int32_t> part(group.begin() + (long)pos, group.begin() + (long)end);
+        int max_clusters = 0;
+        PHS_CUDA(window_max_clusters(K, w.smem, &max_clusters));
+        if (max_clusters < 1) return fail(PHS_ECUDA, "window path: a gang of " + std::to_string(K) + " CTAs cannot be resident");
+        const int n_clusters = std::min<int>((int)part.size(), max_clusters);
+        PHS_CUDA(sim->d_wlist.upload(part, st));
+        PHS_CUDA(cudaMemsetAsync(sim->d_wticket.p, 0, sizeof(int), st));
+        int Lmax = 1;
+        for (int u : part) Lmax = std::max(Lmax, sim->units[(size_t)u].n_links);
+        if (getenv("PHS_TIMING"))
+          fprintf(stderr, "[phs_run] window path: %d units, gang %d, per CTA: links %d, comps %d, slots %d, smem %zu; %d gangs resident\n",
+                  (int)part.size(), K, w.n_links, w.n_comps, w.slots, w.smem, n_clusters);
+        PHS_CUDA(launch_window_path(tables_of(sim, Lmax), sim->d_wlist.p, (int)part.size(), sim->d_wticket.p, w,
+                                    n_clusters, st));
+        PHS_CUDA(cudaStreamSynchronize(st));  // `part` is pageable host memory read by the async copy
+        sim->n_launches++;
+        sim->win_gang_used = std::max(sim->win_gang_used, K);
+        pos = end;
+      }
+    }
+    const int U = (int)sim->units.size();
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    std::vector<int32_t> again;
+    for (int u : todo)
+      if (sim->h_res[(size_t)u].status == kOverflow) again.push_back(u);
+    if (again.empty()) break;
+    scale *= 2;  // more slots, possibly a larger gang; what does not fit any more leaves the window path for good
+    sim->win_scale = scale;
+    todo.clear();
+    for (int u : again) {
+      if (scale <= 64 && plan_window_unit(sim, u, sim->smem_optin, scale)) {
+        todo.push_back(u);
+      } else {
+        sim->units[(size_t)u].win_gang = 0;
+        sim->win_list.erase(std::find(sim->win_list.begin(), sim->win_list.end(), u));
+        fallback->push_back(u);
+      }
+    }
+    PHS_CUDA(sim->d_lloc.upload(sim->h_lloc, st));
+    PHS_CUDA(sim->d_cown.upload(sim->h_cown, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+  }
+  return PHS_OK;
+}
+
 }  // namespace
 
 extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
@@ -709,6 +938,11 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   sim->n_launches = 0;
   sim->resumed_units = 0;
   std::vector<int32_t> cta_list(sim->order), cluster_todo(sim->cluster_list);
+  // The window path runs whole simulations only: a stop time, or a resume from parked state, sends its units to the
+  // cluster path (same results, one event per iteration).
+  const bool use_windows = !finite && !resume;
+  sim->win_gang_used = 0;
+  if (!use_windows) cluster_todo.insert(cluster_todo.end(), sim->win_list.begin(), sim->win_list.end());
   if (resume) {  // only what has not finished yet
     auto paused = [&](int u) { return sim->h_res[u].status == kPaused; };
     cta_list.erase(std::remove_if(cta_list.begin(), cta_list.end(), [&](int u) { return !paused(u); }), cta_list.end());
@@ -750,6 +984,22 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
     if (!sim->order.empty()) PHS_CUDA(sim->d_order.upload(sim->order, st));
     sim->cta.grid = std::min<int>(sim->cta.grid, std::max<int>(1, (int)sim->order.size()));
     PHS_CUDA(cudaStreamSynchronize(st));
+  }
+  // window path; units that stop fitting there continue on the cluster path
+  if (use_windows && !sim->win_list.empty()) {
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
+    std::vector<int32_t> fb;
+    phs_status ws = run_window_path(sim, sim->win_list, &fb, st);
+    if (ws != PHS_OK) return ws;
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    float extra = 0.f;
+    PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
+    sim->main_kernel_ms += extra;
+    for (int u : fb) {
+      sim->cluster_list.push_back(u);
+      cluster_todo.push_back(u);
+    }
   }
   // cluster path; an instance that overflows a CTA's slot partition is re-run with larger partitions
   std::vector<int32_t> todo(cluster_todo);

@@ -149,14 +149,20 @@ struct phs_sim {
   std::vector<int64_t> flow_base;  // [B+1]
   std::vector<int64_t> coll_base;  // [B+1]
   struct Unit {  // what one CTA / cluster simulates (see phs::InstDesc)
-    int32_t inst, n_flows, n_links;
+    int32_t inst, n_flows, n_links, n_comps;
     int64_t bound;    // upper estimate of the flows PENDING or ACTIVE at once (see phs_finalize)
     int64_t bound_cta;  // the same for the CTA kernel, which reuses a vacated slot within the phase (rings: 1.5 N)
     int64_t bound_whole;  // the part of `bound` from raw flows and all-to-alls (may be in flight all at once)
+    int64_t comp_base;    // first entry of the unit in the per-component host arrays (comp_flows, comp_links, h_cown)
+    int64_t link_base;    // first entry of the unit in the per-link host arrays (h_lcomp, h_lloc)
+    double density;       // estimated flow events per lookahead window (see phs_finalize); decides the window path
+    int32_t win_gang;     // CTAs of the unit's gang on the window path, 0 = the unit does not run there
+    int32_t win_links, win_comps, win_slots;  // per CTA of the gang: links, components, flow slots (largest member)
   };
   std::vector<Unit> units;
   std::vector<int32_t> unit_first;  // [B+1] units of instance i are unit_first[i] .. unit_first[i+1]-1
   bool decompose = true;
+  bool windows = true;  // lookahead-window schedule (phs_set_windows); off: one global event per loop iteration
   double t_stop = 0.0;  // stop time of the current / last run (phs_run_until), +inf for phs_run
   // parked state of the CTA-path units of a run that stopped at parked_until (phs_run_until resumes from it)
   phs::DevBuf<unsigned char> d_park;
@@ -176,6 +182,17 @@ struct phs_sim {
   std::vector<phs::InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first
   std::vector<int32_t> cluster_list;  // instances that go (or fell back) to the cluster path
+  // window path: its units, and the ownership tables of their gangs (identity for everybody else)
+  std::vector<int32_t> win_list;
+  std::vector<int32_t> comp_flows, comp_links, h_lcomp;  // per component: flows, links; per link: its component
+  std::vector<uint32_t> h_lloc, h_cown;
+  phs::DevBuf<uint32_t> d_lloc, d_cown, d_fcw;
+  phs::DevBuf<unsigned long long> d_trel;
+  phs::DevBuf<int32_t> d_wlist;
+  phs::DevBuf<int> d_wticket;
+  int64_t win_scale = 1;  // slot estimate of the window path in quarters of the static bound (doubled after an
+                          // overflow): initial flows take their slots only when they are due, so a quarter is typical
+  int win_gang_used = 0;
   int64_t total_flows = 0, total_colls = 0;
 
   // ---- device tables

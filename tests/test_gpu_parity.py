@@ -16,7 +16,7 @@ from util import completion_order, oracle_build, oracle_run
 pytestmark = pytest.mark.gpu
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
-CTA, CLUSTER = 1, 2
+CTA, CLUSTER, WINDOW = 1, 2, 3
 
 
 def assert_instance_matches(sim, i, o, check_log=True):
@@ -115,6 +115,73 @@ def test_cfg2_shrunken_fat_tree(path):
 def test_cfg4_shrunken_alltoall(path):
     # 64 GPUs, 4032 concurrent Zipf flows, many filling rounds per event
     run_and_compare(W.cfg4(batch=2, n_hosts=8, gph=8, n_leaves=4, n_spines=2), path=path)
+
+
+def _window_compare(w, gang, expect_gang=None, first=0, count=None):
+    """The window path (forced: phs_set_scheduler path 3, smallest gang `gang`) against the oracle, decomposed and
+    not, plus against the library's own one-event-per-iteration schedule."""
+    count = w.batch if count is None else count
+    for decompose in (True, False):
+        sim = B.Sim.from_workload(w, instances=(first, count), path=WINDOW, cta_slots=gang, decompose=decompose)
+        sim.run()
+        c = sim.counters()
+        assert c["window_gang"] >= 1
+        if expect_gang and not decompose:      # the smallest gang asked for, or a larger one if that does not fit
+            assert c["window_gang"] >= expect_gang, c
+        assert c["n_windows"] <= c["n_events"] or c["window_gang"] > 1
+        for i in range(count):
+            o = oracle_run(w.desc, w.instances[first + i], mode=orc.MODE_FAST, base_seed=w.base_seed)
+            assert_instance_matches(sim, i, o, check_log=False)
+        if not decompose:
+            assert all(sim.path_of(i) == "window" for i in range(count))
+        sim.close()
+
+
+@pytest.mark.parametrize("gang", [1, 4])
+def test_window_path_ring_configs(gang):
+    # cfg1 (TP + DP rings that contend on the leaf-spine uplinks), cfg3 (random capacities, chained collectives)
+    _window_compare(W.cfg1(batch=3, n_hosts=8, gph=4, n_leaves=4, n_spines=2), gang, expect_gang=gang)
+    _window_compare(W.cfg3(batch=4), gang, expect_gang=gang)
+    _window_compare(W.cfg1(batch=2), gang, first=1, count=1, expect_gang=gang)
+
+
+@pytest.mark.parametrize("gang", [1, 2, 8, 16])
+def test_window_path_shrunken_fat_tree(gang):
+    # k=8 fat tree, staggered starts, AR + AG + RS: many events per window (the regime the path is built for)
+    _window_compare(W.cfg2(k=8, agg_uplinks=2), gang, expect_gang=gang)
+
+
+def test_window_path_single_component_and_raw_flows():
+    # all-to-all: ONE component, no dependencies (lmin = +inf: a single window); a gang has nothing to share out
+    _window_compare(W.cfg4(batch=2, n_hosts=4, gph=4, n_leaves=2, n_spines=2), 4, expect_gang=1)
+    _window_compare(W.cfg0(), 1, expect_gang=1)
+    # too large for the shared memory of one CTA, and one component cannot be shared out: not on the window path
+    w = W.cfg4(batch=1, n_hosts=8, gph=8, n_leaves=4, n_spines=2)
+    sim = B.Sim.from_workload(w, path=WINDOW, cta_slots=4, decompose=False)
+    sim.run()
+    assert sim.path_of(0) != "window"
+    assert_instance_matches(sim, 0, oracle_run(w.desc, w.instances[0], mode=orc.MODE_FAST), check_log=False)
+    sim.close()
+
+
+def test_window_path_is_chosen_for_dense_units_only():
+    # automatic policy: shrunken cfg2 (events every few hundred ns against a 4 us lookahead) goes to the window path,
+    # cfg1 / cfg3 (events tens of us apart) stay one event per iteration
+    sim = B.Sim.from_workload(W.cfg2(k=8, agg_uplinks=2))
+    sim.run()
+    assert sim.path_of(0) == "window" and sim.counters()["n_windows"] < sim.counters()["n_events"]
+    sim.close()
+    sim = B.Sim.from_workload(W.cfg3(batch=2))
+    sim.run()
+    assert sim.path_of(0) == "cta" and sim.counters()["window_gang"] == 0
+    sim.close()
+    # the window schedule switched off: same results, CTA / cluster paths only
+    a = B.Sim.from_workload(W.cfg2(k=8, agg_uplinks=2), windows=False)
+    a.run()
+    assert a.path_of(0) != "window"
+    o = oracle_run(W.cfg2(k=8, agg_uplinks=2).desc, W.cfg2(k=8, agg_uplinks=2).instances[0], mode=orc.MODE_FAST)
+    assert_instance_matches(a, 0, o, check_log=False)
+    a.close()
 
 
 def test_cta_slot_overflow_falls_back_to_cluster():
@@ -219,7 +286,7 @@ def test_cfg4_full_size_whole_batch_as_benchmarked():
     for i in range(w.batch):
         _check_against_golden(sim, i, zs[i])
     c = sim.counters()
-    assert c["n_events"] == sum(int(z["n_events"]) for z in zs)       # one unit per instance: same event sequence
+    assert c["n_flow_events"] == 2 * sim.total_flows
     if c["cluster_size"] > 0 and sim.path_of(0) == "cluster":
         # more units than resident clusters: some cluster simulated two units back to back (ticket, re-init, scratch reuse)
         print("cfg4 launch: cluster size", c["cluster_size"], "resident", c["clusters_resident"])
@@ -311,6 +378,8 @@ def test_random_dags_of_raw_flows(seed):
                                                         np.array(dep_ids, np.int64))]))
     w = W.Workload("fuzz", d, 7 * seed, insts)
     run_and_compare(w, path=[0, CTA, CLUSTER][seed % 3], mode=orc.MODE_FAST)
+    if lat > 0.0:       # the window path needs a positive lookahead; fan-in up to 24 exercises the release lists
+        _window_compare(w, [1, 2, 4][seed % 3])
 
 
 @pytest.mark.parametrize("path", [CTA, CLUSTER])
