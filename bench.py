@@ -4,7 +4,8 @@ synthetic instances) on N GPUs of one node.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1] [--impl ours|reference]
 
-N=1 workload = BASELINE.json configs[1] (cfg1: 64 instances x 5,632 flows, leaf-spine, TP + DP ring all-reduces).
+N=1 workload = BASELINE.json configs[3] (cfg3: 4,096 instances x 7,168 flows, the largest single-GPU configuration and
+the one whose tables are HBM-resident); the same line carries `per_config`: one short run of each other config.
 Prints ONE JSON line (rank 0).  `value` = flow-events/s with the tables already resident in HBM; `e2e` = the same
 metric through the C-ABI from HOST arrays (submission calls, table build, H2D, run, D2H inside the timed region).
 N>1: instances are independent, so each rank simulates its own block of instances (weak scaling, no data-path
@@ -181,12 +182,13 @@ def run_reference(args, rank, world):
         idx = [(nxt + k) % w.batch for k in range(per_step)]
         nxt = (nxt + per_step) % w.batch
         return oracle_time(w, idx)
-    for _ in range(args.warmup):
-        step()
-    secs = flows = colls = 0
-    for _ in range(args.steps):
-        s, f, c, _w = step()
-        secs += s; flows += f; colls += c
+    with PinnedCore() as pin:
+        for _ in range(args.warmup):
+            step()
+        secs = flows = colls = 0
+        for _ in range(args.steps):
+            s, f, c, _w = step()
+            secs += s; flows += f; colls += c
     val = 2.0 * flows / secs
     sample = sample_txt[0]
     print(json.dumps({
@@ -195,22 +197,76 @@ def run_reference(args, rank, world):
         "vs_baseline": None, "dtype": "f64+i64", "data": "synthetic",
         "config": {"workload": args.workload, "sample": sample},
         "collectives_per_sec": colls / secs,
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model(), "pinned_to_core": pin.core, "host_cores": os.cpu_count()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
 
 # ---------------------------------------------------------------------------------------------- our arm
-def run_ours(args, rank, world, local_rank):
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+class PinnedCore:
+    """Pins the calling process to one core while the single-threaded oracle is timed."""
+    def __enter__(self):
+        self.old = None
+        try:
+            self.old = os.sched_getaffinity(0)
+            self.core = max(self.old)
+            os.sched_setaffinity(0, {self.core})
+        except Exception:
+            self.core = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.old:
+            try:
+                os.sched_setaffinity(0, self.old)
+            except Exception:
+                pass
+
+
+def golden_work(workload, n_inst):
+    """Work counters of the FULL oracle runs of cfg2 / cfg4, stored beside the golden values by
+    tests/golden/make_golden.py (which calls only oracle/): summed over instances 0..n_inst-1."""
+    wk, flows = {}, 0
+    for i in range(n_inst):
+        path = os.path.join(ROOT, "tests", "golden", f"{workload}_inst{i}.npz")
+        if not os.path.exists(path):
+            return None, 0
+        g = np.load(path)
+        for k, v in zip(g["work_keys"].tolist(), g["work_vals"].tolist()):
+            wk[k] = wk.get(k, 0.0) + v
+        flows += int(g["n_flows"])
+    return wk, flows
+
+
+def measured_traffic(workload):
+    """DRAM bytes per launch of the dominant kernel, from the metrics-only ncu capture of the full-size launch
+    committed under profiles/ (profiles/r2_dram_traffic.csv; the .md beside it names the command)."""
+    try:
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv"))):
+            if row["workload"] == workload:
+                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), row["kernel"]
+    except Exception:
+        pass
+    return None, None
+
+
+def measure(name, args, rank, world, local_rank, dist, steps, warmup, want_e2e, want_cpu):
+    """One workload on this rank's share of the instances.  Returns the result dict on rank 0 (None elsewhere)."""
     import torch
     from paper_2505_01616_b200 import binding as B
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    w, per_rank = make_workload(args.workload, world, args.instances)
+    w, per_rank = make_workload(name, world, args.instances)
     mine = shard_instances(w.batch, rank, world)
     first, count = mine[0], len(mine)
     stream = torch.cuda.Stream()
@@ -218,7 +274,8 @@ def run_ours(args, rank, world, local_rank):
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
     # ---- device-resident arm: tables built and uploaded once, each step = phs_run
-    sim = B.Sim.from_workload(w, instances=(first, count), path=args.path, cta_slots=args.gang, windows=not args.no_windows)
+    sim = B.Sim.from_workload(w, instances=(first, count), path=args.path, cta_slots=args.gang,
+                              windows=not args.no_windows)
     sim.finalize(stream=sp)
     flows = sim.total_flows
     colls = sum(w.instances[i].n_collectives for i in mine)
@@ -240,14 +297,14 @@ def run_ours(args, rank, world, local_rank):
         e1.synchronize()
         return e0.elapsed_time(e1), sim.counters()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step()
     barrier()
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
     ms_total, kern_ms, launches = 0.0, 0.0, 0
-    for _ in range(args.steps):
+    for _ in range(steps):
         ms, c = one_step()
         ms_total += ms
         kern_ms += c["main_kernel_ms"]
@@ -256,6 +313,7 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop() if rank == 0 else None
     counters = sim.counters()
     paths = sorted({sim.path_of(i) for i in range(count)})
+    sim.close()
 
     # ---- end-to-end arm: host arrays -> C-ABI submission -> table build -> H2D -> run -> D2H, every step
     def e2e_step():
@@ -268,7 +326,7 @@ def run_ours(args, rank, world, local_rank):
         c = s2.counters()
         s2.close()
         return dt, c["h2d_bytes"], out.nbytes + 40 * count
-    e2e_steps = 0 if args.no_e2e else max(1, min(args.steps, 3))
+    e2e_steps = max(1, min(steps, 3)) if want_e2e else 0
     e2e_s, h2d, d2h = 0.0, 0, 0
     if e2e_steps:
         e2e_step()
@@ -286,60 +344,61 @@ def run_ours(args, rank, world, local_rank):
         dist.all_reduce(work)
     ms_total, e2e_s, kern_ms = tot.tolist()
     flows_all, colls_all, launches_all = work.tolist()
+    del flush_buf
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
+        return None
 
-    value = 2.0 * flows_all * args.steps / (ms_total * 1e-3)
+    value = 2.0 * flows_all * steps / (ms_total * 1e-3)
     e2e_value = 2.0 * flows_all * e2e_steps / e2e_s if e2e_steps else None
+    iters = counters["n_events"]
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64+i64", "data": "synthetic",
-        "config": {"workload": args.workload, "instances_per_gpu": count, "flows_per_gpu": flows,
+        "config": {"workload": name, "instances_per_gpu": count, "flows_per_gpu": flows,
                    "kernel_paths": paths, "l2": "flushed between timed steps (256 MiB write)",
-                   "iterations_per_step": counters["n_events"], "windows_per_step": counters["n_windows"],
+                   "iterations_per_step": iters, "windows_per_step": counters["n_windows"],
                    "lookahead_windows": not args.no_windows,
                    "parallel_rounds_per_step": counters["sum_par_rounds"],
                    "max_active_flows": counters["max_active"], "max_state_slots": counters["max_slots"],
                    "cluster_size": counters["cluster_size"], "clusters_resident": counters["clusters_resident"],
                    "window_gang": counters["window_gang"]},
-        "collectives_per_sec": colls_all * args.steps / (ms_total * 1e-3),
-        "sim_events_per_sec": counters["n_events"] * world * args.steps / (ms_total * 1e-3),
+        "collectives_per_sec": colls_all * steps / (ms_total * 1e-3),
+        "sim_iterations_per_sec": iters * world * steps / (ms_total * 1e-3),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                 "steps": e2e_steps, "note": "host arrays -> phs_add_* -> phs_finalize (H2D) -> phs_run -> D2H"},
         "gpu_launches": int(launches_all),
         "clocks": clocks,
     }
-    # ---- CPU baseline (oracle, bounded sample) and roofline, rank 0 at N=1 only
-    if world == 1 and not args.no_cpu_baseline:
-        n_cpu = {"cfg0": 1, "cfg1": 64, "cfg2": 0, "cfg3": 96, "cfg4": 0}.get(args.workload, 0)
-        golden = os.path.join(ROOT, "tests", "golden", f"{args.workload}_inst0.npz")
+    # ---- CPU baseline (oracle, bounded sample, one pinned core) and roofline, rank 0 at N=1 only
+    if world == 1 and want_cpu:
+        n_cpu = {"cfg0": 1, "cfg1": 64, "cfg2": 0, "cfg3": 96, "cfg4": 0}.get(name, 0)
         wk = None
-        if n_cpu:
-            idx = list(range(min(n_cpu, w.batch)))
-            secs, f_cpu, c_cpu, wk = oracle_time(w, idx)
-            sample = f"instances 0..{len(idx) - 1} of {args.workload} ({f_cpu} flows), oracle fast mode, 1 thread"
-            out["cpu_baseline"] = {"value": 2.0 * f_cpu / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                   "sample": sample, "seconds": secs, "host_cores": os.cpu_count()}
-            # algorithmic bytes of ONE step = the oracle's per-event work counts, scaled to the whole batch
-            scale = flows / float(f_cpu)
-            counted = "counted by the oracle on the cpu_baseline sample and scaled by flows"
-        elif os.path.exists(golden):
-            # cfg2 / cfg4: timed sample = a time prefix of instance 0 (oracle_prefix_time); the work counters of the
-            # FULL oracle run are stored beside the golden values by tests/golden/make_golden.py
-            secs, fe, _ne, sample, g = oracle_prefix_time(w, args.workload)
-            out["cpu_baseline"] = {"value": fe / secs, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
-                                   "seconds": secs, "host_cores": os.cpu_count(),
-                                   "stored_full_run": {"seconds": float(g["oracle_seconds"]), "flows": int(g["n_flows"]),
-                                                       "events": int(g["n_events"]),
-                                                       "note": "whole instance 0, timed where make_golden.py ran "
-                                                               "(another machine): context only"}}
-            wk = dict(zip(g["work_keys"].tolist(), g["work_vals"].tolist()))
-            scale = flows / float(g["n_flows"])
-            counted = ("counted by the oracle over the whole of instance 0 (stored by tests/golden/make_golden.py) "
-                       "and scaled by flows")
+        with PinnedCore() as pin:
+            cpu_info = {"cores": 1, "kind": "oracle", "host_cores": os.cpu_count(), "cpu_model": cpu_model(),
+                        "pinned_to_core": pin.core, "timer": "time.perf_counter around orc_run (ctypes call)"}
+            if n_cpu:
+                idx = list(range(min(n_cpu, w.batch)))
+                secs, f_cpu, c_cpu, wk = oracle_time(w, idx)
+                sample = f"instances 0..{len(idx) - 1} of {name} ({f_cpu} flows), oracle fast mode, 1 thread"
+                out["cpu_baseline"] = dict(cpu_info, value=2.0 * f_cpu / secs, unit=UNIT, sample=sample, seconds=secs)
+                # algorithmic bytes of ONE step = the oracle's per-event work counts, scaled to the whole batch
+                scale = flows / float(f_cpu)
+                counted = "counted by the oracle on the cpu_baseline sample and scaled by flows"
+            elif name in ("cfg2", "cfg4"):
+                # minutes per instance: the timed sample is a time prefix of instance 0 (oracle_prefix_time); the work
+                # counters of the FULL oracle runs of every instance are stored beside the golden values
+                secs, fe, _ne, sample, g = oracle_prefix_time(w, name)
+                out["cpu_baseline"] = dict(cpu_info, value=fe / secs, unit=UNIT, sample=sample, seconds=secs,
+                                           stored_full_run={"seconds": float(g["oracle_seconds"]),
+                                                            "flows": int(g["n_flows"]), "events": int(g["n_events"]),
+                                                            "note": "whole instance 0, timed where make_golden.py ran "
+                                                                    "(another machine): context only"})
+                wk, f_gold = golden_work(name, w.batch)
+                if wk is not None:
+                    scale = flows / float(f_gold)
+                    counted = ("counted by the oracle over the whole of every instance (stored by "
+                               "tests/golden/make_golden.py)")
         if wk is not None:
             alg, survey = algorithmic_bytes(wk)
             peaks = {}
@@ -348,32 +407,70 @@ def run_ours(args, rank, world, local_rank):
             except Exception:
                 pass
             peak = float(peaks.get("hbm_gbs", 6650.0))
-            k_s = (kern_ms / args.steps) * 1e-3
-            traffic = None      # measured DRAM bytes per launch of the dominant kernel (ncu --set full capture)
-            try:
-                import csv
-                for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
-                    if row["workload"] == args.workload:
-                        traffic = float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])
-            except Exception:
-                pass
+            k_s = (kern_ms / steps) * 1e-3
+            traffic, tkernel = measured_traffic(name)
+            kernel = {"cta": "phs_cta_kernel", "cluster": "phs_cluster_kernel", "window": "phs_window_kernel"}
             out["roofline"] = {"bound": "hbm", "achieved": alg * scale / k_s / 1e9, "peak": peak,
                                "unit": "GB/s", "frac": alg * scale / k_s / 1e9 / peak, "traffic": traffic,
+                               "traffic_source": "profiles/r2_dram_traffic.csv (ncu metrics-only capture of this "
+                                                 "full-size launch)" if traffic is not None else None,
                                "peak_source": "MEASURED_PEAKS.json hbm_gbs (measured copy bandwidth)" if peaks
                                else "6650 GB/s (B200_PROFILING.md fallback)",
-                               "kernel": "phs_cta_kernel" if paths == ["cta"] else "+".join(paths),
-                               "kernel_ms": kern_ms / args.steps,
+                               "kernel": "+".join(kernel.get(p, p) for p in paths),
+                               "kernel_ms": kern_ms / steps,
                                "algorithmic_bytes_per_step": alg * scale,
+                               "oracle_events_per_step": wk["events"] * scale,
+                               "us_per_oracle_event": 1e6 * k_s / (wk["events"] * scale) * (count if name != "cfg2" else 1)
+                               if name in ("cfg2", "cfg4") else None,
                                "formula": "sum over events of A(36+20h) + 12*Lambda_act + 40c (DESIGN.md sec 5), "
                                           + counted,
                                "survey_formula": {"bytes_per_step": survey * scale,
                                                   "achieved": survey * scale / k_s / 1e9,
                                                   "note": "SURVEY.md 8(d): link term charged once per sequential "
                                                           "water-filling iteration (12*Lambda_act*R)"},
-                               "note": "state is shared-memory resident: the kernel is bound by the dependent "
-                                       "chain of an event (3 barriers), not by HBM; `traffic` is the measured DRAM "
-                                       "bytes per launch (the one-time table read)"}
-    print(json.dumps(out))
+                               "note": "state is shared-memory resident: the kernels are bound by the dependent "
+                                       "chain of an event, not by HBM; `traffic` is the measured DRAM bytes per "
+                                       "launch (the one-time table read and the result writes)"}
+    return out
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    out = measure(args.workload, args, rank, world, local_rank, dist, args.steps, args.warmup, not args.no_e2e,
+                  not args.no_cpu_baseline)
+    # ---- the other BASELINE.json configs, one short clock-sampled run each (N=1 only): every number of BASELINE.md
+    # sec 4 gets a driver-side twin in the same JSON line
+    if world == 1 and not args.no_per_config and rank == 0:
+        per = {}
+        for name in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg4"):
+            if name == args.workload:
+                continue
+            long_step = name == "cfg4"
+            r = measure(name, args, rank, world, local_rank, None, 1 if long_step else 3, 1, not long_step,
+                        not args.no_cpu_baseline)
+            keep = {k: r[k] for k in ("value", "ms_per_step", "collectives_per_sec", "sim_iterations_per_sec", "steps",
+                                      "warmup", "gpu_launches", "clocks")}
+            keep["flow_events_per_sec"] = keep.pop("value")
+            keep["config"] = {k: r["config"][k] for k in ("instances_per_gpu", "flows_per_gpu", "kernel_paths",
+                                                          "iterations_per_step", "windows_per_step",
+                                                          "parallel_rounds_per_step", "cluster_size",
+                                                          "clusters_resident", "window_gang")}
+            keep["e2e_flow_events_per_sec"] = r["e2e"]["value"]
+            if "roofline" in r:
+                keep["roofline"] = {k: r["roofline"][k] for k in ("frac", "achieved", "peak", "traffic", "kernel",
+                                                                  "kernel_ms", "algorithmic_bytes_per_step")}
+            if "cpu_baseline" in r:
+                keep["cpu_baseline"] = {k: r["cpu_baseline"][k] for k in ("value", "unit", "cores", "sample")}
+            per[name] = keep
+        out["per_config"] = per
+    if rank == 0:
+        print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
@@ -383,7 +480,11 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg1")
+    ap.add_argument("--workload", default="cfg3",
+                    help="BASELINE.json config: cfg0 .. cfg4 (default cfg3, the largest single-GPU configuration: "
+                         "4,096 instances, 29.4 M flows, the one whose tables are HBM-resident)")
+    ap.add_argument("--no-per-config", action="store_true",
+                    help="skip the short runs of the other configs (per_config in the JSON line)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", type=int, default=0,

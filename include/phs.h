@@ -89,6 +89,8 @@ typedef struct {
   int32_t window_gang;   /* CTAs per unit of the window path in the last run (largest gang; 0: path not used)     */
   double main_kernel_ms; /* device time of the simulation kernel(s) of the last phs_run (CUDA events on   */
                          /* the run's stream), excluding the result copies                                */
+  int32_t grid_ctas;     /* CTAs of the cooperative launch of the grid path in the last run (0: path not used)   */
+  int32_t pad_;
   int64_t n_windows;     /* lookahead windows executed (phs_set_windows); = n_events where the window schedule  */
                          /* is off.  n_events then counts window ITERATIONS: one iteration advances every       */
                          /* component that has an event inside the window by one event                          */
@@ -134,8 +136,9 @@ phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);
 /* Batch-scheduler policy; must precede phs_finalize.  path: 0 = automatic (units whose events
  * are dense in simulated time run the lookahead-window schedule on a gang of CTAs; of the others, one CTA per
  * simulation unit with all state in its shared memory when it fits, else one thread-block cluster per unit with the
- * state spread over the shared memory of its CTAs), 1 = CTA path, 2 = cluster path for every unit, 3 = window path
- * for every unit that can run there (positive latency, no event log, no history).  cta_slots > 0 caps the CTA
+ * state spread over the shared memory of its CTAs; a unit that fits no cluster is simulated by the whole grid with
+ * its state in global memory), 1 = CTA path, 2 = cluster path for every unit, 3 = window path for every unit that
+ * can run there (positive latency, no event log, no history), 4 = grid path for every unit (no event log).  cta_slots > 0 caps the CTA
  * path's shared-memory slot count (flows PENDING or ACTIVE at once per unit); a unit that exceeds it is re-run on
  * the cluster path.  With path = 3, cta_slots is instead the smallest gang (CTAs per unit: 1, 2, 4, 8, 16) to use
  * for units that have enough components. */
@@ -206,7 +209,7 @@ phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int
 phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,
                               double *latency_s, int64_t n);
 phs_status phs_get_counters(const phs_sim *sim, phs_counters *out);
-/* Name of the kernel path the last run used for the largest unit of `instance`: "cta", "cluster" or "window". */
+/* Name of the kernel path the last run used for the largest unit of `instance`: "cta", "cluster", "window", "grid". */
 const char *phs_instance_path(const phs_sim *sim, int32_t instance);
 const char *phs_last_error(void); /* thread-local; valid until the next call on this thread */
 

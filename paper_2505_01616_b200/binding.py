@@ -31,7 +31,7 @@ class Counters(C.Structure):
                 ("sum_par_rounds", C.c_int64), ("n_kernel_launches", C.c_int64), ("h2d_bytes", C.c_int64),
                 ("max_active", C.c_int32), ("max_slots", C.c_int32), ("cluster_size", C.c_int32),
                 ("clusters_resident", C.c_int32), ("resumed_units", C.c_int32), ("window_gang", C.c_int32),
-                ("main_kernel_ms", C.c_double), ("n_windows", C.c_int64)]
+                ("main_kernel_ms", C.c_double), ("grid_ctas", C.c_int32), ("pad_", C.c_int32), ("n_windows", C.c_int64)]
 
 
 EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<i4"), ("n_rounds", "<i4"),

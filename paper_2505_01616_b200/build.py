@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libphs.so")
-SOURCES = ["phs_api.cu", "phs_schedule.cu", "phs_build.cpp", "phs_kernels.cu", "phs_cluster.cu", "phs_window.cu"]
+SOURCES = ["phs_api.cu", "phs_schedule.cu", "phs_build.cpp", "phs_kernels.cu", "phs_cluster.cu", "phs_window.cu", "phs_grid.cu"]
 HEADERS = ["phs_internal.h", "phs_device.h", "phs_devutil.cuh", "phs_sim.h", os.path.join("..", "..", "include", "phs.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "-Xcompiler", "-fPIC,-O2,-ffp-contract=off", "-shared", "-cudart", "static"]

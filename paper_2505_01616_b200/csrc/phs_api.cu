@@ -197,7 +197,7 @@ phs_status phs_enable_event_log(phs_sim *sim, int32_t enable) {
 phs_status phs_set_scheduler(phs_sim *sim, int32_t path, int32_t cta_slots) {
   PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
-  if (path < 0 || path > 3 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
+  if (path < 0 || path > 4 || cta_slots < 0) return fail(PHS_EINVAL, "bad scheduler policy");
   if (sim->finalized) return fail(PHS_ESTATE, "scheduler policy must be chosen before phs_finalize");
   sim->policy_path = path;
   sim->policy_slots = cta_slots;
@@ -458,6 +458,7 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   }
   c.cluster_size = sim->scratch_cs;
   c.window_gang = sim->win_gang_used;
+  c.grid_ctas = sim->grid_ctas;
   c.clusters_resident = sim->clusters_resident;
   c.resumed_units = sim->resumed_units;
   c.n_flow_events = 2 * sim->total_flows;
@@ -474,7 +475,9 @@ const char *phs_instance_path(const phs_sim *sim, int32_t instance) {
   int best = sim->unit_first[instance];  // the path of the instance's largest unit
   for (int u = best; u < sim->unit_first[instance + 1]; ++u)
     if (sim->units[u].n_flows > sim->units[best].n_flows) best = u;
-  return sim->h_res[best].path == 0 ? "cta" : sim->h_res[best].path == 1 ? "cluster" : "window";
+  static const char *names[] = {"cta", "cluster", "window", "grid"};
+  const int pth = sim->h_res[best].path;
+  return pth >= 0 && pth < 4 ? names[pth] : "";
 }
 
 }  // extern "C"

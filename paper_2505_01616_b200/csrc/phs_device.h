@@ -120,6 +120,15 @@ cudaError_t window_max_clusters(int gang, size_t smem, int *max_clusters);
 cudaError_t launch_window_path(const DevTables &t, const int32_t *list, int n, int *ticket, const WindowLaunch &w,
                                int n_clusters, cudaStream_t stream);
 
+// Grid path (phs_grid.cu): the whole grid (cooperative launch, n_ctas CTAs of kGridThreads threads) simulates the
+// units of list[0..n) one after the other; per-flow and per-link state in `scratch` (grid_scratch_bytes for the
+// largest unit of the list).
+constexpr int kGridThreads = 512;
+size_t grid_scratch_bytes(int64_t n_flows, int n_links);
+cudaError_t grid_max_ctas(int *n_ctas);
+cudaError_t launch_grid_path(const DevTables &t, const int32_t *list, int n, unsigned char *scratch, int64_t max_flows,
+                             int max_links, int n_ctas, cudaStream_t stream);
+
 // out[c] = max t_done over the flows of collective c, for all collectives of all instances.
 cudaError_t launch_collective_times(const double *t_done, const int64_t *coll_first, const int32_t *coll_nflows,
                                     int64_t n_colls, double *out, cudaStream_t stream);

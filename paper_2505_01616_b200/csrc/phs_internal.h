@@ -58,7 +58,7 @@ struct InstDesc {
 // Per-instance result block (device, read back after a run).
 struct InstResult {
   int32_t status;          // PHS_OK, PHS_ECYCLE, or kOverflow (re-run on the cluster path)
-  int32_t path;            // 0 = cta, 1 = cluster, 2 = window
+  int32_t path;            // 0 = cta, 1 = cluster, 2 = window, 3 = grid
   int64_t n_events;
   int64_t sum_active;
   int64_t sum_par_rounds;

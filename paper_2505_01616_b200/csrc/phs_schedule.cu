@@ -24,6 +24,7 @@ StagingArea &staging_area() {
 }  // namespace phs
 
 #define fail phs_fail
+#define PHS_DBG(...) do { if (getenv("PHS_DEBUG")) { fprintf(stderr, "[phs dbg] " __VA_ARGS__); fputc('\n', stderr); fflush(stderr); } } while (0)
 
 // ================================================================================================ window path plan
 namespace {
@@ -397,13 +398,18 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         std::vector<double> end_of(in.colls.size(), 0.0);
         for (size_t ci = 0; ci < in.colls.size(); ++ci) {
           const Collective &co = in.colls[ci];
-          if (co.n_flows == 0 || unit_of[co.first_flow] != u) continue;
+          if (co.n_flows == 0) continue;
+          bool here = false;  // an all-to-all may be split over several units (intra-host / inter-host links)
+          for (int32_t f = co.first_flow; f < co.first_flow + co.n_flows; ++f)
+            if (unit_of[f] == u) {
+              in_coll[(size_t)flow_loc[f]] = 1;
+              here = true;
+            }
           double begin = co.start;
           for (int32_t a : co.after) begin = std::max(begin, end_of[(size_t)a]);
           const double chunk = co.bytes / (double)co.n_ranks;
           end_of[ci] = begin + (double)co.steps * (in.lat[co.first_flow] + chunk / capmax);
-          span = std::max(span, end_of[ci]);
-          for (int32_t f = co.first_flow; f < co.first_flow + co.n_flows; ++f) in_coll[(size_t)flow_loc[f]] = 1;
+          if (here) span = std::max(span, end_of[ci]);
         }
         for (size_t k = 0; k < fl.size(); ++k)
           if (!in_coll[k]) span = std::max(span, in.start[fl[k]] + in.lat[fl[k]] + in.bytes[fl[k]] / capmax);
@@ -562,6 +568,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   const bool log = sim->want_log;
   sim->order.clear();
   sim->cluster_list.clear();
+  sim->grid_list.clear();
   sim->cta = CtaLaunch{};
   auto need_of = [&](const phs_sim::Unit &u) {
     return (int)std::min<int64_t>(std::min<int64_t>(std::max<int64_t>(u.n_flows, 1), std::max<int64_t>(u.bound_cta, 32)), 1 << 16);
@@ -571,6 +578,10 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const phs_sim::Unit &un = sim->units[u];
     if (un.n_flows == 0) continue;  // nothing to simulate; its result block stays zero (status OK)
     if (un.win_gang > 0) continue;  // runs on the window path
+    if (sim->policy_path == 4 && !log) {  // phs_set_scheduler: the whole grid for every unit
+      sim->grid_list.push_back(u);
+      continue;
+    }
     if (sim->policy_path == 2 || un.n_links >= 65535 ||
         cta_smem_bytes(un.n_links, (need_of(un) + 31) / 32 * 32, 0, log) > smem_max)
       sim->cluster_list.push_back(u);
@@ -708,8 +719,9 @@ DevTables tables_of(phs_sim *sim, int n_links) {
 // Cluster path (a9): every instance in `list` is simulated by one thread-block cluster with all dynamic state in
 // the shared memory of its CTAs; clusters pull instances from the list until it is empty.  `slot_scale` scales the
 // guess of how many flows are PENDING or ACTIVE at once (doubled after an overflow).
-phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int64_t slot_scale, bool park,
-                            bool resume, cudaStream_t st) {
+phs_status run_cluster_path(phs_sim *sim, std::vector<int32_t> list, int64_t slot_scale, bool park, bool resume,
+                            cudaStream_t st, std::vector<int32_t> *too_big) {
+retry:
   if (list.empty()) return PHS_OK;
   int L = 1;  // the shared-memory layout is sized for the unit with the most links
   for (int u : list) L = std::max(L, sim->units[u].n_links);
@@ -752,8 +764,20 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
       max_clusters = n;
     }
   }
-  if (!cs)
-    return fail(PHS_ERANGE, "cluster path: the instance's pending + active flows do not fit the shared memory of a cluster");
+  if (!cs) {
+    // the unit with the most concurrent flows fits no cluster: the whole grid simulates it, with its state in global
+    // memory (grid path); the event log is not written there
+    if (log)
+      return fail(PHS_ERANGE, "a unit's pending + active flows do not fit the shared memory of a cluster, and the grid "
+                              "path does not write the event log");
+    auto big = std::max_element(list.begin(), list.end(), [&](int a, int b) {
+      const phs_sim::Unit &x = sim->units[(size_t)a], &y = sim->units[(size_t)b];
+      return x.bound_whole + (x.bound - x.bound_whole) / 4 < y.bound_whole + (y.bound - y.bound_whole) / 4;
+    });
+    too_big->push_back(*big);
+    list.erase(big);
+    goto retry;
+  }
   const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
   const size_t region = cold ? 0 : cluster_region_bytes(Sc, cs);
   if (region * n_clusters > sim->g_scratch.n) PHS_CUDA(sim->g_scratch.alloc(region * n_clusters));
@@ -815,6 +839,34 @@ phs_status run_cluster_path(phs_sim *sim, const std::vector<int32_t> &list, int6
   return PHS_OK;
 }
 
+
+// Grid path (a9): the whole grid (cooperative launch) simulates the units of `list` one after the other.
+phs_status run_grid_path(phs_sim *sim, const std::vector<int32_t> &list, cudaStream_t st) {
+  if (list.empty()) return PHS_OK;
+  int64_t Fm = 1;
+  int Lm = 1;
+  for (int u : list) {
+    Fm = std::max<int64_t>(Fm, sim->units[(size_t)u].n_flows);
+    Lm = std::max(Lm, sim->units[(size_t)u].n_links);
+  }
+  const size_t bytes = grid_scratch_bytes(Fm, Lm);
+  PHS_DBG("grid path: %d units, Fm %lld Lm %d scratch %zu", (int)list.size(), (long long)Fm, Lm, bytes);
+  if (bytes > sim->d_gscratch.n) PHS_CUDA(sim->d_gscratch.alloc(bytes));
+  int n_ctas = 0;
+  PHS_CUDA(grid_max_ctas(&n_ctas));
+  PHS_DBG("grid path: max ctas %d", n_ctas);
+  if (n_ctas < 1) return fail(PHS_ECUDA, "grid path: the kernel cannot be resident");
+  // no more CTAs than the largest unit can use (one flow per thread)
+  n_ctas = (int)std::max<int64_t>(1, std::min<int64_t>(n_ctas, (Fm + kGridThreads - 1) / kGridThreads));
+  PHS_CUDA(sim->d_glist.upload(list, st));
+  PHS_CUDA(launch_grid_path(tables_of(sim, Lm), sim->d_glist.p, (int)list.size(), sim->d_gscratch.p, Fm, Lm, n_ctas, st));
+  PHS_DBG("grid path: launched");
+  PHS_CUDA(cudaStreamSynchronize(st));  // `list` may be pageable host memory read by the async copy
+  PHS_DBG("grid path: done");
+  sim->grid_ctas = n_ctas;
+  sim->n_launches++;
+  return PHS_OK;
+}
 
 // Window path (a9): the units of `todo` run the lookahead-window schedule, one gang of CTAs each; gangs of one size
 // share a launch.  Units that run out of slots are planned again with a larger estimate (possibly a larger gang);
@@ -915,6 +967,8 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   }
   sim->last_stream = st;
   const int U = (int)sim->units.size();
+  PHS_DBG("run: %d units, cta %d cluster %d window %d grid %d", U, (int)sim->order.size(), (int)sim->cluster_list.size(),
+          (int)sim->win_list.size(), (int)sim->grid_list.size());
   const bool finite = std::isfinite(sim->t_stop);
   // Resume: a run that stopped at an earlier time left its units parked (shared memory + registers in global
   // memory); a later stop time continues them from there.  When the time goes backwards (or a unit changed its
@@ -1005,8 +1059,16 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   std::vector<int32_t> todo(cluster_todo);
   for (int64_t scale = sim->cluster_scale; !todo.empty(); scale *= 2) {
     PHS_CUDA(cudaEventRecord(sim->ev0, st));
-    phs_status gs = run_cluster_path(sim, todo, scale, finite, resume, st);
+    std::vector<int32_t> too_big;
+    PHS_DBG("cluster path: %d units, scale %lld", (int)todo.size(), (long long)scale);
+    phs_status gs = run_cluster_path(sim, todo, scale, finite, resume, st, &too_big);
+    PHS_DBG("cluster path: returned %d, %d too big", (int)gs, (int)too_big.size());
     if (gs != PHS_OK) return gs;
+    for (int u : too_big) {  // for good: later runs go straight to the grid path
+      sim->grid_list.push_back(u);
+      sim->cluster_list.erase(std::remove(sim->cluster_list.begin(), sim->cluster_list.end(), u), sim->cluster_list.end());
+      todo.erase(std::remove(todo.begin(), todo.end(), u), todo.end());
+    }
     sim->n_launches++;
     PHS_CUDA(cudaEventRecord(sim->ev1, st));
     PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
@@ -1022,6 +1084,20 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
       sim->cluster_scale = scale * 2;  // remember for later runs
     }
     todo.swap(again);
+  }
+  // grid path: units that fit no cluster.  They keep no parked state: a later phs_run_until starts them again from
+  // t = 0 (deterministic, same results).
+  sim->grid_ctas = 0;
+  if (!sim->grid_list.empty()) {
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
+    phs_status gs = run_grid_path(sim, sim->grid_list, st);
+    if (gs != PHS_OK) return gs;
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * U, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    float extra = 0.f;
+    PHS_CUDA(cudaEventElapsedTime(&extra, sim->ev0, sim->ev1));
+    sim->main_kernel_ms += extra;
   }
   if (sim->total_colls > 0) sim->n_launches++;
   PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,

@@ -182,6 +182,11 @@ struct phs_sim {
   std::vector<phs::InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first
   std::vector<int32_t> cluster_list;  // instances that go (or fell back) to the cluster path
+  // grid path: units that fit no cluster (or all of them under phs_set_scheduler path 4), and its scratch
+  std::vector<int32_t> grid_list;
+  phs::DevBuf<unsigned char> d_gscratch;
+  phs::DevBuf<int32_t> d_glist;
+  int grid_ctas = 0;
   // window path: its units, and the ownership tables of their gangs (identity for everybody else)
   std::vector<int32_t> win_list;
   std::vector<int32_t> comp_flows, comp_links, h_lcomp;  // per component: flows, links; per link: its component

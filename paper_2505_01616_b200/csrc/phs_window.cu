@@ -509,43 +509,26 @@ __global__ void __launch_bounds__(kWindowThreads, 1)
             }
           }
 #pragma unroll
-          for (int h = 0; h < kMaxHops; ++h)
-            if (p[h] != (int)kNoLink && p[h] != arg) S.l_beat[p[h]] = g;
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = p[h];
+            if (l == (int)kNoLink) continue;
+            if (l != arg) S.l_beat[l] = g;
+            // working state of the solve's links (idempotent stores; debited from F0 on, after the barrier)
+            S.l_caprem[l] = S.l_cap[l];
+            S.l_nw[l] = S.l_n0[l];
+            S.l_sharew[l] = sh[h];
+          }
           S.s_meta[s].w = arg;
         }
         __syncthreads();
         bool left = false;
-        for (int s = tid; s < hi; s += NT) {  // F0: unbeaten arg-min links freeze their flows (a7), fold (a8)
+        for (int s = tid; s < hi; s += NT) {  // F0: unbeaten arg-min links freeze their flows and debit (a7), fold (a8)
           const int4 m = S.s_meta[s];
           if (m.x < 0 || m.y != -1) continue;  // only flows V0 opened are unfrozen here
           if (S.l_beat[m.w] != g) {
-            freeze(s, m.w, S.l_share0[m.w], S.c_now[m.z]);
+            const long long rq = S.l_share0[m.w];
+            freeze(s, m.w, rq, S.c_now[m.z]);
             smem_min_f64(&S.c_next[m.z], S.s_tc[s]);
-          } else {
-            left = true;
-          }
-        }
-        left = __syncthreads_or(left);
-        PHS_TICK(8)
-        if (left) {
-          for (int s = tid; s < hi; s += NT) {  // I: working capacities of the links of this solve
-            const int4 m = S.s_meta[s];
-            if (m.x < 0 || m.y == -2 || S.c_solve[m.z] != solve) continue;
-            const uint4 pv = S.s_path[s];
-#pragma unroll
-            for (int h = 0; h < kMaxHops; ++h) {
-              const int l = path_at(pv, h);
-              if (l == (int)kNoLink) continue;
-              S.l_caprem[l] = S.l_cap[l];
-              S.l_nw[l] = S.l_n0[l];
-              S.l_sharew[l] = S.l_share0[l];
-            }
-          }
-          __syncthreads();
-          for (int s = tid; s < hi; s += NT) {  // D: flows frozen in the first round debit their paths
-            const int4 m = S.s_meta[s];
-            if (m.x < 0 || m.y < 0 || S.c_solve[m.z] != solve) continue;
-            const long long rq = S.s_rq[s];
             const uint4 pv = S.s_path[s];
 #pragma unroll
             for (int h = 0; h < kMaxHops; ++h) {
@@ -557,8 +540,13 @@ __global__ void __launch_bounds__(kWindowThreads, 1)
                 S.l_deb[l] = g;
               }
             }
+          } else {
+            left = true;
           }
-          __syncthreads();
+        }
+        left = __syncthreads_or(left);
+        PHS_TICK(8)
+        if (left) {
           for (;;) {
             ++g;
             ++rounds;

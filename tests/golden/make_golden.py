@@ -5,7 +5,7 @@ Calls ONLY the CPU oracle (oracle/, fast mode) on the seeded inputs of paper_250
 here touches the CUDA path.  One instance takes ~5 min (cfg4) or ~12 min (cfg2) of one CPU core; the instances
 of cfg4 run as separate processes.
 
-    python tests/golden/make_golden.py [cfg4] [cfg2] [cfg4:3]        # cfg4:3 = only instance 3 of cfg4
+    python tests/golden/make_golden.py [cfg4] [cfg2] [a2a304] [cfg4:3]        # cfg4:3 = only instance 3 of cfg4
 
 Per instance the file holds: 4096 sampled flows (index, completion time, bottleneck), the SHA-256 of ALL completion
 times, of ALL bottleneck ids and of the `t` column of the event log, the event count, the oracle's work counters
@@ -31,8 +31,13 @@ from util import oracle_run  # noqa: E402
 CFG4_BATCH = 8
 
 
+def a2a304():
+    """A unit that fits no 16-CTA cluster (grid path): cfg4's recipe on 304 GPUs = 92,112 concurrent flows."""
+    return W.cfg4(batch=1, n_hosts=38, gph=8, n_leaves=2, n_spines=4)
+
+
 def make(name, inst):
-    w = W.cfg4(batch=CFG4_BATCH) if name == "cfg4" else W.cfg2()
+    w = W.cfg4(batch=CFG4_BATCH) if name == "cfg4" else a2a304() if name == "a2a304" else W.cfg2()
     t0 = time.time()
     o = oracle_run(w.desc, w.instances[inst], mode=orc.MODE_FAST, base_seed=w.base_seed)
     t = o.completion_times()

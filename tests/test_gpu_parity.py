@@ -16,7 +16,7 @@ from util import completion_order, oracle_build, oracle_run
 pytestmark = pytest.mark.gpu
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
-CTA, CLUSTER, WINDOW = 1, 2, 3
+CTA, CLUSTER, WINDOW, GRID = 1, 2, 3, 4
 
 
 def assert_instance_matches(sim, i, o, check_log=True):
@@ -312,15 +312,64 @@ def test_cfg2_full_size_as_benchmarked():
     sim.close()
 
 
-def test_unit_larger_than_a_cluster_is_refused_not_silently_wrong():
-    """The cluster path keeps all dynamic state on chip; an instance whose concurrent flows exceed the shared memory
-    of 16 SMs is refused with PHS_ERANGE (there is no CPU or global-memory fallback)."""
+def _grid_compare(w, first=0, count=None, decompose=False):
+    """The grid path (forced: phs_set_scheduler path 4; it does not write the event log) against the oracle."""
+    count = w.batch if count is None else count
+    sim = B.Sim.from_workload(w, instances=(first, count), path=GRID, decompose=decompose)
+    sim.run()
+    c = sim.counters()
+    assert c["grid_ctas"] >= 1
+    for i in range(count):
+        o = oracle_run(w.desc, w.instances[first + i], mode=orc.MODE_FAST, base_seed=w.base_seed)
+        assert_instance_matches(sim, i, o, check_log=False)
+        assert sim.path_of(i) == "grid"
+    sim.close()
+
+
+def test_grid_path_small_configs():
+    _grid_compare(W.cfg0())
+    _grid_compare(W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2))
+    _grid_compare(W.cfg3(batch=2), decompose=True)            # several units, one after the other
+    _grid_compare(W.cfg2(k=4, agg_uplinks=1))
+    _grid_compare(W.cfg4(batch=1, n_hosts=8, gph=8, n_leaves=4, n_spines=2))      # many rounds per event
+
+
+def test_unit_larger_than_a_cluster_runs_on_the_whole_grid():
+    """BASELINE.json north_star: "the whole grid to each large instance".  A unit whose concurrent flows exceed the
+    shared memory of 16 SMs used to be refused (PHS_ERANGE); the scheduler now hands it to the grid path.  Uniform
+    304-GPU all-to-all (92,112 concurrent flows, P8: every flow B/(N-1)) against the oracle run live."""
     d = W.topo_desc(W.TOPO_SINGLE, 38, 8)                      # 304 GPUs on one switch
+    ranks = np.arange(304, dtype=np.int32)
     sim = B.Sim(d, batch=1)
-    B.phs_add_collective(sim.h, 0, B.ALLTOALL, np.arange(304, dtype=np.int32), 304e6)   # 92,112 concurrent flows
+    B.phs_add_collective(sim.h, 0, B.ALLTOALL, ranks, 304e6)
+    sim.run()
+    assert sim.path_of(0) == "grid" and sim.counters()["grid_ctas"] > 100
+    o = orc.Sim(d, 0)
+    o.add_collective(orc.ALLTOALL, ranks, 304e6)
+    o.run(mode=orc.MODE_FAST)
+    assert_instance_matches(sim, 0, o, check_log=False)
+    sim.run()                                                   # later runs go straight to the grid path
+    assert_instance_matches(sim, 0, o, check_log=False)
+    sim.close()
+    with_log = B.Sim(d, batch=1, event_log=True)                # the grid path does not write the event log
+    B.phs_add_collective(with_log.h, 0, B.ALLTOALL, ranks, 304e6)
     with pytest.raises(B.PhsError) as e:
-        sim.run()
+        with_log.run()
     assert e.value.code == B.PHS_ERANGE
+    with_log.close()
+
+
+def test_grid_path_skewed_alltoall_92k_flows_against_stored_oracle():
+    """cfg4's recipe on 304 GPUs: 92,112 concurrent Zipf-skewed flows, ~92 K events with many filling rounds each --
+    fits no cluster.  Expected values written by tests/golden/make_golden.py a2a304 (oracle only)."""
+    path = os.path.join(GOLD, "a2a304_inst0.npz")
+    if not os.path.exists(path):
+        pytest.skip("golden file not generated")
+    w = W.cfg4(batch=1, n_hosts=38, gph=8, n_leaves=2, n_spines=4)
+    sim = B.Sim.from_workload(w, decompose=False)
+    sim.run()
+    assert sim.path_of(0) == "grid"
+    _check_against_golden(sim, 0, _golden("a2a304_inst0.npz"))
     sim.close()
 
 
