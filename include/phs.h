@@ -45,7 +45,13 @@ typedef enum {
   PHS_ALLREDUCE_RING = 0,     /* 2(N-1) steps of N flows, chunk = bytes/N      */
   PHS_ALLGATHER_RING = 1,     /* (N-1) steps; bytes = total gathered size      */
   PHS_REDUCESCATTER_RING = 2, /* (N-1) steps; bytes = total input size         */
-  PHS_ALLTOALL = 3            /* N(N-1) concurrent flows of bytes/N            */
+  PHS_ALLTOALL = 3,           /* N(N-1) concurrent flows of bytes/N            */
+  /* further collective algorithms ("the communication patterns of different collective operations"),
+   * with C = `chunks` pipeline chunks of bytes/C (phs_add_collective_ex): */
+  PHS_BROADCAST_CHAIN = 4,    /* root ranks[0]; hop i: ranks[i] -> ranks[i+1]; C(N-1) flows, chunk-major        */
+  PHS_REDUCE_CHAIN = 5,       /* towards the root: hop i: ranks[N-1-i] -> ranks[N-2-i]                           */
+  PHS_ALLREDUCE_TREE = 6      /* binary tree in heap order over the ranks: per chunk N-1 up flows (child ->      */
+                              /* parent), then N-1 down flows; 2C(N-1) flows                                      */
 } phs_coll_kind;
 
 /* Topology descriptor (S1).  GPU g = host*gpus_per_host + local.  Every physical link is two
@@ -119,6 +125,14 @@ phs_status phs_set_link_capacities_batch(phs_sim *sim, const double *cap_Bps);
 phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                               double bytes, double start_time_s, const int32_t *after_coll_ids, int32_t n_after,
                               int32_t *out_coll_id);
+/* The same with `chunks` >= 1 pipeline chunks for the chain and tree kinds (must be 1 for the ring kinds and the
+ * all-to-all).  A flow of chunk c on a hop waits for the previous hop's flow of chunk c (the data is there) and for
+ * the same hop's flow of chunk c-1 (FIFO per connection); S3 gives ids and dependencies.  `start_time_s` and
+ * the `after` edges apply to every flow without a predecessor inside the collective; as an `after` target such a
+ * collective contributes, per rank, the flows of its last chunk the rank sends or receives. */
+phs_status phs_add_collective_ex(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                 double bytes, double start_time_s, const int32_t *after_coll_ids, int32_t n_after,
+                                 int32_t chunks, int32_t *out_coll_id);
 /* Same collective on EVERY instance with per-instance sizes / start times: bytes[batch], start_time_s[batch]
  * (nullable = 0). */
 phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *ranks, int32_t n_ranks,

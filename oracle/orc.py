@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 OK, EINVAL, ENOMEM, ECYCLE, ESTATE, ERANGE = 0, -1, -2, -4, -5, -6
 TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE = 0, 1, 2
 ALLREDUCE_RING, ALLGATHER_RING, REDUCESCATTER_RING, ALLTOALL = 0, 1, 2, 3
+BROADCAST_CHAIN, REDUCE_CHAIN, ALLREDUCE_TREE = 4, 5, 6
 MODE_NAIVE, MODE_FAST = 0, 1
 FLAG_SETTLE_EVERY_EVENT, FLAG_F64_SHARES = 1, 2     # orc_run_ex: SURVEY.md 8(c) S4.4 / S5 as written (see orc_netsim.h)
 
@@ -123,14 +124,14 @@ class Sim:
         _chk(lib().orc_get_link_capacities(self._h, _p(cap, C.c_double)), "orc_get_link_capacities")
         return cap
 
-    def add_collective(self, kind, ranks, nbytes, start=0.0, after=()):
+    def add_collective(self, kind, ranks, nbytes, start=0.0, after=(), chunks=1):
         ranks = np.ascontiguousarray(ranks, dtype=np.int32)
         after = np.ascontiguousarray(after, dtype=np.int32)
         cid = C.c_int32()
-        _chk(lib().orc_add_collective(self._h, C.c_int32(kind), _p(ranks, C.c_int32), C.c_int32(len(ranks)),
-                                      C.c_double(nbytes), C.c_double(start),
-                                      _p(after, C.c_int32) if len(after) else None, C.c_int32(len(after)),
-                                      C.byref(cid)), "orc_add_collective")
+        _chk(lib().orc_add_collective_ex(self._h, C.c_int32(kind), _p(ranks, C.c_int32), C.c_int32(len(ranks)),
+                                         C.c_double(nbytes), C.c_double(start),
+                                         _p(after, C.c_int32) if len(after) else None, C.c_int32(len(after)),
+                                         C.c_int32(chunks), C.byref(cid)), "orc_add_collective_ex")
         return cid.value
 
     def add_flows(self, src, dst, nbytes, start=None, dep_off=None, dep_ids=None, conn_id=None):

@@ -19,6 +19,7 @@ enum { WAITING = 0, PENDING = 1, ACTIVE = 2, DONE = 3 };
 
 typedef struct {
   int32_t kind, n, first_flow, n_flows, steps;
+  int32_t chunks; /* pipeline chunks of the chain / tree kinds (1 for the ring kinds and the all-to-all) */
   int32_t *ranks;
 } coll_t;
 
@@ -274,12 +275,60 @@ static int32_t ring_index_of(const coll_t *c, int32_t rho) {
   return -1;
 }
 
+/* S3, `after` edges.  F_A(rho) = the flows of collective A that must have finished before rank rho may start a
+ * later collective: ring kinds: A's last-step flow sent by rho and the one received by rho; all-to-all: every flow
+ * from / to rho; chain and tree kinds: the flows of A's LAST chunk that rho sends or receives.  rho not in A: none.
+ * The flows of A are in the flow table already, so the chain / tree case simply looks at their endpoints. */
+static int push_after_edges(orc_sim *s, const int32_t *after, int32_t n_after, int32_t rho) {
+  for (int32_t a = 0; a < n_after; a++) {
+    const coll_t *A = &s->coll[after[a]];
+    int32_t ia = ring_index_of(A, rho);
+    if (ia < 0) continue;
+    if (A->kind == ORC_ALLTOALL) {
+      for (int32_t x = 0; x < A->n; x++) {
+        if (x == ia) continue;
+        /* flow ia->x is entry (ia, x) of the row-major list without the diagonal */
+        if (push_pred(s, A->first_flow + ia * (A->n - 1) + (x < ia ? x : x - 1))) return -1;
+        if (push_pred(s, A->first_flow + x * (A->n - 1) + (ia < x ? ia : ia - 1))) return -1;
+      }
+    } else if (A->kind <= ORC_REDUCESCATTER_RING) {
+      int32_t last = A->first_flow + (A->steps - 1) * A->n;
+      if (push_pred(s, last + ia)) return -1;                    /* sent by rho */
+      if (push_pred(s, last + (ia + A->n - 1) % A->n)) return -1; /* received by rho */
+    } else {
+      int32_t per_chunk = A->n_flows / A->chunks;
+      for (int32_t f = A->first_flow + (A->chunks - 1) * per_chunk; f < A->first_flow + A->n_flows; f++)
+        if (s->src[f] == rho || s->dst[f] == rho)
+          if (push_pred(s, f)) return -1;
+    }
+  }
+  return 0;
+}
+
 int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t N, double bytes, double start,
                            const int32_t *after, int32_t n_after, int32_t *out_id) {
+  return orc_add_collective_ex(s, kind, ranks, N, bytes, start, after, n_after, 1, out_id);
+}
+
+/* S3 with the NEXT-3 kinds ("the communication patterns of different collective operations").
+ * `chunks` = C >= 1 pipeline chunks of the chain / tree kinds (must be 1 for the ring kinds and the all-to-all):
+ *   ORC_BROADCAST_CHAIN   root r[0]; hop i = 0..N-2 is r[i] -> r[i+1]; flow (c, i), id first + c (N-1) + i, carries
+ *                         bytes / C; it waits for (c, i-1) (the chunk has arrived at r[i]) and (c-1, i) (sender FIFO).
+ *   ORC_REDUCE_CHAIN      the same towards the root: hop i is r[N-1-i] -> r[N-2-i].
+ *   ORC_ALLREDUCE_TREE    binary tree in heap order over the positions (parent(i) = (i-1)/2); per chunk c a block of
+ *                         2 (N-1) flows: up(c, i), i = 1..N-1, id first + c 2(N-1) + (i-1), r[i] -> r[parent(i)],
+ *                         waits for up(c, 2i+1), up(c, 2i+2) (the subtree's partial sums) and up(c-1, i) (FIFO);
+ *                         down(c, i), id first + c 2(N-1) + (N-1) + (i-1), r[parent(i)] -> r[i], waits for
+ *                         down(c, parent(i)) -- or, below the root, for up(c, 1) and up(c, 2) -- and down(c-1, i).
+ * `start` and the `after` edges apply to every flow that has no predecessor inside the collective. */
+int32_t orc_add_collective_ex(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t N, double bytes, double start,
+                              const int32_t *after, int32_t n_after, int32_t chunks, int32_t *out_id) {
   if (!s || !ranks) return ORC_EINVAL;
   if (s->ran) return ORC_ESTATE;
-  if (kind < 0 || kind > 3 || N < 2 || !(bytes > 0) || !(bytes < INFINITY) || !(start >= 0) || !(start < INFINITY))
+  if (kind < 0 || kind > ORC_ALLREDUCE_TREE || N < 2 || !(bytes > 0) || !(bytes < INFINITY) || !(start >= 0) ||
+      !(start < INFINITY))
     return ORC_EINVAL;
+  if (chunks < 1 || chunks > 65536 || (kind <= ORC_ALLTOALL && chunks != 1)) return ORC_EINVAL;
   if (n_after < 0 || (n_after > 0 && !after)) return ORC_EINVAL;
   for (int32_t i = 0; i < N; i++) {
     if (ranks[i] < 0 || ranks[i] >= s->G) return ORC_EINVAL;
@@ -289,7 +338,10 @@ int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32
   for (int32_t a = 0; a < n_after; a++)
     if (after[a] < 0 || after[a] >= s->n_coll) return ORC_EINVAL;
   int32_t S = coll_steps(kind, N);
-  int64_t nf = kind == ORC_ALLTOALL ? (int64_t)N * (N - 1) : (int64_t)S * N;
+  int64_t nf = kind == ORC_ALLTOALL ? (int64_t)N * (N - 1)
+             : kind == ORC_ALLREDUCE_TREE ? (int64_t)chunks * 2 * (N - 1)
+             : kind >= ORC_BROADCAST_CHAIN ? (int64_t)chunks * (N - 1)
+                                           : (int64_t)S * N;
   if (s->F + nf > 0x7ffffff0) return ORC_ERANGE;
   if (s->n_coll == s->coll_cap) {
     int32_t c = s->coll_cap ? 2 * s->coll_cap : 16;
@@ -300,36 +352,16 @@ int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32
   }
   int32_t cid = s->n_coll;
   coll_t *c = &s->coll[cid];
-  c->kind = kind; c->n = N; c->first_flow = (int32_t)s->F; c->n_flows = (int32_t)nf; c->steps = S;
+  c->kind = kind; c->n = N; c->first_flow = (int32_t)s->F; c->n_flows = (int32_t)nf; c->steps = S; c->chunks = chunks;
   c->ranks = (int32_t *)malloc(sizeof(int32_t) * N);
   if (!c->ranks) return ORC_ENOMEM;
   memcpy(c->ranks, ranks, sizeof(int32_t) * N);
   s->n_coll++; /* (ranks now owned by the table) */
-  double chunk = bytes / (double)N; /* S3: one f64 division */
   int32_t first = c->first_flow;
-
-  /* `after` edges for an initial flow whose sender is rho: A's last-step flow sent by rho and the one received
-   * by rho (ring); every flow from / to rho (all-to-all).  rho not in A: no edge. */
-#define PUSH_AFTER(rho)                                                                      \
-  for (int32_t a_ = 0; a_ < n_after; a_++) {                                                 \
-    const coll_t *A = &s->coll[after[a_]];                                                   \
-    int32_t ia = ring_index_of(A, (rho));                                                    \
-    if (ia < 0) continue;                                                                    \
-    if (A->kind == ORC_ALLTOALL) {                                                           \
-      for (int32_t x = 0; x < A->n; x++) {                                                   \
-        if (x == ia) continue;                                                               \
-        /* flow ia->x is entry (ia, x) of the row-major list without the diagonal */         \
-        if (push_pred(s, A->first_flow + ia * (A->n - 1) + (x < ia ? x : x - 1))) return ORC_ENOMEM; \
-        if (push_pred(s, A->first_flow + x * (A->n - 1) + (ia < x ? ia : ia - 1))) return ORC_ENOMEM; \
-      }                                                                                      \
-    } else {                                                                                 \
-      int32_t last = A->first_flow + (A->steps - 1) * A->n;                                  \
-      if (push_pred(s, last + ia)) return ORC_ENOMEM;                    /* sent by rho */    \
-      if (push_pred(s, last + (ia + A->n - 1) % A->n)) return ORC_ENOMEM; /* received by rho */ \
-    }                                                                                        \
-  }
+#define PUSH_AFTER(rho) if (push_after_edges(s, after, n_after, (rho))) return ORC_ENOMEM
 
   if (kind == ORC_ALLTOALL) {
+    double chunk = bytes / (double)N; /* S3: one f64 division */
     for (int32_t i = 0; i < N; i++)
       for (int32_t j = 0; j < N; j++) {
         if (i == j) continue;
@@ -337,7 +369,8 @@ int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32
         PUSH_AFTER(ranks[i]);
         commit_flow(s);
       }
-  } else {
+  } else if (kind <= ORC_REDUCESCATTER_RING) {
+    double chunk = bytes / (double)N; /* S3: one f64 division */
     for (int32_t st = 0; st < S; st++)
       for (int32_t i = 0; i < N; i++) { /* flow (st,i): r[i] -> r[(i+1) mod N] */
         if (begin_flow(s, ranks[i], ranks[(i + 1) % N], chunk, st == 0 ? start : 0.0, cid)) return ORC_ENOMEM;
@@ -349,7 +382,46 @@ int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32
         }
         commit_flow(s);
       }
+  } else if (kind == ORC_BROADCAST_CHAIN || kind == ORC_REDUCE_CHAIN) {
+    double piece = bytes / (double)chunks;
+    for (int32_t ch = 0; ch < chunks; ch++)
+      for (int32_t i = 0; i < N - 1; i++) {
+        int32_t from = kind == ORC_BROADCAST_CHAIN ? ranks[i] : ranks[N - 1 - i];
+        int32_t to = kind == ORC_BROADCAST_CHAIN ? ranks[i + 1] : ranks[N - 2 - i];
+        int no_pred = ch == 0 && i == 0;
+        if (begin_flow(s, from, to, piece, no_pred ? start : 0.0, cid)) return ORC_ENOMEM;
+        if (no_pred) PUSH_AFTER(from);
+        if (i > 0 && push_pred(s, first + ch * (N - 1) + i - 1)) return ORC_ENOMEM;  /* the chunk has arrived */
+        if (ch > 0 && push_pred(s, first + (ch - 1) * (N - 1) + i)) return ORC_ENOMEM; /* sender FIFO */
+        commit_flow(s);
+      }
+  } else { /* ORC_ALLREDUCE_TREE */
+    double piece = bytes / (double)chunks;
+    int32_t per = 2 * (N - 1);
+    for (int32_t ch = 0; ch < chunks; ch++) {
+      for (int32_t i = 1; i < N; i++) { /* up(ch, i): r[i] -> r[parent(i)] */
+        int32_t l = 2 * i + 1, r = 2 * i + 2;
+        int no_pred = ch == 0 && l >= N; /* a leaf's first chunk */
+        if (begin_flow(s, ranks[i], ranks[(i - 1) / 2], piece, no_pred ? start : 0.0, cid)) return ORC_ENOMEM;
+        if (no_pred) PUSH_AFTER(ranks[i]);
+        if (l < N && push_pred(s, first + ch * per + (l - 1))) return ORC_ENOMEM;
+        if (r < N && push_pred(s, first + ch * per + (r - 1))) return ORC_ENOMEM;
+        if (ch > 0 && push_pred(s, first + (ch - 1) * per + (i - 1))) return ORC_ENOMEM;
+        commit_flow(s);
+      }
+      for (int32_t i = 1; i < N; i++) { /* down(ch, i): r[parent(i)] -> r[i] */
+        int32_t p = (i - 1) / 2;
+        if (begin_flow(s, ranks[p], ranks[i], piece, 0.0, cid)) return ORC_ENOMEM;
+        if (p == 0) { /* the root holds the full sum of the chunk once its children's partial sums are in */
+          if (push_pred(s, first + ch * per + 0)) return ORC_ENOMEM;
+          if (N > 2 && push_pred(s, first + ch * per + 1)) return ORC_ENOMEM;
+        } else if (push_pred(s, first + ch * per + (N - 1) + (p - 1))) return ORC_ENOMEM;
+        if (ch > 0 && push_pred(s, first + (ch - 1) * per + (N - 1) + (i - 1))) return ORC_ENOMEM;
+        commit_flow(s);
+      }
+    }
   }
+#undef PUSH_AFTER
   if (out_id) *out_id = cid;
   return ORC_OK;
 }

@@ -47,7 +47,9 @@ typedef struct orc_sim orc_sim;
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ECYCLE = -4, ORC_ESTATE = -5, ORC_ERANGE = -6 };
 enum { ORC_TOPO_SINGLE = 0, ORC_TOPO_LEAF_SPINE = 1, ORC_TOPO_FAT_TREE = 2 };
-enum { ORC_ALLREDUCE_RING = 0, ORC_ALLGATHER_RING = 1, ORC_REDUCESCATTER_RING = 2, ORC_ALLTOALL = 3 };
+enum { ORC_ALLREDUCE_RING = 0, ORC_ALLGATHER_RING = 1, ORC_REDUCESCATTER_RING = 2, ORC_ALLTOALL = 3,
+       /* NEXT-3: pipelined chain broadcast / reduce, binary-tree all-reduce; see orc_add_collective_ex */
+       ORC_BROADCAST_CHAIN = 4, ORC_REDUCE_CHAIN = 5, ORC_ALLREDUCE_TREE = 6 };
 enum { ORC_MODE_NAIVE = 0, ORC_MODE_FAST = 1 };
 /* orc_run_ex flags: the two readings of SURVEY.md 8(c) that DESIGN.md sec 2 replaced, kept for comparison */
 enum { ORC_FLAG_SETTLE_EVERY_EVENT = 1, /* S4.4 as written: every ACTIVE flow is debited at every event (not R-LZ) */
@@ -76,6 +78,10 @@ int32_t orc_set_link_capacities(orc_sim *s, const double *cap_Bps);
 int32_t orc_get_link_capacities(const orc_sim *s, double *cap_Bps);
 int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t n_ranks, double bytes,
                            double start_time_s, const int32_t *after, int32_t n_after, int32_t *out_coll_id);
+/* the same with `chunks` pipeline chunks (chain and tree kinds; 1 for the others) */
+int32_t orc_add_collective_ex(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t n_ranks, double bytes,
+                              double start_time_s, const int32_t *after, int32_t n_after, int32_t chunks,
+                              int32_t *out_coll_id);
 int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *dst, const double *bytes,
                       const double *start_time_s, const int64_t *dep_off, const int64_t *dep_flow_ids,
                       const int32_t *conn_id, int64_t *out_first_flow_id);

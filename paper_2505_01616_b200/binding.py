@@ -16,6 +16,7 @@ _LIB_PATH = os.path.join(_HERE, "libphs.so")
 PHS_OK, PHS_EINVAL, PHS_ENOMEM, PHS_ECUDA, PHS_ECYCLE, PHS_ESTATE, PHS_ERANGE = 0, -1, -2, -3, -4, -5, -6
 TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE = 0, 1, 2
 ALLREDUCE_RING, ALLGATHER_RING, REDUCESCATTER_RING, ALLTOALL = 0, 1, 2, 3
+BROADCAST_CHAIN, REDUCE_CHAIN, ALLREDUCE_TREE = 4, 5, 6
 
 
 class TopologyDesc(C.Structure):
@@ -40,7 +41,7 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
 # every symbol include/phs.h declares (tests check that the library exports all of them)
 SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
            "phs_set_link_capacities_batch",
-           "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_batch", "phs_add_flows",
+           "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
            "phs_set_decomposition", "phs_set_windows", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
@@ -126,13 +127,18 @@ def phs_get_link_capacities(h, instance):
     return cap
 
 
-def phs_add_collective(h, instance, kind, ranks, nbytes, start=0.0, after=()):
+def phs_add_collective(h, instance, kind, ranks, nbytes, start=0.0, after=(), chunks=1):
     ranks = _arr(ranks, np.int32)
     after = _arr(after, np.int32)
     cid = C.c_int32()
-    _chk(lib().phs_add_collective(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
-                                  C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
-                                  C.c_int32(len(after)), C.byref(cid)), "phs_add_collective")
+    if chunks == 1:
+        _chk(lib().phs_add_collective(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
+                                      C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
+                                      C.c_int32(len(after)), C.byref(cid)), "phs_add_collective")
+    else:
+        _chk(lib().phs_add_collective_ex(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
+                                         C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
+                                         C.c_int32(len(after)), C.c_int32(chunks), C.byref(cid)), "phs_add_collective_ex")
     return cid.value
 
 
@@ -380,7 +386,7 @@ class Sim:
         same = getattr(w, "uniform_ops", False)      # the generator states it; otherwise compare
         if not same and count > 1:
             same = all(len(x.ops) == len(insts[0].ops) for x in insts) and all(
-                isinstance(o, W.Coll) for x in insts for o in x.ops)
+                isinstance(o, W.Coll) and o.chunks == 1 for x in insts for o in x.ops)
             for k, op0 in enumerate(insts[0].ops) if same else ():
                 ok = all(x.ops[k].kind == op0.kind and np.array_equal(x.ops[k].ranks, op0.ranks)
                          and tuple(x.ops[k].after) == tuple(op0.after) for x in insts)
@@ -394,7 +400,8 @@ class Sim:
         else:
             for i, inst in enumerate(insts):
                 W.apply(inst,
-                        lambda kind, ranks, nb, st, after, i=i: phs_add_collective(sim.h, i, kind, ranks, nb, st, after),
+                        lambda kind, ranks, nb, st, after, chunks=1, i=i: phs_add_collective(sim.h, i, kind, ranks, nb, st,
+                                                                                             after, chunks),
                         lambda src, dst, nb, st, do, di, conn, i=i: phs_add_flows(sim.h, i, src, dst, nb, st, do, di, conn))
         return sim
 

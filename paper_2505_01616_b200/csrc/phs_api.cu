@@ -117,6 +117,12 @@ phs_status phs_get_link_capacities(const phs_sim *sim, int32_t instance, double 
 
 phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                               double bytes, double start, const int32_t *after, int32_t n_after, int32_t *out_id) {
+  return phs_add_collective_ex(sim, instance, kind, ranks, n_ranks, bytes, start, after, n_after, 1, out_id);
+}
+
+phs_status phs_add_collective_ex(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                 double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
+                                 int32_t *out_id) {
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
@@ -128,7 +134,7 @@ phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, cons
         return fail(PHS_ESTATE, "instance -1 needs the same number of collectives in every instance");
   std::string why;
   for (int i = lo; i < hi; ++i) {
-    st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes, start, after, n_after, &why);
+    st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes, start, after, n_after, chunks, &why);
     if (st != PHS_OK) return fail(st, why);  // validation fails on the first instance, before any mutation
   }
   if (out_id) *out_id = (int32_t)sim->inst[lo].colls.size() - 1;
@@ -154,7 +160,7 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
   std::string why;
   for (int i = 0; i < sim->batch; ++i) {
     phs_status sti = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
-                                       after, n_after, &why);
+                                       after, n_after, 1, &why);
     if (sti != PHS_OK) return fail(sti, why);
   }
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;

@@ -177,7 +177,8 @@ inline void push_dep(Instance &inst, int32_t on) {
 }
 
 // Flows of collective `a` that must finish before rank `rho` may start a later collective: what rho sent and
-// what rho received in a's last step (ring), or everything from / to rho (all-to-all).
+// what rho received in a's last step (ring), everything from / to rho (all-to-all), or what rho sends and receives
+// in a's last chunk (chain and tree kinds; positions worked out from the decomposition rule, see expand_collective).
 void chain_after(Instance &inst, const Collective &a, int32_t rho) {
   int pos = -1;
   for (int i = 0; i < a.n_ranks; ++i)
@@ -186,13 +187,30 @@ void chain_after(Instance &inst, const Collective &a, int32_t rho) {
       break;
     }
   if (pos < 0) return;  // rho did not take part: no edge
+  const int N = a.n_ranks;
   if (a.kind == PHS_ALLTOALL) {
-    const int N = a.n_ranks;
     for (int other = 0; other < N; ++other) {
       if (other == pos) continue;
       push_dep(inst, a.first_flow + pos * (N - 1) + (other > pos ? other - 1 : other));  // pos -> other
       push_dep(inst, a.first_flow + other * (N - 1) + (pos > other ? pos - 1 : pos));    // other -> pos
     }
+  } else if (a.kind == PHS_BROADCAST_CHAIN || a.kind == PHS_REDUCE_CHAIN) {
+    // hop i of the last chunk: broadcast r[i] -> r[i+1]; reduce r[N-1-i] -> r[N-2-i].  In ascending flow id.
+    const int32_t last = a.first_flow + (a.chunks - 1) * (N - 1);
+    const int q = a.kind == PHS_BROADCAST_CHAIN ? pos : N - 1 - pos;  // rho sends hop q and receives hop q-1
+    if (q >= 1) push_dep(inst, last + q - 1);
+    if (q <= N - 2) push_dep(inst, last + q);
+  } else if (a.kind == PHS_ALLREDUCE_TREE) {
+    // last chunk's block: up(i) at offset i-1, down(i) at offset (N-1) + i-1.  rho at position pos sends up(pos) and
+    // down(children), receives up(children) and down(pos).  In ascending flow id.
+    const int32_t blk = a.first_flow + (a.chunks - 1) * 2 * (N - 1);
+    const int l = 2 * pos + 1, r = 2 * pos + 2;
+    if (pos >= 1) push_dep(inst, blk + pos - 1);
+    if (l < N) push_dep(inst, blk + l - 1);
+    if (r < N) push_dep(inst, blk + r - 1);
+    if (pos >= 1) push_dep(inst, blk + (N - 1) + pos - 1);
+    if (l < N) push_dep(inst, blk + (N - 1) + l - 1);
+    if (r < N) push_dep(inst, blk + (N - 1) + r - 1);
   } else {
     const int32_t last_step = a.first_flow + (a.steps - 1) * a.n_ranks;
     push_dep(inst, last_step + pos);                                  // sent by rho
@@ -203,13 +221,16 @@ void chain_after(Instance &inst, const Collective &a, int32_t rho) {
 }  // namespace
 
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t N,
-                             double bytes, double start, const int32_t *after, int32_t n_after, std::string *why) {
+                             double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
+                             std::string *why) {
   auto bad = [&](const char *m) {
     if (why) *why = m;
     return PHS_EINVAL;
   };
   if (!ranks) return bad("ranks is null");
-  if (kind < PHS_ALLREDUCE_RING || kind > PHS_ALLTOALL) return bad("unknown collective kind");
+  if (kind < PHS_ALLREDUCE_RING || kind > PHS_ALLREDUCE_TREE) return bad("unknown collective kind");
+  if (chunks < 1 || chunks > 65536) return bad("chunks must be in [1, 65536]");
+  if (kind <= PHS_ALLTOALL && chunks != 1) return bad("chunks applies to the chain and tree kinds only");
   if (N < 2) return bad("a collective needs at least 2 ranks");
   if (!(bytes > 0.0) || !std::isfinite(bytes)) return bad("bytes must be positive and finite");
   if (!(start >= 0.0) || !std::isfinite(start)) return bad("start_time_s must be >= 0 and finite");
@@ -225,7 +246,10 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   for (int a = 0; a < n_after; ++a)
     if (after[a] < 0 || after[a] >= (int32_t)inst.colls.size()) return bad("after_coll_ids names an unknown collective");
   const int steps = kind == PHS_ALLREDUCE_RING ? 2 * (N - 1) : kind == PHS_ALLTOALL ? 1 : N - 1;
-  const int64_t nf = kind == PHS_ALLTOALL ? (int64_t)N * (N - 1) : (int64_t)steps * N;
+  const int64_t nf = kind == PHS_ALLTOALL          ? (int64_t)N * (N - 1)
+                     : kind == PHS_ALLREDUCE_TREE  ? (int64_t)chunks * 2 * (N - 1)
+                     : kind >= PHS_BROADCAST_CHAIN ? (int64_t)chunks * (N - 1)
+                                                   : (int64_t)steps * N;
   if (inst.n_flows() + nf > 0x7ffffff0LL) {
     if (why) *why = "too many flows in one instance";
     return PHS_ERANGE;
@@ -236,6 +260,7 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   c.first_flow = (int32_t)inst.n_flows();
   c.n_flows = (int32_t)nf;
   c.steps = steps;
+  c.chunks = chunks;
   c.ranks.assign(ranks, ranks + N);
   c.chain = (int32_t)inst.colls.size();
   for (int a = 0; a < n_after; ++a) c.chain = std::min(c.chain, inst.colls[after[a]].chain);
@@ -259,7 +284,61 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
   const double start = c.start;
   const int32_t conn = id;  // ECMP key: one path per (pair, collective)
   const double chunk = c.bytes / (double)N;
-  if (c.kind == PHS_ALLTOALL) {
+  if (c.kind == PHS_BROADCAST_CHAIN || c.kind == PHS_REDUCE_CHAIN) {
+    // NEXT-3: pipelined chain.  Hop i carries every chunk in turn: chunk-major flow order, hop i of
+    // chunk ch waits for hop i-1 of the same chunk (the data is there) and for hop i of the previous chunk (FIFO).
+    // Chunks ch > 0 take the route of chunk 0 (ECMP keys on pair + collective).
+    const double piece = c.bytes / (double)c.chunks;
+    const int hops = N - 1;
+    for (int ch = 0; ch < c.chunks; ++ch)
+      for (int i = 0; i < hops; ++i) {
+        if (ch == 0) {
+          const int a = c.kind == PHS_BROADCAST_CHAIN ? i : N - 1 - i, b = c.kind == PHS_BROADCAST_CHAIN ? i + 1 : N - 2 - i;
+          push_flow(fab, inst, ranks[a], ranks[b], piece, i == 0 ? start : 0.0, conn);
+          if (i == 0)
+            for (int k = 0; k < n_after; ++k) chain_after(inst, inst.colls[after[k]], ranks[a]);
+        } else {
+          repeat_flow(inst, (size_t)c.first_flow + (size_t)i);
+        }
+        if (i > 0) push_dep(inst, c.first_flow + ch * hops + i - 1);
+        if (ch > 0) push_dep(inst, c.first_flow + (ch - 1) * hops + i);
+      }
+  } else if (c.kind == PHS_ALLREDUCE_TREE) {
+    // NEXT-3: binary tree in heap order; per chunk the N-1 up flows (child -> parent), then the N-1 down flows
+    const double piece = c.bytes / (double)c.chunks;
+    const int blk = 2 * (N - 1);
+    for (int ch = 0; ch < c.chunks; ++ch) {
+      const int32_t base = c.first_flow + ch * blk, prev = base - blk;
+      for (int i = 1; i < N; ++i) {  // up(ch, i)
+        const int l = 2 * i + 1, r = 2 * i + 2;
+        const bool leaf_first = ch == 0 && l >= N;
+        if (ch == 0) {
+          push_flow(fab, inst, ranks[i], ranks[(i - 1) / 2], piece, leaf_first ? start : 0.0, conn);
+          if (leaf_first)
+            for (int k = 0; k < n_after; ++k) chain_after(inst, inst.colls[after[k]], ranks[i]);
+        } else {
+          repeat_flow(inst, (size_t)c.first_flow + (size_t)(i - 1));
+        }
+        if (l < N) push_dep(inst, base + l - 1);
+        if (r < N) push_dep(inst, base + r - 1);
+        if (ch > 0) push_dep(inst, prev + i - 1);
+      }
+      for (int i = 1; i < N; ++i) {  // down(ch, i)
+        const int p = (i - 1) / 2;
+        if (ch == 0)
+          push_flow(fab, inst, ranks[p], ranks[i], piece, 0.0, conn);
+        else
+          repeat_flow(inst, (size_t)c.first_flow + (size_t)(N - 1 + i - 1));
+        if (p == 0) {  // the root has the chunk's sum once both of its children have delivered
+          push_dep(inst, base + 0);
+          if (N > 2) push_dep(inst, base + 1);
+        } else {
+          push_dep(inst, base + (N - 1) + p - 1);
+        }
+        if (ch > 0) push_dep(inst, prev + (N - 1) + i - 1);
+      }
+    }
+  } else if (c.kind == PHS_ALLTOALL) {
     for (int i = 0; i < N; ++i)
       for (int j = 0; j < N; ++j) {
         if (i == j) continue;

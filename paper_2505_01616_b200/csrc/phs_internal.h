@@ -73,6 +73,7 @@ constexpr int32_t kPaused = 2;    // internal: stopped before the first event la
 // ---- host-side instance tables (built by phs_build.cpp) ----
 struct Collective {
   int32_t kind, n_ranks, first_flow, n_flows, steps;
+  int32_t chunks = 1;  // pipeline chunks of the chain / tree kinds
   int32_t chain;  // smallest id among the collectives this one is (transitively) chained `after`, else its own id
   std::vector<int32_t> ranks;
   // as submitted: the flows are appended to the instance arrays later (Instance::expanded), on the host threads
@@ -121,7 +122,8 @@ void expand_pending(const Fabric &fab, Instance &inst);
 // Appends flows / collectives to an instance (S3).  Return PHS_OK or an error with *why set.  append_collective
 // validates and records the collective; its flows appear with the next expand_pending.
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t n_ranks,
-                             double bytes, double start, const int32_t *after, int32_t n_after, std::string *why);
+                             double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
+                             std::string *why);
 phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,
                         const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
                         const int32_t *conn_id, std::string *why);

@@ -277,13 +277,15 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         ubound[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
         ubound_cta[unit_of[in.colls[c].first_flow]] -= in.colls[c].n_flows;
         const int64_t nr = in.colls[c].n_ranks;
+        // chain / tree kinds: one flow per hop (tree edge) and direction is in flight, its successors may be PENDING
+        const bool ringk = in.colls[c].kind <= PHS_REDUCESCATTER_RING;
         const int64_t need_cta = in.colls[c].kind == PHS_ALLTOALL
                                      ? in.colls[c].n_flows
-                                     : std::min<int64_t>(in.colls[c].n_flows, nr + (nr + 1) / 2);
+                                     : std::min<int64_t>(in.colls[c].n_flows, ringk ? nr + (nr + 1) / 2 : 4 * nr);
         chain_max_cta[in.colls[c].chain] = std::max(chain_max_cta[in.colls[c].chain], need_cta);
         const int64_t need = in.colls[c].kind == PHS_ALLTOALL
                                  ? in.colls[c].n_flows
-                                 : std::min<int64_t>(in.colls[c].n_flows, 2 * (int64_t)in.colls[c].n_ranks);
+                                 : std::min<int64_t>(in.colls[c].n_flows, (ringk ? 2 : 4) * (int64_t)in.colls[c].n_ranks);
         chain_max[in.colls[c].chain] = std::max(chain_max[in.colls[c].chain], need);
       }
       for (size_t c = 0; c < in.colls.size(); ++c) {

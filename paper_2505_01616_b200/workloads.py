@@ -13,6 +13,7 @@ import numpy as np
 
 TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE = 0, 1, 2
 ALLREDUCE_RING, ALLGATHER_RING, REDUCESCATTER_RING, ALLTOALL = 0, 1, 2, 3
+BROADCAST_CHAIN, REDUCE_CHAIN, ALLREDUCE_TREE = 4, 5, 6
 
 MiB = float(2 ** 20)
 GiB = float(2 ** 30)
@@ -38,6 +39,7 @@ class Coll:
     nbytes: float
     start: float = 0.0
     after: tuple = ()
+    chunks: int = 1          # pipeline chunks of the chain / tree kinds
 
 
 @dataclass
@@ -109,7 +111,8 @@ def n_flows_of(op):
         return len(op.src)
     N = len(op.ranks)
     return {ALLREDUCE_RING: 2 * (N - 1) * N, ALLGATHER_RING: (N - 1) * N, REDUCESCATTER_RING: (N - 1) * N,
-            ALLTOALL: N * (N - 1)}[op.kind]
+            ALLTOALL: N * (N - 1), BROADCAST_CHAIN: op.chunks * (N - 1), REDUCE_CHAIN: op.chunks * (N - 1),
+            ALLREDUCE_TREE: op.chunks * 2 * (N - 1)}[op.kind]
 
 
 def _rng(cfg, instance):
@@ -123,10 +126,14 @@ def _loguniform(rng, lo, hi, size=None):
 
 def apply(inst: Instance, add_collective, add_flows):
     """Replay an instance's ops through two callables with the signatures
-    add_collective(kind, ranks, nbytes, start, after) -> id ; add_flows(src, dst, nbytes, start, dep_off, dep_ids, conn_id)."""
+    add_collective(kind, ranks, nbytes, start, after[, chunks]) -> id ; add_flows(src, dst, nbytes, start, dep_off, dep_ids,
+    conn_id)."""
     for op in inst.ops:
         if isinstance(op, Coll):
-            add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after)
+            if op.chunks == 1:
+                add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after)
+            else:
+                add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after, op.chunks)
         else:
             add_flows(op.src, op.dst, op.nbytes, op.start, op.dep_off, op.dep_ids, op.conn_id)
 

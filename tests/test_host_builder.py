@@ -72,6 +72,34 @@ def test_after_and_alltoall_dag_equal_the_oracle():
     _compare_tables(W.Workload("mixed", d, 5, [W.Instance(seed=0, ops=ops), W.Instance(seed=1, ops=ops)]))
 
 
+def test_chain_and_tree_collectives_equal_the_oracle():
+    """NEXT-3 kinds: flows, routes and DAG (incl. `after` edges in both directions with every other kind) built by the
+    library equal the oracle's, which is pinned against hand-written lists and closed forms (test_oracle_pins.py)."""
+    d = W.topo_desc(W.TOPO_FAT_TREE, 8, 2, k=4, agg_uplinks=1)
+    rng = np.random.default_rng(3)
+    insts = []
+    for i in range(3):
+        perm = rng.permutation(16).astype(np.int32)
+        ops = [W.Coll(W.BROADCAST_CHAIN, perm[:7], 8e6, 0.0, (), 5),
+               W.Coll(W.ALLREDUCE_TREE, perm[3:14], 6e6, 1e-5, (), 3),
+               W.Coll(W.REDUCE_CHAIN, perm[5:12], 4e6, 0.0, (0, 1), 4),
+               W.Coll(W.ALLREDUCE_RING, perm[:6], 16e6, 0.0, (1, 2)),
+               W.Coll(W.ALLTOALL, perm[8:14], 3e6, 2e-5, (2,)),
+               W.Coll(W.ALLREDUCE_TREE, perm[1:9], 2e6, 0.0, (3, 4), 1),
+               W.Coll(W.ALLREDUCE_TREE, np.array([perm[0], perm[15]], np.int32), 2e6, 0.0, (5,), 2),
+               W.Coll(W.BROADCAST_CHAIN, perm[9:16], 5e6, 0.0, (5, 4, 6), 2),
+               W.Coll(W.ALLGATHER_RING, perm[2:10], 5e6, 0.0, (7, 0))]
+        insts.append(W.Instance(seed=i, ops=ops))
+    _compare_tables(W.Workload("next3", d, 4, insts))
+    sim = B.Sim(d, batch=1)
+    for bad in (dict(kind=B.ALLREDUCE_RING, chunks=2), dict(kind=B.ALLREDUCE_TREE, chunks=0), dict(kind=7, chunks=1)):
+        with pytest.raises(B.PhsError) as e:
+            B.phs_add_collective(sim.h, 0, bad["kind"], [0, 1, 2], 1e6, chunks=bad["chunks"]) if bad["chunks"] != 1 else \
+                B.phs_add_collective(sim.h, 0, bad["kind"], [0, 1, 2], 1e6)
+        assert e.value.code == B.PHS_EINVAL
+    sim.close()
+
+
 def test_deferred_expansion_keeps_submission_order():
     """phs_add_collective records the collective and its flows are expanded later (by the next raw-flow submission,
     a table getter, or phs_finalize).  Flow ids must still follow submission order, and reading tables between

@@ -22,17 +22,24 @@ MUTANTS = [
      "down_lane"),
     ("M5_no_fifo_pred", "if (push_pred(s, first + (st - 1) * N + i)) return ORC_ENOMEM;               /* sender FIFO */",
      "", "ring_dag"),
-    ("M6_no_received_edge", "if (push_pred(s, last + (ia + A->n - 1) % A->n)) return ORC_ENOMEM; /* received by rho */ \\",
-     "\\", "after_chains or mixed_kind"),
+    ("M6_no_received_edge", "if (push_pred(s, last + (ia + A->n - 1) % A->n)) return -1; /* received by rho */", "",
+     "after_chains or mixed_kind"),
     ("M7_tie_to_highest_id", "int64_t sh = w->cap_rem[l] / w->n[l];\n        if (b < 0 || sh < s) { b = l; s = sh; }",
      "int64_t sh = w->cap_rem[l] / w->n[l];\n        if (b < 0 || sh <= s) { b = l; s = sh; }", "p1_lone or p3_cfg0"),
     ("M8_no_latency_on_release", "t_act[g] = st + s->Lat[g];", "t_act[g] = st;", "p2_uniform or input_validation"),
     ("M9_a2a_after_edges_to_rho_dropped",
-     "if (push_pred(s, A->first_flow + x * (A->n - 1) + (ia < x ? ia : ia - 1))) return ORC_ENOMEM; \\", "\\",
+     "if (push_pred(s, A->first_flow + x * (A->n - 1) + (ia < x ? ia : ia - 1))) return -1;", "",
      "mixed_kind or alltoall_after"),
     ("M10_sum_R_counts_events", "s->work[2] += R;", "s->work[2] += 1;", "work_counters"),
     ("M11_settle_sign", "double r = rem - m;", "double r = rem + m;", "p6 or q11"),
-    ("M12_chunk_not_divided", "double chunk = bytes / (double)N;", "double chunk = bytes;", "p2_uniform"),
+    ("M12_chunk_not_divided", "} else if (kind <= ORC_REDUCESCATTER_RING) {\n    double chunk = bytes / (double)N;",
+     "} else if (kind <= ORC_REDUCESCATTER_RING) {\n    double chunk = bytes;", "p2_uniform"),
+    ("M13_chain_no_fifo", "if (ch > 0 && push_pred(s, first + (ch - 1) * (N - 1) + i)) return ORC_ENOMEM; /* sender FIFO */",
+     "", "next3_pipelined"),
+    ("M14_tree_root_waits_for_one_child", "if (N > 2 && push_pred(s, first + ch * per + 1)) return ORC_ENOMEM;", "",
+     "next3_tree"),
+    ("M15_chain_after_ignores_last_chunk", "for (int32_t f = A->first_flow + (A->chunks - 1) * per_chunk;",
+     "for (int32_t f = A->first_flow;", "next3_after"),
 ]
 
 

@@ -536,6 +536,80 @@ def test_mixed_kind_after_edges_against_hand_written_lists():
         assert sorted(pr[off[f]:off[f + 1]].tolist()) == p
 
 
+# ------------------------------------------------------------------------------------------------ NEXT-3 collectives
+@pytest.mark.parametrize("kind", [W.BROADCAST_CHAIN, W.REDUCE_CHAIN])
+@pytest.mark.parametrize("N,C", [(5, 4), (8, 1), (3, 7)])
+def test_next3_pipelined_chain_closed_form(kind, N, C):
+    """A chain of N ranks moving C chunks over link-disjoint hops is the max-plus recurrence
+    T(c, i) = max(T(c, i-1), T(c-1, i)) + d, d = Lat + (bytes / C) / B: the last chunk leaves the last hop at
+    (C + N - 2) d; flow (c, i) finishes at (c + i + 1) d."""
+    d = single(n_hosts=1, gph=8)
+    s = orc.Sim(d, 0)
+    ranks = np.array([5, 2, 7, 0, 3, 6, 1, 4][:N], np.int32)
+    s.add_collective(kind, ranks, 6e6, chunks=C)
+    s.run()
+    step = 2e-6 + (6e6 / C) / 450e9
+    t = s.completion_times().reshape(C, N - 1)
+    want = np.array([[(c + i + 1) * step for i in range(N - 1)] for c in range(C)])
+    np.testing.assert_allclose(t, want, rtol=1e-12)
+    assert s.collective_times()[0] == pytest.approx((C + N - 2) * step, rel=1e-12)
+    src, dst, b, _ = s.flows()
+    hops = [(ranks[i], ranks[i + 1]) if kind == W.BROADCAST_CHAIN else (ranks[N - 1 - i], ranks[N - 2 - i])
+            for i in range(N - 1)]
+    assert [(a, b_) for a, b_ in zip(src, dst)] == hops * C and np.all(b == 6e6 / C)
+
+
+def test_next3_tree_allreduce_structure_and_closed_form():
+    """Binary tree in heap order, hand-written for N = 4, C = 2: positions 0 <- 1, 2 ; 1 <- 3.  Per chunk: up(1), up(2),
+    up(3), down(1), down(2), down(3).  Then the closed form of a perfect tree of 7 on one NVSwitch: the two children of
+    a node share its down link on the way up and its up link on the way down, so each of the 4 levels takes
+    Lat + 2 bytes / B."""
+    d = single(n_hosts=1, gph=8)
+    s = orc.Sim(d, 0)
+    r = np.array([6, 1, 4, 3], np.int32)
+    s.add_collective(orc.ALLREDUCE_TREE, r, 8e6, chunks=2)
+    off, pr = s.preds()
+    s.run()
+    src, dst, b, _ = s.flows()
+    edges = [(1, 6), (4, 6), (3, 1), (6, 1), (6, 4), (1, 3)]           # up(1) up(2) up(3) down(1) down(2) down(3)
+    assert [(a, b_) for a, b_ in zip(src, dst)] == edges * 2 and np.all(b == 4e6)
+    want = {0: [2], 1: [], 2: [], 3: [0, 1], 4: [0, 1], 5: [3],          # chunk 0
+            6: [0, 8], 7: [1], 8: [2], 9: [3, 6, 7], 10: [4, 6, 7], 11: [5, 9]}
+    for f, p in want.items():
+        assert sorted(pr[off[f]:off[f + 1]].tolist()) == p, f
+    s = orc.Sim(d, 0)
+    s.add_collective(orc.ALLREDUCE_TREE, np.arange(7, dtype=np.int32), 4e6)
+    s.run()
+    assert s.collective_times()[0] == pytest.approx(4 * (2e-6 + 2 * 4e6 / 450e9), rel=1e-12)
+
+
+def test_next3_after_edges_against_hand_written_lists():
+    """`after` with the chain / tree kinds on either side (N = 3), lists written out by hand."""
+    d = single(n_hosts=1, gph=8)
+    # A = chain broadcast over [0,1,2], 2 chunks: flows 0:(c0) 0->1, 1:(c0) 1->2, 2:(c1) 0->1, 3:(c1) 1->2.
+    # B = ring all-gather over [2,0,1] after A: sender 2 receives 3; sender 0 sends 2; sender 1 receives 2, sends 3
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.BROADCAST_CHAIN, np.array([0, 1, 2], np.int32), 2e6, chunks=2)
+    s.add_collective(orc.ALLGATHER_RING, np.array([2, 0, 1], np.int32), 3e6, after=[a])
+    off, pr = s.preds()
+    assert [sorted(pr[off[f]:off[f + 1]].tolist()) for f in (4, 5, 6)] == [[3], [2], [2, 3]]
+    # A = ring reduce-scatter over [1,2,0] (2 steps x 3: last step = flows 3: 1->2, 4: 2->0, 5: 0->1);
+    # B = tree all-reduce over [2,0,1] (up(1): 0->2, up(2): 1->2, down(1), down(2)) after A: the leaves' up flows wait:
+    # sender 0 sent 5, received 4; sender 1 sent 3, received 5
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.REDUCESCATTER_RING, np.array([1, 2, 0], np.int32), 3e6)
+    s.add_collective(orc.ALLREDUCE_TREE, np.array([2, 0, 1], np.int32), 3e6, after=[a])
+    off, pr = s.preds()
+    assert [sorted(pr[off[f]:off[f + 1]].tolist()) for f in (6, 7, 8, 9)] == [[4, 5], [3, 5], [6, 7], [6, 7]]
+    # A = tree over [0,1,2], 1 chunk: 0: up(1) 1->0, 1: up(2) 2->0, 2: down(1) 0->1, 3: down(2) 0->2; B = reduce chain
+    # over [2,1] (hop 0: 1->2) after A: sender 1 sent 0, received 2
+    s = orc.Sim(d, 0)
+    a = s.add_collective(orc.ALLREDUCE_TREE, np.array([0, 1, 2], np.int32), 3e6)
+    s.add_collective(orc.REDUCE_CHAIN, np.array([2, 1], np.int32), 3e6, after=[a], chunks=3)
+    off, pr = s.preds()
+    assert [sorted(pr[off[f]:off[f + 1]].tolist()) for f in (4, 5, 6)] == [[0, 2], [4], [5]]
+
+
 # ------------------------------------------------------------------------------------------------ S2 routing pins
 def test_routing_leaf_spine_down_lane_comes_from_the_high_hash_word():
     """S2: with P parallel uplinks per (leaf, spine) the up lane is (H mod (n_spines P)) mod P and the down lane

@@ -12,7 +12,8 @@ def oracle_build(desc, inst, base_seed=0):
     if cap is not None:
         sim.set_link_capacities(cap)
     W.apply(inst,
-            lambda kind, ranks, nbytes, start, after: sim.add_collective(kind, ranks, nbytes, start, after),
+            lambda kind, ranks, nbytes, start, after, chunks=1: sim.add_collective(kind, ranks, nbytes, start, after,
+                                                                                   chunks),
             lambda src, dst, nbytes, start, dep_off, dep_ids, conn: sim.add_flows(src, dst, nbytes, start, dep_off,
                                                                                    dep_ids, conn))
     return sim
