@@ -66,6 +66,9 @@ typedef struct {
   int32_t n_leaves, n_spines, uplinks_per_leaf_spine; /* leaf-spine: hosts in contiguous blocks per leaf  */
   int32_t k, agg_uplinks;       /* fat tree: k pods, k/2 edge (= hosts) and k/2 agg switches per pod,
                                    gpus_per_host = k/2, n_hosts = k*k/2; agg_uplinks per agg switch       */
+  int32_t compute_lanes;        /* compute engines per GPU for phs_add_spans (0 = none): engine links are
+                                   numbered after all network links, n_network_links + gpu * compute_lanes + lane,
+                                   capacity 2^32 work units / s, latency 0                                 */
 } phs_topology_desc;
 
 /* One row of the event log (S6/O4): one loop iteration = one distinct time. */
@@ -143,6 +146,24 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
 phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_t *src, const int32_t *dst,
                          const double *bytes, const double *start_time_s, const int64_t *dep_off,
                          const int64_t *dep_flow_ids, const int32_t *conn_id, int64_t *out_first_flow_id);
+
+/* Compute spans (PAPER.md L84 / L94 / L106: the event queue holds compute and communication spans with explicit
+ * dependencies; L206 / Fig. 7: computation overlapping communication).  A span is a DAG node of fixed length bound to
+ * a compute lane of a GPU: a flow of duration_s * 2^32 work units over that lane's engine link (src = dst = gpu).
+ * Alone on its lane it finishes at exactly t_act + duration_s; spans that overlap on one lane share it max-min fairly.
+ * Spans take flow ids like raw flows (out_first_flow_id), may depend on earlier flows / spans (dep_off / dep_flow_ids
+ * as in phs_add_flows) and may be depended upon; their "bottleneck" is the engine link.  lane nullable (= 0),
+ * start_time_s nullable (= 0); duration in (0, 2^20) s.  Needs compute_lanes > 0 in the topology descriptor. */
+phs_status phs_add_spans(phs_sim *sim, int32_t instance, int64_t n, const int32_t *gpu, const int32_t *lane,
+                         const double *duration_s, const double *start_time_s, const int64_t *dep_off,
+                         const int64_t *dep_flow_ids, int64_t *out_first_flow_id);
+/* phs_add_collective_ex plus flow-level predecessors: every flow of the collective that has no predecessor inside it
+ * and is sent by rank rho additionally waits for each listed EARLIER flow or span whose source or destination is rho
+ * (a span's is its GPU): "the all-reduce of a layer's gradients starts when that rank's backward kernel is done". */
+phs_status phs_add_collective_full(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                   double bytes, double start_time_s, const int32_t *after_coll_ids, int32_t n_after,
+                                   const int64_t *after_flow_ids, int32_t n_after_flows, int32_t chunks,
+                                   int32_t *out_coll_id);
 
 /* Event log on/off (default off) for subsequent runs; must precede phs_finalize. */
 phs_status phs_enable_event_log(phs_sim *sim, int32_t enable);

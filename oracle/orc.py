@@ -24,7 +24,7 @@ class TopologyDesc(C.Structure):
                 ("nvlink_Bps", C.c_double), ("nic_Bps", C.c_double), ("fabric_Bps", C.c_double),
                 ("hop_latency_s", C.c_double),
                 ("n_leaves", C.c_int32), ("n_spines", C.c_int32), ("uplinks_per_leaf_spine", C.c_int32),
-                ("k", C.c_int32), ("agg_uplinks", C.c_int32)]
+                ("k", C.c_int32), ("agg_uplinks", C.c_int32), ("compute_lanes", C.c_int32)]
 
 
 EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<i4"), ("n_rounds", "<i4"),
@@ -124,15 +124,31 @@ class Sim:
         _chk(lib().orc_get_link_capacities(self._h, _p(cap, C.c_double)), "orc_get_link_capacities")
         return cap
 
-    def add_collective(self, kind, ranks, nbytes, start=0.0, after=(), chunks=1):
+    def add_collective(self, kind, ranks, nbytes, start=0.0, after=(), chunks=1, after_flows=()):
         ranks = np.ascontiguousarray(ranks, dtype=np.int32)
         after = np.ascontiguousarray(after, dtype=np.int32)
+        after_flows = np.ascontiguousarray(after_flows, dtype=np.int64)
         cid = C.c_int32()
-        _chk(lib().orc_add_collective_ex(self._h, C.c_int32(kind), _p(ranks, C.c_int32), C.c_int32(len(ranks)),
-                                         C.c_double(nbytes), C.c_double(start),
-                                         _p(after, C.c_int32) if len(after) else None, C.c_int32(len(after)),
-                                         C.c_int32(chunks), C.byref(cid)), "orc_add_collective_ex")
+        _chk(lib().orc_add_collective_full(self._h, C.c_int32(kind), _p(ranks, C.c_int32), C.c_int32(len(ranks)),
+                                           C.c_double(nbytes), C.c_double(start),
+                                           _p(after, C.c_int32) if len(after) else None, C.c_int32(len(after)),
+                                           _p(after_flows, C.c_int64) if len(after_flows) else None,
+                                           C.c_int32(len(after_flows)), C.c_int32(chunks), C.byref(cid)),
+             "orc_add_collective_full")
         return cid.value
+
+    def add_spans(self, gpu, duration, lane=None, start=None, dep_off=None, dep_ids=None):
+        gpu = np.ascontiguousarray(gpu, dtype=np.int32)
+        duration = np.ascontiguousarray(duration, dtype=np.float64)
+        lane = None if lane is None else np.ascontiguousarray(lane, dtype=np.int32)
+        start = None if start is None else np.ascontiguousarray(start, dtype=np.float64)
+        dep_off = None if dep_off is None else np.ascontiguousarray(dep_off, dtype=np.int64)
+        dep_ids = None if dep_ids is None else np.ascontiguousarray(dep_ids, dtype=np.int64)
+        first = C.c_int64()
+        _chk(lib().orc_add_spans(self._h, C.c_int64(len(gpu)), _p(gpu, C.c_int32), _p(lane, C.c_int32),
+                                 _p(duration, C.c_double), _p(start, C.c_double), _p(dep_off, C.c_int64),
+                                 _p(dep_ids, C.c_int64), C.byref(first)), "orc_add_spans")
+        return first.value
 
     def add_flows(self, src, dst, nbytes, start=None, dep_off=None, dep_ids=None, conn_id=None):
         src = np.ascontiguousarray(src, dtype=np.int32)

@@ -32,7 +32,7 @@ typedef struct {
 struct orc_sim {
   orc_topology_desc d;
   uint64_t seed;
-  int32_t G, n_links, ran;
+  int32_t G, n_links, n_net_links, ran;
   double *cap, *lat; /* per directed link */
   /* flows */
   int64_t F, Fcap;
@@ -100,6 +100,9 @@ int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim *
     L += 2 * (int64_t)k * (k / 2) * (k / 2) + 2 * (int64_t)k * (k / 2) * d->agg_uplinks;
   } else if (d->kind != ORC_TOPO_SINGLE)
     return ORC_EINVAL;
+  if (d->compute_lanes < 0 || d->compute_lanes > 64) return ORC_EINVAL;
+  int64_t L_net = L;
+  L += G * d->compute_lanes; /* S7: compute engine links after all network links */
   if (L > 0x3fffffff) return ORC_ERANGE;
   orc_sim *s = (orc_sim *)calloc(1, sizeof(orc_sim));
   if (!s) return ORC_ENOMEM;
@@ -115,9 +118,10 @@ int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim *
     orc_destroy(s);
     return ORC_ENOMEM;
   }
+  s->n_net_links = (int32_t)L_net;
   for (int64_t l = 0; l < L; l++) {
-    s->lat[l] = d->hop_latency_s;
-    s->cap[l] = l < 2 * G ? d->nvlink_Bps : l < 4 * G ? d->nic_Bps : d->fabric_Bps;
+    s->lat[l] = l < L_net ? d->hop_latency_s : 0.0;
+    s->cap[l] = l < 2 * G ? d->nvlink_Bps : l < 4 * G ? d->nic_Bps : l < L_net ? d->fabric_Bps : 0x1p32;
   }
   *out = s;
   return ORC_OK;
@@ -163,6 +167,10 @@ uint64_t orc_mix64(uint64_t x) { /* SplitMix64 step (Steele, Lea, Flood 2014) */
 /* writes the path of (src,dst,conn) into p[0..5], returns its length */
 static int32_t route(const orc_sim *s, int32_t src, int32_t dst, int32_t conn, int32_t *p) {
   const orc_topology_desc *d = &s->d;
+  if (src == dst) { /* S7: a compute span; conn is its lane */
+    p[0] = s->n_net_links + src * d->compute_lanes + conn;
+    return 1;
+  }
   int32_t hs = src / d->gpus_per_host, hd = dst / d->gpus_per_host;
   if (hs == hd) {
     p[0] = nvl_up(src);
@@ -323,7 +331,16 @@ int32_t orc_add_collective(orc_sim *s, int32_t kind, const int32_t *ranks, int32
  * `start` and the `after` edges apply to every flow that has no predecessor inside the collective. */
 int32_t orc_add_collective_ex(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t N, double bytes, double start,
                               const int32_t *after, int32_t n_after, int32_t chunks, int32_t *out_id) {
+  return orc_add_collective_full(s, kind, ranks, N, bytes, start, after, n_after, NULL, 0, chunks, out_id);
+}
+
+int32_t orc_add_collective_full(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t N, double bytes, double start,
+                                const int32_t *after, int32_t n_after, const int64_t *after_flows, int32_t n_after_flows,
+                                int32_t chunks, int32_t *out_id) {
   if (!s || !ranks) return ORC_EINVAL;
+  if (n_after_flows < 0 || (n_after_flows > 0 && !after_flows)) return ORC_EINVAL;
+  for (int32_t k = 0; k < n_after_flows; k++)
+    if (after_flows[k] < 0 || after_flows[k] >= s->F) return ORC_EINVAL; /* only flows submitted before */
   if (s->ran) return ORC_ESTATE;
   if (kind < 0 || kind > ORC_ALLREDUCE_TREE || N < 2 || !(bytes > 0) || !(bytes < INFINITY) || !(start >= 0) ||
       !(start < INFINITY))
@@ -358,7 +375,14 @@ int32_t orc_add_collective_ex(orc_sim *s, int32_t kind, const int32_t *ranks, in
   memcpy(c->ranks, ranks, sizeof(int32_t) * N);
   s->n_coll++; /* (ranks now owned by the table) */
   int32_t first = c->first_flow;
-#define PUSH_AFTER(rho) if (push_after_edges(s, after, n_after, (rho))) return ORC_ENOMEM
+  /* edges of an initial flow sent by rho: the `after` collectives, then the listed flows / spans that touch rho */
+#define PUSH_AFTER(rho)                                                              \
+  do {                                                                               \
+    if (push_after_edges(s, after, n_after, (rho))) return ORC_ENOMEM;               \
+    for (int32_t k_ = 0; k_ < n_after_flows; k_++)                                   \
+      if (s->src[after_flows[k_]] == (rho) || s->dst[after_flows[k_]] == (rho))      \
+        if (push_pred(s, (int32_t)after_flows[k_])) return ORC_ENOMEM;               \
+  } while (0)
 
   if (kind == ORC_ALLTOALL) {
     double chunk = bytes / (double)N; /* S3: one f64 division */
@@ -446,6 +470,36 @@ int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *
   for (int64_t i = 0; i < n; i++) {
     int32_t conn = conn_id ? conn_id[i] : (int32_t)(first + i);
     if (begin_flow(s, src[i], dst[i], bytes[i], start ? start[i] : 0.0, conn)) return ORC_ENOMEM;
+    if (dep_off)
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; e++)
+        if (push_pred(s, (int32_t)dep_ids[e])) return ORC_ENOMEM;
+    commit_flow(s);
+  }
+  if (out_first) *out_first = first;
+  return ORC_OK;
+}
+
+/* S7: compute spans = flows of duration * 2^32 work units over the engine link of (gpu, lane) */
+int32_t orc_add_spans(orc_sim *s, int64_t n, const int32_t *gpu, const int32_t *lane, const double *duration,
+                      const double *start, const int64_t *dep_off, const int64_t *dep_ids, int64_t *out_first) {
+  if (!s || n < 0 || (n > 0 && (!gpu || !duration))) return ORC_EINVAL;
+  if (s->ran) return ORC_ESTATE;
+  if (s->d.compute_lanes <= 0) return ORC_EINVAL;
+  if (s->F + n > 0x7ffffff0) return ORC_ERANGE;
+  int64_t first = s->F;
+  for (int64_t i = 0; i < n; i++) {
+    if (gpu[i] < 0 || gpu[i] >= s->G) return ORC_EINVAL;
+    if (lane && (lane[i] < 0 || lane[i] >= s->d.compute_lanes)) return ORC_EINVAL;
+    if (!(duration[i] > 0) || !(duration[i] < 0x1p20)) return ORC_EINVAL;
+    if (start && (!(start[i] >= 0) || !(start[i] < INFINITY))) return ORC_EINVAL;
+    if (dep_off) {
+      if (dep_off[i + 1] < dep_off[i] || (dep_off[i + 1] > dep_off[i] && !dep_ids)) return ORC_EINVAL;
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; e++)
+        if (dep_ids[e] < 0 || dep_ids[e] >= first + i) return ORC_EINVAL;
+    }
+  }
+  for (int64_t i = 0; i < n; i++) {
+    if (begin_flow(s, gpu[i], gpu[i], duration[i] * 0x1p32, start ? start[i] : 0.0, lane ? lane[i] : 0)) return ORC_ENOMEM;
     if (dep_off)
       for (int64_t e = dep_off[i]; e < dep_off[i + 1]; e++)
         if (push_pred(s, (int32_t)dep_ids[e])) return ORC_ENOMEM;

@@ -60,6 +60,7 @@ typedef struct {
   double nvlink_Bps, nic_Bps, fabric_Bps, hop_latency_s; /* per direction */
   int32_t n_leaves, n_spines, uplinks_per_leaf_spine;    /* leaf-spine */
   int32_t k, agg_uplinks;                                /* fat tree */
+  int32_t compute_lanes;                                 /* NEXT-2: compute engines per GPU (0 = none), see orc_add_spans */
 } orc_topology_desc;
 
 typedef struct {
@@ -85,6 +86,22 @@ int32_t orc_add_collective_ex(orc_sim *s, int32_t kind, const int32_t *ranks, in
 int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *dst, const double *bytes,
                       const double *start_time_s, const int64_t *dep_off, const int64_t *dep_flow_ids,
                       const int32_t *conn_id, int64_t *out_first_flow_id);
+/* NEXT-2, compute spans (PAPER.md L84 / L94 / L106: the event queue holds compute and communication spans with
+ * explicit dependencies; L206 / Fig. 7: computation overlaps communication).  A span is a DAG node of fixed length
+ * bound to a compute engine ("lane") of a GPU.  Reading S7: every GPU has `compute_lanes` engine links,
+ * numbered after all network links (id = n_network_links + gpu * compute_lanes + lane), of capacity 2^32 work
+ * units / s and latency 0; a span of d seconds is a flow of d * 2^32 units over its engine link (src = dst = gpu).
+ * Alone on its lane it runs at 2^32 units / s, so it finishes at exactly t_act + d (scaling by a power of two is
+ * exact); spans that overlap on one lane share it max-min fairly (processor sharing).  Spans take flow ids like
+ * raw flows, depend on earlier flows / spans, and flows may depend on them. */
+int32_t orc_add_spans(orc_sim *s, int64_t n, const int32_t *gpu, const int32_t *lane, const double *duration_s,
+                      const double *start_time_s, const int64_t *dep_off, const int64_t *dep_flow_ids,
+                      int64_t *out_first_flow_id);
+/* orc_add_collective_ex plus flow-level predecessors: every flow of the collective that has no predecessor inside it
+ * and is sent by rank rho additionally waits for each listed EARLIER flow or span whose source or destination is rho */
+int32_t orc_add_collective_full(orc_sim *s, int32_t kind, const int32_t *ranks, int32_t n_ranks, double bytes,
+                                double start_time_s, const int32_t *after, int32_t n_after, const int64_t *after_flows,
+                                int32_t n_after_flows, int32_t chunks, int32_t *out_coll_id);
 /* trace != 0 additionally records, for every loop iteration, the active flows and their rates */
 int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace);
 /* same, but stops before the first event later than t_stop ("advancing the simulation ... up to a

@@ -24,7 +24,7 @@ class TopologyDesc(C.Structure):
                 ("nvlink_Bps", C.c_double), ("nic_Bps", C.c_double), ("fabric_Bps", C.c_double),
                 ("hop_latency_s", C.c_double),
                 ("n_leaves", C.c_int32), ("n_spines", C.c_int32), ("uplinks_per_leaf_spine", C.c_int32),
-                ("k", C.c_int32), ("agg_uplinks", C.c_int32)]
+                ("k", C.c_int32), ("agg_uplinks", C.c_int32), ("compute_lanes", C.c_int32)]
 
 
 class Counters(C.Structure):
@@ -41,7 +41,7 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
 # every symbol include/phs.h declares (tests check that the library exports all of them)
 SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
            "phs_set_link_capacities_batch",
-           "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_batch", "phs_add_flows",
+           "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_full", "phs_add_spans", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
            "phs_set_decomposition", "phs_set_windows", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
@@ -127,19 +127,36 @@ def phs_get_link_capacities(h, instance):
     return cap
 
 
-def phs_add_collective(h, instance, kind, ranks, nbytes, start=0.0, after=(), chunks=1):
+def phs_add_collective(h, instance, kind, ranks, nbytes, start=0.0, after=(), chunks=1, after_flows=()):
     ranks = _arr(ranks, np.int32)
     after = _arr(after, np.int32)
+    after_flows = _arr(after_flows, np.int64)
     cid = C.c_int32()
-    if chunks == 1:
+    if chunks == 1 and not len(after_flows):
         _chk(lib().phs_add_collective(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
                                       C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
                                       C.c_int32(len(after)), C.byref(cid)), "phs_add_collective")
     else:
-        _chk(lib().phs_add_collective_ex(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
-                                         C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
-                                         C.c_int32(len(after)), C.c_int32(chunks), C.byref(cid)), "phs_add_collective_ex")
+        _chk(lib().phs_add_collective_full(h, C.c_int32(instance), C.c_int32(kind), _p(ranks), C.c_int32(len(ranks)),
+                                           C.c_double(nbytes), C.c_double(start), _p(after) if len(after) else None,
+                                           C.c_int32(len(after)), _p(after_flows) if len(after_flows) else None,
+                                           C.c_int32(len(after_flows)), C.c_int32(chunks), C.byref(cid)),
+             "phs_add_collective_full")
     return cid.value
+
+
+def phs_add_spans(h, instance, gpu, duration, lane=None, start=None, dep_off=None, dep_ids=None):
+    gpu, lane = _arr(gpu, np.int32), _arr(lane, np.int32)
+    duration, start = _arr(duration, np.float64), _arr(start, np.float64)
+    dep_off, dep_ids = _arr(dep_off, np.int64), _arr(dep_ids, np.int64)
+    n = len(gpu)
+    if len(duration) != n or (lane is not None and len(lane) != n) or (start is not None and len(start) != n) or \
+            (dep_off is not None and len(dep_off) != n + 1):
+        raise ValueError("span arrays have inconsistent lengths")
+    first = C.c_int64()
+    _chk(lib().phs_add_spans(h, C.c_int32(instance), C.c_int64(n), _p(gpu), _p(lane), _p(duration), _p(start),
+                             _p(dep_off), _p(dep_ids), C.byref(first)), "phs_add_spans")
+    return first.value
 
 
 def phs_add_collective_batch(h, kind, ranks, nbytes, start=None, after=()):
@@ -386,7 +403,7 @@ class Sim:
         same = getattr(w, "uniform_ops", False)      # the generator states it; otherwise compare
         if not same and count > 1:
             same = all(len(x.ops) == len(insts[0].ops) for x in insts) and all(
-                isinstance(o, W.Coll) and o.chunks == 1 for x in insts for o in x.ops)
+                isinstance(o, W.Coll) and o.chunks == 1 and not len(o.after_flows) for x in insts for o in x.ops)
             for k, op0 in enumerate(insts[0].ops) if same else ():
                 ok = all(x.ops[k].kind == op0.kind and np.array_equal(x.ops[k].ranks, op0.ranks)
                          and tuple(x.ops[k].after) == tuple(op0.after) for x in insts)
@@ -400,9 +417,10 @@ class Sim:
         else:
             for i, inst in enumerate(insts):
                 W.apply(inst,
-                        lambda kind, ranks, nb, st, after, chunks=1, i=i: phs_add_collective(sim.h, i, kind, ranks, nb, st,
-                                                                                             after, chunks),
-                        lambda src, dst, nb, st, do, di, conn, i=i: phs_add_flows(sim.h, i, src, dst, nb, st, do, di, conn))
+                        lambda kind, ranks, nb, st, after, chunks=1, after_flows=(), i=i: phs_add_collective(
+                            sim.h, i, kind, ranks, nb, st, after, chunks, after_flows),
+                        lambda src, dst, nb, st, do, di, conn, i=i: phs_add_flows(sim.h, i, src, dst, nb, st, do, di, conn),
+                        lambda gpu, dur, lane, st, do, di, i=i: phs_add_spans(sim.h, i, gpu, dur, lane, st, do, di))
         return sim
 
     def finalize(self, stream=None):

@@ -123,6 +123,36 @@ phs_status phs_add_collective(phs_sim *sim, int32_t instance, int32_t kind, cons
 phs_status phs_add_collective_ex(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                                  double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
                                  int32_t *out_id) {
+  return phs_add_collective_full(sim, instance, kind, ranks, n_ranks, bytes, start, after, n_after, nullptr, 0, chunks,
+                                 out_id);
+}
+
+phs_status phs_add_spans(phs_sim *sim, int32_t instance, int64_t n, const int32_t *gpu, const int32_t *lane,
+                         const double *duration, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                         int64_t *out_first) {
+  PHS_API_BEGIN
+  phs_status st = check_instance(sim, instance, true);
+  if (st != PHS_OK) return st;
+  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
+  if (instance < 0)
+    for (int i = 1; i < sim->batch; ++i)
+      if (sim->inst[i].n_flows() != sim->inst[0].n_flows())
+        return fail(PHS_ESTATE, "instance -1 needs the same number of flows in every instance");
+  const int64_t first = sim->inst[lo].n_flows();
+  std::string why;
+  for (int i = lo; i < hi; ++i) {
+    st = append_spans(*sim->fab, sim->inst[i], n, gpu, lane, duration, start, dep_off, dep_ids, &why);
+    if (st != PHS_OK) return fail(st, why);
+  }
+  if (out_first) *out_first = first;
+  return PHS_OK;
+  PHS_API_END
+}
+
+phs_status phs_add_collective_full(phs_sim *sim, int32_t instance, int32_t kind, const int32_t *ranks, int32_t n_ranks,
+                                   double bytes, double start, const int32_t *after, int32_t n_after,
+                                   const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, int32_t *out_id) {
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
@@ -134,7 +164,8 @@ phs_status phs_add_collective_ex(phs_sim *sim, int32_t instance, int32_t kind, c
         return fail(PHS_ESTATE, "instance -1 needs the same number of collectives in every instance");
   std::string why;
   for (int i = lo; i < hi; ++i) {
-    st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes, start, after, n_after, chunks, &why);
+    st = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes, start, after, n_after, after_flows,
+                           n_after_flows, chunks, &why);
     if (st != PHS_OK) return fail(st, why);  // validation fails on the first instance, before any mutation
   }
   if (out_id) *out_id = (int32_t)sim->inst[lo].colls.size() - 1;
@@ -160,7 +191,7 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
   std::string why;
   for (int i = 0; i < sim->batch; ++i) {
     phs_status sti = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
-                                       after, n_after, 1, &why);
+                                       after, n_after, nullptr, 0, 1, &why);
     if (sti != PHS_OK) return fail(sti, why);
   }
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;

@@ -46,6 +46,8 @@ phs_status Fabric::validate(const phs_topology_desc &d, std::string *why) {
     default:
       return bad("unknown topology kind");
   }
+  if (d.compute_lanes < 0 || d.compute_lanes > 64) return bad("compute_lanes must be in [0, 64]");
+  links += (int64_t)d.n_hosts * d.gpus_per_host * d.compute_lanes;
   if (links > 0x3fffffff) {
     if (why) *why = "too many links";
     return PHS_ERANGE;
@@ -65,11 +67,14 @@ Fabric::Fabric(const phs_topology_desc &d) : d_(d) {
     tier2_base_ = tier1_base_ + 2 * d.k * half * half;
     links_ = tier2_base_ + 2 * d.k * half * d.agg_uplinks;
   }
+  net_links_ = links_;
+  links_ += gpus_ * d.compute_lanes;  // compute engine links (phs_add_spans) follow the network links
 }
 
 double Fabric::default_capacity(int32_t link) const {
   if (link < 2 * gpus_) return d_.nvlink_Bps;
   if (link < 4 * gpus_) return d_.nic_Bps;
+  if (link >= net_links_) return 0x1p32;  // work units per second of a compute lane
   return d_.fabric_Bps;
 }
 
@@ -86,6 +91,10 @@ uint64_t splitmix64_step(uint64_t x) {
 
 // ------------------------------------------------------------------------------------------------ ECMP (S2)
 int Fabric::route(uint64_t seed, int32_t src, int32_t dst, int32_t conn, int32_t *out) const {
+  if (src == dst) {  // a compute span: the engine link of lane `conn` of the GPU
+    out[0] = net_links_ + src * d_.compute_lanes + conn;
+    return 1;
+  }
   const int gph = d_.gpus_per_host;
   const int host_s = src / gph, host_d = dst / gph;
   if (host_s == host_d) {  // stays on the host's NVSwitch
@@ -221,8 +230,8 @@ void chain_after(Instance &inst, const Collective &a, int32_t rho) {
 }  // namespace
 
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t N,
-                             double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
-                             std::string *why) {
+                             double bytes, double start, const int32_t *after, int32_t n_after,
+                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why) {
   auto bad = [&](const char *m) {
     if (why) *why = m;
     return PHS_EINVAL;
@@ -245,6 +254,9 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   }
   for (int a = 0; a < n_after; ++a)
     if (after[a] < 0 || after[a] >= (int32_t)inst.colls.size()) return bad("after_coll_ids names an unknown collective");
+  if (n_after_flows < 0 || (n_after_flows > 0 && !after_flows)) return bad("bad after_flow_ids");
+  for (int a = 0; a < n_after_flows; ++a)
+    if (after_flows[a] < 0 || after_flows[a] >= inst.n_flows()) return bad("after_flow_ids must name earlier flows");
   const int steps = kind == PHS_ALLREDUCE_RING ? 2 * (N - 1) : kind == PHS_ALLTOALL ? 1 : N - 1;
   const int64_t nf = kind == PHS_ALLTOALL          ? (int64_t)N * (N - 1)
                      : kind == PHS_ALLREDUCE_TREE  ? (int64_t)chunks * 2 * (N - 1)
@@ -267,6 +279,7 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   c.bytes = bytes;
   c.start = start;
   c.after.assign(after, after + n_after);
+  c.after_flows.assign(after_flows, after_flows + n_after_flows);
   inst.flow_count += nf;
   inst.colls.push_back(std::move(c));
   return PHS_OK;
@@ -283,6 +296,13 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
   const int n_after = (int)c.after.size();
   const double start = c.start;
   const int32_t conn = id;  // ECMP key: one path per (pair, collective)
+  // dependencies of an initial flow sent by rank rho: the `after` collectives, then the listed earlier flows / spans
+  // that start or end at rho
+  auto initial_edges = [&](int32_t rho) {
+    for (int k = 0; k < n_after; ++k) chain_after(inst, inst.colls[after[k]], rho);
+    for (int32_t f : inst.colls[(size_t)id].after_flows)
+      if (inst.src[(size_t)f] == rho || inst.dst[(size_t)f] == rho) push_dep(inst, f);
+  };
   const double chunk = c.bytes / (double)N;
   if (c.kind == PHS_BROADCAST_CHAIN || c.kind == PHS_REDUCE_CHAIN) {
     // NEXT-3: pipelined chain.  Hop i carries every chunk in turn: chunk-major flow order, hop i of
@@ -295,8 +315,7 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
         if (ch == 0) {
           const int a = c.kind == PHS_BROADCAST_CHAIN ? i : N - 1 - i, b = c.kind == PHS_BROADCAST_CHAIN ? i + 1 : N - 2 - i;
           push_flow(fab, inst, ranks[a], ranks[b], piece, i == 0 ? start : 0.0, conn);
-          if (i == 0)
-            for (int k = 0; k < n_after; ++k) chain_after(inst, inst.colls[after[k]], ranks[a]);
+          if (i == 0) initial_edges(ranks[a]);
         } else {
           repeat_flow(inst, (size_t)c.first_flow + (size_t)i);
         }
@@ -314,8 +333,7 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
         const bool leaf_first = ch == 0 && l >= N;
         if (ch == 0) {
           push_flow(fab, inst, ranks[i], ranks[(i - 1) / 2], piece, leaf_first ? start : 0.0, conn);
-          if (leaf_first)
-            for (int k = 0; k < n_after; ++k) chain_after(inst, inst.colls[after[k]], ranks[i]);
+          if (leaf_first) initial_edges(ranks[i]);
         } else {
           repeat_flow(inst, (size_t)c.first_flow + (size_t)(i - 1));
         }
@@ -343,7 +361,7 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
       for (int j = 0; j < N; ++j) {
         if (i == j) continue;
         push_flow(fab, inst, ranks[i], ranks[j], chunk, start, conn);
-        for (int a = 0; a < n_after; ++a) chain_after(inst, inst.colls[after[a]], ranks[i]);
+        initial_edges(ranks[i]);
       }
   } else {
     // step-major: flow (s, i) sends chunk from ranks[i] to ranks[i+1]; it waits for the chunk it forwards
@@ -355,7 +373,7 @@ void expand_collective(const Fabric &fab, Instance &inst, int32_t id) {
         if (s == 0) {
           const int next_rank = i + 1 == N ? 0 : i + 1;
           push_flow(fab, inst, ranks[i], ranks[next_rank], chunk, start, conn);
-          for (int a = 0; a < n_after; ++a) chain_after(inst, inst.colls[after[a]], ranks[i]);
+          initial_edges(ranks[i]);
         } else {
           repeat_flow(inst, (size_t)c.first_flow + (size_t)i);
           push_dep(inst, prev + (i == 0 ? N - 1 : i - 1));
@@ -410,6 +428,43 @@ phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int3
   for (int64_t i = 0; i < n; ++i) {
     const int32_t id = (int32_t)(first + i);
     push_flow(fab, inst, src[i], dst[i], bytes[i], start ? start[i] : 0.0, conn_id ? conn_id[i] : id);
+    if (dep_off)
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) push_dep(inst, (int32_t)dep_ids[e]);
+  }
+  inst.flow_count += n;
+  return PHS_OK;
+}
+
+// Compute spans: flows of duration * 2^32 work units over the engine link of (gpu, lane); src = dst = gpu marks them.
+phs_status append_spans(const Fabric &fab, Instance &inst, int64_t n, const int32_t *gpu, const int32_t *lane,
+                        const double *duration, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                        std::string *why) {
+  auto bad = [&](const char *m) {
+    if (why) *why = m;
+    return PHS_EINVAL;
+  };
+  if (n < 0 || (n > 0 && (!gpu || !duration))) return bad("null span arrays");
+  if (fab.compute_lanes() <= 0) return bad("the topology has no compute lanes (phs_topology_desc.compute_lanes)");
+  expand_pending(fab, inst);  // flow ids follow submission order
+  const int64_t first = inst.n_flows();
+  if (first + n > 0x7ffffff0LL) {
+    if (why) *why = "too many flows in one instance";
+    return PHS_ERANGE;
+  }
+  for (int64_t i = 0; i < n; ++i) {
+    if (gpu[i] < 0 || gpu[i] >= fab.n_gpus()) return bad("gpu out of range");
+    if (lane && (lane[i] < 0 || lane[i] >= fab.compute_lanes())) return bad("lane out of range");
+    if (!(duration[i] > 0.0) || !(duration[i] < 0x1p20)) return bad("duration_s must be in (0, 2^20)");
+    if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return bad("start_time_s must be >= 0 and finite");
+    if (dep_off) {
+      if (dep_off[i + 1] < dep_off[i]) return bad("dep_off must be non-decreasing");
+      if (dep_off[i + 1] > dep_off[i] && !dep_ids) return bad("dep_flow_ids is null");
+      for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e)
+        if (dep_ids[e] < 0 || dep_ids[e] >= first + i) return bad("a span may only depend on earlier flows");
+    }
+  }
+  for (int64_t i = 0; i < n; ++i) {
+    push_flow(fab, inst, gpu[i], gpu[i], duration[i] * 0x1p32, start ? start[i] : 0.0, lane ? lane[i] : 0);
     if (dep_off)
       for (int64_t e = dep_off[i]; e < dep_off[i + 1]; ++e) push_dep(inst, (int32_t)dep_ids[e]);
   }

@@ -80,6 +80,7 @@ struct Collective {
   // that build the instance's tables
   double bytes = 0.0, start = 0.0;
   std::vector<int32_t> after;
+  std::vector<int32_t> after_flows;  // earlier flows / spans the initial flows additionally wait for, per rank
 };
 
 struct Instance {
@@ -105,13 +106,15 @@ class Fabric {
   int32_t n_gpus() const { return gpus_; }
   int32_t n_links() const { return links_; }
   double default_capacity(int32_t link) const;
-  double latency(int32_t /*link*/) const { return d_.hop_latency_s; }
+  double latency(int32_t link) const { return link < net_links_ ? d_.hop_latency_s : 0.0; }  // engine links: 0
+  int32_t n_net_links() const { return net_links_; }
+  int32_t compute_lanes() const { return d_.compute_lanes; }
   // writes the links of (src -> dst) for connection key `conn` into out[0..kMaxHops), returns the hop count
   int route(uint64_t seed, int32_t src, int32_t dst, int32_t conn, int32_t *out) const;
 
  private:
   phs_topology_desc d_;
-  int32_t gpus_, links_, tier1_base_, tier2_base_;
+  int32_t gpus_, links_, net_links_, tier1_base_, tier2_base_;
 };
 
 uint64_t splitmix64_step(uint64_t x);
@@ -122,8 +125,11 @@ void expand_pending(const Fabric &fab, Instance &inst);
 // Appends flows / collectives to an instance (S3).  Return PHS_OK or an error with *why set.  append_collective
 // validates and records the collective; its flows appear with the next expand_pending.
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t n_ranks,
-                             double bytes, double start, const int32_t *after, int32_t n_after, int32_t chunks,
-                             std::string *why);
+                             double bytes, double start, const int32_t *after, int32_t n_after,
+                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why);
+phs_status append_spans(const Fabric &fab, Instance &inst, int64_t n, const int32_t *gpu, const int32_t *lane,
+                        const double *duration, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
+                        std::string *why);
 phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int32_t *src, const int32_t *dst,
                         const double *bytes, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
                         const int32_t *conn_id, std::string *why);

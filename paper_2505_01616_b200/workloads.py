@@ -26,10 +26,11 @@ def gbps(x):
 
 
 def topo_desc(kind, n_hosts, gpus_per_host, nvlink_Bps=450e9, nic_Bps=50e9, fabric_Bps=50e9, hop_latency_s=1e-6,
-              n_leaves=0, n_spines=0, uplinks_per_leaf_spine=0, k=0, agg_uplinks=0):
+              n_leaves=0, n_spines=0, uplinks_per_leaf_spine=0, k=0, agg_uplinks=0, compute_lanes=0):
     return dict(kind=kind, n_hosts=n_hosts, gpus_per_host=gpus_per_host, nvlink_Bps=nvlink_Bps, nic_Bps=nic_Bps,
                 fabric_Bps=fabric_Bps, hop_latency_s=hop_latency_s, n_leaves=n_leaves, n_spines=n_spines,
-                uplinks_per_leaf_spine=uplinks_per_leaf_spine, k=k, agg_uplinks=agg_uplinks)
+                uplinks_per_leaf_spine=uplinks_per_leaf_spine, k=k, agg_uplinks=agg_uplinks,
+                compute_lanes=compute_lanes)
 
 
 @dataclass
@@ -40,6 +41,18 @@ class Coll:
     start: float = 0.0
     after: tuple = ()
     chunks: int = 1          # pipeline chunks of the chain / tree kinds
+    after_flows: tuple = ()  # flow / span ids its initial flows additionally wait for (per rank)
+
+
+@dataclass
+class Spans:
+    """Compute spans (NEXT-2): fixed-duration DAG nodes on a compute lane of a GPU."""
+    gpu: np.ndarray
+    duration: np.ndarray
+    lane: Optional[np.ndarray] = None
+    start: Optional[np.ndarray] = None
+    dep_off: Optional[np.ndarray] = None
+    dep_ids: Optional[np.ndarray] = None
 
 
 @dataclass
@@ -65,11 +78,13 @@ class Instance:
         if self.cap_pairs_Gbps is None:
             return None
         G = desc["n_hosts"] * desc["gpus_per_host"]
+        n_net = n_links - G * desc.get("compute_lanes", 0)       # compute engine links follow the network links
         cap = np.full(n_links, desc["nvlink_Bps"], dtype=np.float64)
-        pairs = (n_links - 2 * G) // 2
+        pairs = (n_net - 2 * G) // 2
         assert len(self.cap_pairs_Gbps) == pairs
-        cap[2 * G::2] = gbps(self.cap_pairs_Gbps)
-        cap[2 * G + 1::2] = gbps(self.cap_pairs_Gbps)
+        cap[2 * G:n_net:2] = gbps(self.cap_pairs_Gbps)
+        cap[2 * G + 1:n_net:2] = gbps(self.cap_pairs_Gbps)
+        cap[n_net:] = 2.0 ** 32                                   # work units / s of a compute lane
         return cap
 
     @property
@@ -84,12 +99,14 @@ def capacity_matrix(desc, insts, n_links):
     if not insts or any(x.cap_pairs_Gbps is None for x in insts):
         return None
     G = desc["n_hosts"] * desc["gpus_per_host"]
-    pairs = (n_links - 2 * G) // 2
+    n_net = n_links - G * desc.get("compute_lanes", 0)
+    pairs = (n_net - 2 * G) // 2
     p = np.stack([np.asarray(x.cap_pairs_Gbps, dtype=np.float64) for x in insts])
     assert p.shape == (len(insts), pairs)
     cap = np.full((len(insts), n_links), desc["nvlink_Bps"], dtype=np.float64)
-    cap[:, 2 * G::2] = gbps(p)
-    cap[:, 2 * G + 1::2] = gbps(p)
+    cap[:, 2 * G:n_net:2] = gbps(p)
+    cap[:, 2 * G + 1:n_net:2] = gbps(p)
+    cap[:, n_net:] = 2.0 ** 32
     return cap
 
 
@@ -109,6 +126,8 @@ class Workload:
 def n_flows_of(op):
     if isinstance(op, RawFlows):
         return len(op.src)
+    if isinstance(op, Spans):
+        return len(op.gpu)
     N = len(op.ranks)
     return {ALLREDUCE_RING: 2 * (N - 1) * N, ALLGATHER_RING: (N - 1) * N, REDUCESCATTER_RING: (N - 1) * N,
             ALLTOALL: N * (N - 1), BROADCAST_CHAIN: op.chunks * (N - 1), REDUCE_CHAIN: op.chunks * (N - 1),
@@ -124,13 +143,17 @@ def _loguniform(rng, lo, hi, size=None):
     return np.floor(np.exp(rng.uniform(np.log(lo), np.log(hi), size)))
 
 
-def apply(inst: Instance, add_collective, add_flows):
-    """Replay an instance's ops through two callables with the signatures
-    add_collective(kind, ranks, nbytes, start, after[, chunks]) -> id ; add_flows(src, dst, nbytes, start, dep_off, dep_ids,
-    conn_id)."""
+def apply(inst: Instance, add_collective, add_flows, add_spans=None):
+    """Replay an instance's ops through callables with the signatures
+    add_collective(kind, ranks, nbytes, start, after[, chunks[, after_flows]]) -> id ;
+    add_flows(src, dst, nbytes, start, dep_off, dep_ids, conn_id) ; add_spans(gpu, duration, lane, start, dep_off, dep_ids)."""
     for op in inst.ops:
-        if isinstance(op, Coll):
-            if op.chunks == 1:
+        if isinstance(op, Spans):
+            add_spans(op.gpu, op.duration, op.lane, op.start, op.dep_off, op.dep_ids)
+        elif isinstance(op, Coll):
+            if len(op.after_flows):
+                add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after, op.chunks, op.after_flows)
+            elif op.chunks == 1:
                 add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after)
             else:
                 add_collective(op.kind, op.ranks, op.nbytes, op.start, op.after, op.chunks)
@@ -238,6 +261,56 @@ def cfg4(batch=8, n_hosts=32, gph=8, n_leaves=8, n_spines=8, mean_bytes=4 * MiB,
         nbytes = np.maximum(np.floor(nbytes), 1.0)
         insts.append(Instance(seed=i, ops=[RawFlows(src, dst, nbytes)]))
     return Workload("cfg4", d, 0, insts)
+
+
+# ---------------------------------------------------------------------------------------------- training step
+def train_step(batch=4, n_hosts=8, gph=8, n_leaves=2, n_spines=2, layers=4, buckets=4):
+    """cfg3's sweep with the compute of the step in the DAG (NEXT-2, PAPER.md L84 / L206): per layer one compute span
+    per GPU (U[20, 200] us; it waits for what that GPU sent and received in the previous layer's tensor-parallel
+    all-reduce), then the layer's TP all-reduce per host (a rank starts when its span is done); after the last layer
+    the gradient buckets, one DP all-reduce per local rank each, chained, the first behind the last layer's spans."""
+    d = topo_desc(TOPO_LEAF_SPINE, n_hosts, gph, fabric_Bps=gbps(400.0), n_leaves=n_leaves, n_spines=n_spines,
+                  uplinks_per_leaf_spine=1, compute_lanes=1)
+    G = n_hosts * gph
+    pairs = G + n_leaves * n_spines
+    tp_flows = 2 * (gph - 1) * gph
+    insts = []
+    for i in range(batch):
+        rng = _rng(5, i)
+        caps = rng.uniform(100.0, 800.0, pairs)
+        ops, nf, nc = [], 0, 0
+        prev_tp_first = None                       # first flow id of the previous layer's TP all-reduce, per host
+        span_first = 0
+        for layer in range(layers):
+            dep_off, dep_ids = [0], []
+            for g in range(G):
+                if prev_tp_first is not None:
+                    h, pos = divmod(g, gph)
+                    last = prev_tp_first[h] + (2 * (gph - 1) - 1) * gph
+                    dep_ids += [last + pos, last + (pos - 1) % gph]
+                dep_off.append(len(dep_ids))
+            span_first = nf
+            ops.append(Spans(np.arange(G, dtype=np.int32), rng.uniform(20e-6, 200e-6, G), None, None,
+                             np.array(dep_off, np.int64), np.array(dep_ids, np.int64)))
+            nf += G
+            prev_tp_first = []
+            for h in range(n_hosts):
+                prev_tp_first.append(nf)
+                ops.append(Coll(ALLREDUCE_RING, np.arange(h * gph, (h + 1) * gph, dtype=np.int32),
+                                float(_loguniform(rng, 1 * MiB, 64 * MiB)), 0.0, (), 1,
+                                tuple(range(span_first + h * gph, span_first + (h + 1) * gph))))
+                nf += tp_flows
+                nc += 1
+        base = nc
+        for b in range(buckets):
+            for j in range(gph):
+                after = () if b == 0 else (base + (b - 1) * gph + j,)
+                after_flows = tuple(range(span_first + j, span_first + G, gph)) if b == 0 else ()
+                ops.append(Coll(ALLREDUCE_RING, np.arange(j, G, gph, dtype=np.int32),
+                                float(_loguniform(rng, 1 * MiB, 256 * MiB)), 0.0, after, 1, after_flows))
+                nc += 1
+        insts.append(Instance(seed=i, ops=ops, cap_pairs_Gbps=caps))
+    return Workload("train_step", d, 0, insts)
 
 
 def by_name(name, **kw):

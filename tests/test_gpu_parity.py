@@ -207,6 +207,21 @@ def test_chain_and_tree_collectives_on_every_path():
     _grid_compare(w)
 
 
+def test_compute_spans_training_step_on_every_path():
+    """NEXT-2 (PAPER.md L84 / L206): compute spans in the DAG, overlapping the collectives; zero-latency engine links, so
+    released spans activate within the releasing event."""
+    w = W.train_step(batch=3, n_hosts=4, gph=4, layers=3, buckets=2)
+    for path in (0, CTA, CLUSTER):
+        run_and_compare(w, path=path)
+    _grid_compare(w)
+    # a span alone ends at exactly start + duration on the GPU as well
+    sim = B.Sim(W.topo_desc(W.TOPO_SINGLE, 1, 8, compute_lanes=2), batch=1)
+    B.phs_add_spans(sim.h, 0, [0, 5, 5], [1e-3, 3.3e-4, 7e-5], lane=[0, 0, 1], start=[0.0, 1e-4, 2.5e-4])
+    sim.run()
+    assert list(sim.completion_times(0)) == [1e-3, 1e-4 + 3.3e-4, 2.5e-4 + 7e-5]
+    sim.close()
+
+
 def test_cta_slot_overflow_falls_back_to_cluster():
     w = W.cfg4(batch=3, n_hosts=4, gph=8, n_leaves=2, n_spines=2)      # 992 flows pending at t=0 > 64 slots
     sim = B.Sim.from_workload(w, event_log=True, cta_slots=64)

@@ -100,6 +100,28 @@ def test_chain_and_tree_collectives_equal_the_oracle():
     sim.close()
 
 
+def test_compute_spans_and_flow_level_after_edges_equal_the_oracle():
+    """NEXT-2: a training step with compute spans in the DAG (spans behind collectives, collectives behind spans)."""
+    _compare_tables(W.train_step(batch=3, n_hosts=4, gph=4, layers=3, buckets=2))
+    d = W.topo_desc(W.TOPO_SINGLE, 2, 4)
+    sim = B.Sim(d, batch=1)
+    with pytest.raises(B.PhsError) as e:
+        B.phs_add_spans(sim.h, 0, [0], [1e-3])                    # the topology has no compute lanes
+    assert e.value.code == B.PHS_EINVAL
+    sim.close()
+    sim = B.Sim(W.topo_desc(W.TOPO_SINGLE, 2, 4, compute_lanes=1), batch=1)
+    assert B.phs_num_links(sim.h) == 32 + 8
+    for kw in (dict(gpu=[9], duration=[1e-3]), dict(gpu=[0], duration=[0.0]), dict(gpu=[0], duration=[1e-3], lane=[1]),
+               dict(gpu=[0], duration=[1e-3], dep_off=[0, 1], dep_ids=[0])):
+        with pytest.raises(B.PhsError) as e:
+            B.phs_add_spans(sim.h, 0, **kw)
+        assert e.value.code == B.PHS_EINVAL
+    assert B.phs_add_spans(sim.h, 0, [0, 1], [1e-3, 2e-3]) == 0
+    with pytest.raises(B.PhsError):
+        B.phs_add_collective(sim.h, 0, B.ALLGATHER_RING, [0, 1, 2], 1e6, after_flows=[5])      # not an earlier flow
+    sim.close()
+
+
 def test_deferred_expansion_keeps_submission_order():
     """phs_add_collective records the collective and its flows are expanded later (by the next raw-flow submission,
     a table getter, or phs_finalize).  Flow ids must still follow submission order, and reading tables between

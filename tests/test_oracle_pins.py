@@ -610,6 +610,51 @@ def test_next3_after_edges_against_hand_written_lists():
     assert [sorted(pr[off[f]:off[f + 1]].tolist()) for f in (4, 5, 6)] == [[0, 2], [4], [5]]
 
 
+# ------------------------------------------------------------------------------------------------ NEXT-2 compute spans
+def test_next2_compute_spans_closed_forms():
+    """Reading S7 (PAPER.md L84 / L94 / L106 / L206): a span alone on its lane ends at EXACTLY t_act + d (the 2^32
+    scaling is exact in binary64); spans overlapping on one lane share it (processor sharing, P6); a collective
+    chained behind compute is fully exposed (Dc + Tc), next to it fully overlapped (max)."""
+    d = single(n_hosts=1, gph=8, compute_lanes=2)
+    s = orc.Sim(d, 0)
+    assert s.num_links == 32 + 16                                     # engine links follow the network links
+    dur = [1e-3, 3.3e-4, 7e-5]
+    s.add_spans([0, 5, 5], dur, lane=[0, 0, 1], start=[0.0, 1e-4, 2.5e-4])
+    s.run()
+    assert list(s.completion_times()) == [0.0 + dur[0], 1e-4 + dur[1], 2.5e-4 + dur[2]]          # bit-equal
+    assert list(s.bottlenecks()) == [32 + 0, 32 + 5 * 2, 32 + 5 * 2 + 1]
+    # two spans on ONE lane at the same time: each gets half the engine (P6 with C = 2^32): 2 d, then the longer alone
+    s = orc.Sim(d, 0)
+    s.add_spans([3, 3], [1e-4, 3e-4], lane=[1, 1])
+    s.run()
+    np.testing.assert_allclose(s.completion_times(), [2e-4, 4e-4], rtol=1e-12)
+    # exposed: all-gather over ranks 0..3 behind a span on every rank; overlapped: the same side by side
+    Tc = 3 * (2e-6 + 1e6 / 450e9)
+    Dc = [2e-4, 5e-4, 1e-4, 3e-4]
+    s = orc.Sim(d, 0)
+    s.add_spans([0, 1, 2, 3], Dc)
+    s.add_collective(orc.ALLGATHER_RING, np.arange(4, dtype=np.int32), 4e6, after_flows=[0, 1, 2, 3])
+    last = s.add_spans([0], [1e-5], dep_off=[0, 2], dep_ids=[4 + 2 * 4 + 0, 4 + 2 * 4 + 3])     # rank 0's last send / receive
+    s.run()
+    t = s.completion_times()
+    step = 2e-6 + 1e6 / 450e9
+    # ring recurrence with staggered starts: T(0,i) = Dc[i] + step; T(s,i) = max(T(s-1,i), T(s-1,i-1)) + step
+    T = np.zeros((3, 4)); T[0] = np.array(Dc) + step
+    for st in range(1, 3):
+        for i in range(4):
+            T[st, i] = max(T[st - 1, i], T[st - 1, (i - 1) % 4]) + step
+    np.testing.assert_allclose(t[4:16].reshape(3, 4), T, rtol=1e-12)
+    assert t[last] == pytest.approx(max(T[2, 0], T[2, 3]) + 1e-5, rel=1e-12)
+    assert s.collective_times()[0] > max(Dc) + Tc * 0.99                                       # exposed
+    s = orc.Sim(d, 0)
+    s.add_spans([0, 1, 2, 3], Dc)
+    s.add_collective(orc.ALLGATHER_RING, np.arange(4, dtype=np.int32), 4e6)
+    s.run()
+    assert s.collective_times()[0] == pytest.approx(Tc, rel=1e-12)                             # overlapped
+    with pytest.raises(orc.OrcError):
+        orc.Sim(single(), 0).add_spans([0], [1e-3])                                            # no compute lanes
+
+
 # ------------------------------------------------------------------------------------------------ S2 routing pins
 def test_routing_leaf_spine_down_lane_comes_from_the_high_hash_word():
     """S2: with P parallel uplinks per (leaf, spine) the up lane is (H mod (n_spines P)) mod P and the down lane

@@ -12,10 +12,12 @@ def oracle_build(desc, inst, base_seed=0):
     if cap is not None:
         sim.set_link_capacities(cap)
     W.apply(inst,
-            lambda kind, ranks, nbytes, start, after, chunks=1: sim.add_collective(kind, ranks, nbytes, start, after,
-                                                                                   chunks),
+            lambda kind, ranks, nbytes, start, after, chunks=1, after_flows=(): sim.add_collective(
+                kind, ranks, nbytes, start, after, chunks, after_flows),
             lambda src, dst, nbytes, start, dep_off, dep_ids, conn: sim.add_flows(src, dst, nbytes, start, dep_off,
-                                                                                   dep_ids, conn))
+                                                                                   dep_ids, conn),
+            lambda gpu, duration, lane, start, dep_off, dep_ids: sim.add_spans(gpu, duration, lane, start, dep_off,
+                                                                               dep_ids))
     return sim
 
 
