@@ -174,6 +174,15 @@ class Sim:
             _chk(lib().orc_run_until(self._h, C.c_int32(mode), C.c_int32(1 if trace else 0), C.c_double(until)),
                  "orc_run_until")
 
+    def rollback(self, T):
+        _chk(lib().orc_rollback(self._h, C.c_double(T)), "orc_rollback")
+
+    def update_flow_start(self, flow, start):
+        _chk(lib().orc_update_flow_start(self._h, C.c_int64(flow), C.c_double(start)), "orc_update_flow_start")
+
+    def gc(self, T):
+        _chk(lib().orc_gc(self._h, C.c_double(T)), "orc_gc")
+
     @property
     def num_flows(self):
         n = C.c_int64()

@@ -57,9 +57,19 @@ struct orc_sim {
   /* throughput history: one record per rate change of a flow */
   int32_t *h_flow;
   double *h_t, *h_rate;
+  double *h_rem;     /* remaining bytes at h_t, after the settle (what a rollback restores, PAPER.md L128 / L167) */
+  int64_t *h_ev;     /* loop iteration (= index of the event it precedes) that wrote the record */
+  int64_t *h_rq;     /* the rate in quanta of 2^-20 byte/s (h_rate is its binary64 image, inexact above 2^53 quanta) */
   int64_t n_h, h_cap;
+  int64_t *done_ev;  /* per flow: index of the event in which it completed, -1 if it has not */
+  int64_t F_res;     /* flows t_done / bneck / done_ev are allocated for */
+  int64_t gc_events; /* events below this index cannot be rolled back into any more (orc_gc) */
   double work[7];
 };
+
+/* NEXT-1 (defined with the event loop): events with t < T; forget the events from index K on */
+static int64_t events_before(const orc_sim *s, double T);
+static int32_t rollback_events(orc_sim *s, int64_t K);
 
 /* ------------------------------------------------------------------ S1: topology & link numbering */
 static int32_t nvl_up(int32_t g) { return 2 * g; }
@@ -133,7 +143,7 @@ void orc_destroy(orc_sim *s) {
   free(s->coll); free(s->cap); free(s->lat); free(s->src); free(s->dst); free(s->conn); free(s->bytes);
   free(s->start); free(s->Lat); free(s->path_off); free(s->path); free(s->pred_off); free(s->pred);
   free(s->t_done); free(s->bneck); free(s->ev); free(s->tr);
-  free(s->h_flow); free(s->h_t); free(s->h_rate);
+  free(s->h_flow); free(s->h_t); free(s->h_rate); free(s->h_rem); free(s->h_ev); free(s->h_rq); free(s->done_ev);
   free(s);
 }
 
@@ -338,10 +348,11 @@ int32_t orc_add_collective_full(orc_sim *s, int32_t kind, const int32_t *ranks, 
                                 const int32_t *after, int32_t n_after, const int64_t *after_flows, int32_t n_after_flows,
                                 int32_t chunks, int32_t *out_id) {
   if (!s || !ranks) return ORC_EINVAL;
+  /* submitted after the simulation has run past its start time (L124): roll back to that time first */
+  if (s->n_ev > 0 && start >= 0 && rollback_events(s, events_before(s, start)) != ORC_OK) return ORC_EINVAL;
   if (n_after_flows < 0 || (n_after_flows > 0 && !after_flows)) return ORC_EINVAL;
   for (int32_t k = 0; k < n_after_flows; k++)
     if (after_flows[k] < 0 || after_flows[k] >= s->F) return ORC_EINVAL; /* only flows submitted before */
-  if (s->ran) return ORC_ESTATE;
   if (kind < 0 || kind > ORC_ALLREDUCE_TREE || N < 2 || !(bytes > 0) || !(bytes < INFINITY) || !(start >= 0) ||
       !(start < INFINITY))
     return ORC_EINVAL;
@@ -454,9 +465,13 @@ int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *
                       const double *start, const int64_t *dep_off, const int64_t *dep_ids, const int32_t *conn_id,
                       int64_t *out_first) {
   if (!s || n < 0 || (n > 0 && (!src || !dst || !bytes))) return ORC_EINVAL;
-  if (s->ran) return ORC_ESTATE;
   if (s->F + n > 0x7ffffff0) return ORC_ERANGE;
   int64_t first = s->F;
+  if (s->n_ev > 0 && n > 0) { /* late submission (L124): roll back to the earliest new start time */
+    double T2 = INFINITY;
+    for (int64_t i = 0; i < n; i++) { double st = start ? start[i] : 0.0; if (st < T2) T2 = st; }
+    if (!(T2 >= 0) || rollback_events(s, events_before(s, T2)) != ORC_OK) return ORC_EINVAL;
+  }
   for (int64_t i = 0; i < n; i++) { /* validate everything before mutating */
     if (src[i] < 0 || src[i] >= s->G || dst[i] < 0 || dst[i] >= s->G || src[i] == dst[i]) return ORC_EINVAL;
     if (!(bytes[i] > 0) || !(bytes[i] < INFINITY)) return ORC_EINVAL;
@@ -483,10 +498,14 @@ int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *
 int32_t orc_add_spans(orc_sim *s, int64_t n, const int32_t *gpu, const int32_t *lane, const double *duration,
                       const double *start, const int64_t *dep_off, const int64_t *dep_ids, int64_t *out_first) {
   if (!s || n < 0 || (n > 0 && (!gpu || !duration))) return ORC_EINVAL;
-  if (s->ran) return ORC_ESTATE;
   if (s->d.compute_lanes <= 0) return ORC_EINVAL;
   if (s->F + n > 0x7ffffff0) return ORC_ERANGE;
   int64_t first = s->F;
+  if (s->n_ev > 0 && n > 0) { /* late submission (L124): roll back to the earliest new start time */
+    double T2 = INFINITY;
+    for (int64_t i = 0; i < n; i++) { double st = start ? start[i] : 0.0; if (st < T2) T2 = st; }
+    if (!(T2 >= 0) || rollback_events(s, events_before(s, T2)) != ORC_OK) return ORC_EINVAL;
+  }
   for (int64_t i = 0; i < n; i++) {
     if (gpu[i] < 0 || gpu[i] >= s->G) return ORC_EINVAL;
     if (lane && (lane[i] < 0 || lane[i] >= s->d.compute_lanes)) return ORC_EINVAL;
@@ -747,6 +766,86 @@ int32_t orc_maxmin(int32_t n_links, const double *cap, int32_t n_flows, const in
   return rc;
 }
 
+/* ------------------------------------------------------------------ NEXT-1: time rollback
+ * The simulator may have run ahead (to T1) when something arrives with an earlier timestamp T2.  Rolling back keeps
+ * the events before T2 and forgets the rest: completion times, bottlenecks and history records written from the first
+ * dropped event on are discarded; the next run call rebuilds the state after the last kept event from the
+ * throughput history (see orc_run_ex) and simulates forward again. */
+static int64_t events_before(const orc_sim *s, double T) { /* events are in time order */
+  int64_t k = 0;
+  while (k < s->n_ev && s->ev[k].t < T) k++;
+  return k;
+}
+static int32_t rollback_events(orc_sim *s, int64_t K) {
+  if (K >= s->n_ev) return ORC_OK; /* nothing at or after that point has been simulated */
+  if (K < s->gc_events) return ORC_EINVAL; /* the history below the watermark is gone */
+  s->n_ev = K;
+  for (int64_t f = 0; f < s->F_res; f++)
+    if (s->done_ev[f] >= K) { s->done_ev[f] = -1; s->t_done[f] = NAN; s->bneck[f] = -1; }
+  int64_t keep = 0;
+  for (int64_t i = 0; i < s->n_h; i++)
+    if (s->h_ev[i] < K) {
+      s->h_flow[keep] = s->h_flow[i]; s->h_t[keep] = s->h_t[i]; s->h_rate[keep] = s->h_rate[i];
+      s->h_rem[keep] = s->h_rem[i]; s->h_ev[keep] = s->h_ev[i]; s->h_rq[keep] = s->h_rq[i];
+      keep++;
+    }
+  s->n_h = keep;
+  return ORC_OK;
+}
+/* everything from time T on is forgotten (events with t < T stay) */
+int32_t orc_rollback(orc_sim *s, double T) {
+  if (!s || !(T >= 0)) return ORC_EINVAL;
+  return rollback_events(s, events_before(s, T));
+}
+/* "updating the start time of an existing flow" (L167): rolls back to min(old, new) start time, then changes it */
+int32_t orc_update_flow_start(orc_sim *s, int64_t flow, double start) {
+  if (!s || flow < 0 || flow >= s->F || !(start >= 0) || !(start < INFINITY)) return ORC_EINVAL;
+  /* The start time acts through t_act = max(start, release) + Lat, release = completion of the flow's last
+   * predecessor (0 without predecessors).  If the flow has not been released in what was simulated so far, its start
+   * time has not been used yet; otherwise the past differs from max(old, release) or max(new, release) on, whichever is
+   * earlier -- unless the two are equal. */
+  double rel = 0.0;
+  int released = 1;
+  for (int64_t e = s->pred_off[flow]; e < s->pred_off[flow + 1]; e++) {
+    int32_t p = s->pred[e];
+    if (p >= s->F_res || s->done_ev[p] < 0) { released = 0; break; }
+    if (s->t_done[p] > rel) rel = s->t_done[p];
+  }
+  if (released && s->n_ev > 0) {
+    double a = s->start[flow] > rel ? s->start[flow] : rel, b = start > rel ? start : rel;
+    if (a != b) {
+      int32_t rc = rollback_events(s, events_before(s, a < b ? a : b));
+      if (rc != ORC_OK) return rc;
+    }
+  }
+  s->start[flow] = start;
+  return ORC_OK;
+}
+/* garbage collection (L130): nothing will ever be rolled back to a time before T, so every flow keeps only the last
+ * of its history records older than that; later rollbacks to times >= T are unaffected */
+int32_t orc_gc(orc_sim *s, double T) {
+  if (!s || !(T >= 0)) return ORC_EINVAL;
+  int64_t K = events_before(s, T);
+  if (K <= s->gc_events) return ORC_OK;
+  int64_t *last = (int64_t *)malloc(sizeof(int64_t) * (s->F + 1));
+  if (!last) return ORC_ENOMEM;
+  for (int64_t f = 0; f < s->F; f++) last[f] = -1;
+  for (int64_t i = 0; i < s->n_h; i++)
+    if (s->h_ev[i] < K) last[s->h_flow[i]] = i;
+  int64_t keep = 0;
+  for (int64_t i = 0; i < s->n_h; i++) {
+    int32_t f = s->h_flow[i];
+    if (s->h_ev[i] < K && (last[f] != i || (s->done_ev[f] >= 0 && s->done_ev[f] < K))) continue; /* superseded / done */
+    s->h_flow[keep] = s->h_flow[i]; s->h_t[keep] = s->h_t[i]; s->h_rate[keep] = s->h_rate[i];
+    s->h_rem[keep] = s->h_rem[i]; s->h_ev[keep] = s->h_ev[i]; s->h_rq[keep] = s->h_rq[i];
+    keep++;
+  }
+  s->n_h = keep;
+  s->gc_events = K;
+  free(last);
+  return ORC_OK;
+}
+
 /* ------------------------------------------------------------------ S4: flow states & event loop */
 /* S4.4 / Q11: remaining bytes after draining at `rate` for dt seconds: mul, then sub, then clamp at 0.  (Under
  * R-LZ the clamp is a guard: DESIGN.md sec 2 argues that a flow still active at `now` < tc cannot have drained
@@ -775,8 +874,13 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
   if (!s || (mode != ORC_MODE_NAIVE && mode != ORC_MODE_FAST)) return ORC_EINVAL;
   if (flags & ~(ORC_FLAG_SETTLE_EVERY_EVENT | ORC_FLAG_F64_SHARES)) return ORC_EINVAL;
   if ((flags & ORC_FLAG_F64_SHARES) && mode != ORC_MODE_NAIVE) return ORC_EINVAL; /* dense argmin only */
-  if (s->ran) return ORC_ESTATE;
+  /* A run CONTINUES from the events kept so far (s->n_ev of them: all of an earlier run that stopped at a time, or
+   * fewer after orc_rollback): the state after event K-1 is rebuilt from the throughput history, as PAPER.md L128
+   * describes ("we know each flow's throughput at any given time, we can calculate the amount of data transferred
+   * ... and consequently recover the simulator state").  The comparison modes and the trace are whole runs only. */
+  if ((s->ran || s->n_ev > 0) && (flags || trace)) return ORC_ESTATE;
   int64_t F = s->F;
+  const int64_t K = s->n_ev;
   int32_t L = s->n_links, rc = ORC_OK;
   ws_t w;
   memset(&w, 0, sizeof(w));
@@ -796,8 +900,17 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
   int32_t *act = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *pend = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
   int32_t *comp = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
-  s->t_done = (double *)malloc(sizeof(double) * (F + 1));
-  s->bneck = (int32_t *)malloc(sizeof(int32_t) * (F + 1));
+  if (s->F_res < F || !s->t_done) { /* results: kept across runs, extended for flows added since */
+    void *a = realloc(s->t_done, sizeof(double) * (F + 1)), *b, *d;
+    if (a) s->t_done = (double *)a;
+    b = realloc(s->bneck, sizeof(int32_t) * (F + 1));
+    if (b) s->bneck = (int32_t *)b;
+    d = realloc(s->done_ev, sizeof(int64_t) * (F + 1));
+    if (d) s->done_ev = (int64_t *)d;
+    if (!a || !b || !d) { rc = ORC_ENOMEM; goto out; }
+    for (int64_t f = s->F_res; f < F; f++) { s->t_done[f] = NAN; s->bneck[f] = -1; s->done_ev[f] = -1; }
+    s->F_res = F;
+  }
   if (!capq || !succ_off || !succ || !pred_cnt || !state || !t_act || !rem || !tc || !rq || !rq_cur || !t_last || !rate_d || !rate_cur || !act || !pend || !comp ||
       !s->t_done || !s->bneck || ws_init(&w, L)) {
     rc = ORC_ENOMEM;
@@ -807,8 +920,7 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
     capq[l] = rate_to_q(s->cap[l]);
     if (capq[l] < F + 1) { rc = ORC_ERANGE; goto out; } /* every fair share stays >= 1 quantum */
   }
-  for (int64_t f = 0; f < F; f++) { s->t_done[f] = NAN; s->bneck[f] = -1; }
-  memset(s->work, 0, sizeof(s->work));
+  if (K == 0) memset(s->work, 0, sizeof(s->work));
   /* successor lists = transpose of the pred lists */
   for (int64_t e = 0; e < s->pred_off[F]; e++) succ_off[s->pred[e] + 1]++;
   for (int64_t f = 0; f < F; f++) succ_off[f + 1] += succ_off[f];
@@ -822,13 +934,56 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
   }
   int32_t nA = 0, nP = 0, stopped = 0;
   int64_t n_done = 0;
-  double now = 0.0;
-  for (int64_t f = 0; f < F; f++) {
-    pred_cnt[f] = (int32_t)(s->pred_off[f + 1] - s->pred_off[f]);
-    if (pred_cnt[f] == 0) { /* no preds: t_act = start + Lat -> PENDING */
-      t_act[f] = s->start[f] + s->Lat[f];
-      state[f] = PENDING;
-      pend[nP++] = (int32_t)f;
+  double now = K > 0 ? s->ev[K - 1].t : 0.0;
+  /* ---- the state after event K-1 (K = 0: the initial state).  History records of iteration K and later are
+   * dropped: the loop below writes them again.  A flow is DONE if it completed in an event < K; ACTIVE if it has a
+   * record left -- the last one holds (time, rate, remaining bytes) of its current constant-throughput interval, and
+   * its completion time is time + remaining / rate exactly as when the record was written; otherwise it waits for
+   * its predecessors, or (all of them done) is PENDING with t_act = max(start, latest predecessor) + Lat. */
+  {
+    int64_t keep = 0;
+    for (int64_t i = 0; i < s->n_h; i++)
+      if (s->h_ev[i] < K) {
+        s->h_flow[keep] = s->h_flow[i]; s->h_t[keep] = s->h_t[i]; s->h_rate[keep] = s->h_rate[i];
+        s->h_rem[keep] = s->h_rem[i]; s->h_ev[keep] = s->h_ev[i]; s->h_rq[keep] = s->h_rq[i];
+        keep++;
+      }
+    s->n_h = keep;
+    for (int64_t f = 0; f < F; f++) {
+      rq_cur[f] = -1;
+      if (s->done_ev[f] >= K) { s->done_ev[f] = -1; s->t_done[f] = NAN; }
+      if (s->done_ev[f] >= 0) { state[f] = DONE; n_done++; } else s->bneck[f] = -1;
+    }
+    for (int64_t i = 0; i < s->n_h; i++) { /* records are chronological: the last one of a flow wins */
+      int32_t f = s->h_flow[i];
+      if (state[f] == DONE) continue;
+      t_last[f] = s->h_t[i];
+      rate_cur[f] = s->h_rate[i];
+      rq_cur[f] = s->h_rq[i];
+      rem[f] = s->h_rem[i];
+    }
+    for (int64_t f = 0; f < F; f++) {
+      if (state[f] == DONE) continue;
+      if (rq_cur[f] >= 0) {
+        state[f] = ACTIVE;
+        double q = rem[f] / rate_cur[f];
+        tc[f] = t_last[f] + q;
+        act[nA++] = (int32_t)f;
+        continue;
+      }
+      double latest = 0.0;
+      pred_cnt[f] = 0;
+      for (int64_t e = s->pred_off[f]; e < s->pred_off[f + 1]; e++) {
+        int32_t p = s->pred[e];
+        if (s->done_ev[p] >= 0) { if (s->t_done[p] > latest) latest = s->t_done[p]; }
+        else pred_cnt[f]++;
+      }
+      if (pred_cnt[f] == 0) { /* released (or no preds): t_act = max(start, latest predecessor) + Lat -> PENDING */
+        double st = s->start[f] > latest ? s->start[f] : latest;
+        t_act[f] = st + s->Lat[f];
+        state[f] = PENDING;
+        pend[nP++] = (int32_t)f;
+      }
     }
   }
   for (;;) {
@@ -881,9 +1036,17 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
           d = realloc(s->h_rate, sizeof(double) * c);
           if (!d) { rc = ORC_ENOMEM; goto out; }
           s->h_rate = (double *)d;
+          a = realloc(s->h_rem, sizeof(double) * c);
+          if (!a) { rc = ORC_ENOMEM; goto out; }
+          s->h_rem = (double *)a;
+          b = realloc(s->h_ev, sizeof(int64_t) * c);
+          if (!b) { rc = ORC_ENOMEM; goto out; }
+          s->h_ev = (int64_t *)b;
+          d = realloc(s->h_rq, sizeof(int64_t) * c);
+          if (!d) { rc = ORC_ENOMEM; goto out; }
+          s->h_rq = (int64_t *)d;
           s->h_cap = c;
         }
-        s->h_flow[s->n_h] = f; s->h_t[s->n_h] = now; s->h_rate[s->n_h] = new_rate; s->n_h++;
       }
       if (changed || ((flags & ORC_FLAG_SETTLE_EVERY_EVENT) && rq_cur[f] >= 0)) {
         if (rq_cur[f] >= 0) rem[f] = settle(rem[f], rate_cur[f], now - t_last[f]);
@@ -892,6 +1055,10 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
         rate_cur[f] = new_rate;
         double q = rem[f] / new_rate;
         tc[f] = now + q;
+      }
+      if (changed) { /* the record: (time, new rate, remaining bytes), written in iteration n_ev */
+        s->h_flow[s->n_h] = f; s->h_t[s->n_h] = now; s->h_rate[s->n_h] = new_rate; s->h_rem[s->n_h] = rem[f];
+        s->h_ev[s->n_h] = s->n_ev; s->h_rq[s->n_h] = rq_cur[f]; s->n_h++;
       }
       if (tc[f] < t_next) t_next = tc[f];
       ah += (double)(s->path_off[f + 1] - s->path_off[f]);
@@ -915,6 +1082,7 @@ int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32
       }
       if (tc[f] == t_next) { /* bit-equal absolute time: completes */
         s->t_done[f] = t_next;
+        s->done_ev[f] = s->n_ev;
         state[f] = DONE;
         comp[nC++] = f;
       } else {

@@ -107,6 +107,15 @@ int32_t orc_run(orc_sim *s, int32_t mode, int32_t trace);
 /* same, but stops before the first event later than t_stop ("advancing the simulation ... up to a
  * specified time"); unfinished flows keep t_done = NaN and bneck = -1 */
 int32_t orc_run_until(orc_sim *s, int32_t mode, int32_t trace, double t_stop);
+/* NEXT-1, time rollback (sec 4.2, L167 sec 5).  orc_run / orc_run_until may be called again: a
+ * call CONTINUES from the events simulated so far (a larger stop time advances "up to a specified time", L167), after
+ * rebuilding the simulator state from the per-flow throughput history (L128).  Submissions after a run
+ * (orc_add_flows / orc_add_collective* / orc_add_spans) and orc_update_flow_start roll back to the (earlier) start
+ * time involved; orc_rollback does it explicitly; orc_gc drops history that no later rollback to a time >= T needs
+ * (L130) -- a rollback below the watermark then fails with ORC_EINVAL. */
+int32_t orc_rollback(orc_sim *s, double T);
+int32_t orc_update_flow_start(orc_sim *s, int64_t flow, double start_time_s);
+int32_t orc_gc(orc_sim *s, double T);
 /* the same with `flags` (see above); flags = 0 is orc_run_until */
 int32_t orc_run_ex(orc_sim *s, int32_t mode, int32_t trace, double t_stop, int32_t flags);
 /* S4.4 / Q11 settle step on its own: max(rem - rate * dt, 0) with mul, sub, clamp in that order */

@@ -38,6 +38,11 @@ MUTANTS = [
      "", "next3_pipelined"),
     ("M14_tree_root_waits_for_one_child", "if (N > 2 && push_pred(s, first + ch * per + 1)) return ORC_ENOMEM;", "",
      "next3_tree"),
+    ("M16_rollback_completion_time_from_now", "tc[f] = t_last[f] + q;", "tc[f] = now + q;", "next1"),
+    ("M17_rollback_ignores_latest_predecessor", "if (s->done_ev[p] >= 0) { if (s->t_done[p] > latest) latest = s->t_done[p]; }",
+     "if (s->done_ev[p] >= 0) { }", "next1"),
+    ("M18_rollback_keeps_the_event_at_T", "while (k < s->n_ev && s->ev[k].t < T) k++;",
+     "while (k < s->n_ev && s->ev[k].t <= T) k++;", "next1"),
     ("M15_chain_after_ignores_last_chunk", "for (int32_t f = A->first_flow + (A->chunks - 1) * per_chunk;",
      "for (int32_t f = A->first_flow;", "next3_after"),
 ]

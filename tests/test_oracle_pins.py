@@ -655,6 +655,132 @@ def test_next2_compute_spans_closed_forms():
         orc.Sim(single(), 0).add_spans([0], [1e-3])                                            # no compute lanes
 
 
+# ------------------------------------------------------------------------------------------------ NEXT-1 time rollback
+def _same_results(a, b):
+    assert np.array_equal(a.completion_times(), b.completion_times())
+    assert np.array_equal(a.bottlenecks(), b.bottlenecks())
+    assert np.array_equal(a.event_log(), b.event_log())
+    for x, y in zip(a.history(), b.history()):
+        assert np.array_equal(x, y)
+
+
+def _rollback_workloads():
+    yield W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2), 1
+    yield W.train_step(batch=1, n_hosts=4, gph=4, layers=2, buckets=2), 0
+    yield W.cfg4(batch=1, n_hosts=4, gph=4, n_leaves=2, n_spines=2), 0
+
+
+def test_next1_advancing_in_steps_equals_one_run():
+    """PAPER.md L167 "advancing the simulation ... up to a specified time", repeatedly: every call rebuilds the state
+    from the throughput history (L128) and continues; the end result is the one-shot run, bit for bit."""
+    from util import oracle_build
+    for w, i in _rollback_workloads():
+        ref = oracle_run(w.desc, w.instances[i])
+        t_end = ref.completion_times().max()
+        o = oracle_build(w.desc, w.instances[i])
+        for frac in (0.0, 0.13, 0.13, 0.5, 0.77):
+            o.run(until=frac * t_end)
+            done = ref.completion_times() <= frac * t_end
+            assert np.array_equal(o.completion_times()[done], ref.completion_times()[done])
+            assert np.isnan(o.completion_times()[~done]).all()
+        o.run()
+        _same_results(o, ref)
+
+
+def test_next1_rollback_and_rerun_equals_a_fresh_run():
+    """The property that fixes the rollback (Fig. 4): after the simulator has run ahead to T1,
+    changing a flow's start time (L167) or submitting flows with an earlier timestamp T2 rolls back to T2, and the
+    re-simulation equals -- completion times, bottlenecks, event log, throughput history, all bit for bit -- a fresh
+    run that had the change from t = 0.  T2 before, inside and after the lives of the affected flows."""
+    from util import oracle_build
+    rng = np.random.default_rng(9)
+    for w, i in _rollback_workloads():
+        inst = w.instances[i]
+        base = oracle_run(w.desc, inst)
+        t0 = base.completion_times()
+        t_end = t0.max()
+        F = base.num_flows
+        mattered = 0
+        for case in range(6):
+            flows = rng.choice(F, 3, replace=False)
+            T1 = [0.3, 0.6, 1.0, 0.9, 0.5, 2.0][case] * t_end          # how far the simulator ran ahead
+            new_start = [0.1, 0.55, 0.2, 1.3, 0.0, 0.7][case] * t_end * np.array([1.0, 0.5, 1.1])
+            late = W.RawFlows(np.array([0, 1], np.int32), np.array([5, 6], np.int32), np.array([3e6, 5e5]),
+                              start=np.array([0.4, 0.05]) * t_end, dep_off=np.array([0, 1, 1], np.int64),
+                              dep_ids=np.array([int(flows[0])], np.int64))
+            fresh = oracle_build(w.desc, inst)                          # the change known from t = 0
+            for f, st in zip(flows, new_start):
+                fresh.update_flow_start(int(f), float(st))
+            fresh.add_flows(late.src, late.dst, late.nbytes, late.start, late.dep_off, late.dep_ids)
+            fresh.run()
+            live = oracle_build(w.desc, inst)                           # the change arrives at T1
+            live.run(until=T1)
+            n_before = len(live.event_log())
+            for f, st in zip(flows, new_start):
+                live.update_flow_start(int(f), float(st))
+            live.add_flows(late.src, late.dst, late.nbytes, late.start, late.dep_off, late.dep_ids)
+            assert len(live.event_log()) <= n_before                   # rolled back (or nothing to roll back)
+            live.run()
+            _same_results(live, fresh)
+            mattered += not np.array_equal(fresh.completion_times()[:F], t0)
+        assert mattered >= 3                                             # the changes do move the old flows
+    # an explicit rollback forgets the future and nothing else
+    w, i = next(_rollback_workloads())
+    ref = oracle_run(w.desc, w.instances[i])
+    o = oracle_run(w.desc, w.instances[i])
+    T = 0.4 * ref.completion_times().max()
+    o.rollback(T)
+    assert np.isnan(o.completion_times()[ref.completion_times() >= T]).all()
+    assert np.array_equal(o.event_log(), ref.event_log()[ref.event_log()["t"] < T])
+    o.run()
+    _same_results(o, ref)
+    T = float(ref.event_log()["t"][len(ref.event_log()) // 2])            # exactly an event time: that event goes too
+    o.rollback(T)
+    assert np.array_equal(o.event_log(), ref.event_log()[ref.event_log()["t"] < T])
+    assert np.isnan(o.completion_times()[ref.completion_times() >= T]).all()
+    o.run()
+    _same_results(o, ref)
+
+
+def test_next1_gc_keeps_every_later_rollback_exact():
+    """history older than the watermark is dropped; results after GC(T) equal results without GC for
+    every later rollback target >= T, and a rollback below T is refused."""
+    from util import oracle_build
+    w, i = next(_rollback_workloads())
+    inst = w.instances[i]
+    ref = oracle_run(w.desc, inst)
+    t_end = ref.completion_times().max()
+    n_hist = len(ref.history()[0])
+    off, pr = ref.preds()
+    t_ref = ref.completion_times()
+    rel = np.array([t_ref[pr[off[f]:off[f + 1]]].max() if off[f + 1] > off[f] else 0.0 for f in range(ref.num_flows)])
+    flow = int(np.flatnonzero((rel > 0.62 * t_end) & (rel < 0.75 * t_end))[0])     # released between the watermarks and T1
+    for Tw, T2 in ((0.3, 0.7), (0.5, 0.9), (0.6, 0.78)):
+        o = oracle_build(w.desc, inst)
+        o.run(until=0.8 * t_end)
+        o.gc(Tw * t_end)
+        assert len(o.history()[0]) < n_hist
+        with pytest.raises(orc.OrcError):
+            o.rollback(0.5 * Tw * t_end)
+        with pytest.raises(orc.OrcError):
+            o.update_flow_start(0, 0.1 * t_end)          # a flow that started at t = 0: below the watermark
+        o.update_flow_start(flow, T2 * t_end)
+        assert len(o.event_log()) < len(ref.event_log()[ref.event_log()["t"] <= 0.8 * t_end])     # it did roll back
+        o.run()
+        fresh = oracle_build(w.desc, inst)
+        fresh.update_flow_start(flow, T2 * t_end)
+        fresh.run()
+        assert not np.array_equal(fresh.completion_times(), t_ref)
+        assert np.array_equal(o.completion_times(), fresh.completion_times())
+        assert np.array_equal(o.bottlenecks(), fresh.bottlenecks())
+        assert np.array_equal(o.event_log(), fresh.event_log())
+        fo, to, ro = o.history()
+        ff, tf, rf = fresh.history()
+        keep = tf >= Tw * t_end                                           # what GC may not touch
+        late = to >= Tw * t_end
+        assert np.array_equal(fo[late], ff[keep]) and np.array_equal(to[late], tf[keep]) and np.array_equal(ro[late], rf[keep])
+
+
 # ------------------------------------------------------------------------------------------------ S2 routing pins
 def test_routing_leaf_spine_down_lane_comes_from_the_high_hash_word():
     """S2: with P parallel uplinks per (leaf, spine) the up lane is (H mod (n_spines P)) mod P and the down lane
@@ -887,5 +1013,6 @@ def test_input_validation():
     s.run()
     t = s.completion_times()
     assert t[1] == pytest.approx(2 * (2e-6 + 1e6 / 450e9), rel=1e-12)
-    with pytest.raises(orc.OrcError):
-        s.add_flows([0], [1], [1.0])                 # after run -> ESTATE
+    s.add_flows([0], [1], [1.0])                     # after a run: a late submission (NEXT-1), not an error
+    s.run()
+    assert s.num_flows == 3 and not np.isnan(s.completion_times()).any()
