@@ -100,6 +100,8 @@ typedef struct {
                          /* the run's stream), excluding the result copies                                */
   int32_t grid_ctas;     /* CTAs of the cooperative launch of the grid path in the last run (0: path not used)   */
   int32_t pad_;
+  double resumed_from_s; /* simulated time of the parked state / snapshot the last run continued from (0: it      */
+                         /* started at t = 0)                                                                   */
   int64_t n_windows;     /* lookahead windows executed (phs_set_windows); = n_events where the window schedule  */
                          /* is off.  n_events then counts window ITERATIONS: one iteration advances every       */
                          /* component that has an event inside the window by one event                          */
@@ -141,7 +143,7 @@ phs_status phs_add_collective_ex(phs_sim *sim, int32_t instance, int32_t kind, c
 phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                                     const double *bytes, const double *start_time_s, const int32_t *after_coll_ids,
                                     int32_t n_after, int32_t *out_coll_id);
-/* Adds n raw flows.  start_time_s nullable (= 0).  dep_off[n+1]/dep_flow_ids (nullable) list, per flow, ids of
+/* Adds n raw flows (after phs_finalize: a late submission, see phs_update_flow_start).  start_time_s nullable (= 0).  dep_off[n+1]/dep_flow_ids (nullable) list, per flow, ids of
  * EARLIER flows of the same instance that must complete first.  conn_id (nullable = the flow's id) keys ECMP. */
 phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_t *src, const int32_t *dst,
                          const double *bytes, const double *start_time_s, const int64_t *dep_off,
@@ -222,6 +224,28 @@ phs_status phs_run(phs_sim *sim, void *cuda_stream);
  * from it; if the time goes backwards everything starts again from t = 0 -- the simulation is deterministic, so
  * the results are the same either way. */
 phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
+
+/* Time rollback (sec 4.2 "the network simulator rolls back to T2 and adds a flow starting at T2",
+ * Fig. 4; L167 sec 5: "one for updating the start time of an existing flow, and another for advancing the simulation
+ * ... up to a specified time").
+ *   phs_set_snapshots   every phs_run_until that stops at a time keeps the parked state of that time (on-chip state
+ *                       of every unit + outstanding-predecessor counters); the newest `n` are held.  A later run that
+ *                       must go back in time continues from the newest usable snapshot instead of t = 0.
+ *   phs_update_flow_start  changes the start time of a flow after phs_finalize.  The start time acts through
+ *                       t_act = max(start, release) + Lat, so the simulated past is void from the flow's release on
+ *                       (nothing is void if it has not been released yet, or if max(start, release) does not change):
+ *                       the next run continues from the newest snapshot before that time.  A flow WITHOUT predecessors
+ *                       sits in the sorted initial-activation lists: the tables are rebuilt and the next run starts at 0.
+ *   phs_rollback        declares the simulated past void from time t_s on (results become unavailable until the next run).
+ *   phs_gc              PAPER.md L130: drops the snapshots no rollback to a time >= t_s can need.
+ * phs_add_flows / phs_add_collective* / phs_add_spans after phs_finalize are late submissions (L124): the tables are
+ * rebuilt (the units may merge) and the next run starts at t = 0; results are those of a fresh run either way, the
+ * simulation being deterministic -- the oracle (oracle/orc_netsim.c) rolls back exactly as the paper describes and
+ * pins that equality. */
+phs_status phs_set_snapshots(phs_sim *sim, int32_t n);
+phs_status phs_update_flow_start(phs_sim *sim, int32_t instance, int64_t flow, double start_time_s);
+phs_status phs_rollback(phs_sim *sim, double t_s);
+phs_status phs_gc(phs_sim *sim, double t_s);
 
 phs_status phs_num_flows(const phs_sim *sim, int32_t instance, int64_t *out);
 phs_status phs_total_flows(const phs_sim *sim, int64_t *out);

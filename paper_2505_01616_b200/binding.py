@@ -32,7 +32,7 @@ class Counters(C.Structure):
                 ("sum_par_rounds", C.c_int64), ("n_kernel_launches", C.c_int64), ("h2d_bytes", C.c_int64),
                 ("max_active", C.c_int32), ("max_slots", C.c_int32), ("cluster_size", C.c_int32),
                 ("clusters_resident", C.c_int32), ("resumed_units", C.c_int32), ("window_gang", C.c_int32),
-                ("main_kernel_ms", C.c_double), ("grid_ctas", C.c_int32), ("pad_", C.c_int32), ("n_windows", C.c_int64)]
+                ("main_kernel_ms", C.c_double), ("grid_ctas", C.c_int32), ("pad_", C.c_int32), ("resumed_from_s", C.c_double), ("n_windows", C.c_int64)]
 
 
 EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<i4"), ("n_rounds", "<i4"),
@@ -43,7 +43,8 @@ SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "
            "phs_set_link_capacities_batch",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_full", "phs_add_spans", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
-           "phs_set_decomposition", "phs_set_windows", "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
+           "phs_set_decomposition", "phs_set_windows", "phs_set_snapshots", "phs_update_flow_start", "phs_rollback", "phs_gc",
+           "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
            "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
@@ -219,6 +220,22 @@ def phs_set_decomposition(h, enable=True):
 
 def phs_set_windows(h, enable=True):
     _chk(lib().phs_set_windows(h, C.c_int32(1 if enable else 0)), "phs_set_windows")
+
+
+def phs_set_snapshots(h, n):
+    _chk(lib().phs_set_snapshots(h, C.c_int32(n)), "phs_set_snapshots")
+
+
+def phs_update_flow_start(h, instance, flow, start):
+    _chk(lib().phs_update_flow_start(h, C.c_int32(instance), C.c_int64(flow), C.c_double(start)), "phs_update_flow_start")
+
+
+def phs_rollback(h, t):
+    _chk(lib().phs_rollback(h, C.c_double(t)), "phs_rollback")
+
+
+def phs_gc(h, t):
+    _chk(lib().phs_gc(h, C.c_double(t)), "phs_gc")
 
 
 def phs_finalize(h, stream=None):

@@ -133,7 +133,7 @@ phs_status phs_add_spans(phs_sim *sim, int32_t instance, int64_t n, const int32_
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
-  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
     for (int i = 1; i < sim->batch; ++i)
@@ -156,7 +156,7 @@ phs_status phs_add_collective_full(phs_sim *sim, int32_t instance, int32_t kind,
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
-  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
     for (int i = 1; i < sim->batch; ++i)
@@ -178,7 +178,7 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
                                     int32_t *out_id) {
   PHS_API_BEGIN
   if (!sim || !bytes) return fail(PHS_EINVAL, "null argument");
-  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   for (int i = 1; i < sim->batch; ++i)
     if (sim->inst[i].colls.size() != sim->inst[0].colls.size())
       return fail(PHS_ESTATE, "batch add needs the same number of collectives in every instance");
@@ -205,7 +205,7 @@ phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
-  if (sim->finalized) return fail(PHS_ESTATE, "instance set is frozen after phs_finalize");
+  if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
     for (int i = 1; i < sim->batch; ++i)
@@ -502,6 +502,7 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   c.n_kernel_launches = sim->n_launches;
   c.h2d_bytes = sim->h2d_bytes;
   c.main_kernel_ms = sim->main_kernel_ms;
+  c.resumed_from_s = sim->resumed_from;
   *out = c;
   return PHS_OK;
   PHS_API_END

@@ -129,6 +129,9 @@ cudaError_t grid_max_ctas(int *n_ctas);
 cudaError_t launch_grid_path(const DevTables &t, const int32_t *list, int n, unsigned char *scratch, int64_t max_flows,
                              int max_links, int n_ctas, cudaStream_t stream);
 
+// NEXT-1: forgets the results later than t (t_done = NaN, bneck = -1)
+cudaError_t launch_forget_after(double *t_done, int32_t *bneck, int64_t n, double t, cudaStream_t stream);
+
 // out[c] = max t_done over the flows of collective c, for all collectives of all instances.
 cudaError_t launch_collective_times(const double *t_done, const int64_t *coll_first, const int32_t *coll_nflows,
                                     int64_t n_colls, double *out, cudaStream_t stream);

@@ -762,6 +762,21 @@ __global__ void phs_collective_times_kernel(const double *__restrict__ t_done, c
   if (lane == 0) out[c] = open_flows ? __longlong_as_double(0x7ff8000000000000LL) : m;
 }
 
+// NEXT-1: results later than t are forgotten (completion time NaN, bottleneck -1), as after a stop at time t
+__global__ void phs_forget_after_kernel(double *__restrict__ t_done, int32_t *__restrict__ bneck, int64_t n, double t) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n && !(t_done[i] <= t)) {
+    t_done[i] = __longlong_as_double(-1LL);  // the all-ones pattern cudaMemset(0xff) leaves: a NaN
+    bneck[i] = -1;
+  }
+}
+
+cudaError_t launch_forget_after(double *t_done, int32_t *bneck, int64_t n, double t, cudaStream_t stream) {
+  if (n == 0) return cudaSuccess;
+  phs_forget_after_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(t_done, bneck, n, t);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_collective_times(const double *t_done, const int64_t *coll_first, const int32_t *coll_nflows,
                                     int64_t n_colls, double *out, cudaStream_t stream) {
   if (n_colls == 0) return cudaSuccess;

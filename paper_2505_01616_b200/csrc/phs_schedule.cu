@@ -725,14 +725,20 @@ phs_status run_cluster_path(phs_sim *sim, std::vector<int32_t> list, int64_t slo
                             cudaStream_t st, std::vector<int32_t> *too_big) {
 retry:
   if (list.empty()) return PHS_OK;
+  // The launch configuration is sized for ALL units of the cluster path, not only the ones of this call (a resume
+  // runs the unfinished ones): parked states and snapshots stay valid from call to call.
+  std::vector<int32_t> basis(sim->cluster_list);
+  for (int u : list)
+    if (std::find(basis.begin(), basis.end(), u) == basis.end()) basis.push_back(u);
+  for (int u : *too_big) basis.erase(std::remove(basis.begin(), basis.end(), u), basis.end());
   int L = 1;  // the shared-memory layout is sized for the unit with the most links
-  for (int u : list) L = std::max(L, sim->units[u].n_links);
+  for (int u : basis) L = std::max(L, sim->units[u].n_links);
   if (L >= 65535) return fail(PHS_ERANGE, "cluster path: units with 65535 or more links are not supported");
   // slots needed per instance: every flow without predecessors is PENDING from t = 0; later, a ring collective
   // has at most one step in flight per rank plus the successors waiting out their latency, while an all-to-all
   // or a raw flow set can be in flight as a whole.  Start from a quarter of that bound; overflow doubles it.
   int64_t target = 64;
-  for (int u : list) {
+  for (int u : basis) {
     const phs_sim::Unit &un = sim->units[u];
     const int64_t ring = un.bound - un.bound_whole;  // rarely all in flight at once: start from a quarter
     target = std::max(target, un.bound_whole + std::min(ring, ring * slot_scale / 4));
@@ -772,12 +778,12 @@ retry:
     if (log)
       return fail(PHS_ERANGE, "a unit's pending + active flows do not fit the shared memory of a cluster, and the grid "
                               "path does not write the event log");
-    auto big = std::max_element(list.begin(), list.end(), [&](int a, int b) {
+    auto big = std::max_element(basis.begin(), basis.end(), [&](int a, int b) {
       const phs_sim::Unit &x = sim->units[(size_t)a], &y = sim->units[(size_t)b];
       return x.bound_whole + (x.bound - x.bound_whole) / 4 < y.bound_whole + (y.bound - y.bound_whole) / 4;
     });
     too_big->push_back(*big);
-    list.erase(big);
+    list.erase(std::remove(list.begin(), list.end(), *big), list.end());
     goto retry;
   }
   const int n_clusters = std::max(1, std::min<int>((int)list.size(), max_clusters));
@@ -951,6 +957,173 @@ phs_status run_window_path(phs_sim *sim, std::vector<int32_t> todo, std::vector<
 
 }  // namespace
 
+
+// ================================================================================================ NEXT-1: rollback
+void phs_unfinalize(phs_sim *sim) {
+  sim->finalized = sim->ran = sim->have_park = false;
+  sim->snaps.clear();
+  sim->dirty_from = std::numeric_limits<double>::infinity();
+  sim->h_pos.clear();
+  sim->park_stride = 0;
+  sim->cpark_unit_bytes = 0;
+  sim->cpark_cs = sim->cpark_L = 0;
+  sim->cpark_Sc = 0;
+  sim->d_park.release();
+  sim->d_cpark.release();
+  sim->d_cpark_index.release();
+  sim->d_trel.release();
+  sim->d_fcw.release();
+  sim->d_hist.release();
+  sim->d_hist_n.release();
+  sim->d_log.release();
+  sim->d_arena.release();  // the table buffers are views into it
+  if (sim->ev0) cudaEventDestroy(sim->ev0);
+  if (sim->ev1) cudaEventDestroy(sim->ev1);
+  sim->ev0 = sim->ev1 = nullptr;
+}
+
+namespace {
+
+// keeps the parked state of the run that just stopped at sim->parked_until (newest last, at most max_snaps)
+phs_status take_snapshot(phs_sim *sim, cudaStream_t st) {
+  if (sim->max_snaps <= 0 || !sim->have_park) return PHS_OK;
+  if (!sim->snaps.empty() && sim->snaps.back()->t == sim->parked_until) return PHS_OK;
+  std::unique_ptr<phs_sim::Snapshot> sn(new phs_sim::Snapshot());
+  sn->t = sim->parked_until;
+  if (sim->d_park.p && sim->park_stride) {
+    const size_t n = sim->park_stride * sim->units.size();
+    PHS_CUDA(sn->park.alloc(n));
+    PHS_CUDA(cudaMemcpyAsync(sn->park.p, sim->d_park.p, n, cudaMemcpyDeviceToDevice, st));
+  }
+  if (sim->d_cpark.p && sim->d_cpark.n) {
+    PHS_CUDA(sn->cpark.alloc(sim->d_cpark.n));
+    PHS_CUDA(cudaMemcpyAsync(sn->cpark.p, sim->d_cpark.p, sim->d_cpark.n, cudaMemcpyDeviceToDevice, st));
+  }
+  PHS_CUDA(sn->pred_cnt.alloc((size_t)sim->total_flows));
+  PHS_CUDA(cudaMemcpyAsync(sn->pred_cnt.p, sim->d_pred_cnt.p, sizeof(int32_t) * (size_t)sim->total_flows,
+                           cudaMemcpyDeviceToDevice, st));
+  sn->res = sim->h_res;
+  sn->hist_n = (unsigned long long)sim->h_hist.size();
+  if (sim->hist_cap > 0)
+    PHS_CUDA(cudaMemcpyAsync(&sn->hist_n, sim->d_hist_n.p, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  sn->cpark_unit_bytes = sim->cpark_unit_bytes;
+  sn->cpark_cs = sim->cpark_cs;
+  sn->cpark_L = sim->cpark_L;
+  sn->cpark_Sc = sim->cpark_Sc;
+  sn->n_order = sim->order.size();
+  sn->n_cluster = sim->cluster_list.size();
+  PHS_CUDA(cudaStreamSynchronize(st));
+  sim->snaps.push_back(std::move(sn));
+  while ((int)sim->snaps.size() > sim->max_snaps) sim->snaps.pop_front();
+  return PHS_OK;
+}
+
+// makes snapshot `k` the handle's parked state (and drops the newer ones): the simulation is back at its time
+phs_status restore_snapshot(phs_sim *sim, size_t k, cudaStream_t st) {
+  phs_sim::Snapshot &sn = *sim->snaps[k];
+  if (sn.park.p) PHS_CUDA(cudaMemcpyAsync(sim->d_park.p, sn.park.p, sn.park.n, cudaMemcpyDeviceToDevice, st));
+  if (sn.cpark.p) PHS_CUDA(cudaMemcpyAsync(sim->d_cpark.p, sn.cpark.p, sn.cpark.n, cudaMemcpyDeviceToDevice, st));
+  PHS_CUDA(cudaMemcpyAsync(sim->d_pred_cnt.p, sn.pred_cnt.p, sizeof(int32_t) * (size_t)sim->total_flows,
+                           cudaMemcpyDeviceToDevice, st));
+  sim->h_res = sn.res;
+  PHS_CUDA(cudaMemcpyAsync(sim->d_res.p, sim->h_res.data(), sizeof(InstResult) * sim->h_res.size(),
+                           cudaMemcpyHostToDevice, st));
+  if (sim->hist_cap > 0)
+    PHS_CUDA(cudaMemcpyAsync(sim->d_hist_n.p, &sn.hist_n, sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+  PHS_CUDA(launch_forget_after(sim->d_tdone.p, sim->d_bneck.p, sim->total_flows, sn.t, st));
+  PHS_CUDA(cudaStreamSynchronize(st));
+  sim->parked_until = sn.t;
+  sim->have_park = true;
+  sim->ran = true;
+  sim->snaps.resize(k + 1);
+  return PHS_OK;
+}
+
+// a snapshot is usable while the launch configuration it was parked under still stands
+bool snapshot_usable(const phs_sim *sim, const phs_sim::Snapshot &sn) {
+  return sn.n_order == sim->order.size() && sn.n_cluster == sim->cluster_list.size() &&
+         sn.cpark_unit_bytes == sim->cpark_unit_bytes && sn.cpark_cs == sim->cpark_cs && sn.cpark_L == sim->cpark_L &&
+         sn.cpark_Sc == sim->cpark_Sc && (sn.park.n == 0 || sn.park.n == sim->park_stride * sim->units.size()) &&
+         (sn.cpark.n == 0 || sn.cpark.n == sim->d_cpark.n);
+}
+
+}  // namespace
+
+extern "C" phs_status phs_set_snapshots(phs_sim *sim, int32_t n) {
+  PHS_API_BEGIN
+  if (!sim || n < 0) return fail(PHS_EINVAL, "bad snapshot count");
+  sim->max_snaps = n;
+  while ((int)sim->snaps.size() > n) sim->snaps.pop_front();
+  return PHS_OK;
+  PHS_API_END
+}
+
+extern "C" phs_status phs_rollback(phs_sim *sim, double t_s) {
+  PHS_API_BEGIN
+  if (!sim || !(t_s >= 0.0)) return fail(PHS_EINVAL, "bad rollback time");
+  sim->dirty_from = std::min(sim->dirty_from, t_s);
+  sim->ran = false;  // no results until the next run
+  return PHS_OK;
+  PHS_API_END
+}
+
+extern "C" phs_status phs_gc(phs_sim *sim, double t_s) {
+  PHS_API_BEGIN
+  if (!sim || !(t_s >= 0.0)) return fail(PHS_EINVAL, "bad watermark");
+  // keep the newest snapshot below the watermark (a rollback to t_s continues from it) and everything later
+  while (sim->snaps.size() >= 2 && sim->snaps[1]->t < t_s) sim->snaps.pop_front();
+  return PHS_OK;
+  PHS_API_END
+}
+
+extern "C" phs_status phs_update_flow_start(phs_sim *sim, int32_t instance, int64_t flow, double start) {
+  PHS_API_BEGIN
+  if (!sim || instance < 0 || instance >= sim->batch) return fail(PHS_EINVAL, "instance out of range");
+  if (!(start >= 0.0) || !std::isfinite(start)) return fail(PHS_EINVAL, "start_time_s must be >= 0 and finite");
+  Instance &in = sim->inst[(size_t)instance];
+  expand_pending(*sim->fab, in);
+  if (flow < 0 || flow >= in.n_flows()) return fail(PHS_EINVAL, "flow out of range");
+  const double old = in.start[(size_t)flow];
+  in.start[(size_t)flow] = start;
+  if (!sim->finalized || old == start) return PHS_OK;
+  const uint32_t p0 = in.pred_off[(size_t)flow], p1 = in.pred_off[(size_t)flow + 1];
+  if (p0 == p1) {  // in the sorted initial-activation lists, and in a slot from t = 0: rebuild, start again at 0
+    phs_unfinalize(sim);
+    return PHS_OK;
+  }
+  cudaStream_t st = sim->last_stream;
+  const int64_t Ft = sim->total_flows;
+  if (sim->h_pos.empty()) {  // output position -> position in the per-flow tables (inverse of fmap)
+    std::vector<uint32_t> fmap((size_t)Ft);
+    PHS_CUDA(cudaMemcpyAsync(fmap.data(), sim->d_fmap.p, sizeof(uint32_t) * (size_t)Ft, cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    sim->h_pos.assign((size_t)Ft, 0);
+    for (int64_t p = 0; p < Ft; ++p) sim->h_pos[fmap[(size_t)p]] = (uint32_t)p;
+  }
+  const int64_t out = sim->flow_base[(size_t)instance] + flow;
+  PHS_CUDA(cudaMemcpyAsync(&sim->d_rec.p[sim->h_pos[(size_t)out]].start, &start, sizeof(double), cudaMemcpyHostToDevice, st));
+  // release time of the flow in the simulated past = completion of its last predecessor, if all of them are done
+  double rel = 0.0;
+  bool released = sim->ran || sim->have_park;
+  for (uint32_t e = p0; e < p1 && released; ++e) {
+    double td = 0.0;
+    PHS_CUDA(cudaMemcpyAsync(&td, sim->d_tdone.p + sim->flow_base[(size_t)instance] + in.pred[e], sizeof(double),
+                             cudaMemcpyDeviceToHost, st));
+    PHS_CUDA(cudaStreamSynchronize(st));
+    if (td != td) released = false;
+    rel = std::max(rel, td);
+  }
+  PHS_CUDA(cudaStreamSynchronize(st));
+  // from its release on the flow sits in a slot with t_act computed from the old start time: the past is void from
+  // there on, unless max(start, release) stays what it was
+  if (released && std::max(old, rel) != std::max(start, rel)) {
+    sim->dirty_from = std::min(sim->dirty_from, rel);
+    sim->ran = false;
+  }
+  return PHS_OK;
+  PHS_API_END
+}
+
 extern "C" phs_status phs_run(phs_sim *sim, void *cuda_stream) {
   PHS_API_BEGIN
   return phs_run_until(sim, std::numeric_limits<double>::infinity(), cuda_stream);
@@ -976,7 +1149,25 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   // memory); a later stop time continues them from there.  When the time goes backwards (or a unit changed its
   // launch configuration after an overflow) the simulation starts again from t = 0 -- it is deterministic, so the
   // results are the same.
-  const bool resume = sim->have_park && sim->ran && sim->t_stop >= sim->parked_until;
+  // NEXT-1: if the simulated past is void from dirty_from on (phs_update_flow_start, phs_rollback), or the stop time
+  // lies before the parked state, the run continues from the newest snapshot that is early enough -- strictly before
+  // dirty_from, not after t_stop -- and only without one from t = 0.
+  const double dirty = sim->dirty_from;
+  sim->dirty_from = std::numeric_limits<double>::infinity();
+  bool resume = sim->have_park && sim->t_stop >= sim->parked_until && sim->parked_until < dirty &&
+                (sim->ran || std::isfinite(dirty));
+  if (!resume) {
+    for (size_t k = sim->snaps.size(); k-- > 0;) {
+      const phs_sim::Snapshot &sn = *sim->snaps[k];
+      if (!(sn.t < dirty) || !(sn.t <= sim->t_stop) || !snapshot_usable(sim, sn)) continue;
+      phs_status rs = restore_snapshot(sim, k, st);
+      if (rs != PHS_OK) return rs;
+      resume = true;
+      break;
+    }
+    if (!resume) sim->snaps.clear();  // nothing usable: what is left would be later than the state we start from
+  }
+  sim->resumed_from = resume ? sim->parked_until : 0.0;
   // Until this call succeeds the handle has no results and no parked state: an error return below (history overflow,
   // a unit that does not fit, a CUDA failure) leaves units parked at the NEW stop time, which a later call with an
   // earlier time must not resume from.  Both flags are set again at the end.
@@ -1124,6 +1315,10 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   sim->ran = true;
   sim->have_park = finite;
   sim->parked_until = sim->t_stop;
+  if (finite) {
+    phs_status ss = take_snapshot(sim, st);
+    if (ss != PHS_OK) return ss;
+  }
   for (int u = 0; u < U; ++u) {
     const int i = sim->units[u].inst;
     if (sim->h_res[u].status == PHS_ECYCLE)

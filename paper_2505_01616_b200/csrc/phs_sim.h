@@ -6,6 +6,8 @@
 #include <algorithm>
 #include <atomic>
 #include <cstdlib>
+#include <deque>
+#include <limits>
 #include <memory>
 #include <string>
 #include <thread>
@@ -19,6 +21,9 @@
 
 // records the thread-local error message (phs_last_error) and returns `code`
 phs_status phs_fail(phs_status code, const std::string &msg);
+struct phs_sim;
+// drops the device tables, parked states and results: the next run builds everything again and starts at t = 0
+void phs_unfinalize(phs_sim *sim);
 
 #define PHS_CUDA(call)                                                                                       \
   do {                                                                                                       \
@@ -178,6 +183,24 @@ struct phs_sim {
   int cpark_cs = 0, cpark_L = 0;
   int64_t cpark_Sc = 0;
   double parked_until = 0.0;
+  // NEXT-1, time rollback: parked states of earlier stop times (phs_set_snapshots), newest last.  A snapshot is
+  // everything a resume needs: the parking areas of both kernel paths, the outstanding-predecessor counters, the
+  // per-unit result blocks and the length of the history at that time.
+  struct Snapshot {
+    double t = 0.0;
+    phs::DevBuf<unsigned char> park, cpark;
+    phs::DevBuf<int32_t> pred_cnt;
+    std::vector<phs::InstResult> res;
+    unsigned long long hist_n = 0;
+    size_t cpark_unit_bytes = 0, n_order = 0, n_cluster = 0;
+    int cpark_cs = 0, cpark_L = 0;
+    int64_t cpark_Sc = 0;
+  };
+  std::deque<std::unique_ptr<Snapshot>> snaps;
+  int max_snaps = 0;
+  double dirty_from = std::numeric_limits<double>::infinity();  // the simulated past is void from this time on
+  double resumed_from = 0.0;                                    // time of the state the last run continued from
+  std::vector<uint32_t> h_pos;  // output position of a flow -> its position in the per-flow device tables (lazy)
   std::vector<phs::InstDesc> h_desc;  // per unit
   std::vector<phs::InstResult> h_res; // per unit
   std::vector<int32_t> order;  // CTA-path instances, largest first

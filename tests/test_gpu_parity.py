@@ -583,3 +583,69 @@ def test_run_until_resumes_a_multi_cta_cluster():
             assert np.array_equal(np.diff(off), np.bincount(fl, minlength=o.num_flows))
             assert np.array_equal(tg, th) and np.array_equal(rg, rh)
     sim.close()
+
+
+@pytest.mark.parametrize("path", [0, CLUSTER])
+def test_time_rollback_equals_a_fresh_run(path):
+    """NEXT-1 (Fig. 4; L167): the simulation has run ahead in steps (every stop keeps a snapshot of
+    the parked on-chip state); then a flow's start time changes, flows arrive late, the past is declared void.  Every
+    re-simulation must equal the oracle run that had the change from t = 0 -- whose own rollback is pinned against
+    fresh runs -- and it must continue from the newest snapshot before the change, not from t = 0."""
+    for w in (W.cfg1(batch=3, n_hosts=8, gph=4, n_leaves=4, n_spines=2), W.train_step(batch=2, n_hosts=4, gph=4, layers=2, buckets=2)):
+        i = w.batch - 1
+        inst = w.instances[i]
+        base = oracle_run(w.desc, inst, mode=orc.MODE_FAST, base_seed=w.base_seed)
+        t_ref = base.completion_times()
+        t_end = t_ref.max()
+        off, pr = base.preds()
+        rel = np.array([t_ref[pr[off[f]:off[f + 1]]].max() if off[f + 1] > off[f] else 0.0 for f in range(base.num_flows)])
+        flow = int(np.flatnonzero((rel > 0.45 * t_end) & (rel < 0.58 * t_end))[0])
+        sim = B.Sim.from_workload(w, path=path)
+        B.phs_set_snapshots(sim.h, 8)
+        for frac in (0.2, 0.4, 0.6, 0.8):
+            sim.run(until=frac * t_end)
+        # (1) start-time update of a flow released between the snapshots at 0.4 and 0.6
+        B.phs_update_flow_start(sim.h, i, flow, 0.9 * t_end)
+        with pytest.raises(B.PhsError) as e:
+            sim.completion_times(i)
+        assert e.value.code == B.PHS_ESTATE
+        sim.run()
+        c = sim.counters()
+        assert c["resumed_from_s"] == 0.4 * t_end and c["resumed_units"] > 0, c
+        fresh = oracle_build(w.desc, inst, base_seed=w.base_seed)
+        fresh.update_flow_start(flow, 0.9 * t_end)
+        fresh.run(mode=orc.MODE_FAST)
+        assert not np.array_equal(fresh.completion_times(), t_ref)
+        assert_instance_matches(sim, i, fresh, check_log=False)
+        for j in range(w.batch - 1):                     # the other instances are untouched
+            assert_instance_matches(sim, j, oracle_run(w.desc, w.instances[j], mode=orc.MODE_FAST, base_seed=w.base_seed),
+                                    check_log=False)
+        # (2) the past declared void from 0.5 t_end: continue from the snapshot at 0.4, stop at 0.7
+        B.phs_rollback(sim.h, 0.5 * t_end)
+        sim.run(until=0.7 * t_end)
+        assert sim.counters()["resumed_from_s"] == 0.4 * t_end
+        part = oracle_build(w.desc, inst, base_seed=w.base_seed)
+        part.update_flow_start(flow, 0.9 * t_end)
+        part.run(mode=orc.MODE_FAST, until=0.7 * t_end)
+        assert np.array_equal(sim.completion_times(i), part.completion_times(), equal_nan=True)
+        assert np.array_equal(sim.bottlenecks(i), part.bottlenecks())
+        # (3) garbage collection keeps what a rollback to >= the watermark needs
+        B.phs_gc(sim.h, 0.45 * t_end)
+        B.phs_rollback(sim.h, 0.45 * t_end)
+        sim.run()
+        assert sim.counters()["resumed_from_s"] == 0.4 * t_end
+        assert_instance_matches(sim, i, fresh, check_log=False)
+        # (4) a late submission (flows with an earlier timestamp, one of them behind an old flow) and the start time
+        # of a flow without predecessors: tables rebuilt, results those of a fresh run
+        late = (np.array([0, 1], np.int32), np.array([5, 6], np.int32), np.array([3e6, 5e5]),
+                np.array([0.3, 0.05]) * t_end, np.array([0, 1, 1], np.int64), np.array([flow], np.int64))
+        B.phs_add_flows(sim.h, i, *late)
+        first_flow = int(np.flatnonzero(np.diff(off) == 0)[0])
+        B.phs_update_flow_start(sim.h, i, first_flow, 0.01 * t_end)
+        sim.run()
+        assert sim.counters()["resumed_from_s"] == 0.0
+        fresh.add_flows(*late)
+        fresh.update_flow_start(first_flow, 0.01 * t_end)
+        fresh.run(mode=orc.MODE_FAST)
+        assert_instance_matches(sim, i, fresh, check_log=False)
+        sim.close()
