@@ -110,6 +110,17 @@ typedef struct {
 /* Creates `batch` independent instances of one topology.  Instance i routes with ECMP seed `seed + i`.
  * Host-only; never touches the GPU. */
 phs_status phs_create_topology(const phs_topology_desc *desc, uint64_t seed, int32_t batch, phs_sim **out);
+/* User-supplied topology ("netsim takes a cluster topology configuration as input ... switch port
+ * bandwidth, cluster interconnection, multipath routing and load balancing strategies").  Nodes 0 .. n_gpus-1 are the
+ * GPUs, the others switches; link i (its id in every output) is the directed edge link_from[i] -> link_to[i] with
+ * capacity cap_Bps[i] and latency latency_s[i]; compute engine links (compute_lanes per GPU) follow.  Routing:
+ * shortest paths by hop count with seeded ECMP -- at a node the candidates are the out-links that lead one hop closer
+ * to the destination, in ascending link id, and hop k takes candidate mix(H ^ (k+1)) mod #candidates, H the hash of
+ * (seed, src, dst, connection) of the preset topologies.  Flows between GPUs without a route of at most 6 links are
+ * refused (PHS_EINVAL) when they are added. */
+phs_status phs_create_topology_graph(int32_t n_gpus, int32_t n_nodes, int32_t n_links, const int32_t *link_from,
+                                     const int32_t *link_to, const double *cap_Bps, const double *latency_s,
+                                     int32_t compute_lanes, uint64_t seed, int32_t batch, phs_sim **out);
 void phs_destroy(phs_sim *sim);
 phs_status phs_num_links(const phs_sim *sim, int32_t *out);
 phs_status phs_batch(const phs_sim *sim, int32_t *out);

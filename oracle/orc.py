@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
 OK, EINVAL, ENOMEM, ECYCLE, ESTATE, ERANGE = 0, -1, -2, -4, -5, -6
-TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE = 0, 1, 2
+TOPO_SINGLE, TOPO_LEAF_SPINE, TOPO_FAT_TREE, TOPO_GRAPH = 0, 1, 2, 3
 ALLREDUCE_RING, ALLGATHER_RING, REDUCESCATTER_RING, ALLTOALL = 0, 1, 2, 3
 BROADCAST_CHAIN, REDUCE_CHAIN, ALLREDUCE_TREE = 4, 5, 6
 MODE_NAIVE, MODE_FAST = 0, 1
@@ -94,6 +94,15 @@ class Sim:
 
     def __init__(self, desc: dict, seed: int = 0):
         self._h = C.c_void_p()
+        if "graph" in desc:          # user-supplied topology (NEXT-4): link list between nodes, GPUs are nodes 0..G-1
+            g = desc["graph"]
+            lf = np.ascontiguousarray(g["link_from"], dtype=np.int32); lt = np.ascontiguousarray(g["link_to"], dtype=np.int32)
+            cap = np.ascontiguousarray(g["cap_Bps"], dtype=np.float64); lat = np.ascontiguousarray(g["latency_s"], dtype=np.float64)
+            _chk(lib().orc_create_topology_graph(C.c_int32(g["n_gpus"]), C.c_int32(g["n_nodes"]), C.c_int32(len(lf)),
+                                                 _p(lf, C.c_int32), _p(lt, C.c_int32), _p(cap, C.c_double),
+                                                 _p(lat, C.c_double), C.c_int32(g.get("compute_lanes", 0)),
+                                                 C.c_uint64(seed), C.byref(self._h)), "orc_create_topology_graph")
+            return
         d = TopologyDesc(**desc)
         _chk(lib().orc_create_topology(C.byref(d), C.c_uint64(seed), C.byref(self._h)), "orc_create_topology")
 

@@ -33,6 +33,8 @@ struct orc_sim {
   orc_topology_desc d;
   uint64_t seed;
   int32_t G, n_links, n_net_links, ran;
+  /* ORC_TOPO_GRAPH: out-links of every node (CSR, ascending link id), endpoints, hop distance to every GPU */
+  int32_t n_nodes, *adj_off, *adj, *l_from, *l_to, *dist;
   double *cap, *lat; /* per directed link */
   /* flows */
   int64_t F, Fcap;
@@ -137,9 +139,75 @@ int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim *
   return ORC_OK;
 }
 
+int32_t orc_create_topology_graph(int32_t G, int32_t N, int32_t Ln, const int32_t *from, const int32_t *to,
+                                  const double *cap, const double *lat, int32_t lanes, uint64_t seed, orc_sim **out) {
+  if (!out || !from || !to || !cap || !lat || G < 2 || N < G || Ln < 1 || lanes < 0 || lanes > 64) return ORC_EINVAL;
+  for (int32_t i = 0; i < Ln; i++) {
+    if (from[i] < 0 || from[i] >= N || to[i] < 0 || to[i] >= N || from[i] == to[i]) return ORC_EINVAL;
+    if (!(cap[i] > 0) || !(cap[i] < 0x1p42) || !(lat[i] >= 0) || !(lat[i] < INFINITY)) return ORC_EINVAL;
+  }
+  int64_t L = (int64_t)Ln + (int64_t)G * lanes;
+  if (L > 0x3fffffff) return ORC_ERANGE;
+  orc_sim *s = (orc_sim *)calloc(1, sizeof(orc_sim));
+  if (!s) return ORC_ENOMEM;
+  s->d.kind = ORC_TOPO_GRAPH;
+  s->d.n_hosts = G; s->d.gpus_per_host = 1; s->d.compute_lanes = lanes;
+  s->seed = seed;
+  s->G = G; s->n_nodes = N; s->n_links = (int32_t)L; s->n_net_links = Ln;
+  s->cap = (double *)malloc(sizeof(double) * L);
+  s->lat = (double *)malloc(sizeof(double) * L);
+  s->path_off = (int64_t *)calloc(1, sizeof(int64_t));
+  s->pred_off = (int64_t *)calloc(1, sizeof(int64_t));
+  s->adj_off = (int32_t *)calloc(N + 1, sizeof(int32_t));
+  s->adj = (int32_t *)malloc(sizeof(int32_t) * Ln);
+  s->l_from = (int32_t *)malloc(sizeof(int32_t) * Ln);
+  s->l_to = (int32_t *)malloc(sizeof(int32_t) * Ln);
+  s->dist = (int32_t *)malloc(sizeof(int32_t) * (size_t)G * N);
+  int32_t *q = (int32_t *)malloc(sizeof(int32_t) * N), *rin_off = (int32_t *)calloc(N + 1, sizeof(int32_t)),
+          *rin = (int32_t *)malloc(sizeof(int32_t) * Ln);
+  if (!s->cap || !s->lat || !s->path_off || !s->pred_off || !s->adj_off || !s->adj || !s->l_from || !s->l_to || !s->dist ||
+      !q || !rin_off || !rin) {
+    free(q); free(rin_off); free(rin);
+    orc_destroy(s);
+    return ORC_ENOMEM;
+  }
+  for (int64_t l = 0; l < L; l++) { s->cap[l] = l < Ln ? cap[l] : 0x1p32; s->lat[l] = l < Ln ? lat[l] : 0.0; }
+  memcpy(s->l_from, from, sizeof(int32_t) * Ln);
+  memcpy(s->l_to, to, sizeof(int32_t) * Ln);
+  /* out-links per node in ascending link id (counting sort keeps the order), in-links likewise for the BFS */
+  for (int32_t i = 0; i < Ln; i++) { s->adj_off[from[i] + 1]++; rin_off[to[i] + 1]++; }
+  for (int32_t v = 0; v < N; v++) { s->adj_off[v + 1] += s->adj_off[v]; rin_off[v + 1] += rin_off[v]; }
+  {
+    int32_t *c1 = (int32_t *)malloc(sizeof(int32_t) * N), *c2 = (int32_t *)malloc(sizeof(int32_t) * N);
+    if (!c1 || !c2) { free(c1); free(c2); free(q); free(rin_off); free(rin); orc_destroy(s); return ORC_ENOMEM; }
+    memcpy(c1, s->adj_off, sizeof(int32_t) * N);
+    memcpy(c2, rin_off, sizeof(int32_t) * N);
+    for (int32_t i = 0; i < Ln; i++) { s->adj[c1[from[i]]++] = i; rin[c2[to[i]]++] = i; }
+    free(c1); free(c2);
+  }
+  /* dist[g][v] = links on a shortest path v -> GPU g (breadth-first search from g over the reversed links) */
+  for (int32_t g = 0; g < G; g++) {
+    int32_t *dg = s->dist + (size_t)g * N;
+    for (int32_t v = 0; v < N; v++) dg[v] = -1;
+    int32_t head = 0, tail = 0;
+    dg[g] = 0; q[tail++] = g;
+    while (head < tail) {
+      int32_t v = q[head++];
+      for (int32_t e = rin_off[v]; e < rin_off[v + 1]; e++) {
+        int32_t u = from[rin[e]];
+        if (dg[u] < 0) { dg[u] = dg[v] + 1; q[tail++] = u; }
+      }
+    }
+  }
+  free(q); free(rin_off); free(rin);
+  *out = s;
+  return ORC_OK;
+}
+
 void orc_destroy(orc_sim *s) {
   if (!s) return;
   for (int32_t c = 0; c < s->n_coll; c++) free(s->coll[c].ranks);
+  free(s->adj_off); free(s->adj); free(s->l_from); free(s->l_to); free(s->dist);
   free(s->coll); free(s->cap); free(s->lat); free(s->src); free(s->dst); free(s->conn); free(s->bytes);
   free(s->start); free(s->Lat); free(s->path_off); free(s->path); free(s->pred_off); free(s->pred);
   free(s->t_done); free(s->bneck); free(s->ev); free(s->tr);
@@ -180,6 +248,22 @@ static int32_t route(const orc_sim *s, int32_t src, int32_t dst, int32_t conn, i
   if (src == dst) { /* S7: a compute span; conn is its lane */
     p[0] = s->n_net_links + src * d->compute_lanes + conn;
     return 1;
+  }
+  if (d->kind == ORC_TOPO_GRAPH) { /* S8: hop by hop along shortest paths, seeded choice among the candidates */
+    uint64_t Hg = orc_mix64(orc_mix64(orc_mix64(orc_mix64(s->seed) ^ (uint64_t)(uint32_t)src) ^ (uint64_t)(uint32_t)dst) ^
+                            (uint64_t)(uint32_t)conn);
+    const int32_t *dg = s->dist + (size_t)dst * s->n_nodes;
+    int32_t u = src, k = 0;
+    if (dg[u] < 0 || dg[u] > 6) return -1; /* unreachable / too long */
+    while (u != dst) {
+      int32_t cand[64], nc = 0;
+      for (int32_t e = s->adj_off[u]; e < s->adj_off[u + 1]; e++)
+        if (dg[s->l_to[s->adj[e]]] == dg[u] - 1 && nc < 64) cand[nc++] = s->adj[e];
+      int32_t l = cand[orc_mix64(Hg ^ (uint64_t)(k + 1)) % (uint64_t)nc];
+      p[k++] = l;
+      u = s->l_to[l];
+    }
+    return k;
   }
   int32_t hs = src / d->gpus_per_host, hd = dst / d->gpus_per_host;
   if (hs == hd) {
@@ -229,6 +313,13 @@ static int32_t route(const orc_sim *s, int32_t src, int32_t dst, int32_t conn, i
   return 6;
 }
 
+/* graph topologies: is there a route of at most 6 links?  (the presets always have one) */
+static int routable(const orc_sim *s, int32_t src, int32_t dst) {
+  if (s->d.kind != ORC_TOPO_GRAPH || src == dst) return 1;
+  int32_t dd = s->dist[(size_t)dst * s->n_nodes + src];
+  return dd >= 1 && dd <= 6;
+}
+
 /* ------------------------------------------------------------------ flow table growth */
 static int grow_flows(orc_sim *s, int64_t need) {
   if (need <= s->Fcap) return 0;
@@ -264,6 +355,7 @@ static int begin_flow(orc_sim *s, int32_t src, int32_t dst, double bytes, double
   s->src[f] = src; s->dst[f] = dst; s->bytes[f] = bytes; s->start[f] = start; s->conn[f] = conn;
   int32_t p[6];
   int32_t h = route(s, src, dst, conn, p);
+  if (h < 0) return -2; /* no route of at most 6 links (graph topologies) */
   int64_t po = s->path_off[f];
   if (po + h > s->path_cap) {
     int64_t c = s->path_cap ? s->path_cap * 2 : 256;
@@ -365,6 +457,10 @@ int32_t orc_add_collective_full(orc_sim *s, int32_t kind, const int32_t *ranks, 
   }
   for (int32_t a = 0; a < n_after; a++)
     if (after[a] < 0 || after[a] >= s->n_coll) return ORC_EINVAL;
+  if (s->d.kind == ORC_TOPO_GRAPH) /* every pair of its ranks must be routable, whatever pairs the kind uses */
+    for (int32_t i = 0; i < N; i++)
+      for (int32_t j = 0; j < N; j++)
+        if (!routable(s, ranks[i], ranks[j])) return ORC_EINVAL;
   int32_t S = coll_steps(kind, N);
   int64_t nf = kind == ORC_ALLTOALL ? (int64_t)N * (N - 1)
              : kind == ORC_ALLREDUCE_TREE ? (int64_t)chunks * 2 * (N - 1)
@@ -474,6 +570,7 @@ int32_t orc_add_flows(orc_sim *s, int64_t n, const int32_t *src, const int32_t *
   }
   for (int64_t i = 0; i < n; i++) { /* validate everything before mutating */
     if (src[i] < 0 || src[i] >= s->G || dst[i] < 0 || dst[i] >= s->G || src[i] == dst[i]) return ORC_EINVAL;
+    if (!routable(s, src[i], dst[i])) return ORC_EINVAL;
     if (!(bytes[i] > 0) || !(bytes[i] < INFINITY)) return ORC_EINVAL;
     if (start && (!(start[i] >= 0) || !(start[i] < INFINITY))) return ORC_EINVAL;
     if (dep_off) {

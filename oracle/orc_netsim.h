@@ -46,7 +46,7 @@ extern "C" {
 typedef struct orc_sim orc_sim;
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ECYCLE = -4, ORC_ESTATE = -5, ORC_ERANGE = -6 };
-enum { ORC_TOPO_SINGLE = 0, ORC_TOPO_LEAF_SPINE = 1, ORC_TOPO_FAT_TREE = 2 };
+enum { ORC_TOPO_SINGLE = 0, ORC_TOPO_LEAF_SPINE = 1, ORC_TOPO_FAT_TREE = 2, ORC_TOPO_GRAPH = 3 };
 enum { ORC_ALLREDUCE_RING = 0, ORC_ALLGATHER_RING = 1, ORC_REDUCESCATTER_RING = 2, ORC_ALLTOALL = 3,
        /* NEXT-3: pipelined chain broadcast / reduce, binary-tree all-reduce; see orc_add_collective_ex */
        ORC_BROADCAST_CHAIN = 4, ORC_REDUCE_CHAIN = 5, ORC_ALLREDUCE_TREE = 6 };
@@ -73,6 +73,16 @@ typedef struct {
 
 /* One simulation instance.  `seed` is the instance's ECMP seed. */
 int32_t orc_create_topology(const orc_topology_desc *d, uint64_t seed, orc_sim **out);
+/* NEXT-4, user-supplied topology ("netsim takes a cluster topology configuration as input ... switch
+ * port bandwidth, cluster interconnection, multipath routing").  Reading S8: nodes 0..n_gpus-1 are the
+ * GPUs, the others switches; link i is the directed edge link_from[i] -> link_to[i] with its own capacity (byte/s)
+ * and latency (s); link ids are the caller's.  Routing = shortest paths by hop count with seeded ECMP: at node u
+ * the candidates are the out-links (u -> v) with dist(v, dst) = dist(u, dst) - 1, in ascending link id, and hop k
+ * (k = 0, 1, ...) takes candidate mix(H ^ (k + 1)) mod #candidates, H = the S2 hash of (seed, src, dst, conn).
+ * Paths longer than 6 links and unreachable pairs are refused when the flow is added. */
+int32_t orc_create_topology_graph(int32_t n_gpus, int32_t n_nodes, int32_t n_links, const int32_t *link_from,
+                                  const int32_t *link_to, const double *cap_Bps, const double *latency_s,
+                                  int32_t compute_lanes, uint64_t seed, orc_sim **out);
 void orc_destroy(orc_sim *s);
 int32_t orc_num_links(const orc_sim *s, int32_t *out);
 int32_t orc_set_link_capacities(orc_sim *s, const double *cap_Bps);

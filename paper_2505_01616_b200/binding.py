@@ -39,7 +39,7 @@ EVENT_DTYPE = np.dtype([("t", "<f8"), ("n_completed", "<i4"), ("n_activated", "<
                         ("first_bneck", "<i4")])
 
 # every symbol include/phs.h declares (tests check that the library exports all of them)
-SYMBOLS = ["phs_create_topology", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
+SYMBOLS = ["phs_create_topology", "phs_create_topology_graph", "phs_destroy", "phs_num_links", "phs_batch", "phs_set_link_capacities",
            "phs_set_link_capacities_batch",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_full", "phs_add_spans", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
@@ -91,6 +91,16 @@ def _p(a):
 # ---------------------------------------------------------------------------------------------- C-named calls
 def phs_create_topology(desc: dict, seed: int, batch: int):
     h = C.c_void_p()
+    if "graph" in desc:          # user-supplied topology: workloads.graph_desc
+        g = desc["graph"]
+        lf, lt = _arr(g["link_from"], np.int32), _arr(g["link_to"], np.int32)
+        cap, lat = _arr(g["cap_Bps"], np.float64), _arr(g["latency_s"], np.float64)
+        if not (len(lf) == len(lt) == len(cap) == len(lat)):
+            raise ValueError("link arrays have inconsistent lengths")
+        _chk(lib().phs_create_topology_graph(C.c_int32(g["n_gpus"]), C.c_int32(g["n_nodes"]), C.c_int32(len(lf)), _p(lf),
+                                             _p(lt), _p(cap), _p(lat), C.c_int32(g.get("compute_lanes", 0)),
+                                             C.c_uint64(seed), C.c_int32(batch), C.byref(h)), "phs_create_topology_graph")
+        return h
     d = TopologyDesc(**desc)
     _chk(lib().phs_create_topology(C.byref(d), C.c_uint64(seed), C.c_int32(batch), C.byref(h)), "phs_create_topology")
     return h

@@ -43,6 +43,39 @@ phs_status phs_create_topology(const phs_topology_desc *desc, uint64_t seed, int
   PHS_API_END
 }
 
+phs_status phs_create_topology_graph(int32_t n_gpus, int32_t n_nodes, int32_t n_links, const int32_t *link_from,
+                                     const int32_t *link_to, const double *cap_Bps, const double *latency_s,
+                                     int32_t compute_lanes, uint64_t seed, int32_t batch, phs_sim **out) {
+  PHS_API_BEGIN
+  if (!out || !link_from || !link_to || !cap_Bps || !latency_s || n_links < 1) return fail(PHS_EINVAL, "null argument");
+  if (batch <= 0) return fail(PHS_EINVAL, "batch must be positive");
+  GraphLinks g;
+  g.n_gpus = n_gpus;
+  g.n_nodes = n_nodes;
+  g.compute_lanes = compute_lanes;
+  g.from.assign(link_from, link_from + n_links);
+  g.to.assign(link_to, link_to + n_links);
+  g.cap.assign(cap_Bps, cap_Bps + n_links);
+  g.lat.assign(latency_s, latency_s + n_links);
+  std::string why;
+  phs_status st = Fabric::validate_graph(g, &why);
+  if (st != PHS_OK) return fail(st, why);
+  std::unique_ptr<phs_sim> s(new phs_sim());
+  s->desc = phs_topology_desc{};
+  s->desc.kind = 3;
+  s->desc.n_hosts = n_gpus;
+  s->desc.gpus_per_host = 1;
+  s->desc.compute_lanes = compute_lanes;
+  s->seed = seed;
+  s->batch = batch;
+  s->fab.reset(new Fabric(std::move(g)));
+  s->inst.resize((size_t)batch);
+  for (int32_t i = 0; i < batch; ++i) s->inst[i].seed = seed + (uint64_t)i;
+  *out = s.release();
+  return PHS_OK;
+  PHS_API_END
+}
+
 void phs_destroy(phs_sim *sim) { delete sim; }
 
 phs_status phs_num_links(const phs_sim *sim, int32_t *out) {

@@ -71,7 +71,78 @@ Fabric::Fabric(const phs_topology_desc &d) : d_(d) {
   links_ += gpus_ * d.compute_lanes;  // compute engine links (phs_add_spans) follow the network links
 }
 
+// ------------------------------------------------------------------------------------------------ graph (S8)
+phs_status Fabric::validate_graph(const GraphLinks &g, std::string *why) {
+  auto bad = [&](const char *m) {
+    if (why) *why = m;
+    return PHS_EINVAL;
+  };
+  if (g.n_gpus < 2 || g.n_nodes < g.n_gpus) return bad("a graph topology needs n_gpus >= 2 and n_nodes >= n_gpus");
+  if (g.compute_lanes < 0 || g.compute_lanes > 64) return bad("compute_lanes must be in [0, 64]");
+  if (g.from.empty()) return bad("a graph topology needs links");
+  for (size_t i = 0; i < g.from.size(); ++i) {
+    if (g.from[i] < 0 || g.from[i] >= g.n_nodes || g.to[i] < 0 || g.to[i] >= g.n_nodes || g.from[i] == g.to[i])
+      return bad("link endpoint out of range");
+    if (!(g.cap[i] > 0.0) || !(g.cap[i] < 0x1p42)) return bad("link capacity must be in (0, 2^42) byte/s");
+    if (!(g.lat[i] >= 0.0) || !std::isfinite(g.lat[i])) return bad("link latency must be >= 0 and finite");
+  }
+  if ((int64_t)g.from.size() + (int64_t)g.n_gpus * g.compute_lanes > 0x3fffffff) {
+    if (why) *why = "too many links";
+    return PHS_ERANGE;
+  }
+  return PHS_OK;
+}
+
+Fabric::Fabric(GraphLinks g) : d_{}, graph_(true), g_(std::move(g)) {
+  d_.kind = 3;
+  d_.n_hosts = g_.n_gpus;
+  d_.gpus_per_host = 1;
+  d_.compute_lanes = g_.compute_lanes;
+  gpus_ = g_.n_gpus;
+  net_links_ = (int32_t)g_.from.size();
+  links_ = net_links_ + gpus_ * g_.compute_lanes;
+  tier1_base_ = tier2_base_ = net_links_;
+  const int N = g_.n_nodes;
+  // out-links grouped by node: link ids sorted by (from, id)
+  out_link_.resize((size_t)net_links_);
+  for (int32_t i = 0; i < net_links_; ++i) out_link_[(size_t)i] = i;
+  std::stable_sort(out_link_.begin(), out_link_.end(), [&](int32_t a, int32_t b) { return g_.from[a] < g_.from[b]; });
+  out_off_.assign((size_t)N + 1, 0);
+  for (int32_t i = 0; i < net_links_; ++i) out_off_[(size_t)g_.from[i] + 1]++;
+  for (int v = 0; v < N; ++v) out_off_[(size_t)v + 1] += out_off_[(size_t)v];
+  // hop distance of every node to every GPU: level-synchronous search over the in-links
+  std::vector<std::vector<int32_t>> in_links((size_t)N);
+  for (int32_t i = 0; i < net_links_; ++i) in_links[(size_t)g_.to[i]].push_back(i);
+  hops_.assign((size_t)gpus_ * N, -1);
+  std::vector<int32_t> frontier, next;
+  for (int g0 = 0; g0 < gpus_; ++g0) {
+    int16_t *h = hops_.data() + (size_t)g0 * N;
+    h[g0] = 0;
+    frontier.assign(1, g0);
+    for (int16_t level = 1; !frontier.empty(); ++level) {
+      next.clear();
+      for (int32_t v : frontier)
+        for (int32_t l : in_links[(size_t)v]) {
+          const int32_t u = g_.from[(size_t)l];
+          if (h[u] < 0) {
+            h[u] = level;
+            next.push_back(u);
+          }
+        }
+      frontier.swap(next);
+    }
+  }
+}
+
+bool Fabric::routable(int32_t src, int32_t dst) const {
+  if (!graph_ || src == dst) return true;
+  const int16_t h = hops_[(size_t)dst * g_.n_nodes + src];
+  return h >= 1 && h <= kMaxHops;
+}
+
 double Fabric::default_capacity(int32_t link) const {
+  if (link >= net_links_) return 0x1p32;  // work units per second of a compute lane
+  if (graph_) return g_.cap[(size_t)link];
   if (link < 2 * gpus_) return d_.nvlink_Bps;
   if (link < 4 * gpus_) return d_.nic_Bps;
   if (link >= net_links_) return 0x1p32;  // work units per second of a compute lane
@@ -94,6 +165,32 @@ int Fabric::route(uint64_t seed, int32_t src, int32_t dst, int32_t conn, int32_t
   if (src == dst) {  // a compute span: the engine link of lane `conn` of the GPU
     out[0] = net_links_ + src * d_.compute_lanes + conn;
     return 1;
+  }
+  if (graph_) {  // S8: walk towards dst along shortest paths; hop k takes candidate mix(H ^ (k+1)) mod #candidates
+    uint64_t h = splitmix64_step(seed);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)src);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)dst);
+    h = splitmix64_step(h ^ (uint64_t)(uint32_t)conn);
+    const int16_t *left = hops_.data() + (size_t)dst * g_.n_nodes;
+    int n = 0;
+    for (int32_t at = src; at != dst && n < kMaxHops;) {
+      const uint64_t pick = splitmix64_step(h ^ (uint64_t)(n + 1));
+      // count the candidates, then take the pick-th (out-links are in ascending link id)
+      int n_cand = 0;
+      for (int32_t e = out_off_[(size_t)at]; e < out_off_[(size_t)at + 1]; ++e)
+        n_cand += left[g_.to[(size_t)out_link_[(size_t)e]]] == left[at] - 1;
+      int want = (int)(pick % (uint64_t)n_cand);
+      for (int32_t e = out_off_[(size_t)at]; e < out_off_[(size_t)at + 1]; ++e) {
+        const int32_t l = out_link_[(size_t)e];
+        if (left[g_.to[(size_t)l]] != left[at] - 1) continue;
+        if (want-- == 0) {
+          out[n++] = l;
+          at = g_.to[(size_t)l];
+          break;
+        }
+      }
+    }
+    return n;
   }
   const int gph = d_.gpus_per_host;
   const int host_s = src / gph, host_d = dst / gph;
@@ -254,6 +351,9 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   }
   for (int a = 0; a < n_after; ++a)
     if (after[a] < 0 || after[a] >= (int32_t)inst.colls.size()) return bad("after_coll_ids names an unknown collective");
+  for (int i = 0; i < N; ++i)
+    for (int j = 0; j < N; ++j)
+      if (!fab.routable(ranks[i], ranks[j])) return bad("two ranks of the collective have no route of at most 6 links");
   if (n_after_flows < 0 || (n_after_flows > 0 && !after_flows)) return bad("bad after_flow_ids");
   for (int a = 0; a < n_after_flows; ++a)
     if (after_flows[a] < 0 || after_flows[a] >= inst.n_flows()) return bad("after_flow_ids must name earlier flows");
@@ -416,6 +516,7 @@ phs_status append_flows(const Fabric &fab, Instance &inst, int64_t n, const int3
   for (int64_t i = 0; i < n; ++i) {  // validate first, mutate after
     if (src[i] < 0 || src[i] >= fab.n_gpus() || dst[i] < 0 || dst[i] >= fab.n_gpus()) return bad("rank out of range");
     if (src[i] == dst[i]) return bad("src == dst");
+    if (!fab.routable(src[i], dst[i])) return bad("no route of at most 6 links between src and dst");
     if (!(bytes[i] > 0.0) || !std::isfinite(bytes[i])) return bad("bytes must be positive and finite");
     if (start && (!(start[i] >= 0.0) || !std::isfinite(start[i]))) return bad("start_time_s must be >= 0 and finite");
     if (dep_off) {

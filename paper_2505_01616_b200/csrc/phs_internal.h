@@ -99,14 +99,28 @@ struct Instance {
 };
 
 // Link numbering and ECMP routing of one topology (S1, S2).
+// A user-supplied topology (phs_create_topology_graph): nodes 0 .. n_gpus-1 are the GPUs, the others switches; link i
+// is the directed edge from[i] -> to[i].
+struct GraphLinks {
+  int32_t n_gpus = 0, n_nodes = 0, compute_lanes = 0;
+  std::vector<int32_t> from, to;
+  std::vector<double> cap, lat;
+};
+
 class Fabric {
  public:
   explicit Fabric(const phs_topology_desc &d);
+  explicit Fabric(GraphLinks g);  // shortest-path ECMP over the link list (S8)
+  static phs_status validate_graph(const GraphLinks &g, std::string *why);
+  // is there a route of at most kMaxHops links?  (always, on the preset topologies)
+  bool routable(int32_t src, int32_t dst) const;
   static phs_status validate(const phs_topology_desc &d, std::string *why);
   int32_t n_gpus() const { return gpus_; }
   int32_t n_links() const { return links_; }
   double default_capacity(int32_t link) const;
-  double latency(int32_t link) const { return link < net_links_ ? d_.hop_latency_s : 0.0; }  // engine links: 0
+  double latency(int32_t link) const {  // engine links: 0
+    return link >= net_links_ ? 0.0 : graph_ ? g_.lat[(size_t)link] : d_.hop_latency_s;
+  }
   int32_t n_net_links() const { return net_links_; }
   int32_t compute_lanes() const { return d_.compute_lanes; }
   // writes the links of (src -> dst) for connection key `conn` into out[0..kMaxHops), returns the hop count
@@ -115,6 +129,10 @@ class Fabric {
  private:
   phs_topology_desc d_;
   int32_t gpus_, links_, net_links_, tier1_base_, tier2_base_;
+  bool graph_ = false;
+  GraphLinks g_;
+  std::vector<int32_t> out_off_, out_link_;  // out-links of every node, ascending link id
+  std::vector<int16_t> hops_;                // [gpu][node] links on a shortest path node -> gpu, -1 = unreachable
 };
 
 uint64_t splitmix64_step(uint64_t x);

@@ -33,6 +33,15 @@ def topo_desc(kind, n_hosts, gpus_per_host, nvlink_Bps=450e9, nic_Bps=50e9, fabr
                 compute_lanes=compute_lanes)
 
 
+def graph_desc(n_gpus, n_nodes, link_from, link_to, cap_Bps, latency_s, compute_lanes=0):
+    """User-supplied topology (NEXT-4): nodes 0..n_gpus-1 are GPUs, the rest switches; link i is the directed edge
+    link_from[i] -> link_to[i]."""
+    return dict(graph=dict(n_gpus=n_gpus, n_nodes=n_nodes, link_from=np.asarray(link_from, np.int32),
+                           link_to=np.asarray(link_to, np.int32), cap_Bps=np.asarray(cap_Bps, np.float64),
+                           latency_s=np.asarray(latency_s, np.float64), compute_lanes=compute_lanes),
+                n_hosts=n_gpus, gpus_per_host=1, compute_lanes=compute_lanes, nvlink_Bps=0.0)
+
+
 @dataclass
 class Coll:
     kind: int
@@ -311,6 +320,36 @@ def train_step(batch=4, n_hosts=8, gph=8, n_leaves=2, n_spines=2, layers=4, buck
                 nc += 1
         insts.append(Instance(seed=i, ops=ops, cap_pairs_Gbps=caps))
     return Workload("train_step", d, 0, insts)
+
+
+def graph_fabric(batch=2, n_gpus=16, gpus_per_leaf=4, n_spines=3, seed0=0):
+    """A user-supplied topology (NEXT-4): GPUs on leaf switches, every leaf wired to every spine, per-link capacities
+    U[100, 800] Gb/s and latencies U[0.5, 2] us (both directions drawn separately), one compute lane per GPU; on it a
+    mix of ring, tree and chain collectives with compute spans."""
+    n_leaves = n_gpus // gpus_per_leaf
+    rng = _rng(6, seed0)
+    lf, lt = [], []
+    for g in range(n_gpus):
+        leaf = n_gpus + g // gpus_per_leaf
+        lf += [g, leaf]; lt += [leaf, g]
+    for leaf in range(n_leaves):
+        for sp in range(n_spines):
+            a, b = n_gpus + leaf, n_gpus + n_leaves + sp
+            lf += [a, b]; lt += [b, a]
+    n = len(lf)
+    d = graph_desc(n_gpus, n_gpus + n_leaves + n_spines, lf, lt, gbps(rng.uniform(100.0, 800.0, n)),
+                   rng.uniform(0.5e-6, 2e-6, n), compute_lanes=1)
+    insts = []
+    for i in range(batch):
+        r = _rng(6, 100 + i)
+        perm = r.permutation(n_gpus).astype(np.int32)
+        ops = [Spans(np.arange(n_gpus, dtype=np.int32), r.uniform(10e-6, 80e-6, n_gpus)),
+               Coll(ALLREDUCE_RING, perm[:8], float(_loguniform(r, 1 * MiB, 64 * MiB)), 0.0, (), 1, tuple(range(n_gpus))),
+               Coll(ALLREDUCE_TREE, perm[4:15], float(_loguniform(r, 1 * MiB, 16 * MiB)), 1e-5, (), 3),
+               Coll(BROADCAST_CHAIN, perm[8:], float(_loguniform(r, 1 * MiB, 16 * MiB)), 0.0, (0,), 4),
+               Coll(ALLTOALL, perm[2:10], float(_loguniform(r, 1 * MiB, 8 * MiB)), 2e-5, (1,))]
+        insts.append(Instance(seed=i, ops=ops))
+    return Workload("graph_fabric", d, 7, insts)
 
 
 def by_name(name, **kw):

@@ -222,6 +222,14 @@ def test_compute_spans_training_step_on_every_path():
     sim.close()
 
 
+def test_graph_topology_on_every_path():
+    """NEXT-4: a user-supplied topology with per-link capacities and latencies."""
+    w = W.graph_fabric(batch=3)
+    for path in (0, CTA, CLUSTER):
+        run_and_compare(w, path=path)
+    _grid_compare(w)
+
+
 def test_cta_slot_overflow_falls_back_to_cluster():
     w = W.cfg4(batch=3, n_hosts=4, gph=8, n_leaves=2, n_spines=2)      # 992 flows pending at t=0 > 64 slots
     sim = B.Sim.from_workload(w, event_log=True, cta_slots=64)

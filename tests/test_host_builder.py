@@ -122,6 +122,28 @@ def test_compute_spans_and_flow_level_after_edges_equal_the_oracle():
     sim.close()
 
 
+def test_graph_topology_equals_the_oracle():
+    """NEXT-4: user-supplied link list with shortest-path ECMP -- routes, latencies, DAG equal the oracle's."""
+    _compare_tables(W.graph_fabric(batch=3))
+    _compare_tables(W.graph_fabric(batch=2, n_gpus=32, gpus_per_leaf=8, n_spines=4, seed0=1))
+    g = W.graph_fabric(batch=1).desc["graph"]
+    for bad in (dict(n_gpus=1), dict(n_nodes=3), dict(link_to=np.where(np.arange(len(g["link_to"])) == 0, 999, g["link_to"])),
+                dict(cap_Bps=np.where(np.arange(len(g["cap_Bps"])) == 3, 0.0, g["cap_Bps"]))):
+        with pytest.raises(B.PhsError) as e:
+            B.phs_create_topology(dict(graph=dict(g, **bad)), 0, 1)
+        assert e.value.code == B.PHS_EINVAL
+    # two GPUs eight switches apart: refused when the flow is added, nothing half-added
+    n = 10
+    lf = [0] + list(range(2, n)) + [1]; lt = list(range(2, n)) + [1] + [0]
+    sim = B.Sim(W.graph_desc(2, n, lf, lt, [1e9] * len(lf), [0.0] * len(lf)), batch=1)
+    with pytest.raises(B.PhsError) as e:
+        B.phs_add_flows(sim.h, 0, [0], [1], [1.0])
+    assert e.value.code == B.PHS_EINVAL and sim.num_flows(0) == 0
+    B.phs_add_flows(sim.h, 0, [1], [0], [1e3])
+    assert list(sim.paths(0)[1]) == [len(lf) - 1]
+    sim.close()
+
+
 def test_deferred_expansion_keeps_submission_order():
     """phs_add_collective records the collective and its flows are expanded later (by the next raw-flow submission,
     a table getter, or phs_finalize).  Flow ids must still follow submission order, and reading tables between

@@ -781,6 +781,76 @@ def test_next1_gc_keeps_every_later_rollback_exact():
         assert np.array_equal(fo[late], ff[keep]) and np.array_equal(to[late], tf[keep]) and np.array_equal(ro[late], rf[keep])
 
 
+# ------------------------------------------------------------------------------------------------ NEXT-4 graph topologies
+def _star(G, cap=50e9, lat=1e-6):
+    lf, lt = [], []
+    for g in range(G):
+        lf += [g, G]; lt += [G, g]          # link 2g: GPU g -> switch, 2g+1: switch -> GPU g
+    return W.graph_desc(G, G + 1, lf, lt, [cap] * (2 * G), [lat] * (2 * G))
+
+
+def test_next4_graph_topology_closed_forms_and_structure():
+    """Reading S8 (topology configuration as input): a user-supplied link list, shortest-path ECMP.
+    (1) a line GPU0 - s - s - GPU1 with different capacities and latencies: t = sum(lat) + bytes / min(cap), and the
+    bottleneck is the slowest link; (2) a star equals the single-switch preset on the NIC links, time for time;
+    (3) in a two-spine fabric every path is a shortest path made of consecutive links, both spines are used about
+    equally, and a connection keeps its path; (4) unroutable or too long pairs are refused."""
+    d = W.graph_desc(2, 4, [0, 2, 3, 1, 3, 2], [2, 3, 1, 3, 2, 0], [40e9, 10e9, 25e9, 40e9, 10e9, 25e9],
+                     [1e-6, 3e-6, 2e-6, 1e-6, 3e-6, 2e-6])
+    s = orc.Sim(d, 0)
+    s.add_flows([0, 1], [1, 0], [5e6, 2e6])
+    s.run()
+    assert list(s.paths()[1]) == [0, 1, 2, 3, 4, 5]
+    assert s.completion_times()[0] == pytest.approx(6e-6 + 5e6 / 10e9, rel=1e-12)
+    assert s.completion_times()[1] == pytest.approx(6e-6 + 2e6 / 10e9, rel=1e-12)
+    assert list(s.bottlenecks()) == [1, 4]
+    # (2) star == TOPO_SINGLE with one GPU per host (NIC links only), same workload
+    ops = [W.Coll(W.ALLREDUCE_RING, np.arange(8, dtype=np.int32), 32 * MiB), W.Coll(W.ALLTOALL, np.arange(8, dtype=np.int32), 8 * MiB, 1e-4)]
+    a = oracle_run(_star(8), W.Instance(seed=3, ops=ops))
+    b = oracle_run(W.topo_desc(W.TOPO_SINGLE, 8, 1), W.Instance(seed=3, ops=ops))
+    assert np.array_equal(a.completion_times(), b.completion_times())
+    assert np.array_equal(a.bottlenecks() + 16, b.bottlenecks())          # the preset numbers its NIC links from 2G on
+    # (3) 8 GPUs, 2 leaves (nodes 8, 9), 2 spines (10, 11)
+    lf, lt = [], []
+    for g in range(8):
+        leaf = 8 + g // 4
+        lf += [g, leaf]; lt += [leaf, g]
+    for leaf in (8, 9):
+        for sp in (10, 11):
+            lf += [leaf, sp]; lt += [sp, leaf]
+    d = W.graph_desc(8, 12, lf, lt, [50e9] * len(lf), [1e-6] * len(lf))
+    rng = np.random.default_rng(1)
+    src = rng.integers(0, 4, 2000).astype(np.int32)
+    dst = rng.integers(4, 8, 2000).astype(np.int32)
+    s = orc.Sim(d, 5)
+    s.add_flows(src, dst, np.ones(2000), conn_id=np.arange(2000, dtype=np.int32) % 97)
+    off, links = s.paths()
+    lf, lt = np.array(lf), np.array(lt)
+    via = np.zeros(2)
+    seen = {}
+    for f in range(2000):
+        p = links[off[f]:off[f + 1]]
+        assert len(p) == 4 and lf[p[0]] == src[f] and lt[p[-1]] == dst[f]
+        assert all(lt[p[k]] == lf[p[k + 1]] for k in range(3))
+        via[lt[p[1]] - 10] += 1
+        key = (src[f], dst[f], f % 97)
+        assert seen.setdefault(key, tuple(p)) == tuple(p)                 # same connection, same path
+    assert abs(via[0] - via[1]) < 4 * np.sqrt(2000)
+    s2 = orc.Sim(d, 6)
+    s2.add_flows(src, dst, np.ones(2000), conn_id=np.arange(2000, dtype=np.int32) % 97)
+    assert not np.array_equal(s2.paths()[1], links)                       # the seed moves flows
+    # (4) a chain of 8 switches between two GPUs is too long; an isolated GPU is unreachable
+    n = 10
+    lf = [0] + list(range(2, n)) + [1]; lt = list(range(2, n)) + [1] + [0]
+    s = orc.Sim(W.graph_desc(2, n, lf, lt, [1e9] * len(lf), [0.0] * len(lf)), 0)
+    with pytest.raises(orc.OrcError):
+        s.add_flows([0], [1], [1.0])
+    s.add_flows([1], [0], [1e3])                                          # the way back is one link
+    with pytest.raises(orc.OrcError):
+        s.add_collective(orc.ALLGATHER_RING, [0, 1], 1e3)
+    assert s.num_flows == 1
+
+
 # ------------------------------------------------------------------------------------------------ S2 routing pins
 def test_routing_leaf_spine_down_lane_comes_from_the_high_hash_word():
     """S2: with P parallel uplinks per (leaf, spine) the up lane is (H mod (n_spines P)) mod P and the down lane
