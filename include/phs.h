@@ -206,6 +206,17 @@ phs_status phs_set_decomposition(phs_sim *sim, int32_t enable);
  * always run one event per iteration.  Must precede phs_finalize. */
 phs_status phs_set_windows(phs_sim *sim, int32_t enable);
 
+/* Multi-GPU (batches shard naturally, a single instance does not).  Binds the handle to n CUDA
+ * devices of this process: phs_finalize cuts the batch into n contiguous blocks of instances (instance i keeps its ECMP
+ * seed `seed + i`) and builds block k's tables on device_ids[k]; phs_run / phs_run_until simulate all blocks at once
+ * (one host thread per device, each device's default stream: the cuda_stream argument is ignored); result getters go
+ * to the device that holds the instance, and an out_is_device buffer must live there.  No data-path collective
+ * exists or is needed.  A device may be listed more than once.  phs_get_all_* return host arrays only, and late
+ * submissions (after phs_finalize) are not supported on such a handle (PHS_ESTATE).  Must precede phs_finalize. */
+phs_status phs_set_devices(phs_sim *sim, int32_t n, const int32_t *device_ids);
+/* Device that holds `instance` after phs_finalize (the current device for a single-device handle). */
+phs_status phs_instance_device(const phs_sim *sim, int32_t instance, int32_t *out);
+
 /* Throughput history ("between neighboring events, network flows are assumed to have stable
  * throughput"; L167: a flow's history is a few floating point numbers per throughput change, from which a time
  * rollback reconstructs the state).  When enabled, every rate change of every flow is recorded as (time, new rate);

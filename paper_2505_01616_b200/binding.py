@@ -43,7 +43,7 @@ SYMBOLS = ["phs_create_topology", "phs_create_topology_graph", "phs_destroy", "p
            "phs_set_link_capacities_batch",
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_full", "phs_add_spans", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
-           "phs_set_decomposition", "phs_set_windows", "phs_set_snapshots", "phs_update_flow_start", "phs_rollback", "phs_gc",
+           "phs_set_decomposition", "phs_set_devices", "phs_instance_device", "phs_set_windows", "phs_set_snapshots", "phs_update_flow_start", "phs_rollback", "phs_gc",
            "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
@@ -230,6 +230,17 @@ def phs_set_decomposition(h, enable=True):
 
 def phs_set_windows(h, enable=True):
     _chk(lib().phs_set_windows(h, C.c_int32(1 if enable else 0)), "phs_set_windows")
+
+
+def phs_set_devices(h, device_ids):
+    d = _arr(device_ids, np.int32)
+    _chk(lib().phs_set_devices(h, C.c_int32(len(d)), _p(d)), "phs_set_devices")
+
+
+def phs_instance_device(h, instance):
+    d = C.c_int32()
+    _chk(lib().phs_instance_device(h, C.c_int32(instance), C.byref(d)), "phs_instance_device")
+    return d.value
 
 
 def phs_set_snapshots(h, n):

@@ -109,6 +109,46 @@ static phs_status check_instance(const phs_sim *sim, int32_t instance, bool allo
   return PHS_OK;
 }
 
+// multi-device handle after phs_finalize: the shard that holds `instance` (nullptr otherwise), the instance's index
+// there and the shard's device
+static phs_sim *shard_of(const phs_sim *sim, int32_t instance, int32_t *local, int *dev) {
+  if (!sim || sim->shards.empty() || instance < 0 || instance >= sim->batch) return nullptr;
+  const size_t k = (size_t)(std::upper_bound(sim->shard_first.begin(), sim->shard_first.end(), instance) -
+                            sim->shard_first.begin()) - 1;
+  *local = instance - sim->shard_first[k];
+  *dev = sim->devices[k];
+  return sim->shards[k].get();
+}
+
+phs_status phs_set_devices(phs_sim *sim, int32_t n, const int32_t *device_ids) {
+  PHS_API_BEGIN
+  if (!sim || n < 1 || !device_ids) return fail(PHS_EINVAL, "bad device list");
+  if (sim->finalized) return fail(PHS_ESTATE, "the devices must be chosen before phs_finalize");
+  for (int i = 0; i < n; ++i)
+    if (device_ids[i] < 0) return fail(PHS_EINVAL, "negative device id");
+  if (n > sim->batch) return fail(PHS_EINVAL, "more devices than instances: a single instance does not shard");
+  sim->devices.assign(device_ids, device_ids + n);
+  return PHS_OK;
+  PHS_API_END
+}
+
+phs_status phs_instance_device(const phs_sim *sim, int32_t instance, int32_t *out) {
+  PHS_API_BEGIN
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  if (!out) return fail(PHS_EINVAL, "null output");
+  int32_t li = 0;
+  int dev = 0;
+  if (shard_of(sim, instance, &li, &dev)) {
+    *out = dev;
+    return PHS_OK;
+  }
+  PHS_CUDA(cudaGetDevice(&dev));
+  *out = sim->devices.size() == 1 ? sim->devices[0] : dev;
+  return PHS_OK;
+  PHS_API_END
+}
+
 phs_status phs_set_link_capacities(phs_sim *sim, int32_t instance, const double *cap) {
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
@@ -166,6 +206,7 @@ phs_status phs_add_spans(phs_sim *sim, int32_t instance, int64_t n, const int32_
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
+  if (sim->finalized && !sim->shards.empty()) return fail(PHS_ESTATE, "late submissions are not supported on a multi-device handle");
   if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
@@ -189,6 +230,7 @@ phs_status phs_add_collective_full(phs_sim *sim, int32_t instance, int32_t kind,
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
+  if (sim->finalized && !sim->shards.empty()) return fail(PHS_ESTATE, "late submissions are not supported on a multi-device handle");
   if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
@@ -211,6 +253,7 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
                                     int32_t *out_id) {
   PHS_API_BEGIN
   if (!sim || !bytes) return fail(PHS_EINVAL, "null argument");
+  if (sim->finalized && !sim->shards.empty()) return fail(PHS_ESTATE, "late submissions are not supported on a multi-device handle");
   if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   for (int i = 1; i < sim->batch; ++i)
     if (sim->inst[i].colls.size() != sim->inst[0].colls.size())
@@ -238,6 +281,7 @@ phs_status phs_add_flows(phs_sim *sim, int32_t instance, int64_t n, const int32_
   PHS_API_BEGIN
   phs_status st = check_instance(sim, instance, true);
   if (st != PHS_OK) return st;
+  if (sim->finalized && !sim->shards.empty()) return fail(PHS_ESTATE, "late submissions are not supported on a multi-device handle");
   if (sim->finalized) phs_unfinalize(sim);  // a late submission: the tables are rebuilt by the next run
   const int lo = instance < 0 ? 0 : instance, hi = instance < 0 ? sim->batch : instance + 1;
   if (instance < 0)
@@ -395,6 +439,8 @@ namespace {
 template <typename T>
 phs_status fetch(const phs_sim *sim, const T *dev, int64_t first, int64_t count, T *out, int32_t out_is_device) {
   if (count == 0) return PHS_OK;
+  std::unique_ptr<DeviceGuard> on_device;  // phs_set_devices with one device
+  if (sim->devices.size() == 1) on_device.reset(new DeviceGuard(sim->devices[0]));
   const size_t bytes = sizeof(T) * (size_t)count;
   if (!out_is_device && bytes >= (256u << 10)) {
     // host output: through the page-locked staging area (phs_finalize sized it for the tables, so results fit),
@@ -424,6 +470,14 @@ extern "C" {
 
 phs_status phs_get_completion_times(const phs_sim *sim, int32_t instance, double *out, int64_t n, int32_t dev) {
   PHS_API_BEGIN
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) {
+      DeviceGuard guard_(dev_);
+      return phs_get_completion_times(sh_, li_, out, n, dev);
+    }
+  }
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -434,6 +488,14 @@ phs_status phs_get_completion_times(const phs_sim *sim, int32_t instance, double
 
 phs_status phs_get_bottlenecks(const phs_sim *sim, int32_t instance, int32_t *out, int64_t n, int32_t dev) {
   PHS_API_BEGIN
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) {
+      DeviceGuard guard_(dev_);
+      return phs_get_bottlenecks(sh_, li_, out, n, dev);
+    }
+  }
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -445,6 +507,17 @@ phs_status phs_get_bottlenecks(const phs_sim *sim, int32_t instance, int32_t *ou
 phs_status phs_get_all_completion_times(const phs_sim *sim, double *out, int64_t n, int32_t dev) {
   PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  if (!sim->shards.empty()) {  // one block per device, concatenated in instance order
+    if (dev) return fail(PHS_EINVAL, "a multi-device handle returns host arrays only");
+    if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
+    for (size_t k = 0; k < sim->shards.size(); ++k) {
+      DeviceGuard guard_(sim->devices[k]);
+      const phs_sim *sh = sim->shards[k].get();
+      phs_status st = phs_get_all_completion_times(sh, out + sim->flow_base[(size_t)sim->shard_first[k]], sh->total_flows, 0);
+      if (st != PHS_OK) return st;
+    }
+    return PHS_OK;
+  }
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
   return fetch(sim, sim->d_tdone.p, 0, n, out, dev);
@@ -454,6 +527,17 @@ phs_status phs_get_all_completion_times(const phs_sim *sim, double *out, int64_t
 phs_status phs_get_all_bottlenecks(const phs_sim *sim, int32_t *out, int64_t n, int32_t dev) {
   PHS_API_BEGIN
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
+  if (!sim->shards.empty()) {
+    if (dev) return fail(PHS_EINVAL, "a multi-device handle returns host arrays only");
+    if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
+    for (size_t k = 0; k < sim->shards.size(); ++k) {
+      DeviceGuard guard_(sim->devices[k]);
+      const phs_sim *sh = sim->shards[k].get();
+      phs_status st = phs_get_all_bottlenecks(sh, out + sim->flow_base[(size_t)sim->shard_first[k]], sh->total_flows, 0);
+      if (st != PHS_OK) return st;
+    }
+    return PHS_OK;
+  }
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
   return fetch(sim, sim->d_bneck.p, 0, n, out, dev);
@@ -462,6 +546,14 @@ phs_status phs_get_all_bottlenecks(const phs_sim *sim, int32_t *out, int64_t n, 
 
 phs_status phs_get_collective_times(const phs_sim *sim, int32_t instance, double *out, int32_t n) {
   PHS_API_BEGIN
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) {
+      DeviceGuard guard_(dev_);
+      return phs_get_collective_times(sh_, li_, out, n);
+    }
+  }
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -472,6 +564,14 @@ phs_status phs_get_collective_times(const phs_sim *sim, int32_t instance, double
 
 phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *out, int64_t cap, int64_t *n_events) {
   PHS_API_BEGIN
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) {
+      DeviceGuard guard_(dev_);
+      return phs_get_event_log(sh_, li_, out, cap, n_events);
+    }
+  }
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -487,6 +587,14 @@ phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *ou
 phs_status phs_get_flow_history(const phs_sim *sim, int32_t instance, int64_t *off, double *t, double *rate,
                                 int64_t cap, int64_t *n_records) {
   PHS_API_BEGIN
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) {
+      DeviceGuard guard_(dev_);
+      return phs_get_flow_history(sh_, li_, off, t, rate, cap, n_records);
+    }
+  }
   phs_status st = check_instance(sim, instance, false);
   if (st != PHS_OK) return st;
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
@@ -518,6 +626,24 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
   if (!sim || !out) return fail(PHS_EINVAL, "null argument");
   if (!sim->ran) return fail(PHS_ESTATE, "phs_run has not completed");
   phs_counters c{};
+  if (!sim->shards.empty()) {  // sums over the devices; kernel time = the slowest device (they run at once)
+    for (const auto &sh : sim->shards) {
+      phs_counters k{};
+      phs_status st = phs_get_counters(sh.get(), &k);
+      if (st != PHS_OK) return st;
+      c.n_events += k.n_events; c.n_flow_events += k.n_flow_events; c.sum_active += k.sum_active;
+      c.sum_par_rounds += k.sum_par_rounds; c.n_kernel_launches += k.n_kernel_launches; c.h2d_bytes += k.h2d_bytes;
+      c.n_windows += k.n_windows; c.resumed_units += k.resumed_units;
+      c.max_active = std::max(c.max_active, k.max_active); c.max_slots = std::max(c.max_slots, k.max_slots);
+      c.cluster_size = std::max(c.cluster_size, k.cluster_size);
+      c.clusters_resident = std::max(c.clusters_resident, k.clusters_resident);
+      c.window_gang = std::max(c.window_gang, k.window_gang); c.grid_ctas = std::max(c.grid_ctas, k.grid_ctas);
+      c.main_kernel_ms = std::max(c.main_kernel_ms, k.main_kernel_ms);
+      c.resumed_from_s = k.resumed_from_s;
+    }
+    *out = c;
+    return PHS_OK;
+  }
   for (size_t i = 0; i < sim->units.size(); ++i) {
     c.n_events += sim->h_res[i].n_events;
     c.sum_active += sim->h_res[i].sum_active;
@@ -543,6 +669,11 @@ phs_status phs_get_counters(const phs_sim *sim, phs_counters *out) {
 
 const char *phs_instance_path(const phs_sim *sim, int32_t instance) {
   if (!sim || instance < 0 || instance >= sim->batch || !sim->ran) return "";
+  {
+    int32_t li_ = 0;
+    int dev_ = 0;
+    if (phs_sim *sh_ = shard_of(sim, instance, &li_, &dev_)) return phs_instance_path(sh_, li_);
+  }
   int best = sim->unit_first[instance];  // the path of the instance's largest unit
   for (int u = best; u < sim->unit_first[instance + 1]; ++u)
     if (sim->units[u].n_flows > sim->units[best].n_flows) best = u;

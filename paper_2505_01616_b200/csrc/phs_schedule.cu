@@ -97,6 +97,74 @@ bool plan_window_unit(phs_sim *sim, int u, size_t smem_max, int64_t scale) {
 
 }  // namespace
 
+
+// ================================================================================================ multi-GPU shards
+namespace {
+
+// fn(k, shard) on one host thread per shard, the shard's device current; returns the first error (message included)
+template <typename Fn>
+phs_status for_each_shard(phs_sim *sim, Fn fn) {
+  const size_t n = sim->shards.size();
+  std::vector<phs_status> rc(n, PHS_OK);
+  std::vector<std::string> msg(n);
+  std::vector<std::thread> pool;
+  for (size_t k = 0; k < n; ++k)
+    pool.emplace_back([&, k] {
+      DeviceGuard guard(sim->devices[k]);
+      rc[k] = fn(k, sim->shards[k].get());
+      if (rc[k] != PHS_OK) msg[k] = phs_last_error();  // the message is thread-local: take it along
+    });
+  for (std::thread &th : pool) th.join();
+  for (size_t k = 0; k < n; ++k)
+    if (rc[k] != PHS_OK) return fail(rc[k], "device " + std::to_string(sim->devices[k]) + ": " + msg[k]);
+  return PHS_OK;
+}
+
+// phs_set_devices with several devices: contiguous blocks of instances, one child handle per device
+phs_status finalize_sharded(phs_sim *sim) {
+  const int n = (int)sim->devices.size(), B = sim->batch;
+  sim->flow_base.assign((size_t)B + 1, 0);
+  sim->coll_base.assign((size_t)B + 1, 0);
+  for (int i = 0; i < B; ++i) {
+    sim->flow_base[(size_t)i + 1] = sim->flow_base[(size_t)i] + sim->inst[(size_t)i].n_flows();
+    sim->coll_base[(size_t)i + 1] = sim->coll_base[(size_t)i] + (int64_t)sim->inst[(size_t)i].colls.size();
+  }
+  sim->total_flows = sim->flow_base[(size_t)B];
+  sim->total_colls = sim->coll_base[(size_t)B];
+  sim->shards.clear();
+  sim->shard_first.assign((size_t)n + 1, 0);
+  for (int k = 0; k < n; ++k) sim->shard_first[(size_t)k + 1] = sim->shard_first[(size_t)k] + B / n + (k < B % n ? 1 : 0);
+  for (int k = 0; k < n; ++k) {
+    const int first = sim->shard_first[(size_t)k], cnt = sim->shard_first[(size_t)k + 1] - first;
+    std::unique_ptr<phs_sim> c(new phs_sim());
+    c->desc = sim->desc;
+    c->seed = sim->seed + (uint64_t)first;  // instance i keeps its ECMP seed
+    c->batch = cnt;
+    c->fab = sim->fab;
+    c->inst.assign(sim->inst.begin() + first, sim->inst.begin() + first + cnt);
+    c->want_log = sim->want_log;
+    c->policy_path = sim->policy_path;
+    c->policy_slots = sim->policy_slots;
+    c->decompose = sim->decompose;
+    c->windows = sim->windows;
+    c->hist_cap = sim->hist_cap;
+    c->max_snaps = sim->max_snaps;
+    c->devices.assign(1, sim->devices[(size_t)k]);
+    sim->shards.push_back(std::move(c));
+  }
+  phs_status st = for_each_shard(sim, [](size_t, phs_sim *c) { return phs_finalize(c, nullptr); });
+  if (st != PHS_OK) {
+    sim->shards.clear();
+    return st;
+  }
+  sim->h2d_bytes = 0;
+  for (const auto &c : sim->shards) sim->h2d_bytes += c->h2d_bytes;
+  sim->finalized = true;
+  return PHS_OK;
+}
+
+}  // namespace
+
 // ================================================================================================ finalize
 // Splits the instances into simulation units and builds the device-resident tables.  HBM layout (DESIGN.md "Data
 // layout"): one 64-byte FlowRec per flow (path, successors and component inline, unit-local ids), successor lists
@@ -107,6 +175,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
   PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (sim->finalized) return PHS_OK;
+  if (sim->devices.size() > 1) return finalize_sharded(sim);
+  std::unique_ptr<DeviceGuard> on_device;  // phs_set_devices with one device
+  if (sim->devices.size() == 1) on_device.reset(new DeviceGuard(sim->devices[0]));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const bool timing_ = getenv("PHS_TIMING") != nullptr;
   auto tp_ = std::chrono::steady_clock::now();
@@ -1052,6 +1123,7 @@ bool snapshot_usable(const phs_sim *sim, const phs_sim::Snapshot &sn) {
 extern "C" phs_status phs_set_snapshots(phs_sim *sim, int32_t n) {
   PHS_API_BEGIN
   if (!sim || n < 0) return fail(PHS_EINVAL, "bad snapshot count");
+  for (auto &c : sim->shards) phs_set_snapshots(c.get(), n);
   sim->max_snaps = n;
   while ((int)sim->snaps.size() > n) sim->snaps.pop_front();
   return PHS_OK;
@@ -1061,6 +1133,7 @@ extern "C" phs_status phs_set_snapshots(phs_sim *sim, int32_t n) {
 extern "C" phs_status phs_rollback(phs_sim *sim, double t_s) {
   PHS_API_BEGIN
   if (!sim || !(t_s >= 0.0)) return fail(PHS_EINVAL, "bad rollback time");
+  for (auto &c : sim->shards) phs_rollback(c.get(), t_s);
   sim->dirty_from = std::min(sim->dirty_from, t_s);
   sim->ran = false;  // no results until the next run
   return PHS_OK;
@@ -1070,6 +1143,7 @@ extern "C" phs_status phs_rollback(phs_sim *sim, double t_s) {
 extern "C" phs_status phs_gc(phs_sim *sim, double t_s) {
   PHS_API_BEGIN
   if (!sim || !(t_s >= 0.0)) return fail(PHS_EINVAL, "bad watermark");
+  for (auto &c : sim->shards) phs_gc(c.get(), t_s);
   // keep the newest snapshot below the watermark (a rollback to t_s continues from it) and everything later
   while (sim->snaps.size() >= 2 && sim->snaps[1]->t < t_s) sim->snaps.pop_front();
   return PHS_OK;
@@ -1086,6 +1160,14 @@ extern "C" phs_status phs_update_flow_start(phs_sim *sim, int32_t instance, int6
   const double old = in.start[(size_t)flow];
   in.start[(size_t)flow] = start;
   if (!sim->finalized || old == start) return PHS_OK;
+  if (!sim->shards.empty()) {  // the shard that holds the instance does the rest, on its device
+    const size_t k = (size_t)(std::upper_bound(sim->shard_first.begin(), sim->shard_first.end(), instance) -
+                              sim->shard_first.begin()) - 1;
+    DeviceGuard guard(sim->devices[k]);
+    return phs_update_flow_start(sim->shards[k].get(), instance - sim->shard_first[k], flow, start);
+  }
+  std::unique_ptr<DeviceGuard> on_device;
+  if (sim->devices.size() == 1) on_device.reset(new DeviceGuard(sim->devices[0]));
   const uint32_t p0 = in.pred_off[(size_t)flow], p1 = in.pred_off[(size_t)flow + 1];
   if (p0 == p1) {  // in the sorted initial-activation lists, and in a slot from t = 0: rebuild, start again at 0
     phs_unfinalize(sim);
@@ -1134,6 +1216,19 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   PHS_API_BEGIN
   if (!sim) return fail(PHS_EINVAL, "null handle");
   if (!(t_stop_s >= 0.0)) return fail(PHS_EINVAL, "t_stop_s must be >= 0");
+  if (sim->devices.size() > 1) {  // every device simulates its block of instances, all at once
+    if (!sim->finalized) {
+      phs_status fs = phs_finalize(sim, nullptr);
+      if (fs != PHS_OK) return fs;
+    }
+    sim->ran = false;
+    phs_status rs = for_each_shard(sim, [t_stop_s](size_t, phs_sim *c) { return phs_run_until(c, t_stop_s, nullptr); });
+    if (rs != PHS_OK) return rs;
+    sim->ran = true;
+    return PHS_OK;
+  }
+  std::unique_ptr<DeviceGuard> on_device;  // phs_set_devices with one device
+  if (sim->devices.size() == 1) on_device.reset(new DeviceGuard(sim->devices[0]));
   sim->t_stop = t_stop_s;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (!sim->finalized) {

@@ -49,6 +49,18 @@ void phs_unfinalize(phs_sim *sim);
 
 namespace phs {
 
+// makes `dev` the current CUDA device for a scope (multi-device handles)
+struct DeviceGuard {
+  int old = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&old) != cudaSuccess) old = -1;
+    cudaSetDevice(dev);
+  }
+  ~DeviceGuard() {
+    if (old >= 0) cudaSetDevice(old);
+  }
+};
+
 // fn(i) for every i in [0, n) on up to `max_threads` (<= 16) host threads; the iterations must be independent
 template <typename F>
 void parallel_for(int n, F fn, int max_threads = 16) {
@@ -145,10 +157,17 @@ struct phs_sim {
   phs_topology_desc desc;
   uint64_t seed;
   int32_t batch;
-  std::unique_ptr<phs::Fabric> fab;
+  std::shared_ptr<phs::Fabric> fab;  // immutable after construction: shared with the shards of a multi-device handle
   std::vector<phs::Instance> inst;
   bool want_log = false, finalized = false, ran = false;
   int32_t policy_path = 0, policy_slots = 0;
+
+  // ---- NEXT-4, multi-GPU (phs_set_devices): instances are independent, so a handle bound to several devices is cut
+  // into contiguous blocks of instances, one child handle ("shard") per device, built at phs_finalize; runs go to
+  // all shards at once (one host thread each), result getters to the shard that holds the instance.
+  std::vector<int> devices;
+  std::vector<std::unique_ptr<phs_sim>> shards;
+  std::vector<int32_t> shard_first;  // [n_shards + 1] first instance of every shard
 
   // ---- host mirrors built by finalize
   std::vector<int64_t> flow_base;  // [B+1]

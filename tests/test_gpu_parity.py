@@ -657,3 +657,56 @@ def test_time_rollback_equals_a_fresh_run(path):
         fresh.run(mode=orc.MODE_FAST)
         assert_instance_matches(sim, i, fresh, check_log=False)
         sim.close()
+
+
+def test_multi_device_handle_shards_the_batch():
+    """NEXT-4 / SURVEY.md 8(e): a handle bound to several devices cuts the batch into blocks of instances, one child
+    handle per device, no data-path collective.  One GPU is visible here, so it is listed three times: three shards,
+    three host threads, three sets of tables -- same results as the unsharded handle and the oracle."""
+    import torch
+    w = W.cfg3(batch=7)
+    ref = B.Sim.from_workload(w)
+    ref.run()
+    sim = B.Sim.from_workload(w)
+    B.phs_set_devices(sim.h, [0, 0, 0])
+    B.phs_set_snapshots(sim.h, 4)
+    sim.run()
+    assert [B.phs_instance_device(sim.h, i) for i in range(7)] == [0] * 7
+    for i in range(7):
+        assert np.array_equal(sim.completion_times(i), ref.completion_times(i))
+        assert np.array_equal(sim.bottlenecks(i), ref.bottlenecks(i))
+        assert np.array_equal(sim.collective_times(i), ref.collective_times(i))
+        assert sim.path_of(i) == ref.path_of(i)
+    for i in (0, 3, 6):                                  # first, middle and last block: seeds follow the instance index
+        assert_instance_matches(sim, i, oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST), check_log=False)
+    assert np.array_equal(B.phs_get_all_completion_times(sim.h), B.phs_get_all_completion_times(ref.h))
+    assert np.array_equal(B.phs_get_all_bottlenecks(sim.h), B.phs_get_all_bottlenecks(ref.h))
+    c, cr = sim.counters(), ref.counters()
+    assert c["n_events"] == cr["n_events"] and c["n_flow_events"] == cr["n_flow_events"] and c["sum_active"] == cr["sum_active"]
+    out = torch.empty(sim.num_flows(5), dtype=torch.float64, device="cuda")
+    B.phs_get_completion_times(sim.h, 5, device_ptr=out.data_ptr())
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), ref.completion_times(5))
+    with pytest.raises(B.PhsError) as e:                 # late submissions are a single-device feature
+        B.phs_add_flows(sim.h, 0, [0], [9], [1e6])
+    assert e.value.code == B.PHS_ESTATE
+    # stop times, rollback and start-time updates are routed to the shards
+    t_end = max(ref.completion_times(i).max() for i in range(7))
+    for frac in (0.3, 0.6):
+        sim.run(until=frac * t_end)
+        ref.run(until=frac * t_end)
+        for i in range(7):
+            assert np.array_equal(sim.completion_times(i), ref.completion_times(i), equal_nan=True)
+    base = oracle_run(w.desc, w.instances[4], mode=orc.MODE_FAST)
+    off, pr = base.preds()
+    t4 = base.completion_times()
+    rel = np.array([t4[pr[off[f]:off[f + 1]]].max() if off[f + 1] > off[f] else 0.0 for f in range(base.num_flows)])
+    flow = int(np.flatnonzero((rel > 0.3 * t4.max()) & (rel < 0.7 * t4.max()))[0])
+    B.phs_update_flow_start(sim.h, 4, flow, 0.9 * t_end)
+    sim.run()
+    fresh = oracle_build(w.desc, w.instances[4])
+    fresh.update_flow_start(flow, 0.9 * t_end)
+    fresh.run(mode=orc.MODE_FAST)
+    assert_instance_matches(sim, 4, fresh, check_log=False)
+    assert_instance_matches(sim, 2, oracle_run(w.desc, w.instances[2], mode=orc.MODE_FAST), check_log=False)
+    sim.close(); ref.close()

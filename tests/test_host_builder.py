@@ -144,6 +144,19 @@ def test_graph_topology_equals_the_oracle():
     sim.close()
 
 
+def test_set_devices_is_validated_on_the_host():
+    w = W.cfg3(batch=3)
+    sim = B.Sim.from_workload(w)
+    for bad in ([], [-1], [0, 0, 0, 0]):                # empty, negative id, more devices than instances
+        with pytest.raises((B.PhsError, ValueError, TypeError)):
+            B.phs_set_devices(sim.h, bad)
+    B.phs_set_devices(sim.h, [0, 0])
+    with pytest.raises(B.PhsError) as e:                # no CUDA device here: the shards fail loudly, nothing falls back
+        sim.run()
+    assert e.value.code == B.PHS_ECUDA
+    sim.close()
+
+
 def test_deferred_expansion_keeps_submission_order():
     """phs_add_collective records the collective and its flows are expanded later (by the next raw-flow submission,
     a table getter, or phs_finalize).  Flow ids must still follow submission order, and reading tables between
