@@ -247,6 +247,29 @@ phs_status phs_run(phs_sim *sim, void *cuda_stream);
  * the results are the same either way. */
 phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
 
+/* phs_run without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  Same computation as phs_run (PAPER.md L165 water-filling, L128 / L308 event
+ * loop, L104 completion times), every unit simulated by the whole grid (the grid path of phs_set_scheduler), but the
+ * kernel's scratch -- per-flow and per-link state, and the unit list -- is a fixed __device__ array of
+ * PHS_STATIC_SCRATCH_BYTES inside the library (every GPU that loads libphs holds it until the process exits) instead of
+ * memory from cudaMalloc.  The call makes no cudaMalloc / cudaFree / cudaHostAlloc and calls no allocating routine; it
+ * enqueues on `cuda_stream` and waits for the status, like phs_run.
+ *   inputs   the handle: it must be finalized (phs_finalize builds the device tables -- call it at set-up), bound to
+ *            one device (the current one, or the one of phs_set_devices), without event log and throughput history.
+ *   outputs  t_done_dev[n], bneck_dev[n]: DEVICE arrays of the caller on the handle's device, n = phs_total_flows,
+ *            all instances concatenated in instance order (either may be NULL).  The handle holds the same results:
+ *            the phs_get_* calls work after it as after phs_run.
+ *   limits   PHS_ERANGE (nothing ran; the message names the sizes) if the handle has more than PHS_STATIC_MAX_UNITS
+ *            simulation units, or if its largest unit needs more than PHS_STATIC_SCRATCH_BYTES - 4 * PHS_STATIC_MAX_UNITS
+ *            bytes of state: 40 bytes per flow + 56 per link + 1 KiB, i.e. about 200,000 flows in one unit.
+ *   sharing  every call on a device uses the one array, which keeps the contents of the last call; the kernel
+ *            initialises all of it that it reads, so nothing carries over.  Two calls that overlap on one GPU (two
+ *            streams, two threads, two handles) race: serialise them.
+ * PHS_ESTATE if the handle is not finalized, has several devices, or has the event log / history enabled. */
+#define PHS_STATIC_SCRATCH_BYTES (8u << 20)
+#define PHS_STATIC_MAX_UNITS 4096
+phs_status phs_run_static(phs_sim *sim, void *cuda_stream, double *t_done_dev, int32_t *bneck_dev, int64_t n);
+
 /* Time rollback (sec 4.2 "the network simulator rolls back to T2 and adds a flow starting at T2",
  * Fig. 4; L167 sec 5: "one for updating the start time of an existing flow, and another for advancing the simulation
  * ... up to a specified time").

@@ -44,7 +44,7 @@ SYMBOLS = ["phs_create_topology", "phs_create_topology_graph", "phs_destroy", "p
            "phs_get_link_capacities", "phs_add_collective", "phs_add_collective_ex", "phs_add_collective_full", "phs_add_spans", "phs_add_collective_batch", "phs_add_flows",
            "phs_enable_event_log", "phs_enable_history", "phs_get_flow_history", "phs_set_scheduler",
            "phs_set_decomposition", "phs_set_devices", "phs_instance_device", "phs_set_windows", "phs_set_snapshots", "phs_update_flow_start", "phs_rollback", "phs_gc",
-           "phs_finalize", "phs_run", "phs_run_until", "phs_num_flows", "phs_total_flows",
+           "phs_finalize", "phs_run", "phs_run_until", "phs_run_static", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
            "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
@@ -271,6 +271,16 @@ def phs_run(h, stream=None):
     _chk(lib().phs_run(h, C.c_void_p(stream or 0)), "phs_run")
 
 
+PHS_STATIC_SCRATCH_BYTES = 8 << 20
+PHS_STATIC_MAX_UNITS = 4096
+
+
+def phs_run_static(h, t_done_dev, bneck_dev, n, stream=None):
+    """t_done_dev / bneck_dev: DEVICE addresses (int, e.g. torch.Tensor.data_ptr()) of n doubles / n int32, or None."""
+    _chk(lib().phs_run_static(h, C.c_void_p(stream or 0), C.c_void_p(t_done_dev or 0), C.c_void_p(bneck_dev or 0),
+                              C.c_int64(n)), "phs_run_static")
+
+
 def phs_num_flows(h, instance):
     n = C.c_int64()
     _chk(lib().phs_num_flows(h, C.c_int32(instance), C.byref(n)), "phs_num_flows")
@@ -469,6 +479,9 @@ class Sim:
             phs_run(self.h, stream)
         else:
             phs_run_until(self.h, until, stream)
+
+    def run_static(self, t_done_dev=None, bneck_dev=None, stream=None):
+        phs_run_static(self.h, t_done_dev, bneck_dev, self.total_flows, stream)
 
     def num_flows(self, i):
         return phs_num_flows(self.h, i)

@@ -129,6 +129,14 @@ cudaError_t grid_max_ctas(int *n_ctas);
 cudaError_t launch_grid_path(const DevTables &t, const int32_t *list, int n, unsigned char *scratch, int64_t max_flows,
                              int max_links, int n_ctas, cudaStream_t stream);
 
+// phs_run_static: the same kernel with its scratch (and the unit list 0 .. n_units-1) in a file-scope __device__ array
+// of kStaticScratchBytes; allocates nothing.  cudaErrorInvalidValue if the list or the state does not fit.
+constexpr size_t kStaticScratchBytes = PHS_STATIC_SCRATCH_BYTES;
+constexpr size_t kStaticListBytes = (size_t)PHS_STATIC_MAX_UNITS * sizeof(int32_t);
+size_t grid_static_capacity();  // bytes left for per-flow / per-link state (grid_scratch_bytes must not exceed it)
+cudaError_t launch_grid_static(const DevTables &t, int n_units, int64_t max_flows, int max_links, int n_ctas,
+                               cudaStream_t stream);
+
 // NEXT-1: forgets the results later than t (t_done = NaN, bneck = -1)
 cudaError_t launch_forget_after(double *t_done, int32_t *bneck, int64_t n, double t, cudaStream_t stream);
 

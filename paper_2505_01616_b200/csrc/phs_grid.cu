@@ -375,4 +375,61 @@ cudaError_t launch_grid_path(const DevTables &t, const int32_t *list, int n, uns
   return cudaLaunchCooperativeKernel(fn, dim3((unsigned)n_ctas), dim3(kGridThreads), args, 0, stream);
 }
 
+// ------------------------------------------------------------------------------------------ phs_run_static
+// The grid path without any allocation: the kernel's scratch (unit list, per-flow and per-link state) is this
+// file-scope array, kStaticScratchBytes on every device that loads the library, held until the process exits.  Every
+// call shares it: calls that overlap on one GPU race.  Nothing has to be cleared between calls -- the kernel's init
+// phase writes every word it later reads (per unit: link counts, stamps, control words, every flow's state) and the
+// unit list is rewritten by phs_static_list_kernel at the start of every call.
+static __device__ __align__(256) unsigned char phs_static_scratch[kStaticScratchBytes];
+
+namespace {
+
+// the unit list of a static run is 0 .. n-1, in the first kStaticListBytes of the array (device code names it directly)
+__global__ void phs_static_list_kernel(int n) {
+  int32_t *list = reinterpret_cast<int32_t *>(phs_static_scratch);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) list[i] = i;
+}
+
+// In host code `phs_static_scratch` is a host-side stand-in, not a device address: the address the kernel gets comes
+// from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kMaxStaticDevices = 64;
+cudaError_t static_scratch_address(unsigned char **out) {
+  static unsigned char *addr[kMaxStaticDevices] = {};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxStaticDevices) return cudaErrorInvalidDevice;
+  unsigned char *p = __atomic_load_n(&addr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    void *sym = nullptr;
+    e = cudaGetSymbolAddress(&sym, phs_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!sym) return cudaErrorInvalidSymbol;
+    p = static_cast<unsigned char *>(sym);
+    __atomic_store_n(&addr[dev], p, __ATOMIC_RELEASE);  // every thread gets the same answer for one device
+  }
+  *out = p;
+  return cudaSuccess;
+}
+
+}  // namespace
+
+size_t grid_static_capacity() { return kStaticScratchBytes - kStaticListBytes; }
+
+cudaError_t launch_grid_static(const DevTables &t, int n_units, int64_t max_flows, int max_links, int n_ctas,
+                               cudaStream_t stream) {
+  if (n_units < 1 || (size_t)n_units * sizeof(int32_t) > kStaticListBytes ||
+      grid_scratch_bytes(max_flows, max_links) > grid_static_capacity())
+    return cudaErrorInvalidValue;  // the caller (phs_run_static) checks first and says which limit it was
+  unsigned char *base = nullptr;
+  cudaError_t e = static_scratch_address(&base);
+  if (e != cudaSuccess) return e;
+  phs_static_list_kernel<<<(n_units + 255) / 256, 256, 0, stream>>>(n_units);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  return launch_grid_path(t, reinterpret_cast<const int32_t *>(base), n_units, base + kStaticListBytes, max_flows,
+                          max_links, n_ctas, stream);
+}
+
 }  // namespace phs

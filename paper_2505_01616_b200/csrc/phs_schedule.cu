@@ -1426,3 +1426,88 @@ extern "C" phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_st
   PHS_API_END
 }
 
+
+// phs_run without allocation (include/phs.h): every unit on the grid path, the kernel's scratch in the library's static
+// __device__ array (phs_grid.cu).  Only enqueues kernels, memsets and copies on buffers phs_finalize made.
+extern "C" phs_status phs_run_static(phs_sim *sim, void *cuda_stream, double *t_done_dev, int32_t *bneck_dev, int64_t n) {
+  PHS_API_BEGIN
+  if (!sim) return fail(PHS_EINVAL, "null handle");
+  if (!sim->shards.empty() || sim->devices.size() > 1)
+    return fail(PHS_ESTATE, "phs_run_static: the handle is bound to several devices");
+  if (!sim->finalized) return fail(PHS_ESTATE, "phs_run_static builds nothing: call phs_finalize first");
+  if (sim->want_log || sim->hist_cap > 0)
+    return fail(PHS_ESTATE, "phs_run_static: the grid path writes no event log and the static run keeps no history");
+  if (n != sim->total_flows) return fail(PHS_EINVAL, "n must equal the total flow count");
+  const int U = (int)sim->units.size();
+  int64_t Fm = 1;
+  int Lm = 1;
+  for (int u = 0; u < U; ++u) {
+    Fm = std::max<int64_t>(Fm, sim->units[(size_t)u].n_flows);
+    Lm = std::max(Lm, sim->units[(size_t)u].n_links);
+  }
+  if (U > PHS_STATIC_MAX_UNITS)
+    return fail(PHS_ERANGE, "phs_run_static: " + std::to_string(U) + " simulation units, the static unit list holds " +
+                                std::to_string(PHS_STATIC_MAX_UNITS));
+  if (grid_scratch_bytes(Fm, Lm) > grid_static_capacity())
+    return fail(PHS_ERANGE, "phs_run_static: the largest unit (" + std::to_string(Fm) + " flows, " + std::to_string(Lm) +
+                                " links) needs " + std::to_string(grid_scratch_bytes(Fm, Lm)) +
+                                " bytes of state, the static scratch holds " + std::to_string(grid_static_capacity()));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int cur = 0;
+  PHS_CUDA(cudaGetDevice(&cur));
+  const int want = sim->devices.size() == 1 ? sim->devices[0] : cur;
+  struct Restore {  // phs_set_devices with one device: run there, leave the caller's device as it was
+    int dev;
+    bool on;
+    ~Restore() {
+      if (on) cudaSetDevice(dev);
+    }
+  } restore{cur, want != cur};
+  if (want != cur) PHS_CUDA(cudaSetDevice(want));
+  // like phs_run: until the call succeeds the handle has no results and no parked state
+  // (dirty_from is left alone: snapshots later than it stay void for the next phs_run_until)
+  sim->t_stop = std::numeric_limits<double>::infinity();
+  sim->have_park = false;
+  sim->ran = false;
+  sim->last_stream = st;
+  sim->resumed_from = 0.0;
+  sim->resumed_units = 0;
+  sim->win_gang_used = 0;
+  sim->n_launches = 0;
+  sim->grid_ctas = 0;
+  sim->main_kernel_ms = 0.f;
+  if (U > 0) {
+    int n_ctas = 0;
+    PHS_CUDA(grid_max_ctas(&n_ctas));
+    if (n_ctas < 1) return fail(PHS_ECUDA, "grid path: the kernel cannot be resident");
+    n_ctas = (int)std::max<int64_t>(1, std::min<int64_t>(n_ctas, (Fm + kGridThreads - 1) / kGridThreads));
+    PHS_CUDA(cudaMemsetAsync(sim->d_res.p, 0, sizeof(InstResult) * (size_t)U, st));  // empty units report status OK
+    PHS_CUDA(cudaEventRecord(sim->ev0, st));
+    PHS_CUDA(launch_grid_static(tables_of(sim, Lm), U, Fm, Lm, n_ctas, st));
+    PHS_CUDA(cudaEventRecord(sim->ev1, st));
+    sim->grid_ctas = n_ctas;
+    sim->n_launches = 2;  // the unit-list kernel and the grid kernel
+    PHS_CUDA(cudaMemcpyAsync(sim->h_res.data(), sim->d_res.p, sizeof(InstResult) * (size_t)U, cudaMemcpyDeviceToHost, st));
+  }
+  if (sim->total_colls > 0) sim->n_launches++;
+  PHS_CUDA(launch_collective_times(sim->d_tdone.p, sim->d_coll_first.p, sim->d_coll_n.p, sim->total_colls,
+                                   sim->d_coll_t.p, st));
+  if (t_done_dev && n > 0)
+    PHS_CUDA(cudaMemcpyAsync(t_done_dev, sim->d_tdone.p, sizeof(double) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+  if (bneck_dev && n > 0)
+    PHS_CUDA(cudaMemcpyAsync(bneck_dev, sim->d_bneck.p, sizeof(int32_t) * (size_t)n, cudaMemcpyDeviceToDevice, st));
+  PHS_CUDA(cudaStreamSynchronize(st));
+  if (U > 0) PHS_CUDA(cudaEventElapsedTime(&sim->main_kernel_ms, sim->ev0, sim->ev1));
+  sim->ran = true;
+  sim->parked_until = sim->t_stop;
+  for (int u = 0; u < U; ++u) {
+    const int i = sim->units[(size_t)u].inst;
+    if (sim->h_res[(size_t)u].status == PHS_ECYCLE)
+      return fail(PHS_ECYCLE, "instance " + std::to_string(i) + ": flows left waiting on dependencies that never complete");
+    if (sim->h_res[(size_t)u].status != PHS_OK)
+      return fail(PHS_ECUDA, "instance " + std::to_string(i) + ": unexpected kernel status " +
+                                 std::to_string(sim->h_res[(size_t)u].status));
+  }
+  return PHS_OK;
+  PHS_API_END
+}
