@@ -55,7 +55,8 @@ struct DevTables {
 
 // Shared-memory footprint of the CTA kernel for given capacities (pc_flows > 0: predecessor counters of that
 // many flows are kept in shared memory as bytes).
-size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log);
+size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log, int lean = 0);
+size_t cta_lean_scratch_bytes(int n_links);  // global scratch per CTA of a lean launch
 
 // One CTA per instance (persistent CTAs pull instance indices from order[0..n) through *ticket).
 // Instances that run out of shared-memory slots finish with status kOverflow.
@@ -64,6 +65,12 @@ struct CtaLaunch {
   int n_links;  // largest link count among the units of the launch
   size_t smem;
   bool log;
+  // Lean shared-memory layout, for batches with many times more units than can be resident (the SMs' issue slots are
+  // the limit and every further resident CTA hides latency): bit 0 = the per-link arrays that only a solve with a
+  // second filling round touches, and the link ids, live in global memory (lean_scratch: grid * cta_lean_scratch_bytes,
+  // L2-resident) and in the unit's tables; bit 1 = so do the capacities.  0 = everything in shared memory.
+  int lean;
+  unsigned char *lean_scratch;
 };
 cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &cfg,
                             cudaStream_t stream);

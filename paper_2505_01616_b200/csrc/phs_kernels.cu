@@ -74,30 +74,35 @@ __device__ __forceinline__ int path_at(const uint4 &p, int h) {
   return (int)((h & 1) ? (w >> 16) : (w & 0xffffu));
 }
 
-__host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, int S, int pcf, bool log) {
+// `lean` (CtaLaunch::lean): bit 0 = the arrays only a solve with a second round touches (l_caprem, l_sharew, l_nw,
+// l_deb) and the link ids (l_gid, read once per completion) are not in shared memory -- the kernel points them at a
+// per-CTA global scratch region and at the unit's linkid table; bit 1 = l_cap likewise reads the unit's capq table.
+// With `lean` the carved pointers of those fields are not valid.
+__host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, int S, int pcf, bool log, int lean) {
   size_t o = 0, a;
 #define PHS_TAKE(field, type, count)                    \
   a = o;                                                \
   o = align_up(o + sizeof(type) * (size_t)(count), 16); \
   if (s) s->field = (type *)(base + a);
-  PHS_TAKE(l_cap, long long, L)
+  const int Lw = (lean & 1) ? 0 : L, Lcap = (lean & 2) ? 0 : L;
+  PHS_TAKE(l_cap, long long, Lcap)
   PHS_TAKE(l_share0, long long, L)
-  PHS_TAKE(l_caprem, long long, L)
-  PHS_TAKE(l_sharew, long long, L)
+  PHS_TAKE(l_caprem, long long, Lw)
+  PHS_TAKE(l_sharew, long long, Lw)
   PHS_TAKE(s_tc, double, S)
   PHS_TAKE(s_rem, double, S)
   PHS_TAKE(s_tl, double, S)
   PHS_TAKE(s_rq, long long, S)
   PHS_TAKE(red, double, 32)
-  PHS_TAKE(red_key, long long, 32)
+  PHS_TAKE(red_key, long long, log ? 32 : 0)
   PHS_TAKE(l_n0, int, L)
   PHS_TAKE(l_chg, int, L)
   PHS_TAKE(l_beat, int, L)
-  PHS_TAKE(l_nw, int, L)
-  PHS_TAKE(l_deb, int, L)
+  PHS_TAKE(l_nw, int, Lw)
+  PHS_TAKE(l_deb, int, Lw)
   PHS_TAKE(l_solve, int, L)
   PHS_TAKE(l_won, int, log ? L : 0)
-  PHS_TAKE(l_gid, int, L)
+  PHS_TAKE(l_gid, int, Lw)
   PHS_TAKE(s_meta, int4, S)
   PHS_TAKE(s_path, uint4, S)
   PHS_TAKE(s_succ_cnt, int, S)
@@ -105,7 +110,7 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   PHS_TAKE(s_succ1, int, S)
   PHS_TAKE(free_q, int, S)
   PHS_TAKE(pc8, unsigned, (pcf + 7) / 8)
-  PHS_TAKE(red_id, int, 32)
+  PHS_TAKE(red_id, int, log ? 32 : 0)
   PHS_TAKE(ctl, int, 32)
 #undef PHS_TAKE
   return o;
@@ -133,8 +138,11 @@ __device__ __forceinline__ double warp_min_nonneg(double v) {
 
 }  // namespace
 
-size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
-  return carve(nullptr, nullptr, n_links, slots, pc_flows, log);
+size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log, int lean) {
+  return carve(nullptr, nullptr, n_links, slots, pc_flows, log, lean);
+}
+size_t cta_lean_scratch_bytes(int n_links) {  // per CTA: l_caprem, l_sharew (8 each), l_nw, l_deb (4 each)
+  return align_up((size_t)n_links * 24, 256);
 }
 
 // ================================================================================================ CTA kernel
@@ -143,12 +151,20 @@ size_t cta_smem_bytes(int n_links, int slots, int pc_flows, bool log) {
 // HIST: record the throughput history (a call in the hottest block of the kernel: compiled out when not wanted).
 template <int NT, bool LOG, bool PCS, bool HIST>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
-                                                     int *ticket, int SC, int pcf) {
+                                                     int *ticket, int SC, int pcf, int lean,
+                                                     unsigned char *lean_scratch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ int sh_inst;
   CtaSmem S;
   const int L = T.n_links;
-  const size_t smem_used = carve(&S, smem_raw, L, SC, pcf, LOG);
+  const size_t smem_used = carve(&S, smem_raw, L, SC, pcf, LOG, lean);
+  if (lean & 1) {  // working arrays of multi-round solves: this CTA's region of the global scratch (L2-resident)
+    unsigned char *w = lean_scratch + (size_t)blockIdx.x * align_up((size_t)L * 24, 256);
+    S.l_caprem = (long long *)w;
+    S.l_sharew = S.l_caprem + L;
+    S.l_nw = (int *)(S.l_sharew + L);
+    S.l_deb = S.l_nw + L;
+  }
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = NT / 32;
 
@@ -177,10 +193,13 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
     const bool resuming =
         T.resume && T.park && ((const ParkRegs *)(T.park + (size_t)inst * T.park_stride))->valid;
     // ---- init: nothing active, every slot free
+    // lean layout: capacities and link ids are read where they are (the unit's tables)
+    const long long *l_cap = (lean & 2) ? (const long long *)capq : S.l_cap;
+    const int *l_gid = (lean & 1) ? (const int *)linkid : S.l_gid;
     if (!resuming)
     for (int l = tid; l < Li; l += NT) {
-      S.l_cap[l] = capq[l];
-      S.l_gid[l] = linkid[l];
+      if (!(lean & 2)) S.l_cap[l] = capq[l];
+      if (!(lean & 1)) S.l_gid[l] = linkid[l];
       S.l_n0[l] = 0;
       S.l_chg[l] = 0;
       S.l_beat[l] = 0;
@@ -188,6 +207,10 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       S.l_solve[l] = 0;
       if (LOG) S.l_won[l] = 0;
     }
+    // the scratch region served another unit (or another CTA parked this one): no debit stamp may look current.
+    // No solve is in progress between events, and round numbers compared with l_deb are >= 1.
+    if (resuming && (lean & 1))
+      for (int l = tid; l < Li; l += NT) S.l_deb[l] = 0;
     if (!resuming) {
     for (int s = tid; s < SC; s += NT) {
       S.s_meta[s].x = -1;
@@ -373,7 +396,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         // the flow completes at t_next (bit-equal absolute time, S4.4)
         const int f = S.s_meta[s].x;
         t_done[f] = t_next;
-        bneck_out[f] = S.l_gid[S.s_meta[s].y];
+        bneck_out[f] = l_gid[S.s_meta[s].y];
         const uint4 pv = S.s_path[s];
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
@@ -436,7 +459,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       for (int l = tid; l < Li; l += NT) {
         if (S.l_chg[l] != solve) continue;
         const int n = S.l_n0[l];
-        if (n > 0) S.l_share0[l] = fair_share(S.l_cap[l], n);
+        if (n > 0) S.l_share0[l] = fair_share(l_cap[l], n);
       }
       __syncthreads();
 
@@ -547,7 +570,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           for (int h = 0; h < kMaxHops; ++h) {
             const int l = path_at(pv, h);
             if (l == (int)kNoLink) continue;
-            S.l_caprem[l] = S.l_cap[l];
+            S.l_caprem[l] = l_cap[l];
             S.l_nw[l] = S.l_n0[l];
             S.l_sharew[l] = S.l_share0[l];
           }
@@ -702,7 +725,8 @@ cudaError_t launch_hist(const DevTables &t, const int32_t *order, int n, int *ti
   cudaError_t e = cudaFuncSetAttribute(phs_cta_kernel<NT, LOG, PCS, HIST>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
   if (e != cudaSuccess) return e;
-  phs_cta_kernel<NT, LOG, PCS, HIST><<<c.grid, NT, c.smem, stream>>>(t, order, n, ticket, c.slots, c.pc_flows);
+  phs_cta_kernel<NT, LOG, PCS, HIST><<<c.grid, NT, c.smem, stream>>>(t, order, n, ticket, c.slots, c.pc_flows, c.lean,
+                                                                    c.lean_scratch);
   return cudaGetLastError();
 }
 template <int NT, bool LOG, bool PCS>

@@ -684,17 +684,17 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const int want = std::max(1, std::min(2048 / threads / 2, ((int)cand.size() + sim->sm_count - 1) / sim->sm_count));
     // largest number of resident CTAs per SM (<= want) whose shared memory holds `need` slots, with or without the
     // predecessor counters on chip; returns 0 if not even one fits
-    auto fit = [&](bool pcs, int *slots_out) {
+    auto fit = [&](bool pcs, int lean, int *slots_out) {
       const int pcf = pcs ? (int)maxF : 0;
       for (int w = want; w >= 1; --w) {
         const size_t budget = std::min(smem_max, per_sm / w - 1024);
-        if (cta_smem_bytes(Lm, 32, pcf, log) > budget) continue;
+        if (cta_smem_bytes(Lm, 32, pcf, log, lean) > budget) continue;
         int lo = 32, hi = (int)std::min<int64_t>(std::max<int64_t>(maxF, 32), 1 << 16);
         if (sim->policy_slots > 0 && sim->policy_path != 3) hi = std::max(32, std::min(hi, (int)sim->policy_slots));
         hi = (hi + 31) / 32 * 32;
         while (lo < hi) {  // largest multiple of 32 that fits the budget
           const int mid = ((lo + hi + 32) / 64) * 32;
-          if (cta_smem_bytes(Lm, mid, pcf, log) <= budget)
+          if (cta_smem_bytes(Lm, mid, pcf, log, lean) <= budget)
             lo = mid;
           else
             hi = mid - 32;
@@ -708,8 +708,27 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       }
       return 0;
     };
+    // Lean layout (CtaLaunch::lean): in the throughput regime (the same test as for the thread count) every further
+    // resident CTA hides latency, so the per-link arrays that only multi-round solves touch -- and, if that buys
+    // another CTA, the capacities -- leave shared memory.  Latency-bound batches keep everything on chip.
+    int lean = 0;
+    if ((int64_t)cand.size() >= 64LL * sim->sm_count && !log) {
+      int best_w = 0;
+      for (int cand_lean : {0, 1, 3}) {
+        int sl = 0;
+        const int w = std::max(pc8_ok ? fit(true, cand_lean, &sl) : 0, fit(false, cand_lean, &sl));
+        if (w > best_w) {
+          best_w = w;
+          lean = cand_lean;
+        }
+      }
+    }
+    if (const char *ev = getenv("PHS_CTA_LEAN")) {  // tuning experiments
+      const int v = atoi(ev);
+      if (v == 0 || v == 1 || v == 3) lean = log ? 0 : v;
+    }
     int slots_p = 0, slots_n = 0;
-    const int w_p = pc8_ok ? fit(true, &slots_p) : 0, w_n = fit(false, &slots_n);
+    const int w_p = pc8_ok ? fit(true, lean, &slots_p) : 0, w_n = fit(false, lean, &slots_n);
     if (w_p == 0 && w_n == 0) {
       // the largest links x slots combination does not fit one SM: the unit with the most flows goes to a cluster
       auto big = std::max_element(cand.begin(), cand.end(), [&](int a, int b) {
@@ -724,7 +743,9 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     sim->cta.threads = threads;
     sim->cta.slots = pcs ? slots_p : slots_n;
     sim->cta.pc_flows = pcs ? (int)maxF : 0;
-    sim->cta.smem = cta_smem_bytes(Lm, sim->cta.slots, sim->cta.pc_flows, log);
+    sim->cta.smem = cta_smem_bytes(Lm, sim->cta.slots, sim->cta.pc_flows, log, lean);
+    sim->cta.lean = lean;
+    sim->cta.lean_scratch = nullptr;  // allocated below, once the grid is known
     sim->cta.log = log;
     sim->cta.n_links = Lm;
     sim->order = cand;
@@ -733,9 +754,13 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const int per = std::max(1, std::min<int>((int)(per_sm / (sim->cta.smem + 1024)), 2048 / threads));
     sim->cta.grid = std::min((int)cand.size(), per * sim->sm_count);
     PHS_CUDA(sim->d_order.upload(sim->order, st));
+    if (lean & 1) {
+      PHS_CUDA(sim->d_lean.alloc(cta_lean_scratch_bytes(Lm) * (size_t)sim->cta.grid));
+      sim->cta.lean_scratch = sim->d_lean.p;
+    }
     if (timing_)
-      fprintf(stderr, "[phs_finalize] cta path: %d units, threads %d, need %d, links %d, slots %d, smem %zu, grid %d (%d per SM)\n",
-              (int)cand.size(), threads, need, Lm, sim->cta.slots, sim->cta.smem, sim->cta.grid, per);
+      fprintf(stderr, "[phs_finalize] cta path: %d units, threads %d, need %d, links %d, slots %d, smem %zu, lean %d, grid %d (%d per SM)\n",
+              (int)cand.size(), threads, need, Lm, sim->cta.slots, sim->cta.smem, lean, sim->cta.grid, per);
     break;
   }
   std::sort(sim->cluster_list.begin(), sim->cluster_list.end());
@@ -937,6 +962,10 @@ phs_status run_grid_path(phs_sim *sim, const std::vector<int32_t> &list, cudaStr
   if (n_ctas < 1) return fail(PHS_ECUDA, "grid path: the kernel cannot be resident");
   // no more CTAs than the largest unit can use (one flow per thread)
   n_ctas = (int)std::max<int64_t>(1, std::min<int64_t>(n_ctas, (Fm + kGridThreads - 1) / kGridThreads));
+  if (const char *ev = getenv("PHS_GRID_CTAS")) {  // tuning experiments: fewer CTAs than the default
+    const int v = atoi(ev);
+    if (v >= 1 && v < n_ctas) n_ctas = v;
+  }
   PHS_CUDA(sim->d_glist.upload(list, st));
   PHS_CUDA(launch_grid_path(tables_of(sim, Lm), sim->d_glist.p, (int)list.size(), sim->d_gscratch.p, Fm, Lm, n_ctas, st));
   PHS_DBG("grid path: launched");

@@ -260,6 +260,7 @@ struct phs_sim {
   phs::DevBuf<phs::InstResult> d_res;
   phs::DevBuf<phs_event> d_log;
   phs::DevBuf<int> d_ticket;
+  phs::DevBuf<unsigned char> d_lean;  // CTA path, lean layout: per-CTA global scratch of the working link arrays
   // cluster-path scratch: one region per concurrently running cluster
   phs::DevBuf<uint8_t> g_scratch;
   phs::DevBuf<int32_t> d_clist, d_lcomp;

@@ -570,6 +570,43 @@ def test_run_until_resumes_from_the_parked_state(path):
         sim.close()
 
 
+@pytest.mark.parametrize("lean", ["1", "3"])
+def test_cta_path_lean_layout(monkeypatch, lean):
+    """CtaLaunch::lean (csrc/phs_device.h): in the throughput regime the scheduler moves the per-link arrays that only
+    multi-round solves touch (and the capacities) from shared memory to a per-CTA global scratch, so that more CTAs
+    are resident.  Forced here (PHS_CTA_LEAN) on small batches: ring traffic with single-round solves, all-to-all
+    traffic with many rounds per event, several units per CTA in a row (the scratch is reused), and a run that is
+    stopped and resumed (a parked unit continues on another CTA's scratch region)."""
+    monkeypatch.setenv("PHS_CTA_LEAN", lean)
+    for w in (W.cfg3(batch=5), W.cfg1(batch=2, n_hosts=8, gph=4, n_leaves=4, n_spines=2),
+              W.cfg4(batch=3, n_hosts=8, gph=8, n_leaves=4, n_spines=2), W.cfg2(k=4, agg_uplinks=1)):
+        for decompose in (True, False):
+            sim = B.Sim.from_workload(w, path=CTA, decompose=decompose)
+            sim.run()
+            for i in range(w.batch):
+                o = oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST, base_seed=w.base_seed)
+                assert_instance_matches(sim, i, o, check_log=False)
+            assert sim.path_of(0) in ("cta", "cluster")         # a unit that runs out of slots moves to a cluster
+            sim.close()
+    w = W.cfg4(batch=2, n_hosts=4, gph=8, n_leaves=2, n_spines=2)
+    ref = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST) for i in range(w.batch)]
+    t_end = max(o.completion_times().max() for o in ref)
+    sim = B.Sim.from_workload(w, path=CTA, decompose=False)
+    for k, frac in enumerate((0.2, 0.6, 1.2)):
+        sim.run(until=frac * t_end)
+        assert (sim.counters()["resumed_units"] > 0) == (k > 0)
+        for i in range(w.batch):
+            o = oracle_build(w.desc, w.instances[i])
+            o.run(mode=orc.MODE_FAST, until=frac * t_end)
+            assert np.array_equal(sim.completion_times(i), o.completion_times(), equal_nan=True), (frac, i)
+            assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+    sim.close()
+    sim = B.Sim.from_workload(W.cfg3(batch=5), path=CTA)
+    sim.run()
+    assert all(sim.path_of(i) == "cta" for i in range(5))
+    sim.close()
+
+
 def test_run_until_resumes_a_multi_cta_cluster():
     """Parking on the cluster path with several CTAs per unit (replicated shares, debit pre-aggregation): 4032
     concurrent flows per instance, stopped twice on the way."""
