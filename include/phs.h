@@ -13,6 +13,15 @@
  *   phs_run                  L165 max-min fair allocation by iterative water-filling; L128 piecewise-constant
  *                                  throughput between events; L308 flows reach their fair share at once
  *   phs_get_completion_times L104 "computes the completion time of each flow"
+ *   phs_get_bottlenecks, phs_get_event_log   L165 "the simulator identifies the bottleneck link" (per flow: the link
+ *                                  that froze it in its last solve; per event: iterations and first bottleneck)
+ *   phs_get_collective_times L104 the collective completes when its last flow does
+ *   phs_set_link_capacities*, phs_get_paths, phs_get_preds, phs_get_flow_table   L98 port bandwidth, routing; L104 the
+ *                                  flow patterns of the collectives, as tables for integer parity
+ *   phs_run_until, phs_update_flow_start, phs_rollback, phs_gc   L124-130, L167 (time rollback, advancing up to a time)
+ *   phs_enable_history / phs_get_flow_history   L128, L167 (piecewise-constant throughput, a few numbers per change)
+ *   phs_add_spans            L84 / L94 / L106 / L206 (compute spans in the event DAG)
+ *   phs_create_topology_graph, phs_set_devices   L98 (topology configuration as input); SURVEY.md 8(e)
  *
  * Ownership: the caller owns every array it passes; the library copies inputs before returning.  Outputs go
  * to caller-provided buffers.  Ids are dense and assigned in call order: flow ids per instance start at 0, a

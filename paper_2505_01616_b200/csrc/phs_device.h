@@ -1,5 +1,5 @@
-// phs_device.h -- kernel-side table of device pointers and the launch entry points (implemented in
-// phs_kernels.cu, called from phs_api.cu).
+// phs_device.h -- kernel-side table of device pointers and the launch entry points of the four kernel paths
+// (phs_kernels.cu, phs_cluster.cu, phs_window.cu, phs_grid.cu), called from phs_schedule.cu.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -75,9 +75,12 @@ struct CtaLaunch {
 cudaError_t launch_cta_path(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &cfg,
                             cudaStream_t stream);
 
-// Cluster path: one thread-block cluster (up to 16 CTAs, hardware cluster barrier) per large instance; link state
-// in global memory (L2-resident), flow slots in CTA-private partitions of a global slot array.  Clusters pull
-// instance indices from list[0..n) through *ticket; the cluster with rank k in the grid uses scratch region k.
+// Cluster path (phs_cluster.cu): one thread-block cluster (1-16 CTAs, hardware cluster barrier) per unit that does not
+// fit one SM.  All dynamic state stays on chip: link l is owned by CTA (l mod cluster size) and lives in the owner's
+// shared memory, reached by the others through distributed shared memory; every CTA owns private flow slots in its own
+// shared memory (only the cold slot fields spill to `base`, a CTA-private global partition, when shared memory is
+// short).  Clusters pull unit indices from list[0..n) through *ticket; the cluster with rank k in the grid uses spill
+// region k.
 struct ClusterScratch {
   unsigned char *base;  // global spill area of the cold slot fields (n_regions * region_bytes), unused if cold_smem
   size_t region_bytes;
