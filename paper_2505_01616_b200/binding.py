@@ -459,9 +459,9 @@ class Sim:
                     same = False
                     break
         if same and count > 1:
+            nb, st = W.batched_sizes(w, first, count)        # host arrays [n_ops][count]
             for k, op0 in enumerate(insts[0].ops):
-                phs_add_collective_batch(sim.h, op0.kind, op0.ranks, [x.ops[k].nbytes for x in insts],
-                                         [x.ops[k].start for x in insts], op0.after)
+                phs_add_collective_batch(sim.h, op0.kind, op0.ranks, nb[k], st[k], op0.after)
         else:
             for i, inst in enumerate(insts):
                 W.apply(inst,

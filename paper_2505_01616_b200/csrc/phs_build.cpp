@@ -328,11 +328,15 @@ void chain_after(Instance &inst, const Collective &a, int32_t rho) {
 
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t N,
                              double bytes, double start, const int32_t *after, int32_t n_after,
-                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why) {
+                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why,
+                             bool checked) {
   auto bad = [&](const char *m) {
     if (why) *why = m;
     return PHS_EINVAL;
   };
+  // `checked`: the same kind / ranks / after lists were validated on another instance of the same topology with as many
+  // collectives (phs_add_collective_batch); only what depends on the instance is looked at again
+  if (checked) goto record;
   if (!ranks) return bad("ranks is null");
   if (kind < PHS_ALLREDUCE_RING || kind > PHS_ALLREDUCE_TREE) return bad("unknown collective kind");
   if (chunks < 1 || chunks > 65536) return bad("chunks must be in [1, 65536]");
@@ -357,6 +361,7 @@ phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, co
   if (n_after_flows < 0 || (n_after_flows > 0 && !after_flows)) return bad("bad after_flow_ids");
   for (int a = 0; a < n_after_flows; ++a)
     if (after_flows[a] < 0 || after_flows[a] >= inst.n_flows()) return bad("after_flow_ids must name earlier flows");
+record:
   const int steps = kind == PHS_ALLREDUCE_RING ? 2 * (N - 1) : kind == PHS_ALLTOALL ? 1 : N - 1;
   const int64_t nf = kind == PHS_ALLTOALL          ? (int64_t)N * (N - 1)
                      : kind == PHS_ALLREDUCE_TREE  ? (int64_t)chunks * 2 * (N - 1)

@@ -144,7 +144,8 @@ void expand_pending(const Fabric &fab, Instance &inst);
 // validates and records the collective; its flows appear with the next expand_pending.
 phs_status append_collective(const Fabric &fab, Instance &inst, int32_t kind, const int32_t *ranks, int32_t n_ranks,
                              double bytes, double start, const int32_t *after, int32_t n_after,
-                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why);
+                             const int64_t *after_flows, int32_t n_after_flows, int32_t chunks, std::string *why,
+                             bool checked = false);
 phs_status append_spans(const Fabric &fab, Instance &inst, int64_t n, const int32_t *gpu, const int32_t *lane,
                         const double *duration, const double *start, const int64_t *dep_off, const int64_t *dep_ids,
                         std::string *why);

@@ -243,7 +243,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
     const int64_t fb = sim->flow_base[i];
     int64_t flow_cursor = 0, log_cursor = 0;
     std::vector<int64_t> capq_inst((size_t)L);
-    std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L);
+    std::vector<int32_t> parent((size_t)L), uparent((size_t)L), link_loc((size_t)L), link_seen((size_t)L, 0);
     // capacities -> rate quanta (floor); every fair share must stay >= 1 quantum
     for (int l = 0; l < L; ++l) {
       const double cap_l = in.cap.empty() ? sim->fab->default_capacity(l) : in.cap[l];
@@ -366,6 +366,25 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
         if (chain_max_cta[c] > 0) ubound_cta[unit_of[in.colls[c].first_flow]] += chain_max_cta[c];
       }
     }
+    // which units hold flows of which collective (ascending per collective), and which flows belong to a collective at
+    // all: one pass over the instance, used by the density estimate of every unit below
+    std::vector<uint8_t> flow_in_coll((size_t)F, 0);
+    std::vector<int32_t> coll_units, coll_units_off(in.colls.size() + 1, 0);
+    {
+      std::vector<int32_t> seen_by((size_t)std::max(n_units, 1), -1);
+      for (size_t ci = 0; ci < in.colls.size(); ++ci) {
+        const Collective &co = in.colls[ci];
+        for (int32_t f = co.first_flow; f < co.first_flow + co.n_flows; ++f) {
+          flow_in_coll[(size_t)f] = 1;
+          if (seen_by[(size_t)unit_of[f]] != (int32_t)ci) {
+            seen_by[(size_t)unit_of[f]] = (int32_t)ci;
+            coll_units.push_back(unit_of[f]);
+          }
+        }
+        std::sort(coll_units.begin() + coll_units_off[ci], coll_units.end());
+        coll_units_off[ci + 1] = (int32_t)coll_units.size();
+      }
+    }
     if (n_units == 0) {  // an instance without flows is one empty unit
       n_units = 1;
       uflows.resize(1);
@@ -380,11 +399,16 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       if (n_units == 1) {
         links.resize((size_t)L);
         std::iota(links.begin(), links.end(), 0);
-      } else {
+      } else {  // every link once (stamp per link and unit), then ascending: far fewer entries than path hops
         for (int32_t f : fl)
-          for (uint32_t e = in.path_off[f]; e < in.path_off[f + 1]; ++e) links.push_back(in.path[e]);
+          for (uint32_t e = in.path_off[f]; e < in.path_off[f + 1]; ++e) {
+            const int32_t l = in.path[e];
+            if (link_seen[(size_t)l] != u + 1) {
+              link_seen[(size_t)l] = u + 1;
+              links.push_back(l);
+            }
+          }
         std::sort(links.begin(), links.end());
-        links.erase(std::unique(links.begin(), links.end()), links.end());
       }
       for (size_t k = 0; k < links.size(); ++k) link_loc[links[k]] = (int32_t)k;
       InstDesc d;
@@ -467,17 +491,13 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       if (lmin > 0.0 && !fl.empty()) {
         const double capmax = (double)capmax_q / 1048576.0;
         double span = 0.0;
-        std::vector<uint8_t> in_coll(fl.size(), 0);
         std::vector<double> end_of(in.colls.size(), 0.0);
         for (size_t ci = 0; ci < in.colls.size(); ++ci) {
           const Collective &co = in.colls[ci];
           if (co.n_flows == 0) continue;
-          bool here = false;  // an all-to-all may be split over several units (intra-host / inter-host links)
-          for (int32_t f = co.first_flow; f < co.first_flow + co.n_flows; ++f)
-            if (unit_of[f] == u) {
-              in_coll[(size_t)flow_loc[f]] = 1;
-              here = true;
-            }
+          // an all-to-all may be split over several units (intra-host / inter-host links)
+          const bool here = std::binary_search(coll_units.begin() + coll_units_off[ci],
+                                               coll_units.begin() + coll_units_off[ci + 1], (int32_t)u);
           double begin = co.start;
           for (int32_t a : co.after) begin = std::max(begin, end_of[(size_t)a]);
           const double chunk = co.bytes / (double)co.n_ranks;
@@ -485,7 +505,7 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
           if (here) span = std::max(span, end_of[ci]);
         }
         for (size_t k = 0; k < fl.size(); ++k)
-          if (!in_coll[k]) span = std::max(span, in.start[fl[k]] + in.lat[fl[k]] + in.bytes[fl[k]] / capmax);
+          if (!flow_in_coll[(size_t)fl[k]]) span = std::max(span, in.start[fl[k]] + in.lat[fl[k]] + in.bytes[fl[k]] / capmax);
         density = std::isinf(lmin) ? std::numeric_limits<double>::infinity()
                                    : 2.0 * (double)fl.size() * lmin / std::max(span, 1e-300);
       }

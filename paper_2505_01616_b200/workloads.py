@@ -152,6 +152,21 @@ def _loguniform(rng, lo, hi, size=None):
     return np.floor(np.exp(rng.uniform(np.log(lo), np.log(hi), size)))
 
 
+def batched_sizes(w, first, count):
+    """For a workload whose instances have the same collectives (uniform_ops): the per-instance sizes and start times of
+    collective k as host arrays nbytes[k][count], start[k][count] -- the form phs_add_collective_batch takes.  Built
+    once per (first, count) and kept on the workload (input preparation, like the generator itself)."""
+    cache = w.__dict__.setdefault("_batched", {})
+    if (first, count) not in cache:
+        insts = w.instances[first:first + count]
+        n_ops = len(insts[0].ops)
+        nb = np.array([[op.nbytes for op in x.ops] for x in insts], np.float64).T.copy()
+        st = np.array([[op.start for op in x.ops] for x in insts], np.float64).T.copy()
+        assert nb.shape == (n_ops, count)
+        cache[(first, count)] = (nb, st)
+    return cache[(first, count)]
+
+
 def apply(inst: Instance, add_collective, add_flows, add_spans=None):
     """Replay an instance's ops through callables with the signatures
     add_collective(kind, ranks, nbytes, start, after[, chunks[, after_flows]]) -> id ;
