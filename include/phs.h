@@ -317,6 +317,9 @@ phs_status phs_get_event_log(const phs_sim *sim, int32_t instance, phs_event *ou
  * preds as CSR. */
 phs_status phs_num_path_entries(const phs_sim *sim, int32_t instance, int64_t *out);
 phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *links, int64_t cap);
+/* The transpose, link -> flow incidence (PAPER.md L98 routing): off[n_links + 1], flows[cap] with
+ * cap >= phs_num_path_entries: per link the flows whose path crosses it, ascending flow id. */
+phs_status phs_get_link_flows(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *flows, int64_t cap);
 phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *preds, int64_t cap,
                          int64_t *n_entries);
 phs_status phs_get_flow_table(const phs_sim *sim, int32_t instance, int32_t *src, int32_t *dst, double *bytes,

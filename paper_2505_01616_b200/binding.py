@@ -47,7 +47,7 @@ SYMBOLS = ["phs_create_topology", "phs_create_topology_graph", "phs_destroy", "p
            "phs_finalize", "phs_run", "phs_run_until", "phs_run_static", "phs_num_flows", "phs_total_flows",
            "phs_num_collectives", "phs_get_completion_times", "phs_get_bottlenecks",
            "phs_get_all_completion_times", "phs_get_all_bottlenecks", "phs_get_collective_times",
-           "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_preds", "phs_get_flow_table",
+           "phs_get_event_log", "phs_num_path_entries", "phs_get_paths", "phs_get_link_flows", "phs_get_preds", "phs_get_flow_table",
            "phs_get_counters", "phs_instance_path", "phs_last_error"]
 
 _lib = None
@@ -369,6 +369,15 @@ def phs_get_paths(h, instance):
     return off, links
 
 
+def phs_get_link_flows(h, instance):
+    n = C.c_int64()
+    _chk(lib().phs_num_path_entries(h, C.c_int32(instance), C.byref(n)), "phs_num_path_entries")
+    off = np.zeros(phs_num_links(h) + 1, np.int64)
+    flows = np.zeros(n.value, np.int32)
+    _chk(lib().phs_get_link_flows(h, C.c_int32(instance), _p(off), _p(flows), C.c_int64(n.value)), "phs_get_link_flows")
+    return off, flows
+
+
 def phs_get_preds(h, instance):
     n = C.c_int64()
     _chk(lib().phs_get_preds(h, C.c_int32(instance), None, None, C.c_int64(0), C.byref(n)), "phs_get_preds")
@@ -504,6 +513,9 @@ class Sim:
 
     def paths(self, i):
         return phs_get_paths(self.h, i)
+
+    def link_flows(self, i):
+        return phs_get_link_flows(self.h, i)
 
     def preds(self, i):
         return phs_get_preds(self.h, i)

@@ -404,6 +404,25 @@ phs_status phs_get_paths(const phs_sim *sim, int32_t instance, int64_t *off, int
   PHS_API_END
 }
 
+// a3: the transpose of the flow -> link incidence (lf_off[n_links + 1], lf[sum of path lengths]):
+// per link the flows that cross it, ascending flow id.  Counting sort over the path entries.
+phs_status phs_get_link_flows(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *flows, int64_t cap) {
+  PHS_API_BEGIN
+  phs_status st = check_instance(sim, instance, false);
+  if (st != PHS_OK) return st;
+  const Instance &in = expanded(sim, instance);
+  if (!off || !flows || cap < (int64_t)in.path.size()) return fail(PHS_EINVAL, "output too small");
+  const int32_t L = sim->fab->n_links();
+  std::fill(off, off + L + 1, (int64_t)0);
+  for (int32_t l : in.path) off[l + 1]++;
+  for (int32_t l = 0; l < L; ++l) off[l + 1] += off[l];
+  std::vector<int64_t> cur(off, off + L);
+  for (size_t f = 0; f + 1 < in.path_off.size(); ++f)
+    for (uint32_t e = in.path_off[f]; e < in.path_off[f + 1]; ++e) flows[cur[(size_t)in.path[e]]++] = (int32_t)f;
+  return PHS_OK;
+  PHS_API_END
+}
+
 phs_status phs_get_preds(const phs_sim *sim, int32_t instance, int64_t *off, int32_t *preds, int64_t cap,
                          int64_t *n_entries) {
   PHS_API_BEGIN

@@ -34,6 +34,12 @@ def _compare_tables(w, first=0, count=None):
         off, links = sim.paths(i)
         ooff, olinks = o.paths()
         assert np.array_equal(off, ooff) and np.array_equal(links, olinks)
+        # a3, the transpose (link -> flows, ascending flow id), against the transpose of the ORACLE's paths
+        loff, lflows = sim.link_flows(i)
+        flow_of_entry = np.repeat(np.arange(len(ooff) - 1, dtype=np.int32), np.diff(ooff))
+        order = np.argsort(olinks, kind="stable")
+        assert np.array_equal(lflows, flow_of_entry[order])
+        assert np.array_equal(loff, np.concatenate([[0], np.cumsum(np.bincount(olinks, minlength=len(loff) - 1))]))
         poff, pr = sim.preds(i)
         opoff, opr = o.preds()
         assert np.array_equal(poff, opoff) and np.array_equal(pr, opr)
