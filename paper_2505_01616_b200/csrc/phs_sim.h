@@ -244,6 +244,7 @@ struct phs_sim {
 
   // ---- device tables
   phs::DevBuf<unsigned char> d_arena;  // one allocation for every table phs_finalize places (the buffers below are views)
+  phs::DevBuf<unsigned char> d_flowtab;  // the per-flow tables (rec, pc0, fmap): allocated before the build, filled group by group
   phs::DevBuf<phs::InstDesc> d_desc;
   phs::DevBuf<phs::FlowRec> d_rec;
   phs::DevBuf<int32_t> d_succ, d_pc0, d_pred_cnt, d_bneck, d_order, d_coll_n, d_linkid;
