@@ -95,7 +95,9 @@ __host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool ag
   if (o_agg) *o_agg = o;
   o += agg ? up16((size_t)L * 16) : 0;
   if (o_repl) *o_repl = o;
-  o += repl ? up16((size_t)L * 22) : 0;  // sh_loc[L], sh0_loc[L] (8 each), chg_loc[L] (4), comp_loc[L] (2)
+  // crmin[L] (8, incremental re-solve: with replicas and pre-aggregation, without the log), sh_loc[L], sh0_loc[L] (8 each),
+  // chg_loc[L] (4), comp_loc[L] (2)
+  o += repl ? up16((size_t)L * 22 + ((agg && !log) ? (size_t)L * 8 : 0)) : 0;
   if (o_hot) *o_hot = o;
   o += up16((size_t)Sc * kSlotHotBytes);
   if (o_cold) *o_cold = o;
@@ -156,7 +158,15 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   // REPL: every CTA keeps its own copy of the links' current fair shares, so that voting reads local shared
   // memory; owners broadcast the shares they recompute after debits, stale first-round shares are refreshed by the
   // flows that need them
-  long long *sh_loc = (long long *)(smem_raw + o_repl);  // [L] share in the current round
+  // INC, incremental re-solve: an event that only removes flows leaves untouched every flow whose rate
+  // is below the smallest rate among the removed ones -- the one-bottleneck-per-iteration algorithm freezes links in
+  // ascending (share, id) order, and its iterations before the removed flow's own bottleneck do not see the removal.
+  // Per component, crmin = that smallest rate (0 when a flow was added: everything is re-solved); link capacities
+  // left after ALL frozen flows (caprem) persist from solve to solve, the flows to re-solve credit their rates back.
+  const bool INCS = REPL && AGG && !LOG;            // the layout has crmin[]
+  const bool INC = INCS && SC.incremental != 0;
+  long long *crmin = (long long *)(smem_raw + o_repl);  // [L] per component (representative link), replicated per CTA
+  long long *sh_loc = crmin + (INCS ? L : 0);             // [L] share in the current round
   long long *sh0_loc = sh_loc + L;                        // [L] share at the start of a solve
   int *chg_loc = (int *)(sh0_loc + L);                    // [L] solve id of the last change of the link's flow count
   unsigned short *comp_loc = (unsigned short *)(chg_loc + L);  // [L] static component of every link
@@ -240,13 +250,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       a.share0 = 0; a.cap = l < Li ? capq[l] : 0; a.n0 = 0; a.chg = 0; a.beat = 0; a.solve = 0;
       la[li] = a;
       LinkB b;
-      b.caprem = 0; b.sharew = 0; b.nw = 0; b.deb = 0; b.wsolve = 0; b.comp = l < Li ? lcomp[l] : 0;
+      b.caprem = INC ? a.cap : 0; b.sharew = 0; b.nw = 0; b.deb = 0; b.wsolve = 0; b.comp = l < Li ? lcomp[l] : 0;
       lb[li] = b;
       if (LOG) won[li] = 0;
     }
     for (int l = tid; l < L; l += NT) {
       beatf[l] = 0;
       csolve[l] = 0;
+      if (INCS) crmin[l] = LLONG_MAX;
       if (REPL) {
         sh_loc[l] = 0;
         sh0_loc[l] = 0;
@@ -347,11 +358,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         LinkA *a = LA(l);
         atomicAdd(&a->n0, delta);
         a->chg = solve;
-        if (REPL)
+        if (REPL && !INC)
           for (int r = 0; r < CS; ++r) cluster.map_shared_rank(chg_loc, (unsigned)r)[l] = solve;
       };
       auto mark_comp = [&](int c) {  // the component must be re-solved: tell every CTA
         for (int r = 0; r < CS; ++r) cluster.map_shared_rank(csolve, (unsigned)r)[c] = solve;
+      };
+      auto limit_comp = [&](int c, long long rq) {  // INC: flows of component c with a rate >= rq must be re-solved
+        for (int r = 0; r < CS; ++r) atomicMin(cluster.map_shared_rank(crmin, (unsigned)r) + c, rq);
       };
       auto activate = [&](int slot) {
 #pragma unroll
@@ -361,6 +375,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           touch_link(l, 1);
         }
         mark_comp(S.comp[slot]);
+        if (INC) limit_comp(S.comp[slot], 0);  // a flow was added: the whole component
         S.rq[slot] = -1;
         S.bn[slot] = -1;
         S.tc[slot] = kInf;
@@ -416,8 +431,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           const int l = S.path[s * kMaxHops + h];
           if (l == kNoLink) break;
           touch_link(l, -1);
+          if (INC) add64_2x32(&LB(l)->caprem, S.rq[s]);  // the flow's rate goes back to its links
         }
         mark_comp(S.comp[s]);
+        if (INC) limit_comp(S.comp[s], S.rq[s]);
         S.bn[s] = -3;
         S.tc[s] = kInf;
         S.freeq[atomicAdd(&ctl[M_QTAIL], 1) % Sc] = s;
@@ -512,13 +529,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       max_pending = max(max_pending, nPend);
 
       // ======== P: working capacities of the own links that will be re-solved (first debited after barrier 1)
+      if (!INC)
       for (int li = tid; li < Lc; li += NT) {
         if (LOG || csolve[lb[li].comp] == solve) {
           lb[li].caprem = la[li].cap;
           lb[li].nw = la[li].n0;
         }
       }
-      if (REPL) {
+      if (REPL && !INC) {
         for (int l = tid; l < L; l += NT)
           if (LOG || csolve[comp_loc[l]] == solve) sh_loc[l] = sh0_loc[l];
         __syncthreads();
@@ -633,14 +651,29 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         for (int s = tid; s < hi; s += NT) {
           const int bn0 = S.bn[s];
           if (bn0 == -3) continue;
-          const bool in = bn0 != -2 && (LOG || csolve[S.comp[s]] == solve);
+          bool in = bn0 != -2 && (LOG || csolve[S.comp[s]] == solve);
+          if (INC && in) {  // rates below the smallest removed rate stand (never solved: rq = -1, always in)
+            const long long rq = S.rq[s];
+            in = rq < 0 || rq >= crmin[S.comp[s]];
+          }
           if (!in) {
             mymin = dmin(mymin, S.tc[s]);
             continue;
           }
           S.bn[s] = -1;
-          const longlong2 v = vote(s, true);
           wl[atomicAdd(&ctl[nwl_idx], 1)] = (unsigned short)s;
+          if (INC) {  // the flow's rate goes back to its links, which count it as unfrozen again (pre-summed per CTA)
+            const long long rq = S.rq[s];
+#pragma unroll
+            for (int h = 0; h < kMaxHops; ++h) {
+              const int l = S.path[s * kMaxHops + h];
+              if (l == kNoLink) break;
+              if (atomicAdd(&dn_loc[l], 1) == 0) touched[atomicAdd(&ctl[M_NTOUCH], 1)] = l;
+              if (rq > 0) add64_2x32(&dcap_loc[l], rq);
+            }
+            continue;  // the vote follows once the owners have the links' new shares
+          }
+          const longlong2 v = vote(s, true);
           if (LOG && (v.x < bk || (v.x == bk && (int)v.y < bl))) {
             bk = v.x;
             bl = (int)v.y;
@@ -671,6 +704,40 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
             comb0->f[crank].fb_id = bl;
           }
         }
+      }
+      if (INC) {
+        // ---- C: credits to the owners (stamp deb = g marks the links whose share must be computed)
+        __syncthreads();
+        {
+          const int nt = ctl[M_NTOUCH];
+          for (int i = tid; i < nt; i += NT) {
+            const int l = touched[i];
+            LinkB *bp = LB(l);
+            if (dcap_loc[l] != 0) add64_2x32(&bp->caprem, dcap_loc[l]);
+            atomicAdd(&bp->nw, dn_loc[l]);
+            bp->deb = g;
+            dcap_loc[l] = 0;
+            dn_loc[l] = 0;
+          }
+        }
+        for (int c = tid; c < L; c += NT)  // this CTA has read its limits: ready for the next event
+          if (csolve[c] == solve) crmin[c] = LLONG_MAX;
+        __syncthreads();
+        if (tid == 0) ctl[M_NTOUCH] = 0;
+        cluster.sync();  // ---------------------------------------------------------------- cluster barrier C
+        // ---- R0: owners compute the share of their credited links and tell every CTA
+        for (int li = tid; li < Lc; li += NT) {
+          if (lb[li].deb != g) continue;
+          const int nw = lb[li].nw;
+          if (nw <= 0) continue;
+          const long long shv = fair_share(lb[li].caprem, nw);
+          const int l = li * CS + crank;
+          for (int r = 0; r < CS; ++r) cluster.map_shared_rank(sh_loc, (unsigned)r)[l] = shv;
+        }
+        cluster.sync();  // ---------------------------------------------------------------- cluster barrier R0
+        ++g;
+        const int nv = ctl[nwl_idx];
+        for (int i = tid; i < nv; i += NT) vote(wl[i], false);
       }
       for (;;) {
         PHS_TICK(3)

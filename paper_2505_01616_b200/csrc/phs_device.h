@@ -88,6 +88,8 @@ struct ClusterScratch {
   int aggregate;        // 1: a CTA pre-sums its debits per link in shared memory (16 bytes per link and CTA)
   int cold_smem;        // 1: the cold slot fields live in shared memory too
   int replicate;        // 1: every CTA keeps a copy of the links' current fair shares (22 bytes per link and CTA)
+  int incremental;      // 1 (needs aggregate and replicate, no event log): an event that only removes flows re-solves
+                        // just the flows whose rate is at least the smallest removed rate (phs_cluster.cu, INC)
   // phs_run_until: parking areas of units that stopped at t_stop (per unit: ClusterParkRegs, then per CTA a copy
   // of its shared memory, control words and cold slot fields), or nullptr
   unsigned char *park;

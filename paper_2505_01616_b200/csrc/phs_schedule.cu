@@ -936,6 +936,8 @@ retry:
   sc.aggregate = agg ? 1 : 0;
   sc.cold_smem = cold ? 1 : 0;
   sc.replicate = repl ? 1 : 0;
+  sc.incremental = (repl && agg && !log) ? 1 : 0;
+  if (const char *ev = getenv("PHS_CLUSTER_INC")) sc.incremental = (atoi(ev) != 0 && repl && agg && !log) ? 1 : 0;  // tuning
   // phs_run_until: parking areas, one per cluster-path unit, valid for one launch configuration
   sc.park = nullptr;
   sc.park_unit_stride = sc.park_cta_stride = 0;
