@@ -28,6 +28,7 @@ namespace {
 constexpr int NT = kClusterThreads;
 constexpr unsigned short kNoLink = 0xffff;
 constexpr int kMaxCS = 16;
+constexpr int kRminShift = 30;  // capacities are below 2^42 byte/s = 2^62 quanta (phs_set_link_capacities): 32 bits left
 
 struct LinkA {  // 32 bytes: what a flow reads when it votes in the first round
   long long share0;  // floor(cap / n0), valid unless chg == current solve id
@@ -95,9 +96,9 @@ __host__ __device__ inline size_t smem_layout(int L, int CS, int64_t Sc, bool ag
   if (o_agg) *o_agg = o;
   o += agg ? up16((size_t)L * 16) : 0;
   if (o_repl) *o_repl = o;
-  // crmin[L] (8, incremental re-solve: with replicas and pre-aggregation, without the log), sh_loc[L], sh0_loc[L] (8 each),
-  // chg_loc[L] (4), comp_loc[L] (2)
-  o += repl ? up16((size_t)L * 22 + ((agg && !log) ? (size_t)L * 8 : 0)) : 0;
+  // sh_loc[L], sh0_loc[L] (8 each), chg_loc[L] (4), comp_loc[L] (2); with pre-aggregation and without the log (incremental
+  // re-solve) also crmin[L] (4)
+  o += repl ? up16(up16((size_t)L * 22) + ((agg && !log) ? (size_t)L * 4 : 0)) : 0;
   if (o_hot) *o_hot = o;
   o += up16((size_t)Sc * kSlotHotBytes);
   if (o_cold) *o_cold = o;
@@ -165,11 +166,14 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   // left after ALL frozen flows (caprem) persist from solve to solve, the flows to re-solve credit their rates back.
   const bool INCS = REPL && AGG && !LOG;            // the layout has crmin[]
   const bool INC = INCS && SC.incremental != 0;
-  long long *crmin = (long long *)(smem_raw + o_repl);  // [L] per component (representative link), replicated per CTA
-  long long *sh_loc = crmin + (INCS ? L : 0);             // [L] share in the current round
+  long long *sh_loc = (long long *)(smem_raw + o_repl);  // [L] share in the current round
   long long *sh0_loc = sh_loc + L;                        // [L] share at the start of a solve
   int *chg_loc = (int *)(sh0_loc + L);                    // [L] solve id of the last change of the link's flow count
   unsigned short *comp_loc = (unsigned short *)(chg_loc + L);  // [L] static component of every link
+  // [L] per component (representative link), replicated per CTA: the smallest removed rate of the event, truncated to
+  // rate >> kRminShift so that it is one 32-bit word (a remote 32-bit min needs no answer; truncation only makes the cut
+  // more careful: (rate >> k) < (r_min >> k) implies rate < r_min)
+  unsigned *crmin = (unsigned *)(smem_raw + o_repl + up16((size_t)L * 22));
   LinkA *la = (LinkA *)smem_raw;
   LinkB *lb = (LinkB *)(smem_raw + o_lb);
   int *won = (int *)(smem_raw + o_won);
@@ -257,7 +261,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     for (int l = tid; l < L; l += NT) {
       beatf[l] = 0;
       csolve[l] = 0;
-      if (INCS) crmin[l] = LLONG_MAX;
+      if (INCS) crmin[l] = 0xffffffffu;
       if (REPL) {
         sh_loc[l] = 0;
         sh0_loc[l] = 0;
@@ -365,7 +369,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         for (int r = 0; r < CS; ++r) cluster.map_shared_rank(csolve, (unsigned)r)[c] = solve;
       };
       auto limit_comp = [&](int c, long long rq) {  // INC: flows of component c with a rate >= rq must be re-solved
-        for (int r = 0; r < CS; ++r) atomicMin(cluster.map_shared_rank(crmin, (unsigned)r) + c, rq);
+        const unsigned key = (unsigned)(rq >> kRminShift);
+        for (int r = 0; r < CS; ++r) atomicMin(cluster.map_shared_rank(crmin, (unsigned)r) + c, key);
       };
       auto activate = [&](int slot) {
 #pragma unroll
@@ -654,7 +659,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           bool in = bn0 != -2 && (LOG || csolve[S.comp[s]] == solve);
           if (INC && in) {  // rates below the smallest removed rate stand (never solved: rq = -1, always in)
             const long long rq = S.rq[s];
-            in = rq < 0 || rq >= crmin[S.comp[s]];
+            in = rq < 0 || (unsigned)(rq >> kRminShift) >= crmin[S.comp[s]];
           }
           if (!in) {
             mymin = dmin(mymin, S.tc[s]);
@@ -721,7 +726,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           }
         }
         for (int c = tid; c < L; c += NT)  // this CTA has read its limits: ready for the next event
-          if (csolve[c] == solve) crmin[c] = LLONG_MAX;
+          if (csolve[c] == solve) crmin[c] = 0xffffffffu;
         __syncthreads();
         if (tid == 0) ctl[M_NTOUCH] = 0;
         cluster.sync();  // ---------------------------------------------------------------- cluster barrier C
