@@ -270,7 +270,7 @@ phs_status phs_run_until(phs_sim *sim, double t_stop_s, void *cuda_stream);
  *            the phs_get_* calls work after it as after phs_run.
  *   limits   PHS_ERANGE (nothing ran; the message names the sizes) if the handle has more than PHS_STATIC_MAX_UNITS
  *            simulation units, or if its largest unit needs more than PHS_STATIC_SCRATCH_BYTES - 4 * PHS_STATIC_MAX_UNITS
- *            bytes of state: 40 bytes per flow + 56 per link + 1 KiB, i.e. about 200,000 flows in one unit.
+ *            bytes of state: 40 bytes per flow + 64 per link + 1 KiB, i.e. about 200,000 flows in one unit.
  *   sharing  every call on a device uses the one array, which keeps the contents of the last call; the kernel
  *            initialises all of it that it reads, so nothing carries over.  Two calls that overlap on one GPU (two
  *            streams, two threads, two handles) race: serialise them.

@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 
 #include <climits>
+#include <cstdlib>
 
 #include "phs_device.h"
 #include "phs_devutil.cuh"
@@ -46,12 +47,16 @@ __device__ __forceinline__ double block_min(double v, double *red) {
 }  // namespace
 
 size_t grid_scratch_bytes(int64_t n_flows, int n_links) {
-  const size_t per_flow = 4 * 8 + 2 * 4, per_link = 4 * 8 + 6 * 4;
+  const size_t per_flow = 4 * 8 + 2 * 4, per_link = 5 * 8 + 6 * 4;
   return ((size_t)n_flows * per_flow + 255) / 256 * 256 + ((size_t)n_links * per_link + 255) / 256 * 256 + 1024;
 }
 
 // HIST: record the throughput history.  The event log is not written on this path.
-template <bool HIST>
+// INC: incremental re-solve (the same rule as in phs_cluster.cu): an event that only removes flows
+// leaves every flow whose rate is below the smallest removed rate of its component alone.  l_caprem then persists
+// from solve to solve (capacity left after ALL frozen flows), a completing flow credits its rate back in phase X, the
+// flows at or above the limit credit theirs in a pass of their own and are solved by the rounds >= 2 code.
+template <bool HIST, bool INC>
 __global__ void __launch_bounds__(kGridThreads, 1)
     phs_grid_kernel(DevTables T, const int32_t *__restrict__ list, int n_list, unsigned char *scratch, int64_t max_flows,
                     int max_links) {
@@ -83,6 +88,7 @@ __global__ void __launch_bounds__(kGridThreads, 1)
   int *l_nw = (int *)take((size_t)max_links * 4);
   int *l_deb = (int *)take((size_t)max_links * 4);
   int *c_solve = (int *)take((size_t)max_links * 4);       // per component (dense ids < links)
+  unsigned long long *c_rmin = (unsigned long long *)take((size_t)max_links * 8);  // INC: smallest removed rate
   unsigned long long *gmin = (unsigned long long *)take(4 * 8);
   int *ctl = (int *)take(G_NCTL * 4);
 
@@ -106,6 +112,11 @@ __global__ void __launch_bounds__(kGridThreads, 1)
       l_beat[l] = 0;
       l_deb[l] = 0;
       c_solve[l] = 0;
+      if (INC) {
+        l_caprem[l] = capq[l];
+        l_nw[l] = 0;
+        c_rmin[l] = ~0ull;
+      }
     }
     if (gtid < G_NCTL) ctl[gtid] = 0;
     if (gtid < 3) gmin[gtid] = 0xffffffffffffffffull;
@@ -146,6 +157,7 @@ __global__ void __launch_bounds__(kGridThreads, 1)
         l_chg[l] = solve;
       }
       c_solve[r.comp] = solve;
+      if (INC) atomicMin(&c_rmin[r.comp], 0ull);  // a flow was added: the whole component is re-solved
       f_rq[f] = -1;
       f_tc[f] = kInf;
       f_st[f] = kUnfrozen;
@@ -177,13 +189,16 @@ __global__ void __launch_bounds__(kGridThreads, 1)
           T.t_done[out] = t_next;
           T.bneck[out] = linkid[st];
 #pragma unroll
+          const long long rq_done = INC ? f_rq[f] : 0;
           for (int h = 0; h < kMaxHops; ++h) {
             const int l = r.path[h];
             if (l < 0) continue;
             atomicSub(&l_n0[l], 1);
             l_chg[l] = solve;
+            if (INC) atomicAdd((unsigned long long *)&l_caprem[l], (unsigned long long)rq_done);  // its rate goes back
           }
           c_solve[r.comp] = solve;
+          if (INC) atomicMin(&c_rmin[r.comp], (unsigned long long)rq_done);
           f_tc[f] = kInf;
           f_st[f] = kDone;
           --d_act;
@@ -236,6 +251,36 @@ __global__ void __launch_bounds__(kGridThreads, 1)
         }
       };
       int rounds = 0;
+      if (INC) {  // ---- C: the flows to re-solve give their rates back and count as unfrozen again
+        ++g;
+        if (gtid == 0) {  // the credit pass takes part in the rotation of the flag / minimum words like a round
+          ctl[G_LEFT0 + (g + 1) % 3] = 0;
+          gmin[(g + 1) % 3] = 0xffffffffffffffffull;
+        }
+        for (long long ff = gtid; ff < F; ff += GT) {
+          const int f = (int)ff;
+          const int st = __ldcg(&f_st[f]);
+          if (st == kWaiting || st == kDone || st == kPending) continue;
+          const FlowRec r = rec[f];
+          if (__ldcg(&c_solve[r.comp]) != solve) continue;  // component untouched by this event: rates stand
+          const long long rq = f_rq[f];
+          if (rq >= 0 && (unsigned long long)rq < __ldcg(&c_rmin[r.comp])) continue;  // below the limit: stands
+          f_st[f] = kUnfrozen;
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = r.path[h];
+            if (l < 0) continue;
+            if (rq > 0) atomicAdd((unsigned long long *)&l_caprem[l], (unsigned long long)rq);
+            atomicAdd(&l_nw[l], 1);
+            l_deb[l] = g;  // "debited" in this pass: the next vote computes the link's share from (caprem, nw)
+          }
+        }
+        __threadfence();
+        grid.sync();
+        for (long long l = gtid; l < Li; l += GT)  // every thread has read the limits: ready for the next event
+          if (c_solve[l] == solve) c_rmin[l] = ~0ull;
+        rounds = 1;  // the rounds below run as rounds >= 2: shares from the working state, every freeze debits
+      }
       for (;;) {
         ++g;
         ++rounds;
@@ -310,7 +355,7 @@ __global__ void __launch_bounds__(kGridThreads, 1)
               for (int h = 0; h < kMaxHops; ++h) {
                 const int l = r.path[h];
                 if (l < 0) continue;
-                if (__ldcg(&l_n0[l]) > 1) {
+                if (INC || __ldcg(&l_n0[l]) > 1) {  // INC: caprem persists, so every freeze is booked
                   atomicAdd((unsigned long long *)&l_caprem[l], (unsigned long long)(-rq));
                   atomicSub(&l_nw[l], 1);
                   l_deb[l] = g;
@@ -361,7 +406,7 @@ cudaError_t grid_max_ctas(int *n_ctas) {
   if (e != cudaSuccess) return e;
   e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (e != cudaSuccess) return e;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, phs_grid_kernel<false>, kGridThreads, 0);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, phs_grid_kernel<false, true>, kGridThreads, 0);
   if (e != cudaSuccess) return e;
   *n_ctas = sms * std::max(per, 0);
   return cudaSuccess;
@@ -371,7 +416,12 @@ cudaError_t launch_grid_path(const DevTables &t, const int32_t *list, int n, uns
                              int max_links, int n_ctas, cudaStream_t stream) {
   DevTables tt = t;
   void *args[] = {(void *)&tt, (void *)&list, (void *)&n, (void *)&scratch, (void *)&max_flows, (void *)&max_links};
-  const void *fn = t.hist ? (const void *)phs_grid_kernel<true> : (const void *)phs_grid_kernel<false>;
+  static const bool inc = [] {  // PHS_GRID_INC=0: from-scratch solves (tuning / comparison runs)
+    const char *ev = getenv("PHS_GRID_INC");
+    return !(ev && atoi(ev) == 0);
+  }();
+  const void *fn = inc ? (t.hist ? (const void *)phs_grid_kernel<true, true> : (const void *)phs_grid_kernel<false, true>)
+                       : (t.hist ? (const void *)phs_grid_kernel<true, false> : (const void *)phs_grid_kernel<false, false>);
   return cudaLaunchCooperativeKernel(fn, dim3((unsigned)n_ctas), dim3(kGridThreads), args, 0, stream);
 }
 

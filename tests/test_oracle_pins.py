@@ -312,6 +312,45 @@ def test_p4_random_instances_certificate(seed):
         assert fb == bneck[np.argmin(rate)] or rate[bneck == fb].min() == rate.min()
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_removing_flows_leaves_the_slower_part_of_the_allocation_alone(seed):
+    """The property the kernels' incremental re-solve rests on, checked on the ORACLE's from-scratch
+    solves: remove flows from an allocation; every remaining flow whose old rate is below the smallest removed rate
+    keeps its rate and its bottleneck, bit for bit.  (One-bottleneck-per-iteration filling picks links in ascending
+    (share, id) order and its iterations before a removed flow's own bottleneck do not see the removal.)  Equal
+    capacities in half of the cases: ties everywhere."""
+    rng = np.random.default_rng(100 + seed)
+    n_links = int(rng.integers(4, 40))
+    n_flows = int(rng.integers(5, 160))
+    cap = np.floor(rng.uniform(1e9, 4e11, n_links))
+    if seed % 2:
+        cap[:] = 50e9
+    lens = rng.integers(1, min(6, n_links) + 1, n_flows)
+    paths = [rng.choice(n_links, int(h), replace=False).astype(np.int32) for h in lens]
+
+    def solve(keep):
+        off = np.concatenate([[0], np.cumsum([len(paths[f]) for f in keep])])
+        pth = np.concatenate([paths[f] for f in keep]).astype(np.int32)
+        rate, bneck, _, _ = orc.maxmin(cap, off, pth, orc.MODE_FAST)
+        return dict(zip(keep, rate)), dict(zip(keep, bneck))
+
+    alive = list(range(n_flows))
+    rate, bneck = solve(alive)
+    unchanged_total = 0
+    while len(alive) > 2:
+        gone = [int(x) for x in rng.choice(alive, int(rng.integers(1, 4)), replace=False)]
+        r_min = min(rate[f] for f in gone)
+        alive = [f for f in alive if f not in gone]
+        new_rate, new_bneck = solve(alive)
+        for f in alive:
+            if rate[f] < r_min:
+                assert new_rate[f] == rate[f] and new_bneck[f] == bneck[f], (f, rate[f], r_min)
+                unchanged_total += 1
+            assert new_rate[f] >= rate[f] or rate[f] >= r_min          # nobody below the limit loses either
+        rate, bneck = new_rate, new_bneck
+    assert unchanged_total > 0 or n_flows < 8
+
+
 def test_p4_certificate_along_event_loop():
     # a contended mid-size run: shrunken cfg1 (DP rings share 2 uplinks per leaf) -- check EVERY recompute
     w = W.cfg1(batch=3, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
