@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
     S.succ1 = S.succ0 + Sc;
     S.freeq = S.succ1 + Sc;
   }
-  __shared__ Comb comb;  // only CTA 0's copy is used
+  __shared__ Comb comb;  // x / f.tmin / f.left: every CTA has the cluster's values; the rest: CTA 0's copy is used
   __shared__ double red[32];
   __shared__ long long red_key[32];
   __shared__ int red_id[32];
@@ -478,16 +478,19 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       }
       PHS_TICK(0)
       __syncthreads();
-      if (tid == 0) {  // publish this CTA's counts in CTA 0
+      if (warp == 0) {  // publish this CTA's counts: lane r writes them into CTA r's own table (no read trip later)
         CombX x;
         x.n_act = ctl[M_NACT]; x.n_pend = ctl[M_NPEND]; x.n_done = ctl[M_NDONE]; x.over = ctl[M_OVER];
         x.hi = ctl[M_HI]; x.ev_ncomp = ctl[M_EVC]; x.ev_nact = ctl[M_EVA]; x.pad = 0;
-        comb0->x[crank] = x;
-        ctl[M_EVC] = 0;
-        ctl[M_EVA] = 0;
-        if (ctl[M_QHEAD] > qtail) ctl[M_QHEAD] = qtail;
-        ctl[M_NWL0] = 0;
-        ctl[M_NWL1] = 0;
+        if (lane < CS) cluster.map_shared_rank(&comb, (unsigned)lane)->x[crank] = x;
+        __syncwarp();
+        if (lane == 0) {
+          ctl[M_EVC] = 0;
+          ctl[M_EVA] = 0;
+          if (ctl[M_QHEAD] > qtail) ctl[M_QHEAD] = qtail;
+          ctl[M_NWL0] = 0;
+          ctl[M_NWL1] = 0;
+        }
       }
       PHS_TICK(1)
       cluster.sync();  // ---------------------------------------------------------------- cluster barrier X
@@ -496,7 +499,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       if (warp == 0) {  // one warp per CTA sums the per-CTA counts and hands them to the CTA
         CombX x;
         x.n_act = x.n_pend = x.n_done = x.over = x.hi = x.ev_ncomp = x.ev_nact = 0;
-        if (lane < CS) x = comb0->x[lane];
+        if (lane < CS) x = comb.x[lane];
         const int a = __reduce_add_sync(0xffffffffu, x.n_act), b = __reduce_add_sync(0xffffffffu, x.n_pend);
         const int c = __reduce_add_sync(0xffffffffu, x.n_done), d = __reduce_add_sync(0xffffffffu, x.over);
         const int e = __reduce_max_sync(0xffffffffu, x.hi);
@@ -790,9 +793,10 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
         }
         if (warp == 0) {
           const double m = warp_min(lane < NT / 32 ? red[lane] : kInf);
-          if (lane == 0) {
-            comb0->f[crank].tmin = m;
-            comb0->f[crank].left = left ? 1 : 0;
+          if (lane < CS) {  // lane r tells CTA r
+            CombF *cf = &cluster.map_shared_rank(&comb, (unsigned)lane)->f[crank];
+            cf->tmin = m;
+            cf->left = left ? 1 : 0;
           }
         }
         PHS_TICK(5)
@@ -802,8 +806,8 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           double m = kInf;
           int lf = 0;
           if (lane < CS) {
-            m = comb0->f[lane].tmin;
-            lf = comb0->f[lane].left;
+            m = comb.f[lane].tmin;
+            lf = comb.f[lane].left;
           }
           m = warp_min(m);
           lf = __reduce_or_sync(0xffffffffu, lf);
