@@ -265,16 +265,16 @@ phs_status phs_add_collective_batch(phs_sim *sim, int32_t kind, const int32_t *r
   // the arguments shared by all instances (kind, ranks, after) fail on instance 0, before anything is added.  Only
   // the descriptor is recorded here: the flows are expanded per instance on the host threads of phs_finalize.
   std::string why;
-  for (int i = 0; i < sim->batch; ++i)  // the one thing that depends on the instance: its flow count so far
-    if (sim->inst[i].n_flows() != sim->inst[0].n_flows())
-      return fail(PHS_ESTATE, "batch add needs the same number of flows in every instance");
   phs_status st0 = append_collective(*sim->fab, sim->inst[0], kind, ranks, n_ranks, bytes[0], start ? start[0] : 0.0, after,
                                      n_after, nullptr, 0, 1, &why);
   if (st0 != PHS_OK) return fail(st0, why);
-  // the other instances record the same descriptor with their own size and start time
-  for (int i = 1; i < sim->batch; ++i)
-    append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0, after, n_after,
-                      nullptr, 0, 1, nullptr, true);
+  // the other instances record the same descriptor with their own size and start time; what depends on the instance
+  // (its flow count so far: the 2^31 limit) is still checked
+  for (int i = 1; i < sim->batch; ++i) {
+    phs_status sti = append_collective(*sim->fab, sim->inst[i], kind, ranks, n_ranks, bytes[i], start ? start[i] : 0.0,
+                                       after, n_after, nullptr, 0, 1, &why, true);
+    if (sti != PHS_OK) return fail(sti, why);
+  }
   if (out_id) *out_id = (int32_t)sim->inst[0].colls.size() - 1;
   return PHS_OK;
   PHS_API_END
