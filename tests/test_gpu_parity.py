@@ -607,6 +607,37 @@ def test_cta_path_lean_layout(monkeypatch, lean):
     sim.close()
 
 
+@pytest.mark.parametrize("inc", ["1", "0"])
+def test_incremental_resolve_with_flows_added_and_removed(monkeypatch, inc):
+    """The incremental re-solve of the cluster and grid paths where it has to be careful: uniform
+    all-to-alls (every flow of a step has the same rate: ties, many flows completing at one time), a second all-to-all
+    chained behind the first (flows are ADDED to a component that is being re-solved: the limit drops to 0) and raw
+    flows of random sizes that start in the middle of it -- against the oracle, and the same with the incremental
+    re-solve switched off."""
+    monkeypatch.setenv("PHS_CLUSTER_INC", inc)
+    monkeypatch.setenv("PHS_GRID_INC", inc)
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 8, 8, fabric_Bps=W.gbps(400.0), n_leaves=4, n_spines=2, uplinks_per_leaf_spine=2)
+    insts = []
+    for i in range(2):
+        rng = np.random.default_rng(70 + i)
+        n = 1500
+        src = rng.integers(0, 64, n).astype(np.int32)
+        dst = ((src + rng.integers(1, 64, n)) % 64).astype(np.int32)
+        ops = [W.Coll(W.ALLTOALL, np.arange(64, dtype=np.int32), 64 * 3e5),
+               W.Coll(W.ALLTOALL, np.arange(0, 64, 2, dtype=np.int32), 32 * 5e5, 0.0, (0,)),
+               W.RawFlows(src, dst, np.floor(rng.uniform(1e4, 2e6, n)), start=rng.uniform(0.0, 4e-4, n))]
+        insts.append(W.Instance(seed=i, ops=ops))
+    w = W.Workload("a2a_chain", d, 3, insts)
+    for path in (CLUSTER, GRID):
+        sim = B.Sim.from_workload(w, path=path, decompose=False)
+        sim.run()
+        for i in range(w.batch):
+            o = oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST, base_seed=w.base_seed)
+            assert_instance_matches(sim, i, o, check_log=False)
+        assert sim.path_of(0) == ("cluster" if path == CLUSTER else "grid")
+        sim.close()
+
+
 def test_run_until_resumes_a_multi_cta_cluster():
     """Parking on the cluster path with several CTAs per unit (replicated shares, debit pre-aggregation): 4032
     concurrent flows per instance, stopped twice on the way."""
