@@ -114,7 +114,8 @@ __device__ __forceinline__ void add64_2x32(long long *p, long long v) {  // work
   if (hi + carry) atomicAdd(w + 1, hi + carry);
 }
 
-enum { M_HI = 0, M_QHEAD, M_QTAIL, M_NACT, M_NPEND, M_NDONE, M_NWL0, M_NWL1, M_NTOUCH, M_OVER, M_EVC, M_EVA, M_NCTL };
+enum { M_HI = 0, M_QHEAD, M_QTAIL, M_NACT, M_NPEND, M_NDONE, M_NWL0, M_NWL1, M_NTOUCH, M_OVER, M_EVC, M_EVA, M_ADDED,
+       M_NCTL };
 
 }  // namespace
 
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   __shared__ long long red_key[32];
   __shared__ int red_id[32];
   __shared__ int ctl[M_NCTL];
-  __shared__ int bc[8];       // broadcast of the cluster-wide counts to the CTA
+  __shared__ int bc[10];      // broadcast of the cluster-wide counts to the CTA
   __shared__ double bc_t;     // ... and of the next event time
   Comb *comb0 = cluster.map_shared_rank(&comb, 0);
 
@@ -380,7 +381,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
           touch_link(l, 1);
         }
         mark_comp(S.comp[slot]);
-        if (INC) limit_comp(S.comp[slot], 0);  // a flow was added: the whole component
+        if (INC) ctl[M_ADDED] = 1;  // a flow was added: its links bound what stands (pass A after the X barrier)
         S.rq[slot] = -1;
         S.bn[slot] = -1;
         S.tc[slot] = kInf;
@@ -481,12 +482,13 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       if (warp == 0) {  // publish this CTA's counts: lane r writes them into CTA r's own table (no read trip later)
         CombX x;
         x.n_act = ctl[M_NACT]; x.n_pend = ctl[M_NPEND]; x.n_done = ctl[M_NDONE]; x.over = ctl[M_OVER];
-        x.hi = ctl[M_HI]; x.ev_ncomp = ctl[M_EVC]; x.ev_nact = ctl[M_EVA]; x.pad = 0;
+        x.hi = ctl[M_HI]; x.ev_ncomp = ctl[M_EVC]; x.ev_nact = ctl[M_EVA]; x.pad = ctl[M_ADDED];
         if (lane < CS) cluster.map_shared_rank(&comb, (unsigned)lane)->x[crank] = x;
         __syncwarp();
         if (lane == 0) {
           ctl[M_EVC] = 0;
           ctl[M_EVA] = 0;
+          ctl[M_ADDED] = 0;
           if (ctl[M_QHEAD] > qtail) ctl[M_QHEAD] = qtail;
           ctl[M_NWL0] = 0;
           ctl[M_NWL1] = 0;
@@ -498,14 +500,15 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       now = t_next;
       if (warp == 0) {  // one warp per CTA sums the per-CTA counts and hands them to the CTA
         CombX x;
-        x.n_act = x.n_pend = x.n_done = x.over = x.hi = x.ev_ncomp = x.ev_nact = 0;
+        x.n_act = x.n_pend = x.n_done = x.over = x.hi = x.ev_ncomp = x.ev_nact = x.pad = 0;
         if (lane < CS) x = comb.x[lane];
+        const int added = __reduce_or_sync(0xffffffffu, x.pad);
         const int a = __reduce_add_sync(0xffffffffu, x.n_act), b = __reduce_add_sync(0xffffffffu, x.n_pend);
         const int c = __reduce_add_sync(0xffffffffu, x.n_done), d = __reduce_add_sync(0xffffffffu, x.over);
         const int e = __reduce_max_sync(0xffffffffu, x.hi);
         const int nc = __reduce_add_sync(0xffffffffu, x.ev_ncomp), na = __reduce_add_sync(0xffffffffu, x.ev_nact);
         if (lane == 0) {
-          bc[0] = a; bc[1] = b; bc[2] = c; bc[3] = d; bc[4] = e; bc[5] = nc; bc[6] = na;
+          bc[0] = a; bc[1] = b; bc[2] = c; bc[3] = d; bc[4] = e; bc[5] = nc; bc[6] = na; bc[8] = added;
         }
       }
       __syncthreads();
@@ -536,6 +539,25 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 
+      if (INC && bc[8]) {
+        // ======== A: flows were ADDED in this event.  A link that carries an added flow has a share of at least
+        // floor(cap / n) -- n its flow count now -- all through the new solve, so the old solve's iterations below the
+        // smallest such share are picked again in the same order: every flow slower than that stands.
+        for (int s = tid; s < hi; s += NT) {
+          if (S.bn[s] != -1 || S.rq[s] >= 0) continue;  // ACTIVE and never solved = added
+          long long m = LLONG_MAX;
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = S.path[s * kMaxHops + h];
+            if (l == kNoLink) break;
+            const LinkA *ap = LA(l);
+            const long long sh = fair_share(ap->cap, ap->n0);
+            m = sh < m ? sh : m;
+          }
+          limit_comp(S.comp[s], m);
+        }
+        cluster.sync();  // ---------------------------------------------------------------- cluster barrier A
+      }
       // ======== P: working capacities of the own links that will be re-solved (first debited after barrier 1)
       if (!INC)
       for (int li = tid; li < Lc; li += NT) {

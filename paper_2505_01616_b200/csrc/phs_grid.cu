@@ -27,7 +27,7 @@ namespace phs {
 namespace {
 
 constexpr int NT = kGridThreads;
-enum { G_NACT = 0, G_NPEND, G_NDONE, G_LEFT0, G_LEFT1, G_LEFT2, G_NCTL };
+enum { G_NACT = 0, G_NPEND, G_NDONE, G_LEFT0, G_LEFT1, G_LEFT2, G_ADD0, G_ADD1, G_NCTL };
 constexpr int kWaiting = -4, kDone = -3, kPending = -2, kUnfrozen = -1;
 
 __device__ __forceinline__ double block_min(double v, double *red) {
@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(kGridThreads, 1)
         l_chg[l] = solve;
       }
       c_solve[r.comp] = solve;
-      if (INC) atomicMin(&c_rmin[r.comp], 0ull);  // a flow was added: the whole component is re-solved
+      if (INC) ctl[G_ADD0 + (solve & 1)] = 1;  // a flow was added: its links bound what stands (pass A below)
       f_rq[f] = -1;
       f_tc[f] = kInf;
       f_st[f] = kUnfrozen;
@@ -170,6 +170,7 @@ __global__ void __launch_bounds__(kGridThreads, 1)
       }
       // ======== phase X (a8 + a4)
       ++solve;
+      if (INC && gtid == 0) ctl[G_ADD0 + ((solve + 1) & 1)] = 0;  // last read after the X barrier of the event before
       {
         int d_act = 0, d_pend = 0, d_done = 0;
         for (long long ff = gtid; ff < F; ff += GT) {
@@ -188,8 +189,8 @@ __global__ void __launch_bounds__(kGridThreads, 1)
           const uint32_t out = fmap[f];
           T.t_done[out] = t_next;
           T.bneck[out] = linkid[st];
-#pragma unroll
           const long long rq_done = INC ? f_rq[f] : 0;
+#pragma unroll
           for (int h = 0; h < kMaxHops; ++h) {
             const int l = r.path[h];
             if (l < 0) continue;
@@ -251,6 +252,27 @@ __global__ void __launch_bounds__(kGridThreads, 1)
         }
       };
       int rounds = 0;
+      if (INC && __ldcg(&ctl[G_ADD0 + (solve & 1)])) {
+        // ---- A: flows were ADDED.  A link that carries an added flow has a share of at least floor(cap / n) -- n its
+        // flow count now -- all through the new solve, so the old solve's iterations below the smallest such share are
+        // picked again in the same order: every flow slower than that stands.
+        for (long long ff = gtid; ff < F; ff += GT) {
+          const int f = (int)ff;
+          if (__ldcg(&f_st[f]) != kUnfrozen || f_rq[f] >= 0) continue;  // ACTIVE and never solved = added
+          const FlowRec r = rec[f];
+          long long m = LLONG_MAX;
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = r.path[h];
+            if (l < 0) continue;
+            const long long sh = fair_share(l_cap[l], __ldcg(&l_n0[l]));
+            m = sh < m ? sh : m;
+          }
+          atomicMin(&c_rmin[r.comp], (unsigned long long)m);
+        }
+        __threadfence();
+        grid.sync();
+      }
       if (INC) {  // ---- C: the flows to re-solve give their rates back and count as unfrozen again
         ++g;
         if (gtid == 0) {  // the credit pass takes part in the rotation of the flag / minimum words like a round

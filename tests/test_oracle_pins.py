@@ -351,6 +351,52 @@ def test_removing_flows_leaves_the_slower_part_of_the_allocation_alone(seed):
     assert unchanged_total > 0 or n_flows < 8
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_adding_flows_leaves_the_slowest_part_of_the_allocation_alone(seed):
+    """The other half of the incremental re-solve: add flows to an allocation; every old flow whose
+    rate is below s* = min over the links of the added flows of floor(cap / n_new), n_new the link's flow count with the
+    added flows, keeps its rate and its bottleneck, bit for bit.  (A link that carries an added flow has a share of at
+    least s* throughout the new run, so the iterations of the old run below s* are picked again, in the same order.)
+    Combined with removals in the same step: the limit is the smaller of the two."""
+    rng = np.random.default_rng(300 + seed)
+    n_links = int(rng.integers(4, 40))
+    n_flows = int(rng.integers(20, 200))
+    cap = np.floor(rng.uniform(1e9, 4e11, n_links))
+    if seed % 2:
+        cap[:] = 50e9
+    capq = np.floor(cap * 2.0 ** 20)                    # exact in binary64 for these magnitudes
+    lens = rng.integers(1, min(6, n_links) + 1, n_flows)
+    paths = [rng.choice(n_links, int(h), replace=False).astype(np.int32) for h in lens]
+
+    def solve(keep):
+        off = np.concatenate([[0], np.cumsum([len(paths[f]) for f in keep])])
+        pth = np.concatenate([paths[f] for f in keep]).astype(np.int32)
+        rate, bneck, _, _ = orc.maxmin(cap, off, pth, orc.MODE_FAST)
+        return dict(zip(keep, rate)), dict(zip(keep, bneck))
+
+    alive = list(range(n_flows // 3))
+    waiting = list(range(n_flows // 3, n_flows))
+    rate, bneck = solve(alive)
+    kept = 0
+    while waiting:
+        k = int(rng.integers(1, 4))
+        new, waiting = waiting[:k], waiting[k:]
+        gone = [int(x) for x in rng.choice(alive, int(rng.integers(0, 3)), replace=False)] if len(alive) > 4 else []
+        alive2 = [f for f in alive if f not in gone] + new
+        cnt = np.zeros(n_links)
+        for f in alive2:
+            cnt[paths[f]] += 1
+        s_star = min(int(capq[l]) // int(cnt[l]) for f in new for l in paths[f]) * 2.0 ** -20   # exact integers
+        limit = min([s_star] + [rate[f] for f in gone])
+        new_rate, new_bneck = solve(alive2)
+        for f in alive2:
+            if f in rate and rate[f] < limit:
+                assert new_rate[f] == rate[f] and new_bneck[f] == bneck[f], (f, rate[f], limit)
+                kept += 1
+        alive, rate, bneck = alive2, new_rate, new_bneck
+    assert kept > 0
+
+
 def test_p4_certificate_along_event_loop():
     # a contended mid-size run: shrunken cfg1 (DP rings share 2 uplinks per leaf) -- check EVERY recompute
     w = W.cfg1(batch=3, n_hosts=8, gph=4, n_leaves=4, n_spines=2)
