@@ -263,6 +263,22 @@ def test_no_cpu_fallback_without_a_gpu():
     sim.close()
 
 
+def test_run_static_needs_a_finalized_handle():
+    """phs_run_static builds nothing and allocates nothing: on a handle that is not finalized it is a state error
+    (checked before any CUDA call, so this runs without a GPU), and the output size must match."""
+    sim = B.Sim.from_workload(W.cfg0())
+    with pytest.raises(B.PhsError) as e:
+        sim.run_static()
+    assert e.value.code == B.PHS_ESTATE and "phs_finalize" in str(e.value)
+    with pytest.raises(B.PhsError) as e:
+        B.phs_run_static(None, None, None, 0)
+    assert e.value.code == B.PHS_EINVAL
+    sim.close()
+    assert B.PHS_STATIC_SCRATCH_BYTES == 8 << 20 and B.PHS_STATIC_MAX_UNITS == 4096
+    hdr = open(os.path.join(ROOT, "include", "phs.h")).read()
+    assert "#define PHS_STATIC_SCRATCH_BYTES (8u << 20)" in hdr and "#define PHS_STATIC_MAX_UNITS 4096" in hdr
+
+
 def test_world_size_2_sharding_over_gloo():
     """N>1 path of bench.py: instances are sharded round-robin over ranks with no data-path collective; only the
     timing max and the counts are reduced.  Run the sharding + reduction logic on CPU over gloo."""
