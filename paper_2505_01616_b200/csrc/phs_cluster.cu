@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   // [L] per component (representative link), replicated per CTA: the smallest removed rate of the event, truncated to
   // rate >> kRminShift so that it is one 32-bit word (a remote 32-bit min needs no answer; truncation only makes the cut
   // more careful: (rate >> k) < (r_min >> k) implies rate < r_min)
-  unsigned *crmin = (unsigned *)(smem_raw + o_repl + up16((size_t)L * 22));
+  unsigned *crmin = INCS ? (unsigned *)(smem_raw + o_repl + up16((size_t)L * 22)) : nullptr;
   LinkA *la = (LinkA *)smem_raw;
   LinkB *lb = (LinkB *)(smem_raw + o_lb);
   int *won = (int *)(smem_raw + o_won);
