@@ -57,6 +57,8 @@ def make_workload(name, n_gpus, per_gpu=0):
         return W.cfg2(k=8, agg_uplinks=2), 1
     if name == "cfg4s":
         return W.cfg4(batch=(per_gpu or 2) * n_gpus, n_hosts=8, gph=8, n_leaves=4, n_spines=2), per_gpu or 2
+    if name == "a2a304":      # cfg4's recipe on 304 GPUs: 92,112 concurrent flows in one unit -> the grid path
+        return W.cfg4(batch=1, n_hosts=38, gph=8, n_leaves=2, n_spines=4), 1
     raise SystemExit(f"unknown workload {name}")
 
 
