@@ -160,11 +160,12 @@ __global__ void __launch_bounds__(kClusterThreads, 1)
   // REPL: every CTA keeps its own copy of the links' current fair shares, so that voting reads local shared
   // memory; owners broadcast the shares they recompute after debits, stale first-round shares are refreshed by the
   // flows that need them
-  // INC, incremental re-solve: an event that only removes flows leaves untouched every flow whose rate
-  // is below the smallest rate among the removed ones -- the one-bottleneck-per-iteration algorithm freezes links in
-  // ascending (share, id) order, and its iterations before the removed flow's own bottleneck do not see the removal.
-  // Per component, crmin = that smallest rate (0 when a flow was added: everything is re-solved); link capacities
-  // left after ALL frozen flows (caprem) persist from solve to solve, the flows to re-solve credit their rates back.
+  // INC, incremental re-solve: an event leaves untouched every flow whose rate is below the smallest
+  // rate among the flows it REMOVES -- the one-bottleneck-per-iteration algorithm freezes links in ascending (share, id)
+  // order, and its iterations before a removed flow's own bottleneck do not see the removal -- and below the smallest
+  // floor(cap / n) over the links of the flows it ADDS (such a link's share never falls below that in the new solve).
+  // Per component, crmin = the smaller of the two limits; the capacity left on every link after ALL frozen flows
+  // (caprem) persists from solve to solve, and the flows at or above the limit credit their rates back.
   const bool INCS = REPL && AGG && !LOG;            // the layout has crmin[]
   const bool INC = INCS && SC.incremental != 0;
   long long *sh_loc = (long long *)(smem_raw + o_repl);  // [L] share in the current round

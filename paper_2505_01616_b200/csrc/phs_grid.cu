@@ -52,10 +52,11 @@ size_t grid_scratch_bytes(int64_t n_flows, int n_links) {
 }
 
 // HIST: record the throughput history.  The event log is not written on this path.
-// INC: incremental re-solve (the same rule as in phs_cluster.cu): an event that only removes flows
-// leaves every flow whose rate is below the smallest removed rate of its component alone.  l_caprem then persists
-// from solve to solve (capacity left after ALL frozen flows), a completing flow credits its rate back in phase X, the
-// flows at or above the limit credit theirs in a pass of their own and are solved by the rounds >= 2 code.
+// INC: incremental re-solve (the same rule as in phs_cluster.cu): an event leaves alone every flow
+// whose rate is below the smallest rate it removes from the component and below the smallest floor(cap / n) over the
+// links of the flows it adds.  l_caprem then persists from solve to solve (capacity left after ALL frozen flows), a
+// completing flow credits its rate back in phase X, the flows at or above the limit credit theirs in a pass of their
+// own and are solved by the rounds >= 2 code.
 template <bool HIST, bool INC>
 __global__ void __launch_bounds__(kGridThreads, 1)
     phs_grid_kernel(DevTables T, const int32_t *__restrict__ list, int n_list, unsigned char *scratch, int64_t max_flows,
