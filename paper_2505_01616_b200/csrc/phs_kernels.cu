@@ -43,6 +43,7 @@ struct CtaSmem {
   int *l_solve;   // per component (indexed by its representative link): id of the solve that must redo it
   int *l_won;     // LOG: round in which the link froze flows (counts bottleneck links once)
   int *l_gid;     // link id of the topology (the links of a unit are numbered densely)
+  unsigned *l_rmin;  // INC, per component (representative link): limit below which rates stand in this event's solve
   // per slot [S]: one slot per PENDING or ACTIVE flow
   double *s_tc;   // PENDING: activation time; ACTIVE: completion time; free: +inf
   double *s_rem;  // remaining bytes at time s_tl
@@ -61,12 +62,13 @@ struct CtaSmem {
 };
 enum {
   C_HI = 0, C_QHEAD, C_QTAIL, C_NACTIVE, C_NPEND, C_OVERFLOW, C_DONE, C_EV_NCOMP, C_EV_ROUNDS, C_EV_NACT0,
-  C_EV_NACT1, C_NCTL
+  C_EV_NACT1, C_ADDED, C_NCTL
 };
 
 __host__ __device__ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 constexpr unsigned kNoLink = 0xffffu;
+constexpr int kRminShift = 30;  // rates are below 2^62 quanta: rate >> 30 is one 32-bit word (a more careful limit)
 static_assert(kMaxHops <= 8, "a path is stored as 8 x uint16");
 // unpack link h of a packed path
 __device__ __forceinline__ int path_at(const uint4 &p, int h) {
@@ -103,6 +105,7 @@ __host__ __device__ inline size_t carve(CtaSmem *s, unsigned char *base, int L, 
   PHS_TAKE(l_solve, int, L)
   PHS_TAKE(l_won, int, log ? L : 0)
   PHS_TAKE(l_gid, int, Lw)
+  PHS_TAKE(l_rmin, unsigned, (lean & 4) ? L : 0)  // bit 2: incremental re-solve (never together with bits 0 / 1)
   PHS_TAKE(s_meta, int4, S)
   PHS_TAKE(s_path, uint4, S)
   PHS_TAKE(s_succ_cnt, int, S)
@@ -149,7 +152,10 @@ size_t cta_lean_scratch_bytes(int n_links) {  // per CTA: l_caprem, l_sharew (8 
 // NT threads; LOG: write the event log (and solve every component at every event, so that the log's iteration
 // count and first bottleneck are those of a from-scratch solve); PCS: predecessor counters live in shared memory;
 // HIST: record the throughput history (a call in the hottest block of the kernel: compiled out when not wanted).
-template <int NT, bool LOG, bool PCS, bool HIST>
+// INC: incremental re-solve (the rule of phs_cluster.cu / phs_grid.cu): for units whose solves take
+// several filling rounds (all-to-all, raw flow sets).  l_caprem then persists from solve to solve, an event re-solves
+// only the flows at or above its limit; ring traffic (one round per solve) is better off without it.
+template <int NT, bool LOG, bool PCS, bool HIST, bool INC = false>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_kernel(DevTables T, const int32_t *__restrict__ order, int n_order,
                                                      int *ticket, int SC, int pcf, int lean,
                                                      unsigned char *lean_scratch) {
@@ -206,6 +212,11 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       S.l_deb[l] = 0;
       S.l_solve[l] = 0;
       if (LOG) S.l_won[l] = 0;
+      if (INC) {
+        S.l_caprem[l] = capq[l];
+        S.l_nw[l] = 0;
+        S.l_rmin[l] = 0xffffffffu;
+      }
     }
     // the scratch region served another unit (or another CTA parked this one): no debit stamp may look current.
     // No solve is in progress between events, and round numbers compared with l_deb are >= 1.
@@ -330,6 +341,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           }
         }
         S.l_solve[S.s_meta[slot].z] = solve;
+        if (INC) S.ctl[C_ADDED] = 1;  // its links bound what stands (pass A)
         S.s_rq[slot] = -1;
         S.s_meta[slot].y = -1;
         S.s_tc[slot] = kInf;
@@ -398,15 +410,18 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         t_done[f] = t_next;
         bneck_out[f] = l_gid[S.s_meta[s].y];
         const uint4 pv = S.s_path[s];
+        const long long rq_done = INC ? S.s_rq[s] : 0;
 #pragma unroll
         for (int h = 0; h < kMaxHops; ++h) {
           const int l = path_at(pv, h);
           if (l != (int)kNoLink) {
             atomicSub(&S.l_n0[l], 1);
             S.l_chg[l] = solve;
+            if (INC) smem_add64(&S.l_caprem[l], rq_done);  // the flow's rate goes back to its links
           }
         }
         S.l_solve[S.s_meta[s].z] = solve;
+        if (INC) atomicMin(&S.l_rmin[S.s_meta[s].z], (unsigned)(rq_done >> kRminShift));
         const int nsucc = S.s_succ_cnt[s], sc0 = S.s_succ0[s], sc1 = S.s_succ1[s];
         S.s_meta[s].x = -1;
         S.s_tc[s] = kInf;
@@ -455,13 +470,16 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       max_active = max(max_active, nA);
       max_pending = max(max_pending, nPend);
 
+      const int added = INC ? S.ctl[C_ADDED] : 0;  // (reset after the next barrier, below)
       // ======== a5: fair share of the links whose flow count changed in this event, one thread per link
-      for (int l = tid; l < Li; l += NT) {
-        if (S.l_chg[l] != solve) continue;
-        const int n = S.l_n0[l];
-        if (n > 0) S.l_share0[l] = fair_share(l_cap[l], n);
+      if (!INC) {
+        for (int l = tid; l < Li; l += NT) {
+          if (S.l_chg[l] != solve) continue;
+          const int n = S.l_n0[l];
+          if (n > 0) S.l_share0[l] = fair_share(l_cap[l], n);
+        }
+        __syncthreads();
       }
-      __syncthreads();
 
       // ======== rates (a6-a7): parallel progressive filling over the components this event touched
       auto in_solve = [&](int s) {  // ACTIVE flow of a component that must be re-solved
@@ -487,8 +505,48 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
         if (LOG && atomicExch(&S.l_won[arg], g) != g) atomicAdd(&S.ctl[C_EV_ROUNDS], 1);
       };
       int rounds = 1;
-      ++g;
-      {  // ---- V0: fair share of the links whose flow count changed (a5), arg-min link of every flow (a6)
+      if (INC) {
+        if (added) {
+          // ---- A: flows were ADDED.  A link that carries an added flow keeps a share of at least floor(cap / n) -- n its
+          // flow count now -- all through the new solve: every flow slower than the smallest such share stands.
+          for (int s = tid; s < hi; s += NT) {
+            const int4 m = S.s_meta[s];
+            if (m.x < 0 || m.y != -1 || S.s_rq[s] >= 0) continue;  // ACTIVE and never solved = added
+            const uint4 pv = S.s_path[s];
+            long long mn = LLONG_MAX;
+#pragma unroll
+            for (int h = 0; h < kMaxHops; ++h) {
+              const int l = path_at(pv, h);
+              if (l == (int)kNoLink) continue;
+              const long long sh = fair_share(l_cap[l], S.l_n0[l]);
+              mn = sh < mn ? sh : mn;
+            }
+            atomicMin(&S.l_rmin[m.z], (unsigned)(mn >> kRminShift));
+          }
+          __syncthreads();
+        }
+        // ---- C: the flows at or above their component's limit give their rates back to their links and count as
+        // unfrozen again; stamp l_deb = g makes the first vote below compute the links' shares from (caprem, nw)
+        ++g;
+        for (int s = tid; s < hi; s += NT) {
+          const int4 m = S.s_meta[s];
+          if (m.x < 0 || m.y == -2 || S.l_solve[m.z] != solve) continue;
+          const long long rq = S.s_rq[s];
+          if (rq >= 0 && (unsigned)(rq >> kRminShift) < S.l_rmin[m.z]) continue;  // below the limit: stands
+          S.s_meta[s].y = -1;
+          const uint4 pv = S.s_path[s];
+#pragma unroll
+          for (int h = 0; h < kMaxHops; ++h) {
+            const int l = path_at(pv, h);
+            if (l == (int)kNoLink) continue;
+            if (rq > 0) smem_add64(&S.l_caprem[l], rq);
+            atomicAdd(&S.l_nw[l], 1);
+            S.l_deb[l] = g;
+          }
+        }
+      }
+      if (!INC) ++g;
+      if (!INC) {  // ---- V0: fair share of the links whose flow count changed (a5), arg-min link of every flow (a6)
         long long bk = LLONG_MAX;
         int bl = INT_MAX;
         for (int s = tid; s < hi; s += NT) {
@@ -541,8 +599,13 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       PHS_TICK(2)
       __syncthreads();
       PHS_TICK(3)
-      bool left = false;
-      {  // ---- F0: unbeaten arg-min links freeze their flows (a7); fold the slot times (a8)
+      bool left = INC;  // INC: the rounds below do all the solving (and fold the slot times even if nothing is unfrozen)
+      if (INC) {        // every thread has read the limits and the flag: ready for the next event
+        for (int l = tid; l < Li; l += NT)
+          if (S.l_solve[l] == solve) S.l_rmin[l] = 0xffffffffu;
+        if (tid == 0) S.ctl[C_ADDED] = 0;
+      }
+      if (!INC) {  // ---- F0: unbeaten arg-min links freeze their flows (a7); fold the slot times (a8)
         double mymin = kInf;
         for (int s = tid; s < hi; s += NT) {
           if (S.s_meta[s].x < 0) continue;
@@ -562,6 +625,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
       left = __syncthreads_or(left);
       PHS_TICK(5)
       if (left) {
+        if (!INC) {
         // ---- I: working capacities of the links of this solve (idempotent stores)
         for (int s = tid; s < hi; s += NT) {
           if (!in_solve(s)) continue;
@@ -593,6 +657,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
           }
         }
         __syncthreads();
+        }
         for (;;) {
           ++g;
           ++rounds;
@@ -640,7 +705,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 1024 : 512) / NT) phs_cta_ker
                 for (int h = 0; h < kMaxHops; ++h) {
                   const int l = path_at(pv, h);
                   if (l == (int)kNoLink) continue;
-                  if (S.l_n0[l] > 1) {
+                  if (INC || S.l_n0[l] > 1) {  // INC: caprem persists, so every freeze is booked
                     smem_add64(&S.l_caprem[l], -rq);
                     atomicSub(&S.l_nw[l], 1);
                     S.l_deb[l] = g;
@@ -729,6 +794,16 @@ cudaError_t launch_hist(const DevTables &t, const int32_t *order, int n, int *ti
                                                                     c.lean_scratch);
   return cudaGetLastError();
 }
+template <int NT, bool PCS>
+cudaError_t launch_inc(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
+                       cudaStream_t stream) {  // incremental re-solve: no event log, no history
+  cudaError_t e = cudaFuncSetAttribute(phs_cta_kernel<NT, false, PCS, false, true>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  phs_cta_kernel<NT, false, PCS, false, true><<<c.grid, NT, c.smem, stream>>>(t, order, n, ticket, c.slots, c.pc_flows,
+                                                                             c.lean, c.lean_scratch);
+  return cudaGetLastError();
+}
 template <int NT, bool LOG, bool PCS>
 cudaError_t launch_one(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
                        cudaStream_t stream) {
@@ -739,6 +814,8 @@ template <int NT>
 cudaError_t launch_nt(const DevTables &t, const int32_t *order, int n, int *ticket, const CtaLaunch &c,
                       cudaStream_t stream) {
   const bool pcs = c.pc_flows > 0;
+  if ((c.lean & 4) && !c.log && !t.hist)
+    return pcs ? launch_inc<NT, true>(t, order, n, ticket, c, stream) : launch_inc<NT, false>(t, order, n, ticket, c, stream);
   if (c.log) return pcs ? launch_one<NT, true, true>(t, order, n, ticket, c, stream)
                         : launch_one<NT, true, false>(t, order, n, ticket, c, stream);
   return pcs ? launch_one<NT, false, true>(t, order, n, ticket, c, stream)

@@ -762,6 +762,19 @@ extern "C" phs_status phs_finalize(phs_sim *sim, void *cuda_stream) {
       const int v = atoi(ev);
       if (v == 0 || v == 1 || v == 3) lean = log ? 0 : v;
     }
+    // Incremental re-solve (bit 2 of `lean`): where most of the launch's flows are all-to-all or raw
+    // flow sets -- solves of several filling rounds -- and nothing else claims the working arrays (no lean layout, no
+    // event log, no history).  Ring traffic solves in one round and is better off without it.
+    {
+      int64_t whole = 0, all = 0;
+      for (int u : cand) {
+        whole += std::min<int64_t>(sim->units[u].bound_whole, sim->units[u].n_flows);
+        all += sim->units[u].n_flows;
+      }
+      bool inc = lean == 0 && !log && sim->hist_cap == 0 && 2 * whole >= all;
+      if (const char *ev = getenv("PHS_CTA_INC")) inc = atoi(ev) != 0 && lean == 0 && !log && sim->hist_cap == 0;
+      if (inc) lean = 4;
+    }
     int slots_p = 0, slots_n = 0;
     const int w_p = pc8_ok ? fit(true, lean, &slots_p) : 0, w_n = fit(false, lean, &slots_n);
     if (w_p == 0 && w_n == 0) {

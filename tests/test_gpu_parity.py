@@ -636,6 +636,35 @@ def test_incremental_resolve_with_flows_added_and_removed(monkeypatch, inc):
             assert_instance_matches(sim, i, o, check_log=False)
         assert sim.path_of(0) == ("cluster" if path == CLUSTER else "grid")
         sim.close()
+    # the CTA path: a batch of small instances of the same kind (the scheduler turns the incremental re-solve on when
+    # most flows of the launch are all-to-all / raw flows), stopped and resumed on the way
+    monkeypatch.setenv("PHS_CTA_INC", inc)
+    d = W.topo_desc(W.TOPO_LEAF_SPINE, 4, 8, fabric_Bps=W.gbps(200.0), n_leaves=2, n_spines=2, uplinks_per_leaf_spine=1)
+    insts = []
+    for i in range(6):
+        rng = np.random.default_rng(90 + i)
+        n = 300
+        src = rng.integers(0, 32, n).astype(np.int32)
+        dst = ((src + rng.integers(1, 32, n)) % 32).astype(np.int32)
+        ops = [W.Coll(W.ALLTOALL, np.arange(32, dtype=np.int32), 32 * 2e5),
+               W.Coll(W.ALLTOALL, np.arange(0, 32, 2, dtype=np.int32), 16 * 4e5, 0.0, (0,)),
+               W.RawFlows(src, dst, np.floor(rng.uniform(1e4, 1e6, n)), start=rng.uniform(0.0, 2e-4, n))]
+        insts.append(W.Instance(seed=i, ops=ops))
+    w = W.Workload("a2a_chain_small", d, 5, insts)
+    ref = [oracle_run(w.desc, w.instances[i], mode=orc.MODE_FAST, base_seed=w.base_seed) for i in range(w.batch)]
+    t_end = max(o.completion_times().max() for o in ref)
+    sim = B.Sim.from_workload(w, path=CTA, decompose=False)
+    for frac in (0.3, 0.7, 1.5):
+        sim.run(until=frac * t_end)
+        for i in range(w.batch):
+            o = oracle_build(w.desc, w.instances[i], base_seed=w.base_seed)
+            o.run(mode=orc.MODE_FAST, until=frac * t_end)
+            assert np.array_equal(sim.completion_times(i), o.completion_times(), equal_nan=True), (frac, i)
+            assert np.array_equal(sim.bottlenecks(i), o.bottlenecks())
+    for i in range(w.batch):
+        assert_instance_matches(sim, i, ref[i], check_log=False)
+        assert sim.path_of(i) == "cta"
+    sim.close()
 
 
 def test_run_until_resumes_a_multi_cta_cluster():
